@@ -1,0 +1,173 @@
+/*
+ * nao.h -- C-ABI boundary of the B200-native (sm_100a) generalized eigensolver + density-matrix library.
+ *
+ * The path (paper = /root/reference/PAPER.md, arxiv/paper_2606_09058):
+ *   nao_geneig          H C = S C diag(e)              Eq. 5, per k-point Eq. 11,
+ *                                                      noncollinear 2N x 2N form Eq. 21/25-27 (PAPER.md:113-115,
+ *                                                      175-179); the paper's "Part 2" (section 3.1,
+ *                                                      PAPER.md:157-163) / "Part 3" (section 3.2)
+ *   nao_fermi_mu        sum g w_k f((e-mu)/kT) = N_e   Fermi-Dirac occupation (after Eq. 3); the
+ *                                                      paper's "Part 3"/"Part 4"
+ *   nao_density_matrix  D = C diag(f) C^H              Eq. 8 / Eq. 23; the paper's
+ *                                                      "Part 4"/"Part 5"
+ *
+ * Conventions common to every entry point
+ *   - All matrix/vector pointers are DEVICE pointers unless the name starts with h_ (host).
+ *   - Matrices are column-major with a leading dimension in ELEMENTS (LAPACK convention); element (i,j) of item b
+ *     is at  base + b*stride + j*ld + i.  dtype NAO_REAL = double, NAO_COMPLEX = interleaved (re,im) doubles.
+ *   - The library allocates NO device memory: the caller owns every buffer, the workspace and the stream.
+ *     `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Work is enqueued on
+ *     that stream; only nao_fermi_mu synchronises it (to hand back *h_mu).
+ *   - Return value: NAO_OK (0); -i if argument number i (1-based) is invalid (checked on the host before any
+ *     launch); a positive NAO_ERR_* code for run-time failures.  Numerical outcomes are reported per batch item
+ *     in d_info (device int[batch]).
+ *   - There is no CPU fallback anywhere: every step runs in CUDA kernels of this library.
+ */
+#ifndef NAO_H
+#define NAO_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* dtype */
+#define NAO_REAL 0
+#define NAO_COMPLEX 1
+
+/* flags for nao_geneig / nao_geneig_workspace */
+#define NAO_S_FACTORED 1u      /* dS already holds the factor written by an earlier nao_geneig call on the same S
+                                  (S and V = its orthogonaliser do not change during the SCF loop) */
+#define NAO_NC_BLOCK_S 2u      /* noncollinear fast path: n = 2N, dtype = NAO_COMPLEX, basis spin-major [alpha;beta]
+                                  (Eq. 25-27); dS is the N x N REAL overlap (S_NC = diag(S,S)) */
+#define NAO_TRD_ONE_STAGE 4u   /* force the one-stage (HEMV-based, HBM-bound) Householder tridiagonalisation */
+#define NAO_TRD_TWO_STAGE 8u   /* force the two-stage (dense->band->tridiagonal) reduction */
+
+/* return codes */
+#define NAO_OK 0
+#define NAO_ERR_WORKSPACE 1    /* work_bytes smaller than nao_geneig_workspace / nao_density_workspace reports */
+#define NAO_ERR_CUDA 2         /* a CUDA runtime call or kernel launch failed */
+#define NAO_ERR_ELECTRONS 3    /* nao_fermi_mu: n_electrons outside (0, sum of weights * n) or kT <= 0 */
+#define NAO_ERR_UNSUPPORTED 4  /* combination of arguments not implemented */
+
+/* Bytes of device workspace nao_geneig needs for (n, batch, dtype, flags).  Host-only, no launch. */
+int nao_geneig_workspace(int n, int batch, int dtype, unsigned flags, size_t *bytes);
+
+/*
+ * Generalized Hermitian-definite eigenproblem, all eigenpairs, batched over (spin, k) items.
+ *   1 n        order of H (2N with NAO_NC_BLOCK_S), n >= 1
+ *   2 batch    number of independent (H,S) items, >= 1
+ *   3 dtype    NAO_REAL or NAO_COMPLEX
+ *   4 flags    OR of NAO_* flags above
+ *   5 dH,ldh,strideH   in : Hermitian H; ONLY the lower triangle (i >= j) is referenced.  Not modified.
+ *   8 dS,lds,strideS   in : Hermitian positive definite S, lower triangle referenced (with NAO_NC_BLOCK_S:
+ *                           real, order n/2, shared by all batch items if strideS == 0).
+ *                      out: lower triangle = Cholesky factor L (S = L L^H); strict upper triangle = strict upper
+ *                           triangle of L^{-H} (kept so that a later call with NAO_S_FACTORED skips both the
+ *                           factorisation and the inversion).  With NAO_S_FACTORED: read only.
+ *  11 dE       out: batch*n eigenvalues, ascending within each item (item b at dE + b*n)
+ *  12 dC,ldc,strideC   out: eigenvectors as columns, normalised so that C^H S C = I.  Phases/signs and the basis
+ *                           inside degenerate clusters are unspecified (compare e, mu, f, D, not C).
+ *  15 dwork,work_bytes  device scratch of at least nao_geneig_workspace() bytes, 256-byte aligned
+ *  17 d_info   out: device int[batch]; 0 = ok; j in 1..n: leading minor j of S not positive definite (LAPACK
+ *                   potrf convention; the item's e and C are then undefined); n+1 = the tridiagonal
+ *                   divide-and-conquer secular solver failed to converge.
+ *  18 cuda_stream
+ */
+int nao_geneig(int n, int batch, int dtype, unsigned flags,
+               const void *dH, long ldh, long strideH,
+               void *dS, long lds, long strideS,
+               double *dE,
+               void *dC, long ldc, long strideC,
+               void *dwork, size_t work_bytes, int *d_info, void *cuda_stream);
+
+/*
+ * Fermi level and occupations (reading C5).  States are all (item b, level i) pairs; state weight is
+ * h_weight[b] (= spin degeneracy g times k-point weight w_k, reading C4).  Finds the unique mu with
+ *     sum_b h_weight[b] * sum_i f_bi = n_electrons,   f_bi = 1/(1 + exp((e_bi - mu)/kT)),
+ * solved in particle/hole form so that mu is resolved inside a gap.
+ *   1 n, 2 batch
+ *   3 dE        in : device, batch*n eigenvalues (any order)
+ *   4 h_weight  in : HOST double[batch]
+ *   5 n_electrons, 6 kT (Hartree, > 0)
+ *   7 h_mu      out: HOST double, the Fermi level (the call synchronises the stream to write it)
+ *   8 dF        out: device, batch*n occupations f in [0,1]
+ *   9 dwork     device scratch of at least nao_fermi_workspace(n, batch) bytes
+ *  10 cuda_stream
+ */
+int nao_fermi_workspace(int n, int batch, size_t *bytes);
+int nao_fermi_mu(int n, int batch, const double *dE, const double *h_weight,
+                 double n_electrons, double kT, double *h_mu, double *dF,
+                 void *dwork, void *cuda_stream);
+
+/*
+ * Density matrix D_b = C_b diag(f_b) C_b^H per batch item, full Hermitian matrix written (both triangles).
+ * Columns with f < 1e-17 are skipped (their contribution is < 1e-17 * |C|^2, reading C6).
+ *   1 n, 2 batch, 3 dtype
+ *   4 dC,ldc,strideC  in : eigenvectors (columns)
+ *   7 dF              in : device, batch*n occupations (any values >= 0; e.g. f*e gives the energy-weighted DM)
+ *   8 dD,ldd,strideD  out
+ *  11 dwork, work_bytes  device scratch of at least nao_density_workspace() bytes
+ *  13 cuda_stream
+ */
+int nao_density_workspace(int n, int batch, int dtype, size_t *bytes);
+int nao_density_matrix(int n, int batch, int dtype,
+                       const void *dC, long ldc, long strideC,
+                       const double *dF,
+                       void *dD, long ldd, long strideD,
+                       void *dwork, size_t work_bytes, void *cuda_stream);
+
+/* Human-readable text for a return code (static storage). */
+const char *nao_status_string(int status);
+
+/* Library version string, e.g. "nao-b200 0.1 (sm_100a)". */
+const char *nao_version(void);
+
+/*
+ * Number of kernel launches this process has issued through the library since load (host counter, all entry
+ * points).  bench.py uses it for its "gpu_launches" field.
+ */
+long nao_launch_count(void);
+
+/* ---- building blocks exported for tests and per-kernel measurement (same pointer/stream conventions) ---- */
+
+/*
+ * C <- alpha * op(A) * op(B) + beta * C on the FP64 tensor cores (DMMA), batched with strides.
+ * op codes: 0 = N, 1 = T (transpose), 2 = C (conjugate transpose).  m,n,k are the dimensions of the product.
+ * uplo_c: 0 = full C, 1 = only tiles touching the lower triangle are computed/written.
+ */
+int nao_gemm(int dtype, int opA, int opB, int m, int n, int k, double alpha,
+             const void *dA, long lda, long strideA, const void *dB, long ldb, long strideB,
+             double beta, void *dC, long ldc, long strideC, int batch, int uplo_c, void *cuda_stream);
+
+/*
+ * Cholesky factor and its inverse: dS (lower referenced) -> lower = L, strict upper = strict upper of L^{-H};
+ * dLinv (n x n, ld n) <- L^{-1} (lower, zeros above).  dtmp: n*n elements of scratch per item.  d_info as in
+ * nao_geneig.
+ */
+int nao_potrf_trtri(int n, int batch, int dtype, void *dS, long lds, long strideS,
+                    void *dLinv, void *dtmp, int *d_info, void *cuda_stream);
+
+/*
+ * Hermitian eigen-decomposition A = Z diag(e) Z^H of a standard problem (lower triangle of dA referenced,
+ * dA destroyed): tridiagonalisation, tridiagonal divide-and-conquer, back-transformation.
+ * Workspace: nao_heev_workspace bytes.
+ */
+int nao_heev_workspace(int n, int batch, int dtype, unsigned flags, size_t *bytes);
+int nao_heev(int n, int batch, int dtype, unsigned flags, void *dA, long lda, long strideA,
+             double *dE, void *dZ, long ldz, long strideZ, void *dwork, size_t work_bytes, int *d_info,
+             void *cuda_stream);
+
+/*
+ * Symmetric tridiagonal eigen-decomposition T = Q diag(e) Q^T by divide and conquer (real, all eigenpairs).
+ * dD[n], dEoff[n-1] per item (item stride n) are destroyed; dE ascending; dQ n x n (ld ldq).
+ */
+int nao_stedc_workspace(int n, int batch, size_t *bytes);
+int nao_stedc(int n, int batch, double *dD, double *dEoff, double *dE, double *dQ, long ldq, long strideQ,
+              void *dwork, size_t work_bytes, int *d_info, void *cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NAO_H */

@@ -1,0 +1,8 @@
+"""B200-native (sm_100a) generalized eigensolver + Fermi level + density matrix for NAO-based DFT
+(arxiv/paper_2606_09058 hot path).  See include/nao.h for the C-ABI and DESIGN.md for the design.
+
+`paper_2606_09058_b200.synth` (input generator) is importable without CUDA; everything else needs libnao.so.
+"""
+from .binding import (NAO_REAL, NAO_COMPLEX, NAO_S_FACTORED, NAO_NC_BLOCK_S, NAO_TRD_ONE_STAGE,  # noqa: F401
+                      NAO_TRD_TWO_STAGE, EXPORTS, NaoError, lib, geneig, geneig_workspace, fermi_mu, density_matrix,
+                      gemm, potrf_trtri, heev, stedc, launch_count, version)

@@ -1,0 +1,233 @@
+"""Thin ctypes binding of libnao.so (include/nao.h).  Argument marshalling ONLY: every step of the path runs in
+the library's CUDA kernels.  PyTorch supplies device memory and the stream, nothing else.
+
+Storage convention (same as paper_2606_09058_b200.synth): a batch of matrices is a contiguous tensor of shape
+(batch, n, n) holding COLUMN-MAJOR items, i.e. ``t[b, j, i] == M_b(i, j)``; ``t.mT`` is the mathematical matrix.
+Real = torch.float64, complex = torch.complex128 (interleaved re, im).
+
+There is no CPU fallback: if the CUDA library cannot be built/loaded, or a tensor is not on a CUDA device, the
+call raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+from . import build as _build
+
+NAO_REAL, NAO_COMPLEX = 0, 1
+NAO_S_FACTORED, NAO_NC_BLOCK_S, NAO_TRD_ONE_STAGE, NAO_TRD_TWO_STAGE = 1, 2, 4, 8
+
+_LIB = None
+_vp, _i, _l, _d, _sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_long, ctypes.c_double, ctypes.c_size_t
+_szp = ctypes.POINTER(ctypes.c_size_t)
+_dp = ctypes.POINTER(ctypes.c_double)
+
+_SIGNATURES = {
+    "nao_geneig_workspace": ([_i, _i, _i, ctypes.c_uint, _szp], _i),
+    "nao_geneig": ([_i, _i, _i, ctypes.c_uint, _vp, _l, _l, _vp, _l, _l, _vp, _vp, _l, _l, _vp, _sz, _vp, _vp], _i),
+    "nao_fermi_workspace": ([_i, _i, _szp], _i),
+    "nao_fermi_mu": ([_i, _i, _vp, _dp, _d, _d, _dp, _vp, _vp, _vp], _i),
+    "nao_density_workspace": ([_i, _i, _i, _szp], _i),
+    "nao_density_matrix": ([_i, _i, _i, _vp, _l, _l, _vp, _vp, _l, _l, _vp, _sz, _vp], _i),
+    "nao_status_string": ([_i], ctypes.c_char_p),
+    "nao_version": ([], ctypes.c_char_p),
+    "nao_launch_count": ([], _l),
+    "nao_gemm": ([_i, _i, _i, _i, _i, _i, _d, _vp, _l, _l, _vp, _l, _l, _d, _vp, _l, _l, _i, _i, _vp], _i),
+    "nao_potrf_trtri": ([_i, _i, _i, _vp, _l, _l, _vp, _vp, _vp, _vp], _i),
+    "nao_heev_workspace": ([_i, _i, _i, ctypes.c_uint, _szp], _i),
+    "nao_heev": ([_i, _i, _i, ctypes.c_uint, _vp, _l, _l, _vp, _vp, _l, _l, _vp, _sz, _vp, _vp], _i),
+    "nao_stedc_workspace": ([_i, _i, _szp], _i),
+    "nao_stedc": ([_i, _i, _vp, _vp, _vp, _vp, _l, _l, _vp, _sz, _vp, _vp], _i),
+}
+EXPORTS = tuple(_SIGNATURES)
+
+
+class NaoError(RuntimeError):
+    pass
+
+
+class _Lib:
+    """ctypes handle with typed signatures; a symbol the header declares but the library lacks raises on use."""
+
+    def __init__(self, path):
+        self._cdll = ctypes.CDLL(path)
+        self.path = path
+
+    def __getattr__(self, name):
+        argtypes, restype = _SIGNATURES[name]
+        fn = getattr(self._cdll, name)          # AttributeError if the library lacks a declared symbol
+        fn.argtypes = argtypes
+        fn.restype = restype
+        setattr(self, name, fn)
+        return fn
+
+
+def lib():
+    """Load (building if stale) libnao.so.  Raises if that is impossible -- there is no fallback path."""
+    global _LIB
+    if _LIB is None:
+        _LIB = _Lib(_build.build())
+    return _LIB
+
+
+def _check(rc, what):
+    if rc != 0:
+        raise NaoError("%s failed: status %d (%s)" % (what, rc, lib().nao_status_string(rc).decode()))
+
+
+def _dtype_code(t: torch.Tensor) -> int:
+    if t.dtype == torch.float64:
+        return NAO_REAL
+    if t.dtype == torch.complex128:
+        return NAO_COMPLEX
+    raise TypeError("expected float64 or complex128, got %s" % t.dtype)
+
+
+def _dev(t: torch.Tensor, name: str):
+    if not t.is_cuda:
+        raise NaoError("%s must be a CUDA tensor (no CPU path exists)" % name)
+    if not t.is_contiguous():
+        raise NaoError("%s must be contiguous" % name)
+    return t.data_ptr()
+
+
+def _stream(t: torch.Tensor):
+    return torch.cuda.current_stream(t.device).cuda_stream
+
+
+def _workspace(nbytes: int, device) -> torch.Tensor:
+    return torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=device)
+
+
+def launch_count() -> int:
+    return int(lib().nao_launch_count())
+
+
+def version() -> str:
+    return lib().nao_version().decode()
+
+
+# ------------------------------------------------------------------------------------------------- entry points
+def geneig_workspace(n: int, batch: int, dtype: int, flags: int = 0) -> int:
+    out = ctypes.c_size_t(0)
+    _check(lib().nao_geneig_workspace(n, batch, dtype, flags, ctypes.byref(out)), "nao_geneig_workspace")
+    return out.value
+
+
+def geneig(H: torch.Tensor, S: torch.Tensor, flags: int = 0, work: torch.Tensor | None = None):
+    """nao_geneig on (batch, n, n) column-major items.  S is overwritten by its factor (see nao.h).
+    Returns (E (batch, n), C (batch, n, n) column-major items, info (batch,) int32 device tensor)."""
+    batch, n, _ = H.shape
+    dt = _dtype_code(H)
+    if flags & NAO_NC_BLOCK_S:
+        sb, sn = S.shape[0], S.shape[-1]
+        strideS = 0 if sb == 1 else sn * sn
+        lds = sn
+    else:
+        strideS, lds = n * n, n
+    E = torch.empty((batch, n), dtype=torch.float64, device=H.device)
+    C = torch.empty_like(H)
+    info = torch.zeros(batch, dtype=torch.int32, device=H.device)
+    need = geneig_workspace(n, batch, dt, flags)
+    if work is None or work.numel() < need:
+        work = _workspace(need, H.device)
+    rc = lib().nao_geneig(n, batch, dt, flags, _dev(H, "H"), n, n * n, _dev(S, "S"), lds, strideS, _dev(E, "E"),
+                          _dev(C, "C"), n, n * n, _dev(work, "work"), work.numel(), _dev(info, "info"), _stream(H))
+    _check(rc, "nao_geneig")
+    return E, C, info
+
+
+def fermi_mu(E: torch.Tensor, weights, n_electrons: float, kT: float):
+    """nao_fermi_mu: E (batch, n) device tensor, weights = g*w_k per item (host sequence).  Returns (mu, F)."""
+    batch, n = E.shape
+    w = (ctypes.c_double * batch)(*[float(x) for x in weights])
+    need = ctypes.c_size_t(0)
+    _check(lib().nao_fermi_workspace(n, batch, ctypes.byref(need)), "nao_fermi_workspace")
+    work = _workspace(need.value, E.device)
+    F = torch.empty_like(E)
+    mu = ctypes.c_double(0.0)
+    rc = lib().nao_fermi_mu(n, batch, _dev(E, "E"), w, float(n_electrons), float(kT), ctypes.byref(mu), _dev(F, "F"),
+                            _dev(work, "work"), _stream(E))
+    _check(rc, "nao_fermi_mu")
+    return mu.value, F
+
+
+def density_matrix(C: torch.Tensor, F: torch.Tensor, out: torch.Tensor | None = None):
+    """nao_density_matrix: D_b = C_b diag(F_b) C_b^H, (batch, n, n) column-major items."""
+    batch, n, _ = C.shape
+    dt = _dtype_code(C)
+    D = torch.empty_like(C) if out is None else out
+    need = ctypes.c_size_t(0)
+    _check(lib().nao_density_workspace(n, batch, dt, ctypes.byref(need)), "nao_density_workspace")
+    work = _workspace(need.value, C.device)
+    rc = lib().nao_density_matrix(n, batch, dt, _dev(C, "C"), n, n * n, _dev(F, "F"), _dev(D, "D"), n, n * n,
+                                  _dev(work, "work"), work.numel(), _stream(C))
+    _check(rc, "nao_density_matrix")
+    return D
+
+
+# ------------------------------------------------------------------------------------------ building blocks
+def gemm(A: torch.Tensor, B: torch.Tensor, opA: int = 0, opB: int = 0, alpha: float = 1.0, beta: float = 0.0,
+         C: torch.Tensor | None = None, lower_only: bool = False):
+    """C <- alpha op(A) op(B) + beta C.  A, B, C are (batch, cols, rows) column-major items (see module doc)."""
+    batch = A.shape[0]
+    dt = _dtype_code(A)
+    a_rows, a_cols = A.shape[2], A.shape[1]
+    b_rows, b_cols = B.shape[2], B.shape[1]
+    m, k = (a_rows, a_cols) if opA == 0 else (a_cols, a_rows)
+    k2, n = (b_rows, b_cols) if opB == 0 else (b_cols, b_rows)
+    assert k == k2, (k, k2)
+    if C is None:
+        C = torch.zeros((batch, n, m), dtype=A.dtype, device=A.device)
+    rc = lib().nao_gemm(dt, opA, opB, m, n, k, alpha, _dev(A, "A"), a_rows, a_rows * a_cols, _dev(B, "B"), b_rows,
+                        b_rows * b_cols, beta, _dev(C, "C"), m, m * n, batch, int(lower_only), _stream(A))
+    _check(rc, "nao_gemm")
+    return C
+
+
+def potrf_trtri(S: torch.Tensor):
+    """In place on S (batch, n, n): lower = L, strict upper = strict upper of L^{-H}.  Returns (Linv, info)."""
+    batch, n, _ = S.shape
+    dt = _dtype_code(S)
+    W = torch.zeros_like(S)
+    T = torch.empty_like(S)
+    info = torch.zeros(batch, dtype=torch.int32, device=S.device)
+    rc = lib().nao_potrf_trtri(n, batch, dt, _dev(S, "S"), n, n * n, _dev(W, "W"), _dev(T, "T"), _dev(info, "info"),
+                               _stream(S))
+    _check(rc, "nao_potrf_trtri")
+    return W, info
+
+
+def heev(A: torch.Tensor, flags: int = 0):
+    """Standard Hermitian eigenproblem (lower triangle of A referenced, A destroyed).  Returns (E, Z, info)."""
+    batch, n, _ = A.shape
+    dt = _dtype_code(A)
+    need = ctypes.c_size_t(0)
+    _check(lib().nao_heev_workspace(n, batch, dt, flags, ctypes.byref(need)), "nao_heev_workspace")
+    work = _workspace(need.value, A.device)
+    E = torch.empty((batch, n), dtype=torch.float64, device=A.device)
+    Z = torch.empty_like(A)
+    info = torch.zeros(batch, dtype=torch.int32, device=A.device)
+    rc = lib().nao_heev(n, batch, dt, flags, _dev(A, "A"), n, n * n, _dev(E, "E"), _dev(Z, "Z"), n, n * n,
+                        _dev(work, "work"), work.numel(), _dev(info, "info"), _stream(A))
+    _check(rc, "nao_heev")
+    return E, Z, info
+
+
+def stedc(d: torch.Tensor, e: torch.Tensor):
+    """Symmetric tridiagonal eigenproblem by divide and conquer.  d (batch, n), e (batch, n) [last entry unused];
+    both destroyed.  Returns (E (batch, n), Q (batch, n, n) column-major items, info)."""
+    batch, n = d.shape
+    need = ctypes.c_size_t(0)
+    _check(lib().nao_stedc_workspace(n, batch, ctypes.byref(need)), "nao_stedc_workspace")
+    work = _workspace(need.value, d.device)
+    E = torch.empty_like(d)
+    Q = torch.empty((batch, n, n), dtype=torch.float64, device=d.device)
+    info = torch.zeros(batch, dtype=torch.int32, device=d.device)
+    rc = lib().nao_stedc(n, batch, _dev(d, "d"), _dev(e, "e"), _dev(E, "E"), _dev(Q, "Q"), n, n * n,
+                         _dev(work, "work"), work.numel(), _dev(info, "info"), _stream(d))
+    _check(rc, "nao_stedc")
+    return E, Q, info

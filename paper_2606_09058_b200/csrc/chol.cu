@@ -1,0 +1,180 @@
+// chol.cu -- Cholesky factor S = L L^H and its inverse W = L^{-1} (the paper's role for it is
+// Part 2-1/2-2 and 3-1/3-2, "diagonalise S, form V", PAPER.md:159-163, 189-193 -- computed once and reused in every
+// later SCF step).
+//
+// Recursive blocked algorithm in which everything above the leaves is a DMMA GEMM:
+//   [S11 .; S21 S22]:  (L11, W11) <- rec(S11);  L21 = S21 W11^H;  S22 -= L21 L21^H (lower tiles only);
+//                      (L22, W22) <- rec(S22);  W21 = -W22 (L21 W11).
+// Leaves (order <= 64) are factored and inverted inside shared memory by one CTA per batch item.
+// L^{-1} is formed explicitly because the per-step reduction A = L^{-1} H L^{-H} and the back-substitution
+// C = L^{-H} Z then become plain (triangular-masked) GEMMs -- the same choice the paper makes with its explicit
+// V = U s^{-1/2} and V^H H V / V C' products.
+#include "nao_internal.cuh"
+#include "scalar.cuh"
+
+namespace nao {
+
+static const int CHOL_LEAF = 64;
+
+// One CTA per batch item.  nb <= 64.  S block (lower referenced) -> L in place; W block <- L^{-1} (lower; the
+// strict upper part of the W block is zeroed).  info: first failing pivot (1-based, global index).
+template <class T>
+__global__ void __launch_bounds__(256) chol_leaf_kernel(int nb, int off, T *S, long lds, long sS, T *W, long ldw,
+                                                        long sW, int *info) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T *sL = (T *)smem_raw;                 // [nb][nb+1]  sL[i*(nb+1) + j] = L(i,j)
+    T *sX = sL + nb * (nb + 1);            // inverse, same layout
+    const int ld = nb + 1;
+    const int b = blockIdx.x;
+    S += (long)b * sS + off + (long)off * lds;
+    W += (long)b * sW + off + (long)off * ldw;
+    const int tid = threadIdx.x, nt = blockDim.x;
+    for (int e = tid; e < nb * nb; e += nt) {
+        int i = e % nb, j = e / nb;
+        sL[i * ld + j] = (i >= j) ? S[i + (long)j * lds] : Ops<T>::zero();
+    }
+    __syncthreads();
+    __shared__ double s_piv;
+    for (int j = 0; j < nb; ++j) {
+        if (tid == 0) {
+            double ajj = Ops<T>::real(sL[j * ld + j]);
+            if (!(ajj > 0.0)) {
+                if (info[b] == 0) info[b] = off + j + 1;
+                ajj = 1.0;
+            }
+            s_piv = sqrt(ajj);
+            sL[j * ld + j] = Ops<T>::from_real(s_piv);
+        }
+        __syncthreads();
+        const double rinv = 1.0 / s_piv;
+        for (int i = j + 1 + tid; i < nb; i += nt) sL[i * ld + j] = Ops<T>::scale(sL[i * ld + j], rinv);
+        __syncthreads();
+        // trailing update of the lower triangle: (i,k) with j < k <= i
+        const int r = nb - 1 - j;
+        for (int e = tid; e < r * r; e += nt) {
+            int i = j + 1 + e % r, k = j + 1 + e / r;
+            if (i >= k) sL[i * ld + k] = Ops<T>::sub(sL[i * ld + k], Ops<T>::mul_conj(sL[i * ld + j], sL[k * ld + j]));
+        }
+        __syncthreads();
+    }
+    // inverse by forward substitution, one column per thread group: X(i,c) = (delta_ic - sum_{k=c}^{i-1} L(i,k) X(k,c)) / L(i,i)
+    // 4 threads cooperate on a column (split the k-sum), 64 columns -> 256 threads.
+    {
+        const int c = tid >> 2, part = tid & 3;
+        for (int i = 0; i < nb; ++i) {
+            T acc = Ops<T>::zero();
+            if (c < nb && i > c)
+                for (int k = c + part; k < i; k += 4) acc = Ops<T>::sub(acc, Ops<T>::mul(sL[i * ld + k], sX[k * ld + c]));
+            // reduce over the 4 cooperating lanes (they are adjacent lanes of one warp)
+            if (sizeof(T) == 8) {
+                double *a = (double *)&acc;
+                a[0] += __shfl_xor_sync(0xffffffffu, a[0], 1); a[0] += __shfl_xor_sync(0xffffffffu, a[0], 2);
+            } else {
+                double *a = (double *)&acc;
+                a[0] += __shfl_xor_sync(0xffffffffu, a[0], 1); a[0] += __shfl_xor_sync(0xffffffffu, a[0], 2);
+                a[1] += __shfl_xor_sync(0xffffffffu, a[1], 1); a[1] += __shfl_xor_sync(0xffffffffu, a[1], 2);
+            }
+            if (c < nb && part == 0) {
+                double dinv = 1.0 / Ops<T>::real(sL[i * ld + i]);
+                T v;
+                if (i < c) v = Ops<T>::zero();
+                else if (i == c) v = Ops<T>::from_real(dinv);
+                else v = Ops<T>::scale(acc, dinv);
+                sX[i * ld + c] = v;
+            }
+            __syncthreads();
+        }
+    }
+    for (int e = tid; e < nb * nb; e += nt) {
+        int i = e % nb, j = e / nb;
+        if (i >= j) S[i + (long)j * lds] = sL[i * ld + j];
+        W[i + (long)j * ldw] = sX[i * ld + j];
+    }
+}
+
+template <class T>
+static int leaf(int nb, int off, int batch, void *S, long lds, long sS, void *W, long ldw, long sW, int *info,
+                cudaStream_t st) {
+    size_t smem = 2 * (size_t)nb * (nb + 1) * sizeof(T);
+    static bool attr = false;
+    if (!attr) {
+        NAO_CUDA_CHECK(cudaFuncSetAttribute(chol_leaf_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                            (int)(2 * CHOL_LEAF * (CHOL_LEAF + 1) * sizeof(T))));
+        attr = true;
+    }
+    chol_leaf_kernel<T><<<batch, 256, smem, st>>>(nb, off, (T *)S, lds, sS, (T *)W, ldw, sW, info);
+    NAO_LAUNCHED();
+    NAO_CUDA_CHECK(cudaGetLastError());
+    return NAO_OK;
+}
+
+struct CholCtx {
+    int dtype, batch; size_t es;
+    char *S; long lds, sS; char *W; long ldw, sW; char *T; long ldt, sT; int *info; cudaStream_t st;
+    void *s(int i, int j) const { return S + ((size_t)i + (size_t)j * lds) * es; }
+    void *w(int i, int j) const { return W + ((size_t)i + (size_t)j * ldw) * es; }
+    void *t(int i, int j) const { return T + ((size_t)i + (size_t)j * ldt) * es; }
+};
+
+static int rec(const CholCtx &c, int off, int n) {
+    int rc;
+    if (n <= CHOL_LEAF) {
+        return c.dtype == NAO_COMPLEX ? leaf<cplx>(n, off, c.batch, c.S, c.lds, c.sS, c.W, c.ldw, c.sW, c.info, c.st)
+                                      : leaf<double>(n, off, c.batch, c.S, c.lds, c.sS, c.W, c.ldw, c.sW, c.info, c.st);
+    }
+    int n1 = ((n / 2 + CHOL_LEAF - 1) / CHOL_LEAF) * CHOL_LEAF;
+    if (n1 >= n) n1 = n / 2;
+    int n2 = n - n1, o2 = off + n1;
+    if ((rc = rec(c, off, n1))) return rc;
+    // T21 = S21 * W11^H
+    GemmDesc d = gemm_desc(OP_N, OP_C, n2, n1, n1, 1.0, c.s(o2, off), c.lds, c.w(off, off), c.ldw, 0.0, c.t(o2, off), c.ldt);
+    d.sA = c.sS; d.sB = c.sW; d.sC = c.sT; d.maskB = MASK_LOWER;
+    if ((rc = gemm_launch(c.dtype, d, c.batch, c.st))) return rc;
+    if ((rc = copy_matrix(c.dtype, n2, n1, c.t(o2, off), c.ldt, c.sT, c.s(o2, off), c.lds, c.sS, c.batch, 0, c.st))) return rc;
+    // S22 -= L21 L21^H  (lower tiles)
+    d = gemm_desc(OP_N, OP_C, n2, n2, n1, -1.0, c.s(o2, off), c.lds, c.s(o2, off), c.lds, 1.0, c.s(o2, o2), c.lds);
+    d.sA = c.sS; d.sB = c.sS; d.sC = c.sS; d.cmode = 1;
+    if ((rc = gemm_launch(c.dtype, d, c.batch, c.st))) return rc;
+    if ((rc = rec(c, o2, n2))) return rc;
+    // T21 = L21 * W11
+    d = gemm_desc(OP_N, OP_N, n2, n1, n1, 1.0, c.s(o2, off), c.lds, c.w(off, off), c.ldw, 0.0, c.t(o2, off), c.ldt);
+    d.sA = c.sS; d.sB = c.sW; d.sC = c.sT; d.maskB = MASK_LOWER;
+    if ((rc = gemm_launch(c.dtype, d, c.batch, c.st))) return rc;
+    // W21 = -W22 * T21
+    d = gemm_desc(OP_N, OP_N, n2, n1, n2, -1.0, c.w(o2, o2), c.ldw, c.t(o2, off), c.ldt, 0.0, c.w(o2, off), c.ldw);
+    d.sA = c.sW; d.sB = c.sT; d.sC = c.sW; d.maskA = MASK_LOWER;
+    return gemm_launch(c.dtype, d, c.batch, c.st);
+}
+
+int potrf_trtri(int dtype, int n, int batch, void *S, long lds, long sS, void *W, long ldw, long sW, void *T, long ldt,
+                long sT, int *d_info, cudaStream_t st) {
+    CholCtx c{dtype, batch, esize(dtype), (char *)S, lds, sS, (char *)W, ldw, sW, (char *)T, ldt, sT, d_info, st};
+    // W's strict upper triangle must read as zero: leaves write their own blocks, the rest is cleared here
+    for (int b = 0; b < batch; ++b) {
+        // clear column by column only if ldw != n; the common case is a dense n x n buffer
+        if (ldw == n) { if (int rc = set_zero((char *)W + (size_t)b * sW * c.es, (size_t)n * n * c.es, st)) return rc; }
+        else for (int j = 0; j < n; ++j) if (int rc = set_zero((char *)W + ((size_t)b * sW + (size_t)j * ldw) * c.es, (size_t)n * c.es, st)) return rc;
+    }
+    return rec(c, 0, n);
+}
+
+}  // namespace nao
+
+NAO_EXPORT int nao_potrf_trtri(int n, int batch, int dtype, void *dS, long lds, long strideS, void *dLinv, void *dtmp,
+                               int *d_info, void *cuda_stream) {
+    using namespace nao;
+    if (n < 1) return -1;
+    if (batch < 1) return -2;
+    if (dtype != NAO_REAL && dtype != NAO_COMPLEX) return -3;
+    if (!dS) return -4;
+    if (lds < n) return -5;
+    if (batch > 1 && strideS < (long)lds * n) return -6;
+    if (!dLinv) return -7;
+    if (!dtmp) return -8;
+    if (!d_info) return -9;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (cudaMemsetAsync(d_info, 0, sizeof(int) * batch, st) != cudaSuccess) return NAO_ERR_CUDA;
+    int rc = potrf_trtri(dtype, n, batch, dS, lds, strideS, dLinv, n, (long)n * n, dtmp, n, (long)n * n, d_info, st);
+    if (rc) return rc;
+    return pack_linv(dtype, n, dS, lds, strideS, dLinv, n, (long)n * n, batch, st);
+}

@@ -1,0 +1,320 @@
+// gemm.cu -- FP64 tensor-core (DMMA) GEMM core for sm_100a.
+//
+// Every GEMM-class phase of the path (Cholesky trailing update, L^{-1} H L^{-H}, rank-2k updates of the
+// tridiagonalisation, divide-and-conquer merges, block-reflector back-transformation, C = L^{-H} Z and the
+// density matrix D = C f C^H) runs through this one kernel.
+//
+// sm_100a has no FP64 kind in tcgen05.mma; the FP64 tensor path is warp-level mma.sync.m8n8k4 (SASS DMMA.8x8x4),
+// fed from registers.  One DMMA per warp is 512 flop and occupies the FP64 pipe for ~16 issue slots, so the
+// instruction-issue and shared-memory load rates are far from limiting; what matters is (i) a CTA tile large
+// enough that L2->SM traffic stays small (128x128 real: 8 B/clk/SM), (ii) a multi-stage cp.async pipeline so the
+// DMMA pipe never waits, (iii) conflict-free 64/128-bit fragment loads (padding chosen per layout below).
+//
+// Complex products use real-arithmetic DMMAs on the (re, im) planes of interleaved operands:
+//   Cr += Ar*Br + (-Ai)*Bi ;  Ci += Ar*Bi + Ai*Br        (4 real DMMAs per complex tile product).
+//
+// Features: op(A), op(B) in {N, T, C}; real alpha/beta; triangular masks on either stored operand (elements
+// outside the triangle read as zero and the k-range is clipped, so TRMM/SYRK-shaped products skip the empty
+// half); "lower tiles only" output; optional scaling of op(A)'s k-th column by s[k] (Fermi weights);
+// strided batches and grouped launches whose descriptors (incl. m,n,k) live in device memory.
+#include "nao_internal.cuh"
+
+namespace nao {
+
+long g_launch_count = 0;
+
+__device__ __forceinline__ void cp_async8(void *smem, const void *g, bool pred) {
+    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    int sz = pred ? 8 : 0;
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(s), "l"(g), "r"(sz));
+}
+__device__ __forceinline__ void cp_async16(void *smem, const void *g, bool pred) {
+    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    int sz = pred ? 16 : 0;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(g), "r"(sz));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
+
+__device__ __forceinline__ void dmma(double &c0, double &c1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+__device__ __forceinline__ double negate(double x) { return -x; }
+
+__device__ __forceinline__ bool mask_keep(int mask, int off, int r, int c) {
+    int t = r - c + off;
+    return mask == MASK_NONE || (mask == MASK_LOWER && t >= 0) || (mask == MASK_SLOWER && t > 0) ||
+           (mask == MASK_UPPER && t <= 0) || (mask == MASK_SUPPER && t < 0);
+}
+// clip [kb, ke) given the mask on an operand whose other index spans [x0, x1]; k_is_col: stored (r,c) = (x,k)
+__device__ __forceinline__ void mask_krange(int mask, int off, bool k_is_col, int x0, int x1, int &kb, int &ke) {
+    if (mask == MASK_NONE) return;
+    bool lower = (mask == MASK_LOWER || mask == MASK_SLOWER);
+    if (k_is_col) {            // keep x - k + off >= 0 (lower) / <= 0 (upper)
+        if (lower) ke = min(ke, x1 + off + 1); else kb = max(kb, x0 + off);
+    } else {                   // (r,c) = (k,x): keep k - x + off >= 0 / <= 0
+        if (lower) kb = max(kb, x0 - off); else ke = min(ke, x1 - off + 1);
+    }
+}
+
+template <bool CPLX> struct Cfg;
+template <> struct Cfg<false> {
+    typedef double T;
+    static const int BM = 128, BN = 128, BK = 16, WM = 32, WN = 64, STAGES = 3, PADX = 4, PADK = 4;
+};
+template <> struct Cfg<true> {
+    typedef cplx T;
+    static const int BM = 128, BN = 64, BK = 16, WM = 32, WN = 32, STAGES = 3, PADX = 2, PADK = 2;
+};
+static const int GEMM_THREADS = 256;
+
+template <int BX, int BK, int PADX, int PADK> struct TileSize {
+    static const int XC = BK * (BX + PADX), KC = BX * (BK + PADK);
+    static const int value = XC > KC ? XC : KC;
+};
+
+// Load one BX x BK tile of op(P) into shared memory.
+//   xcontig: stored element (x,k) at P[x + k*ld]  -> smem [k][x], else stored at P[k + x*ld] -> smem [x][k].
+template <bool CPLX, int BX, int BK, int PADX, int PADK>
+__device__ __forceinline__ void load_tile(typename Cfg<CPLX>::T *s, const typename Cfg<CPLX>::T *P, long ld,
+                                          bool xcontig, int x0, int X, int k0, int kb, int ke, int mask, int off,
+                                          bool k_is_col) {
+    const int tid = threadIdx.x;
+    if (xcontig) {
+#pragma unroll
+        for (int it = 0; it < BX * BK / GEMM_THREADS; ++it) {
+            int e = tid + it * GEMM_THREADS;
+            int x = e % BX, k = e / BX;
+            int gx = x0 + x, gk = k0 + k;
+            bool p = gx < X && gk >= kb && gk < ke && (k_is_col ? mask_keep(mask, off, gx, gk) : mask_keep(mask, off, gk, gx));
+            const typename Cfg<CPLX>::T *src = p ? P + gx + (long)gk * ld : P;
+            if constexpr (CPLX) cp_async16(s + k * (BX + PADX) + x, src, p); else cp_async8(s + k * (BX + PADX) + x, src, p);
+        }
+    } else {
+#pragma unroll
+        for (int it = 0; it < BX * BK / GEMM_THREADS; ++it) {
+            int e = tid + it * GEMM_THREADS;
+            int k = e % BK, x = e / BK;
+            int gx = x0 + x, gk = k0 + k;
+            bool p = gx < X && gk >= kb && gk < ke && (k_is_col ? mask_keep(mask, off, gx, gk) : mask_keep(mask, off, gk, gx));
+            const typename Cfg<CPLX>::T *src = p ? P + gk + (long)gx * ld : P;
+            if constexpr (CPLX) cp_async16(s + x * (BK + PADK) + k, src, p); else cp_async8(s + x * (BK + PADK) + k, src, p);
+        }
+    }
+}
+
+template <bool CPLX>
+__global__ void __launch_bounds__(GEMM_THREADS, 1)
+gemm_kernel(const GemmDesc hd, const GemmDesc *__restrict__ dd) {
+    typedef Cfg<CPLX> G;
+    typedef typename G::T T;
+    constexpr int BM = G::BM, BN = G::BN, BK = G::BK, WM = G::WM, WN = G::WN, ST = G::STAGES;
+    constexpr int MI = WM / 8, NI = WN / 8;
+    constexpr int ASZ = TileSize<BM, BK, G::PADX, G::PADK>::value;
+    constexpr int BSZ = TileSize<BN, BK, G::PADX, G::PADK>::value;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T *sA = (T *)smem_raw;
+    T *sB = sA + ST * ASZ;
+    double *sS = (double *)(sB + ST * BSZ);     // ST * BK scale factors
+
+    const GemmDesc d = dd ? dd[blockIdx.z] : hd;
+    const int M = d.m, N = d.n, K = d.k;
+    if (M <= 0 || N <= 0) return;
+    const int tiles_m = (M + BM - 1) / BM, tiles_n = (N + BN - 1) / BN;
+    if ((int)blockIdx.x >= tiles_m * tiles_n) return;
+    const int tm = blockIdx.x % tiles_m, tn = blockIdx.x / tiles_m;
+    const int m0 = tm * BM, n0 = tn * BN;
+    if (d.cmode == 1 && n0 > m0 + BM - 1) return;
+
+    const long b = blockIdx.y;
+    const T *A = (const T *)d.A + b * d.sA;
+    const T *B = (const T *)d.B + b * d.sB;
+    T *C = (T *)d.C + b * d.sC;
+    const double *scaleK = d.scaleK ? d.scaleK + b * d.sScale : nullptr;
+
+    // op(A)(i,k): N -> stored (r,c) = (i,k), m-contiguous;  T/C -> stored (k,i), k-contiguous
+    const bool a_xc = (d.opA == OP_N), b_xc = (d.opB != OP_N);     // op(B)(k,j): N -> stored (k,j) k-contig
+    const bool a_kcol = a_xc, b_kcol = b_xc;                        // is k the stored column index?
+    const bool conjA = CPLX && d.opA == OP_C, conjB = CPLX && d.opB == OP_C;
+
+    int kb = 0, ke = K;
+    mask_krange(d.maskA, d.offA, a_kcol, m0, min(m0 + BM, M) - 1, kb, ke);
+    mask_krange(d.maskB, d.offB, b_kcol, n0, min(n0 + BN, N) - 1, kb, ke);
+    kb = max(kb, 0); ke = min(ke, K);
+    const int kt0 = kb / BK;
+    const int nkt = ke > kb ? (ke - 1) / BK + 1 - kt0 : 0;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    constexpr int WARPS_M = BM / WM;
+    const int wm = (warp % WARPS_M) * WM, wn = (warp / WARPS_M) * WN;
+    const int lr = lane >> 2, lc = lane & 3;
+
+    double acc[MI][NI][CPLX ? 4 : 2];
+#pragma unroll
+    for (int i = 0; i < MI; ++i)
+#pragma unroll
+        for (int j = 0; j < NI; ++j)
+#pragma unroll
+            for (int q = 0; q < (CPLX ? 4 : 2); ++q) acc[i][j][q] = 0.0;
+
+    const int a_sx = a_xc ? 1 : (BK + G::PADK), a_sk = a_xc ? (BM + G::PADX) : 1;
+    const int b_sx = b_xc ? 1 : (BK + G::PADK), b_sk = b_xc ? (BN + G::PADX) : 1;
+
+    auto issue = [&](int kt_rel) {
+        if (kt_rel < nkt) {
+            int stg = kt_rel % ST;
+            int k0 = (kt0 + kt_rel) * BK;
+            load_tile<CPLX, BM, BK, G::PADX, G::PADK>(sA + stg * ASZ, A, d.lda, a_xc, m0, M, k0, kb, ke, d.maskA, d.offA, a_kcol);
+            load_tile<CPLX, BN, BK, G::PADX, G::PADK>(sB + stg * BSZ, B, d.ldb, b_xc, n0, N, k0, kb, ke, d.maskB, d.offB, b_kcol);
+            if (scaleK && threadIdx.x < BK) {
+                int gk = k0 + threadIdx.x;
+                bool p = gk < ke;
+                cp_async8(sS + stg * BK + threadIdx.x, p ? scaleK + gk : scaleK, p);
+            }
+        }
+        cp_async_commit();
+    };
+
+    for (int s = 0; s < ST - 1; ++s) issue(s);
+
+    for (int kt = 0; kt < nkt; ++kt) {
+        cp_async_wait<ST - 2>();
+        __syncthreads();
+        issue(kt + ST - 1);
+        const T *a_s = sA + (kt % ST) * ASZ;
+        const T *b_s = sB + (kt % ST) * BSZ;
+        const double *s_s = sS + (kt % ST) * BK;
+#pragma unroll
+        for (int kk = 0; kk < BK; kk += 4) {
+            if constexpr (!CPLX) {
+                double af[MI], bf[NI];
+#pragma unroll
+                for (int i = 0; i < MI; ++i) af[i] = ((const double *)a_s)[(wm + i * 8 + lr) * a_sx + (kk + lc) * a_sk];
+#pragma unroll
+                for (int j = 0; j < NI; ++j) bf[j] = ((const double *)b_s)[(wn + j * 8 + lr) * b_sx + (kk + lc) * b_sk];
+                if (scaleK) {
+                    double sc = s_s[kk + lc];
+#pragma unroll
+                    for (int i = 0; i < MI; ++i) af[i] *= sc;
+                }
+#pragma unroll
+                for (int i = 0; i < MI; ++i)
+#pragma unroll
+                    for (int j = 0; j < NI; ++j) dmma(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+            } else {
+                double ar[MI], ai[MI], nai[MI], br[NI], bi[NI];
+#pragma unroll
+                for (int i = 0; i < MI; ++i) {
+                    cplx v = ((const cplx *)a_s)[(wm + i * 8 + lr) * a_sx + (kk + lc) * a_sk];
+                    ar[i] = v.x; ai[i] = conjA ? -v.y : v.y;
+                }
+#pragma unroll
+                for (int j = 0; j < NI; ++j) {
+                    cplx v = ((const cplx *)b_s)[(wn + j * 8 + lr) * b_sx + (kk + lc) * b_sk];
+                    br[j] = v.x; bi[j] = conjB ? -v.y : v.y;
+                }
+                if (scaleK) {
+                    double sc = s_s[kk + lc];
+#pragma unroll
+                    for (int i = 0; i < MI; ++i) { ar[i] *= sc; ai[i] *= sc; }
+                }
+#pragma unroll
+                for (int i = 0; i < MI; ++i) nai[i] = -ai[i];
+#pragma unroll
+                for (int i = 0; i < MI; ++i)
+#pragma unroll
+                    for (int j = 0; j < NI; ++j) {
+                        dmma(acc[i][j][0], acc[i][j][1], ar[i], br[j]);
+                        dmma(acc[i][j][0], acc[i][j][1], nai[i], bi[j]);
+                        dmma(acc[i][j][2], acc[i][j][3], ar[i], bi[j]);
+                        dmma(acc[i][j][2], acc[i][j][3], ai[i], br[j]);
+                    }
+            }
+        }
+    }
+    cp_async_wait<0>();
+
+    // epilogue: lane holds C[row = lr][cols 2*lc, 2*lc+1] of each 8x8 block
+    const double alpha = d.alpha, beta = d.beta;
+#pragma unroll
+    for (int i = 0; i < MI; ++i) {
+        int gi = m0 + wm + i * 8 + lr;
+        if (gi >= M) continue;
+#pragma unroll
+        for (int j = 0; j < NI; ++j) {
+#pragma unroll
+            for (int q = 0; q < 2; ++q) {
+                int gj = n0 + wn + j * 8 + 2 * lc + q;
+                if (gj >= N) continue;
+                T *p = C + gi + (long)gj * d.ldc;
+                if constexpr (!CPLX) {
+                    double v = alpha * acc[i][j][q];
+                    if (beta != 0.0) v += beta * *(double *)p;
+                    *(double *)p = v;
+                } else {
+                    cplx v; v.x = alpha * acc[i][j][q]; v.y = alpha * acc[i][j][2 + q];
+                    if (beta != 0.0) { cplx o = *(cplx *)p; v.x += beta * o.x; v.y += beta * o.y; }
+                    *(cplx *)p = v;
+                }
+            }
+        }
+    }
+}
+
+template <bool CPLX> static size_t gemm_smem_bytes() {
+    typedef Cfg<CPLX> G;
+    size_t a = TileSize<G::BM, G::BK, G::PADX, G::PADK>::value, b = TileSize<G::BN, G::BK, G::PADX, G::PADK>::value;
+    return G::STAGES * (a + b) * sizeof(typename G::T) + G::STAGES * G::BK * sizeof(double);
+}
+
+template <bool CPLX>
+static int launch_impl(const GemmDesc *hd, const GemmDesc *dd, int ngroups, int max_m, int max_n, int batch,
+                       cudaStream_t st) {
+    typedef Cfg<CPLX> G;
+    static bool attr_set = false;
+    size_t smem = gemm_smem_bytes<CPLX>();
+    if (!attr_set) {
+        NAO_CUDA_CHECK(cudaFuncSetAttribute(gemm_kernel<CPLX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set = true;
+    }
+    if (max_m <= 0 || max_n <= 0 || batch <= 0 || ngroups <= 0) return NAO_OK;
+    long tiles = (long)ceil_div(max_m, G::BM) * ceil_div(max_n, G::BN);
+    dim3 grid((unsigned)tiles, (unsigned)batch, (unsigned)ngroups);
+    GemmDesc dummy = hd ? *hd : gemm_desc(0, 0, 0, 0, 0, 0, nullptr, 0, nullptr, 0, 0, nullptr, 0);
+    gemm_kernel<CPLX><<<grid, GEMM_THREADS, smem, st>>>(dummy, dd);
+    NAO_LAUNCHED();
+    NAO_CUDA_CHECK(cudaGetLastError());
+    return NAO_OK;
+}
+
+int gemm_launch(int dtype, const GemmDesc &d, int batch, cudaStream_t st) {
+    if (d.m <= 0 || d.n <= 0) return NAO_OK;
+    return dtype == NAO_COMPLEX ? launch_impl<true>(&d, nullptr, 1, d.m, d.n, batch, st)
+                                : launch_impl<false>(&d, nullptr, 1, d.m, d.n, batch, st);
+}
+int gemm_launch_grouped(int dtype, const GemmDesc *dd, int ngroups, int max_m, int max_n, int batch, cudaStream_t st) {
+    return dtype == NAO_COMPLEX ? launch_impl<true>(nullptr, dd, ngroups, max_m, max_n, batch, st)
+                                : launch_impl<false>(nullptr, dd, ngroups, max_m, max_n, batch, st);
+}
+
+}  // namespace nao
+
+NAO_EXPORT int nao_gemm(int dtype, int opA, int opB, int m, int n, int k, double alpha, const void *dA, long lda,
+                        long strideA, const void *dB, long ldb, long strideB, double beta, void *dC, long ldc,
+                        long strideC, int batch, int uplo_c, void *cuda_stream) {
+    using namespace nao;
+    if (dtype != NAO_REAL && dtype != NAO_COMPLEX) return -1;
+    if (opA < 0 || opA > 2) return -2;
+    if (opB < 0 || opB > 2) return -3;
+    if (m < 0) return -4;
+    if (n < 0) return -5;
+    if (k < 0) return -6;
+    if (!dA && m > 0 && k > 0) return -8;
+    if (!dB && n > 0 && k > 0) return -11;
+    if (!dC && m > 0 && n > 0) return -15;
+    if (batch < 0) return -18;
+    GemmDesc d = gemm_desc(opA, opB, m, n, k, alpha, dA, lda, dB, ldb, beta, dC, ldc);
+    d.sA = strideA; d.sB = strideB; d.sC = strideC; d.cmode = uplo_c ? 1 : 0;
+    return gemm_launch(dtype, d, batch, (cudaStream_t)cuda_stream);
+}

@@ -1,0 +1,124 @@
+// nao_internal.cuh -- shared declarations of the sm_100a kernels behind include/nao.h.
+// Product code: shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include "../../include/nao.h"
+
+#define NAO_EXPORT extern "C" __attribute__((visibility("default")))
+
+namespace nao {
+
+typedef double2 cplx;   // interleaved complex FP64 (x = re, y = im)
+
+// ---------------------------------------------------------------------------------------------------------
+// launch bookkeeping
+// ---------------------------------------------------------------------------------------------------------
+extern long g_launch_count;          // host-side count of kernel launches (nao_launch_count)
+#define NAO_LAUNCHED() (++::nao::g_launch_count)
+
+#define NAO_CUDA_CHECK(expr)                                        \
+    do {                                                            \
+        cudaError_t e__ = (expr);                                   \
+        if (e__ != cudaSuccess) return NAO_ERR_CUDA;                \
+    } while (0)
+
+static inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+static inline int ceil_div(int a, int b) { return (a + b - 1) / b; }
+static inline size_t esize(int dtype) { return dtype == NAO_COMPLEX ? 16 : 8; }
+
+// bump allocator over the caller's workspace
+struct Arena {
+    char *base; size_t cap; size_t off;
+    Arena(void *p, size_t c) : base((char *)p), cap(c), off(0) {}
+    void *take(size_t bytes) {
+        size_t o = off; off += align_up(bytes);
+        return (off <= cap) ? (void *)(base + o) : nullptr;
+    }
+    template <class T> T *get(size_t count) { return (T *)take(count * sizeof(T)); }
+};
+
+// ---------------------------------------------------------------------------------------------------------
+// DMMA GEMM (gemm.cu)
+// ---------------------------------------------------------------------------------------------------------
+enum { OP_N = 0, OP_T = 1, OP_C = 2 };
+// triangular masks on the STORED operand, coordinates (r, c):  keep the element iff (r - c + off) REL 0
+enum { MASK_NONE = 0, MASK_LOWER = 1 /* >= */, MASK_SLOWER = 2 /* > */, MASK_UPPER = 3 /* <= */, MASK_SUPPER = 4 /* < */ };
+
+struct GemmDesc {
+    const void *A; const void *B; void *C;
+    long lda, ldb, ldc;
+    long sA, sB, sC;          // batch strides (elements)
+    int m, n, k;              // product dimensions: C (m x n) = op(A) (m x k) * op(B) (k x n)
+    int opA, opB;
+    int maskA, offA, maskB, offB;
+    int cmode;                // 0 full; 1 = skip tiles entirely above the diagonal of C
+    int conjC;                // unused (reserved)
+    double alpha, beta;
+    const double *scaleK;     // optional: op(A)[:,k] is multiplied by scaleK[k]
+    long sScale;              // batch stride of scaleK
+};
+
+static inline GemmDesc gemm_desc(int opA, int opB, int m, int n, int k, double alpha, const void *A, long lda,
+                                 const void *B, long ldb, double beta, void *C, long ldc) {
+    GemmDesc d;
+    d.A = A; d.B = B; d.C = C; d.lda = lda; d.ldb = ldb; d.ldc = ldc; d.sA = d.sB = d.sC = 0;
+    d.m = m; d.n = n; d.k = k; d.opA = opA; d.opB = opB; d.maskA = d.maskB = MASK_NONE; d.offA = d.offB = 0;
+    d.cmode = 0; d.conjC = 0; d.alpha = alpha; d.beta = beta; d.scaleK = nullptr; d.sScale = 0;
+    return d;
+}
+
+// One problem described on the host (passed by value), `batch` items via the strides in the descriptor.
+int gemm_launch(int dtype, const GemmDesc &d, int batch, cudaStream_t st);
+// `ngroups` problems described by descriptors in DEVICE memory (their m,n,k may have been written by a kernel);
+// max_m/max_n bound the grid.  Each group runs `batch` items.
+int gemm_launch_grouped(int dtype, const GemmDesc *d_descs, int ngroups, int max_m, int max_n, int batch,
+                        cudaStream_t st);
+
+// ---------------------------------------------------------------------------------------------------------
+// element-wise helpers (util.cu)
+// ---------------------------------------------------------------------------------------------------------
+// B <- A for the m x n block (both column-major); uplo: 0 all, 1 lower only (i >= j), 2 strict upper only
+int copy_matrix(int dtype, int m, int n, const void *A, long lda, long sA, void *B, long ldb, long sB, int batch,
+                int uplo, cudaStream_t st);
+// B (full) <- Hermitian completion of the lower triangle of A (B may equal A: in-place mirror)
+int herm_fill(int dtype, int n, const void *A, long lda, long sA, void *B, long ldb, long sB, int batch,
+              cudaStream_t st);
+int set_zero(void *p, size_t bytes, cudaStream_t st);
+// real n x n (ldq) -> complex n x n (ldz)
+int real_to_complex(int m, int n, const double *Q, long ldq, long sQ, cplx *Z, long ldz, long sZ, int batch,
+                    cudaStream_t st);
+// Linv (n x n lower, explicit zeros above, diagonal = 1/L_ii) from the packed factor in S (see nao.h)
+int unpack_linv(int dtype, int n, const void *S, long lds, long sS, void *W, long ldw, long sW, int batch,
+                cudaStream_t st);
+int pack_linv(int dtype, int n, void *S, long lds, long sS, const void *W, long ldw, long sW, int batch,
+              cudaStream_t st);
+
+// ---------------------------------------------------------------------------------------------------------
+// phases
+// ---------------------------------------------------------------------------------------------------------
+// chol.cu: S -> L (in S lower), W <- L^{-1}; T = n*n scratch.  info[b] = 0 or failing pivot (1-based)
+int potrf_trtri(int dtype, int n, int batch, void *S, long lds, long sS, void *W, long ldw, long sW, void *T,
+                long ldt, long sT, int *d_info, cudaStream_t st);
+
+// trd1.cu: one-stage Householder tridiagonalisation of the lower triangle of A (n x n); reflectors left below the
+// first sub-diagonal of A (LAPACK xHETRD lower convention), d[n], e[n-1] real, tau[n-1].
+size_t hetrd_workspace(int dtype, int n, int batch);
+int hetrd(int dtype, int n, int batch, void *A, long lda, long sA, double *d, double *e, void *tau, void *work,
+          cudaStream_t st);
+// Z <- Q_house * Z where Q_house = H_0 H_1 ... H_{n-2} from hetrd (Z n x ncols)
+size_t ormtr_workspace(int dtype, int n, int batch);
+int ormtr(int dtype, int n, int ncols, int batch, const void *A, long lda, long sA, const void *tau, void *Z,
+          long ldz, long sZ, void *work, cudaStream_t st);
+
+// stedc.cu
+size_t stedc_workspace(int n, int batch);
+int stedc(int n, int batch, double *d, double *e, double *evals, double *Q, long ldq, long sQ, void *work,
+          int *d_info, cudaStream_t st);
+
+// fermi.cu / density
+int fermi_mu(int n, int batch, const double *dE, const double *h_weight, double n_electrons, double kT, double *h_mu,
+             double *dF, void *dwork, cudaStream_t st);
+
+}  // namespace nao
