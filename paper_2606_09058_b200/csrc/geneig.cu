@@ -1,0 +1,183 @@
+// geneig.cu -- drivers: nao_heev (standard Hermitian problem) and nao_geneig (H C = S C diag(e)).
+//
+// nao_geneig (Eq. 5/11/21; the paper's Part 2 / Part 3):
+//   1. S = L L^H, W = L^{-1}                (skipped with NAO_S_FACTORED: W is unpacked from dS)
+//   2. A = W H W^H                          (paper: H' = V^H H V, Part 2-3 / 3-3; here V = W^H)
+//   3. A = Z diag(e) Z^H                    (Part 2-4 / 3-5)
+//   4. C = W^H Z                            (Part 2-5 / 3-6)
+// With NAO_NC_BLOCK_S the overlap is S_NC = diag(S, S) with S real N x N (Eq. 25-27): only the
+// real N x N S is factored and steps 2 and 4 run block-wise on the four N x N spin blocks.
+#include "nao_internal.cuh"
+#include <algorithm>
+
+namespace nao {
+
+// ----------------------------------------------------------------------------------------------------- heev
+struct HeevPlan { size_t d, e, tau, qt, sub, bytes; size_t sub_bytes; };
+static HeevPlan heev_plan(int dtype, int n, int batch) {
+    HeevPlan p; size_t off = 0;
+    auto take = [&](size_t b) { size_t o = off; off += align_up(b); return o; };
+    p.d = take((size_t)batch * n * 8); p.e = take((size_t)batch * n * 8); p.tau = take((size_t)batch * n * esize(dtype));
+    p.qt = take(dtype == NAO_COMPLEX ? (size_t)batch * n * n * 8 : 0);
+    p.sub_bytes = std::max(hetrd_workspace(dtype, n, batch), std::max(stedc_workspace(n, batch), ormtr_workspace(dtype, n, batch)));
+    p.sub = take(p.sub_bytes);
+    p.bytes = off;
+    return p;
+}
+
+static int heev(int dtype, int n, int batch, unsigned flags, void *A, long lda, long sA, double *E, void *Z, long ldz,
+                long sZ, void *work, int *d_info, cudaStream_t st) {
+    (void)flags;
+    HeevPlan p = heev_plan(dtype, n, batch);
+    char *w = (char *)work;
+    double *d = (double *)(w + p.d), *e = (double *)(w + p.e);
+    void *tau = w + p.tau, *sub = w + p.sub;
+    int rc;
+    if ((rc = hetrd(dtype, n, batch, A, lda, sA, d, e, tau, sub, st))) return rc;
+    if (dtype == NAO_COMPLEX) {
+        double *qt = (double *)(w + p.qt);
+        if ((rc = stedc(n, batch, d, e, E, qt, n, (long)n * n, sub, d_info, st))) return rc;
+        if ((rc = real_to_complex(n, n, qt, n, (long)n * n, (cplx *)Z, ldz, sZ, batch, st))) return rc;
+    } else {
+        if ((rc = stedc(n, batch, d, e, E, (double *)Z, ldz, sZ, sub, d_info, st))) return rc;
+    }
+    return ormtr(dtype, n, n, batch, A, lda, sA, tau, Z, ldz, sZ, sub, st);
+}
+
+// ----------------------------------------------------------------------------------------------------- geneig
+struct GePlan { size_t W, Wc, A, X, heev, bytes; int nS, sdtype, nitemsS; };
+static GePlan ge_plan(int n, int batch, int dtype, unsigned flags, bool shared_S) {
+    GePlan p; size_t off = 0;
+    auto take = [&](size_t b) { size_t o = off; off += align_up(b); return o; };
+    const bool nc = flags & NAO_NC_BLOCK_S;
+    p.nS = nc ? n / 2 : n; p.sdtype = nc ? NAO_REAL : dtype; p.nitemsS = shared_S ? 1 : batch;
+    p.W = take((size_t)p.nitemsS * p.nS * p.nS * esize(p.sdtype));
+    p.Wc = take(nc ? (size_t)p.nitemsS * p.nS * p.nS * 16 : 0);
+    p.A = take((size_t)batch * n * n * esize(dtype));
+    p.X = take((size_t)batch * n * n * esize(dtype));
+    p.heev = take(heev_plan(dtype, n, batch).bytes);
+    p.bytes = off;
+    return p;
+}
+
+}  // namespace nao
+
+NAO_EXPORT int nao_heev_workspace(int n, int batch, int dtype, unsigned flags, size_t *bytes) {
+    (void)flags;
+    if (n < 1) return -1;
+    if (batch < 1) return -2;
+    if (dtype != NAO_REAL && dtype != NAO_COMPLEX) return -3;
+    if (!bytes) return -5;
+    *bytes = nao::heev_plan(dtype, n, batch).bytes;
+    return NAO_OK;
+}
+
+NAO_EXPORT int nao_heev(int n, int batch, int dtype, unsigned flags, void *dA, long lda, long strideA, double *dE, void *dZ,
+                        long ldz, long strideZ, void *dwork, size_t work_bytes, int *d_info, void *cuda_stream) {
+    using namespace nao;
+    if (n < 1) return -1;
+    if (batch < 1) return -2;
+    if (dtype != NAO_REAL && dtype != NAO_COMPLEX) return -3;
+    if (!dA) return -5;
+    if (lda < n) return -6;
+    if (batch > 1 && strideA < lda * (long)n) return -7;
+    if (!dE) return -8;
+    if (!dZ) return -9;
+    if (ldz < n) return -10;
+    if (batch > 1 && strideZ < ldz * (long)n) return -11;
+    if (!dwork) return -12;
+    if (work_bytes < heev_plan(dtype, n, batch).bytes) return NAO_ERR_WORKSPACE;
+    if (!d_info) return -14;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (cudaMemsetAsync(d_info, 0, sizeof(int) * batch, st) != cudaSuccess) return NAO_ERR_CUDA;
+    return heev(dtype, n, batch, flags, dA, lda, strideA, dE, dZ, ldz, strideZ, dwork, d_info, st);
+}
+
+NAO_EXPORT int nao_geneig_workspace(int n, int batch, int dtype, unsigned flags, size_t *bytes) {
+    if (n < 1) return -1;
+    if (batch < 1) return -2;
+    if (dtype != NAO_REAL && dtype != NAO_COMPLEX) return -3;
+    if ((flags & NAO_NC_BLOCK_S) && (dtype != NAO_COMPLEX || (n & 1))) return -4;
+    if (!bytes) return -5;
+    *bytes = nao::ge_plan(n, batch, dtype, flags, false).bytes;
+    return NAO_OK;
+}
+
+NAO_EXPORT int nao_geneig(int n, int batch, int dtype, unsigned flags, const void *dH, long ldh, long strideH, void *dS,
+                          long lds, long strideS, double *dE, void *dC, long ldc, long strideC, void *dwork,
+                          size_t work_bytes, int *d_info, void *cuda_stream) {
+    using namespace nao;
+    if (n < 1) return -1;
+    if (batch < 1) return -2;
+    if (dtype != NAO_REAL && dtype != NAO_COMPLEX) return -3;
+    const bool nc = flags & NAO_NC_BLOCK_S;
+    if (nc && (dtype != NAO_COMPLEX || (n & 1))) return -4;
+    const int nS = nc ? n / 2 : n;
+    if (!dH) return -5;
+    if (ldh < n) return -6;
+    if (batch > 1 && strideH < ldh * (long)n) return -7;
+    if (!dS) return -8;
+    if (lds < nS) return -9;
+    const bool shared_S = (strideS == 0);
+    if (shared_S && !nc && batch > 1) return -10;
+    if (!shared_S && batch > 1 && strideS < lds * (long)nS) return -10;
+    if (!dE) return -11;
+    if (!dC) return -12;
+    if (ldc < n) return -13;
+    if (batch > 1 && strideC < ldc * (long)n) return -14;
+    if (!dwork) return -15;
+    GePlan p = ge_plan(n, batch, dtype, flags, shared_S);
+    if (work_bytes < p.bytes) return NAO_ERR_WORKSPACE;
+    if (!d_info) return -17;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    char *w = (char *)dwork;
+    const size_t es = esize(dtype);
+    void *W = w + p.W, *A = w + p.A, *X = w + p.X;
+    const long sW = (long)nS * nS, sAX = (long)n * n;
+    int rc;
+    NAO_CUDA_CHECK(cudaMemsetAsync(d_info, 0, sizeof(int) * batch, st));
+
+    // 1. factor (or unpack) S
+    if (!(flags & NAO_S_FACTORED)) {
+        // with a shared S the (single) status goes to d_info[0]
+        if ((rc = potrf_trtri(p.sdtype, nS, p.nitemsS, dS, lds, strideS, W, nS, sW, X, nS, sW, d_info, st))) return rc;
+        if ((rc = pack_linv(p.sdtype, nS, dS, lds, strideS, W, nS, sW, p.nitemsS, st))) return rc;
+    } else {
+        if ((rc = unpack_linv(p.sdtype, nS, dS, lds, strideS, W, nS, sW, p.nitemsS, st))) return rc;
+    }
+    const void *Wm = W;          // the operand used in the products (complex copy in the NC case)
+    if (nc) {
+        if ((rc = real_to_complex(nS, nS, (const double *)W, nS, sW, (cplx *)(w + p.Wc), nS, sW, p.nitemsS, st))) return rc;
+        Wm = w + p.Wc;
+    }
+    const long sWm = shared_S ? 0 : sW;
+
+    // 2. A = W H W^H : full Hermitian copy of H, X = W A (triangular W), A = X W^H (lower tiles)
+    if ((rc = herm_fill(dtype, n, dH, ldh, strideH, A, n, sAX, batch, st))) return rc;
+    const int nb = nc ? 2 : 1;
+    auto blk = [&](void *base, int bi, int bj) { return (void *)((char *)base + ((size_t)bi * nS + (size_t)bj * nS * n) * es); };
+    for (int bi = 0; bi < nb; ++bi)
+        for (int bj = 0; bj <= bi; ++bj) {
+            GemmDesc g = gemm_desc(OP_N, OP_N, nS, nS, nS, 1.0, Wm, nS, blk(A, bi, bj), n, 0.0, blk(X, bi, bj), n);
+            g.sA = sWm; g.sB = sAX; g.sC = sAX; g.maskA = MASK_LOWER;
+            if ((rc = gemm_launch(dtype, g, batch, st))) return rc;
+        }
+    for (int bi = 0; bi < nb; ++bi)
+        for (int bj = 0; bj <= bi; ++bj) {
+            GemmDesc g = gemm_desc(OP_N, OP_C, nS, nS, nS, 1.0, blk(X, bi, bj), n, Wm, nS, 0.0, blk(A, bi, bj), n);
+            g.sA = sAX; g.sB = sWm; g.sC = sAX; g.maskB = MASK_LOWER; g.cmode = (bi == bj) ? 1 : 0;
+            if ((rc = gemm_launch(dtype, g, batch, st))) return rc;
+        }
+
+    // 3. standard problem; eigenvectors into X
+    if ((rc = heev(dtype, n, batch, flags, A, n, sAX, dE, X, n, sAX, w + p.heev, d_info, st))) return rc;
+
+    // 4. C = W^H Z, per row block
+    for (int bi = 0; bi < nb; ++bi) {
+        GemmDesc g = gemm_desc(OP_C, OP_N, nS, n, nS, 1.0, Wm, nS, (char *)X + (size_t)bi * nS * es, n, 0.0,
+                               (char *)dC + (size_t)bi * nS * es, ldc);
+        g.sA = sWm; g.sB = sAX; g.sC = strideC; g.maskA = MASK_LOWER;
+        if ((rc = gemm_launch(dtype, g, batch, st))) return rc;
+    }
+    return NAO_OK;
+}

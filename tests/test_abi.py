@@ -1,0 +1,80 @@
+"""Host-side checks that need no GPU: the C-ABI library builds for sm_100a, loads, and exports every symbol that
+include/nao.h declares; argument validation happens on the host before any launch."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def libpath():
+    from paper_2606_09058_b200 import build as nao_build
+    return nao_build.build()
+
+
+def _declared_symbols():
+    text = open(os.path.join(ROOT, "include", "nao.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(nao_[a-z_0-9]+)\s*\(", text)))
+
+
+def test_header_symbols_are_exported(libpath):
+    lib = ctypes.CDLL(libpath)
+    names = _declared_symbols()
+    assert len(names) >= 14
+    for name in names:
+        assert hasattr(lib, name), "libnao.so does not export %s" % name
+
+
+def test_binding_covers_header():
+    from paper_2606_09058_b200 import binding
+    assert sorted(binding.EXPORTS) == _declared_symbols()
+
+
+def test_library_is_sm100a_with_fp64_tensor_instructions(libpath):
+    """The GEMM core must contain DMMA (FP64 tensor) SASS for sm_100a."""
+    import subprocess
+    out = subprocess.run(["cuobjdump", "-sass", libpath], capture_output=True, text=True).stdout
+    assert "arch = sm_100a" in out
+    assert "DMMA" in out and "gemm_kernel" in out
+
+
+def test_host_side_argument_validation(libpath):
+    """Bad arguments are rejected on the host with -(argument index): no CUDA call is made (works without a GPU)."""
+    lib = ctypes.CDLL(libpath)
+    sz = ctypes.c_size_t(0)
+    assert lib.nao_geneig_workspace(0, 1, 0, 0, ctypes.byref(sz)) == -1
+    assert lib.nao_geneig_workspace(8, 0, 0, 0, ctypes.byref(sz)) == -2
+    assert lib.nao_geneig_workspace(8, 1, 7, 0, ctypes.byref(sz)) == -3
+    assert lib.nao_geneig_workspace(7, 1, 1, 2, ctypes.byref(sz)) == -4      # NC needs even n
+    assert lib.nao_geneig_workspace(104, 1, 0, 0, ctypes.byref(sz)) == 0 and sz.value > 104 * 104 * 8 * 2
+    assert lib.nao_fermi_workspace(104, 1, ctypes.byref(sz)) == 0 and sz.value >= 2 * 104 * 8
+    assert lib.nao_density_workspace(104, 3, 1, ctypes.byref(sz)) == 0 and sz.value > 0
+    lib.nao_status_string.restype = ctypes.c_char_p
+    assert lib.nao_status_string(0) == b"ok"
+    assert b"workspace" in lib.nao_status_string(1)
+    lib.nao_version.restype = ctypes.c_char_p
+    assert b"sm_100a" in lib.nao_version()
+    # nao_fermi_mu: electron count outside (0, sum w n) is an error before anything is launched
+    lib.nao_fermi_mu.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_void_p, ctypes.POINTER(ctypes.c_double),
+                                 ctypes.c_double, ctypes.c_double, ctypes.POINTER(ctypes.c_double), ctypes.c_void_p,
+                                 ctypes.c_void_p, ctypes.c_void_p]
+    w = (ctypes.c_double * 1)(2.0)
+    mu = ctypes.c_double(0)
+    assert lib.nao_fermi_mu(4, 1, 1, w, 9.0, 1e-3, ctypes.byref(mu), 1, 1, None) == 3      # NAO_ERR_ELECTRONS
+    assert lib.nao_fermi_mu(4, 1, 1, w, 2.0, 0.0, ctypes.byref(mu), 1, 1, None) == 3
+    assert lib.nao_fermi_mu(4, 1, None, w, 2.0, 1e-3, ctypes.byref(mu), 1, 1, None) == -3
+
+
+def test_no_product_import_of_oracle():
+    """The product package must never import or call oracle/ (or a CPU fallback)."""
+    pkg = os.path.join(ROOT, "paper_2606_09058_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".c", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in text and "from oracle" not in text, f
+                assert "nao_oracle" not in text and "oracle_impl" not in text, f
