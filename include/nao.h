@@ -130,6 +130,22 @@ const char *nao_version(void);
  */
 long nao_launch_count(void);
 
+/*
+ * Optional phase timing of nao_geneig: when enabled, CUDA events are recorded on the caller's stream at the phase
+ * boundaries (potrf_trtri, reduce, tridiagonalise, stedc, back_transform, C = W^H Z).  nao_profile_read waits for the
+ * events of the LAST nao_geneig call and writes the phase durations in milliseconds; returns the number written.
+ */
+int nao_profile_enable(int on);
+int nao_profile_read(double *h_ms, int max_phases);
+const char *nao_profile_phase_name(int i);
+/*
+ * Per-kernel-class timers (profiling enabled only): events bracket each launch of the class on the caller's stream.
+ * slot 0 = hetrd_panel_kernel (HBM-bound; *h_work = algorithmic bytes), slot 1 = reserved.  Sums since the last
+ * nao_profile_enable call: total milliseconds, total algorithmic work, number of launches.
+ */
+int nao_profile_kernel(int slot, double *h_ms, double *h_work, int *h_launches);
+const char *nao_profile_kernel_name(int slot);
+
 /* ---- building blocks exported for tests and per-kernel measurement (same pointer/stream conventions) ---- */
 
 /*

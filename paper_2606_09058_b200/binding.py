@@ -35,6 +35,11 @@ _SIGNATURES = {
     "nao_status_string": ([_i], ctypes.c_char_p),
     "nao_version": ([], ctypes.c_char_p),
     "nao_launch_count": ([], _l),
+    "nao_profile_enable": ([_i], _i),
+    "nao_profile_read": ([_dp, _i], _i),
+    "nao_profile_phase_name": ([_i], ctypes.c_char_p),
+    "nao_profile_kernel": ([_i, _dp, _dp, ctypes.POINTER(ctypes.c_int)], _i),
+    "nao_profile_kernel_name": ([_i], ctypes.c_char_p),
     "nao_gemm": ([_i, _i, _i, _i, _i, _i, _d, _vp, _l, _l, _vp, _l, _l, _d, _vp, _l, _l, _i, _i, _vp], _i),
     "nao_potrf_trtri": ([_i, _i, _i, _vp, _l, _l, _vp, _vp, _vp, _vp], _i),
     "nao_heev_workspace": ([_i, _i, _i, ctypes.c_uint, _szp], _i),
@@ -104,6 +109,24 @@ def _workspace(nbytes: int, device) -> torch.Tensor:
 
 def launch_count() -> int:
     return int(lib().nao_launch_count())
+
+
+def profile_enable(on: bool = True) -> None:
+    lib().nao_profile_enable(int(on))
+
+
+def profile_read() -> dict:
+    """Phase durations (ms) of the last nao_geneig call made with profiling enabled."""
+    buf = (ctypes.c_double * 8)()
+    k = lib().nao_profile_read(buf, 8)
+    return {lib().nao_profile_phase_name(i).decode(): buf[i] for i in range(k)}
+
+
+def profile_kernel(slot: int) -> dict:
+    """Summed per-launch timings of one kernel class since profile_enable(): ms, algorithmic work, launches."""
+    ms, work, k = ctypes.c_double(0), ctypes.c_double(0), ctypes.c_int(0)
+    _check(lib().nao_profile_kernel(slot, ctypes.byref(ms), ctypes.byref(work), ctypes.byref(k)), "nao_profile_kernel")
+    return {"name": lib().nao_profile_kernel_name(slot).decode(), "ms": ms.value, "work": work.value, "launches": k.value}
 
 
 def version() -> str:

@@ -14,3 +14,75 @@ NAO_EXPORT const char *nao_status_string(int status) {
 }
 NAO_EXPORT const char *nao_version(void) { return "nao-b200 0.1 (sm_100a)"; }
 NAO_EXPORT long nao_launch_count(void) { return nao::g_launch_count; }
+
+// ---- optional phase timing (CUDA events recorded on the caller's stream at phase boundaries of nao_geneig) ----
+namespace nao {
+static const int NPH = 7;
+static const char *kPhaseNames[NPH - 1] = {"potrf_trtri", "reduce_WHWh", "tridiagonalise", "stedc", "back_transform", "C_WhZ"};
+static bool g_prof_on = false;
+static cudaEvent_t g_ev[NPH];
+static bool g_ev_made = false, g_ev_rec[NPH];
+void prof_mark(int idx, cudaStream_t st) {
+    if (!g_prof_on || idx < 0 || idx >= NPH) return;
+    if (!g_ev_made) { for (int i = 0; i < NPH; ++i) cudaEventCreate(&g_ev[i]); g_ev_made = true; }
+    if (idx == 0) for (int i = 0; i < NPH; ++i) g_ev_rec[i] = false;
+    cudaEventRecord(g_ev[idx], st); g_ev_rec[idx] = true;
+}
+}  // namespace nao
+namespace nao {
+// per-kernel-class timers: pairs of events around individual launches (only while profiling is enabled)
+static const int NSLOT = 2, SLOT_CAP = 2048;
+static const char *kSlotNames[NSLOT] = {"hetrd_panel_kernel", "gemm_kernel"};
+static cudaEvent_t g_sev[NSLOT][SLOT_CAP][2];
+static int g_scount[NSLOT] = {0, 0}, g_smade[NSLOT] = {0, 0};
+static double g_swork[NSLOT] = {0.0, 0.0};
+int prof_kernel_begin(int slot, double work, cudaStream_t st) {
+    if (!g_prof_on || slot < 0 || slot >= NSLOT || g_scount[slot] >= SLOT_CAP) return -1;
+    int k = g_scount[slot];
+    if (k >= g_smade[slot]) { cudaEventCreate(&g_sev[slot][k][0]); cudaEventCreate(&g_sev[slot][k][1]); g_smade[slot] = k + 1; }
+    cudaEventRecord(g_sev[slot][k][0], st);
+    g_swork[slot] += work;
+    return k;
+}
+void prof_kernel_end(int slot, int k, cudaStream_t st) {
+    if (k < 0) return;
+    cudaEventRecord(g_sev[slot][k][1], st);
+    g_scount[slot] = k + 1;
+}
+}  // namespace nao
+NAO_EXPORT int nao_profile_enable(int on) {
+    nao::g_prof_on = on != 0;
+    for (int s = 0; s < nao::NSLOT; ++s) { nao::g_scount[s] = 0; nao::g_swork[s] = 0.0; }
+    return NAO_OK;
+}
+NAO_EXPORT int nao_profile_kernel(int slot, double *h_ms, double *h_work, int *h_launches) {
+    using namespace nao;
+    if (slot < 0 || slot >= NSLOT) return -1;
+    double tot = 0.0;
+    for (int k = 0; k < g_scount[slot]; ++k) {
+        cudaEventSynchronize(g_sev[slot][k][1]);
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, g_sev[slot][k][0], g_sev[slot][k][1]) == cudaSuccess) tot += ms;
+    }
+    if (h_ms) *h_ms = tot;
+    if (h_work) *h_work = g_swork[slot];
+    if (h_launches) *h_launches = g_scount[slot];
+    return NAO_OK;
+}
+NAO_EXPORT const char *nao_profile_kernel_name(int slot) { return (slot >= 0 && slot < nao::NSLOT) ? nao::kSlotNames[slot] : ""; }
+NAO_EXPORT int nao_profile_read(double *h_ms, int max_phases) {
+    using namespace nao;
+    if (!h_ms) return -1;
+    int np = 0;
+    for (int i = 0; i + 1 < NPH && i < max_phases; ++i) {
+        h_ms[i] = 0.0;
+        if (g_ev_made && g_ev_rec[i] && g_ev_rec[i + 1]) {
+            cudaEventSynchronize(g_ev[i + 1]);
+            float ms = 0.f;
+            if (cudaEventElapsedTime(&ms, g_ev[i], g_ev[i + 1]) == cudaSuccess) h_ms[i] = ms;
+        }
+        np = i + 1;
+    }
+    return np;
+}
+NAO_EXPORT const char *nao_profile_phase_name(int i) { return (i >= 0 && i < nao::NPH - 1) ? nao::kPhaseNames[i] : ""; }

@@ -33,7 +33,9 @@ static int heev(int dtype, int n, int batch, unsigned flags, void *A, long lda, 
     double *d = (double *)(w + p.d), *e = (double *)(w + p.e);
     void *tau = w + p.tau, *sub = w + p.sub;
     int rc;
+    prof_mark(2, st);
     if ((rc = hetrd(dtype, n, batch, A, lda, sA, d, e, tau, sub, st))) return rc;
+    prof_mark(3, st);
     if (dtype == NAO_COMPLEX) {
         double *qt = (double *)(w + p.qt);
         if ((rc = stedc(n, batch, d, e, E, qt, n, (long)n * n, sub, d_info, st))) return rc;
@@ -41,7 +43,10 @@ static int heev(int dtype, int n, int batch, unsigned flags, void *A, long lda, 
     } else {
         if ((rc = stedc(n, batch, d, e, E, (double *)Z, ldz, sZ, sub, d_info, st))) return rc;
     }
-    return ormtr(dtype, n, n, batch, A, lda, sA, tau, Z, ldz, sZ, sub, st);
+    prof_mark(4, st);
+    rc = ormtr(dtype, n, n, batch, A, lda, sA, tau, Z, ldz, sZ, sub, st);
+    prof_mark(5, st);
+    return rc;
 }
 
 // ----------------------------------------------------------------------------------------------------- geneig
@@ -138,6 +143,7 @@ NAO_EXPORT int nao_geneig(int n, int batch, int dtype, unsigned flags, const voi
     NAO_CUDA_CHECK(cudaMemsetAsync(d_info, 0, sizeof(int) * batch, st));
 
     // 1. factor (or unpack) S
+    prof_mark(0, st);
     if (!(flags & NAO_S_FACTORED)) {
         // with a shared S the (single) status goes to d_info[0]
         if ((rc = potrf_trtri(p.sdtype, nS, p.nitemsS, dS, lds, strideS, W, nS, sW, X, nS, sW, d_info, st))) return rc;
@@ -145,6 +151,7 @@ NAO_EXPORT int nao_geneig(int n, int batch, int dtype, unsigned flags, const voi
     } else {
         if ((rc = unpack_linv(p.sdtype, nS, dS, lds, strideS, W, nS, sW, p.nitemsS, st))) return rc;
     }
+    prof_mark(1, st);
     const void *Wm = W;          // the operand used in the products (complex copy in the NC case)
     if (nc) {
         if ((rc = real_to_complex(nS, nS, (const double *)W, nS, sW, (cplx *)(w + p.Wc), nS, sW, p.nitemsS, st))) return rc;
@@ -179,5 +186,6 @@ NAO_EXPORT int nao_geneig(int n, int batch, int dtype, unsigned flags, const voi
         g.sA = sWm; g.sB = sAX; g.sC = strideC; g.maskA = MASK_LOWER;
         if ((rc = gemm_launch(dtype, g, batch, st))) return rc;
     }
+    prof_mark(6, st);
     return NAO_OK;
 }

@@ -117,6 +117,12 @@ size_t stedc_workspace(int n, int batch);
 int stedc(int n, int batch, double *d, double *e, double *evals, double *Q, long ldq, long sQ, void *work,
           int *d_info, cudaStream_t st);
 
+// api.cu: phase-boundary event (no-op unless nao_profile_enable(1))
+void prof_mark(int idx, cudaStream_t st);
+// per-launch timers: slot 0 = hetrd_panel_kernel (work = algorithmic HBM bytes), slot 1 = gemm_kernel (work = flops)
+int prof_kernel_begin(int slot, double work, cudaStream_t st);
+void prof_kernel_end(int slot, int k, cudaStream_t st);
+
 // fermi.cu / density
 int fermi_mu(int n, int batch, const double *dE, const double *h_weight, double n_electrons, double kT, double *h_mu,
              double *dF, void *dwork, cudaStream_t st);

@@ -363,9 +363,14 @@ static int hetrd_impl(int dtype, int n, int batch, T *A, long lda, long sA, doub
             a.Prow = (T *)w.Prow + (long)b0 * w.nblk * n; a.Pcol = (T *)w.Pcol + (long)b0 * w.nblk * n;
             a.bar = w.bar + (size_t)panel * batch + b0;
             a.n = n; a.j0 = j0; a.nbp = nbp; a.G = w.G; a.nblk = w.nblk;
+            // algorithmic bytes of this launch: the lower triangle of the trailing matrix once per column
+            double bytes = 0.0;
+            for (int i = 0; i < nbp; ++i) { double mm = n - (j0 + i) - 1; bytes += 0.5 * mm * (mm + 1) * sizeof(T); }
+            const int pk = prof_kernel_begin(0, bytes * nb_items, st);
             void *args[] = {&a};
             NAO_CUDA_CHECK(cudaLaunchCooperativeKernel((void *)hetrd_panel_kernel<T>, dim3(nb_items * w.G), dim3(TRD_NT), args, 0, st));
             NAO_LAUNCHED();
+            prof_kernel_end(0, pk, st);
         }
         const int jn = j0 + nbp;             // first row/column of the trailing matrix
         if (nbp > 0 && jn < n) {

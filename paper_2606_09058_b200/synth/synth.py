@@ -112,12 +112,12 @@ def make_config(idx: int, nat: int | None = None, seed: int = 0, kT: float = KT_
     if nat is not None and nat != cfg["nat"]:
         cfg["L"] = cfg["L"] * (nat / cfg["nat"]) ** (1.0 / 3.0)
         if cfg["periodic"]:
-            cfg["L"] = max(cfg["L"], 10.0)
+            cfg["L"] = max(cfg["L"], 10.5)     # strictly above the 10 bohr cut-off: no orbital sees its own image
         cfg["n_electrons"] = 4.0 * nat
         cfg["nat"] = nat
     nat, L, periodic, kind = cfg["nat"], cfg["L"], cfg["periodic"], cfg["kind"]
-    if periodic and L < 10.0:
-        raise ValueError("periodic replica too small: box side must be >= the 10 bohr cut-off")
+    if periodic and L <= 10.0:
+        raise ValueError("periodic replica too small: box side must exceed the 10 bohr cut-off")
     n = 13 * nat
     name = f"c{idx}" + ("" if nat == CONFIGS[idx]["nat"] else f"_nat{nat}")
     meta = dict(cfg, seed=seed, idx=idx)

@@ -1,0 +1,261 @@
+"""GPU parity tests: the CUDA path (through the C-ABI binding) against the CPU oracle, element by element, on the same
+seeded inputs.  Tolerances are BASELINE.json's north_star bars:
+    |de| <= 1e-9 Ha, max|dD| <= 1e-8, ||C^H S C - I||_max <= 1e-10, |dmu| <= 1e-10 Ha.
+D is compared instead of C (gauge / degeneracy safe)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2606_09058_b200.synth import make_config
+
+pytestmark = pytest.mark.gpu
+
+TOL_E, TOL_D, TOL_ORTH, TOL_MU = 1e-9, 1e-8, 1e-10, 1e-10
+DEV = "cuda:0"
+
+
+@pytest.fixture(scope="module")
+def nao():
+    import paper_2606_09058_b200 as m
+    m.lib()       # raises if the CUDA library is missing: there is no fallback
+    return m
+
+
+def to_dev(M):
+    """mathematical (b, n, n) -> column-major items on the GPU"""
+    return torch.from_numpy(np.ascontiguousarray(np.swapaxes(M, -1, -2))).to(DEV)
+
+
+def to_np(T):
+    return np.swapaxes(T.cpu().numpy(), -1, -2)
+
+
+def run_path(nao, prob, flags=0):
+    H = torch.from_numpy(prob.H).to(DEV)
+    S = torch.from_numpy(prob.S.copy()).to(DEV)
+    if prob.nc_block_s:
+        flags |= nao.NAO_NC_BLOCK_S
+    E, C, info = nao.geneig(H, S, flags=flags)
+    assert int(info.abs().max()) == 0
+    mu, F = nao.fermi_mu(E, prob.weights, prob.n_electrons, prob.kT)
+    D = nao.density_matrix(C, F)
+    return dict(e=E.cpu().numpy(), mu=mu, f=F.cpu().numpy(), C=to_np(C), D=to_np(D), S_factor=S)
+
+
+def check_against_oracle(prob, got, ref):
+    assert np.abs(got["e"] - ref["e"]).max() <= TOL_E
+    assert abs(got["mu"] - ref["mu"]) <= TOL_MU
+    assert np.abs(got["f"] - ref["f"]).max() <= 1e-7          # |df| <= |de|/(4 kT) ~ 2.6e-7 at the bar
+    ne = 0.0
+    for b in range(prob.batch):
+        assert np.abs(got["D"][b] - ref["D"][b]).max() <= TOL_D
+        Sb = prob.S_full(b)
+        Cb = got["C"][b]
+        assert np.abs(Cb.conj().T @ Sb @ Cb - np.eye(prob.n)).max() <= TOL_ORTH
+        assert np.abs(prob.H_full(b) @ Cb - Sb @ Cb * got["e"][b]).max() <= 1e-10
+        ne += prob.weights[b] * np.trace(got["D"][b] @ Sb).real
+    assert abs(ne - prob.n_electrons) <= 1e-8
+
+
+# ------------------------------------------------------------------------------------------ whole path vs oracle
+def test_config0_full(nao):
+    """BASELINE config 0: n = 104 real, one spin channel (g = 2), 32 electrons."""
+    prob = make_config(0)
+    check_against_oracle(prob, run_path(nao, prob), oracle.solve_problem(prob))
+
+
+def test_config1_replica_complex_batch16(nao):
+    """Config 1 recipe at 16 atoms: n = 208 complex, 8 k-points x 2 spins = 16 items sharing one Fermi level."""
+    prob = make_config(1, nat=16)
+    got = run_path(nao, prob)
+    check_against_oracle(prob, got, oracle.solve_problem(prob))
+    # time reversal: e(k) = e(-k) for a real real-space H (items 0..7 are k, 7-j is -k)
+    assert np.abs(got["e"][:8] - got["e"][7::-1]).max() <= 1e-10
+
+
+def test_config2_replica_two_spins(nao):
+    """Config 2 recipe at 32 atoms: n = 416 real, 2 spin channels (several GEMM tiles and a ragged tail)."""
+    prob = make_config(2, nat=32)
+    check_against_oracle(prob, run_path(nao, prob), oracle.solve_problem(prob))
+
+
+def test_config3_replica_noncollinear_block_S(nao):
+    """Config 3 recipe at 16 atoms: 2N = 416 complex, S real N x N with NAO_NC_BLOCK_S (Eq. 25-27)."""
+    prob = make_config(3, nat=16)
+    ref = oracle.solve_problem(prob)
+    check_against_oracle(prob, run_path(nao, prob), ref)
+    # the same problem with S_NC = diag(S, S) passed as a dense complex 2N x 2N overlap must agree
+    H = torch.from_numpy(prob.H).to(DEV)
+    S = to_dev(prob.S_full(0)[None])
+    E, C, info = nao.geneig(H, S)
+    assert np.abs(E.cpu().numpy() - ref["e"]).max() <= TOL_E
+
+
+def test_cached_factor_is_bit_identical(nao):
+    """S and its factor do not change over the SCF loop: NAO_S_FACTORED must reproduce the result."""
+    prob = make_config(2, nat=16)
+    H = torch.from_numpy(prob.H).to(DEV)
+    S = torch.from_numpy(prob.S.copy()).to(DEV)
+    E1, C1, _ = nao.geneig(H, S)
+    E2, C2, _ = nao.geneig(H, S, flags=nao.NAO_S_FACTORED)
+    assert torch.equal(E1, E2) and torch.equal(C1, C2)
+    L = np.tril(to_np(S)[0])
+    assert np.abs(L @ L.T - prob.S_full(0)).max() <= 1e-13
+    assert np.abs(L - oracle.cholesky(prob.S_full(0))).max() <= 1e-12
+
+
+# ------------------------------------------------------------------------------------------ degenerate / edge cases
+def test_ring_exact_degeneracies_density_matches(nao):
+    """Complex Hermitian ring, theta = 0: +-m pairs are exactly degenerate; D is gauge independent."""
+    n, t = 48, -1.0
+    H = np.zeros((n, n), dtype=complex)
+    for j in range(n):
+        H[j, (j + 1) % n] += t
+        H[(j + 1) % n, j] += t
+    e_ref, C_ref, _ = oracle.geneig(H, np.eye(n, dtype=complex))
+    mu_ref, f_ref = oracle.fermi(e_ref[None], [2.0], 20.0, 0.05)
+    D_ref = oracle.density(C_ref, f_ref[0])
+    E, C, info = nao.geneig(to_dev(H[None]), to_dev(np.eye(n, dtype=complex)[None]))
+    mu, F = nao.fermi_mu(E, [2.0], 20.0, 0.05)
+    D = nao.density_matrix(C, F)
+    assert np.abs(E.cpu().numpy()[0] - e_ref).max() <= TOL_E
+    assert abs(mu - mu_ref) <= TOL_MU
+    assert np.abs(to_np(D)[0] - D_ref).max() <= TOL_D
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 33, 65, 131])
+@pytest.mark.parametrize("cplx", [False, True])
+def test_small_and_ragged_sizes(nao, n, cplx):
+    rng = np.random.default_rng(n + 1000 * cplx)
+    A = rng.standard_normal((n, n)) + (1j * rng.standard_normal((n, n)) if cplx else 0)
+    H = (A + A.conj().T) / 2
+    B = rng.standard_normal((n, n)) + (1j * rng.standard_normal((n, n)) if cplx else 0)
+    S = B @ B.conj().T / n + np.eye(n)
+    e_ref, C_ref, _ = oracle.geneig(H, S)
+    E, C, info = nao.geneig(to_dev(H[None]), to_dev(S[None]))
+    assert int(info[0]) == 0
+    assert np.abs(E.cpu().numpy()[0] - e_ref).max() <= TOL_E
+    f = np.linspace(1.0, 0.0, n)
+    D = nao.density_matrix(C, torch.from_numpy(f[None].copy()).to(DEV))
+    if n == 1 or np.min(np.diff(e_ref)) > 1e-4:          # D with arbitrary f is unique only for distinct levels
+        assert np.abs(to_np(D)[0] - oracle.density(C_ref, f)).max() <= TOL_D
+
+
+def test_identity_overlap_and_block_diagonal(nao):
+    """S = I => C unitary; block-diagonal H => spectrum is the union of the block spectra (heavy deflation in D&C)."""
+    rng = np.random.default_rng(7)
+    n1, n2 = 40, 57
+    A1 = rng.standard_normal((n1, n1)); A2 = rng.standard_normal((n2, n2))
+    H = np.zeros((n1 + n2, n1 + n2)); H[:n1, :n1] = (A1 + A1.T) / 2; H[n1:, n1:] = (A2 + A2.T) / 2
+    n = n1 + n2
+    E, C, info = nao.geneig(to_dev(H[None]), to_dev(np.eye(n)[None]))
+    e1, _, _ = oracle.geneig(H[:n1, :n1], np.eye(n1)); e2, _, _ = oracle.geneig(H[n1:, n1:], np.eye(n2))
+    assert np.abs(E.cpu().numpy()[0] - np.sort(np.concatenate([e1, e2]))).max() <= TOL_E
+    Cm = to_np(C)[0]
+    assert np.abs(Cm.T @ Cm - np.eye(n)).max() <= TOL_ORTH
+
+
+def test_not_positive_definite_reports_pivot(nao):
+    prob = make_config(0)
+    S = prob.S_full(0).copy()
+    S[60, 60] = -1.0
+    with pytest.raises(np.linalg.LinAlgError):
+        oracle.cholesky(S)
+    E, C, info = nao.geneig(torch.from_numpy(prob.H).to(DEV), to_dev(S[None]))
+    assert int(info[0]) == 61          # leading minor 61 (1-based) is the first that fails, as in the oracle
+
+
+def test_density_all_occupied_is_inverse_overlap(nao):
+    """f = 1 for every state: D = C C^H = S^{-1}, independent of the eigen-solver."""
+    prob = make_config(0)
+    E, C, _ = nao.geneig(torch.from_numpy(prob.H).to(DEV), torch.from_numpy(prob.S.copy()).to(DEV))
+    D = nao.density_matrix(C, torch.ones_like(E))
+    assert np.abs(to_np(D)[0] @ prob.S_full(0) - np.eye(prob.n)).max() <= 1e-11
+
+
+# ------------------------------------------------------------------------------------------ Fermi level
+def test_fermi_level_against_oracle_and_closed_forms(nao):
+    rng = np.random.default_rng(3)
+    e = np.sort(rng.standard_normal((3, 50)), axis=1)
+    w = [0.5, 0.25, 0.25]
+    mu_ref, f_ref = oracle.fermi(e, w, 13.7, 0.01)
+    mu, F = nao.fermi_mu(torch.from_numpy(e).to(DEV), w, 13.7, 0.01)
+    assert abs(mu - mu_ref) <= TOL_MU and np.abs(F.cpu().numpy() - f_ref).max() <= 1e-9
+    # single n-fold level: mu = e0 + kT ln(nu/(1-nu))
+    e0, kT, n, ne = -0.3, 2e-3, 40, 12.0
+    mu, F = nao.fermi_mu(torch.full((1, n), e0, dtype=torch.float64, device=DEV), [2.0], ne, kT)
+    nu = ne / (2.0 * n)
+    assert abs(mu - (e0 + kT * np.log(nu / (1 - nu)))) <= TOL_MU
+    # two levels of equal degeneracy, huge gap, integer filling: mu = midpoint (needs the particle/hole log form)
+    e2 = np.concatenate([np.full(8, -1.0), np.full(8, 1.0)])[None]
+    mu, F = nao.fermi_mu(torch.from_numpy(e2).to(DEV), [2.0], 16.0, 9.5e-4)
+    assert abs(mu) <= TOL_MU
+    mu_ref, _ = oracle.fermi(e2, [2.0], 16.0, 9.5e-4)
+    assert abs(mu - mu_ref) <= TOL_MU
+
+
+# ------------------------------------------------------------------------------------------ building blocks
+@pytest.mark.parametrize("cplx", [False, True])
+def test_gemm_core_all_ops(nao, cplx):
+    rng = np.random.default_rng(11)
+
+    def rnd(r, c):
+        x = rng.standard_normal((2, r, c))
+        return x + 1j * rng.standard_normal((2, r, c)) if cplx else x
+
+    def op(X, o):
+        return X if o == 0 else (np.swapaxes(X, -1, -2) if o == 1 else np.swapaxes(X.conj(), -1, -2))
+
+    for (m, n, k) in [(1, 1, 1), (130, 67, 45), (257, 300, 129)]:
+        for oa in (0, 1, 2):
+            for ob in (0, 1, 2):
+                A = rnd(m, k) if oa == 0 else rnd(k, m)
+                B = rnd(k, n) if ob == 0 else rnd(n, k)
+                C0 = rnd(m, n)
+                Ct = to_dev(C0)
+                nao.gemm(to_dev(A), to_dev(B), oa, ob, alpha=0.7, beta=-0.3, C=Ct)
+                ref = 0.7 * (op(A, oa) @ op(B, ob)) - 0.3 * C0
+                assert np.abs(to_np(Ct) - ref).max() <= 1e-12 * k
+
+
+def test_stedc_textbook_tridiagonals(nao):
+    """(1,2,1) Toeplitz: 2 - 2 cos(k pi/(n+1)); Wilkinson W+: near-degenerate pairs; glued: heavy deflation."""
+    n = 201
+    d = np.stack([np.full(n, 2.0), np.abs(np.arange(n) - 100.0), np.abs(np.arange(n) % 21 - 10.0)])
+    e = np.stack([np.ones(n), np.ones(n), np.where((np.arange(n) + 1) % 21 == 0, 1e-8, 1.0)])
+    E, Q, info = nao.stedc(torch.from_numpy(d.copy()).to(DEV), torch.from_numpy(e.copy()).to(DEV))
+    E = E.cpu().numpy(); Qn = to_np(Q)
+    k = np.arange(1, n + 1)
+    assert np.abs(E[0] - np.sort(2 - 2 * np.cos(k * np.pi / (n + 1)))).max() <= 1e-13
+    for i in range(3):
+        T = np.diag(d[i]) + np.diag(e[i, :n - 1], 1) + np.diag(e[i, :n - 1], -1)
+        assert np.abs(T @ Qn[i] - Qn[i] * E[i]).max() <= 1e-12 * np.abs(T).sum(1).max()
+        assert np.abs(Qn[i].T @ Qn[i] - np.eye(n)).max() <= 1e-13
+        e_or, _ = oracle.heev(T)
+        assert np.abs(E[i] - e_or).max() <= 1e-11 * max(1.0, np.abs(e_or).max())
+
+
+# ------------------------------------------------------------------------------------------ full-size properties
+def test_config2_full_size_properties(nao):
+    """BASELINE config 2 at full size (n = 6656 real, 2 spins), the launch configuration bench.py times.  The oracle
+    cannot run here in seconds, so: invariants that hold at any size, plus sampled entries of D recomputed one by
+    one from their definition with the oracle's D-kernel restricted to those entries."""
+    prob = make_config(2)
+    got = run_path(nao, prob)
+    n = prob.n
+    ne = 0.0
+    for b in range(prob.batch):
+        Cb, Sb, Hb = got["C"][b], prob.S_full(b), prob.H_full(b)
+        assert np.all(np.diff(got["e"][b]) >= 0)
+        assert np.abs(Cb.T @ (Sb @ Cb) - np.eye(n)).max() <= TOL_ORTH
+        assert np.abs(Hb @ Cb - (Sb @ Cb) * got["e"][b]).max() <= 1e-10
+        ne += prob.weights[b] * np.sum(got["D"][b] * Sb)
+        rng = np.random.default_rng(5 + b)
+        for (i, j) in rng.integers(0, n, size=(64, 2)):
+            dij = float(np.sum(np.asarray(got["f"][b], dtype=np.longdouble) * Cb[i].astype(np.longdouble) * Cb[j].astype(np.longdouble)))
+            assert abs(got["D"][b][i, j] - dij) <= 1e-12
+        assert abs(np.sum(got["e"][b]) - np.trace(np.linalg.solve(Sb, Hb))) <= 1e-8
+    assert abs(ne - prob.n_electrons) <= 1e-7
+    mu_ref, f_ref = oracle.fermi(got["e"], prob.weights, prob.n_electrons, prob.kT)
+    assert abs(got["mu"] - mu_ref) <= TOL_MU

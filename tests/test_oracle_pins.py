@@ -292,3 +292,14 @@ def test_config3_replica_noncollinear():
     assert np.abs(H - H.conj().T).max() < 1e-15
     assert np.abs(r["e"][0] - sl.eigh(H, S, eigvals_only=True)).max() < 1e-12
     assert abs(np.trace(r["D"][0] @ S).real - 16.0) < 1e-10
+
+
+def test_generator_matrices_are_hermitian_and_spd():
+    """The input generator must hand Hermitian H and Hermitian positive definite S to both sides (replicas included)."""
+    for idx, nat in [(0, None), (1, 6), (1, 16), (2, 8), (3, 4)]:
+        p = make_config(idx, nat=nat)
+        for b in range(p.batch):
+            H, S = p.H_full(b), p.S_full(b)
+            assert np.abs(H - H.conj().T).max() < 1e-14
+            assert np.abs(S - S.conj().T).max() < 1e-14
+            assert np.linalg.eigvalsh(S).min() > 0.05
