@@ -1,0 +1,121 @@
+// ormtr.cu -- blocked back-transformation Z <- Q Z of the one-stage tridiagonalisation.
+#include "nao_internal.cuh"
+#include "scalar.cuh"
+
+namespace nao {
+
+
+// ----------------------------------------------------------------------------------------------------------------
+// Back-transformation: Z <- Q Z, Q = H(0) H(1) ... H(n-2), H(j) = I - tau_j v_j v_j^H, v_j = A[j+1:, j] (unit first
+// element stored explicitly by hetrd).  Blocks of KB reflectors, last block first:
+//   Vb (explicit, zeros above the unit diagonal), G = Vb^H Vb, T by the xLARFT recurrence, then three GEMMs
+//   X = Vb^H Z ; X <- T X ; Z -= Vb X.
+// ----------------------------------------------------------------------------------------------------------------
+static const int ORM_KB = 64;
+
+template <class T>
+__global__ void build_v_kernel(int n, int jb, int kb, const T *A, long lda, long sA, T *V, long ldv, long sV) {
+    // V (m x kb), m = n - jb - 1, row r <-> global row jb+1+r; column k <-> reflector jb+k whose unit sits at r == k
+    A += (long)blockIdx.z * sA; V += (long)blockIdx.z * sV;
+    const int m = n - jb - 1;
+    int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= m) return;
+    for (int k = blockIdx.y; k < kb; k += gridDim.y) {
+        T v;
+        if (r < k) v = Ops<T>::zero();
+        else if (r == k) v = Ops<T>::one();
+        else v = A[(jb + 1 + r) + (long)(jb + k) * lda];
+        V[r + (long)k * ldv] = v;
+    }
+}
+
+// T (kb x kb upper) from G = V^H V and tau: T(i,i) = tau_i ; T(0:i, i) = -tau_i T(0:i,0:i) G(0:i, i)
+template <class T>
+__global__ void __launch_bounds__(256) larft_kernel(int kb, const T *G, long sG, const T *tau, long sTau, T *Tm, long sT) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T *sT_ = (T *)smem_raw;             // kb x kb, column-major
+    __shared__ T s_g[ORM_KB];
+    G += (long)blockIdx.x * sG; tau += (long)blockIdx.x * sTau; Tm += (long)blockIdx.x * sT;
+    const int tid = threadIdx.x;
+    for (int e = tid; e < kb * kb; e += blockDim.x) sT_[e] = Ops<T>::zero();
+    __syncthreads();
+    for (int i = 0; i < kb; ++i) {
+        const T ti = tau[i];
+        if (tid < i) s_g[tid] = G[tid + (long)i * kb];
+        __syncthreads();
+        if (tid < i) {
+            // row tid of T(0:i,0:i) times g  (T upper: columns c >= tid)
+            T acc = Ops<T>::zero();
+            for (int c = tid; c < i; ++c) acc = Ops<T>::fma(sT_[tid + c * kb], s_g[c], acc);
+            T v = Ops<T>::mul(ti, acc);
+            sT_[tid + i * kb] = Ops<T>::sub(Ops<T>::zero(), v);
+        }
+        if (tid == 0) sT_[i + i * kb] = ti;
+        __syncthreads();
+    }
+    for (int e = tid; e < kb * kb; e += blockDim.x) Tm[e] = sT_[e];
+}
+
+struct OrmWork { void *V, *G, *T, *X, *X2; size_t bytes; };
+static OrmWork orm_plan(int dtype, int n, int ncols, int batch, void *work) {
+    OrmWork w; const size_t es = esize(dtype);
+    Arena ar(work, (size_t)-1);
+    w.V = ar.take((size_t)batch * n * ORM_KB * es);
+    w.G = ar.take((size_t)batch * ORM_KB * ORM_KB * es);
+    w.T = ar.take((size_t)batch * ORM_KB * ORM_KB * es);
+    w.X = ar.take((size_t)batch * ORM_KB * ncols * es);
+    w.X2 = ar.take((size_t)batch * ORM_KB * ncols * es);
+    w.bytes = ar.off;
+    return w;
+}
+size_t ormtr_workspace(int dtype, int n, int batch) { return orm_plan(dtype, n, n, batch, nullptr).bytes; }
+
+template <class T>
+static int ormtr_impl(int dtype, int n, int ncols, int batch, const T *A, long lda, long sA, const T *tau, T *Z, long ldz,
+                      long sZ, void *work, cudaStream_t st) {
+    if (n < 2) return NAO_OK;
+    OrmWork w = orm_plan(dtype, n, ncols, batch, work);
+    const int nref = n - 1;
+    static bool attr = false;
+    if (!attr) {
+        NAO_CUDA_CHECK(cudaFuncSetAttribute(larft_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                            (int)(ORM_KB * ORM_KB * sizeof(T))));
+        attr = true;
+    }
+    const int nblocks = ceil_div(nref, ORM_KB);
+    for (int blk = nblocks - 1; blk >= 0; --blk) {
+        const int jb = blk * ORM_KB, kb = min(ORM_KB, nref - jb), m = n - jb - 1;
+        const long ldv = m, sV = (long)n * ORM_KB;
+        build_v_kernel<T><<<dim3(ceil_div(m, 256), kb, batch), 256, 0, st>>>(n, jb, kb, A, lda, sA, (T *)w.V, ldv, sV);
+        NAO_LAUNCHED();
+        // G = V^H V
+        GemmDesc g = gemm_desc(OP_C, OP_N, kb, kb, m, 1.0, w.V, ldv, w.V, ldv, 0.0, w.G, kb);
+        g.sA = sV; g.sB = sV; g.sC = ORM_KB * ORM_KB;
+        if (int rc = gemm_launch(dtype, g, batch, st)) return rc;
+        larft_kernel<T><<<batch, 256, kb * kb * sizeof(T), st>>>(kb, (const T *)w.G, ORM_KB * ORM_KB, tau + jb, n, (T *)w.T, ORM_KB * ORM_KB);
+        NAO_LAUNCHED();
+        // X = V^H Z[jb+1:, :]
+        GemmDesc x = gemm_desc(OP_C, OP_N, kb, ncols, m, 1.0, w.V, ldv, Z + jb + 1, ldz, 0.0, w.X, kb);
+        x.sA = sV; x.sB = sZ; x.sC = (long)ORM_KB * ncols;
+        if (int rc = gemm_launch(dtype, x, batch, st)) return rc;
+        // X2 = T X
+        GemmDesc t = gemm_desc(OP_N, OP_N, kb, ncols, kb, 1.0, w.T, kb, w.X, kb, 0.0, w.X2, kb);
+        t.sA = ORM_KB * ORM_KB; t.sB = (long)ORM_KB * ncols; t.sC = (long)ORM_KB * ncols; t.maskA = MASK_UPPER;
+        if (int rc = gemm_launch(dtype, t, batch, st)) return rc;
+        // Z[jb+1:, :] -= V X2
+        GemmDesc u = gemm_desc(OP_N, OP_N, m, ncols, kb, -1.0, w.V, ldv, w.X2, kb, 1.0, Z + jb + 1, ldz);
+        u.sA = sV; u.sB = (long)ORM_KB * ncols; u.sC = sZ;
+        if (int rc = gemm_launch(dtype, u, batch, st)) return rc;
+    }
+    NAO_CUDA_CHECK(cudaGetLastError());
+    return NAO_OK;
+}
+
+int ormtr(int dtype, int n, int ncols, int batch, const void *A, long lda, long sA, const void *tau, void *Z, long ldz,
+          long sZ, void *work, cudaStream_t st) {
+    return dtype == NAO_COMPLEX
+               ? ormtr_impl<cplx>(dtype, n, ncols, batch, (const cplx *)A, lda, sA, (const cplx *)tau, (cplx *)Z, ldz, sZ, work, st)
+               : ormtr_impl<double>(dtype, n, ncols, batch, (const double *)A, lda, sA, (const double *)tau, (double *)Z, ldz, sZ, work, st);
+}
+
+}  // namespace nao

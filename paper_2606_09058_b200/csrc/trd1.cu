@@ -1,6 +1,5 @@
 // trd1.cu -- one-stage Householder tridiagonalisation (SURVEY.md 8a row a3/a4 role, 8d ambiguity M1: this is the
-// HBM-bound "BLAS2 half" the paper describes for the one-stage reduction) and the blocked
-// back-transformation Z <- Q Z (row a6).
+// HBM-bound "BLAS2 half" the paper describes for the one-stage reduction).
 //
 // Algorithm: LAPACK xHETRD/xLATRD, lower storage, panels of NB columns.  Inside a panel the trailing matrix is NOT
 // updated; column j is brought up to date with the panel's (V, W), a reflector is generated, and
@@ -11,12 +10,19 @@
 // at a software grid barrier only TWICE per column:
 //   phase A: finalise w of the previous column for the CTA's own rows, update column j, partial norm   | barrier
 //   phase B: reflector scalars (every CTA, redundantly), v written to A, partial W^H v / V^H v,
-//            HEMV over 64x64 tiles of the lower triangle (each element read from HBM exactly once per column,
-//            both its row and its column contribution formed from registers), partial v^H A v          | barrier
-// Every cross-CTA reduction goes through per-CTA partial buffers summed in a fixed order: results are bit-reproducible
-// (no floating-point atomics).  HEMV tile loads are 512 B (real) / 1 KB (complex) contiguous per column and the
-// next tile is prefetched into registers while the current one is reduced, so the kernel runs at HBM speed once the
-// trailing matrix exceeds L2.
+//            HEMV of the lower triangle, partial v^H A v                                               | barrier
+// The CTA's own rows of the panel's V and W live in shared memory for the whole panel.
+//
+// HEMV (the HBM-bound part): the lower triangle is cut into units of 64 rows x SW columns (SW = 64 real, 32 complex),
+// enumerated strip by strip (column-major), and every WARP owns a contiguous run of units -- the loop has no
+// __syncthreads at all.  Within a unit a lane owns 4 rows (q, q+16, q+32, q+48: each half-warp reads 128/256
+// contiguous bytes per column) and half of the strip's columns; every element is loaded once (ld.global.cg, next
+// batch in flight while the current one is used) and used for both its row and its column contribution:
+//   row sums   : complete per unit in registers, halves combined with one shuffle, written to Prow[strip][row]
+//   column sums: accumulated in registers over the whole run of units in the strip, reduced across lanes ONCE per
+//                run by a 16-lane transpose-reduction and written to Pcol[first row block of the run][column]
+// Every cross-CTA reduction goes through such partial buffers summed in a fixed order: results are bit-reproducible
+// (no floating-point atomics).
 #include "nao_internal.cuh"
 #include "scalar.cuh"
 #include <cooperative_groups.h>
@@ -24,8 +30,16 @@
 namespace nao {
 
 static const int TRD_NB = 32;        // panel width
-static const int TRD_NT = 512;       // threads per CTA
-static const int TRD_TB = 64;        // HEMV tile edge
+static const int TRD_NT = 256;       // threads per CTA
+static const int TRD_NW = TRD_NT / 32;
+static const int TRD_TB = 64;        // rows per HEMV unit / block edge
+static const int TRD_CH = 96;        // rows of V/W cached in shared memory per CTA
+static const int TRD_CHP = TRD_CH + 1;
+static const int TRD_PASS = 128;     // rows finalised per pass in phase A
+
+template <class T> struct Hv;
+template <> struct Hv<double> { static const int SW = 64, CPT = 32, HS = 1, CB = 4; };
+template <> struct Hv<cplx> { static const int SW = 32, CPT = 16, HS = 2, CB = 2; };
 
 template <class T> struct TrdArgs {
     T *A; long lda, sA;
@@ -35,35 +49,187 @@ template <class T> struct TrdArgs {
     double *pn;                      // per item: G
     T *pt;                           // per item: G x 2NB
     double *pvav;                    // per item: G
-    T *Prow, *Pcol;                  // per item: nblk x n each
+    T *Prow, *Pcol;                  // per item: (HS*nblk) x n and nblk x n
     unsigned *bar;                   // per item: one counter for this launch
     int n, j0, nbp, G, nblk;
 };
 
-template <class T> __device__ __forceinline__ T block_sum_T(T v, T *red /* TRD_NT/32 */) {
-    v = warp_sum(v);
-    __syncthreads();
-    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
-    __syncthreads();
-    T s = Ops<T>::zero();
-    for (int w = 0; w < TRD_NT / 32; ++w) s = Ops<T>::add(s, red[w]);
-    __syncthreads();
-    return s;
-}
-__device__ __forceinline__ double block_sum_d(double v, double *red) {
+__device__ __forceinline__ double block_sum_d(double v, double *red /* TRD_NW */) {
     v = warp_sum(v);
     __syncthreads();
     if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
     __syncthreads();
     double s = 0.0;
-    for (int w = 0; w < TRD_NT / 32; ++w) s += red[w];
+    for (int w = 0; w < TRD_NW; ++w) s += red[w];
     __syncthreads();
     return s;
+}
+
+// units of the lower triangle of an nbk x nbk block matrix, strip-major: block column J', half h, row block I >= J'
+__device__ __forceinline__ int tri_off(int Jp, int nbk) { return Jp * nbk - Jp * (Jp - 1) / 2; }
+__device__ __forceinline__ int tri_decode(int t, int nbk) {      // largest J' with tri_off(J') <= t
+    const double b = 2.0 * nbk + 1.0;
+    int Jp = (int)((b - sqrt(fmax(b * b - 8.0 * (double)t, 0.0))) * 0.5);
+    Jp = max(0, min(Jp, nbk - 1));
+    while (Jp + 1 < nbk && tri_off(Jp + 1, nbk) <= t) ++Jp;
+    while (Jp > 0 && tri_off(Jp, nbk) > t) --Jp;
+    return Jp;
+}
+template <int HS> __device__ __forceinline__ void unit_decode(int u, int nbk, int &Jp, int &h, int &Irel) {
+    Jp = tri_decode(u / HS, nbk);
+    const int len = nbk - Jp, w = u - HS * tri_off(Jp, nbk);
+    h = w / len; Irel = Jp + w % len;
+}
+__device__ __forceinline__ int units_per_warp(int U, int G) { return (U + G * TRD_NW - 1) / (G * TRD_NW); }
+
+__device__ __forceinline__ double shfl_xor_T(double v, int o) { return __shfl_xor_sync(0xffffffffu, v, o); }
+__device__ __forceinline__ cplx shfl_xor_T(cplx v, int o) {
+    return make_double2(__shfl_xor_sync(0xffffffffu, v.x, o), __shfl_xor_sync(0xffffffffu, v.y, o));
+}
+
+// Transpose-reduction over the 16 lanes of a half-warp: every lane enters with NV partial sums cs[0..NV) and leaves
+// with the complete sums of indices q*(NV/16) + i, i < NV/16, in cs[0..NV/16)  (q = lane & 15).  Fixed tree order.
+template <class T, int N, int NV, int XO>
+__device__ __forceinline__ void treduce16(T (&cs)[N], int lane) {
+    if constexpr (XO >= 1) {
+        constexpr int half = NV / 2;
+        const bool up = (lane & XO) != 0;
+#pragma unroll
+        for (int i = 0; i < half; ++i) {
+            const T send = up ? cs[i] : cs[i + half];
+            const T keep = up ? cs[i + half] : cs[i];
+            cs[i] = Ops<T>::add(keep, shfl_xor_T(send, XO));
+        }
+        treduce16<T, N, half, XO / 2>(cs, lane);
+    }
+}
+
+// HEMV y = A22 v over this warp's run of units (see the header).  Returns the lane's share of v^H A22 v.
+template <class T>
+__device__ __forceinline__ double hemv_warp(const T *__restrict__ A, long lda, int n, int j, int nblk, int G, int g,
+                                            const T *acol, T scale, T *sx, T *__restrict__ Prow, T *__restrict__ Pcol) {
+    typedef Ops<T> O;
+    typedef Hv<T> H;
+    constexpr int SW = H::SW, CPT = H::CPT, HS = H::HS, CB = H::CB, NBATCH = CPT / CB, CPL = CPT / 16;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, q = lane & 15, hh = lane >> 4;
+    const int bmin = (j + 1) / TRD_TB, nbk = nblk - bmin;
+    const int U = HS * (nbk * (nbk + 1) / 2);
+    const int per = units_per_warp(U, G);
+    const int gw = g * TRD_NW + warp;
+    const int u0 = min(U, gw * per), u1 = min(U, u0 + per);
+    if (u0 >= u1) return 0.0;
+
+    auto vval = [&](int x) -> T {
+        if (x < j + 1 || x >= n) return O::zero();
+        if (x == j + 1) return O::one();
+        return O::mul(ldcg(acol + x), scale);
+    };
+    auto load = [&](T (&buf)[CB][4], int Jp_, int h_, int Irel_, int b) {
+        const int rbase = (bmin + Irel_) * TRD_TB + q;
+        const int cbase = (bmin + Jp_) * TRD_TB + h_ * SW + hh * CPT + b * CB;
+        const bool diag = (Irel_ == Jp_);
+#pragma unroll
+        for (int cc = 0; cc < CB; ++cc) {
+            const int col = cbase + cc;
+            const T *pc = A + (long)col * lda + rbase;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const int r = rbase + 16 * k;
+                const bool ok = r < n && col < n && (!diag || r >= col);
+                T v = O::zero();
+                if (ok) v = ldcg(pc + 16 * k);
+                buf[cc][k] = v;
+            }
+        }
+    };
+
+    int Jp, h, Irel;
+    unit_decode<HS>(u0, nbk, Jp, h, Irel);
+    double vav = 0.0;
+    T cs[CPT];
+    T cur[CB][4], nxt[CB][4];
+    int runI = Irel;
+    auto strip_begin = [&](int Jp_, int h_) {
+        __syncwarp();
+        for (int c = lane; c < SW; c += 32) sx[c] = vval((bmin + Jp_) * TRD_TB + h_ * SW + c);
+        __syncwarp();
+#pragma unroll
+        for (int c = 0; c < CPT; ++c) cs[c] = O::zero();
+    };
+    strip_begin(Jp, h);
+    load(cur, Jp, h, Irel, 0);
+
+    for (int u = u0; u < u1; ++u) {
+        int Jn = Jp, hn = h, In = Irel + 1;
+        if (In >= nbk) {
+            hn = h + 1;
+            if (hn >= HS) { hn = 0; Jn = Jp + 1; }
+            In = Jn;
+        }
+        const bool more = (u + 1 < u1);
+        const bool diag = (Irel == Jp);
+        const int rbase = (bmin + Irel) * TRD_TB + q;
+        const int cb0 = (bmin + Jp) * TRD_TB + h * SW + hh * CPT;
+        T xr[4], rs[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) { xr[k] = vval(rbase + 16 * k); rs[k] = O::zero(); }
+#pragma unroll
+        for (int b = 0; b < NBATCH; ++b) {
+            if (b + 1 < NBATCH) load(nxt, Jp, h, Irel, b + 1);
+            else if (more) load(nxt, Jn, hn, In, 0);
+#pragma unroll
+            for (int cc = 0; cc < CB; ++cc) {
+                const T xc = sx[hh * CPT + b * CB + cc];
+                const int col = cb0 + b * CB + cc;
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    T a = cur[cc][k], ac = a;
+                    if (diag) {
+                        const int r = rbase + 16 * k;
+                        if (r == col) a = O::from_real(O::real(a));
+                        if (r <= col) ac = O::zero();
+                    }
+                    rs[k] = O::fma(a, xc, rs[k]);
+                    cs[b * CB + cc] = O::add(cs[b * CB + cc], O::conj_mul(ac, xr[k]));
+                }
+            }
+#pragma unroll
+            for (int cc = 0; cc < CB; ++cc)
+#pragma unroll
+                for (int k = 0; k < 4; ++k) cur[cc][k] = nxt[cc][k];
+        }
+        // row sums of this unit: combine the two column halves, lanes 0..15 write 4 x 16 consecutive rows
+#pragma unroll
+        for (int k = 0; k < 4; ++k) rs[k] = O::add(rs[k], shfl_xor_T(rs[k], 16));
+        if (hh == 0) {
+            T *pr = Prow + (long)(HS * (bmin + Jp) + h) * n;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const int r = rbase + 16 * k;
+                if (r < n) { pr[r] = rs[k]; vav += O::real(O::conj_mul(xr[k], rs[k])); }
+            }
+        }
+        if (!more || Jn != Jp || hn != h) {
+            // end of this warp's run in the strip: one cross-lane reduction of the column sums
+            treduce16<T, CPT, CPT, 8>(cs, lane);
+            T *pcl = Pcol + (long)(bmin + runI) * n;
+#pragma unroll
+            for (int c = 0; c < CPL; ++c) {
+                const int col = cb0 + q * CPL + c;
+                if (col < n) { pcl[col] = cs[c]; vav += O::real(O::conj_mul(sx[hh * CPT + q * CPL + c], cs[c])); }
+            }
+            if (more) { strip_begin(Jn, hn); runI = In; }
+        }
+        Jp = Jn; h = hn; Irel = In;
+    }
+    return vav;
 }
 
 template <class T>
 __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
     typedef Ops<T> O;
+    typedef Hv<T> H;
+    constexpr int HS = H::HS, SW = H::SW;
     const int G = p.G;
     const int item = blockIdx.x / G, g = blockIdx.x % G;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -77,69 +243,108 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
     double *pn = p.pn + (long)item * G;
     T *pt = p.pt + (long)item * G * 2 * TRD_NB;
     double *pvav = p.pvav + (long)item * G;
-    T *Prow = p.Prow + (long)item * nblk * n, *Pcol = p.Pcol + (long)item * nblk * n;
+    T *Prow = p.Prow + (long)item * HS * nblk * n, *Pcol = p.Pcol + (long)item * nblk * n;
     unsigned *bar = p.bar + item;
     unsigned bar_ord = 0;
 
     const int m = n - j0;
     const int chunk = (m + G - 1) / G;
     const int r0 = j0 + g * chunk, r1 = min(n, r0 + chunk);     // rows owned by this CTA
+    const bool cached = chunk <= TRD_CH;
 
-    __shared__ T s_t[2 * TRD_NB];          // t1 = W^H v at [0,NB), t2 = V^H v at [NB,2NB)
+    extern __shared__ __align__(16) unsigned char trd_smem[];
+    T *sV = (T *)trd_smem;                       // [NB][CHP]  own rows of V (reflectors of this panel)
+    T *sW = sV + TRD_NB * TRD_CHP;               // [NB][CHP]  own rows of W
+    T *s_part = sW + TRD_NB * TRD_CHP;           // [NW][PASS]
+    T *sx = s_part + TRD_NW * TRD_PASS;          // [NW][SW]
+    __shared__ T s_t[2 * TRD_NB];                // t1 = W^H v at [0,NB), t2 = V^H v at [NB,2NB)
     __shared__ T s_wrow[TRD_NB], s_vrow[TRD_NB];
+    __shared__ T s_red4[4][2 * TRD_NB];
     __shared__ T s_tau, s_scale;
-    __shared__ double s_alpha, s_dred[TRD_NT / 32];
-    __shared__ T s_red[TRD_NT / 32];
-    __shared__ T xs_row[TRD_TB], xs_col[TRD_TB];
-    __shared__ T red_row[8][TRD_TB];
-    __shared__ T red_col[TRD_NT / 32][8];
-    __shared__ T s_wpart[TRD_NT / 32][2 * TRD_NB];
+    __shared__ double s_alpha, s_vav, s_dred[TRD_NW];
+
+    auto getV = [&](int r, int k) -> T { return cached ? sV[k * TRD_CHP + (r - r0)] : A[r + (long)(j0 + k) * lda]; };
+    auto getW = [&](int r, int k) -> T { return cached ? sW[k * TRD_CHP + (r - r0)] : Wp[r + (long)k * n]; };
 
     for (int i = 0; i <= p.nbp; ++i) {
         const int j = j0 + i;
+        const int ra = max(r0, j);                 // first own row still in play
         // =============================== phase A ===============================
         if (i > 0) {
-            // reduce the partials of phase B(i-1): t1, t2 (k < i-1) and v^H A v
             const int nk = i - 1;
-            if (tid < 2 * TRD_NB) {
+            // (1) reduce the partials of phase B(i-1): t1, t2 (k < i-1) and v^H A v, fixed order
+            {
+                const int idx = tid & 63, part = tid >> 6;
+                const int k = idx < TRD_NB ? idx : idx - TRD_NB;
                 T s = O::zero();
-                int k = tid < TRD_NB ? tid : tid - TRD_NB;
                 if (k < nk)
-                    for (int q = 0; q < G; ++q) s = O::add(s, ldcg(pt + (long)q * 2 * TRD_NB + tid));
-                s_t[tid] = s;
+                    for (int qq = part; qq < G; qq += 4) s = O::add(s, ldcg(pt + (long)qq * 2 * TRD_NB + idx));
+                s_red4[part][idx] = s;
+                if (warp == 0) {
+                    double sv = 0.0;
+                    for (int qq = lane; qq < G; qq += 32) sv += ldcg(pvav + qq);
+                    sv = warp_sum(sv);
+                    if (lane == 0) s_vav = sv;
+                }
+                __syncthreads();
+                if (tid < 2 * TRD_NB)
+                    s_t[tid] = O::add(O::add(s_red4[0][tid], s_red4[1][tid]), O::add(s_red4[2][tid], s_red4[3][tid]));
+                __syncthreads();
+                if (tid == 0) {
+                    double s = s_vav;
+                    for (int k2 = 0; k2 < nk; ++k2) s -= 2.0 * O::real(O::conj_mul(s_t[k2], s_t[TRD_NB + k2]));
+                    s_alpha = -0.5 * O::abs2(s_tau) * s;
+                }
+                __syncthreads();
             }
-            if (warp == 4) {
-                double s = 0.0;
-                for (int q = lane; q < G; q += 32) s += ldcg(pvav + q);
-                s = warp_sum(s);
-                if (lane == 0) s_dred[0] = s;
+            // (2) w_{i-1} for the own rows r >= j and (redundantly, every CTA) for row j
+            const int nown = max(0, r1 - ra);
+            const bool extra = !(j >= r0 && j < r1);
+            const int nloc = nown + (extra ? 1 : 0);
+            const int bminp = j / TRD_TB, nbkp = nblk - bminp;           // geometry of the HEMV of column j-1
+            const int perp = units_per_warp(HS * (nbkp * (nbkp + 1) / 2), G);
+            for (int base = 0; base < nloc; base += TRD_PASS) {
+                const int np = min(TRD_PASS, nloc - base);
+                for (int lg = 0; lg < np; lg += 32) {
+                    if (lg + lane < np) {
+                        const int l = base + lg + lane;
+                        const int r = l < nown ? ra + l : j;
+                        const int Send = HS * (r / TRD_TB) + HS - 1;
+                        T s = O::zero();
+                        for (int S = HS * bminp + warp; S <= Send; S += TRD_NW) s = O::add(s, ldcg(Prow + (long)S * n + r));
+                        s_part[warp * TRD_PASS + lg + lane] = s;
+                    }
+                }
+                __syncthreads();
+                for (int lp = tid; lp < np; lp += TRD_NT) {
+                    const int l = base + lp;
+                    const bool own = l < nown;
+                    const int r = own ? ra + l : j;
+                    T y = O::zero();
+#pragma unroll
+                    for (int w = 0; w < TRD_NW; ++w) y = O::add(y, s_part[w * TRD_PASS + lp]);
+                    // column partials: one per run of units in the strip of column r
+                    const int Jp = r / TRD_TB - bminp, h = (r % TRD_TB) / SW, len = nbkp - Jp;
+                    const int ua = HS * tri_off(Jp, nbkp) + h * len, ub = ua + len;
+                    y = O::add(y, ldcg(Pcol + (long)(bminp + Jp) * n + r));
+                    for (int kk = ua / perp + 1; kk * perp < ub; ++kk)
+                        y = O::add(y, ldcg(Pcol + (long)(bminp + Jp + kk * perp - ua) * n + r));
+                    T acc = y;
+                    for (int k = 0; k < nk; ++k) {
+                        const T v = own ? getV(r, k) : ldcg(A + r + (long)(j0 + k) * lda);
+                        const T w = own ? getW(r, k) : ldcg(Wp + r + (long)k * n);
+                        acc = O::sub(acc, O::add(O::mul(v, s_t[k]), O::mul(w, s_t[TRD_NB + k])));
+                    }
+                    const T vr = (r == j) ? O::one() : getV(r, i - 1);
+                    const T wv = O::add(O::mul(s_tau, acc), O::scale(vr, s_alpha));
+                    if (own) {
+                        Wp[r + (long)(i - 1) * n] = wv;
+                        if (cached) sW[(i - 1) * TRD_CHP + (r - r0)] = wv;
+                    }
+                    if (r == j) s_wrow[i - 1] = wv;
+                }
+                __syncthreads();
             }
-            __syncthreads();
-            if (tid == 0) {
-                double s = s_dred[0];
-                for (int k = 0; k < nk; ++k) s -= 2.0 * O::real(O::conj_mul(s_t[k], s_t[TRD_NB + k]));
-                s_alpha = -0.5 * O::abs2(s_tau) * s;
-            }
-            __syncthreads();
-        }
-        // w_{i-1}(r) for a row r >= j, from the tile partials of phase B(i-1)
-        auto wfinal = [&](int r, bool own) -> T {
-            const int jm1 = j - 1, nk = i - 1;
-            const int bmin = (jm1 + 1) / TRD_TB, br = r / TRD_TB;
-            T acc = O::zero();
-            for (int J = bmin; J <= br; ++J) acc = O::add(acc, ldcg(Prow + (long)J * n + r));
-            for (int I = br; I < nblk; ++I) acc = O::add(acc, ldcg(Pcol + (long)I * n + r));
-            for (int k = 0; k < nk; ++k) {
-                T v = own ? A[r + (long)(j0 + k) * lda] : ldcg(A + r + (long)(j0 + k) * lda);
-                T w = own ? Wp[r + (long)k * n] : ldcg(Wp + r + (long)k * n);
-                acc = O::sub(acc, O::add(O::mul(v, s_t[k]), O::mul(w, s_t[TRD_NB + k])));
-            }
-            T vr = (r == j) ? O::one() : (own ? A[r + (long)jm1 * lda] : ldcg(A + r + (long)jm1 * lda));
-            return O::add(O::mul(s_tau, acc), O::scale(vr, s_alpha));
-        };
-        if (i > 0) {
-            if (tid == 0) s_wrow[i - 1] = wfinal(j, false);
-            for (int r = max(r0, j) + tid; r < r1; r += TRD_NT) Wp[r + (long)(i - 1) * n] = wfinal(r, true);
         }
         const bool do_col = (i < p.nbp) || (j == n - 1);
         if (do_col) {
@@ -151,13 +356,11 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
         __syncthreads();
         if (do_col) {
             double nrm = 0.0;
-            for (int r = max(r0, j) + tid; r < r1; r += TRD_NT) {
+            for (int r = ra + tid; r < r1; r += TRD_NT) {
                 T a = A[r + (long)j * lda];
                 if (r == j) a = O::from_real(O::real(a));
-                for (int k = 0; k < i; ++k) {
-                    T v = A[r + (long)(j0 + k) * lda], w = Wp[r + (long)k * n];
-                    a = O::sub(a, O::add(O::mul_conj(v, s_wrow[k]), O::mul_conj(w, s_vrow[k])));
-                }
+                for (int k = 0; k < i; ++k)
+                    a = O::sub(a, O::add(O::mul_conj(getV(r, k), s_wrow[k]), O::mul_conj(getW(r, k), s_vrow[k])));
                 if (r == j) dd[j] = O::real(a);
                 else { acol[r] = a; if (r >= j + 2) nrm += O::abs2(a); }
             }
@@ -170,7 +373,7 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
         // =============================== phase B ===============================
         if (warp == 0) {
             double s = 0.0;
-            for (int q = lane; q < G; q += 32) s += ldcg(pn + q);
+            for (int qq = lane; qq < G; qq += 32) s += ldcg(pn + qq);
             s = warp_sum(s);
             if (lane == 0) {
                 T alpha0 = ldcg(acol + j + 1);
@@ -200,104 +403,31 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
             if (x == j + 1) return O::one();
             return O::mul(ldcg(acol + x), scale);
         };
-        // v into column j of A (own rows), and partial t1 = W^H v, t2 = V^H v over own rows
-        {
-            const int rb = max(r0, j + 1);
-            for (int k = tid; k < 2 * TRD_NB * (TRD_NT / 32); k += TRD_NT) (&s_wpart[0][0])[k] = O::zero();
-            __syncthreads();
-            for (int base = rb + warp * 32; base < r1; base += TRD_NT) {
-                int r = base + lane;
-                T v = O::zero();
-                if (r < r1) { v = vval(r); A[r + (long)j * lda] = v; }
-                for (int k = 0; k < i; ++k) {
-                    T w = r < r1 ? Wp[r + (long)k * n] : O::zero();
-                    T a = r < r1 ? A[r + (long)(j0 + k) * lda] : O::zero();
-                    T p1 = warp_sum(O::conj_mul(w, v)), p2 = warp_sum(O::conj_mul(a, v));
-                    if (lane == 0) {
-                        s_wpart[warp][k] = O::add(s_wpart[warp][k], p1);
-                        s_wpart[warp][TRD_NB + k] = O::add(s_wpart[warp][TRD_NB + k], p2);
-                    }
-                }
-            }
-            __syncthreads();
-            if (tid < 2 * TRD_NB) {
-                T s = O::zero();
-                for (int w = 0; w < TRD_NT / 32; ++w) s = O::add(s, s_wpart[w][tid]);
-                pt[(long)g * 2 * TRD_NB + tid] = s;
-            }
+        // v into column j of A (own rows) and into the shared-memory panel
+        const int rb = max(r0, j + 1);
+        for (int r = rb + tid; r < r1; r += TRD_NT) {
+            const T v = vval(r);
+            A[r + (long)j * lda] = v;
+            if (cached) sV[i * TRD_CHP + (r - r0)] = v;
         }
-        // HEMV over the 64x64 tiles (I >= J >= bmin) of the lower triangle of A[j+1:, j+1:]
-        double vav = 0.0;
+        __syncthreads();
+        // partial t1 = W^H v, t2 = V^H v over the own rows: thread <-> (which, k, quarter of the rows)
         {
-            const int bmin = (j + 1) / TRD_TB, nbk = nblk - bmin, ntiles = nbk * (nbk + 1) / 2;
-            const int r = tid & 63, cg = tid >> 6;
-            auto decode = [&](int t, int &I, int &J) {
-                int ii = (int)((sqrt(8.0 * (double)t + 1.0) - 1.0) * 0.5);
-                while ((ii + 1) * (ii + 2) / 2 <= t) ++ii;
-                while (ii * (ii + 1) / 2 > t) --ii;
-                I = bmin + ii; J = bmin + (t - ii * (ii + 1) / 2);
-            };
-            auto load = [&](T a[8], int t) {
-                int I, J; decode(t, I, J);
-                const int gr = I * TRD_TB + r;
-#pragma unroll
-                for (int q = 0; q < 8; ++q) {
-                    const int gc = J * TRD_TB + cg * 8 + q;
-                    T v = O::zero();
-                    if (gr < n && gc >= j + 1 && gr >= gc) {
-                        v = A[gr + (long)gc * lda];
-                        if (gr == gc) v = O::from_real(O::real(v));
-                    }
-                    a[q] = v;
-                }
-            };
-            T cur[8], nxt[8];
-            int t = g;
-            if (t < ntiles) load(cur, t);
-            while (t < ntiles) {
-                const int tn = t + G;
-                if (tn < ntiles) load(nxt, tn);
-                int I, J; decode(t, I, J);
-                if (tid < TRD_TB) xs_col[tid] = vval(J * TRD_TB + tid);
-                else if (tid < 2 * TRD_TB) xs_row[tid - TRD_TB] = vval(I * TRD_TB + tid - TRD_TB);
-                __syncthreads();
-                const T xr = xs_row[r];
-                T rs = O::zero();
-                T cs[8];
-#pragma unroll
-                for (int q = 0; q < 8; ++q) {
-                    const int c = cg * 8 + q;
-                    rs = O::fma(cur[q], xs_col[c], rs);
-                    const bool strict = (I > J) || (r > c);
-                    cs[q] = strict ? O::conj_mul(cur[q], xr) : O::zero();
-                }
-                red_row[cg][r] = rs;
-#pragma unroll
-                for (int q = 0; q < 8; ++q) {
-                    T s = warp_sum(cs[q]);
-                    if (lane == 0) red_col[warp][q] = s;
-                }
-                __syncthreads();
-                if (tid < TRD_TB) {
-                    T s = O::zero();
-#pragma unroll
-                    for (int q = 0; q < 8; ++q) s = O::add(s, red_row[q][tid]);
-                    const int gr = I * TRD_TB + tid;
-                    if (gr < n) Prow[(long)J * n + gr] = s;
-                    vav += O::real(O::conj_mul(xs_row[tid], s));
-                } else if (tid < 2 * TRD_TB) {
-                    const int c = tid - TRD_TB, cg2 = c >> 3, q = c & 7;
-                    T s = O::add(red_col[2 * cg2][q], red_col[2 * cg2 + 1][q]);
-                    const int gc = J * TRD_TB + c;
-                    if (gc < n) Pcol[(long)I * n + gc] = s;
-                    vav += O::real(O::conj_mul(xs_col[c], s));
-                }
-                __syncthreads();
-#pragma unroll
-                for (int q = 0; q < 8; ++q) cur[q] = nxt[q];
-                t = tn;
+            const int idx = tid & 63, part = tid >> 6;
+            const int k = idx < TRD_NB ? idx : idx - TRD_NB;
+            T s = O::zero();
+            if (k < i) {
+                if (idx < TRD_NB)
+                    for (int r = rb + part; r < r1; r += 4) s = O::add(s, O::conj_mul(getW(r, k), cached ? sV[i * TRD_CHP + (r - r0)] : vval(r)));
+                else
+                    for (int r = rb + part; r < r1; r += 4) s = O::add(s, O::conj_mul(getV(r, k), cached ? sV[i * TRD_CHP + (r - r0)] : vval(r)));
             }
+            s_red4[part][idx] = s;
+            __syncthreads();
+            if (tid < 2 * TRD_NB)
+                pt[(long)g * 2 * TRD_NB + tid] = O::add(O::add(s_red4[0][tid], s_red4[1][tid]), O::add(s_red4[2][tid], s_red4[3][tid]));
         }
+        double vav = hemv_warp<T>(A, lda, n, j, nblk, G, g, acol, scale, sx + warp * SW, Prow, Pcol);
         vav = block_sum_d(vav, s_dred);
         if (tid == 0) pvav[g] = vav;
         group_barrier(bar, G, ++bar_ord);
@@ -334,7 +464,7 @@ static TrdWork trd_plan(int dtype, int n, int batch, void *work) {
     w.Wp = ar.take((size_t)batch * n * TRD_NB * es);
     w.acol = ar.take((size_t)batch * n * es);
     w.pt = ar.take((size_t)batch * w.G * 2 * TRD_NB * es);
-    w.Prow = ar.take((size_t)batch * w.nblk * n * es);
+    w.Prow = ar.take((size_t)batch * (dtype == NAO_COMPLEX ? 2 : 1) * w.nblk * n * es);
     w.Pcol = ar.take((size_t)batch * w.nblk * n * es);
     w.pn = (double *)ar.take((size_t)batch * w.G * 8);
     w.pvav = (double *)ar.take((size_t)batch * w.G * 8);
@@ -349,6 +479,12 @@ static int hetrd_impl(int dtype, int n, int batch, T *A, long lda, long sA, doub
                       cudaStream_t st) {
     TrdWork w = trd_plan(dtype, n, batch, work);
     const int npanels = ceil_div(n, TRD_NB) + 1;
+    const size_t smem = (size_t)(2 * TRD_NB * TRD_CHP + TRD_NW * TRD_PASS + TRD_NW * Hv<T>::SW) * sizeof(T);
+    static bool attr_set = false;
+    if (!attr_set) {
+        NAO_CUDA_CHECK(cudaFuncSetAttribute(hetrd_panel_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set = true;
+    }
     NAO_CUDA_CHECK(cudaMemsetAsync(w.bar, 0, (size_t)batch * npanels * 4, st));
     int panel = 0;
     for (int j0 = 0; j0 == 0 || j0 < n - 1; j0 += TRD_NB, ++panel) {
@@ -360,7 +496,7 @@ static int hetrd_impl(int dtype, int n, int batch, T *A, long lda, long sA, doub
             a.d = d + (long)b0 * n; a.e = e + (long)b0 * n; a.tau = tau + (long)b0 * n;
             a.Wp = (T *)w.Wp + (long)b0 * n * TRD_NB; a.acol = (T *)w.acol + (long)b0 * n;
             a.pn = w.pn + (long)b0 * w.G; a.pt = (T *)w.pt + (long)b0 * w.G * 2 * TRD_NB; a.pvav = w.pvav + (long)b0 * w.G;
-            a.Prow = (T *)w.Prow + (long)b0 * w.nblk * n; a.Pcol = (T *)w.Pcol + (long)b0 * w.nblk * n;
+            a.Prow = (T *)w.Prow + (long)b0 * Hv<T>::HS * w.nblk * n; a.Pcol = (T *)w.Pcol + (long)b0 * w.nblk * n;
             a.bar = w.bar + (size_t)panel * batch + b0;
             a.n = n; a.j0 = j0; a.nbp = nbp; a.G = w.G; a.nblk = w.nblk;
             // algorithmic bytes of this launch: the lower triangle of the trailing matrix once per column
@@ -368,7 +504,7 @@ static int hetrd_impl(int dtype, int n, int batch, T *A, long lda, long sA, doub
             for (int i = 0; i < nbp; ++i) { double mm = n - (j0 + i) - 1; bytes += 0.5 * mm * (mm + 1) * sizeof(T); }
             const int pk = prof_kernel_begin(0, bytes * nb_items, st);
             void *args[] = {&a};
-            NAO_CUDA_CHECK(cudaLaunchCooperativeKernel((void *)hetrd_panel_kernel<T>, dim3(nb_items * w.G), dim3(TRD_NT), args, 0, st));
+            NAO_CUDA_CHECK(cudaLaunchCooperativeKernel((void *)hetrd_panel_kernel<T>, dim3(nb_items * w.G), dim3(TRD_NT), args, smem, st));
             NAO_LAUNCHED();
             prof_kernel_end(0, pk, st);
         }
@@ -394,118 +530,4 @@ int hetrd(int dtype, int n, int batch, void *A, long lda, long sA, double *d, do
     return dtype == NAO_COMPLEX ? hetrd_impl<cplx>(dtype, n, batch, (cplx *)A, lda, sA, d, e, (cplx *)tau, work, st)
                                 : hetrd_impl<double>(dtype, n, batch, (double *)A, lda, sA, d, e, (double *)tau, work, st);
 }
-
-// ----------------------------------------------------------------------------------------------------------------
-// Back-transformation: Z <- Q Z, Q = H(0) H(1) ... H(n-2), H(j) = I - tau_j v_j v_j^H, v_j = A[j+1:, j] (unit first
-// element stored explicitly by hetrd).  Blocks of KB reflectors, last block first:
-//   Vb (explicit, zeros above the unit diagonal), G = Vb^H Vb, T by the xLARFT recurrence, then three GEMMs
-//   X = Vb^H Z ; X <- T X ; Z -= Vb X.
-// ----------------------------------------------------------------------------------------------------------------
-static const int ORM_KB = 64;
-
-template <class T>
-__global__ void build_v_kernel(int n, int jb, int kb, const T *A, long lda, long sA, T *V, long ldv, long sV) {
-    // V (m x kb), m = n - jb - 1, row r <-> global row jb+1+r; column k <-> reflector jb+k whose unit sits at r == k
-    A += (long)blockIdx.z * sA; V += (long)blockIdx.z * sV;
-    const int m = n - jb - 1;
-    int r = blockIdx.x * blockDim.x + threadIdx.x;
-    if (r >= m) return;
-    for (int k = blockIdx.y; k < kb; k += gridDim.y) {
-        T v;
-        if (r < k) v = Ops<T>::zero();
-        else if (r == k) v = Ops<T>::one();
-        else v = A[(jb + 1 + r) + (long)(jb + k) * lda];
-        V[r + (long)k * ldv] = v;
-    }
-}
-
-// T (kb x kb upper) from G = V^H V and tau: T(i,i) = tau_i ; T(0:i, i) = -tau_i T(0:i,0:i) G(0:i, i)
-template <class T>
-__global__ void __launch_bounds__(256) larft_kernel(int kb, const T *G, long sG, const T *tau, long sTau, T *Tm, long sT) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    T *sT_ = (T *)smem_raw;             // kb x kb, column-major
-    __shared__ T s_g[ORM_KB];
-    G += (long)blockIdx.x * sG; tau += (long)blockIdx.x * sTau; Tm += (long)blockIdx.x * sT;
-    const int tid = threadIdx.x;
-    for (int e = tid; e < kb * kb; e += blockDim.x) sT_[e] = Ops<T>::zero();
-    __syncthreads();
-    for (int i = 0; i < kb; ++i) {
-        const T ti = tau[i];
-        if (tid < i) s_g[tid] = G[tid + (long)i * kb];
-        __syncthreads();
-        if (tid < i) {
-            // row tid of T(0:i,0:i) times g  (T upper: columns c >= tid)
-            T acc = Ops<T>::zero();
-            for (int c = tid; c < i; ++c) acc = Ops<T>::fma(sT_[tid + c * kb], s_g[c], acc);
-            T v = Ops<T>::mul(ti, acc);
-            sT_[tid + i * kb] = Ops<T>::sub(Ops<T>::zero(), v);
-        }
-        if (tid == 0) sT_[i + i * kb] = ti;
-        __syncthreads();
-    }
-    for (int e = tid; e < kb * kb; e += blockDim.x) Tm[e] = sT_[e];
-}
-
-struct OrmWork { void *V, *G, *T, *X, *X2; size_t bytes; };
-static OrmWork orm_plan(int dtype, int n, int ncols, int batch, void *work) {
-    OrmWork w; const size_t es = esize(dtype);
-    Arena ar(work, (size_t)-1);
-    w.V = ar.take((size_t)batch * n * ORM_KB * es);
-    w.G = ar.take((size_t)batch * ORM_KB * ORM_KB * es);
-    w.T = ar.take((size_t)batch * ORM_KB * ORM_KB * es);
-    w.X = ar.take((size_t)batch * ORM_KB * ncols * es);
-    w.X2 = ar.take((size_t)batch * ORM_KB * ncols * es);
-    w.bytes = ar.off;
-    return w;
-}
-size_t ormtr_workspace(int dtype, int n, int batch) { return orm_plan(dtype, n, n, batch, nullptr).bytes; }
-
-template <class T>
-static int ormtr_impl(int dtype, int n, int ncols, int batch, const T *A, long lda, long sA, const T *tau, T *Z, long ldz,
-                      long sZ, void *work, cudaStream_t st) {
-    if (n < 2) return NAO_OK;
-    OrmWork w = orm_plan(dtype, n, ncols, batch, work);
-    const int nref = n - 1;
-    static bool attr = false;
-    if (!attr) {
-        NAO_CUDA_CHECK(cudaFuncSetAttribute(larft_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                            (int)(ORM_KB * ORM_KB * sizeof(T))));
-        attr = true;
-    }
-    const int nblocks = ceil_div(nref, ORM_KB);
-    for (int blk = nblocks - 1; blk >= 0; --blk) {
-        const int jb = blk * ORM_KB, kb = min(ORM_KB, nref - jb), m = n - jb - 1;
-        const long ldv = m, sV = (long)n * ORM_KB;
-        build_v_kernel<T><<<dim3(ceil_div(m, 256), kb, batch), 256, 0, st>>>(n, jb, kb, A, lda, sA, (T *)w.V, ldv, sV);
-        NAO_LAUNCHED();
-        // G = V^H V
-        GemmDesc g = gemm_desc(OP_C, OP_N, kb, kb, m, 1.0, w.V, ldv, w.V, ldv, 0.0, w.G, kb);
-        g.sA = sV; g.sB = sV; g.sC = ORM_KB * ORM_KB;
-        if (int rc = gemm_launch(dtype, g, batch, st)) return rc;
-        larft_kernel<T><<<batch, 256, kb * kb * sizeof(T), st>>>(kb, (const T *)w.G, ORM_KB * ORM_KB, tau + jb, n, (T *)w.T, ORM_KB * ORM_KB);
-        NAO_LAUNCHED();
-        // X = V^H Z[jb+1:, :]
-        GemmDesc x = gemm_desc(OP_C, OP_N, kb, ncols, m, 1.0, w.V, ldv, Z + jb + 1, ldz, 0.0, w.X, kb);
-        x.sA = sV; x.sB = sZ; x.sC = (long)ORM_KB * ncols;
-        if (int rc = gemm_launch(dtype, x, batch, st)) return rc;
-        // X2 = T X
-        GemmDesc t = gemm_desc(OP_N, OP_N, kb, ncols, kb, 1.0, w.T, kb, w.X, kb, 0.0, w.X2, kb);
-        t.sA = ORM_KB * ORM_KB; t.sB = (long)ORM_KB * ncols; t.sC = (long)ORM_KB * ncols; t.maskA = MASK_UPPER;
-        if (int rc = gemm_launch(dtype, t, batch, st)) return rc;
-        // Z[jb+1:, :] -= V X2
-        GemmDesc u = gemm_desc(OP_N, OP_N, m, ncols, kb, -1.0, w.V, ldv, w.X2, kb, 1.0, Z + jb + 1, ldz);
-        u.sA = sV; u.sB = (long)ORM_KB * ncols; u.sC = sZ;
-        if (int rc = gemm_launch(dtype, u, batch, st)) return rc;
-    }
-    NAO_CUDA_CHECK(cudaGetLastError());
-    return NAO_OK;
-}
-
-int ormtr(int dtype, int n, int ncols, int batch, const void *A, long lda, long sA, const void *tau, void *Z, long ldz,
-          long sZ, void *work, cudaStream_t st) {
-    return dtype == NAO_COMPLEX
-               ? ormtr_impl<cplx>(dtype, n, ncols, batch, (const cplx *)A, lda, sA, (const cplx *)tau, (cplx *)Z, ldz, sZ, work, st)
-               : ormtr_impl<double>(dtype, n, ncols, batch, (const double *)A, lda, sA, (const double *)tau, (double *)Z, ldz, sZ, work, st);
-}
-
 }  // namespace nao
