@@ -145,6 +145,8 @@ const char *nao_profile_phase_name(int i);
  */
 int nao_profile_kernel(int slot, double *h_ms, double *h_work, int *h_launches);
 const char *nao_profile_kernel_name(int slot);
+/* Per-launch durations (ms) of the launches recorded in `slot`, in launch order; returns the number written. */
+int nao_profile_kernel_launches(int slot, double *h_ms, int max_launches);
 
 /* ---- building blocks exported for tests and per-kernel measurement (same pointer/stream conventions) ---- */
 

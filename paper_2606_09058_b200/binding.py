@@ -40,6 +40,7 @@ _SIGNATURES = {
     "nao_profile_phase_name": ([_i], ctypes.c_char_p),
     "nao_profile_kernel": ([_i, _dp, _dp, ctypes.POINTER(ctypes.c_int)], _i),
     "nao_profile_kernel_name": ([_i], ctypes.c_char_p),
+    "nao_profile_kernel_launches": ([_i, _dp, _i], _i),
     "nao_gemm": ([_i, _i, _i, _i, _i, _i, _d, _vp, _l, _l, _vp, _l, _l, _d, _vp, _l, _l, _i, _i, _vp], _i),
     "nao_potrf_trtri": ([_i, _i, _i, _vp, _l, _l, _vp, _vp, _vp, _vp], _i),
     "nao_heev_workspace": ([_i, _i, _i, ctypes.c_uint, _szp], _i),
@@ -127,6 +128,15 @@ def profile_kernel(slot: int) -> dict:
     ms, work, k = ctypes.c_double(0), ctypes.c_double(0), ctypes.c_int(0)
     _check(lib().nao_profile_kernel(slot, ctypes.byref(ms), ctypes.byref(work), ctypes.byref(k)), "nao_profile_kernel")
     return {"name": lib().nao_profile_kernel_name(slot).decode(), "ms": ms.value, "work": work.value, "launches": k.value}
+
+
+def profile_kernel_launches(slot: int, max_launches: int = 2048) -> list:
+    """Per-launch durations (ms) of one kernel class since profile_enable(), in launch order."""
+    buf = (ctypes.c_double * max_launches)()
+    k = lib().nao_profile_kernel_launches(slot, buf, max_launches)
+    if k < 0:
+        raise NaoError("nao_profile_kernel_launches failed: %d" % k)
+    return [buf[i] for i in range(k)]
 
 
 def version() -> str:

@@ -69,6 +69,18 @@ NAO_EXPORT int nao_profile_kernel(int slot, double *h_ms, double *h_work, int *h
     if (h_launches) *h_launches = g_scount[slot];
     return NAO_OK;
 }
+NAO_EXPORT int nao_profile_kernel_launches(int slot, double *h_ms, int max_launches) {
+    using namespace nao;
+    if (slot < 0 || slot >= NSLOT) return -1;
+    if (!h_ms) return -2;
+    int k = 0;
+    for (; k < g_scount[slot] && k < max_launches; ++k) {
+        cudaEventSynchronize(g_sev[slot][k][1]);
+        float ms = 0.f;
+        h_ms[k] = (cudaEventElapsedTime(&ms, g_sev[slot][k][0], g_sev[slot][k][1]) == cudaSuccess) ? ms : -1.0;
+    }
+    return k;
+}
 NAO_EXPORT const char *nao_profile_kernel_name(int slot) { return (slot >= 0 && slot < nao::NSLOT) ? nao::kSlotNames[slot] : ""; }
 NAO_EXPORT int nao_profile_read(double *h_ms, int max_phases) {
     using namespace nao;

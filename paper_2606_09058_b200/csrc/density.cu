@@ -23,7 +23,7 @@ __global__ void dm_setup_kernel(int n, int dtype, const void *C, long ldc, long 
         d.lda = ldc; d.ldb = ldc; d.ldc = ldd; d.sA = d.sB = d.sC = 0;
         d.m = n; d.n = n; d.k = last + 1;
         d.opA = OP_N; d.opB = OP_C; d.maskA = d.maskB = MASK_NONE; d.offA = d.offB = 0;
-        d.cmode = 1; d.conjC = 0; d.alpha = 1.0; d.beta = 0.0; d.scaleK = f; d.sScale = 0;
+        d.cmode = 1; d.conjC = 0; d.alpha = 1.0; d.beta = 0.0; d.scaleK = f; d.sScale = 0; d.ksplit = 1; d.sSplit = 0;
         descs[b] = d;
     }
 }

@@ -127,10 +127,12 @@ gemm_kernel(const GemmDesc hd, const GemmDesc *__restrict__ dd) {
     const int m0 = tm * BM, n0 = tn * BN;
     if (d.cmode == 1 && n0 > m0 + BM - 1) return;
 
-    const long b = blockIdx.y;
+    const int ks = d.ksplit > 1 ? d.ksplit : 1;
+    const long b = blockIdx.y / ks;
+    const int slice = blockIdx.y % ks;
     const T *A = (const T *)d.A + b * d.sA;
     const T *B = (const T *)d.B + b * d.sB;
-    T *C = (T *)d.C + b * d.sC;
+    T *C = (T *)d.C + b * d.sC + (long)slice * d.sSplit;
     const double *scaleK = d.scaleK ? d.scaleK + b * d.sScale : nullptr;
 
     // op(A)(i,k): N -> stored (r,c) = (i,k), m-contiguous;  T/C -> stored (k,i), k-contiguous
@@ -142,6 +144,10 @@ gemm_kernel(const GemmDesc hd, const GemmDesc *__restrict__ dd) {
     mask_krange(d.maskA, d.offA, a_kcol, m0, min(m0 + BM, M) - 1, kb, ke);
     mask_krange(d.maskB, d.offB, b_kcol, n0, min(n0 + BN, N) - 1, kb, ke);
     kb = max(kb, 0); ke = min(ke, K);
+    if (ks > 1) {
+        const int kchunk = ((K + ks - 1) / ks + BK - 1) / BK * BK;
+        kb = max(kb, slice * kchunk); ke = min(ke, (slice + 1) * kchunk);
+    }
     const int kt0 = kb / BK;
     const int nkt = ke > kb ? (ke - 1) / BK + 1 - kt0 : 0;
 
@@ -290,8 +296,51 @@ static int launch_impl(const GemmDesc *hd, const GemmDesc *dd, int ngroups, int 
 
 int gemm_launch(int dtype, const GemmDesc &d, int batch, cudaStream_t st) {
     if (d.m <= 0 || d.n <= 0) return NAO_OK;
-    return dtype == NAO_COMPLEX ? launch_impl<true>(&d, nullptr, 1, d.m, d.n, batch, st)
-                                : launch_impl<false>(&d, nullptr, 1, d.m, d.n, batch, st);
+    const int by = batch * (d.ksplit > 1 ? d.ksplit : 1);
+    return dtype == NAO_COMPLEX ? launch_impl<true>(&d, nullptr, 1, d.m, d.n, by, st)
+                                : launch_impl<false>(&d, nullptr, 1, d.m, d.n, by, st);
+}
+
+template <class T>
+__global__ void splitk_reduce_kernel(int m, int n, int ks, const T *P, T *C, long ldc, long sC, double alpha, double beta) {
+    const long b = blockIdx.z;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= m) return;
+    P += b * (long)ks * m * n; C += b * sC;
+    for (int j = blockIdx.y; j < n; j += gridDim.y) {
+        double sr = 0.0, si = 0.0;
+        for (int s = 0; s < ks; ++s) {
+            const T v = P[((long)s * n + j) * m + i];
+            if constexpr (sizeof(T) == 16) { sr += v.x; si += v.y; } else { sr += v; }
+        }
+        T *c = C + i + (long)j * ldc;
+        if constexpr (sizeof(T) == 16) {
+            cplx o = make_double2(alpha * sr, alpha * si);
+            if (beta != 0.0) { o.x += beta * c->x; o.y += beta * c->y; }
+            *c = o;
+        } else {
+            double o = alpha * sr;
+            if (beta != 0.0) o += beta * *c;
+            *c = o;
+        }
+    }
+}
+
+int gemm_splitk(int dtype, const GemmDesc &d0, int batch, int ksplit, void *partial, cudaStream_t st) {
+    if (d0.m <= 0 || d0.n <= 0 || batch <= 0) return NAO_OK;
+    if (ksplit <= 1) return gemm_launch(dtype, d0, batch, st);
+    GemmDesc d = d0;
+    d.C = partial; d.ldc = d0.m; d.sC = (long)ksplit * d0.m * d0.n; d.sSplit = (long)d0.m * d0.n; d.ksplit = ksplit;
+    d.alpha = 1.0; d.beta = 0.0; d.cmode = 0;
+    if (int rc = gemm_launch(dtype, d, batch, st)) return rc;
+    dim3 grid((unsigned)ceil_div(d0.m, 128), (unsigned)(d0.n < 4096 ? d0.n : 4096), (unsigned)batch);
+    if (dtype == NAO_COMPLEX)
+        splitk_reduce_kernel<cplx><<<grid, 128, 0, st>>>(d0.m, d0.n, ksplit, (const cplx *)partial, (cplx *)d0.C, d0.ldc, d0.sC, d0.alpha, d0.beta);
+    else
+        splitk_reduce_kernel<double><<<grid, 128, 0, st>>>(d0.m, d0.n, ksplit, (const double *)partial, (double *)d0.C, d0.ldc, d0.sC, d0.alpha, d0.beta);
+    NAO_LAUNCHED();
+    NAO_CUDA_CHECK(cudaGetLastError());
+    return NAO_OK;
 }
 int gemm_launch_grouped(int dtype, const GemmDesc *dd, int ngroups, int max_m, int max_n, int batch, cudaStream_t st) {
     return dtype == NAO_COMPLEX ? launch_impl<true>(nullptr, dd, ngroups, max_m, max_n, batch, st)

@@ -58,6 +58,8 @@ struct GemmDesc {
     double alpha, beta;
     const double *scaleK;     // optional: op(A)[:,k] is multiplied by scaleK[k]
     long sScale;              // batch stride of scaleK
+    int ksplit;               // > 1: the k range is cut into ksplit slices, slice s writes C + s * sSplit (grid.y = batch * ksplit)
+    long sSplit;
 };
 
 static inline GemmDesc gemm_desc(int opA, int opB, int m, int n, int k, double alpha, const void *A, long lda,
@@ -65,7 +67,7 @@ static inline GemmDesc gemm_desc(int opA, int opB, int m, int n, int k, double a
     GemmDesc d;
     d.A = A; d.B = B; d.C = C; d.lda = lda; d.ldb = ldb; d.ldc = ldc; d.sA = d.sB = d.sC = 0;
     d.m = m; d.n = n; d.k = k; d.opA = opA; d.opB = opB; d.maskA = d.maskB = MASK_NONE; d.offA = d.offB = 0;
-    d.cmode = 0; d.conjC = 0; d.alpha = alpha; d.beta = beta; d.scaleK = nullptr; d.sScale = 0;
+    d.cmode = 0; d.conjC = 0; d.alpha = alpha; d.beta = beta; d.scaleK = nullptr; d.sScale = 0; d.ksplit = 1; d.sSplit = 0;
     return d;
 }
 
@@ -73,6 +75,9 @@ static inline GemmDesc gemm_desc(int opA, int opB, int m, int n, int k, double a
 int gemm_launch(int dtype, const GemmDesc &d, int batch, cudaStream_t st);
 // `ngroups` problems described by descriptors in DEVICE memory (their m,n,k may have been written by a kernel);
 // max_m/max_n bound the grid.  Each group runs `batch` items.
+// Split-K product for short-and-wide outputs (m, n small, k long): `ksplit` slices write partial products into
+// `partial` (batch * ksplit * m * n elements), then C <- alpha * (sum of slices, fixed order) + beta * C.
+int gemm_splitk(int dtype, const GemmDesc &d, int batch, int ksplit, void *partial, cudaStream_t st);
 int gemm_launch_grouped(int dtype, const GemmDesc *d_descs, int ngroups, int max_m, int max_n, int batch,
                         cudaStream_t st);
 

@@ -1,6 +1,7 @@
 // ormtr.cu -- blocked back-transformation Z <- Q Z of the one-stage tridiagonalisation.
 #include "nao_internal.cuh"
 #include "scalar.cuh"
+#include <algorithm>
 
 namespace nao {
 
@@ -11,7 +12,7 @@ namespace nao {
 //   Vb (explicit, zeros above the unit diagonal), G = Vb^H Vb, T by the xLARFT recurrence, then three GEMMs
 //   X = Vb^H Z ; X <- T X ; Z -= Vb X.
 // ----------------------------------------------------------------------------------------------------------------
-static const int ORM_KB = 64;
+static const int ORM_KB = 128;
 
 template <class T>
 __global__ void build_v_kernel(int n, int jb, int kb, const T *A, long lda, long sA, T *V, long ldv, long sV) {
@@ -29,42 +30,49 @@ __global__ void build_v_kernel(int n, int jb, int kb, const T *A, long lda, long
     }
 }
 
-// T (kb x kb upper) from G = V^H V and tau: T(i,i) = tau_i ; T(0:i, i) = -tau_i T(0:i,0:i) G(0:i, i)
+// T (kb x kb upper) from G = V^H V and tau: T(i,i) = tau_i ; T(0:i, i) = -tau_i T(0:i,0:i) G(0:i, i).
+// T is built in shared memory in packed upper storage ((r,c), r <= c, at c(c+1)/2 + r) and written out dense.
 template <class T>
-__global__ void __launch_bounds__(256) larft_kernel(int kb, const T *G, long sG, const T *tau, long sTau, T *Tm, long sT) {
+__global__ void __launch_bounds__(256) larft_kernel(int kb, const T *G, long ldg, long sG, const T *tau, long sTau, T *Tm, long sT) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    T *sT_ = (T *)smem_raw;             // kb x kb, column-major
+    T *sT_ = (T *)smem_raw;             // packed upper, kb(kb+1)/2
     __shared__ T s_g[ORM_KB];
     G += (long)blockIdx.x * sG; tau += (long)blockIdx.x * sTau; Tm += (long)blockIdx.x * sT;
     const int tid = threadIdx.x;
-    for (int e = tid; e < kb * kb; e += blockDim.x) sT_[e] = Ops<T>::zero();
-    __syncthreads();
     for (int i = 0; i < kb; ++i) {
         const T ti = tau[i];
-        if (tid < i) s_g[tid] = G[tid + (long)i * kb];
+        if (tid < i) s_g[tid] = G[tid + (long)i * ldg];
         __syncthreads();
         if (tid < i) {
             // row tid of T(0:i,0:i) times g  (T upper: columns c >= tid)
             T acc = Ops<T>::zero();
-            for (int c = tid; c < i; ++c) acc = Ops<T>::fma(sT_[tid + c * kb], s_g[c], acc);
-            T v = Ops<T>::mul(ti, acc);
-            sT_[tid + i * kb] = Ops<T>::sub(Ops<T>::zero(), v);
+            for (int c = tid; c < i; ++c) acc = Ops<T>::fma(sT_[c * (c + 1) / 2 + tid], s_g[c], acc);
+            sT_[i * (i + 1) / 2 + tid] = Ops<T>::sub(Ops<T>::zero(), Ops<T>::mul(ti, acc));
         }
-        if (tid == 0) sT_[i + i * kb] = ti;
+        if (tid == 0) sT_[i * (i + 1) / 2 + i] = ti;
         __syncthreads();
     }
-    for (int e = tid; e < kb * kb; e += blockDim.x) Tm[e] = sT_[e];
+    for (int e = tid; e < kb * kb; e += blockDim.x) {
+        const int r = e % kb, c = e / kb;
+        Tm[e] = r <= c ? sT_[c * (c + 1) / 2 + r] : Ops<T>::zero();
+    }
 }
 
-struct OrmWork { void *V, *G, *T, *X, *X2; size_t bytes; };
+struct OrmWork { void *V, *G, *T, *X, *X2, *P; size_t bytes; int ksG, ksX; };
 static OrmWork orm_plan(int dtype, int n, int ncols, int batch, void *work) {
     OrmWork w; const size_t es = esize(dtype);
     Arena ar(work, (size_t)-1);
+    // split-K factors for the two tall-skinny^H products (k = m up to n): fill ~2 waves of 148 SMs
+    const int tilesX = ceil_div(ncols, dtype == NAO_COMPLEX ? 64 : 128) * batch;
+    w.ksX = std::max(1, std::min(std::min(296 / std::max(1, tilesX), ceil_div(n, 512)), 16));
+    const int tilesG = (dtype == NAO_COMPLEX ? 2 : 1) * batch;
+    w.ksG = std::max(1, std::min(std::min(148 / std::max(1, tilesG), ceil_div(n, 256)), 64));
     w.V = ar.take((size_t)batch * n * ORM_KB * es);
     w.G = ar.take((size_t)batch * ORM_KB * ORM_KB * es);
     w.T = ar.take((size_t)batch * ORM_KB * ORM_KB * es);
     w.X = ar.take((size_t)batch * ORM_KB * ncols * es);
     w.X2 = ar.take((size_t)batch * ORM_KB * ncols * es);
+    w.P = ar.take((size_t)batch * std::max((size_t)w.ksX * ORM_KB * ncols, (size_t)w.ksG * ORM_KB * ORM_KB) * es);
     w.bytes = ar.off;
     return w;
 }
@@ -77,27 +85,27 @@ static int ormtr_impl(int dtype, int n, int ncols, int batch, const T *A, long l
     OrmWork w = orm_plan(dtype, n, ncols, batch, work);
     const int nref = n - 1;
     static bool attr = false;
+    const size_t larft_smem = (size_t)ORM_KB * (ORM_KB + 1) / 2 * sizeof(T);
     if (!attr) {
-        NAO_CUDA_CHECK(cudaFuncSetAttribute(larft_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                            (int)(ORM_KB * ORM_KB * sizeof(T))));
+        NAO_CUDA_CHECK(cudaFuncSetAttribute(larft_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)larft_smem));
         attr = true;
     }
     const int nblocks = ceil_div(nref, ORM_KB);
     for (int blk = nblocks - 1; blk >= 0; --blk) {
-        const int jb = blk * ORM_KB, kb = min(ORM_KB, nref - jb), m = n - jb - 1;
+        const int jb = blk * ORM_KB, kb = std::min(ORM_KB, nref - jb), m = n - jb - 1;
         const long ldv = m, sV = (long)n * ORM_KB;
         build_v_kernel<T><<<dim3(ceil_div(m, 256), kb, batch), 256, 0, st>>>(n, jb, kb, A, lda, sA, (T *)w.V, ldv, sV);
         NAO_LAUNCHED();
-        // G = V^H V
+        // G = V^H V  (kb x kb, k = m: split-K)
         GemmDesc g = gemm_desc(OP_C, OP_N, kb, kb, m, 1.0, w.V, ldv, w.V, ldv, 0.0, w.G, kb);
         g.sA = sV; g.sB = sV; g.sC = ORM_KB * ORM_KB;
-        if (int rc = gemm_launch(dtype, g, batch, st)) return rc;
-        larft_kernel<T><<<batch, 256, kb * kb * sizeof(T), st>>>(kb, (const T *)w.G, ORM_KB * ORM_KB, tau + jb, n, (T *)w.T, ORM_KB * ORM_KB);
+        if (int rc = gemm_splitk(dtype, g, batch, std::min(w.ksG, ceil_div(m, 256)), w.P, st)) return rc;
+        larft_kernel<T><<<batch, 256, larft_smem, st>>>(kb, (const T *)w.G, kb, ORM_KB * ORM_KB, tau + jb, n, (T *)w.T, ORM_KB * ORM_KB);
         NAO_LAUNCHED();
-        // X = V^H Z[jb+1:, :]
+        // X = V^H Z[jb+1:, :]  (kb x ncols, k = m: split-K)
         GemmDesc x = gemm_desc(OP_C, OP_N, kb, ncols, m, 1.0, w.V, ldv, Z + jb + 1, ldz, 0.0, w.X, kb);
         x.sA = sV; x.sB = sZ; x.sC = (long)ORM_KB * ncols;
-        if (int rc = gemm_launch(dtype, x, batch, st)) return rc;
+        if (int rc = gemm_splitk(dtype, x, batch, std::min(w.ksX, ceil_div(m, 512)), w.P, st)) return rc;
         // X2 = T X
         GemmDesc t = gemm_desc(OP_N, OP_N, kb, ncols, kb, 1.0, w.T, kb, w.X, kb, 0.0, w.X2, kb);
         t.sA = ORM_KB * ORM_KB; t.sB = (long)ORM_KB * ncols; t.sC = (long)ORM_KB * ncols; t.maskA = MASK_UPPER;

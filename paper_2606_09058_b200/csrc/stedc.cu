@@ -207,7 +207,7 @@ __global__ void __launch_bounds__(1024) dc_setup_kernel(DcBuf b, const DcNode *_
             GemmDesc g;
             g.lda = n; g.ldb = n; g.ldc = b.ldq; g.sA = g.sB = g.sC = 0; g.opA = OP_N; g.opB = OP_N;
             g.maskA = g.maskB = MASK_NONE; g.offA = g.offB = 0; g.cmode = 0; g.conjC = 0; g.alpha = 1.0; g.beta = 0.0;
-            g.scaleK = nullptr; g.sScale = 0;
+            g.scaleK = nullptr; g.sScale = 0; g.ksplit = 1; g.sSplit = 0;
             g.A = Qwb; g.B = Sb; g.C = Qb; g.m = n1; g.n = K; g.k = o.c1 + o.c2;
             b.desc[((long)item * nn + node) * 2] = g;
             g.A = Qwb + n1 + (long)o.c1 * n; g.B = Sb + o.c1; g.C = Qb + n1; g.m = n2; g.n = K; g.k = o.c2 + o.c3;
