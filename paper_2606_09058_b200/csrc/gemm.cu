@@ -241,27 +241,39 @@ gemm_kernel(const GemmDesc hd, const GemmDesc *__restrict__ dd) {
     }
     cp_async_wait<0>();
 
-    // epilogue: lane holds C[row = lr][cols 2*lc, 2*lc+1] of each 8x8 block
+    // epilogue: lane holds C[row = lr][cols 2*lc, 2*lc+1] of each 8x8 block.  With beta != 0 all old values of one
+    // row block are loaded first (independent loads in flight together), then combined and stored: a load -> store ->
+    // load chain would serialise on memory latency.
     const double alpha = d.alpha, beta = d.beta;
 #pragma unroll
     for (int i = 0; i < MI; ++i) {
-        int gi = m0 + wm + i * 8 + lr;
+        const int gi = m0 + wm + i * 8 + lr;
         if (gi >= M) continue;
+        T old[NI][2];
+        if (beta != 0.0) {
+#pragma unroll
+            for (int j = 0; j < NI; ++j)
+#pragma unroll
+                for (int q = 0; q < 2; ++q) {
+                    const int gj = n0 + wn + j * 8 + 2 * lc + q;
+                    if (gj < N) old[j][q] = C[gi + (long)gj * d.ldc];
+                }
+        }
 #pragma unroll
         for (int j = 0; j < NI; ++j) {
 #pragma unroll
             for (int q = 0; q < 2; ++q) {
-                int gj = n0 + wn + j * 8 + 2 * lc + q;
+                const int gj = n0 + wn + j * 8 + 2 * lc + q;
                 if (gj >= N) continue;
                 T *p = C + gi + (long)gj * d.ldc;
                 if constexpr (!CPLX) {
                     double v = alpha * acc[i][j][q];
-                    if (beta != 0.0) v += beta * *(double *)p;
-                    *(double *)p = v;
+                    if (beta != 0.0) v += beta * old[j][q];
+                    *p = v;
                 } else {
                     cplx v; v.x = alpha * acc[i][j][q]; v.y = alpha * acc[i][j][2 + q];
-                    if (beta != 0.0) { cplx o = *(cplx *)p; v.x += beta * o.x; v.y += beta * o.y; }
-                    *(cplx *)p = v;
+                    if (beta != 0.0) { v.x += beta * old[j][q].x; v.y += beta * old[j][q].y; }
+                    *p = v;
                 }
             }
         }

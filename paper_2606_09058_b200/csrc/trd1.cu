@@ -44,7 +44,7 @@ template <> struct Hv<cplx> { static const int SW = 32, CPT = 16, HS = 2, CB = 2
 template <class T> struct TrdArgs {
     T *A; long lda, sA;
     double *d, *e; T *tau;           // per item: n each
-    T *Wp;                           // per item: n x NB (ld n)
+    T *Wp;                           // per item: n x 4NB (ld n): [V | W | W | V] so that A22 -= [V W][W V]^H is one GEMM
     T *acol;                         // per item: n
     double *pn;                      // per item: G
     T *pt;                           // per item: G x 2NB
@@ -238,7 +238,8 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
     T *A = p.A + (long)item * p.sA;
     double *dd = p.d + (long)item * n, *ee = p.e + (long)item * n;
     T *tauv = p.tau + (long)item * n;
-    T *Wp = p.Wp + (long)item * n * TRD_NB;
+    T *P2 = p.Wp + (long)item * n * 4 * TRD_NB;       // [V | W | W | V], 32 columns each, ld n
+    T *Wp = P2 + (long)n * TRD_NB;
     T *acol = p.acol + (long)item * n;
     double *pn = p.pn + (long)item * G;
     T *pt = p.pt + (long)item * G * 2 * TRD_NB;
@@ -339,6 +340,7 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
                     const T wv = O::add(O::mul(s_tau, acc), O::scale(vr, s_alpha));
                     if (own) {
                         Wp[r + (long)(i - 1) * n] = wv;
+                        Wp[r + (long)(TRD_NB + i - 1) * n] = wv;
                         if (cached) sW[(i - 1) * TRD_CHP + (r - r0)] = wv;
                     }
                     if (r == j) s_wrow[i - 1] = wv;
@@ -408,6 +410,8 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
         for (int r = rb + tid; r < r1; r += TRD_NT) {
             const T v = vval(r);
             A[r + (long)j * lda] = v;
+            P2[r + (long)i * n] = v;
+            P2[r + (long)(3 * TRD_NB + i) * n] = v;
             if (cached) sV[i * TRD_CHP + (r - r0)] = v;
         }
         __syncthreads();
@@ -461,7 +465,7 @@ static TrdWork trd_plan(int dtype, int n, int batch, void *work) {
     w.items_per_launch = batch < nsm ? batch : nsm;
     const int npanels = ceil_div(n, TRD_NB) + 1;
     Arena ar(work, (size_t)-1);
-    w.Wp = ar.take((size_t)batch * n * TRD_NB * es);
+    w.Wp = ar.take((size_t)batch * n * 4 * TRD_NB * es);
     w.acol = ar.take((size_t)batch * n * es);
     w.pt = ar.take((size_t)batch * w.G * 2 * TRD_NB * es);
     w.Prow = ar.take((size_t)batch * (dtype == NAO_COMPLEX ? 2 : 1) * w.nblk * n * es);
@@ -494,7 +498,7 @@ static int hetrd_impl(int dtype, int n, int batch, T *A, long lda, long sA, doub
             TrdArgs<T> a;
             a.A = A + (long)b0 * sA; a.lda = lda; a.sA = sA;
             a.d = d + (long)b0 * n; a.e = e + (long)b0 * n; a.tau = tau + (long)b0 * n;
-            a.Wp = (T *)w.Wp + (long)b0 * n * TRD_NB; a.acol = (T *)w.acol + (long)b0 * n;
+            a.Wp = (T *)w.Wp + (long)b0 * n * 4 * TRD_NB; a.acol = (T *)w.acol + (long)b0 * n;
             a.pn = w.pn + (long)b0 * w.G; a.pt = (T *)w.pt + (long)b0 * w.G * 2 * TRD_NB; a.pvav = w.pvav + (long)b0 * w.G;
             a.Prow = (T *)w.Prow + (long)b0 * Hv<T>::HS * w.nblk * n; a.Pcol = (T *)w.Pcol + (long)b0 * w.nblk * n;
             a.bar = w.bar + (size_t)panel * batch + b0;
@@ -511,14 +515,24 @@ static int hetrd_impl(int dtype, int n, int batch, T *A, long lda, long sA, doub
         const int jn = j0 + nbp;             // first row/column of the trailing matrix
         if (nbp > 0 && jn < n) {
             const int mt = n - jn;
-            GemmDesc g1 = gemm_desc(OP_N, OP_C, mt, mt, nbp, -1.0, A + jn + (long)j0 * lda, lda, (T *)w.Wp + jn, n, 1.0,
-                                    A + jn + (long)jn * lda, lda);
-            g1.sA = sA; g1.sB = (long)n * TRD_NB; g1.sC = sA; g1.cmode = 1;
-            if (int rc = gemm_launch(dtype, g1, batch, st)) return rc;
-            GemmDesc g2 = gemm_desc(OP_N, OP_C, mt, mt, nbp, -1.0, (T *)w.Wp + jn, n, A + jn + (long)j0 * lda, lda, 1.0,
-                                    A + jn + (long)jn * lda, lda);
-            g2.sA = (long)n * TRD_NB; g2.sB = sA; g2.sC = sA; g2.cmode = 1;
-            if (int rc = gemm_launch(dtype, g2, batch, st)) return rc;
+            const long sP = (long)n * 4 * TRD_NB;
+            T *P2 = (T *)w.Wp;
+            if (nbp == TRD_NB) {
+                // A22 -= [V W] [W V]^H : one rank-64 update, the trailing matrix is read and written once
+                GemmDesc g1 = gemm_desc(OP_N, OP_C, mt, mt, 2 * TRD_NB, -1.0, P2 + jn, n, P2 + jn + (long)n * 2 * TRD_NB, n, 1.0,
+                                        A + jn + (long)jn * lda, lda);
+                g1.sA = sP; g1.sB = sP; g1.sC = sA; g1.cmode = 1;
+                if (int rc = gemm_launch(dtype, g1, batch, st)) return rc;
+            } else {
+                GemmDesc g1 = gemm_desc(OP_N, OP_C, mt, mt, nbp, -1.0, P2 + jn, n, P2 + jn + (long)n * TRD_NB, n, 1.0,
+                                        A + jn + (long)jn * lda, lda);
+                g1.sA = sP; g1.sB = sP; g1.sC = sA; g1.cmode = 1;
+                if (int rc = gemm_launch(dtype, g1, batch, st)) return rc;
+                GemmDesc g2 = gemm_desc(OP_N, OP_C, mt, mt, nbp, -1.0, P2 + jn + (long)n * TRD_NB, n, P2 + jn, n, 1.0,
+                                        A + jn + (long)jn * lda, lda);
+                g2.sA = sP; g2.sB = sP; g2.sC = sA; g2.cmode = 1;
+                if (int rc = gemm_launch(dtype, g2, batch, st)) return rc;
+            }
         }
         if (n == 1) break;
     }
