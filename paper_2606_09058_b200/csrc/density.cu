@@ -59,7 +59,7 @@ NAO_EXPORT int nao_density_matrix(int n, int batch, int dtype, const void *dC, l
     GemmDesc *descs = (GemmDesc *)dwork;
     dm_setup_kernel<<<batch, 32, 0, st>>>(n, dtype, dC, ldc, strideC, dF, dD, ldd, strideD, descs);
     NAO_LAUNCHED();
-    int rc = gemm_launch_grouped(dtype, descs, batch, n, n, 1, st);
+    int rc = gemm_launch_grouped(dtype, descs, batch, n, n, 1, OP_N, OP_C, true, st);
     if (rc) return rc;
     return herm_fill(dtype, n, dD, ldd, strideD, dD, ldd, strideD, batch, st);
 }

@@ -61,11 +61,11 @@ __device__ __forceinline__ void mask_krange(int mask, int off, bool k_is_col, in
 template <bool CPLX> struct Cfg;
 template <> struct Cfg<false> {
     typedef double T;
-    static const int BM = 128, BN = 128, BK = 16, WM = 32, WN = 64, STAGES = 3, PADX = 4, PADK = 4;
+    static const int BM = 128, BN = 128, BK = 16, WM = 32, WN = 64, STAGES = 4, PADX = 4, PADK = 4;
 };
 template <> struct Cfg<true> {
     typedef cplx T;
-    static const int BM = 128, BN = 64, BK = 16, WM = 32, WN = 32, STAGES = 3, PADX = 2, PADK = 2;
+    static const int BM = 128, BN = 64, BK = 16, WM = 32, WN = 32, STAGES = 4, PADX = 2, PADK = 2;
 };
 static const int GEMM_THREADS = 256;
 
@@ -104,7 +104,47 @@ __device__ __forceinline__ void load_tile(typename Cfg<CPLX>::T *s, const typena
     }
 }
 
-template <bool CPLX>
+// is the whole stored rectangle rows [r0,r1] x cols [c0,c1] kept by the mask?
+__device__ __forceinline__ bool mask_all_kept(int mask, int off, int r0, int r1, int c0, int c1) {
+    switch (mask) {
+        case MASK_NONE: return true;
+        case MASK_LOWER: return r0 - c1 + off >= 0;
+        case MASK_SLOWER: return r0 - c1 + off > 0;
+        case MASK_UPPER: return r1 - c0 + off <= 0;
+        default: return r1 - c0 + off < 0;
+    }
+}
+
+// Fast tile loader: 16-byte cp.async, one running global pointer per thread, compile-time shared-memory offsets.
+// Used for k-tiles that lie entirely inside the operand (no edge, no mask boundary, aligned); everything else goes
+// through load_tile.  The NCH chunks of a thread are issued in 4 parts so that the copies interleave with the DMMAs.
+template <bool CPLX, int BX, int BK, int PADX, int PADK, bool XC> struct FastLoad {
+    typedef typename Cfg<CPLX>::T T;
+    static const int VEC = CPLX ? 1 : 2;                       // elements per 16-byte chunk
+    static const int NCH = BX * BK / (VEC * GEMM_THREADS);     // chunks per thread per tile
+    static const int P = XC ? BX / VEC : BK / VEC;             // chunks along the contiguous direction
+    static const int STEP = GEMM_THREADS / P;                  // other-index distance between a thread's chunks
+    const T *g;            // chunk 0 of the current k-tile
+    long cstride;          // elements between consecutive chunks of this thread (STEP * ld)
+    long kadv;             // elements per k-tile
+    int soff;              // shared-memory offset of chunk 0
+    __device__ __forceinline__ void init(const T *Pm, long ld, int x0, int k0) {
+        const int tid = threadIdx.x;
+        const int c = (tid % P) * VEC, o = tid / P;
+        if (XC) { g = Pm + (x0 + c) + (long)(k0 + o) * ld; soff = o * (BX + PADX) + c; kadv = (long)BK * ld; }
+        else { g = Pm + (k0 + c) + (long)(x0 + o) * ld; soff = o * (BK + PADK) + c; kadv = BK; }
+        cstride = (long)STEP * ld;
+    }
+    template <int PART> __device__ __forceinline__ void issue(T *s) const {
+        constexpr int SSTR = XC ? STEP * (BX + PADX) : STEP * (BK + PADK);
+        constexpr int c0 = PART * NCH / 4, c1 = (PART + 1) * NCH / 4;
+#pragma unroll
+        for (int c = c0; c < c1; ++c) cp_async16(s + soff + c * SSTR, g + c * cstride, true);
+    }
+    __device__ __forceinline__ void advance() { g += kadv; }
+};
+
+template <bool CPLX, bool AXC, bool BXC, bool SCALE>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 gemm_kernel(const GemmDesc hd, const GemmDesc *__restrict__ dd) {
     typedef Cfg<CPLX> G;
@@ -125,24 +165,26 @@ gemm_kernel(const GemmDesc hd, const GemmDesc *__restrict__ dd) {
     if ((int)blockIdx.x >= tiles_m * tiles_n) return;
     const int tm = blockIdx.x % tiles_m, tn = blockIdx.x / tiles_m;
     const int m0 = tm * BM, n0 = tn * BN;
-    if (d.cmode == 1 && n0 > m0 + BM - 1) return;
+    const int cmode = d.cmode;
+    if (cmode == 1 && n0 > m0 + BM - 1) return;
 
     const int ks = d.ksplit > 1 ? d.ksplit : 1;
     const long b = blockIdx.y / ks;
     const int slice = blockIdx.y % ks;
     const T *A = (const T *)d.A + b * d.sA;
     const T *B = (const T *)d.B + b * d.sB;
+    const long lda = d.lda, ldb = d.ldb, ldc = d.ldc;
     T *C = (T *)d.C + b * d.sC + (long)slice * d.sSplit;
-    const double *scaleK = d.scaleK ? d.scaleK + b * d.sScale : nullptr;
+    const double *scaleK = SCALE ? d.scaleK + b * d.sScale : nullptr;
+    const int maskA = d.maskA, offA = d.offA, maskB = d.maskB, offB = d.offB;
 
-    // op(A)(i,k): N -> stored (r,c) = (i,k), m-contiguous;  T/C -> stored (k,i), k-contiguous
-    const bool a_xc = (d.opA == OP_N), b_xc = (d.opB != OP_N);     // op(B)(k,j): N -> stored (k,j) k-contig
-    const bool a_kcol = a_xc, b_kcol = b_xc;                        // is k the stored column index?
+    // op(A)(i,k): N -> stored (r,c) = (i,k), m-contiguous (AXC);  T/C -> stored (k,i), k-contiguous
+    // op(B)(k,j): N -> stored (k,j), k-contiguous;  T/C -> stored (j,k), n-contiguous (BXC)
     const bool conjA = CPLX && d.opA == OP_C, conjB = CPLX && d.opB == OP_C;
 
     int kb = 0, ke = K;
-    mask_krange(d.maskA, d.offA, a_kcol, m0, min(m0 + BM, M) - 1, kb, ke);
-    mask_krange(d.maskB, d.offB, b_kcol, n0, min(n0 + BN, N) - 1, kb, ke);
+    mask_krange(maskA, offA, AXC, m0, min(m0 + BM, M) - 1, kb, ke);
+    mask_krange(maskB, offB, BXC, n0, min(n0 + BN, N) - 1, kb, ke);
     kb = max(kb, 0); ke = min(ke, K);
     if (ks > 1) {
         const int kchunk = ((K + ks - 1) / ks + BK - 1) / BK * BK;
@@ -157,50 +199,114 @@ gemm_kernel(const GemmDesc hd, const GemmDesc *__restrict__ dd) {
     const int lr = lane >> 2, lc = lane & 3;
 
     double acc[MI][NI][CPLX ? 4 : 2];
+    const double alpha = d.alpha, beta = d.beta;
+    // beta != 0: the accumulators start from (beta/alpha) C, loaded while the first tiles are in flight, so that the
+    // epilogue is store-only (for alpha = +-1, beta = 1 -- every update on the path -- this is exact)
+    const bool preload = (beta != 0.0 && alpha != 0.0);
+    if (preload) {
+        const double r = beta / alpha;
 #pragma unroll
-    for (int i = 0; i < MI; ++i)
+        for (int i = 0; i < MI; ++i) {
+            const int gi = m0 + wm + i * 8 + lr;
 #pragma unroll
-        for (int j = 0; j < NI; ++j)
+            for (int j = 0; j < NI; ++j)
 #pragma unroll
-            for (int q = 0; q < (CPLX ? 4 : 2); ++q) acc[i][j][q] = 0.0;
+                for (int q = 0; q < 2; ++q) {
+                    const int gj = n0 + wn + j * 8 + 2 * lc + q;
+                    T v;
+                    if constexpr (CPLX) v = make_double2(0.0, 0.0); else v = 0.0;
+                    if (gi < M && gj < N) v = C[gi + (long)gj * ldc];
+                    if constexpr (CPLX) { acc[i][j][q] = r * v.x; acc[i][j][2 + q] = r * v.y; } else acc[i][j][q] = r * v;
+                }
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < MI; ++i)
+#pragma unroll
+            for (int j = 0; j < NI; ++j)
+#pragma unroll
+                for (int q = 0; q < (CPLX ? 4 : 2); ++q) acc[i][j][q] = 0.0;
+    }
 
-    const int a_sx = a_xc ? 1 : (BK + G::PADK), a_sk = a_xc ? (BM + G::PADX) : 1;
-    const int b_sx = b_xc ? 1 : (BK + G::PADK), b_sk = b_xc ? (BN + G::PADX) : 1;
+    constexpr int a_sx = AXC ? 1 : (BK + G::PADK), a_sk = AXC ? (BM + G::PADX) : 1;
+    constexpr int b_sx = BXC ? 1 : (BK + G::PADK), b_sk = BXC ? (BN + G::PADX) : 1;
 
-    auto issue = [&](int kt_rel) {
+    // ---- tile loading: fast (interior, aligned) or generic, decided per k-tile, uniformly over the CTA
+    FastLoad<CPLX, BM, BK, G::PADX, G::PADK, AXC> fa;
+    FastLoad<CPLX, BN, BK, G::PADX, G::PADK, BXC> fb;
+    fa.init(A, lda, m0, kt0 * BK);
+    fb.init(B, ldb, n0, kt0 * BK);
+    const bool a_al = CPLX || ((((size_t)A) & 15) == 0 && (lda & 1) == 0 && ((AXC ? m0 : 0) & 1) == 0);
+    const bool b_al = CPLX || ((((size_t)B) & 15) == 0 && (ldb & 1) == 0 && ((BXC ? n0 : 0) & 1) == 0);
+    const bool a_in = a_al && (m0 + BM <= M), b_in = b_al && (n0 + BN <= N);
+    auto a_fast = [&](int k0) -> bool {
+        if (!a_in || k0 < kb || k0 + BK > ke) return false;
+        return AXC ? mask_all_kept(maskA, offA, m0, m0 + BM - 1, k0, k0 + BK - 1)
+                   : mask_all_kept(maskA, offA, k0, k0 + BK - 1, m0, m0 + BM - 1);
+    };
+    auto b_fast = [&](int k0) -> bool {
+        if (!b_in || k0 < kb || k0 + BK > ke) return false;
+        return BXC ? mask_all_kept(maskB, offB, n0, n0 + BN - 1, k0, k0 + BK - 1)
+                   : mask_all_kept(maskB, offB, k0, k0 + BK - 1, n0, n0 + BN - 1);
+    };
+    // generic part of the load of k-tile kt_rel (+ the scale factors); returns which operands are left to the fast path
+    auto issue_generic = [&](int kt_rel, bool &fa_on, bool &fb_on) {
+        fa_on = fb_on = false;
         if (kt_rel < nkt) {
-            int stg = kt_rel % ST;
-            int k0 = (kt0 + kt_rel) * BK;
-            load_tile<CPLX, BM, BK, G::PADX, G::PADK>(sA + stg * ASZ, A, d.lda, a_xc, m0, M, k0, kb, ke, d.maskA, d.offA, a_kcol);
-            load_tile<CPLX, BN, BK, G::PADX, G::PADK>(sB + stg * BSZ, B, d.ldb, b_xc, n0, N, k0, kb, ke, d.maskB, d.offB, b_kcol);
-            if (scaleK && threadIdx.x < BK) {
-                int gk = k0 + threadIdx.x;
-                bool p = gk < ke;
+            const int stg = kt_rel % ST;
+            const int k0 = (kt0 + kt_rel) * BK;
+            fa_on = a_fast(k0); fb_on = b_fast(k0);
+            if (!fa_on) load_tile<CPLX, BM, BK, G::PADX, G::PADK>(sA + stg * ASZ, A, lda, AXC, m0, M, k0, kb, ke, maskA, offA, AXC);
+            if (!fb_on) load_tile<CPLX, BN, BK, G::PADX, G::PADK>(sB + stg * BSZ, B, ldb, BXC, n0, N, k0, kb, ke, maskB, offB, BXC);
+            if (SCALE && threadIdx.x < BK) {
+                const int gk = k0 + threadIdx.x;
+                const bool p = gk < ke;
                 cp_async8(sS + stg * BK + threadIdx.x, p ? scaleK + gk : scaleK, p);
             }
         }
-        cp_async_commit();
     };
 
-    for (int s = 0; s < ST - 1; ++s) issue(s);
+    for (int s = 0; s < ST - 1; ++s) {
+        bool fa_on, fb_on;
+        issue_generic(s, fa_on, fb_on);
+        T *as = sA + (s % ST) * ASZ, *bs = sB + (s % ST) * BSZ;
+        if (fa_on) { fa.template issue<0>(as); fa.template issue<1>(as); fa.template issue<2>(as); fa.template issue<3>(as); }
+        if (fb_on) { fb.template issue<0>(bs); fb.template issue<1>(bs); fb.template issue<2>(bs); fb.template issue<3>(bs); }
+        fa.advance(); fb.advance();
+        cp_async_commit();
+    }
 
     for (int kt = 0; kt < nkt; ++kt) {
         cp_async_wait<ST - 2>();
         __syncthreads();
-        issue(kt + ST - 1);
+        bool fa_on, fb_on;
+        issue_generic(kt + ST - 1, fa_on, fb_on);
+        T *as_n = sA + ((kt + ST - 1) % ST) * ASZ, *bs_n = sB + ((kt + ST - 1) % ST) * BSZ;
         const T *a_s = sA + (kt % ST) * ASZ;
         const T *b_s = sB + (kt % ST) * BSZ;
         const double *s_s = sS + (kt % ST) * BK;
+        const T *a_p = a_s + (wm + lr) * a_sx + lc * a_sk;
+        const T *b_p = b_s + (wn + lr) * b_sx + lc * b_sk;
 #pragma unroll
-        for (int kk = 0; kk < BK; kk += 4) {
+        for (int kq = 0; kq < BK / 4; ++kq) {
+            const int kk = kq * 4;
+            // one quarter of the next tile's copies per k-step
+            if (fa_on) {
+                if (kq == 0) fa.template issue<0>(as_n); else if (kq == 1) fa.template issue<1>(as_n);
+                else if (kq == 2) fa.template issue<2>(as_n); else fa.template issue<3>(as_n);
+            }
+            if (fb_on) {
+                if (kq == 0) fb.template issue<0>(bs_n); else if (kq == 1) fb.template issue<1>(bs_n);
+                else if (kq == 2) fb.template issue<2>(bs_n); else fb.template issue<3>(bs_n);
+            }
             if constexpr (!CPLX) {
                 double af[MI], bf[NI];
 #pragma unroll
-                for (int i = 0; i < MI; ++i) af[i] = ((const double *)a_s)[(wm + i * 8 + lr) * a_sx + (kk + lc) * a_sk];
+                for (int i = 0; i < MI; ++i) af[i] = a_p[i * 8 * a_sx + kk * a_sk];
 #pragma unroll
-                for (int j = 0; j < NI; ++j) bf[j] = ((const double *)b_s)[(wn + j * 8 + lr) * b_sx + (kk + lc) * b_sk];
-                if (scaleK) {
-                    double sc = s_s[kk + lc];
+                for (int j = 0; j < NI; ++j) bf[j] = b_p[j * 8 * b_sx + kk * b_sk];
+                if constexpr (SCALE) {
+                    const double sc = s_s[kk + lc];
 #pragma unroll
                     for (int i = 0; i < MI; ++i) af[i] *= sc;
                 }
@@ -212,16 +318,16 @@ gemm_kernel(const GemmDesc hd, const GemmDesc *__restrict__ dd) {
                 double ar[MI], ai[MI], nai[MI], br[NI], bi[NI];
 #pragma unroll
                 for (int i = 0; i < MI; ++i) {
-                    cplx v = ((const cplx *)a_s)[(wm + i * 8 + lr) * a_sx + (kk + lc) * a_sk];
+                    const cplx v = a_p[i * 8 * a_sx + kk * a_sk];
                     ar[i] = v.x; ai[i] = conjA ? -v.y : v.y;
                 }
 #pragma unroll
                 for (int j = 0; j < NI; ++j) {
-                    cplx v = ((const cplx *)b_s)[(wn + j * 8 + lr) * b_sx + (kk + lc) * b_sk];
+                    const cplx v = b_p[j * 8 * b_sx + kk * b_sk];
                     br[j] = v.x; bi[j] = conjB ? -v.y : v.y;
                 }
-                if (scaleK) {
-                    double sc = s_s[kk + lc];
+                if constexpr (SCALE) {
+                    const double sc = s_s[kk + lc];
 #pragma unroll
                     for (int i = 0; i < MI; ++i) { ar[i] *= sc; ai[i] *= sc; }
                 }
@@ -238,41 +344,30 @@ gemm_kernel(const GemmDesc hd, const GemmDesc *__restrict__ dd) {
                     }
             }
         }
+        fa.advance(); fb.advance();
+        cp_async_commit();
     }
     cp_async_wait<0>();
 
-    // epilogue: lane holds C[row = lr][cols 2*lc, 2*lc+1] of each 8x8 block.  With beta != 0 all old values of one
-    // row block are loaded first (independent loads in flight together), then combined and stored: a load -> store ->
-    // load chain would serialise on memory latency.
-    const double alpha = d.alpha, beta = d.beta;
+    // epilogue: lane holds C[row = lr][cols 2*lc, 2*lc+1] of each 8x8 block
 #pragma unroll
     for (int i = 0; i < MI; ++i) {
         const int gi = m0 + wm + i * 8 + lr;
         if (gi >= M) continue;
-        T old[NI][2];
-        if (beta != 0.0) {
-#pragma unroll
-            for (int j = 0; j < NI; ++j)
-#pragma unroll
-                for (int q = 0; q < 2; ++q) {
-                    const int gj = n0 + wn + j * 8 + 2 * lc + q;
-                    if (gj < N) old[j][q] = C[gi + (long)gj * d.ldc];
-                }
-        }
 #pragma unroll
         for (int j = 0; j < NI; ++j) {
 #pragma unroll
             for (int q = 0; q < 2; ++q) {
                 const int gj = n0 + wn + j * 8 + 2 * lc + q;
                 if (gj >= N) continue;
-                T *p = C + gi + (long)gj * d.ldc;
+                T *p = C + gi + (long)gj * ldc;
                 if constexpr (!CPLX) {
                     double v = alpha * acc[i][j][q];
-                    if (beta != 0.0) v += beta * old[j][q];
+                    if (beta != 0.0 && !preload) v += beta * *p;
                     *p = v;
                 } else {
                     cplx v; v.x = alpha * acc[i][j][q]; v.y = alpha * acc[i][j][2 + q];
-                    if (beta != 0.0) { v.x += beta * old[j][q].x; v.y += beta * old[j][q].y; }
+                    if (beta != 0.0 && !preload) { const cplx o = *p; v.x += beta * o.x; v.y += beta * o.y; }
                     *p = v;
                 }
             }
@@ -286,31 +381,53 @@ template <bool CPLX> static size_t gemm_smem_bytes() {
     return G::STAGES * (a + b) * sizeof(typename G::T) + G::STAGES * G::BK * sizeof(double);
 }
 
-template <bool CPLX>
-static int launch_impl(const GemmDesc *hd, const GemmDesc *dd, int ngroups, int max_m, int max_n, int batch,
-                       cudaStream_t st) {
+template <bool CPLX, bool AXC, bool BXC, bool SCALE>
+static int launch_variant(const GemmDesc *hd, const GemmDesc *dd, int ngroups, int max_m, int max_n, int batch,
+                          cudaStream_t st) {
     typedef Cfg<CPLX> G;
     static bool attr_set = false;
     size_t smem = gemm_smem_bytes<CPLX>();
     if (!attr_set) {
-        NAO_CUDA_CHECK(cudaFuncSetAttribute(gemm_kernel<CPLX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        NAO_CUDA_CHECK(cudaFuncSetAttribute(gemm_kernel<CPLX, AXC, BXC, SCALE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_set = true;
     }
-    if (max_m <= 0 || max_n <= 0 || batch <= 0 || ngroups <= 0) return NAO_OK;
     long tiles = (long)ceil_div(max_m, G::BM) * ceil_div(max_n, G::BN);
     dim3 grid((unsigned)tiles, (unsigned)batch, (unsigned)ngroups);
     GemmDesc dummy = hd ? *hd : gemm_desc(0, 0, 0, 0, 0, 0, nullptr, 0, nullptr, 0, 0, nullptr, 0);
-    gemm_kernel<CPLX><<<grid, GEMM_THREADS, smem, st>>>(dummy, dd);
+    const double flops = hd ? (CPLX ? 8.0 : 2.0) * hd->m * (double)hd->n * hd->k * (hd->cmode == 1 ? 0.5 : 1.0) *
+                                  (hd->maskA != MASK_NONE || hd->maskB != MASK_NONE ? 0.5 : 1.0) * batch /
+                                  (hd->ksplit > 1 ? hd->ksplit : 1)
+                            : 0.0;
+    const int pk = prof_kernel_begin(1, flops, st);
+    gemm_kernel<CPLX, AXC, BXC, SCALE><<<grid, GEMM_THREADS, smem, st>>>(dummy, dd);
+    prof_kernel_end(1, pk, st);
     NAO_LAUNCHED();
     NAO_CUDA_CHECK(cudaGetLastError());
     return NAO_OK;
 }
 
+// the operand layouts (and the presence of scale factors) select the kernel instantiation; for grouped launches every
+// descriptor must share them
+template <bool CPLX>
+static int launch_impl(const GemmDesc *hd, const GemmDesc *dd, int ngroups, int max_m, int max_n, int batch, int opA,
+                       int opB, bool scale, cudaStream_t st) {
+    if (max_m <= 0 || max_n <= 0 || batch <= 0 || ngroups <= 0) return NAO_OK;
+    const bool axc = (opA == OP_N), bxc = (opB != OP_N);
+    if (scale) {
+        if (!(axc && bxc)) return NAO_ERR_UNSUPPORTED;
+        return launch_variant<CPLX, true, true, true>(hd, dd, ngroups, max_m, max_n, batch, st);
+    }
+    if (axc) return bxc ? launch_variant<CPLX, true, true, false>(hd, dd, ngroups, max_m, max_n, batch, st)
+                        : launch_variant<CPLX, true, false, false>(hd, dd, ngroups, max_m, max_n, batch, st);
+    return bxc ? launch_variant<CPLX, false, true, false>(hd, dd, ngroups, max_m, max_n, batch, st)
+               : launch_variant<CPLX, false, false, false>(hd, dd, ngroups, max_m, max_n, batch, st);
+}
+
 int gemm_launch(int dtype, const GemmDesc &d, int batch, cudaStream_t st) {
     if (d.m <= 0 || d.n <= 0) return NAO_OK;
     const int by = batch * (d.ksplit > 1 ? d.ksplit : 1);
-    return dtype == NAO_COMPLEX ? launch_impl<true>(&d, nullptr, 1, d.m, d.n, by, st)
-                                : launch_impl<false>(&d, nullptr, 1, d.m, d.n, by, st);
+    return dtype == NAO_COMPLEX ? launch_impl<true>(&d, nullptr, 1, d.m, d.n, by, d.opA, d.opB, d.scaleK != nullptr, st)
+                                : launch_impl<false>(&d, nullptr, 1, d.m, d.n, by, d.opA, d.opB, d.scaleK != nullptr, st);
 }
 
 template <class T>
@@ -354,9 +471,10 @@ int gemm_splitk(int dtype, const GemmDesc &d0, int batch, int ksplit, void *part
     NAO_CUDA_CHECK(cudaGetLastError());
     return NAO_OK;
 }
-int gemm_launch_grouped(int dtype, const GemmDesc *dd, int ngroups, int max_m, int max_n, int batch, cudaStream_t st) {
-    return dtype == NAO_COMPLEX ? launch_impl<true>(nullptr, dd, ngroups, max_m, max_n, batch, st)
-                                : launch_impl<false>(nullptr, dd, ngroups, max_m, max_n, batch, st);
+int gemm_launch_grouped(int dtype, const GemmDesc *dd, int ngroups, int max_m, int max_n, int batch, int opA, int opB,
+                        bool scale, cudaStream_t st) {
+    return dtype == NAO_COMPLEX ? launch_impl<true>(nullptr, dd, ngroups, max_m, max_n, batch, opA, opB, scale, st)
+                                : launch_impl<false>(nullptr, dd, ngroups, max_m, max_n, batch, opA, opB, scale, st);
 }
 
 }  // namespace nao

@@ -74,12 +74,13 @@ static inline GemmDesc gemm_desc(int opA, int opB, int m, int n, int k, double a
 // One problem described on the host (passed by value), `batch` items via the strides in the descriptor.
 int gemm_launch(int dtype, const GemmDesc &d, int batch, cudaStream_t st);
 // `ngroups` problems described by descriptors in DEVICE memory (their m,n,k may have been written by a kernel);
-// max_m/max_n bound the grid.  Each group runs `batch` items.
+// max_m/max_n bound the grid.  Each group runs `batch` items.  opA/opB/scale (shared by every descriptor) select the
+// kernel instantiation.
 // Split-K product for short-and-wide outputs (m, n small, k long): `ksplit` slices write partial products into
 // `partial` (batch * ksplit * m * n elements), then C <- alpha * (sum of slices, fixed order) + beta * C.
 int gemm_splitk(int dtype, const GemmDesc &d, int batch, int ksplit, void *partial, cudaStream_t st);
-int gemm_launch_grouped(int dtype, const GemmDesc *d_descs, int ngroups, int max_m, int max_n, int batch,
-                        cudaStream_t st);
+int gemm_launch_grouped(int dtype, const GemmDesc *d_descs, int ngroups, int max_m, int max_n, int batch, int opA,
+                        int opB, bool scale, cudaStream_t st);
 
 // ---------------------------------------------------------------------------------------------------------
 // element-wise helpers (util.cu)

@@ -465,7 +465,7 @@ int stedc(int n, int batch, double *d, double *e, double *evals, double *Qout, l
         NAO_LAUNCHED();
         dc_vectors_kernel<<<dim3(Nmax, nn, batch), 128, 0, st>>>(w.b, nodes, p.maxnodes);
         NAO_LAUNCHED();
-        if (int rc = gemm_launch_grouped(NAO_REAL, w.b.desc, batch * nn * 2, hmax, Nmax, 1, st)) return rc;
+        if (int rc = gemm_launch_grouped(NAO_REAL, w.b.desc, batch * nn * 2, hmax, Nmax, 1, OP_N, OP_N, false, st)) return rc;
         dc_finish_kernel<<<dim3(nn, batch), 256, 0, st>>>(w.b, nodes, p.maxnodes);
         NAO_LAUNCHED();
     }

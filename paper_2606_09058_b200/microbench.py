@@ -1,0 +1,125 @@
+"""Per-kernel micro-benchmarks of libnao.so building blocks (CUDA events, warm-up, L2 flush between repetitions).
+
+    python -m paper_2606_09058_b200.microbench gemm [--m M --n N --k K] [--complex] [--opa 0|1|2] [--opb 0|1|2]
+                                                    [--beta B] [--lower] [--cublas] [--reps R]
+    python -m paper_2606_09058_b200.microbench heev [--n N] [--batch B] [--complex] [--two-stage|--one-stage]
+
+`--cublas` adds torch.matmul on the same operands as a SIDE comparison (never used by the product path).
+Prints one JSON line per measurement.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+
+import torch
+
+from . import binding as B
+
+FP64_DMMA_PEAK_TFLOPS = 148 * 128 * 1.965e9 / 1e12
+
+
+def _flush_l2(buf):
+    buf.zero_()
+
+
+def _time(fn, reps, flush):
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for _ in range(3):
+        fn()
+    times = []
+    for _ in range(reps):
+        _flush_l2(flush)
+        ev0.record()
+        fn()
+        ev1.record()
+        torch.cuda.synchronize()
+        times.append(ev0.elapsed_time(ev1))
+    times.sort()
+    return times[len(times) // 2]
+
+
+def bench_gemm(args):
+    dev = torch.device("cuda:0")
+    m, n, k = args.m, args.n, args.k
+    dt = torch.complex128 if args.complex else torch.float64
+    g = torch.Generator(device=dev)
+    g.manual_seed(0)
+
+    def rnd(cols, rows):
+        x = torch.randn(1, cols, rows, dtype=torch.float64, device=dev, generator=g)
+        if args.complex:
+            x = torch.complex(x, torch.randn(1, cols, rows, dtype=torch.float64, device=dev, generator=g))
+        return x
+
+    # column-major items: shape (batch, cols, rows)
+    A = rnd(k, m) if args.opa == 0 else rnd(m, k)
+    Bm = rnd(n, k) if args.opb == 0 else rnd(k, n)
+    C = torch.zeros(1, n, m, dtype=dt, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    ms = _time(lambda: B.gemm(A, Bm, args.opa, args.opb, 1.0, args.beta, C=C, lower_only=args.lower), args.reps, flush)
+    flops = (8.0 if args.complex else 2.0) * m * n * k * (0.5 if args.lower else 1.0)
+    out = {"kernel": "gemm_kernel", "m": m, "n": n, "k": k, "complex": args.complex, "opA": args.opa, "opB": args.opb,
+           "beta": args.beta, "lower_only": args.lower, "ms": ms, "tflops": flops / ms / 1e9,
+           "frac_of_dmma_peak": flops / ms / 1e9 / FP64_DMMA_PEAK_TFLOPS}
+    if args.cublas:
+        At = A[0].T if args.opa == 0 else (A[0] if args.opa == 1 else A[0].conj())   # logical op(A) (m x k) as a view
+        Bt = Bm[0].T if args.opb == 0 else (Bm[0] if args.opb == 1 else Bm[0].conj())
+        ms_c = _time(lambda: torch.matmul(At, Bt), args.reps, flush)
+        out["cublas_ms"] = ms_c
+        out["cublas_tflops"] = (8.0 if args.complex else 2.0) * m * n * k / ms_c / 1e9
+    print(json.dumps(out))
+
+
+def bench_heev(args):
+    dev = torch.device("cuda:0")
+    n, batch = args.n, args.batch
+    g = torch.Generator(device=dev)
+    g.manual_seed(1)
+    A = torch.randn(batch, n, n, dtype=torch.float64, device=dev, generator=g)
+    if args.complex:
+        A = torch.complex(A, torch.randn(batch, n, n, dtype=torch.float64, device=dev, generator=g))
+    A = A + A.mH
+    flags = B.NAO_TRD_TWO_STAGE if args.two_stage else (B.NAO_TRD_ONE_STAGE if args.one_stage else 0)
+    res = {}
+    for it in range(max(2, args.reps)):
+        B.profile_enable(True)
+        E, Z, info = B.heev(A.clone(), flags=flags)
+        torch.cuda.synchronize()
+        res = B.profile_read()
+        kp = [B.profile_kernel(s) for s in range(2)]
+        B.profile_enable(False)
+    Zm = Z[0].T                                     # column-major item -> logical matrix
+    Am = A[0].T
+    r = (Am @ Zm - Zm * E[0][None, :]).abs().max().item()
+    o = (Zm.mH @ Zm - torch.eye(n, dtype=Zm.dtype, device=dev)).abs().max().item()
+    print(json.dumps({"kernel": "heev", "n": n, "batch": batch, "complex": args.complex, "flags": flags,
+                      "phases_ms": {k: round(v, 3) for k, v in res.items()}, "kernels": kp,
+                      "residual_max": r, "orth_max": o, "info": info.tolist()}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("what", choices=["gemm", "heev"])
+    ap.add_argument("--m", type=int, default=6656)
+    ap.add_argument("--n", type=int, default=6656)
+    ap.add_argument("--k", type=int, default=6656)
+    ap.add_argument("--batch", type=int, default=1)
+    ap.add_argument("--complex", action="store_true")
+    ap.add_argument("--opa", type=int, default=0)
+    ap.add_argument("--opb", type=int, default=0)
+    ap.add_argument("--beta", type=float, default=0.0)
+    ap.add_argument("--lower", action="store_true")
+    ap.add_argument("--cublas", action="store_true")
+    ap.add_argument("--two-stage", action="store_true")
+    ap.add_argument("--one-stage", action="store_true")
+    ap.add_argument("--reps", type=int, default=5)
+    args = ap.parse_args()
+    if not torch.cuda.is_available():
+        raise SystemExit("microbench needs a CUDA device: the product has no CPU path")
+    B.lib()
+    (bench_gemm if args.what == "gemm" else bench_heev)(args)
+
+
+if __name__ == "__main__":
+    main()

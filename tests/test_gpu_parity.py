@@ -207,7 +207,7 @@ def test_gemm_core_all_ops(nao, cplx):
     def op(X, o):
         return X if o == 0 else (np.swapaxes(X, -1, -2) if o == 1 else np.swapaxes(X.conj(), -1, -2))
 
-    for (m, n, k) in [(1, 1, 1), (130, 67, 45), (257, 300, 129)]:
+    for (m, n, k) in [(1, 1, 1), (130, 67, 45), (257, 300, 129), (384, 256, 160), (391, 262, 83)]:
         for oa in (0, 1, 2):
             for ob in (0, 1, 2):
                 A = rnd(m, k) if oa == 0 else rnd(k, m)
