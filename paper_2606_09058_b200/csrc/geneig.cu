@@ -13,28 +13,50 @@
 namespace nao {
 
 // ----------------------------------------------------------------------------------------------------- heev
-struct HeevPlan { size_t d, e, tau, qt, sub, bytes; size_t sub_bytes; };
-static HeevPlan heev_plan(int dtype, int n, int batch) {
+struct HeevPlan { size_t d, e, tau, qt, sub, v2, tau2, sub2, bytes; bool two_stage; };
+static const int TWO_STAGE_MIN_N = 1 << 30;      // default switch-over size (flags force either path)
+static bool use_two_stage(int dtype, int n, int batch, unsigned flags) {
+    if (flags & NAO_TRD_ONE_STAGE) return false;
+    if (!he2hb_supported(dtype, n, batch)) return false;
+    if (flags & NAO_TRD_TWO_STAGE) return true;
+    return n >= TWO_STAGE_MIN_N;
+}
+static HeevPlan heev_plan(int dtype, int n, int batch, unsigned flags) {
     HeevPlan p; size_t off = 0;
     auto take = [&](size_t b) { size_t o = off; off += align_up(b); return o; };
+    p.two_stage = use_two_stage(dtype, n, batch, flags);
     p.d = take((size_t)batch * n * 8); p.e = take((size_t)batch * n * 8); p.tau = take((size_t)batch * n * esize(dtype));
     p.qt = take(dtype == NAO_COMPLEX ? (size_t)batch * n * n * 8 : 0);
-    p.sub_bytes = std::max(hetrd_workspace(dtype, n, batch), std::max(stedc_workspace(n, batch), ormtr_workspace(dtype, n, batch)));
-    p.sub = take(p.sub_bytes);
+    p.v2 = p.tau2 = p.sub2 = 0;
+    if (p.two_stage) {
+        p.v2 = take((size_t)batch * n * n * esize(dtype));
+        p.tau2 = take((size_t)batch * hb2st_nk(n) * n * esize(dtype));
+        const size_t s2 = std::max(std::max(he2hb_workspace(dtype, n, batch), hb2st_workspace(dtype, n, batch)),
+                                   std::max(std::max(stedc_workspace(n, batch), q2_workspace(dtype, n, batch)),
+                                            ormtr_workspace(dtype, n, batch)));
+        p.sub = take(s2);
+    } else {
+        p.sub = take(std::max(hetrd_workspace(dtype, n, batch), std::max(stedc_workspace(n, batch), ormtr_workspace(dtype, n, batch))));
+    }
     p.bytes = off;
     return p;
 }
 
 static int heev(int dtype, int n, int batch, unsigned flags, void *A, long lda, long sA, double *E, void *Z, long ldz,
                 long sZ, void *work, int *d_info, cudaStream_t st) {
-    (void)flags;
-    HeevPlan p = heev_plan(dtype, n, batch);
+    HeevPlan p = heev_plan(dtype, n, batch, flags);
     char *w = (char *)work;
     double *d = (double *)(w + p.d), *e = (double *)(w + p.e);
     void *tau = w + p.tau, *sub = w + p.sub;
+    void *V2 = w + p.v2, *tau2 = w + p.tau2;
     int rc;
     prof_mark(2, st);
-    if ((rc = hetrd(dtype, n, batch, A, lda, sA, d, e, tau, sub, st))) return rc;
+    if (p.two_stage) {
+        if ((rc = he2hb(dtype, n, batch, A, lda, sA, tau, sub, st))) return rc;
+        if ((rc = hb2st(dtype, n, batch, A, lda, sA, d, e, V2, n, (long)n * n, tau2, sub, st))) return rc;
+    } else {
+        if ((rc = hetrd(dtype, n, batch, A, lda, sA, d, e, tau, sub, st))) return rc;
+    }
     prof_mark(3, st);
     if (dtype == NAO_COMPLEX) {
         double *qt = (double *)(w + p.qt);
@@ -44,7 +66,12 @@ static int heev(int dtype, int n, int batch, unsigned flags, void *A, long lda, 
         if ((rc = stedc(n, batch, d, e, E, (double *)Z, ldz, sZ, sub, d_info, st))) return rc;
     }
     prof_mark(4, st);
-    rc = ormtr(dtype, n, n, batch, A, lda, sA, tau, Z, ldz, sZ, sub, st);
+    if (p.two_stage) {
+        if ((rc = q2_apply(dtype, n, n, batch, V2, n, (long)n * n, tau2, Z, ldz, sZ, sub, st))) return rc;
+        rc = ormtr(dtype, n, n, batch, TRD2_B, A, lda, sA, tau, Z, ldz, sZ, sub, st);
+    } else {
+        rc = ormtr(dtype, n, n, batch, 1, A, lda, sA, tau, Z, ldz, sZ, sub, st);
+    }
     prof_mark(5, st);
     return rc;
 }
@@ -60,7 +87,7 @@ static GePlan ge_plan(int n, int batch, int dtype, unsigned flags, bool shared_S
     p.Wc = take(nc ? (size_t)p.nitemsS * p.nS * p.nS * 16 : 0);
     p.A = take((size_t)batch * n * n * esize(dtype));
     p.X = take((size_t)batch * n * n * esize(dtype));
-    p.heev = take(heev_plan(dtype, n, batch).bytes);
+    p.heev = take(heev_plan(dtype, n, batch, flags).bytes);
     p.bytes = off;
     return p;
 }
@@ -68,12 +95,11 @@ static GePlan ge_plan(int n, int batch, int dtype, unsigned flags, bool shared_S
 }  // namespace nao
 
 NAO_EXPORT int nao_heev_workspace(int n, int batch, int dtype, unsigned flags, size_t *bytes) {
-    (void)flags;
     if (n < 1) return -1;
     if (batch < 1) return -2;
     if (dtype != NAO_REAL && dtype != NAO_COMPLEX) return -3;
     if (!bytes) return -5;
-    *bytes = nao::heev_plan(dtype, n, batch).bytes;
+    *bytes = nao::heev_plan(dtype, n, batch, flags).bytes;
     return NAO_OK;
 }
 
@@ -91,7 +117,7 @@ NAO_EXPORT int nao_heev(int n, int batch, int dtype, unsigned flags, void *dA, l
     if (ldz < n) return -10;
     if (batch > 1 && strideZ < ldz * (long)n) return -11;
     if (!dwork) return -12;
-    if (work_bytes < heev_plan(dtype, n, batch).bytes) return NAO_ERR_WORKSPACE;
+    if (work_bytes < heev_plan(dtype, n, batch, flags).bytes) return NAO_ERR_WORKSPACE;
     if (!d_info) return -14;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (cudaMemsetAsync(d_info, 0, sizeof(int) * batch, st) != cudaSuccess) return NAO_ERR_CUDA;

@@ -115,8 +115,31 @@ int hetrd(int dtype, int n, int batch, void *A, long lda, long sA, double *d, do
           cudaStream_t st);
 // Z <- Q_house * Z where Q_house = H_0 H_1 ... H_{n-2} from hetrd (Z n x ncols)
 size_t ormtr_workspace(int dtype, int n, int batch);
-int ormtr(int dtype, int n, int ncols, int batch, const void *A, long lda, long sA, const void *tau, void *Z,
+// shift = 1: reflectors of hetrd (v_j = A[j+1:, j]);  shift = b: reflectors of he2hb (v_j = A[j+b:, j])
+int ormtr(int dtype, int n, int ncols, int batch, int shift, const void *A, long lda, long sA, const void *tau, void *Z,
           long ldz, long sZ, void *work, cudaStream_t st);
+// ormtr.cu helpers shared with trd2.cu: explicit V block and the T factor from G = V^H V and tau
+int build_v(int dtype, int n, int jb, int kb, int shift, const void *A, long lda, long sA, void *V, long ldv, long sV, int batch,
+            cudaStream_t st);
+int larft(int dtype, int kb, const void *G, long ldg, long sG, const void *tau, long sTau, void *Tm, long sT, int batch,
+          cudaStream_t st);   // Tm is kb x kb dense (ld = kb), kb <= 128
+
+// two-stage tridiagonalisation (trd2.cu, trd2_chase.cu, trd2_back.cu), bandwidth TRD2_B
+static const int TRD2_B = 64;
+// dense -> band: band in the lower part of A (0 <= i-j <= b), reflectors below it (v_j = A[j+b:, j], unit implicit), tau[n]
+size_t he2hb_workspace(int dtype, int n, int batch);
+bool he2hb_supported(int dtype, int n, int batch);
+int he2hb(int dtype, int n, int batch, void *A, long lda, long sA, void *tau, void *work, cudaStream_t st);
+// band -> tridiagonal by bulge chasing: reads the band from A, writes d[n], e[n] (real), reflectors V2 (n x n, ldv),
+// tau2 (hb2st_nk(n) x n)
+size_t hb2st_workspace(int dtype, int n, int batch);
+int hb2st_nk(int n);
+int hb2st(int dtype, int n, int batch, const void *A, long lda, long sA, double *d, double *e, void *V2, long ldv, long sV2,
+          void *tau2, void *work, cudaStream_t st);
+// Z <- Q2 Z (Z n x ncols) with the reflectors of hb2st
+size_t q2_workspace(int dtype, int n, int batch);
+int q2_apply(int dtype, int n, int ncols, int batch, const void *V2, long ldv, long sV2, const void *tau2, void *Z, long ldz,
+             long sZ, void *work, cudaStream_t st);
 
 // stedc.cu
 size_t stedc_workspace(int n, int batch);

@@ -7,7 +7,8 @@ namespace nao {
 
 
 // ----------------------------------------------------------------------------------------------------------------
-// Back-transformation: Z <- Q Z, Q = H(0) H(1) ... H(n-2), H(j) = I - tau_j v_j v_j^H, v_j = A[j+1:, j] (unit first
+// Back-transformation: Z <- Q Z, Q = H(0) H(1) ... H(n-1-shift), H(j) = I - tau_j v_j v_j^H, v_j = A[j+shift:, j] (shift = 1:
+// one-stage hetrd; shift = b: dense-to-band he2hb) (unit first
 // element stored explicitly by hetrd).  Blocks of KB reflectors, last block first:
 //   Vb (explicit, zeros above the unit diagonal), G = Vb^H Vb, T by the xLARFT recurrence, then three GEMMs
 //   X = Vb^H Z ; X <- T X ; Z -= Vb X.
@@ -15,17 +16,17 @@ namespace nao {
 static const int ORM_KB = 128;
 
 template <class T>
-__global__ void build_v_kernel(int n, int jb, int kb, const T *A, long lda, long sA, T *V, long ldv, long sV) {
-    // V (m x kb), m = n - jb - 1, row r <-> global row jb+1+r; column k <-> reflector jb+k whose unit sits at r == k
+__global__ void build_v_kernel(int n, int jb, int kb, int shift, const T *A, long lda, long sA, T *V, long ldv, long sV) {
+    // V (m x kb), m = n - jb - shift, row r <-> global row jb+shift+r; column k <-> reflector jb+k whose unit sits at r == k
     A += (long)blockIdx.z * sA; V += (long)blockIdx.z * sV;
-    const int m = n - jb - 1;
+    const int m = n - jb - shift;
     int r = blockIdx.x * blockDim.x + threadIdx.x;
     if (r >= m) return;
     for (int k = blockIdx.y; k < kb; k += gridDim.y) {
         T v;
         if (r < k) v = Ops<T>::zero();
         else if (r == k) v = Ops<T>::one();
-        else v = A[(jb + 1 + r) + (long)(jb + k) * lda];
+        else v = A[(jb + shift + r) + (long)(jb + k) * lda];
         V[r + (long)k * ldv] = v;
     }
 }
@@ -58,6 +59,44 @@ __global__ void __launch_bounds__(256) larft_kernel(int kb, const T *G, long ldg
     }
 }
 
+template <class T> static int larft_attr() {
+    static bool attr = false;
+    if (!attr) {
+        const size_t smem = (size_t)ORM_KB * (ORM_KB + 1) / 2 * sizeof(T);
+        NAO_CUDA_CHECK(cudaFuncSetAttribute(larft_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr = true;
+    }
+    return NAO_OK;
+}
+
+int build_v(int dtype, int n, int jb, int kb, int shift, const void *A, long lda, long sA, void *V, long ldv, long sV, int batch,
+            cudaStream_t st) {
+    const int m = n - jb - shift;
+    if (m <= 0 || kb <= 0) return NAO_OK;
+    dim3 grid(ceil_div(m, 256), kb, batch);
+    if (dtype == NAO_COMPLEX) build_v_kernel<cplx><<<grid, 256, 0, st>>>(n, jb, kb, shift, (const cplx *)A, lda, sA, (cplx *)V, ldv, sV);
+    else build_v_kernel<double><<<grid, 256, 0, st>>>(n, jb, kb, shift, (const double *)A, lda, sA, (double *)V, ldv, sV);
+    NAO_LAUNCHED();
+    NAO_CUDA_CHECK(cudaGetLastError());
+    return NAO_OK;
+}
+
+int larft(int dtype, int kb, const void *G, long ldg, long sG, const void *tau, long sTau, void *Tm, long sT, int batch,
+          cudaStream_t st) {
+    if (kb <= 0) return NAO_OK;
+    if (kb > ORM_KB) return NAO_ERR_UNSUPPORTED;
+    if (dtype == NAO_COMPLEX) {
+        if (int rc = larft_attr<cplx>()) return rc;
+        larft_kernel<cplx><<<batch, 256, (size_t)kb * (kb + 1) / 2 * sizeof(cplx), st>>>(kb, (const cplx *)G, ldg, sG, (const cplx *)tau, sTau, (cplx *)Tm, sT);
+    } else {
+        if (int rc = larft_attr<double>()) return rc;
+        larft_kernel<double><<<batch, 256, (size_t)kb * (kb + 1) / 2 * sizeof(double), st>>>(kb, (const double *)G, ldg, sG, (const double *)tau, sTau, (double *)Tm, sT);
+    }
+    NAO_LAUNCHED();
+    NAO_CUDA_CHECK(cudaGetLastError());
+    return NAO_OK;
+}
+
 struct OrmWork { void *V, *G, *T, *X, *X2, *P; size_t bytes; int ksG, ksX; };
 static OrmWork orm_plan(int dtype, int n, int ncols, int batch, void *work) {
     OrmWork w; const size_t es = esize(dtype);
@@ -79,11 +118,11 @@ static OrmWork orm_plan(int dtype, int n, int ncols, int batch, void *work) {
 size_t ormtr_workspace(int dtype, int n, int batch) { return orm_plan(dtype, n, n, batch, nullptr).bytes; }
 
 template <class T>
-static int ormtr_impl(int dtype, int n, int ncols, int batch, const T *A, long lda, long sA, const T *tau, T *Z, long ldz,
-                      long sZ, void *work, cudaStream_t st) {
-    if (n < 2) return NAO_OK;
+static int ormtr_impl(int dtype, int n, int ncols, int batch, int shift, const T *A, long lda, long sA, const T *tau, T *Z,
+                      long ldz, long sZ, void *work, cudaStream_t st) {
+    if (n < shift + 1) return NAO_OK;
     OrmWork w = orm_plan(dtype, n, ncols, batch, work);
-    const int nref = n - 1;
+    const int nref = n - shift;
     static bool attr = false;
     const size_t larft_smem = (size_t)ORM_KB * (ORM_KB + 1) / 2 * sizeof(T);
     if (!attr) {
@@ -92,9 +131,9 @@ static int ormtr_impl(int dtype, int n, int ncols, int batch, const T *A, long l
     }
     const int nblocks = ceil_div(nref, ORM_KB);
     for (int blk = nblocks - 1; blk >= 0; --blk) {
-        const int jb = blk * ORM_KB, kb = std::min(ORM_KB, nref - jb), m = n - jb - 1;
+        const int jb = blk * ORM_KB, kb = std::min(ORM_KB, nref - jb), m = n - jb - shift;
         const long ldv = m, sV = (long)n * ORM_KB;
-        build_v_kernel<T><<<dim3(ceil_div(m, 256), kb, batch), 256, 0, st>>>(n, jb, kb, A, lda, sA, (T *)w.V, ldv, sV);
+        build_v_kernel<T><<<dim3(ceil_div(m, 256), kb, batch), 256, 0, st>>>(n, jb, kb, shift, A, lda, sA, (T *)w.V, ldv, sV);
         NAO_LAUNCHED();
         // G = V^H V  (kb x kb, k = m: split-K)
         GemmDesc g = gemm_desc(OP_C, OP_N, kb, kb, m, 1.0, w.V, ldv, w.V, ldv, 0.0, w.G, kb);
@@ -103,7 +142,7 @@ static int ormtr_impl(int dtype, int n, int ncols, int batch, const T *A, long l
         larft_kernel<T><<<batch, 256, larft_smem, st>>>(kb, (const T *)w.G, kb, ORM_KB * ORM_KB, tau + jb, n, (T *)w.T, ORM_KB * ORM_KB);
         NAO_LAUNCHED();
         // X = V^H Z[jb+1:, :]  (kb x ncols, k = m: split-K)
-        GemmDesc x = gemm_desc(OP_C, OP_N, kb, ncols, m, 1.0, w.V, ldv, Z + jb + 1, ldz, 0.0, w.X, kb);
+        GemmDesc x = gemm_desc(OP_C, OP_N, kb, ncols, m, 1.0, w.V, ldv, Z + jb + shift, ldz, 0.0, w.X, kb);
         x.sA = sV; x.sB = sZ; x.sC = (long)ORM_KB * ncols;
         if (int rc = gemm_splitk(dtype, x, batch, std::min(w.ksX, ceil_div(m, 512)), w.P, st)) return rc;
         // X2 = T X
@@ -111,7 +150,7 @@ static int ormtr_impl(int dtype, int n, int ncols, int batch, const T *A, long l
         t.sA = ORM_KB * ORM_KB; t.sB = (long)ORM_KB * ncols; t.sC = (long)ORM_KB * ncols; t.maskA = MASK_UPPER;
         if (int rc = gemm_launch(dtype, t, batch, st)) return rc;
         // Z[jb+1:, :] -= V X2
-        GemmDesc u = gemm_desc(OP_N, OP_N, m, ncols, kb, -1.0, w.V, ldv, w.X2, kb, 1.0, Z + jb + 1, ldz);
+        GemmDesc u = gemm_desc(OP_N, OP_N, m, ncols, kb, -1.0, w.V, ldv, w.X2, kb, 1.0, Z + jb + shift, ldz);
         u.sA = sV; u.sB = (long)ORM_KB * ncols; u.sC = sZ;
         if (int rc = gemm_launch(dtype, u, batch, st)) return rc;
     }
@@ -119,11 +158,11 @@ static int ormtr_impl(int dtype, int n, int ncols, int batch, const T *A, long l
     return NAO_OK;
 }
 
-int ormtr(int dtype, int n, int ncols, int batch, const void *A, long lda, long sA, const void *tau, void *Z, long ldz,
-          long sZ, void *work, cudaStream_t st) {
+int ormtr(int dtype, int n, int ncols, int batch, int shift, const void *A, long lda, long sA, const void *tau, void *Z,
+          long ldz, long sZ, void *work, cudaStream_t st) {
     return dtype == NAO_COMPLEX
-               ? ormtr_impl<cplx>(dtype, n, ncols, batch, (const cplx *)A, lda, sA, (const cplx *)tau, (cplx *)Z, ldz, sZ, work, st)
-               : ormtr_impl<double>(dtype, n, ncols, batch, (const double *)A, lda, sA, (const double *)tau, (double *)Z, ldz, sZ, work, st);
+               ? ormtr_impl<cplx>(dtype, n, ncols, batch, shift, (const cplx *)A, lda, sA, (const cplx *)tau, (cplx *)Z, ldz, sZ, work, st)
+               : ormtr_impl<double>(dtype, n, ncols, batch, shift, (const double *)A, lda, sA, (const double *)tau, (double *)Z, ldz, sZ, work, st);
 }
 
 }  // namespace nao

@@ -1,0 +1,306 @@
+// trd2.cu -- stage 1 of the two-stage tridiagonalisation: dense -> band (north_star "dense-to-band
+// uses GEMM-rich panels on FP64 DMMA").  Lower storage, bandwidth b = TRD2_B.
+//
+// For every panel (b columns j0..j0+b-1, rows j0+b..n-1, m = n - j0 - b):
+//   1. panel QR  P = Q R, Q = H_0 ... H_{b-1} = I - V T V^H        (panel_qr_kernel: one cooperative launch)
+//   2. X = A22 V T ;  W = X - 1/2 V (T^H (V^H X))                    (DMMA GEMMs; A22 read through triangular masks)
+//   3. A22 <- A22 - W V^H - V W^H  (lower tiles only)                (one rank-2b DMMA GEMM)
+// R stays in the upper triangle of the panel (those are the band entries b + r - c <= b), V below its diagonal with
+// the unit implicit: reflector of matrix column j has its unit at row j + b -- the layout ormtr(shift = b) applies.
+//
+// panel_qr_kernel: the G CTAs of an item hold their rows of the panel in shared memory for the whole panel and meet
+// at ONE grid barrier per column.  The classical two reductions per column (norm, then v^H A) are fused: with x the
+// column below the diagonal BEFORE the reflector is formed, CTAs publish sigma_c = x^H P[j+1:, c] (c >= j) and the
+// owner of the diagonal row publishes rho_c = P[j, c]; then ||x||^2 = sigma_j and
+//   v = [1; scale x],  v^H P[j:, c] = rho_c + conj(scale) sigma_c
+// so tau, v and the update of the trailing columns follow without a second reduction; the sigma's of column j+1 are
+// accumulated in the same pass that applies H_j.  Partials are summed in a fixed order (bit-reproducible).
+#include "nao_internal.cuh"
+#include "scalar.cuh"
+#include <algorithm>
+
+namespace nao {
+
+static const int QR_NT = 256;
+static const int QR_NW = QR_NT / 32;
+
+template <class T> struct QrArgs {
+    T *A; long lda, sA;          // full matrix (per item stride sA)
+    T *tau; long sTau;           // tau[j0 + c]
+    T *part;                     // per item: 2 x G x b   (double-buffered partial sigma)
+    T *rowb;                     // per item: 2 x b       (double-buffered rho)
+    unsigned *bar;               // per item
+    int n, j0, G, chunk;
+};
+
+template <class T>
+__global__ void __launch_bounds__(QR_NT, 1) panel_qr_kernel(QrArgs<T> p) {
+    typedef Ops<T> O;
+    constexpr int b = TRD2_B;
+    const int G = p.G, item = blockIdx.x / G, g = blockIdx.x % G;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int m = p.n - p.j0 - b;                         // panel rows
+    const int kk = min(m - 1, b);                         // reflectors
+    T *P = p.A + (long)item * p.sA + (p.j0 + b) + (long)p.j0 * p.lda;      // panel (m x b), ld = lda
+    T *tau = p.tau + (long)item * p.sTau + p.j0;
+    T *part = p.part + (long)item * 2 * G * b;
+    T *rowb = p.rowb + (long)item * 2 * b;
+    unsigned *bar = p.bar + item;
+    unsigned bar_ord = 0;
+    const int chunk = p.chunk, CHP = chunk | 1;
+    const int r0 = g * chunk, r1 = min(m, r0 + chunk);    // own rows (panel-local)
+    const int nown = max(0, r1 - r0);
+
+    extern __shared__ __align__(16) unsigned char qr_smem[];
+    T *sP = (T *)qr_smem;                                 // [b][CHP]
+    T *s_x = sP + (size_t)b * CHP;                        // [chunk] new column j+1
+    __shared__ T s_red[4][b];
+    __shared__ T s_sig[b], s_rho[b], s_z[b];
+    __shared__ T s_tau, s_scale;
+    __shared__ double s_beta;
+
+    for (int e = tid; e < nown * b; e += QR_NT) {
+        const int c = e / nown, r = e % nown;
+        sP[c * CHP + r] = P[(r0 + r) + (long)c * p.lda];
+    }
+    __syncthreads();
+
+    // partial sigma of column j over own rows r > j, columns c >= j: warp per column
+    auto publish = [&](int j) {
+        T *pp = part + ((long)(j & 1) * G + g) * b;
+        for (int c = j + warp; c < b; c += QR_NW) {
+            T s = O::zero();
+            for (int r = max(r0, j + 1) - r0 + lane; r < nown; r += 32) s = O::add(s, O::conj_mul(sP[j * CHP + r], sP[c * CHP + r]));
+            s = warp_sum(s);
+            if (lane == 0) pp[c] = s;
+        }
+        if (j >= r0 && j < r1)
+            for (int c = j + tid; c < b; c += QR_NT) rowb[(j & 1) * b + c] = sP[c * CHP + (j - r0)];
+    };
+    if (kk > 0) publish(0);
+
+    for (int j = 0; j < kk; ++j) {
+        group_barrier(bar, G, ++bar_ord);
+        // ---- reduce sigma (fixed order), fetch rho
+        {
+            const int c = tid & (b - 1), q = tid >> 6;
+            T s = O::zero();
+            if (c >= j) {
+                const T *pp = part + (long)(j & 1) * G * b + c;
+                for (int gg = q; gg < G; gg += 4) s = O::add(s, ldcg(pp + (long)gg * b));
+            }
+            s_red[q][c] = s;
+            if (q == 0 && c >= j) s_rho[c] = ldcg(rowb + (j & 1) * b + c);
+        }
+        __syncthreads();
+        if (tid < b) s_sig[tid] = O::add(O::add(s_red[0][tid], s_red[1][tid]), O::add(s_red[2][tid], s_red[3][tid]));
+        __syncthreads();
+        if (tid < b) {
+            // xLARFG from (alpha = rho_j, ||x||^2 = sigma_j), redundantly per thread
+            const double xn2 = O::real(s_sig[j]);
+            const T alpha = s_rho[j];
+            const double ar = O::real(alpha), ai = O::imag(alpha);
+            T tauj, scale; double beta;
+            if (xn2 == 0.0 && ai == 0.0) { tauj = O::zero(); scale = O::zero(); beta = ar; }
+            else {
+                const double nrm = sqrt(ar * ar + ai * ai + xn2);
+                beta = ar >= 0.0 ? -nrm : nrm;
+                if (O::is_complex) {
+                    cplx t = make_double2((beta - ar) / beta, -ai / beta);
+                    const double dr = ar - beta, di = ai, den = dr * dr + di * di;
+                    cplx sc = make_double2(dr / den, -di / den);
+                    tauj = *(T *)&t; scale = *(T *)&sc;
+                } else {
+                    tauj = O::from_real((beta - ar) / beta); scale = O::from_real(1.0 / (ar - beta));
+                }
+            }
+            if (tid > j) s_z[tid] = O::add(s_rho[tid], O::conj_mul(scale, s_sig[tid]));
+            if (tid == j) {
+                s_tau = tauj; s_scale = scale; s_beta = beta;
+                if (g == 0) tau[j] = tauj;
+            }
+        }
+        __syncthreads();
+        const T ctau = O::conj(s_tau), scale = s_scale;
+        // ---- phase a: v into column j; column j+1 brought up to date (s_x); diagonal row (owner)
+        const int lo = max(r0, j + 1) - r0;
+        const bool nextcol = (j + 1 < b);
+        const T zn = nextcol ? s_z[j + 1] : O::zero();
+        for (int r = lo + tid; r < nown; r += QR_NT) {
+            const T v = O::mul(scale, sP[j * CHP + r]);
+            sP[j * CHP + r] = v;
+            if (nextcol) {
+                const T x = O::sub(sP[(j + 1) * CHP + r], O::mul(O::mul(ctau, zn), v));
+                sP[(j + 1) * CHP + r] = x;
+                s_x[r] = x;
+            }
+        }
+        if (j >= r0 && j < r1) {
+            for (int c = j + tid; c < b; c += QR_NT) {
+                if (c == j) sP[c * CHP + (j - r0)] = O::from_real(s_beta);
+                else sP[c * CHP + (j - r0)] = O::sub(sP[c * CHP + (j - r0)], O::mul(ctau, s_z[c]));
+            }
+        }
+        __syncthreads();
+        // ---- phase b: apply H_j^H to columns c > j+1, accumulate sigma of column j+1 for c >= j+1
+        {
+            const bool pub = (j + 1 < kk);
+            T *pp = part + ((long)((j + 1) & 1) * G + g) * b;
+            const int lo2 = max(r0, j + 2) - r0;            // rows that enter the next sigma
+            for (int c = j + 1 + warp; c < b; c += QR_NW) {
+                T s = O::zero();
+                if (c == j + 1) {
+                    if (pub) for (int r = lo2 + lane; r < nown; r += 32) s = O::add(s, O::conj_mul(s_x[r], s_x[r]));
+                } else {
+                    const T f = O::mul(ctau, s_z[c]);
+                    for (int r = lo + lane; r < nown; r += 32) {
+                        const T a = O::sub(sP[c * CHP + r], O::mul(f, sP[j * CHP + r]));
+                        sP[c * CHP + r] = a;
+                        if (r >= lo2) s = O::add(s, O::conj_mul(s_x[r], a));
+                    }
+                }
+                if (pub) {
+                    s = warp_sum(s);
+                    if (lane == 0) pp[c] = s;
+                }
+            }
+            __syncthreads();
+            if (pub && j + 1 >= r0 && j + 1 < r1)
+                for (int c = j + 1 + tid; c < b; c += QR_NT) rowb[((j + 1) & 1) * b + c] = sP[c * CHP + (j + 1 - r0)];
+        }
+    }
+    if (g == 0) for (int c = max(kk, 0) + tid; c < b; c += QR_NT) tau[c] = O::zero();
+    __syncthreads();
+    for (int e = tid; e < nown * b; e += QR_NT) {
+        const int c = e / nown, r = e % nown;
+        P[(r0 + r) + (long)c * p.lda] = sP[c * CHP + r];
+    }
+}
+
+// ----------------------------------------------------------------------------------------------------------------
+// he2hb driver
+// ----------------------------------------------------------------------------------------------------------------
+struct He2hbWork {
+    void *P3, *X, *G, *Tm, *S, *M, *part, *rowb, *splitk; unsigned *bar;
+    int Gq, chunk, ipl, ksX, ksS; size_t smem, bytes;
+};
+static int trd2_num_sms() {
+    static int nsm = 0;
+    if (!nsm) {
+        int dev = 0; cudaGetDevice(&dev);
+        if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm <= 0) nsm = 148;
+    }
+    return nsm;
+}
+static He2hbWork he2hb_plan(int dtype, int n, int batch, void *work) {
+    He2hbWork w; const size_t es = esize(dtype); const int b = TRD2_B;
+    const int nsm = trd2_num_sms();
+    const int m0 = std::max(1, n - b);
+    // rows of the panel a CTA can keep in shared memory (b columns), leaving room for the static arrays
+    const int cap = (int)((200 * 1024) / ((size_t)(b + 1) * es)) - 2;
+    const int Gneed = ceil_div(m0, cap);
+    w.ipl = std::max(1, std::min(batch, nsm / std::max(1, Gneed)));      // items per cooperative launch
+    w.Gq = std::max(1, std::min(nsm / w.ipl, ceil_div(m0, 32)));
+    w.chunk = ceil_div(m0, w.Gq);
+    w.smem = ((size_t)b * (w.chunk | 1) + w.chunk) * es;
+    // split-K factors: X = A22 V (m x b, k = m) and the b x b products
+    const int tilesX = ceil_div(n, 128) * batch;
+    w.ksX = std::max(1, std::min(std::min(2 * nsm / std::max(1, tilesX), ceil_div(n, 512)), 16));
+    w.ksS = std::max(1, std::min(std::min(nsm / std::max(1, batch), ceil_div(n, 256)), 64));
+    Arena ar(work, (size_t)-1);
+    w.P3 = ar.take((size_t)batch * n * 3 * b * es);            // [W | V | W], ld n, rows indexed globally
+    w.X = ar.take((size_t)batch * n * b * es);
+    w.G = ar.take((size_t)batch * b * b * es);
+    w.Tm = ar.take((size_t)batch * b * b * es);
+    w.S = ar.take((size_t)batch * b * b * es);
+    w.M = ar.take((size_t)batch * b * b * es);
+    w.part = ar.take((size_t)batch * 2 * w.Gq * b * es);
+    w.rowb = ar.take((size_t)batch * 2 * b * es);
+    w.splitk = ar.take((size_t)batch * std::max((size_t)w.ksX * n * b, (size_t)w.ksS * b * b) * es);
+    w.bar = (unsigned *)ar.take((size_t)batch * (ceil_div(n, b) + 1) * 4);
+    w.bytes = ar.off;
+    return w;
+}
+size_t he2hb_workspace(int dtype, int n, int batch) { return he2hb_plan(dtype, n, batch, nullptr).bytes; }
+bool he2hb_supported(int dtype, int n, int batch) {
+    He2hbWork w = he2hb_plan(dtype, n, batch, nullptr);
+    return n > TRD2_B + 1 && w.smem <= 210 * 1024 && w.Gq * w.ipl <= trd2_num_sms();
+}
+
+template <class T>
+static int he2hb_impl(int dtype, int n, int batch, T *A, long lda, long sA, T *tau, void *work, cudaStream_t st) {
+    const int b = TRD2_B;
+    He2hbWork w = he2hb_plan(dtype, n, batch, work);
+    static bool attr = false;
+    if (!attr) {
+        NAO_CUDA_CHECK(cudaFuncSetAttribute(panel_qr_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, 210 * 1024));
+        attr = true;
+    }
+    const int npanels = ceil_div(n, b) + 1;
+    NAO_CUDA_CHECK(cudaMemsetAsync(w.bar, 0, (size_t)batch * npanels * 4, st));
+    NAO_CUDA_CHECK(cudaMemsetAsync(tau, 0, (size_t)batch * n * sizeof(T), st));
+    T *P3 = (T *)w.P3, *X = (T *)w.X;
+    const long sP3 = (long)n * 3 * b, sX = (long)n * b, sBB = (long)b * b;
+    T *Wb = P3, *Vb = P3 + (long)n * b;            // column blocks of P3: W at 0, V at b, W copy at 2b
+    int panel = 0;
+    for (int j0 = 0; n - j0 - b > 1; j0 += b, ++panel) {
+        const int m = n - j0 - b, jr = j0 + b;      // panel rows start at global row jr
+        // 1. panel QR (cooperative), items in groups of ipl
+        for (int b0 = 0; b0 < batch; b0 += w.ipl) {
+            const int nit = std::min(w.ipl, batch - b0);
+            QrArgs<T> a;
+            a.A = A + (long)b0 * sA; a.lda = lda; a.sA = sA; a.tau = tau + (long)b0 * n; a.sTau = n;
+            a.part = (T *)w.part + (long)b0 * 2 * w.Gq * b; a.rowb = (T *)w.rowb + (long)b0 * 2 * b;
+            a.bar = w.bar + (size_t)panel * batch + b0;
+            a.n = n; a.j0 = j0;
+            a.G = std::max(1, std::min(w.Gq, ceil_div(m, 32)));
+            a.chunk = ceil_div(m, a.G);
+            const size_t smem = ((size_t)b * (a.chunk | 1) + a.chunk) * sizeof(T);
+            void *args[] = {&a};
+            NAO_CUDA_CHECK(cudaLaunchCooperativeKernel((void *)panel_qr_kernel<T>, dim3(nit * a.G), dim3(QR_NT), args, smem, st));
+            NAO_LAUNCHED();
+        }
+        // 2. explicit V (m x b, zeros above the unit diagonal) at rows jr.. of the V block; T factor
+        if (int rc = build_v(dtype, n, j0, b, b, A, lda, sA, Vb + jr, n, sP3, batch, st)) return rc;
+        GemmDesc g = gemm_desc(OP_C, OP_N, b, b, m, 1.0, Vb + jr, n, Vb + jr, n, 0.0, w.G, b);
+        g.sA = sP3; g.sB = sP3; g.sC = sBB;
+        if (int rc = gemm_splitk(dtype, g, batch, std::min(w.ksS, ceil_div(m, 256)), w.splitk, st)) return rc;
+        if (int rc = larft(dtype, b, w.G, b, sBB, tau + j0, n, w.Tm, sBB, batch, st)) return rc;
+        // 3. X = A22 V : lower triangle as stored + strictly lower triangle transposed
+        T *A22 = A + jr + (long)jr * lda;
+        const int ksx = std::min(w.ksX, ceil_div(m, 512));
+        GemmDesc x1 = gemm_desc(OP_N, OP_N, m, b, m, 1.0, A22, lda, Vb + jr, n, 0.0, X + jr, n);
+        x1.sA = sA; x1.sB = sP3; x1.sC = sX; x1.maskA = MASK_LOWER;
+        if (int rc = gemm_splitk(dtype, x1, batch, ksx, w.splitk, st)) return rc;
+        GemmDesc x2 = gemm_desc(OP_C, OP_N, m, b, m, 1.0, A22, lda, Vb + jr, n, 1.0, X + jr, n);
+        x2.sA = sA; x2.sB = sP3; x2.sC = sX; x2.maskA = MASK_SLOWER;
+        if (int rc = gemm_splitk(dtype, x2, batch, ksx, w.splitk, st)) return rc;
+        // 4. W0 = X T  (into the W block), S = V^H W0, M = T^H S, W = W0 - 1/2 V M
+        GemmDesc xt = gemm_desc(OP_N, OP_N, m, b, b, 1.0, X + jr, n, w.Tm, b, 0.0, Wb + jr, n);
+        xt.sA = sX; xt.sB = sBB; xt.sC = sP3; xt.maskB = MASK_UPPER;
+        if (int rc = gemm_launch(dtype, xt, batch, st)) return rc;
+        GemmDesc s1 = gemm_desc(OP_C, OP_N, b, b, m, 1.0, Vb + jr, n, Wb + jr, n, 0.0, w.S, b);
+        s1.sA = sP3; s1.sB = sP3; s1.sC = sBB;
+        if (int rc = gemm_splitk(dtype, s1, batch, std::min(w.ksS, ceil_div(m, 256)), w.splitk, st)) return rc;
+        GemmDesc m1 = gemm_desc(OP_C, OP_N, b, b, b, 1.0, w.Tm, b, w.S, b, 0.0, w.M, b);
+        m1.sA = sBB; m1.sB = sBB; m1.sC = sBB; m1.maskA = MASK_UPPER;
+        if (int rc = gemm_launch(dtype, m1, batch, st)) return rc;
+        GemmDesc w1 = gemm_desc(OP_N, OP_N, m, b, b, -0.5, Vb + jr, n, w.M, b, 1.0, Wb + jr, n);
+        w1.sA = sP3; w1.sB = sBB; w1.sC = sP3;
+        if (int rc = gemm_launch(dtype, w1, batch, st)) return rc;
+        if (int rc = copy_matrix(dtype, m, b, Wb + jr, n, sP3, P3 + (long)n * 2 * b + jr, n, sP3, batch, 0, st)) return rc;
+        // 5. A22 -= [W V] [V W]^H, lower tiles
+        GemmDesc u = gemm_desc(OP_N, OP_C, m, m, 2 * b, -1.0, Wb + jr, n, Vb + jr, n, 1.0, A22, lda);
+        u.sA = sP3; u.sB = sP3; u.sC = sA; u.cmode = 1;
+        if (int rc = gemm_launch(dtype, u, batch, st)) return rc;
+    }
+    NAO_CUDA_CHECK(cudaGetLastError());
+    return NAO_OK;
+}
+
+int he2hb(int dtype, int n, int batch, void *A, long lda, long sA, void *tau, void *work, cudaStream_t st) {
+    return dtype == NAO_COMPLEX ? he2hb_impl<cplx>(dtype, n, batch, (cplx *)A, lda, sA, (cplx *)tau, work, st)
+                                : he2hb_impl<double>(dtype, n, batch, (double *)A, lda, sA, (double *)tau, work, st);
+}
+
+}  // namespace nao

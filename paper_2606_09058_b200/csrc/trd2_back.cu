@@ -1,0 +1,261 @@
+// trd2_back.cu -- back-transformation of the bulge-chasing stage: Z <- Q2 Z ("stage 2 then
+// stage 1, blocked Householder GEMMs").
+//
+// Q2 = prod_s prod_k H_{s,k} (sweeps s ascending, steps k ascending; reflector (s,k) acts on rows s+1+kb .. s+(k+1)b).
+// Reflectors are grouped in "diamonds": S-block I = sweeps s0 .. s0+NBK-1 (s0 = I*NBK) and step k give the group
+//   G(I,k) = H_{s0,k} H_{s0+1,k} ... = I - V T V^H,   V = (b + NBK - 1) x NBK parallelogram (rows s0+1+kb ..).
+// Reflectors of different steps of one sweep commute, and (s,k) overlaps (s',k+1) only for s' < s, so Q2 Z is obtained
+// by applying the groups with I DESCENDING and, inside an S-block, k ASCENDING (checked against the sweep-by-sweep
+// product in tests).  Columns of Z are independent: each CTA owns NC columns and walks through all groups without any
+// inter-CTA synchronisation; the three products per group (W = V^H Z_w, W <- T W, Z_w -= V W) run on FP64 DMMA from
+// shared memory.  T factors of all groups are precomputed by q2_tfactor_kernel.
+#include "nao_internal.cuh"
+#include "scalar.cuh"
+#include <algorithm>
+
+namespace nao {
+
+static const int Q2_NBK = 32;                 // sweeps per diamond
+static const int Q2_LW = 96;                  // padded window rows (>= TRD2_B + Q2_NBK - 1)
+static const int Q2_NC = 32;                  // columns of Z per CTA
+static const int Q2_NT = 128;
+static const int Q2_LDV = 100, Q2_LDW = 36;   // shared-memory leading dimensions (conflict-free fragment loads)
+
+__host__ __device__ inline int q2_nwin(int n, int s0) {      // windows of the S-block starting at sweep s0
+    return s0 + 1 <= n - 1 ? (n - 2 - s0) / TRD2_B + 1 : 0;
+}
+__host__ __device__ inline long q2_ngroups(int n) {
+    long t = 0;
+    for (int s0 = 0; s0 < n - 1; s0 += Q2_NBK) t += q2_nwin(n, s0);
+    return t;
+}
+
+// masked load of the V parallelogram of group (s0, k) into sV[ci * LDV + r] (zero padded to LW x NBK)
+template <class T>
+__device__ __forceinline__ void q2_load_v(T *sV, const T *V2, long ldv, int n, int s0, int ns, int k, int nthreads) {
+    constexpr int b = TRD2_B;
+    const int w0 = s0 + 1 + k * b;
+    for (int e = threadIdx.x; e < Q2_LW * Q2_NBK; e += nthreads) {
+        const int r = e % Q2_LW, ci = e / Q2_LW;
+        const int s = s0 + ci, gr = w0 + r;
+        T v = Ops<T>::zero();
+        if (ci < ns && gr >= s + 1 + k * b && gr <= min(s + (k + 1) * b, n - 1)) v = V2[gr + (long)s * ldv];
+        sV[ci * Q2_LDV + r] = v;
+    }
+}
+
+template <class T>
+__global__ void __launch_bounds__(256) q2_tfactor_kernel(int n, const T *V2, long ldv, long sV2, const T *tau2, long sTau2,
+                                                         T *Tst, long sTst) {
+    typedef Ops<T> O;
+    constexpr int NBK = Q2_NBK;
+    const int I = blockIdx.x, k = blockIdx.y, item = blockIdx.z;
+    const int s0 = I * NBK;
+    if (k >= q2_nwin(n, s0)) return;
+    const int ns = min(NBK, n - 1 - s0);
+    V2 += (long)item * sV2; tau2 += (long)item * sTau2; Tst += (long)item * sTst;
+    long goff = 0;
+    for (int s = 0; s < s0; s += NBK) goff += q2_nwin(n, s);
+    T *Tout = Tst + (goff + k) * NBK * NBK;
+
+    extern __shared__ __align__(16) unsigned char q2t_smem[];
+    T *sV = (T *)q2t_smem;                    // [NBK][LDV]
+    __shared__ T sG[NBK][NBK + 1], sT[NBK][NBK + 1], s_tau[NBK];
+    const int tid = threadIdx.x;
+    q2_load_v<T>(sV, V2, ldv, n, s0, ns, k, 256);
+    if (tid < NBK) s_tau[tid] = tid < ns ? tau2[(long)k * n + s0 + tid] : O::zero();
+    for (int e = tid; e < NBK * NBK; e += 256) sT[e / NBK][e % NBK] = O::zero();
+    __syncthreads();
+    // G = V^H V (upper part is what the recurrence reads)
+    for (int e = tid; e < NBK * NBK; e += 256) {
+        const int i = e % NBK, j = e / NBK;
+        T s = O::zero();
+        if (i < j) for (int r = 0; r < Q2_LW; ++r) s = O::add(s, O::conj_mul(sV[i * Q2_LDV + r], sV[j * Q2_LDV + r]));
+        sG[i][j] = s;
+    }
+    __syncthreads();
+    // T(i,i) = tau_i ; T(0:i, i) = -tau_i T(0:i,0:i) G(0:i, i)
+    for (int i = 0; i < NBK; ++i) {
+        if (tid < i) {
+            T acc = O::zero();
+            for (int c = tid; c < i; ++c) acc = O::fma(sT[tid][c], sG[c][i], acc);
+            sT[tid][i] = O::sub(O::zero(), O::mul(s_tau[i], acc));
+        }
+        if (tid == i) sT[i][i] = s_tau[i];
+        __syncthreads();
+    }
+    for (int e = tid; e < NBK * NBK; e += 256) Tout[e] = sT[e % NBK][e / NBK];      // column-major, ld = NBK
+}
+
+__device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+// acc (+)= A(8 x 4) B(4 x 8) for real / complex scalars; CONJA conjugates the A fragment, NEG negates it
+template <class T, bool CONJA, bool NEG> struct Frag;
+template <bool CONJA, bool NEG> struct Frag<double, CONJA, NEG> {
+    static __device__ __forceinline__ void mma(double (&acc)[4], double a, double b) {
+        dmma884(acc[0], acc[1], NEG ? -a : a, b);
+    }
+};
+template <bool CONJA, bool NEG> struct Frag<cplx, CONJA, NEG> {
+    static __device__ __forceinline__ void mma(double (&acc)[4], cplx a, cplx b) {
+        double ar = NEG ? -a.x : a.x, ai = (CONJA != NEG) ? -a.y : a.y;
+        dmma884(acc[0], acc[1], ar, b.x);
+        dmma884(acc[0], acc[1], -ai, b.y);
+        dmma884(acc[2], acc[3], ar, b.y);
+        dmma884(acc[2], acc[3], ai, b.x);
+    }
+};
+template <class T> __device__ __forceinline__ T frag_out(const double (&acc)[4], int q);
+template <> __device__ __forceinline__ double frag_out<double>(const double (&acc)[4], int q) { return acc[q]; }
+template <> __device__ __forceinline__ cplx frag_out<cplx>(const double (&acc)[4], int q) { return make_double2(acc[q], acc[2 + q]); }
+
+template <class T>
+__global__ void __launch_bounds__(Q2_NT) q2_apply_kernel(int n, int ncols, const T *V2, long ldv, long sV2, const T *Tst,
+                                                         long sTst, T *Z, long ldz, long sZ) {
+    typedef Ops<T> O;
+    constexpr int b = TRD2_B, NBK = Q2_NBK, LW = Q2_LW, NC = Q2_NC, LDV = Q2_LDV, LDW = Q2_LDW;
+    const int item = blockIdx.y, c0 = blockIdx.x * NC;
+    V2 += (long)item * sV2; Tst += (long)item * sTst; Z += (long)item * sZ;
+    extern __shared__ __align__(16) unsigned char q2_smem[];
+    T *sV = (T *)q2_smem;                 // [NBK][LDV]
+    T *sZ_ = sV + NBK * LDV;              // [NC][LDV]
+    T *sT = sZ_ + NC * LDV;               // [NBK][LDW]  T(i,k) at k*LDW + i
+    T *sW = sT + NBK * LDW;               // [NC][LDW]   W(ci,c) at c*LDW + ci
+    T *sW2 = sW + NC * LDW;               // [NC][LDW]
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, lr = lane >> 2, lc = lane & 3;
+
+    const int nsweeps = n - 1;
+    const int nS = (nsweeps + NBK - 1) / NBK;
+    long goff = q2_ngroups(n);
+    for (int I = nS - 1; I >= 0; --I) {
+        const int s0 = I * NBK, ns = min(NBK, nsweeps - s0), nwin = q2_nwin(n, s0);
+        goff -= nwin;
+        for (int k = 0; k < nwin; ++k) {
+            const int w0 = s0 + 1 + k * b;
+            const int Lw = min(s0 + ns - 1 + (k + 1) * b, n - 1) - w0 + 1;
+            __syncthreads();                                    // previous window's stores / smem reads are done
+            q2_load_v<T>(sV, V2, ldv, n, s0, ns, k, Q2_NT);
+            {
+                const T *Tg = Tst + (goff + k) * NBK * NBK;
+                for (int e = tid; e < NBK * NBK; e += Q2_NT) sT[(e / NBK) * LDW + (e % NBK)] = Tg[e];
+            }
+            for (int e = tid; e < LW * NC; e += Q2_NT) {
+                const int r = e % LW, c = e / LW;
+                T v = O::zero();
+                if (r < Lw && c0 + c < ncols) v = Z[(w0 + r) + (long)(c0 + c) * ldz];
+                sZ_[c * LDV + r] = v;
+            }
+            __syncthreads();
+            // ---- W = V^H Z_w : warp -> 8 rows (ci) x 32 columns
+            {
+                double acc[4][4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) acc[j][q] = 0.0;
+                const T *ap = sV + (warp * 8 + lr) * LDV + lc;
+                const T *bp = sZ_ + lr * LDV + lc;
+#pragma unroll 4
+                for (int k0 = 0; k0 < LW; k0 += 4) {
+                    const T a = ap[k0];
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) Frag<T, true, false>::mma(acc[j], a, bp[j * 8 * LDV + k0]);
+                }
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+#pragma unroll
+                    for (int q = 0; q < 2; ++q) sW[(j * 8 + 2 * lc + q) * LDW + warp * 8 + lr] = frag_out<T>(acc[j], q);
+            }
+            __syncthreads();
+            // ---- W2 = T W
+            {
+                double acc[4][4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) acc[j][q] = 0.0;
+                const T *ap = sT + lc * LDW + warp * 8 + lr;
+                const T *bp = sW + lr * LDW + lc;
+#pragma unroll
+                for (int k0 = 0; k0 < NBK; k0 += 4) {
+                    const T a = ap[k0 * LDW];
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) Frag<T, false, false>::mma(acc[j], a, bp[j * 8 * LDW + k0]);
+                }
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+#pragma unroll
+                    for (int q = 0; q < 2; ++q) sW2[(j * 8 + 2 * lc + q) * LDW + warp * 8 + lr] = frag_out<T>(acc[j], q);
+            }
+            __syncthreads();
+            // ---- Z_w -= V W2 : warp -> 24 rows x 32 columns, result straight to global memory
+#pragma unroll
+            for (int i = 0; i < 3; ++i) {
+                const int m0 = (warp * 3 + i) * 8;
+                double acc[4][4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+#pragma unroll
+                    for (int q = 0; q < 2; ++q) {
+                        const T z = sZ_[(j * 8 + 2 * lc + q) * LDV + m0 + lr];
+                        if constexpr (O::is_complex) { acc[j][q] = z.x; acc[j][2 + q] = z.y; } else { acc[j][q] = z; acc[j][2 + q] = 0.0; }
+                    }
+                const T *ap = sV + lc * LDV + m0 + lr;
+                const T *bp = sW2 + lr * LDW + lc;
+#pragma unroll
+                for (int k0 = 0; k0 < NBK; k0 += 4) {
+                    const T a = ap[k0 * LDV];
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) Frag<T, false, true>::mma(acc[j], a, bp[j * 8 * LDW + k0]);
+                }
+                const int r = m0 + lr;
+                if (r < Lw) {
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)
+#pragma unroll
+                        for (int q = 0; q < 2; ++q) {
+                            const int c = c0 + j * 8 + 2 * lc + q;
+                            if (c < ncols) Z[(w0 + r) + (long)c * ldz] = frag_out<T>(acc[j], q);
+                        }
+                }
+            }
+        }
+    }
+}
+
+size_t q2_workspace(int dtype, int n, int batch) { return align_up((size_t)batch * q2_ngroups(n) * Q2_NBK * Q2_NBK * esize(dtype)); }
+
+template <class T>
+static int q2_apply_impl(int n, int ncols, int batch, const T *V2, long ldv, long sV2, const T *tau2, T *Z, long ldz, long sZ,
+                         void *work, cudaStream_t st) {
+    if (n < 2) return NAO_OK;
+    const long ng = q2_ngroups(n), sTst = ng * Q2_NBK * Q2_NBK, sTau2 = (long)hb2st_nk(n) * n;
+    T *Tst = (T *)work;
+    const int nS = ceil_div(n - 1, Q2_NBK), kmax = q2_nwin(n, 0);
+    const size_t smem_t = (size_t)Q2_NBK * Q2_LDV * sizeof(T);
+    const size_t smem_a = (size_t)(2 * Q2_NBK * Q2_LDV + 3 * Q2_NBK * Q2_LDW) * sizeof(T);
+    static bool attr = false;
+    if (!attr) {
+        NAO_CUDA_CHECK(cudaFuncSetAttribute(q2_tfactor_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_t));
+        NAO_CUDA_CHECK(cudaFuncSetAttribute(q2_apply_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_a));
+        attr = true;
+    }
+    q2_tfactor_kernel<T><<<dim3(nS, kmax, batch), 256, smem_t, st>>>(n, V2, ldv, sV2, tau2, sTau2, Tst, sTst);
+    NAO_LAUNCHED();
+    q2_apply_kernel<T><<<dim3(ceil_div(ncols, Q2_NC), batch), Q2_NT, smem_a, st>>>(n, ncols, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ);
+    NAO_LAUNCHED();
+    NAO_CUDA_CHECK(cudaGetLastError());
+    return NAO_OK;
+}
+
+int q2_apply(int dtype, int n, int ncols, int batch, const void *V2, long ldv, long sV2, const void *tau2, void *Z, long ldz,
+             long sZ, void *work, cudaStream_t st) {
+    return dtype == NAO_COMPLEX
+               ? q2_apply_impl<cplx>(n, ncols, batch, (const cplx *)V2, ldv, sV2, (const cplx *)tau2, (cplx *)Z, ldz, sZ, work, st)
+               : q2_apply_impl<double>(n, ncols, batch, (const double *)V2, ldv, sV2, (const double *)tau2, (double *)Z, ldz, sZ, work, st);
+}
+
+}  // namespace nao

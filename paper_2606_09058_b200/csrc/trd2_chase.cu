@@ -1,0 +1,329 @@
+// trd2_chase.cu -- stage 2 of the two-stage tridiagonalisation: band -> real tridiagonal by bulge chasing, staged in
+// shared memory (north_star "band-to-tridiagonal uses bulge chasing staged in shared memory").
+//
+// Band B (lower, bandwidth b = TRD2_B) is kept in HBM/L2 as AB[(i - j) + j * 2b], 0 <= i - j < 2b (the second b rows
+// hold the bulge).  Sweep s annihilates column s below the sub-diagonal:
+//   step 0   : v = house(B[s+1 : s+b, s]);  D_0 <- H^H D_0 H                         (D_0 = diagonal block of those rows)
+//   step k>=1: O = B[R_k, R_{k-1}] <- O H_{k-1};  v_k = house(O[:, 0]);  O[:, 1:] <- H_k^H O[:, 1:];  D_k <- H_k^H D_k H_k
+// with R_k = rows s+1+kb .. s+(k+1)b.  One CTA runs a whole sweep, carrying the reflector in shared memory; sweeps are
+// pipelined over the co-resident CTAs of a persistent cooperative kernel: sweep s+1 may run step k once sweep s has
+// finished step k+1 (progress counters in global memory, release/acquire).  CTA c of an item runs sweeps c, c+P, ...
+// in order, so the lowest unfinished sweep can always advance (no deadlock).
+//
+// Reflector (s, k) is stored for the back-transformation at V2[R_k, s] (unit stored explicitly), tau2[k * n + s].
+// Complex case: beta of every reflector is real, so the final sub-diagonal is real; the last sweep (length 1) only
+// removes the phase of B[n-1, n-2].
+#include "nao_internal.cuh"
+#include "scalar.cuh"
+#include <algorithm>
+#include <climits>
+
+namespace nao {
+
+static const int CH_NT = 256;
+
+template <class T>
+__global__ void band_extract_kernel(int n, const T *A, long lda, long sA, T *AB, long sAB) {
+    constexpr int b = TRD2_B, ld = 2 * b;
+    A += (long)blockIdx.y * sA; AB += (long)blockIdx.y * sAB;
+    const int j = blockIdx.x;
+    for (int r = threadIdx.x; r < ld; r += blockDim.x) {
+        const int i = j + r;
+        T v = Ops<T>::zero();
+        if (r <= b && i < n) { v = A[i + (long)j * lda]; if (r == 0) v = Ops<T>::from_real(Ops<T>::real(v)); }
+        AB[r + (long)j * ld] = v;
+    }
+}
+
+template <class T> struct ChaseArgs {
+    T *AB; long sAB;             // band, 2b x n per item
+    T *V2; long ldv, sV2;        // n x n per item
+    T *tau2; long sTau2;         // nk x n per item (tau2[k * n + s])
+    double *d, *e;               // n each per item
+    int *prog;                   // n per item, zero-initialised
+    int n, P;
+};
+
+__device__ __forceinline__ int ld_acquire(const int *p) {
+    int v;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release(int *p, int v) {
+    asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+// xLARFG on x[0..L) held in shared memory (x[0] = alpha); executed by warp 0.  Leaves v in x (x[0] = 1), returns
+// (tau, beta) through shared scalars.
+template <class T>
+__device__ __forceinline__ void house_warp(T *x, int L, T *s_tau, double *s_beta) {
+    typedef Ops<T> O;
+    const int lane = threadIdx.x & 31;
+    double xn2 = 0.0;
+    for (int i = 1 + lane; i < L; i += 32) xn2 += O::abs2(x[i]);
+    xn2 = warp_sum(xn2);
+    const T alpha = x[0];
+    const double ar = O::real(alpha), ai = O::imag(alpha);
+    T tau, scale; double beta;
+    if (xn2 == 0.0 && ai == 0.0) { tau = O::zero(); scale = O::zero(); beta = ar; }
+    else {
+        const double nrm = sqrt(ar * ar + ai * ai + xn2);
+        beta = ar >= 0.0 ? -nrm : nrm;
+        if (O::is_complex) {
+            cplx t = make_double2((beta - ar) / beta, -ai / beta);
+            const double dr = ar - beta, di = ai, den = dr * dr + di * di;
+            cplx sc = make_double2(dr / den, -di / den);
+            tau = *(T *)&t; scale = *(T *)&sc;
+        } else {
+            tau = O::from_real((beta - ar) / beta); scale = O::from_real(1.0 / (ar - beta));
+        }
+    }
+    __syncwarp();
+    for (int i = 1 + lane; i < L; i += 32) x[i] = O::mul(scale, x[i]);
+    if (lane == 0) { x[0] = O::one(); *s_tau = tau; *s_beta = beta; }
+}
+
+template <class T>
+__global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
+    typedef Ops<T> O;
+    constexpr int b = TRD2_B, ld = 2 * b, LDS = b + 1;
+    const int P = p.P, item = blockIdx.x / P, c = blockIdx.x % P;
+    const int n = p.n, tid = threadIdx.x, warp = tid >> 5;
+    T *AB = p.AB + (long)item * p.sAB;
+    T *V2 = p.V2 + (long)item * p.sV2;
+    T *tau2 = p.tau2 + (long)item * p.sTau2;
+    double *dd = p.d + (long)item * n, *ee = p.e + (long)item * n;
+    int *prog = p.prog + (long)item * n;
+
+    extern __shared__ __align__(16) unsigned char ch_smem[];
+    T *sO = (T *)ch_smem;              // [b][LDS]  off-diagonal block, column-major
+    T *sD = sO + b * LDS;              // [b][LDS]  diagonal block (full Hermitian)
+    __shared__ T s_vp[b], s_vn[b], s_w[b], s_part[4][b];
+    __shared__ T s_tau_p, s_tau_n;
+    __shared__ double s_beta, s_gamma;
+
+    const int iq = tid & (b - 1), qq = tid >> 6;        // (row or column index, quarter)
+
+    // D <- H^H D H for the L x L block in sD with v = s_vn, tau = s_tau_n  (u = D v, gamma = v^H u,
+    // w = tau u - 1/2 |tau|^2 gamma v,  D -= w v^H + v w^H)
+    auto two_sided = [&](int L) {
+        {
+            T s = O::zero();
+            if (iq < L) for (int cc = qq; cc < L; cc += 4) s = O::fma(sD[cc * LDS + iq], s_vn[cc], s);
+            s_part[qq][iq] = s;
+        }
+        __syncthreads();
+        if (tid < b) s_w[tid] = tid < L ? O::add(O::add(s_part[0][tid], s_part[1][tid]), O::add(s_part[2][tid], s_part[3][tid])) : O::zero();
+        __syncthreads();
+        if (warp == 0) {
+            double gsum = 0.0;
+            for (int i = tid; i < L; i += 32) gsum += O::real(O::conj_mul(s_vn[i], s_w[i]));
+            gsum = warp_sum(gsum);
+            if (tid == 0) s_gamma = gsum;
+        }
+        __syncthreads();
+        {
+            const T tau = s_tau_n;
+            const double f = -0.5 * O::abs2(tau) * s_gamma;
+            T wv = O::zero();
+            if (tid < L) wv = O::add(O::mul(tau, s_w[tid]), O::scale(s_vn[tid], f));
+            __syncthreads();
+            if (tid < b) s_w[tid] = wv;
+        }
+        __syncthreads();
+        if (iq < L)
+            for (int cc = qq; cc < L; cc += 4) {
+                T a = sD[cc * LDS + iq];
+                a = O::sub(a, O::add(O::mul_conj(s_w[iq], s_vn[cc]), O::mul_conj(s_vn[iq], s_w[cc])));
+                if (cc == iq) a = O::from_real(O::real(a));
+                sD[cc * LDS + iq] = a;
+            }
+        __syncthreads();
+    };
+    // diagonal block rows/cols [g0, g0+L): load (Hermitian completion) / store (lower part)
+    auto load_D = [&](int g0, int L) {
+        for (int e = tid; e < b * b; e += CH_NT) {
+            const int i = e & (b - 1), cc = e >> 6;
+            T v = O::zero();
+            if (i < L && cc < L) {
+                if (i >= cc) v = ldcg(AB + (i - cc) + (long)(g0 + cc) * ld);
+                else v = O::conj(ldcg(AB + (cc - i) + (long)(g0 + i) * ld));
+            }
+            sD[cc * LDS + i] = v;
+        }
+    };
+    auto store_D = [&](int g0, int L) {
+        for (int e = tid; e < b * b; e += CH_NT) {
+            const int i = e & (b - 1), cc = e >> 6;
+            if (i < L && cc < L && i >= cc) AB[(i - cc) + (long)(g0 + cc) * ld] = sD[cc * LDS + i];
+        }
+    };
+
+    for (int s = c; s < n - 1; s += P) {
+        // ------------------------------------------------ step 0
+        int r0 = s + 1, Lp = min(s + b, n - 1) - r0 + 1;
+        if (s > 0) {
+            if (tid == 0) { while (ld_acquire(prog + s - 1) < 2) { } }
+            __syncthreads();
+        }
+        if (tid < b) s_vn[tid] = tid < Lp ? ldcg(AB + (1 + tid) + (long)s * ld) : O::zero();
+        load_D(r0, Lp);
+        __syncthreads();
+        if (warp == 0) house_warp<T>(s_vn, Lp, &s_tau_n, &s_beta);
+        __syncthreads();
+        if (tid < Lp) {
+            V2[(r0 + tid) + (long)s * p.ldv] = s_vn[tid];
+            AB[(1 + tid) + (long)s * ld] = tid == 0 ? O::from_real(s_beta) : O::zero();
+        }
+        if (tid == 0) { tau2[s] = s_tau_n; ee[s] = s_beta; dd[s] = O::real(ldcg(AB + (long)s * ld)); }
+        two_sided(Lp);
+        store_D(r0, Lp);
+        if (tid < b) s_vp[tid] = s_vn[tid];
+        if (tid == 0) s_tau_p = s_tau_n;
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) st_release(prog + s, 1);
+        // ------------------------------------------------ steps k >= 1
+        for (int k = 1;; ++k) {
+            const int q0 = s + 1 + k * b;
+            if (q0 > n - 1) break;
+            const int Lq = min(s + (k + 1) * b, n - 1) - q0 + 1;
+            if (s > 0) {
+                if (tid == 0) { while (ld_acquire(prog + s - 1) < k + 2) { } }
+                __syncthreads();
+            }
+            // load O = B[q0 : q0+Lq, r0 : r0+Lp] and D = B[q0.., q0..]
+            for (int e = tid; e < b * b; e += CH_NT) {
+                const int i = e & (b - 1), cc = e >> 6;
+                T v = O::zero();
+                if (i < Lq && cc < Lp) v = ldcg(AB + (q0 + i - r0 - cc) + (long)(r0 + cc) * ld);
+                sO[cc * LDS + i] = v;
+            }
+            load_D(q0, Lq);
+            __syncthreads();
+            // w = O v_prev ; O -= tau_prev w v_prev^H
+            {
+                T sacc = O::zero();
+                if (iq < Lq) for (int cc = qq; cc < Lp; cc += 4) sacc = O::fma(sO[cc * LDS + iq], s_vp[cc], sacc);
+                s_part[qq][iq] = sacc;
+            }
+            __syncthreads();
+            {
+                const T tw = iq < Lq ? O::mul(s_tau_p, O::add(O::add(s_part[0][iq], s_part[1][iq]), O::add(s_part[2][iq], s_part[3][iq]))) : O::zero();
+                if (iq < Lq)
+                    for (int cc = qq; cc < Lp; cc += 4) sO[cc * LDS + iq] = O::sub(sO[cc * LDS + iq], O::mul_conj(tw, s_vp[cc]));
+            }
+            __syncthreads();
+            // new reflector from the first column of O
+            if (tid < b) s_vn[tid] = tid < Lq ? sO[tid] : O::zero();
+            __syncthreads();
+            if (warp == 0) house_warp<T>(s_vn, Lq, &s_tau_n, &s_beta);
+            __syncthreads();
+            if (tid < Lq) {
+                V2[(q0 + tid) + (long)s * p.ldv] = s_vn[tid];
+                sO[tid] = tid == 0 ? O::from_real(s_beta) : O::zero();
+            }
+            if (tid == 0) tau2[(long)k * n + s] = s_tau_n;
+            // z_c = v^H O[:, c] (c >= 1) ; O[:, c] -= conj(tau) v z_c     thread <-> (column iq, row quarter qq)
+            {
+                T sacc = O::zero();
+                if (iq >= 1 && iq < Lp) for (int i = qq; i < Lq; i += 4) sacc = O::add(sacc, O::conj_mul(s_vn[i], sO[iq * LDS + i]));
+                s_part[qq][iq] = sacc;
+            }
+            __syncthreads();
+            if (tid < b) s_w[tid] = O::mul(O::conj(s_tau_n), O::add(O::add(s_part[0][tid], s_part[1][tid]), O::add(s_part[2][tid], s_part[3][tid])));
+            __syncthreads();
+            if (iq < Lq)
+                for (int cc = (qq == 0 ? 4 : qq); cc < Lp; cc += 4)
+                    sO[cc * LDS + iq] = O::sub(sO[cc * LDS + iq], O::mul(s_vn[iq], s_w[cc]));
+            __syncthreads();
+            // store O
+            for (int e = tid; e < b * b; e += CH_NT) {
+                const int i = e & (b - 1), cc = e >> 6;
+                if (i < Lq && cc < Lp) AB[(q0 + i - r0 - cc) + (long)(r0 + cc) * ld] = sO[cc * LDS + i];
+            }
+            two_sided(Lq);
+            store_D(q0, Lq);
+            if (tid < b) s_vp[tid] = s_vn[tid];
+            if (tid == 0) s_tau_p = s_tau_n;
+            __threadfence();
+            __syncthreads();
+            if (tid == 0) st_release(prog + s, k + 1);
+            r0 = q0; Lp = Lq;
+        }
+        __syncthreads();
+        if (tid == 0) st_release(prog + s, INT_MAX);
+    }
+    // the last diagonal entry
+    if (c == (n - 1) % P || n == 1) {
+        if (n >= 2) { if (tid == 0) { while (ld_acquire(prog + n - 2) < INT_MAX) { } } }
+        __syncthreads();
+        if (tid == 0) { dd[n - 1] = O::real(ldcg(AB + (long)(n - 1) * ld)); ee[n - 1] = 0.0; }
+    }
+}
+
+struct ChaseWork { void *AB; int *prog; int P, ipl; size_t bytes; };
+static int ch_num_sms() {
+    static int nsm = 0;
+    if (!nsm) {
+        int dev = 0; cudaGetDevice(&dev);
+        if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm <= 0) nsm = 148;
+    }
+    return nsm;
+}
+static ChaseWork chase_plan(int dtype, int n, int batch, void *work) {
+    ChaseWork w; const size_t es = esize(dtype);
+    const int nsm = ch_num_sms();
+    const int want = ceil_div(n, 2 * TRD2_B) + 1;              // sweeps that can be in flight
+    w.ipl = std::max(1, std::min(batch, nsm / std::min(want, nsm)));
+    w.P = std::max(1, std::min(want, nsm / w.ipl));
+    Arena ar(work, (size_t)-1);
+    w.AB = ar.take((size_t)batch * 2 * TRD2_B * n * es);
+    w.prog = (int *)ar.take((size_t)batch * n * 4);
+    w.bytes = ar.off;
+    return w;
+}
+size_t hb2st_workspace(int dtype, int n, int batch) { return chase_plan(dtype, n, batch, nullptr).bytes; }
+int hb2st_nk(int n) { return ceil_div(n, TRD2_B) + 1; }
+
+template <class T>
+static int hb2st_impl(int dtype, int n, int batch, const T *A, long lda, long sA, double *d, double *e, T *V2, long ldv,
+                      long sV2, T *tau2, void *work, cudaStream_t st) {
+    constexpr int b = TRD2_B;
+    ChaseWork w = chase_plan(dtype, n, batch, work);
+    const size_t smem = (size_t)2 * b * (b + 1) * sizeof(T);
+    static bool attr = false;
+    if (!attr) {
+        NAO_CUDA_CHECK(cudaFuncSetAttribute(chase_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr = true;
+    }
+    const long sAB = (long)2 * b * n, sTau2 = (long)hb2st_nk(n) * n;
+    band_extract_kernel<T><<<dim3(n, batch), 128, 0, st>>>(n, A, lda, sA, (T *)w.AB, sAB);
+    NAO_LAUNCHED();
+    NAO_CUDA_CHECK(cudaMemsetAsync(w.prog, 0, (size_t)batch * n * 4, st));
+    NAO_CUDA_CHECK(cudaMemsetAsync(V2, 0, (size_t)batch * sV2 * sizeof(T), st));
+    NAO_CUDA_CHECK(cudaMemsetAsync(tau2, 0, (size_t)batch * sTau2 * sizeof(T), st));
+    for (int b0 = 0; b0 < batch; b0 += w.ipl) {
+        const int nit = std::min(w.ipl, batch - b0);
+        ChaseArgs<T> a;
+        a.AB = (T *)w.AB + (long)b0 * sAB; a.sAB = sAB;
+        a.V2 = V2 + (long)b0 * sV2; a.ldv = ldv; a.sV2 = sV2;
+        a.tau2 = tau2 + (long)b0 * sTau2; a.sTau2 = sTau2;
+        a.d = d + (long)b0 * n; a.e = e + (long)b0 * n; a.prog = w.prog + (long)b0 * n;
+        a.n = n; a.P = w.P;
+        void *args[] = {&a};
+        NAO_CUDA_CHECK(cudaLaunchCooperativeKernel((void *)chase_kernel<T>, dim3(nit * w.P), dim3(CH_NT), args, smem, st));
+        NAO_LAUNCHED();
+    }
+    NAO_CUDA_CHECK(cudaGetLastError());
+    return NAO_OK;
+}
+
+int hb2st(int dtype, int n, int batch, const void *A, long lda, long sA, double *d, double *e, void *V2, long ldv, long sV2,
+          void *tau2, void *work, cudaStream_t st) {
+    return dtype == NAO_COMPLEX
+               ? hb2st_impl<cplx>(dtype, n, batch, (const cplx *)A, lda, sA, d, e, (cplx *)V2, ldv, sV2, (cplx *)tau2, work, st)
+               : hb2st_impl<double>(dtype, n, batch, (const double *)A, lda, sA, d, e, (double *)V2, ldv, sV2, (double *)tau2, work, st);
+}
+
+}  // namespace nao
