@@ -118,8 +118,8 @@ def profile_enable(on: bool = True) -> None:
 
 def profile_read() -> dict:
     """Phase durations (ms) of the last nao_geneig call made with profiling enabled."""
-    buf = (ctypes.c_double * 8)()
-    k = lib().nao_profile_read(buf, 8)
+    buf = (ctypes.c_double * 16)()
+    k = lib().nao_profile_read(buf, 16)
     return {lib().nao_profile_phase_name(i).decode(): buf[i] for i in range(k)}
 
 

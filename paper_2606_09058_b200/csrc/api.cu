@@ -17,8 +17,8 @@ NAO_EXPORT long nao_launch_count(void) { return nao::g_launch_count; }
 
 // ---- optional phase timing (CUDA events recorded on the caller's stream at phase boundaries of nao_geneig) ----
 namespace nao {
-static const int NPH = 7;
-static const char *kPhaseNames[NPH - 1] = {"potrf_trtri", "reduce_WHWh", "tridiagonalise", "stedc", "back_transform", "C_WhZ"};
+static const int NPH = 9;
+static const char *kPhaseNames[NPH - 1] = {"potrf_trtri", "reduce_WHWh", "tridiagonalise", "band_to_tridiagonal", "stedc", "back_transform_band", "back_transform", "C_WhZ"};
 static bool g_prof_on = false;
 static cudaEvent_t g_ev[NPH];
 static bool g_ev_made = false, g_ev_rec[NPH];

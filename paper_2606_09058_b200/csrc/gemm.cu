@@ -18,23 +18,11 @@
 // half); "lower tiles only" output; optional scaling of op(A)'s k-th column by s[k] (Fermi weights);
 // strided batches and grouped launches whose descriptors (incl. m,n,k) live in device memory.
 #include "nao_internal.cuh"
+#include "scalar.cuh"
 
 namespace nao {
 
 long g_launch_count = 0;
-
-__device__ __forceinline__ void cp_async8(void *smem, const void *g, bool pred) {
-    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-    int sz = pred ? 8 : 0;
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(s), "l"(g), "r"(sz));
-}
-__device__ __forceinline__ void cp_async16(void *smem, const void *g, bool pred) {
-    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-    int sz = pred ? 16 : 0;
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(g), "r"(sz));
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
-template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
 
 __device__ __forceinline__ void dmma(double &c0, double &c1, double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"

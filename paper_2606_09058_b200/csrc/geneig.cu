@@ -53,11 +53,13 @@ static int heev(int dtype, int n, int batch, unsigned flags, void *A, long lda, 
     prof_mark(2, st);
     if (p.two_stage) {
         if ((rc = he2hb(dtype, n, batch, A, lda, sA, tau, sub, st))) return rc;
+        prof_mark(3, st);
         if ((rc = hb2st(dtype, n, batch, A, lda, sA, d, e, V2, n, (long)n * n, tau2, sub, st))) return rc;
     } else {
         if ((rc = hetrd(dtype, n, batch, A, lda, sA, d, e, tau, sub, st))) return rc;
+        prof_mark(3, st);
     }
-    prof_mark(3, st);
+    prof_mark(4, st);
     if (dtype == NAO_COMPLEX) {
         double *qt = (double *)(w + p.qt);
         if ((rc = stedc(n, batch, d, e, E, qt, n, (long)n * n, sub, d_info, st))) return rc;
@@ -65,14 +67,16 @@ static int heev(int dtype, int n, int batch, unsigned flags, void *A, long lda, 
     } else {
         if ((rc = stedc(n, batch, d, e, E, (double *)Z, ldz, sZ, sub, d_info, st))) return rc;
     }
-    prof_mark(4, st);
+    prof_mark(5, st);
     if (p.two_stage) {
         if ((rc = q2_apply(dtype, n, n, batch, V2, n, (long)n * n, tau2, Z, ldz, sZ, sub, st))) return rc;
+        prof_mark(6, st);
         rc = ormtr(dtype, n, n, batch, TRD2_B, A, lda, sA, tau, Z, ldz, sZ, sub, st);
     } else {
+        prof_mark(6, st);
         rc = ormtr(dtype, n, n, batch, 1, A, lda, sA, tau, Z, ldz, sZ, sub, st);
     }
-    prof_mark(5, st);
+    prof_mark(7, st);
     return rc;
 }
 
@@ -212,6 +216,6 @@ NAO_EXPORT int nao_geneig(int n, int batch, int dtype, unsigned flags, const voi
         g.sA = sWm; g.sB = sAX; g.sC = strideC; g.maskA = MASK_LOWER;
         if ((rc = gemm_launch(dtype, g, batch, st))) return rc;
     }
-    prof_mark(6, st);
+    prof_mark(8, st);
     return NAO_OK;
 }

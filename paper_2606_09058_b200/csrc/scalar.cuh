@@ -61,6 +61,20 @@ __device__ __forceinline__ cplx warp_sum(cplx v) {
     return v;
 }
 
+// asynchronous global -> shared copies (LDGSTS); pred = false zero-fills the destination
+__device__ __forceinline__ void cp_async8(void *smem, const void *g, bool pred) {
+    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    int sz = pred ? 8 : 0;
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(s), "l"(g), "r"(sz));
+}
+__device__ __forceinline__ void cp_async16(void *smem, const void *g, bool pred) {
+    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    int sz = pred ? 16 : 0;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(g), "r"(sz));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
+
 // Grid-wide barrier among the `nctas` CTAs that share `ctr` (all co-resident: cooperative launch).
 // `ordinal` = 1 for the first barrier on this counter, 2 for the second, ...
 __device__ __forceinline__ void group_barrier(unsigned *ctr, unsigned nctas, unsigned ordinal) {

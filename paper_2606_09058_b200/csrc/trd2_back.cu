@@ -17,7 +17,6 @@ namespace nao {
 
 static const int Q2_NBK = 32;                 // sweeps per diamond
 static const int Q2_LW = 96;                  // padded window rows (>= TRD2_B + Q2_NBK - 1)
-static const int Q2_NC = 32;                  // columns of Z per CTA
 static const int Q2_NT = 128;
 static const int Q2_LDV = 100, Q2_LDW = 36;   // shared-memory leading dimensions (conflict-free fragment loads)
 
@@ -112,20 +111,38 @@ template <class T> __device__ __forceinline__ T frag_out(const double (&acc)[4],
 template <> __device__ __forceinline__ double frag_out<double>(const double (&acc)[4], int q) { return acc[q]; }
 template <> __device__ __forceinline__ cplx frag_out<cplx>(const double (&acc)[4], int q) { return make_double2(acc[q], acc[2 + q]); }
 
+template <class T> struct Q2Cfg;
+template <> struct Q2Cfg<double> { static const int NC = 32; };     // columns of Z per CTA
+template <> struct Q2Cfg<cplx> { static const int NC = 16; };
+
+template <class T> __device__ __forceinline__ void cp_async_elem(T *s, const T *g, bool pred) {
+    if constexpr (sizeof(T) == 16) cp_async16(s, g, pred); else cp_async8(s, g, pred);
+}
+
 template <class T>
 __global__ void __launch_bounds__(Q2_NT) q2_apply_kernel(int n, int ncols, const T *V2, long ldv, long sV2, const T *Tst,
                                                          long sTst, T *Z, long ldz, long sZ) {
     typedef Ops<T> O;
-    constexpr int b = TRD2_B, NBK = Q2_NBK, LW = Q2_LW, NC = Q2_NC, LDV = Q2_LDV, LDW = Q2_LDW;
+    constexpr int b = TRD2_B, NBK = Q2_NBK, LW = Q2_LW, NC = Q2Cfg<T>::NC, NCT = NC / 8, LDV = Q2_LDV, LDW = Q2_LDW, LDT = NBK;
     const int item = blockIdx.y, c0 = blockIdx.x * NC;
     V2 += (long)item * sV2; Tst += (long)item * sTst; Z += (long)item * sZ;
     extern __shared__ __align__(16) unsigned char q2_smem[];
     T *sV = (T *)q2_smem;                 // [NBK][LDV]
-    T *sZ_ = sV + NBK * LDV;              // [NC][LDV]
-    T *sT = sZ_ + NC * LDV;               // [NBK][LDW]  T(i,k) at k*LDW + i
-    T *sW = sT + NBK * LDW;               // [NC][LDW]   W(ci,c) at c*LDW + ci
+    T *sZ_ = sV + NBK * LDV;              // [NC][LDV]   window of Z, kept across the windows of an S-block
+    T *sT = sZ_ + NC * LDV;               // [NBK][LDT]  T(i,k) at k*LDT + i
+    T *sW = sT + NBK * LDT;               // [NC][LDW]   W(ci,c) at c*LDW + ci
     T *sW2 = sW + NC * LDW;               // [NC][LDW]
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, lr = lane >> 2, lc = lane & 3;
+
+    // rows [ra, rb) of the window starting at global row w0 (Lw valid rows) from global memory, zero beyond Lw
+    auto load_z = [&](int w0, int Lw, int ra, int rb) {
+        const int nr = rb - ra;
+        for (int e = tid; e < nr * NC; e += Q2_NT) {
+            const int r = ra + e % nr, c = e / nr;
+            const bool ok = r < Lw && c0 + c < ncols;
+            cp_async_elem<T>(sZ_ + c * LDV + r, ok ? Z + (w0 + r) + (long)(c0 + c) * ldz : Z, ok);
+        }
+    };
 
     const int nsweeps = n - 1;
     const int nS = (nsweeps + NBK - 1) / NBK;
@@ -136,24 +153,26 @@ __global__ void __launch_bounds__(Q2_NT) q2_apply_kernel(int n, int ncols, const
         for (int k = 0; k < nwin; ++k) {
             const int w0 = s0 + 1 + k * b;
             const int Lw = min(s0 + ns - 1 + (k + 1) * b, n - 1) - w0 + 1;
-            __syncthreads();                                    // previous window's stores / smem reads are done
-            q2_load_v<T>(sV, V2, ldv, n, s0, ns, k, Q2_NT);
+            // ---- V (masked parallelogram), T and -- for the first window of the S-block -- Z, all asynchronous
+            for (int e = tid; e < LW * NBK; e += Q2_NT) {
+                const int r = e % LW, ci = e / LW;
+                const int s = s0 + ci, gr = w0 + r;
+                const bool ok = ci < ns && gr >= s + 1 + k * b && gr <= min(s + (k + 1) * b, n - 1);
+                cp_async_elem<T>(sV + ci * LDV + r, ok ? V2 + gr + (long)s * ldv : V2, ok);
+            }
             {
                 const T *Tg = Tst + (goff + k) * NBK * NBK;
-                for (int e = tid; e < NBK * NBK; e += Q2_NT) sT[(e / NBK) * LDW + (e % NBK)] = Tg[e];
+                for (int e = tid; e < NBK * NBK; e += Q2_NT) cp_async_elem<T>(sT + e, Tg + e, true);
             }
-            for (int e = tid; e < LW * NC; e += Q2_NT) {
-                const int r = e % LW, c = e / LW;
-                T v = O::zero();
-                if (r < Lw && c0 + c < ncols) v = Z[(w0 + r) + (long)(c0 + c) * ldz];
-                sZ_[c * LDV + r] = v;
-            }
+            if (k == 0) load_z(w0, Lw, 0, LW);
+            cp_async_commit();
+            cp_async_wait<0>();
             __syncthreads();
-            // ---- W = V^H Z_w : warp -> 8 rows (ci) x 32 columns
+            // ---- W = V^H Z_w : warp -> 8 rows (ci) x NC columns
             {
-                double acc[4][4];
+                double acc[NCT][4];
 #pragma unroll
-                for (int j = 0; j < 4; ++j)
+                for (int j = 0; j < NCT; ++j)
 #pragma unroll
                     for (int q = 0; q < 4; ++q) acc[j][q] = 0.0;
                 const T *ap = sV + (warp * 8 + lr) * LDV + lc;
@@ -162,42 +181,42 @@ __global__ void __launch_bounds__(Q2_NT) q2_apply_kernel(int n, int ncols, const
                 for (int k0 = 0; k0 < LW; k0 += 4) {
                     const T a = ap[k0];
 #pragma unroll
-                    for (int j = 0; j < 4; ++j) Frag<T, true, false>::mma(acc[j], a, bp[j * 8 * LDV + k0]);
+                    for (int j = 0; j < NCT; ++j) Frag<T, true, false>::mma(acc[j], a, bp[j * 8 * LDV + k0]);
                 }
 #pragma unroll
-                for (int j = 0; j < 4; ++j)
+                for (int j = 0; j < NCT; ++j)
 #pragma unroll
                     for (int q = 0; q < 2; ++q) sW[(j * 8 + 2 * lc + q) * LDW + warp * 8 + lr] = frag_out<T>(acc[j], q);
             }
             __syncthreads();
             // ---- W2 = T W
             {
-                double acc[4][4];
+                double acc[NCT][4];
 #pragma unroll
-                for (int j = 0; j < 4; ++j)
+                for (int j = 0; j < NCT; ++j)
 #pragma unroll
                     for (int q = 0; q < 4; ++q) acc[j][q] = 0.0;
-                const T *ap = sT + lc * LDW + warp * 8 + lr;
+                const T *ap = sT + lc * LDT + warp * 8 + lr;
                 const T *bp = sW + lr * LDW + lc;
 #pragma unroll
                 for (int k0 = 0; k0 < NBK; k0 += 4) {
-                    const T a = ap[k0 * LDW];
+                    const T a = ap[k0 * LDT];
 #pragma unroll
-                    for (int j = 0; j < 4; ++j) Frag<T, false, false>::mma(acc[j], a, bp[j * 8 * LDW + k0]);
+                    for (int j = 0; j < NCT; ++j) Frag<T, false, false>::mma(acc[j], a, bp[j * 8 * LDW + k0]);
                 }
 #pragma unroll
-                for (int j = 0; j < 4; ++j)
+                for (int j = 0; j < NCT; ++j)
 #pragma unroll
                     for (int q = 0; q < 2; ++q) sW2[(j * 8 + 2 * lc + q) * LDW + warp * 8 + lr] = frag_out<T>(acc[j], q);
             }
             __syncthreads();
-            // ---- Z_w -= V W2 : warp -> 24 rows x 32 columns, result straight to global memory
+            // ---- Z_w -= V W2 : warp -> 24 rows x NC columns, in place in shared memory
 #pragma unroll
             for (int i = 0; i < 3; ++i) {
                 const int m0 = (warp * 3 + i) * 8;
-                double acc[4][4];
+                double acc[NCT][4];
 #pragma unroll
-                for (int j = 0; j < 4; ++j)
+                for (int j = 0; j < NCT; ++j)
 #pragma unroll
                     for (int q = 0; q < 2; ++q) {
                         const T z = sZ_[(j * 8 + 2 * lc + q) * LDV + m0 + lr];
@@ -209,18 +228,39 @@ __global__ void __launch_bounds__(Q2_NT) q2_apply_kernel(int n, int ncols, const
                 for (int k0 = 0; k0 < NBK; k0 += 4) {
                     const T a = ap[k0 * LDV];
 #pragma unroll
-                    for (int j = 0; j < 4; ++j) Frag<T, false, true>::mma(acc[j], a, bp[j * 8 * LDW + k0]);
+                    for (int j = 0; j < NCT; ++j) Frag<T, false, true>::mma(acc[j], a, bp[j * 8 * LDW + k0]);
                 }
-                const int r = m0 + lr;
-                if (r < Lw) {
 #pragma unroll
-                    for (int j = 0; j < 4; ++j)
+                for (int j = 0; j < NCT; ++j)
 #pragma unroll
-                        for (int q = 0; q < 2; ++q) {
-                            const int c = c0 + j * 8 + 2 * lc + q;
-                            if (c < ncols) Z[(w0 + r) + (long)c * ldz] = frag_out<T>(acc[j], q);
-                        }
+                    for (int q = 0; q < 2; ++q) sZ_[(j * 8 + 2 * lc + q) * LDV + m0 + lr] = frag_out<T>(acc[j], q);
+            }
+            __syncthreads();
+            // ---- rows leaving the window go to global memory; the overlap with the next window moves to the top
+            const bool last = (k + 1 == nwin);
+            const int nout = last ? Lw : min(b, Lw);
+            for (int e = tid; e < nout * NC; e += Q2_NT) {
+                const int r = e % nout, c = e / nout;
+                if (c0 + c < ncols) Z[(w0 + r) + (long)(c0 + c) * ldz] = sZ_[c * LDV + r];
+            }
+            if (!last) {
+                const int nov = Lw - b;                      // rows shared with the next window (<= NBK - 1)
+                T keep[(NBK * NC + Q2_NT - 1) / Q2_NT];
+#pragma unroll
+                for (int it = 0; it < (NBK * NC + Q2_NT - 1) / Q2_NT; ++it) {
+                    const int e = tid + it * Q2_NT;
+                    if (e < nov * NC) keep[it] = sZ_[(e / nov) * LDV + b + e % nov];
                 }
+                __syncthreads();
+#pragma unroll
+                for (int it = 0; it < (NBK * NC + Q2_NT - 1) / Q2_NT; ++it) {
+                    const int e = tid + it * Q2_NT;
+                    if (e < nov * NC) sZ_[(e / nov) * LDV + e % nov] = keep[it];
+                }
+                const int Lw2 = min(s0 + ns - 1 + (k + 2) * b, n - 1) - (w0 + b) + 1;
+                load_z(w0 + b, Lw2, nov, LW);                // committed and awaited with the next window's V, T
+            } else {
+                __syncthreads();
             }
         }
     }
@@ -236,7 +276,8 @@ static int q2_apply_impl(int n, int ncols, int batch, const T *V2, long ldv, lon
     T *Tst = (T *)work;
     const int nS = ceil_div(n - 1, Q2_NBK), kmax = q2_nwin(n, 0);
     const size_t smem_t = (size_t)Q2_NBK * Q2_LDV * sizeof(T);
-    const size_t smem_a = (size_t)(2 * Q2_NBK * Q2_LDV + 3 * Q2_NBK * Q2_LDW) * sizeof(T);
+    const int NC = Q2Cfg<T>::NC;
+    const size_t smem_a = (size_t)((Q2_NBK + NC) * Q2_LDV + Q2_NBK * Q2_NBK + 2 * NC * Q2_LDW) * sizeof(T);
     static bool attr = false;
     if (!attr) {
         NAO_CUDA_CHECK(cudaFuncSetAttribute(q2_tfactor_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_t));
@@ -245,7 +286,7 @@ static int q2_apply_impl(int n, int ncols, int batch, const T *V2, long ldv, lon
     }
     q2_tfactor_kernel<T><<<dim3(nS, kmax, batch), 256, smem_t, st>>>(n, V2, ldv, sV2, tau2, sTau2, Tst, sTst);
     NAO_LAUNCHED();
-    q2_apply_kernel<T><<<dim3(ceil_div(ncols, Q2_NC), batch), Q2_NT, smem_a, st>>>(n, ncols, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ);
+    q2_apply_kernel<T><<<dim3(ceil_div(ncols, NC), batch), Q2_NT, smem_a, st>>>(n, ncols, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ);
     NAO_LAUNCHED();
     NAO_CUDA_CHECK(cudaGetLastError());
     return NAO_OK;
