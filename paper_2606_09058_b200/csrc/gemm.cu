@@ -46,12 +46,17 @@ __device__ __forceinline__ void mask_krange(int mask, int off, bool k_is_col, in
     }
 }
 
-template <bool CPLX> struct Cfg;
-template <> struct Cfg<false> {
+// NARROW: 128 x 64 tile for real products whose output has at most 64 columns (tall-skinny panels of he2hb)
+template <bool CPLX, bool NARROW = false> struct Cfg;
+template <> struct Cfg<false, true> {
+    typedef double T;
+    static const int BM = 128, BN = 64, BK = 16, WM = 32, WN = 32, STAGES = 4, PADX = 4, PADK = 4;
+};
+template <> struct Cfg<false, false> {
     typedef double T;
     static const int BM = 128, BN = 128, BK = 16, WM = 32, WN = 64, STAGES = 4, PADX = 4, PADK = 4;
 };
-template <> struct Cfg<true> {
+template <> struct Cfg<true, false> {
     typedef cplx T;
     static const int BM = 128, BN = 64, BK = 16, WM = 32, WN = 32, STAGES = 4, PADX = 2, PADK = 2;
 };
@@ -132,10 +137,10 @@ template <bool CPLX, int BX, int BK, int PADX, int PADK, bool XC> struct FastLoa
     __device__ __forceinline__ void advance() { g += kadv; }
 };
 
-template <bool CPLX, bool AXC, bool BXC, bool SCALE>
+template <bool CPLX, bool AXC, bool BXC, bool SCALE, bool NARROW>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 gemm_kernel(const GemmDesc hd, const GemmDesc *__restrict__ dd) {
-    typedef Cfg<CPLX> G;
+    typedef Cfg<CPLX, NARROW> G;
     typedef typename G::T T;
     constexpr int BM = G::BM, BN = G::BN, BK = G::BK, WM = G::WM, WN = G::WN, ST = G::STAGES;
     constexpr int MI = WM / 8, NI = WN / 8;
@@ -175,8 +180,10 @@ gemm_kernel(const GemmDesc hd, const GemmDesc *__restrict__ dd) {
     mask_krange(maskB, offB, BXC, n0, min(n0 + BN, N) - 1, kb, ke);
     kb = max(kb, 0); ke = min(ke, K);
     if (ks > 1) {
-        const int kchunk = ((K + ks - 1) / ks + BK - 1) / BK * BK;
-        kb = max(kb, slice * kchunk); ke = min(ke, (slice + 1) * kchunk);
+        // slices of the CLIPPED range: every slice of a tile carries the same work also under triangular masks
+        const int kb0 = kb / BK * BK;
+        const int kchunk = ((max(ke - kb0, 0) + ks - 1) / ks + BK - 1) / BK * BK;
+        kb = max(kb, kb0 + slice * kchunk); ke = min(ke, kb0 + (slice + 1) * kchunk);
     }
     const int kt0 = kb / BK;
     const int nkt = ke > kb ? (ke - 1) / BK + 1 - kt0 : 0;
@@ -363,20 +370,20 @@ gemm_kernel(const GemmDesc hd, const GemmDesc *__restrict__ dd) {
     }
 }
 
-template <bool CPLX> static size_t gemm_smem_bytes() {
-    typedef Cfg<CPLX> G;
+template <bool CPLX, bool NARROW> static size_t gemm_smem_bytes() {
+    typedef Cfg<CPLX, NARROW> G;
     size_t a = TileSize<G::BM, G::BK, G::PADX, G::PADK>::value, b = TileSize<G::BN, G::BK, G::PADX, G::PADK>::value;
     return G::STAGES * (a + b) * sizeof(typename G::T) + G::STAGES * G::BK * sizeof(double);
 }
 
-template <bool CPLX, bool AXC, bool BXC, bool SCALE>
+template <bool CPLX, bool AXC, bool BXC, bool SCALE, bool NARROW>
 static int launch_variant(const GemmDesc *hd, const GemmDesc *dd, int ngroups, int max_m, int max_n, int batch,
                           cudaStream_t st) {
-    typedef Cfg<CPLX> G;
+    typedef Cfg<CPLX, NARROW> G;
     static bool attr_set = false;
-    size_t smem = gemm_smem_bytes<CPLX>();
+    size_t smem = gemm_smem_bytes<CPLX, NARROW>();
     if (!attr_set) {
-        NAO_CUDA_CHECK(cudaFuncSetAttribute(gemm_kernel<CPLX, AXC, BXC, SCALE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        NAO_CUDA_CHECK(cudaFuncSetAttribute(gemm_kernel<CPLX, AXC, BXC, SCALE, NARROW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_set = true;
     }
     long tiles = (long)ceil_div(max_m, G::BM) * ceil_div(max_n, G::BN);
@@ -387,7 +394,7 @@ static int launch_variant(const GemmDesc *hd, const GemmDesc *dd, int ngroups, i
                                   (hd->ksplit > 1 ? hd->ksplit : 1)
                             : 0.0;
     const int pk = prof_kernel_begin(1, flops, st);
-    gemm_kernel<CPLX, AXC, BXC, SCALE><<<grid, GEMM_THREADS, smem, st>>>(dummy, dd);
+    gemm_kernel<CPLX, AXC, BXC, SCALE, NARROW><<<grid, GEMM_THREADS, smem, st>>>(dummy, dd);
     prof_kernel_end(1, pk, st);
     NAO_LAUNCHED();
     NAO_CUDA_CHECK(cudaGetLastError());
@@ -403,12 +410,20 @@ static int launch_impl(const GemmDesc *hd, const GemmDesc *dd, int ngroups, int 
     const bool axc = (opA == OP_N), bxc = (opB != OP_N);
     if (scale) {
         if (!(axc && bxc)) return NAO_ERR_UNSUPPORTED;
-        return launch_variant<CPLX, true, true, true>(hd, dd, ngroups, max_m, max_n, batch, st);
+        return launch_variant<CPLX, true, true, true, false>(hd, dd, ngroups, max_m, max_n, batch, st);
     }
-    if (axc) return bxc ? launch_variant<CPLX, true, true, false>(hd, dd, ngroups, max_m, max_n, batch, st)
-                        : launch_variant<CPLX, true, false, false>(hd, dd, ngroups, max_m, max_n, batch, st);
-    return bxc ? launch_variant<CPLX, false, true, false>(hd, dd, ngroups, max_m, max_n, batch, st)
-               : launch_variant<CPLX, false, false, false>(hd, dd, ngroups, max_m, max_n, batch, st);
+    if constexpr (!CPLX) {
+        if (max_n <= Cfg<false, true>::BN) {
+            if (axc) return bxc ? launch_variant<false, true, true, false, true>(hd, dd, ngroups, max_m, max_n, batch, st)
+                                : launch_variant<false, true, false, false, true>(hd, dd, ngroups, max_m, max_n, batch, st);
+            return bxc ? launch_variant<false, false, true, false, true>(hd, dd, ngroups, max_m, max_n, batch, st)
+                       : launch_variant<false, false, false, false, true>(hd, dd, ngroups, max_m, max_n, batch, st);
+        }
+    }
+    if (axc) return bxc ? launch_variant<CPLX, true, true, false, false>(hd, dd, ngroups, max_m, max_n, batch, st)
+                        : launch_variant<CPLX, true, false, false, false>(hd, dd, ngroups, max_m, max_n, batch, st);
+    return bxc ? launch_variant<CPLX, false, true, false, false>(hd, dd, ngroups, max_m, max_n, batch, st)
+               : launch_variant<CPLX, false, false, false, false>(hd, dd, ngroups, max_m, max_n, batch, st);
 }
 
 int gemm_launch(int dtype, const GemmDesc &d, int batch, cudaStream_t st) {

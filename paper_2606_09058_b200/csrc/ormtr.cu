@@ -40,9 +40,12 @@ __global__ void __launch_bounds__(256) larft_kernel(int kb, const T *G, long ldg
     __shared__ T s_g[ORM_KB];
     G += (long)blockIdx.x * sG; tau += (long)blockIdx.x * sTau; Tm += (long)blockIdx.x * sT;
     const int tid = threadIdx.x;
+    // column i+1 of G and tau_{i+1} are fetched while step i computes (the recurrence is latency bound)
+    T gnext = Ops<T>::zero(), tnext = tau[0];
     for (int i = 0; i < kb; ++i) {
-        const T ti = tau[i];
-        if (tid < i) s_g[tid] = G[tid + (long)i * ldg];
+        const T ti = tnext;
+        if (tid < i) s_g[tid] = gnext;
+        if (i + 1 < kb) { tnext = tau[i + 1]; if (tid < i + 1) gnext = G[tid + (long)(i + 1) * ldg]; }
         __syncthreads();
         if (tid < i) {
             // row tid of T(0:i,0:i) times g  (T upper: columns c >= tid)

@@ -178,10 +178,63 @@ __global__ void __launch_bounds__(QR_NT, 1) panel_qr_kernel(QrArgs<T> p) {
 }
 
 // ----------------------------------------------------------------------------------------------------------------
+// Small b x b algebra of a panel, one CTA per item:  T from (G = V^H V, tau) by the xLARFT recurrence,
+// M = T^H S0 T with S0 = V^H X, and the stacked coefficient matrix  B2 = [T ; -1/2 M]  (2b x b) so that
+//   W = X T - 1/2 V M = [X | V] B2   is one GEMM.      GS = [S0 | G] (b x 2b, ld b).
+// ----------------------------------------------------------------------------------------------------------------
+template <class T>
+__global__ void __launch_bounds__(256) he2hb_small_kernel(const T *GS, long sGS, const T *tau, long sTau, T *B2, long sB2) {
+    typedef Ops<T> O;
+    constexpr int b = TRD2_B, LD = b + 1;
+    extern __shared__ __align__(16) unsigned char sm_raw[];
+    T *sG = (T *)sm_raw;            // G, later S0
+    T *sT = sG + b * LD;            // T (dense, zeros below the diagonal)
+    T *sX = sT + b * LD;            // S0 T
+    __shared__ T s_tau[b];
+    GS += (long)blockIdx.x * sGS; tau += (long)blockIdx.x * sTau; B2 += (long)blockIdx.x * sB2;
+    const int tid = threadIdx.x;
+    for (int e = tid; e < b * b; e += 256) {
+        const int i = e % b, j = e / b;
+        sG[i * LD + j] = GS[(long)(b + j) * b + i];        // G(i,j), row-major in shared memory
+        sT[i * LD + j] = O::zero();
+    }
+    if (tid < b) s_tau[tid] = tau[tid];
+    __syncthreads();
+    for (int i = 0; i < b; ++i) {
+        if (tid < i) {
+            T acc = O::zero();
+            for (int c = tid; c < i; ++c) acc = O::fma(sT[tid * LD + c], sG[c * LD + i], acc);
+            sT[tid * LD + i] = O::sub(O::zero(), O::mul(s_tau[i], acc));
+        }
+        if (tid == i) sT[i * LD + i] = s_tau[i];
+        __syncthreads();
+    }
+    for (int e = tid; e < b * b; e += 256) {
+        const int i = e % b, j = e / b;
+        sG[i * LD + j] = GS[(long)j * b + i];              // S0(i,j)
+        B2[i + (long)j * 2 * b] = sT[i * LD + j];          // rows 0..b-1 of B2 = T
+    }
+    __syncthreads();
+    for (int e = tid; e < b * b; e += 256) {               // sX = S0 T : sX(i,j) = sum_{k<=j} S0(i,k) T(k,j)
+        const int j = e % b, i = e / b;
+        T acc = O::zero();
+        for (int k = 0; k <= j; ++k) acc = O::fma(sG[i * LD + k], sT[k * LD + j], acc);
+        sX[i * LD + j] = acc;
+    }
+    __syncthreads();
+    for (int e = tid; e < b * b; e += 256) {               // M(i,j) = sum_{k<=i} conj(T(k,i)) sX(k,j)
+        const int j = e % b, i = e / b;
+        T acc = O::zero();
+        for (int k = 0; k <= i; ++k) acc = O::add(acc, O::conj_mul(sT[k * LD + i], sX[k * LD + j]));
+        B2[(b + i) + (long)j * 2 * b] = O::scale(acc, -0.5);
+    }
+}
+
+// ----------------------------------------------------------------------------------------------------------------
 // he2hb driver
 // ----------------------------------------------------------------------------------------------------------------
 struct He2hbWork {
-    void *P3, *X, *G, *Tm, *S, *M, *part, *rowb, *splitk; unsigned *bar;
+    void *P4, *GS, *B2, *part, *rowb, *splitk; unsigned *bar;
     int Gq, chunk, ipl, ksX, ksS; size_t smem, bytes;
 };
 static int trd2_num_sms() {
@@ -203,20 +256,17 @@ static He2hbWork he2hb_plan(int dtype, int n, int batch, void *work) {
     w.Gq = std::max(1, std::min(nsm / w.ipl, ceil_div(m0, 32)));
     w.chunk = ceil_div(m0, w.Gq);
     w.smem = ((size_t)b * (w.chunk | 1) + w.chunk) * es;
-    // split-K factors: X = A22 V (m x b, k = m) and the b x b products
+    // split-K factors: X = A22 V (m x b, k = m) fills ~3 CTAs per SM-slot; the b x 2b product one slice per SM
     const int tilesX = ceil_div(n, 128) * batch;
-    w.ksX = std::max(1, std::min(std::min(2 * nsm / std::max(1, tilesX), ceil_div(n, 512)), 16));
+    w.ksX = std::max(1, std::min(std::min(3 * nsm / std::max(1, tilesX), ceil_div(n, 256)), 16));
     w.ksS = std::max(1, std::min(std::min(nsm / std::max(1, batch), ceil_div(n, 256)), 64));
     Arena ar(work, (size_t)-1);
-    w.P3 = ar.take((size_t)batch * n * 3 * b * es);            // [W | V | W], ld n, rows indexed globally
-    w.X = ar.take((size_t)batch * n * b * es);
-    w.G = ar.take((size_t)batch * b * b * es);
-    w.Tm = ar.take((size_t)batch * b * b * es);
-    w.S = ar.take((size_t)batch * b * b * es);
-    w.M = ar.take((size_t)batch * b * b * es);
+    w.P4 = ar.take((size_t)batch * n * 4 * b * es);            // [X | V | W | V], ld n, rows indexed globally
+    w.GS = ar.take((size_t)batch * 2 * b * b * es);
+    w.B2 = ar.take((size_t)batch * 2 * b * b * es);
     w.part = ar.take((size_t)batch * 2 * w.Gq * b * es);
     w.rowb = ar.take((size_t)batch * 2 * b * es);
-    w.splitk = ar.take((size_t)batch * std::max((size_t)w.ksX * n * b, (size_t)w.ksS * b * b) * es);
+    w.splitk = ar.take((size_t)batch * std::max((size_t)w.ksX * n * b, (size_t)w.ksS * 2 * b * b) * es);
     w.bar = (unsigned *)ar.take((size_t)batch * (ceil_div(n, b) + 1) * 4);
     w.bytes = ar.off;
     return w;
@@ -231,17 +281,19 @@ template <class T>
 static int he2hb_impl(int dtype, int n, int batch, T *A, long lda, long sA, T *tau, void *work, cudaStream_t st) {
     const int b = TRD2_B;
     He2hbWork w = he2hb_plan(dtype, n, batch, work);
+    const size_t small_smem = (size_t)3 * b * (b + 1) * sizeof(T);
     static bool attr = false;
     if (!attr) {
         NAO_CUDA_CHECK(cudaFuncSetAttribute(panel_qr_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, 210 * 1024));
+        NAO_CUDA_CHECK(cudaFuncSetAttribute(he2hb_small_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)small_smem));
         attr = true;
     }
     const int npanels = ceil_div(n, b) + 1;
     NAO_CUDA_CHECK(cudaMemsetAsync(w.bar, 0, (size_t)batch * npanels * 4, st));
     NAO_CUDA_CHECK(cudaMemsetAsync(tau, 0, (size_t)batch * n * sizeof(T), st));
-    T *P3 = (T *)w.P3, *X = (T *)w.X;
-    const long sP3 = (long)n * 3 * b, sX = (long)n * b, sBB = (long)b * b;
-    T *Wb = P3, *Vb = P3 + (long)n * b;            // column blocks of P3: W at 0, V at b, W copy at 2b
+    T *P4 = (T *)w.P4;
+    const long sP4 = (long)n * 4 * b, sGS = (long)2 * b * b;
+    T *Xb = P4, *Vb = P4 + (long)n * b, *Wb = P4 + (long)n * 2 * b, *Vb2 = P4 + (long)n * 3 * b;
     int panel = 0;
     for (int j0 = 0; n - j0 - b > 1; j0 += b, ++panel) {
         const int m = n - j0 - b, jr = j0 + b;      // panel rows start at global row jr
@@ -260,38 +312,30 @@ static int he2hb_impl(int dtype, int n, int batch, T *A, long lda, long sA, T *t
             NAO_CUDA_CHECK(cudaLaunchCooperativeKernel((void *)panel_qr_kernel<T>, dim3(nit * a.G), dim3(QR_NT), args, smem, st));
             NAO_LAUNCHED();
         }
-        // 2. explicit V (m x b, zeros above the unit diagonal) at rows jr.. of the V block; T factor
-        if (int rc = build_v(dtype, n, j0, b, b, A, lda, sA, Vb + jr, n, sP3, batch, st)) return rc;
-        GemmDesc g = gemm_desc(OP_C, OP_N, b, b, m, 1.0, Vb + jr, n, Vb + jr, n, 0.0, w.G, b);
-        g.sA = sP3; g.sB = sP3; g.sC = sBB;
-        if (int rc = gemm_splitk(dtype, g, batch, std::min(w.ksS, ceil_div(m, 256)), w.splitk, st)) return rc;
-        if (int rc = larft(dtype, b, w.G, b, sBB, tau + j0, n, w.Tm, sBB, batch, st)) return rc;
+        // 2. explicit V (m x b, zeros above the unit diagonal) at rows jr.. of both V blocks
+        if (int rc = build_v(dtype, n, j0, b, b, A, lda, sA, Vb + jr, n, sP4, batch, st)) return rc;
+        if (int rc = copy_matrix(dtype, m, b, Vb + jr, n, sP4, Vb2 + jr, n, sP4, batch, 0, st)) return rc;
         // 3. X = A22 V : lower triangle as stored + strictly lower triangle transposed
         T *A22 = A + jr + (long)jr * lda;
-        const int ksx = std::min(w.ksX, ceil_div(m, 512));
-        GemmDesc x1 = gemm_desc(OP_N, OP_N, m, b, m, 1.0, A22, lda, Vb + jr, n, 0.0, X + jr, n);
-        x1.sA = sA; x1.sB = sP3; x1.sC = sX; x1.maskA = MASK_LOWER;
+        const int ksx = std::min(w.ksX, ceil_div(m, 256));
+        GemmDesc x1 = gemm_desc(OP_N, OP_N, m, b, m, 1.0, A22, lda, Vb + jr, n, 0.0, Xb + jr, n);
+        x1.sA = sA; x1.sB = sP4; x1.sC = sP4; x1.maskA = MASK_LOWER;
         if (int rc = gemm_splitk(dtype, x1, batch, ksx, w.splitk, st)) return rc;
-        GemmDesc x2 = gemm_desc(OP_C, OP_N, m, b, m, 1.0, A22, lda, Vb + jr, n, 1.0, X + jr, n);
-        x2.sA = sA; x2.sB = sP3; x2.sC = sX; x2.maskA = MASK_SLOWER;
+        GemmDesc x2 = gemm_desc(OP_C, OP_N, m, b, m, 1.0, A22, lda, Vb + jr, n, 1.0, Xb + jr, n);
+        x2.sA = sA; x2.sB = sP4; x2.sC = sP4; x2.maskA = MASK_SLOWER;
         if (int rc = gemm_splitk(dtype, x2, batch, ksx, w.splitk, st)) return rc;
-        // 4. W0 = X T  (into the W block), S = V^H W0, M = T^H S, W = W0 - 1/2 V M
-        GemmDesc xt = gemm_desc(OP_N, OP_N, m, b, b, 1.0, X + jr, n, w.Tm, b, 0.0, Wb + jr, n);
-        xt.sA = sX; xt.sB = sBB; xt.sC = sP3; xt.maskB = MASK_UPPER;
-        if (int rc = gemm_launch(dtype, xt, batch, st)) return rc;
-        GemmDesc s1 = gemm_desc(OP_C, OP_N, b, b, m, 1.0, Vb + jr, n, Wb + jr, n, 0.0, w.S, b);
-        s1.sA = sP3; s1.sB = sP3; s1.sC = sBB;
-        if (int rc = gemm_splitk(dtype, s1, batch, std::min(w.ksS, ceil_div(m, 256)), w.splitk, st)) return rc;
-        GemmDesc m1 = gemm_desc(OP_C, OP_N, b, b, b, 1.0, w.Tm, b, w.S, b, 0.0, w.M, b);
-        m1.sA = sBB; m1.sB = sBB; m1.sC = sBB; m1.maskA = MASK_UPPER;
-        if (int rc = gemm_launch(dtype, m1, batch, st)) return rc;
-        GemmDesc w1 = gemm_desc(OP_N, OP_N, m, b, b, -0.5, Vb + jr, n, w.M, b, 1.0, Wb + jr, n);
-        w1.sA = sP3; w1.sB = sBB; w1.sC = sP3;
+        // 4. [S0 | G] = V^H [X | V] ; B2 = [T ; -1/2 T^H S0 T] ; W = [X | V] B2
+        GemmDesc gs = gemm_desc(OP_C, OP_N, b, 2 * b, m, 1.0, Vb + jr, n, Xb + jr, n, 0.0, w.GS, b);
+        gs.sA = sP4; gs.sB = sP4; gs.sC = sGS;
+        if (int rc = gemm_splitk(dtype, gs, batch, std::min(w.ksS, ceil_div(m, 256)), w.splitk, st)) return rc;
+        he2hb_small_kernel<T><<<batch, 256, small_smem, st>>>((const T *)w.GS, sGS, tau + j0, n, (T *)w.B2, sGS);
+        NAO_LAUNCHED();
+        GemmDesc w1 = gemm_desc(OP_N, OP_N, m, b, 2 * b, 1.0, Xb + jr, n, w.B2, 2 * b, 0.0, Wb + jr, n);
+        w1.sA = sP4; w1.sB = sGS; w1.sC = sP4;
         if (int rc = gemm_launch(dtype, w1, batch, st)) return rc;
-        if (int rc = copy_matrix(dtype, m, b, Wb + jr, n, sP3, P3 + (long)n * 2 * b + jr, n, sP3, batch, 0, st)) return rc;
-        // 5. A22 -= [W V] [V W]^H, lower tiles
-        GemmDesc u = gemm_desc(OP_N, OP_C, m, m, 2 * b, -1.0, Wb + jr, n, Vb + jr, n, 1.0, A22, lda);
-        u.sA = sP3; u.sB = sP3; u.sC = sA; u.cmode = 1;
+        // 5. A22 -= V W^H + W V^H = [V W] [W V]^H, lower tiles
+        GemmDesc u = gemm_desc(OP_N, OP_C, m, m, 2 * b, -1.0, Vb + jr, n, Wb + jr, n, 1.0, A22, lda);
+        u.sA = sP4; u.sB = sP4; u.sC = sA; u.cmode = 1;
         if (int rc = gemm_launch(dtype, u, batch, st)) return rc;
     }
     NAO_CUDA_CHECK(cudaGetLastError());

@@ -134,13 +134,22 @@ __global__ void __launch_bounds__(Q2_NT) q2_apply_kernel(int n, int ncols, const
     T *sW2 = sW + NC * LDW;               // [NC][LDW]
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, lr = lane >> 2, lc = lane & 3;
 
-    // rows [ra, rb) of the window starting at global row w0 (Lw valid rows) from global memory, zero beyond Lw
-    auto load_z = [&](int w0, int Lw, int ra, int rb) {
-        const int nr = rb - ra;
-        for (int e = tid; e < nr * NC; e += Q2_NT) {
-            const int r = ra + e % nr, c = e / nr;
-            const bool ok = r < Lw && c0 + c < ncols;
-            cp_async_elem<T>(sZ_ + c * LDV + r, ok ? Z + (w0 + r) + (long)(c0 + c) * ldz : Z, ok);
+    // rows [ra, LW) of the window starting at global row w0 (Lw valid rows) from global memory, zero beyond Lw.
+    // warp <-> columns c = warp, warp + 4, ...; lane <-> rows: no integer division anywhere in the window loop
+    constexpr int NWARP = Q2_NT / 32;
+    auto load_z = [&](int w0, int Lw, int ra) {
+#pragma unroll
+        for (int c = warp; c < NC; c += NWARP) {
+            const bool cok = c0 + c < ncols;
+            const T *zc = Z + w0 + (long)(c0 + c) * ldz;
+#pragma unroll
+            for (int rr = 0; rr < LW; rr += 32) {
+                const int r = ra + rr + lane;
+                if (r < LW) {
+                    const bool ok = cok && r < Lw;
+                    cp_async_elem<T>(sZ_ + c * LDV + r, ok ? zc + r : Z, ok);
+                }
+            }
         }
     };
 
@@ -154,17 +163,24 @@ __global__ void __launch_bounds__(Q2_NT) q2_apply_kernel(int n, int ncols, const
             const int w0 = s0 + 1 + k * b;
             const int Lw = min(s0 + ns - 1 + (k + 1) * b, n - 1) - w0 + 1;
             // ---- V (masked parallelogram), T and -- for the first window of the S-block -- Z, all asynchronous
-            for (int e = tid; e < LW * NBK; e += Q2_NT) {
-                const int r = e % LW, ci = e / LW;
-                const int s = s0 + ci, gr = w0 + r;
-                const bool ok = ci < ns && gr >= s + 1 + k * b && gr <= min(s + (k + 1) * b, n - 1);
-                cp_async_elem<T>(sV + ci * LDV + r, ok ? V2 + gr + (long)s * ldv : V2, ok);
+#pragma unroll
+            for (int ci = warp; ci < NBK; ci += NWARP) {
+                const int s = s0 + ci;
+                const int a0 = s + 1 + k * b - w0, a1 = min(s + (k + 1) * b, n - 1) - w0;     // valid window rows of column ci
+                const T *vc = V2 + w0 + (long)s * ldv;
+#pragma unroll
+                for (int rr = 0; rr < LW; rr += 32) {
+                    const int r = rr + lane;
+                    const bool ok = ci < ns && r >= a0 && r <= a1;
+                    cp_async_elem<T>(sV + ci * LDV + r, ok ? vc + r : V2, ok);
+                }
             }
             {
                 const T *Tg = Tst + (goff + k) * NBK * NBK;
+#pragma unroll
                 for (int e = tid; e < NBK * NBK; e += Q2_NT) cp_async_elem<T>(sT + e, Tg + e, true);
             }
-            if (k == 0) load_z(w0, Lw, 0, LW);
+            if (k == 0) load_z(w0, Lw, 0);
             cp_async_commit();
             cp_async_wait<0>();
             __syncthreads();
@@ -239,26 +255,25 @@ __global__ void __launch_bounds__(Q2_NT) q2_apply_kernel(int n, int ncols, const
             // ---- rows leaving the window go to global memory; the overlap with the next window moves to the top
             const bool last = (k + 1 == nwin);
             const int nout = last ? Lw : min(b, Lw);
-            for (int e = tid; e < nout * NC; e += Q2_NT) {
-                const int r = e % nout, c = e / nout;
-                if (c0 + c < ncols) Z[(w0 + r) + (long)(c0 + c) * ldz] = sZ_[c * LDV + r];
+#pragma unroll
+            for (int c = warp; c < NC; c += NWARP) {
+                if (c0 + c < ncols) {
+                    T *zc = Z + w0 + (long)(c0 + c) * ldz;
+                    for (int r = lane; r < nout; r += 32) zc[r] = sZ_[c * LDV + r];
+                }
             }
             if (!last) {
-                const int nov = Lw - b;                      // rows shared with the next window (<= NBK - 1)
-                T keep[(NBK * NC + Q2_NT - 1) / Q2_NT];
+                const int nov = Lw - b;                      // rows shared with the next window (<= NBK - 1 <= 31)
+                T keep[NC / NWARP];
 #pragma unroll
-                for (int it = 0; it < (NBK * NC + Q2_NT - 1) / Q2_NT; ++it) {
-                    const int e = tid + it * Q2_NT;
-                    if (e < nov * NC) keep[it] = sZ_[(e / nov) * LDV + b + e % nov];
-                }
+                for (int jj = 0; jj < NC / NWARP; ++jj)
+                    if (lane < nov) keep[jj] = sZ_[(warp + jj * NWARP) * LDV + b + lane];
                 __syncthreads();
 #pragma unroll
-                for (int it = 0; it < (NBK * NC + Q2_NT - 1) / Q2_NT; ++it) {
-                    const int e = tid + it * Q2_NT;
-                    if (e < nov * NC) sZ_[(e / nov) * LDV + e % nov] = keep[it];
-                }
+                for (int jj = 0; jj < NC / NWARP; ++jj)
+                    if (lane < nov) sZ_[(warp + jj * NWARP) * LDV + lane] = keep[jj];
                 const int Lw2 = min(s0 + ns - 1 + (k + 2) * b, n - 1) - (w0 + b) + 1;
-                load_z(w0 + b, Lw2, nov, LW);                // committed and awaited with the next window's V, T
+                load_z(w0 + b, Lw2, nov);                    // committed and awaited with the next window's V, T
             } else {
                 __syncthreads();
             }

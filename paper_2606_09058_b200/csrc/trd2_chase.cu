@@ -141,15 +141,35 @@ __global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
         __syncthreads();
     };
     // diagonal block rows/cols [g0, g0+L): load (Hermitian completion) / store (lower part)
+    // (all loads of a block are issued before the first shared-memory store: one L2 round trip per block)
     auto load_D = [&](int g0, int L) {
-        for (int e = tid; e < b * b; e += CH_NT) {
-            const int i = e & (b - 1), cc = e >> 6;
+        T buf[b * b / CH_NT];
+#pragma unroll
+        for (int it = 0; it < b * b / CH_NT; ++it) {
+            const int e = tid + it * CH_NT, i = e & (b - 1), cc = e >> 6;
             T v = O::zero();
-            if (i < L && cc < L) {
-                if (i >= cc) v = ldcg(AB + (i - cc) + (long)(g0 + cc) * ld);
-                else v = O::conj(ldcg(AB + (cc - i) + (long)(g0 + i) * ld));
-            }
-            sD[cc * LDS + i] = v;
+            if (i < L && cc < L) v = (i >= cc) ? ldcg(AB + (i - cc) + (long)(g0 + cc) * ld) : ldcg(AB + (cc - i) + (long)(g0 + i) * ld);
+            buf[it] = v;
+        }
+#pragma unroll
+        for (int it = 0; it < b * b / CH_NT; ++it) {
+            const int e = tid + it * CH_NT, i = e & (b - 1), cc = e >> 6;
+            sD[cc * LDS + i] = (i >= cc) ? buf[it] : O::conj(buf[it]);
+        }
+    };
+    auto load_O = [&](int q0, int Lq, int r0, int Lp) {
+        T buf[b * b / CH_NT];
+#pragma unroll
+        for (int it = 0; it < b * b / CH_NT; ++it) {
+            const int e = tid + it * CH_NT, i = e & (b - 1), cc = e >> 6;
+            T v = O::zero();
+            if (i < Lq && cc < Lp) v = ldcg(AB + (q0 + i - r0 - cc) + (long)(r0 + cc) * ld);
+            buf[it] = v;
+        }
+#pragma unroll
+        for (int it = 0; it < b * b / CH_NT; ++it) {
+            const int e = tid + it * CH_NT, i = e & (b - 1), cc = e >> 6;
+            sO[cc * LDS + i] = buf[it];
         }
     };
     auto store_D = [&](int g0, int L) {
@@ -193,12 +213,7 @@ __global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
                 __syncthreads();
             }
             // load O = B[q0 : q0+Lq, r0 : r0+Lp] and D = B[q0.., q0..]
-            for (int e = tid; e < b * b; e += CH_NT) {
-                const int i = e & (b - 1), cc = e >> 6;
-                T v = O::zero();
-                if (i < Lq && cc < Lp) v = ldcg(AB + (q0 + i - r0 - cc) + (long)(r0 + cc) * ld);
-                sO[cc * LDS + i] = v;
-            }
+            load_O(q0, Lq, r0, Lp);
             load_D(q0, Lq);
             __syncthreads();
             // w = O v_prev ; O -= tau_prev w v_prev^H

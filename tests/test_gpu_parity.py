@@ -195,6 +195,62 @@ def test_fermi_level_against_oracle_and_closed_forms(nao):
     assert abs(mu - mu_ref) <= TOL_MU
 
 
+# ------------------------------------------------------------------------------------------ two-stage reduction
+def test_two_stage_config2_replica_against_oracle(nao):
+    """Config 2 recipe at 32 atoms (n = 416 real, 2 spins) through dense->band->tridiagonal (NAO_TRD_TWO_STAGE):
+    6 panels, bulge chasing over 7 band blocks with a ragged last block, 13 diamonds of chase reflectors."""
+    prob = make_config(2, nat=32)
+    check_against_oracle(prob, run_path(nao, prob, flags=nao.NAO_TRD_TWO_STAGE), oracle.solve_problem(prob))
+
+
+def test_two_stage_config3_replica_against_oracle(nao):
+    """Config 3 recipe at 16 atoms (2N = 416 complex, block S) through the two-stage reduction."""
+    prob = make_config(3, nat=16)
+    check_against_oracle(prob, run_path(nao, prob, flags=nao.NAO_TRD_TWO_STAGE), oracle.solve_problem(prob))
+
+
+@pytest.mark.parametrize("n", [66, 67, 129, 193, 200])
+@pytest.mark.parametrize("cplx", [False, True])
+def test_two_stage_heev_ragged_sizes(nao, n, cplx):
+    """nao_heev with the two-stage path at sizes around the band width (64): one short panel, partial band blocks,
+    partial diamonds.  Eigenvalues against the Jacobi oracle; vectors through residual and orthogonality."""
+    rng = np.random.default_rng(100 + n)
+    A = rng.standard_normal((2, n, n))
+    if cplx:
+        A = A + 1j * rng.standard_normal((2, n, n))
+    A = A + np.swapaxes(A.conj(), -1, -2)
+    E, Z, info = nao.heev(to_dev(A), flags=nao.NAO_TRD_TWO_STAGE)
+    assert int(info.abs().max()) == 0
+    E = E.cpu().numpy(); Zn = to_np(Z)
+    for b in range(2):
+        e_or, _ = oracle.heev(A[b])
+        assert np.abs(E[b] - e_or).max() <= TOL_E
+        assert np.abs(A[b] @ Zn[b] - Zn[b] * E[b]).max() <= 1e-11
+        assert np.abs(Zn[b].conj().T @ Zn[b] - np.eye(n)).max() <= 1e-12
+
+
+def test_two_stage_structured_inputs(nao):
+    """Inputs whose panels are rank deficient or already banded: tight-binding chain (tridiagonal), block-diagonal,
+    identity, and a matrix that is already a band of width 64.  Closed form for the chain (north_star)."""
+    n = 300
+    k = np.arange(1, n + 1)
+    chain = np.diag(np.full(n - 1, -1.0), 1) + np.diag(np.full(n - 1, -1.0), -1)
+    rng = np.random.default_rng(3)
+    blk = np.zeros((n, n)); 
+    for a, bnd in ((0, 100), (100, 170), (170, 300)):
+        M = rng.standard_normal((bnd - a, bnd - a)); blk[a:bnd, a:bnd] = M + M.T
+    band = np.triu(np.tril(rng.standard_normal((n, n)), 64), -64); band = band + band.T
+    mats = np.stack([chain, blk, np.eye(n), band])
+    E, Z, info = nao.heev(to_dev(mats), flags=nao.NAO_TRD_TWO_STAGE)
+    assert int(info.abs().max()) == 0
+    E = E.cpu().numpy(); Zn = to_np(Z)
+    assert np.abs(E[0] - np.sort(-2.0 * np.cos(k * np.pi / (n + 1)))).max() <= 1e-12
+    for b in range(4):
+        assert np.abs(E[b] - np.linalg.eigvalsh(mats[b])).max() <= 1e-11
+        assert np.abs(mats[b] @ Zn[b] - Zn[b] * E[b]).max() <= 1e-11
+        assert np.abs(Zn[b].T @ Zn[b] - np.eye(n)).max() <= 1e-12
+
+
 # ------------------------------------------------------------------------------------------ building blocks
 @pytest.mark.parametrize("cplx", [False, True])
 def test_gemm_core_all_ops(nao, cplx):
