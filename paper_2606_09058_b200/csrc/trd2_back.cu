@@ -184,20 +184,37 @@ __global__ void __launch_bounds__(Q2_NT) q2_apply_kernel(int n, int ncols, const
             cp_async_commit();
             cp_async_wait<0>();
             __syncthreads();
-            // ---- W = V^H Z_w : warp -> 8 rows (ci) x NC columns
+            // Zero structure of the parallelogram: column ci of V is non-zero only in rows ci .. ci + b - 1, so
+            //   W rows 8w..8w+7 need window rows 8w .. 8w + b + 7 only (18 of 24 k-steps), and
+            //   Z_w row tile m0 needs columns ci in [m0 - b + 1, m0 + 7]           (72 of 96 k-steps over the 12 tiles).
+            // ---- W = V^H Z_w : warp -> 8 rows (ci) x NC columns; fragments of step k0+4 are loaded before the DMMAs of k0
             {
                 double acc[NCT][4];
 #pragma unroll
                 for (int j = 0; j < NCT; ++j)
 #pragma unroll
                     for (int q = 0; q < 4; ++q) acc[j][q] = 0.0;
-                const T *ap = sV + (warp * 8 + lr) * LDV + lc;
-                const T *bp = sZ_ + lr * LDV + lc;
-#pragma unroll 4
-                for (int k0 = 0; k0 < LW; k0 += 4) {
-                    const T a = ap[k0];
+                constexpr int KS1 = (b + 8) / 4;                                  // 18 k-steps
+                const T *ap = sV + (warp * 8 + lr) * LDV + lc + warp * 8;
+                const T *bp = sZ_ + lr * LDV + lc + warp * 8;
+                T a_c = ap[0], b_c[NCT];
 #pragma unroll
-                    for (int j = 0; j < NCT; ++j) Frag<T, true, false>::mma(acc[j], a, bp[j * 8 * LDV + k0]);
+                for (int j = 0; j < NCT; ++j) b_c[j] = bp[j * 8 * LDV];
+#pragma unroll
+                for (int ks = 0; ks < KS1; ++ks) {
+                    T a_n = a_c, b_n[NCT];
+#pragma unroll
+                    for (int j = 0; j < NCT; ++j) b_n[j] = b_c[j];
+                    if (ks + 1 < KS1) {
+                        a_n = ap[(ks + 1) * 4];
+#pragma unroll
+                        for (int j = 0; j < NCT; ++j) b_n[j] = bp[j * 8 * LDV + (ks + 1) * 4];
+                    }
+#pragma unroll
+                    for (int j = 0; j < NCT; ++j) Frag<T, true, false>::mma(acc[j], a_c, b_c[j]);
+                    a_c = a_n;
+#pragma unroll
+                    for (int j = 0; j < NCT; ++j) b_c[j] = b_n[j];
                 }
 #pragma unroll
                 for (int j = 0; j < NCT; ++j)
@@ -205,7 +222,7 @@ __global__ void __launch_bounds__(Q2_NT) q2_apply_kernel(int n, int ncols, const
                     for (int q = 0; q < 2; ++q) sW[(j * 8 + 2 * lc + q) * LDW + warp * 8 + lr] = frag_out<T>(acc[j], q);
             }
             __syncthreads();
-            // ---- W2 = T W
+            // ---- W2 = T W   (T upper triangular: rows 8w.. need k >= 8w)
             {
                 double acc[NCT][4];
 #pragma unroll
@@ -214,8 +231,7 @@ __global__ void __launch_bounds__(Q2_NT) q2_apply_kernel(int n, int ncols, const
                     for (int q = 0; q < 4; ++q) acc[j][q] = 0.0;
                 const T *ap = sT + lc * LDT + warp * 8 + lr;
                 const T *bp = sW + lr * LDW + lc;
-#pragma unroll
-                for (int k0 = 0; k0 < NBK; k0 += 4) {
+                for (int k0 = warp * 8; k0 < NBK; k0 += 4) {
                     const T a = ap[k0 * LDT];
 #pragma unroll
                     for (int j = 0; j < NCT; ++j) Frag<T, false, false>::mma(acc[j], a, bp[j * 8 * LDW + k0]);
@@ -226,10 +242,11 @@ __global__ void __launch_bounds__(Q2_NT) q2_apply_kernel(int n, int ncols, const
                     for (int q = 0; q < 2; ++q) sW2[(j * 8 + 2 * lc + q) * LDW + warp * 8 + lr] = frag_out<T>(acc[j], q);
             }
             __syncthreads();
-            // ---- Z_w -= V W2 : warp -> 24 rows x NC columns, in place in shared memory
+            // ---- Z_w -= V W2 : warp -> row tiles w, w+4, w+8 (balanced: 18 k-steps per warp), in place in shared memory
 #pragma unroll
             for (int i = 0; i < 3; ++i) {
-                const int m0 = (warp * 3 + i) * 8;
+                const int m0 = (warp + i * NWARP) * 8;
+                const int klo = max(0, m0 - b + 1) / 4 * 4, khi = min(NBK, m0 + 8);    // columns ci of V that touch the tile
                 double acc[NCT][4];
 #pragma unroll
                 for (int j = 0; j < NCT; ++j)
@@ -240,11 +257,23 @@ __global__ void __launch_bounds__(Q2_NT) q2_apply_kernel(int n, int ncols, const
                     }
                 const T *ap = sV + lc * LDV + m0 + lr;
                 const T *bp = sW2 + lr * LDW + lc;
+                T a_c = ap[klo * LDV], b_c[NCT];
 #pragma unroll
-                for (int k0 = 0; k0 < NBK; k0 += 4) {
-                    const T a = ap[k0 * LDV];
+                for (int j = 0; j < NCT; ++j) b_c[j] = bp[j * 8 * LDW + klo];
+                for (int k0 = klo; k0 < khi; k0 += 4) {
+                    T a_n = a_c, b_n[NCT];
 #pragma unroll
-                    for (int j = 0; j < NCT; ++j) Frag<T, false, true>::mma(acc[j], a, bp[j * 8 * LDW + k0]);
+                    for (int j = 0; j < NCT; ++j) b_n[j] = b_c[j];
+                    if (k0 + 4 < khi) {
+                        a_n = ap[(k0 + 4) * LDV];
+#pragma unroll
+                        for (int j = 0; j < NCT; ++j) b_n[j] = bp[j * 8 * LDW + k0 + 4];
+                    }
+#pragma unroll
+                    for (int j = 0; j < NCT; ++j) Frag<T, false, true>::mma(acc[j], a_c, b_c[j]);
+                    a_c = a_n;
+#pragma unroll
+                    for (int j = 0; j < NCT; ++j) b_c[j] = b_n[j];
                 }
 #pragma unroll
                 for (int j = 0; j < NCT; ++j)
