@@ -37,8 +37,24 @@ static const int TRD_CH = 96;        // rows of V/W cached in shared memory per 
 static const int TRD_CHP = TRD_CH + 1;
 static const int TRD_PASS = 128;     // rows finalised per pass in phase A
 
+#ifdef NAO_TRACE
+#ifndef TRD_TRACE_CTA
+#define TRD_TRACE_CTA 0
+#endif
+__device__ unsigned long long g_trd_trace[16];
+#define TRD_T(k)                                                                                   \
+    do {                                                                                           \
+        if (blockIdx.x == TRD_TRACE_CTA && threadIdx.x == 0) {                                     \
+            unsigned long long t__; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t__));      \
+            g_trd_trace[k] += t__ - t_last; t_last = t__;                                          \
+        }                                                                                          \
+    } while (0)
+#else
+#define TRD_T(k)
+#endif
+
 template <class T> struct Hv;
-template <> struct Hv<double> { static const int SW = 64, CPT = 32, HS = 1, CB = 4; };
+template <> struct Hv<double> { static const int SW = 32, CPT = 16, HS = 2, CB = 4; };   // 64 x 32 units: finer load balance
 template <> struct Hv<cplx> { static const int SW = 32, CPT = 16, HS = 2, CB = 2; };
 
 template <class T> struct TrdArgs {
@@ -267,10 +283,20 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
     auto getV = [&](int r, int k) -> T { return cached ? sV[k * TRD_CHP + (r - r0)] : A[r + (long)(j0 + k) * lda]; };
     auto getW = [&](int r, int k) -> T { return cached ? sW[k * TRD_CHP + (r - r0)] : Wp[r + (long)k * n]; };
 
+#ifdef NAO_TRACE
+    unsigned long long t_last; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_last));
+#endif
     for (int i = 0; i <= p.nbp; ++i) {
         const int j = j0 + i;
+        TRD_T(0);
         const int ra = max(r0, j);                 // first own row still in play
         // =============================== phase A ===============================
+        // row j of the panel's V and W (columns < i resp. < i-1): needed by every CTA, fetched first so that the
+        // loads overlap the reduction below
+        if (tid < i) {
+            s_vrow[tid] = ldcg(A + j + (long)(j0 + tid) * lda);
+            if (tid < i - 1) s_wrow[tid] = ldcg(Wp + j + (long)tid * n);
+        }
         if (i > 0) {
             const int nk = i - 1;
             // (1) reduce the partials of phase B(i-1): t1, t2 (k < i-1) and v^H A v, fixed order
@@ -279,11 +305,21 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
                 const int k = idx < TRD_NB ? idx : idx - TRD_NB;
                 T s = O::zero();
                 if (k < nk)
-                    for (int qq = part; qq < G; qq += 4) s = O::add(s, ldcg(pt + (long)qq * 2 * TRD_NB + idx));
+                    for (int q0 = part; q0 < G; q0 += 32) {           // 8 loads in flight, summed in a fixed order
+                        T bq[8];
+#pragma unroll
+                        for (int u = 0; u < 8; ++u) bq[u] = (q0 + 4 * u < G) ? ldcg(pt + (long)(q0 + 4 * u) * 2 * TRD_NB + idx) : O::zero();
+#pragma unroll
+                        for (int u = 0; u < 8; ++u) s = O::add(s, bq[u]);
+                    }
                 s_red4[part][idx] = s;
                 if (warp == 0) {
-                    double sv = 0.0;
-                    for (int qq = lane; qq < G; qq += 32) sv += ldcg(pvav + qq);
+                    double sv = 0.0, bv[5];
+#pragma unroll
+                    for (int u = 0; u < 5; ++u) bv[u] = (lane + 32 * u < G) ? ldcg(pvav + lane + 32 * u) : 0.0;
+#pragma unroll
+                    for (int u = 0; u < 5; ++u) sv += bv[u];
+                    for (int qq = lane + 160; qq < G; qq += 32) sv += ldcg(pvav + qq);
                     sv = warp_sum(sv);
                     if (lane == 0) s_vav = sv;
                 }
@@ -291,13 +327,14 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
                 if (tid < 2 * TRD_NB)
                     s_t[tid] = O::add(O::add(s_red4[0][tid], s_red4[1][tid]), O::add(s_red4[2][tid], s_red4[3][tid]));
                 __syncthreads();
-                if (tid == 0) {
-                    double s = s_vav;
-                    for (int k2 = 0; k2 < nk; ++k2) s -= 2.0 * O::real(O::conj_mul(s_t[k2], s_t[TRD_NB + k2]));
-                    s_alpha = -0.5 * O::abs2(s_tau) * s;
+                if (warp == 0) {
+                    double c = lane < nk ? 2.0 * O::real(O::conj_mul(s_t[lane], s_t[TRD_NB + lane])) : 0.0;
+                    c = warp_sum(c);
+                    if (lane == 0) s_alpha = -0.5 * O::abs2(s_tau) * (s_vav - c);
                 }
                 __syncthreads();
             }
+            TRD_T(1);
             // (2) w_{i-1} for the own rows r >= j and (redundantly, every CTA) for row j
             const int nown = max(0, r1 - ra);
             const bool extra = !(j >= r0 && j < r1);
@@ -306,15 +343,35 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
             const int perp = units_per_warp(HS * (nbkp * (nbkp + 1) / 2), G);
             for (int base = 0; base < nloc; base += TRD_PASS) {
                 const int np = min(TRD_PASS, nloc - base);
-                for (int lg = 0; lg < np; lg += 32) {
-                    if (lg + lane < np) {
-                        const int l = base + lg + lane;
-                        const int r = l < nown ? ra + l : j;
-                        const int Send = HS * (r / TRD_TB) + HS - 1;
-                        T s = O::zero();
-                        for (int S = HS * bminp + warp; S <= Send; S += TRD_NW) s = O::add(s, ldcg(Prow + (long)S * n + r));
-                        s_part[warp * TRD_PASS + lg + lane] = s;
+                {
+                    // row sums of the strips: lane <-> 4 rows of the pass, warp <-> strips S = warp, warp + NW, ...;
+                    // 4 x 4 independent L2 loads in flight per thread, every row summed in ascending strip order
+                    constexpr int NG = TRD_PASS / 32, UB = 4;
+                    int rr[NG], se[NG]; T acc[NG];
+                    int smax = -1;
+#pragma unroll
+                    for (int g4 = 0; g4 < NG; ++g4) {
+                        const int lp = g4 * 32 + lane, l = base + lp;
+                        rr[g4] = l < nown ? ra + l : j;
+                        se[g4] = lp < np ? HS * (rr[g4] / TRD_TB) + HS - 1 : -1;
+                        smax = max(smax, se[g4]);
+                        acc[g4] = O::zero();
                     }
+                    for (int S = HS * bminp + warp; S <= smax; S += UB * TRD_NW) {
+                        T bq[NG][UB];
+#pragma unroll
+                        for (int g4 = 0; g4 < NG; ++g4)
+#pragma unroll
+                            for (int u = 0; u < UB; ++u)
+                                bq[g4][u] = (S + u * TRD_NW <= se[g4]) ? ldcg(Prow + (long)(S + u * TRD_NW) * n + rr[g4]) : O::zero();
+#pragma unroll
+                        for (int g4 = 0; g4 < NG; ++g4)
+#pragma unroll
+                            for (int u = 0; u < UB; ++u) acc[g4] = O::add(acc[g4], bq[g4][u]);
+                    }
+#pragma unroll
+                    for (int g4 = 0; g4 < NG; ++g4)
+                        if (g4 * 32 + lane < np) s_part[warp * TRD_PASS + g4 * 32 + lane] = acc[g4];
                 }
                 __syncthreads();
                 for (int lp = tid; lp < np; lp += TRD_NT) {
@@ -332,8 +389,8 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
                         y = O::add(y, ldcg(Pcol + (long)(bminp + Jp + kk * perp - ua) * n + r));
                     T acc = y;
                     for (int k = 0; k < nk; ++k) {
-                        const T v = own ? getV(r, k) : ldcg(A + r + (long)(j0 + k) * lda);
-                        const T w = own ? getW(r, k) : ldcg(Wp + r + (long)k * n);
+                        const T v = own ? getV(r, k) : s_vrow[k];          // the extra row is row j
+                        const T w = own ? getW(r, k) : s_wrow[k];
                         acc = O::sub(acc, O::add(O::mul(v, s_t[k]), O::mul(w, s_t[TRD_NB + k])));
                     }
                     const T vr = (r == j) ? O::one() : getV(r, i - 1);
@@ -348,13 +405,8 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
                 __syncthreads();
             }
         }
+        TRD_T(2);
         const bool do_col = (i < p.nbp) || (j == n - 1);
-        if (do_col) {
-            if (tid < i) {
-                s_vrow[tid] = ldcg(A + j + (long)(j0 + tid) * lda);
-                if (tid < i - 1) s_wrow[tid] = ldcg(Wp + j + (long)tid * n);
-            }
-        }
         __syncthreads();
         if (do_col) {
             double nrm = 0.0;
@@ -370,12 +422,18 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
             if (tid == 0) pn[g] = nrm;
         }
         if (i == p.nbp) break;
+        TRD_T(3);
         group_barrier(bar, G, ++bar_ord);
+        TRD_T(4);
 
         // =============================== phase B ===============================
         if (warp == 0) {
-            double s = 0.0;
-            for (int qq = lane; qq < G; qq += 32) s += ldcg(pn + qq);
+            double s = 0.0, bn[5];
+#pragma unroll
+            for (int u = 0; u < 5; ++u) bn[u] = (lane + 32 * u < G) ? ldcg(pn + lane + 32 * u) : 0.0;
+#pragma unroll
+            for (int u = 0; u < 5; ++u) s += bn[u];
+            for (int qq = lane + 160; qq < G; qq += 32) s += ldcg(pn + qq);
             s = warp_sum(s);
             if (lane == 0) {
                 T alpha0 = ldcg(acol + j + 1);
@@ -399,6 +457,7 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
             }
         }
         __syncthreads();
+        TRD_T(5);
         const T scale = s_scale;
         auto vval = [&](int x) -> T {
             if (x < j + 1 || x >= n) return O::zero();
@@ -431,10 +490,13 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
             if (tid < 2 * TRD_NB)
                 pt[(long)g * 2 * TRD_NB + tid] = O::add(O::add(s_red4[0][tid], s_red4[1][tid]), O::add(s_red4[2][tid], s_red4[3][tid]));
         }
+        TRD_T(6);
         double vav = hemv_warp<T>(A, lda, n, j, nblk, G, g, acol, scale, sx + warp * SW, Prow, Pcol);
         vav = block_sum_d(vav, s_dred);
         if (tid == 0) pvav[g] = vav;
+        TRD_T(7);
         group_barrier(bar, G, ++bar_ord);
+        TRD_T(8);
     }
 }
 
@@ -468,7 +530,7 @@ static TrdWork trd_plan(int dtype, int n, int batch, void *work) {
     w.Wp = ar.take((size_t)batch * n * 4 * TRD_NB * es);
     w.acol = ar.take((size_t)batch * n * es);
     w.pt = ar.take((size_t)batch * w.G * 2 * TRD_NB * es);
-    w.Prow = ar.take((size_t)batch * (dtype == NAO_COMPLEX ? 2 : 1) * w.nblk * n * es);
+    w.Prow = ar.take((size_t)batch * 2 * w.nblk * n * es);          // HS = 2 strips per block column
     w.Pcol = ar.take((size_t)batch * w.nblk * n * es);
     w.pn = (double *)ar.take((size_t)batch * w.G * 8);
     w.pvav = (double *)ar.take((size_t)batch * w.G * 8);
@@ -538,6 +600,19 @@ static int hetrd_impl(int dtype, int n, int batch, T *A, long lda, long sA, doub
     }
     return NAO_OK;
 }
+
+#ifdef NAO_TRACE
+}  // namespace nao
+NAO_EXPORT int nao_debug_trd_trace(double *out_us, int reset) {
+    unsigned long long h[16];
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(h, nao::g_trd_trace, sizeof(h));
+    for (int i = 0; i < 16; ++i) out_us[i] = h[i] * 1e-3;
+    if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(nao::g_trd_trace, z, sizeof(z)); }
+    return 0;
+}
+namespace nao {
+#endif
 
 int hetrd(int dtype, int n, int batch, void *A, long lda, long sA, double *d, double *e, void *tau, void *work,
           cudaStream_t st) {
