@@ -174,6 +174,10 @@ __device__ __forceinline__ double hemv_warp(const T *__restrict__ A, long lda, i
     };
     strip_begin(Jp, h);
     load(cur, Jp, h, Irel, 0);
+    // x for the rows of the NEXT unit is fetched (L2) one unit ahead, like the matrix batches
+    T xr_n[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) xr_n[k] = vval((bmin + Irel) * TRD_TB + q + 16 * k);
 
     for (int u = u0; u < u1; ++u) {
         int Jn = Jp, hn = h, In = Irel + 1;
@@ -188,7 +192,11 @@ __device__ __forceinline__ double hemv_warp(const T *__restrict__ A, long lda, i
         const int cb0 = (bmin + Jp) * TRD_TB + h * SW + hh * CPT;
         T xr[4], rs[4];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) { xr[k] = vval(rbase + 16 * k); rs[k] = O::zero(); }
+        for (int k = 0; k < 4; ++k) { xr[k] = xr_n[k]; rs[k] = O::zero(); }
+        if (more) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) xr_n[k] = vval((bmin + In) * TRD_TB + q + 16 * k);
+        }
 #pragma unroll
         for (int b = 0; b < NBATCH; ++b) {
             if (b + 1 < NBATCH) load(nxt, Jp, h, Irel, b + 1);
