@@ -179,9 +179,9 @@ def main():
     torch.cuda.synchronize()
     assert int(info.abs().max()) == 0, "numerical failure: info=%s" % info.tolist()
 
-    # ---- timed region: K full steps, device-resident inputs (708 MB of H at c2: larger than the 126 MB L2)
+    # ---- timed region: K full steps, device-resident inputs (708 MB of H at c2: larger than the 126 MB L2);
+    #      no profiling events inside it
     sampler = ClockSampler(local); sampler.start()
-    nao.profile_enable(True)
     l0 = nao.launch_count()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
@@ -192,10 +192,43 @@ def main():
     barrier()
     ms = ev0.elapsed_time(ev1) / args.steps
     launches = (nao.launch_count() - l0) // args.steps
+    clocks = sampler.stop()
+
+    # ---- one more step with the library's event timers on: phase boundaries and per-launch timers of the two
+    #      kernel classes (slot 0 = hetrd_panel_kernel with its algorithmic HBM bytes, slot 1 = gemm_kernel with flops)
+    nao.profile_enable(True)
+    step()
+    torch.cuda.synchronize()
     phases = nao.profile_read()
     kpanel = nao.profile_kernel(0)
+    kgemm = nao.profile_kernel(1)
     nao.profile_enable(False)
-    clocks = sampler.stop()
+    prof_steps = 1
+
+    # ---- the same step through the two-stage reduction (dense -> band -> tridiagonal), for comparison
+    ms_two_stage, phases_two = None, None
+    try:
+        f2 = flags | nao.NAO_TRD_TWO_STAGE
+        work2 = torch.empty(nao.geneig_workspace(prob.n, prob.batch, dt, f2) + 256, dtype=torch.uint8, device=dev)
+
+        def step2():
+            S.copy_(S0)
+            E2, C2, info2 = nao.geneig(H, S, flags=f2, work=work2)
+            mu2, F2 = nao.fermi_mu(E2, weights, prob.n_electrons, prob.kT)
+            nao.density_matrix(C2, F2, out=Dbuf)
+            return E2
+        step2(); torch.cuda.synchronize()
+        ev0.record()
+        for _ in range(2):
+            E2 = step2()
+        ev1.record(); torch.cuda.synchronize()
+        ms_two_stage = ev0.elapsed_time(ev1) / 2
+        nao.profile_enable(True); step2(); torch.cuda.synchronize()
+        phases_two = nao.profile_read(); nao.profile_enable(False)
+        assert float((E2 - E).abs().max()) <= 1e-9, "two-stage eigenvalues differ from one-stage"
+        del work2
+    except Exception as exc:       # reported, never hidden
+        phases_two = {"error": str(exc)}
 
     # later SCF steps reuse the factor of S: same path with NAO_S_FACTORED
     ev0.record()
@@ -233,10 +266,22 @@ def main():
             pass
         hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
         hbm_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6.65 TB/s (B200_PROFILING.md)"
-        panel_ms = kpanel["ms"] / args.steps
-        panel_bytes = kpanel["work"] / args.steps
+        panel_ms = kpanel["ms"] / prof_steps
+        panel_bytes = kpanel["work"] / prof_steps
         achieved = panel_bytes / (panel_ms * 1e-3) / 1e9 if panel_ms > 0 else 0.0
         fl = useful_flops(prob)
+        gemm_tf = kgemm["work"] / (kgemm["ms"] * 1e-3) / 1e12 if kgemm["ms"] > 0 else 0.0
+        # DRAM traffic of the dominant kernel: ratio (dram bytes / algorithmic bytes) of the committed ncu --set full
+        # capture (profiles/r01_traffic.csv) times this run's algorithmic bytes per launch
+        traffic, traffic_src = None, None
+        try:
+            import csv
+            with open(os.path.join(ROOT, "profiles", "r01_traffic.csv")) as fh:
+                tj = [r for r in csv.DictReader(fh) if r["kernel"] == "hetrd_panel_kernel"][0]
+            traffic = float(tj["dram_bytes_per_algorithmic_byte"]) * panel_bytes / max(1, kpanel["launches"] // prof_steps)
+            traffic_src = tj["source"]
+        except Exception:
+            pass
         line = {
             "metric": "s per SCF eigensolve+density matrix", "value": ms * 1e-3, "unit": "s", "n_gpus": world,
             "steps": args.steps, "warmup": W, "ms_per_step": ms, "higher_is_better": False, "scaling": "weak",
@@ -250,9 +295,16 @@ def main():
             "ms_per_step_later_scf_steps": ms_later,
             "phases_ms": {k: round(v, 3) for k, v in phases.items()},
             "roofline": {"kernel": kpanel["name"], "bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s",
-                         "frac": achieved / hbm_peak, "traffic": None, "peak_source": hbm_src,
-                         "kernel_ms_per_step": panel_ms, "launches_per_step": kpanel["launches"] // max(1, args.steps),
-                         "algorithmic_bytes_per_step": panel_bytes},
+                         "frac": achieved / hbm_peak, "traffic": traffic, "traffic_source": traffic_src, "peak_source": hbm_src,
+                         "kernel_ms_per_step": panel_ms, "launches_per_step": kpanel["launches"] // prof_steps,
+                         "algorithmic_bytes_per_step": panel_bytes,
+                         "algorithmic_bytes_per_launch": panel_bytes / max(1, kpanel["launches"] // prof_steps)},
+            "roofline_gemm": {"kernel": kgemm["name"], "bound": "tensor", "achieved": gemm_tf, "peak": FP64_DMMA_PEAK_TFLOPS,
+                              "unit": "TFLOP/s", "frac": gemm_tf / FP64_DMMA_PEAK_TFLOPS,
+                              "peak_source": "derived: 148 SMs x 128 flop/clk x 1.965 GHz (DESIGN.md 5); cuBLAS DGEMM measures 35.6",
+                              "kernel_ms_per_step": kgemm["ms"] / prof_steps, "launches_timed": kgemm["launches"],
+                              "executed_flops_timed": kgemm["work"]},
+            "two_stage": {"ms_per_step": ms_two_stage, "phases_ms": phases_two and {k: round(v, 3) if isinstance(v, float) else v for k, v in phases_two.items()}},
             "e2e": {"value": ms_e2e * 1e-3, "unit": "s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
             "gpu_launches": int(launches) * args.steps,
             "clocks": clocks,
