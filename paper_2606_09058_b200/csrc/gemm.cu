@@ -111,9 +111,9 @@ __device__ __forceinline__ bool mask_all_kept(int mask, int off, int r0, int r1,
 // Fast tile loader: 16-byte cp.async, one running global pointer per thread, compile-time shared-memory offsets.
 // Used for k-tiles that lie entirely inside the operand (no edge, no mask boundary, aligned); everything else goes
 // through load_tile.  The NCH chunks of a thread are issued in 4 parts so that the copies interleave with the DMMAs.
-template <bool CPLX, int BX, int BK, int PADX, int PADK, bool XC> struct FastLoad {
+template <bool CPLX, int BX, int BK, int PADX, int PADK, bool XC, bool AL16> struct FastLoad {
     typedef typename Cfg<CPLX>::T T;
-    static const int VEC = CPLX ? 1 : 2;                       // elements per 16-byte chunk
+    static const int VEC = (CPLX || !AL16) ? 1 : 2;            // elements per chunk (16 bytes; 8 bytes for misaligned real operands)
     static const int NCH = BX * BK / (VEC * GEMM_THREADS);     // chunks per thread per tile
     static const int P = XC ? BX / VEC : BK / VEC;             // chunks along the contiguous direction
     static const int STEP = GEMM_THREADS / P;                  // other-index distance between a thread's chunks
@@ -132,12 +132,15 @@ template <bool CPLX, int BX, int BK, int PADX, int PADK, bool XC> struct FastLoa
         constexpr int SSTR = XC ? STEP * (BX + PADX) : STEP * (BK + PADK);
         constexpr int c0 = PART * NCH / 4, c1 = (PART + 1) * NCH / 4;
 #pragma unroll
-        for (int c = c0; c < c1; ++c) cp_async16(s + soff + c * SSTR, g + c * cstride, true);
+        for (int c = c0; c < c1; ++c) {
+            if constexpr (CPLX || AL16) cp_async16(s + soff + c * SSTR, g + c * cstride, true);
+            else cp_async8(s + soff + c * SSTR, g + c * cstride, true);
+        }
     }
     __device__ __forceinline__ void advance() { g += kadv; }
 };
 
-template <bool CPLX, bool AXC, bool BXC, bool SCALE, bool NARROW>
+template <bool CPLX, bool AXC, bool BXC, bool SCALE, bool NARROW, bool AL16>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 gemm_kernel(const GemmDesc hd, const GemmDesc *__restrict__ dd) {
     typedef Cfg<CPLX, NARROW> G;
@@ -227,12 +230,12 @@ gemm_kernel(const GemmDesc hd, const GemmDesc *__restrict__ dd) {
     constexpr int b_sx = BXC ? 1 : (BK + G::PADK), b_sk = BXC ? (BN + G::PADX) : 1;
 
     // ---- tile loading: fast (interior, aligned) or generic, decided per k-tile, uniformly over the CTA
-    FastLoad<CPLX, BM, BK, G::PADX, G::PADK, AXC> fa;
-    FastLoad<CPLX, BN, BK, G::PADX, G::PADK, BXC> fb;
+    FastLoad<CPLX, BM, BK, G::PADX, G::PADK, AXC, AL16> fa;
+    FastLoad<CPLX, BN, BK, G::PADX, G::PADK, BXC, AL16> fb;
     fa.init(A, lda, m0, kt0 * BK);
     fb.init(B, ldb, n0, kt0 * BK);
-    const bool a_al = CPLX || ((((size_t)A) & 15) == 0 && (lda & 1) == 0 && ((AXC ? m0 : 0) & 1) == 0);
-    const bool b_al = CPLX || ((((size_t)B) & 15) == 0 && (ldb & 1) == 0 && ((BXC ? n0 : 0) & 1) == 0);
+    const bool a_al = CPLX || !AL16 || ((((size_t)A) & 15) == 0 && (lda & 1) == 0 && ((AXC ? m0 : 0) & 1) == 0);
+    const bool b_al = CPLX || !AL16 || ((((size_t)B) & 15) == 0 && (ldb & 1) == 0 && ((BXC ? n0 : 0) & 1) == 0);
     const bool a_in = a_al && (m0 + BM <= M), b_in = b_al && (n0 + BN <= N);
     auto a_fast = [&](int k0) -> bool {
         if (!a_in || k0 < kb || k0 + BK > ke) return false;
@@ -376,14 +379,14 @@ template <bool CPLX, bool NARROW> static size_t gemm_smem_bytes() {
     return G::STAGES * (a + b) * sizeof(typename G::T) + G::STAGES * G::BK * sizeof(double);
 }
 
-template <bool CPLX, bool AXC, bool BXC, bool SCALE, bool NARROW>
-static int launch_variant(const GemmDesc *hd, const GemmDesc *dd, int ngroups, int max_m, int max_n, int batch,
-                          cudaStream_t st) {
+template <bool CPLX, bool AXC, bool BXC, bool SCALE, bool NARROW, bool AL16>
+static int launch_variant2(const GemmDesc *hd, const GemmDesc *dd, int ngroups, int max_m, int max_n, int batch,
+                           cudaStream_t st) {
     typedef Cfg<CPLX, NARROW> G;
     static bool attr_set = false;
     size_t smem = gemm_smem_bytes<CPLX, NARROW>();
     if (!attr_set) {
-        NAO_CUDA_CHECK(cudaFuncSetAttribute(gemm_kernel<CPLX, AXC, BXC, SCALE, NARROW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        NAO_CUDA_CHECK(cudaFuncSetAttribute(gemm_kernel<CPLX, AXC, BXC, SCALE, NARROW, AL16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_set = true;
     }
     long tiles = (long)ceil_div(max_m, G::BM) * ceil_div(max_n, G::BN);
@@ -394,11 +397,26 @@ static int launch_variant(const GemmDesc *hd, const GemmDesc *dd, int ngroups, i
                                   (hd->ksplit > 1 ? hd->ksplit : 1)
                             : 0.0;
     const int pk = prof_kernel_begin(1, flops, st);
-    gemm_kernel<CPLX, AXC, BXC, SCALE, NARROW><<<grid, GEMM_THREADS, smem, st>>>(dummy, dd);
+    gemm_kernel<CPLX, AXC, BXC, SCALE, NARROW, AL16><<<grid, GEMM_THREADS, smem, st>>>(dummy, dd);
     prof_kernel_end(1, pk, st);
     NAO_LAUNCHED();
     NAO_CUDA_CHECK(cudaGetLastError());
     return NAO_OK;
+}
+
+// Real operands that are not 16-byte aligned (odd row offsets such as Z + jb + 1, odd leading dimensions) take the
+// instantiation whose fast loader copies 8 bytes at a time; device-side descriptors keep the 16-byte variant, which checks
+// the alignment per CTA and falls back to the generic loader.
+template <bool CPLX, bool AXC, bool BXC, bool SCALE, bool NARROW>
+static int launch_variant(const GemmDesc *hd, const GemmDesc *dd, int ngroups, int max_m, int max_n, int batch,
+                          cudaStream_t st) {
+    if constexpr (!CPLX && !SCALE) {
+        if (hd) {
+            const bool al = (((size_t)hd->A | (size_t)hd->B) & 15) == 0 && ((hd->lda | hd->ldb | hd->sA | hd->sB) & 1) == 0;
+            if (!al) return launch_variant2<CPLX, AXC, BXC, SCALE, NARROW, false>(hd, dd, ngroups, max_m, max_n, batch, st);
+        }
+    }
+    return launch_variant2<CPLX, AXC, BXC, SCALE, NARROW, true>(hd, dd, ngroups, max_m, max_n, batch, st);
 }
 
 // the operand layouts (and the presence of scale factors) select the kernel instantiation; for grouped launches every
