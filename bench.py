@@ -150,7 +150,8 @@ def main():
     nao.lib()
     W = max(args.warmup, 3)
 
-    prob = make_config(WORKLOADS[args.workload]["idx"], seed=rank)       # replicas: each rank its own seed
+    from paper_2606_09058_b200.replicas import replica_seed
+    prob = make_config(WORKLOADS[args.workload]["idx"], seed=replica_seed(rank))       # replicas: each rank its own seed
     flags = nao.NAO_NC_BLOCK_S if prob.nc_block_s else 0
     dt = nao.NAO_COMPLEX if prob.is_complex else nao.NAO_REAL
     # host (pinned) and device copies
@@ -253,10 +254,8 @@ def main():
     h2d = Hh.numel() * Hh.element_size() + Sh.numel() * Sh.element_size()
     d2h = Dh.numel() * Dh.element_size() + Eh.numel() * Eh.element_size()
 
-    t = torch.tensor([ms, ms_e2e, ms_later], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms, ms_e2e, ms_later = [float(x) for x in t.tolist()]
+    from paper_2606_09058_b200.replicas import max_over_ranks
+    ms, ms_e2e, ms_later = max_over_ranks([ms, ms_e2e, ms_later], dist, dev)
 
     if rank == 0:
         peaks = {}
