@@ -315,3 +315,49 @@ def test_config2_full_size_properties(nao):
     assert abs(ne - prob.n_electrons) <= 1e-7
     mu_ref, f_ref = oracle.fermi(got["e"], prob.weights, prob.n_electrons, prob.kT)
     assert abs(got["mu"] - mu_ref) <= TOL_MU
+
+
+def test_config3_full_size_certificate(nao):
+    """BASELINE config 3 at full size (2N = 9984 complex, S real 4992, NAO_NC_BLOCK_S), the other headline workload.
+    The Jacobi oracle would need ~40 core-hours here, so the a-posteriori certificate of SURVEY.md 8c is used: with
+    F = C^H S C - I and R = H C - S C diag(e), congruence bounds the error of every eigenvalue by
+    (||R||_2 ||C||_2 + max|e| ||F||_2) / (1 - ||F||_2); the products are formed on the GPU by torch (cuBLAS, a checker
+    that shares nothing with the product path).  D is checked on sampled entries from its definition, plus Tr(D S) = N_e."""
+    prob = make_config(3)
+    n = prob.n
+    H = torch.from_numpy(prob.H).to(DEV)
+    S = torch.from_numpy(prob.S.copy()).to(DEV)
+    E, C, info = nao.geneig(H, S, flags=nao.NAO_NC_BLOCK_S)
+    assert int(info.abs().max()) == 0
+    mu, F = nao.fermi_mu(E, prob.weights, prob.n_electrons, prob.kT)
+    D = nao.density_matrix(C, F)
+    e = E[0]
+    assert bool((e[1:] >= e[:-1]).all())
+    Cm = C[0].T                                           # column-major item -> mathematical matrix
+    Hm = torch.from_numpy(prob.H_full(0)).to(DEV)
+    Sm = torch.from_numpy(prob.S_full(0)).to(DEV).to(Hm.dtype)
+    SC = Sm @ Cm
+    Fm = Cm.mH @ SC
+    Fm.diagonal().sub_(1.0)
+    orth = float(Fm.abs().max())
+    R = Hm @ Cm - SC * e[None, :]
+    resid = float(R.abs().max())
+    assert orth <= TOL_ORTH
+    assert resid <= 1e-10
+    # Frobenius norms bound the 2-norms
+    fF = float(torch.linalg.norm(Fm)); fR = float(torch.linalg.norm(R)); cN = float(torch.linalg.norm(Cm, ord=2))
+    bound = (fR * cN + float(e.abs().max()) * fF) / (1.0 - fF)
+    assert bound <= TOL_E, bound
+    Dm = D[0].T
+    ne = float((Dm * Sm.T).sum().real) * prob.weights[0]          # Tr(D S)
+    assert abs(ne - prob.n_electrons) <= 1e-7
+    assert float((Dm - Dm.mH).abs().max()) <= 1e-14
+    f = F[0].cpu().numpy().astype(np.longdouble)
+    Ch = Cm.cpu().numpy()
+    Dh = Dm.cpu().numpy()
+    rng = np.random.default_rng(9)
+    for (i, j) in rng.integers(0, n, size=(48, 2)):
+        dij = np.sum(f * Ch[i].astype(np.clongdouble) * np.conj(Ch[j]).astype(np.clongdouble))
+        assert abs(Dh[i, j] - complex(dij)) <= 1e-12
+    mu_ref, _ = oracle.fermi(E.cpu().numpy(), prob.weights, prob.n_electrons, prob.kT)
+    assert abs(mu - mu_ref) <= TOL_MU
