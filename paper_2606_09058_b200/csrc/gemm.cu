@@ -159,7 +159,12 @@ gemm_kernel(const GemmDesc hd, const GemmDesc *__restrict__ dd) {
     if (M <= 0 || N <= 0) return;
     const int tiles_m = (M + BM - 1) / BM, tiles_n = (N + BN - 1) / BN;
     if ((int)blockIdx.x >= tiles_m * tiles_n) return;
-    const int tm = blockIdx.x % tiles_m, tn = blockIdx.x / tiles_m;
+    // supertile raster: CTAs that run together cover GS tile rows x a few tile columns, so that the A and B panels
+    // they share stay in L2 (a plain column-of-tiles order re-reads A once per tile column)
+    constexpr int GS = 8;
+    const int bid = blockIdx.x, gsize = GS * tiles_n, gid = bid / gsize, first_m = gid * GS;
+    const int gsz = min(tiles_m - first_m, GS);
+    const int tm = first_m + (bid % gsize) % gsz, tn = (bid % gsize) / gsz;
     const int m0 = tm * BM, n0 = tn * BN;
     const int cmode = d.cmode;
     if (cmode == 1 && n0 > m0 + BM - 1) return;

@@ -286,20 +286,36 @@ __global__ void __launch_bounds__(256) dc_secular_kernel(DcBuf b, const DcNode *
 }
 
 // zhat_i = sign(w_i) sqrt | prod_j (d_i - lambda_j) / prod_{j != i} (d_i - d_j) |
+// 32 values of i per CTA (lanes, coalesced rows of Q), the j-range split over the 8 warps; the 8 partial products are
+// multiplied in a fixed order
 __global__ void __launch_bounds__(256) dc_zhat_kernel(DcBuf b, const DcNode *__restrict__ nodes, int maxnodes) {
+    __shared__ double part[8][32];
     const int node = blockIdx.y, item = blockIdx.z, n = b.n;
     const DcNode nd = nodes[node];
     const int K = b.out[(long)item * maxnodes + node].K;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= K) return;
+    if ((int)blockIdx.x * 32 >= K) return;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int i = blockIdx.x * 32 + lane;
     const long ib = (long)item * n + nd.off;
     const double *Qb = b.Q + (long)item * b.sQ + nd.off + (long)nd.off * b.ldq;
     const double *dlam = b.dlam + ib;
-    const double di = dlam[i];
-    double p = Qb[i + (long)i * b.ldq];
-    for (int j = 0; j < K; ++j)
-        if (j != i) p *= Qb[i + (long)j * b.ldq] / (di - dlam[j]);
-    b.zhat[ib + i] = copysign(sqrt(fabs(p)), b.wz[ib + i]);
+    double p = 1.0;
+    if (i < K) {
+        const double di = dlam[i];
+        const int jc = (K + 7) / 8, j0 = w * jc, j1 = min(K, j0 + jc);
+        for (int j = j0; j < j1; ++j) {
+            const double q = Qb[i + (long)j * b.ldq];
+            p *= (j == i) ? q : q / (di - dlam[j]);
+        }
+    }
+    part[w][lane] = p;
+    __syncthreads();
+    if (w == 0 && i < K) {
+        double t = part[0][lane];
+#pragma unroll
+        for (int k = 1; k < 8; ++k) t *= part[k][lane];
+        b.zhat[ib + i] = copysign(sqrt(fabs(t)), b.wz[ib + i]);
+    }
 }
 
 // column j of S (grouped row order): s_i = zhat_i / (d_i - lambda_j), normalised
@@ -461,7 +477,7 @@ int stedc(int n, int batch, double *d, double *e, double *evals, double *Qout, l
         NAO_LAUNCHED();
         dc_secular_kernel<<<dim3(ceil_div(Nmax, 8), nn, batch), 256, 0, st>>>(w.b, nodes, p.maxnodes, d_info);
         NAO_LAUNCHED();
-        dc_zhat_kernel<<<dim3(ceil_div(Nmax, 256), nn, batch), 256, 0, st>>>(w.b, nodes, p.maxnodes);
+        dc_zhat_kernel<<<dim3(ceil_div(Nmax, 32), nn, batch), 256, 0, st>>>(w.b, nodes, p.maxnodes);
         NAO_LAUNCHED();
         dc_vectors_kernel<<<dim3(Nmax, nn, batch), 128, 0, st>>>(w.b, nodes, p.maxnodes);
         NAO_LAUNCHED();
