@@ -313,12 +313,12 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
                 const int k = idx < TRD_NB ? idx : idx - TRD_NB;
                 T s = O::zero();
                 if (k < nk)
-                    for (int q0 = part; q0 < G; q0 += 32) {           // 8 loads in flight, summed in a fixed order
-                        T bq[8];
+                    for (int q0 = part; q0 < G; q0 += 80) {           // 20 loads in flight, summed in a fixed order
+                        T bq[20];
 #pragma unroll
-                        for (int u = 0; u < 8; ++u) bq[u] = (q0 + 4 * u < G) ? ldcg(pt + (long)(q0 + 4 * u) * 2 * TRD_NB + idx) : O::zero();
+                        for (int u = 0; u < 20; ++u) bq[u] = (q0 + 4 * u < G) ? ldcg(pt + (long)(q0 + 4 * u) * 2 * TRD_NB + idx) : O::zero();
 #pragma unroll
-                        for (int u = 0; u < 8; ++u) s = O::add(s, bq[u]);
+                        for (int u = 0; u < 20; ++u) s = O::add(s, bq[u]);
                     }
                 s_red4[part][idx] = s;
                 if (warp == 0) {
@@ -354,7 +354,7 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
                 {
                     // row sums of the strips: lane <-> 4 rows of the pass, warp <-> strips S = warp, warp + NW, ...;
                     // 4 x 4 independent L2 loads in flight per thread, every row summed in ascending strip order
-                    constexpr int NG = TRD_PASS / 32, UB = 4;
+                    constexpr int NG = TRD_PASS / 32, UB = 8;
                     int rr[NG], se[NG]; T acc[NG];
                     int smax = -1;
 #pragma unroll
