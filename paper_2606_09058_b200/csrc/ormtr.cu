@@ -13,7 +13,9 @@ namespace nao {
 //   Vb (explicit, zeros above the unit diagonal), G = Vb^H Vb, T by the xLARFT recurrence, then three GEMMs
 //   X = Vb^H Z ; X <- T X ; Z -= Vb X.
 // ----------------------------------------------------------------------------------------------------------------
-static const int ORM_KB = 128;
+static const int ORM_KB = 128;        // reflectors per T factor built by the recurrence (larft_kernel)
+static const int ORM_BLK = 512;       // reflectors per applied block; its T is assembled from 128-blocks by doubling:
+                                      // T = [T11 T12; 0 T22], T12 = -T11 (V1^H V2) T22
 
 template <class T>
 __global__ void build_v_kernel(int n, int jb, int kb, int shift, const T *A, long lda, long sA, T *V, long ldv, long sV) {
@@ -34,7 +36,7 @@ __global__ void build_v_kernel(int n, int jb, int kb, int shift, const T *A, lon
 // T (kb x kb upper) from G = V^H V and tau: T(i,i) = tau_i ; T(0:i, i) = -tau_i T(0:i,0:i) G(0:i, i).
 // T is built in shared memory in packed upper storage ((r,c), r <= c, at c(c+1)/2 + r) and written out dense.
 template <class T>
-__global__ void __launch_bounds__(256) larft_kernel(int kb, const T *G, long ldg, long sG, const T *tau, long sTau, T *Tm, long sT) {
+__global__ void __launch_bounds__(256) larft_kernel(int kb, const T *G, long ldg, long sG, const T *tau, long sTau, T *Tm, long ldt, long sT) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T *sT_ = (T *)smem_raw;             // packed upper, kb(kb+1)/2
     __shared__ T s_g[ORM_KB];
@@ -58,7 +60,7 @@ __global__ void __launch_bounds__(256) larft_kernel(int kb, const T *G, long ldg
     }
     for (int e = tid; e < kb * kb; e += blockDim.x) {
         const int r = e % kb, c = e / kb;
-        Tm[e] = r <= c ? sT_[c * (c + 1) / 2 + r] : Ops<T>::zero();
+        Tm[r + (long)c * ldt] = r <= c ? sT_[c * (c + 1) / 2 + r] : Ops<T>::zero();
     }
 }
 
@@ -90,10 +92,10 @@ int larft(int dtype, int kb, const void *G, long ldg, long sG, const void *tau, 
     if (kb > ORM_KB) return NAO_ERR_UNSUPPORTED;
     if (dtype == NAO_COMPLEX) {
         if (int rc = larft_attr<cplx>()) return rc;
-        larft_kernel<cplx><<<batch, 256, (size_t)kb * (kb + 1) / 2 * sizeof(cplx), st>>>(kb, (const cplx *)G, ldg, sG, (const cplx *)tau, sTau, (cplx *)Tm, sT);
+        larft_kernel<cplx><<<batch, 256, (size_t)kb * (kb + 1) / 2 * sizeof(cplx), st>>>(kb, (const cplx *)G, ldg, sG, (const cplx *)tau, sTau, (cplx *)Tm, kb, sT);
     } else {
         if (int rc = larft_attr<double>()) return rc;
-        larft_kernel<double><<<batch, 256, (size_t)kb * (kb + 1) / 2 * sizeof(double), st>>>(kb, (const double *)G, ldg, sG, (const double *)tau, sTau, (double *)Tm, sT);
+        larft_kernel<double><<<batch, 256, (size_t)kb * (kb + 1) / 2 * sizeof(double), st>>>(kb, (const double *)G, ldg, sG, (const double *)tau, sTau, (double *)Tm, kb, sT);
     }
     NAO_LAUNCHED();
     NAO_CUDA_CHECK(cudaGetLastError());
@@ -105,16 +107,16 @@ static OrmWork orm_plan(int dtype, int n, int ncols, int batch, void *work) {
     OrmWork w; const size_t es = esize(dtype);
     Arena ar(work, (size_t)-1);
     // split-K factors for the two tall-skinny^H products (k = m up to n): fill ~2 waves of 148 SMs
-    const int tilesX = ceil_div(ncols, dtype == NAO_COMPLEX ? 64 : 128) * batch;
+    const int tilesX = (ORM_BLK / 128) * ceil_div(ncols, dtype == NAO_COMPLEX ? 64 : 128) * batch;
     w.ksX = std::max(1, std::min(std::min(296 / std::max(1, tilesX), ceil_div(n, 512)), 16));
-    const int tilesG = (dtype == NAO_COMPLEX ? 2 : 1) * batch;
+    const int tilesG = (ORM_BLK / 128) * (dtype == NAO_COMPLEX ? 4 : 2) * batch;
     w.ksG = std::max(1, std::min(std::min(148 / std::max(1, tilesG), ceil_div(n, 256)), 64));
-    w.V = ar.take((size_t)batch * n * ORM_KB * es);
-    w.G = ar.take((size_t)batch * ORM_KB * ORM_KB * es);
-    w.T = ar.take((size_t)batch * ORM_KB * ORM_KB * es);
-    w.X = ar.take((size_t)batch * ORM_KB * ncols * es);
-    w.X2 = ar.take((size_t)batch * ORM_KB * ncols * es);
-    w.P = ar.take((size_t)batch * std::max((size_t)w.ksX * ORM_KB * ncols, (size_t)w.ksG * ORM_KB * ORM_KB) * es);
+    w.V = ar.take((size_t)batch * n * ORM_BLK * es);
+    w.G = ar.take((size_t)batch * ORM_BLK * ORM_BLK * es);
+    w.T = ar.take((size_t)batch * ORM_BLK * ORM_BLK * es);
+    w.X = ar.take((size_t)batch * ORM_BLK * ncols * es);
+    w.X2 = ar.take((size_t)batch * ORM_BLK * std::max(ncols, ORM_BLK) * es);
+    w.P = ar.take((size_t)batch * std::max((size_t)w.ksX * ORM_BLK * ncols, (size_t)w.ksG * ORM_BLK * ORM_BLK) * es);
     w.bytes = ar.off;
     return w;
 }
@@ -132,29 +134,46 @@ static int ormtr_impl(int dtype, int n, int ncols, int batch, int shift, const T
         NAO_CUDA_CHECK(cudaFuncSetAttribute(larft_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)larft_smem));
         attr = true;
     }
-    const int nblocks = ceil_div(nref, ORM_KB);
+    const int nblocks = ceil_div(nref, ORM_BLK);
+    const long sGT = (long)ORM_BLK * ORM_BLK, sX = (long)ORM_BLK * ncols, sX2 = (long)ORM_BLK * std::max(ncols, ORM_BLK);
+    T *Gm = (T *)w.G, *Tm = (T *)w.T;
     for (int blk = nblocks - 1; blk >= 0; --blk) {
-        const int jb = blk * ORM_KB, kb = std::min(ORM_KB, nref - jb), m = n - jb - shift;
-        const long ldv = m, sV = (long)n * ORM_KB;
+        const int jb = blk * ORM_BLK, kb = std::min(ORM_BLK, nref - jb), m = n - jb - shift;
+        const long ldv = m, sV = (long)n * ORM_BLK;
         build_v_kernel<T><<<dim3(ceil_div(m, 256), kb, batch), 256, 0, st>>>(n, jb, kb, shift, A, lda, sA, (T *)w.V, ldv, sV);
         NAO_LAUNCHED();
         // G = V^H V  (kb x kb, k = m: split-K)
         GemmDesc g = gemm_desc(OP_C, OP_N, kb, kb, m, 1.0, w.V, ldv, w.V, ldv, 0.0, w.G, kb);
-        g.sA = sV; g.sB = sV; g.sC = ORM_KB * ORM_KB;
+        g.sA = sV; g.sB = sV; g.sC = sGT;
         if (int rc = gemm_splitk(dtype, g, batch, std::min(w.ksG, ceil_div(m, 256)), w.P, st)) return rc;
-        larft_kernel<T><<<batch, 256, larft_smem, st>>>(kb, (const T *)w.G, kb, ORM_KB * ORM_KB, tau + jb, n, (T *)w.T, ORM_KB * ORM_KB);
-        NAO_LAUNCHED();
-        // X = V^H Z[jb+1:, :]  (kb x ncols, k = m: split-K)
+        // T: recurrence on the diagonal 128-blocks, then off-diagonal blocks by doubling (two small GEMMs each)
+        for (int off = 0; off < kb; off += ORM_KB) {
+            const int kd = std::min(ORM_KB, kb - off);
+            larft_kernel<T><<<batch, 256, larft_smem, st>>>(kd, Gm + off + (long)off * kb, kb, sGT, tau + jb + off, n, Tm + off + (long)off * kb, kb, sGT);
+            NAO_LAUNCHED();
+        }
+        for (int sz = ORM_KB; sz < kb; sz *= 2)
+            for (int off = 0; off + sz < kb; off += 2 * sz) {
+                const int k1 = sz, k2 = std::min(sz, kb - off - sz), o2 = off + sz;
+                // tmp = G12 T22 ; T12 = -T11 tmp
+                GemmDesc t1 = gemm_desc(OP_N, OP_N, k1, k2, k2, 1.0, Gm + off + (long)o2 * kb, kb, Tm + o2 + (long)o2 * kb, kb, 0.0, w.X2, k1);
+                t1.sA = sGT; t1.sB = sGT; t1.sC = sX2; t1.maskB = MASK_UPPER;
+                if (int rc = gemm_launch(dtype, t1, batch, st)) return rc;
+                GemmDesc t2 = gemm_desc(OP_N, OP_N, k1, k2, k1, -1.0, Tm + off + (long)off * kb, kb, w.X2, k1, 0.0, Tm + off + (long)o2 * kb, kb);
+                t2.sA = sGT; t2.sB = sX2; t2.sC = sGT; t2.maskA = MASK_UPPER;
+                if (int rc = gemm_launch(dtype, t2, batch, st)) return rc;
+            }
+        // X = V^H Z[jb+shift:, :]  (kb x ncols, k = m: split-K)
         GemmDesc x = gemm_desc(OP_C, OP_N, kb, ncols, m, 1.0, w.V, ldv, Z + jb + shift, ldz, 0.0, w.X, kb);
-        x.sA = sV; x.sB = sZ; x.sC = (long)ORM_KB * ncols;
+        x.sA = sV; x.sB = sZ; x.sC = sX;
         if (int rc = gemm_splitk(dtype, x, batch, std::min(w.ksX, ceil_div(m, 512)), w.P, st)) return rc;
-        // X2 = T X
+        // X2 = T X  (T upper triangular: elements below the diagonal are never read)
         GemmDesc t = gemm_desc(OP_N, OP_N, kb, ncols, kb, 1.0, w.T, kb, w.X, kb, 0.0, w.X2, kb);
-        t.sA = ORM_KB * ORM_KB; t.sB = (long)ORM_KB * ncols; t.sC = (long)ORM_KB * ncols; t.maskA = MASK_UPPER;
+        t.sA = sGT; t.sB = sX; t.sC = sX2; t.maskA = MASK_UPPER;
         if (int rc = gemm_launch(dtype, t, batch, st)) return rc;
-        // Z[jb+1:, :] -= V X2
+        // Z[jb+shift:, :] -= V X2
         GemmDesc u = gemm_desc(OP_N, OP_N, m, ncols, kb, -1.0, w.V, ldv, w.X2, kb, 1.0, Z + jb + shift, ldz);
-        u.sA = sV; u.sB = (long)ORM_KB * ncols; u.sC = sZ;
+        u.sA = sV; u.sB = sX2; u.sC = sZ;
         if (int rc = gemm_launch(dtype, u, batch, st)) return rc;
     }
     NAO_CUDA_CHECK(cudaGetLastError());
