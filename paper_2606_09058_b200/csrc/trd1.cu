@@ -197,17 +197,17 @@ __device__ __forceinline__ double hemv_warp(const T *__restrict__ A, long lda, i
 #pragma unroll
             for (int k = 0; k < 4; ++k) xr_n[k] = vval((bmin + In) * TRD_TB + q + 16 * k);
         }
-#pragma unroll
-        for (int b = 0; b < NBATCH; ++b) {
-            if (b + 1 < NBATCH) load(nxt, Jp, h, Irel, b + 1);
-            else if (more) load(nxt, Jn, hn, In, 0);
+        // Two register buffers used alternately WITHOUT copying between them: a copy "cur = nxt" would have to wait for
+        // nxt before the following request is issued, leaving one batch in flight per warp; this way the request for
+        // batch b+2 is issued before the first use of batch b+1 (two batches = 8 KB per warp in flight).
+        auto consume = [&](T (&buf)[CB][4], int b) {
 #pragma unroll
             for (int cc = 0; cc < CB; ++cc) {
                 const T xc = sx[hh * CPT + b * CB + cc];
                 const int col = cb0 + b * CB + cc;
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
-                    T a = cur[cc][k], ac = a;
+                    T a = buf[cc][k], ac = a;
                     if (diag) {
                         const int r = rbase + 16 * k;
                         if (r == col) a = O::from_real(O::real(a));
@@ -217,10 +217,15 @@ __device__ __forceinline__ double hemv_warp(const T *__restrict__ A, long lda, i
                     cs[b * CB + cc] = O::add(cs[b * CB + cc], O::conj_mul(ac, xr[k]));
                 }
             }
+        };
+        static_assert(NBATCH % 2 == 0, "ping-pong buffers need an even number of batches per unit");
 #pragma unroll
-            for (int cc = 0; cc < CB; ++cc)
-#pragma unroll
-                for (int k = 0; k < 4; ++k) cur[cc][k] = nxt[cc][k];
+        for (int b = 0; b < NBATCH; b += 2) {
+            load(nxt, Jp, h, Irel, b + 1);
+            consume(cur, b);
+            if (b + 2 < NBATCH) load(cur, Jp, h, Irel, b + 2);
+            else if (more) load(cur, Jn, hn, In, 0);
+            consume(nxt, b + 1);
         }
         // row sums of this unit: combine the two column halves, lanes 0..15 write 4 x 16 consecutive rows
 #pragma unroll
