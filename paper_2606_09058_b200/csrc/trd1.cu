@@ -615,7 +615,38 @@ static int hetrd_impl(int dtype, int n, int batch, T *A, long lda, long sA, doub
 }
 
 #ifdef NAO_TRACE
+// HEMV of `ncols` consecutive columns starting at j0 with NOTHING else (no reflector, no barriers, no reductions): isolates
+// the streaming part of hetrd_panel_kernel for timing.  acol must hold n finite values.
+template <class T>
+__global__ void __launch_bounds__(TRD_NT, 1) hemv_only_kernel(const T *A, long lda, long sA, int n, int j0, int ncols, int G,
+                                                              int nblk, const T *acol, T *Prow, T *Pcol, double *out) {
+    extern __shared__ __align__(16) unsigned char trd_smem[];
+    T *sx = (T *)trd_smem;
+    const int item = blockIdx.x / G, g = blockIdx.x % G, warp = threadIdx.x >> 5;
+    A += (long)item * sA; Prow += (long)item * Hv<T>::HS * nblk * n; Pcol += (long)item * nblk * n; acol += (long)item * n;
+    double acc = 0.0;
+    for (int j = j0; j < j0 + ncols; ++j) {
+        acc += hemv_warp<T>(A, lda, n, j, nblk, G, g, acol, Ops<T>::one(), sx + warp * Hv<T>::SW, Prow, Pcol);
+        __syncthreads();
+    }
+    if (acc == 1.2345) out[0] = acc;
+}
 }  // namespace nao
+NAO_EXPORT double nao_debug_hemv_only(int n, int batch, int j0, int ncols, const double *dA, double *dwork, int reps) {
+    using namespace nao;
+    const int G = 148 / batch, nblk = ceil_div(n, TRD_TB);
+    double *acol = dwork, *Prow = acol + (size_t)batch * n, *Pcol = Prow + (size_t)batch * 2 * nblk * n, *out = Pcol + (size_t)batch * nblk * n;
+    cudaMemset(acol, 0, (size_t)batch * n * 8);
+    cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const size_t smem = (size_t)TRD_NW * Hv<double>::SW * 8;
+    hemv_only_kernel<double><<<batch * G, TRD_NT, smem>>>(dA, n, (long)n * n, n, j0, ncols, G, nblk, acol, Prow, Pcol, out);
+    cudaEventRecord(e0);
+    for (int r = 0; r < reps; ++r)
+        hemv_only_kernel<double><<<batch * G, TRD_NT, smem>>>(dA, n, (long)n * n, n, j0, ncols, G, nblk, acol, Prow, Pcol, out);
+    cudaEventRecord(e1); cudaEventSynchronize(e1);
+    float ms = 0.f; cudaEventElapsedTime(&ms, e0, e1);
+    return cudaGetLastError() == cudaSuccess ? ms / reps : -1.0;
+}
 NAO_EXPORT int nao_debug_trd_trace(double *out_us, int reset) {
     unsigned long long h[16];
     cudaDeviceSynchronize();
