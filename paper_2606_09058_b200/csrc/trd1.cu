@@ -42,6 +42,8 @@ static const int TRD_PASS = 128;     // rows finalised per pass in phase A
 #define TRD_TRACE_CTA 0
 #endif
 __device__ unsigned long long g_trd_trace[16];
+__device__ unsigned long long g_trd_stamp[4 * 296];      // per CTA: phase-B start, hemv start, hemv end (own warps), after barrier 2
+__device__ int g_trd_stamp_col = 100;
 #define TRD_T(k)                                                                                   \
     do {                                                                                           \
         if (blockIdx.x == TRD_TRACE_CTA && threadIdx.x == 0) {                                     \
@@ -504,11 +506,24 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
                 pt[(long)g * 2 * TRD_NB + tid] = O::add(O::add(s_red4[0][tid], s_red4[1][tid]), O::add(s_red4[2][tid], s_red4[3][tid]));
         }
         TRD_T(6);
+#ifdef NAO_TRACE
+        unsigned long long ts0 = 0, ts1 = 0;
+        if (j == g_trd_stamp_col && tid == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(ts0));
+#endif
         double vav = hemv_warp<T>(A, lda, n, j, nblk, G, g, acol, scale, sx + warp * SW, Prow, Pcol);
         vav = block_sum_d(vav, s_dred);
         if (tid == 0) pvav[g] = vav;
         TRD_T(7);
+#ifdef NAO_TRACE
+        if (j == g_trd_stamp_col && tid == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(ts1));
+#endif
         group_barrier(bar, G, ++bar_ord);
+#ifdef NAO_TRACE
+        if (j == g_trd_stamp_col && tid == 0) {
+            unsigned long long ts2; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(ts2));
+            g_trd_stamp[4 * blockIdx.x + 1] = ts0; g_trd_stamp[4 * blockIdx.x + 2] = ts1; g_trd_stamp[4 * blockIdx.x + 3] = ts2;
+        }
+#endif
         TRD_T(8);
     }
 }
@@ -646,6 +661,12 @@ NAO_EXPORT double nao_debug_hemv_only(int n, int batch, int j0, int ncols, const
     cudaEventRecord(e1); cudaEventSynchronize(e1);
     float ms = 0.f; cudaEventElapsedTime(&ms, e0, e1);
     return cudaGetLastError() == cudaSuccess ? ms / reps : -1.0;
+}
+NAO_EXPORT int nao_debug_trd_stamps(int col, unsigned long long *out /* 4*296 */) {
+    cudaDeviceSynchronize();
+    if (out) cudaMemcpyFromSymbol(out, nao::g_trd_stamp, sizeof(unsigned long long) * 4 * 296);
+    cudaMemcpyToSymbol(nao::g_trd_stamp_col, &col, sizeof(int));
+    return 0;
 }
 NAO_EXPORT int nao_debug_trd_trace(double *out_us, int reset) {
     unsigned long long h[16];
