@@ -361,3 +361,31 @@ def test_config3_full_size_certificate(nao):
         assert abs(Dh[i, j] - complex(dij)) <= 1e-12
     mu_ref, _ = oracle.fermi(E.cpu().numpy(), prob.weights, prob.n_electrons, prob.kT)
     assert abs(mu - mu_ref) <= TOL_MU
+
+
+def test_config4_size_heev_properties(nao):
+    """Order of BASELINE config 4 (2N = 26 624 complex, 11.3 GB per matrix): 64-bit offsets, the 148-CTA cooperative
+    panel kernel with 180-row chunks, 52 blocks of 512 reflectors.  Seeded Hermitian matrix generated on the device (the
+    config-4 recipe needs > 30 GB of host memory for H alone); invariants that hold at any size, products by torch."""
+    n = 26624
+    g = torch.Generator(device=DEV); g.manual_seed(4)
+    A = torch.complex(torch.randn(n, n, dtype=torch.float64, device=DEV, generator=g),
+                      torch.randn(n, n, dtype=torch.float64, device=DEV, generator=g))
+    A = (A + A.mH).unsqueeze(0)                       # Hermitian; column-major item of A^T = conj(A): same spectrum
+    tr = float(A[0].diagonal().real.sum())
+    fro2 = float((A[0].abs() ** 2).sum())
+    E, Z, info = nao.heev(A.clone())
+    assert int(info.abs().max()) == 0
+    e = E[0]
+    assert bool((e[1:] >= e[:-1]).all())
+    assert abs(float(e.sum()) - tr) <= 1e-9 * n                      # trace
+    assert abs(float((e ** 2).sum()) - fro2) <= 1e-12 * fro2         # ||A||_F^2 = sum e^2
+    Zm = Z[0].T
+    Am = A[0].T
+    R = Am @ Zm - Zm * e[None, :]
+    scale = float(e.abs().max())
+    assert float(R.abs().max()) <= 1e-12 * scale * 10
+    del R
+    G = Zm.mH @ Zm
+    G.diagonal().sub_(1.0)
+    assert float(G.abs().max()) <= 1e-12
