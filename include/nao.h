@@ -83,6 +83,29 @@ int nao_geneig(int n, int batch, int dtype, unsigned flags,
                void *dwork, size_t work_bytes, int *d_info, void *cuda_stream);
 
 /*
+ * Partial-spectrum variant (the paper notes that only the occupied quarter to half of the spectrum is
+ * needed and that its cuSOLVER route cannot exploit this).  Identical to nao_geneig except that only the
+ * eigenvectors of the n_vec LOWEST eigenvalues are back-transformed: all n eigenvalues are still written to dE, columns
+ * 0..n_vec-1 of every item of dC are written, columns n_vec.. are set to zero.  The density matrix built from these
+ * vectors equals the one of the full solve as long as every state with f >= 1e-17 lies below n_vec -- check with
+ * nao_occupied_count after nao_fermi_mu (an SCF loop takes n_vec from the previous step plus a margin).
+ *   1..4 as nao_geneig;  5 n_vec in 1..n;  the remaining arguments as nao_geneig arguments 5..18.
+ * Negative return values count the arguments of THIS signature.
+ */
+int nao_geneig_partial(int n, int batch, int dtype, unsigned flags, int n_vec,
+                       const void *dH, long ldh, long strideH,
+                       void *dS, long lds, long strideS,
+                       double *dE,
+                       void *dC, long ldc, long strideC,
+                       void *dwork, size_t work_bytes, int *d_info, void *cuda_stream);
+
+/*
+ * 1 + the largest level index i (over all batch items) with dF[b*n + i] >= threshold: the number of leading
+ * eigenvectors nao_density_matrix reads.  Synchronises the stream to write *h_count (HOST int).
+ */
+int nao_occupied_count(int n, int batch, const double *dF, double threshold, int *h_count, void *cuda_stream);
+
+/*
  * Fermi level and occupations (reading C5).  States are all (item b, level i) pairs; state weight is
  * h_weight[b] (= spin degeneracy g times k-point weight w_k, reading C4).  Finds the unique mu with
  *     sum_b h_weight[b] * sum_i f_bi = n_electrons,   f_bi = 1/(1 + exp((e_bi - mu)/kT)),

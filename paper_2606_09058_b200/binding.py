@@ -28,6 +28,8 @@ _dp = ctypes.POINTER(ctypes.c_double)
 _SIGNATURES = {
     "nao_geneig_workspace": ([_i, _i, _i, ctypes.c_uint, _szp], _i),
     "nao_geneig": ([_i, _i, _i, ctypes.c_uint, _vp, _l, _l, _vp, _l, _l, _vp, _vp, _l, _l, _vp, _sz, _vp, _vp], _i),
+    "nao_geneig_partial": ([_i, _i, _i, ctypes.c_uint, _i, _vp, _l, _l, _vp, _l, _l, _vp, _vp, _l, _l, _vp, _sz, _vp, _vp], _i),
+    "nao_occupied_count": ([_i, _i, _vp, _d, ctypes.POINTER(ctypes.c_int), _vp], _i),
     "nao_fermi_workspace": ([_i, _i, _szp], _i),
     "nao_fermi_mu": ([_i, _i, _vp, _dp, _d, _d, _dp, _vp, _vp, _vp], _i),
     "nao_density_workspace": ([_i, _i, _i, _szp], _i),
@@ -150,8 +152,9 @@ def geneig_workspace(n: int, batch: int, dtype: int, flags: int = 0) -> int:
     return out.value
 
 
-def geneig(H: torch.Tensor, S: torch.Tensor, flags: int = 0, work: torch.Tensor | None = None):
+def geneig(H: torch.Tensor, S: torch.Tensor, flags: int = 0, work: torch.Tensor | None = None, n_vec: int | None = None):
     """nao_geneig on (batch, n, n) column-major items.  S is overwritten by its factor (see nao.h).
+    n_vec (optional): back-transform only the n_vec lowest eigenvectors (nao_geneig_partial); the other columns of C are zero.
     Returns (E (batch, n), C (batch, n, n) column-major items, info (batch,) int32 device tensor)."""
     batch, n, _ = H.shape
     dt = _dtype_code(H)
@@ -167,10 +170,24 @@ def geneig(H: torch.Tensor, S: torch.Tensor, flags: int = 0, work: torch.Tensor 
     need = geneig_workspace(n, batch, dt, flags)
     if work is None or work.numel() < need:
         work = _workspace(need, H.device)
-    rc = lib().nao_geneig(n, batch, dt, flags, _dev(H, "H"), n, n * n, _dev(S, "S"), lds, strideS, _dev(E, "E"),
-                          _dev(C, "C"), n, n * n, _dev(work, "work"), work.numel(), _dev(info, "info"), _stream(H))
-    _check(rc, "nao_geneig")
+    if n_vec is None:
+        rc = lib().nao_geneig(n, batch, dt, flags, _dev(H, "H"), n, n * n, _dev(S, "S"), lds, strideS, _dev(E, "E"),
+                              _dev(C, "C"), n, n * n, _dev(work, "work"), work.numel(), _dev(info, "info"), _stream(H))
+        _check(rc, "nao_geneig")
+    else:
+        rc = lib().nao_geneig_partial(n, batch, dt, flags, int(n_vec), _dev(H, "H"), n, n * n, _dev(S, "S"), lds, strideS,
+                                      _dev(E, "E"), _dev(C, "C"), n, n * n, _dev(work, "work"), work.numel(),
+                                      _dev(info, "info"), _stream(H))
+        _check(rc, "nao_geneig_partial")
     return E, C, info
+
+
+def occupied_count(F: torch.Tensor, threshold: float = 1e-17) -> int:
+    """nao_occupied_count: number of leading eigenvectors the density matrix needs (1 + last level with f >= threshold)."""
+    batch, n = F.shape
+    out = ctypes.c_int(0)
+    _check(lib().nao_occupied_count(n, batch, _dev(F, "F"), float(threshold), ctypes.byref(out), _stream(F)), "nao_occupied_count")
+    return out.value
 
 
 def fermi_mu(E: torch.Tensor, weights, n_electrons: float, kT: float):

@@ -63,3 +63,34 @@ NAO_EXPORT int nao_density_matrix(int n, int batch, int dtype, const void *dC, l
     if (rc) return rc;
     return herm_fill(dtype, n, dD, ldd, strideD, dD, ldd, strideD, batch, st);
 }
+
+// ---------------------------------------------------------------------------------------------------------------------
+// nao_occupied_count: 1 + last level (over all items) with f >= threshold
+// ---------------------------------------------------------------------------------------------------------------------
+namespace nao {
+__global__ void occupied_count_kernel(int n, int batch, const double *F, double thr, int *out) {
+    int last = -1;
+    for (long e = blockIdx.x * (long)blockDim.x + threadIdx.x; e < (long)n * batch; e += (long)gridDim.x * blockDim.x)
+        if (F[e] >= thr) last = max(last, (int)(e % n));
+    for (int o = 16; o > 0; o >>= 1) last = max(last, __shfl_xor_sync(0xffffffffu, last, o));
+    if ((threadIdx.x & 31) == 0 && last >= 0) atomicMax(out, last + 1);
+}
+}  // namespace nao
+
+NAO_EXPORT int nao_occupied_count(int n, int batch, const double *dF, double threshold, int *h_count, void *cuda_stream) {
+    using namespace nao;
+    if (n < 1) return -1;
+    if (batch < 1) return -2;
+    if (!dF) return -3;
+    if (!h_count) return -5;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int *d_out = nullptr;
+    if (cudaMallocAsync((void **)&d_out, sizeof(int), st) != cudaSuccess) return NAO_ERR_CUDA;
+    if (cudaMemsetAsync(d_out, 0, sizeof(int), st) != cudaSuccess) return NAO_ERR_CUDA;
+    occupied_count_kernel<<<64, 256, 0, st>>>(n, batch, dF, threshold, d_out);
+    NAO_LAUNCHED();
+    if (cudaMemcpyAsync(h_count, d_out, sizeof(int), cudaMemcpyDeviceToHost, st) != cudaSuccess) return NAO_ERR_CUDA;
+    if (cudaStreamSynchronize(st) != cudaSuccess) return NAO_ERR_CUDA;
+    cudaFreeAsync(d_out, st);
+    return NAO_OK;
+}

@@ -43,7 +43,8 @@ static HeevPlan heev_plan(int dtype, int n, int batch, unsigned flags) {
 }
 
 static int heev(int dtype, int n, int batch, unsigned flags, void *A, long lda, long sA, double *E, void *Z, long ldz,
-                long sZ, void *work, int *d_info, cudaStream_t st) {
+                long sZ, void *work, int *d_info, cudaStream_t st, int nvec = -1) {
+    if (nvec < 0 || nvec > n) nvec = n;      // eigenvectors wanted: the nvec lowest
     HeevPlan p = heev_plan(dtype, n, batch, flags);
     char *w = (char *)work;
     double *d = (double *)(w + p.d), *e = (double *)(w + p.e);
@@ -63,18 +64,18 @@ static int heev(int dtype, int n, int batch, unsigned flags, void *A, long lda, 
     if (dtype == NAO_COMPLEX) {
         double *qt = (double *)(w + p.qt);
         if ((rc = stedc(n, batch, d, e, E, qt, n, (long)n * n, sub, d_info, st))) return rc;
-        if ((rc = real_to_complex(n, n, qt, n, (long)n * n, (cplx *)Z, ldz, sZ, batch, st))) return rc;
+        if ((rc = real_to_complex(n, nvec, qt, n, (long)n * n, (cplx *)Z, ldz, sZ, batch, st))) return rc;
     } else {
         if ((rc = stedc(n, batch, d, e, E, (double *)Z, ldz, sZ, sub, d_info, st))) return rc;
     }
     prof_mark(5, st);
     if (p.two_stage) {
-        if ((rc = q2_apply(dtype, n, n, batch, V2, n, (long)n * n, tau2, Z, ldz, sZ, sub, st))) return rc;
+        if ((rc = q2_apply(dtype, n, nvec, batch, V2, n, (long)n * n, tau2, Z, ldz, sZ, sub, st))) return rc;
         prof_mark(6, st);
-        rc = ormtr(dtype, n, n, batch, TRD2_B, A, lda, sA, tau, Z, ldz, sZ, sub, st);
+        rc = ormtr(dtype, n, nvec, batch, TRD2_B, A, lda, sA, tau, Z, ldz, sZ, sub, st);
     } else {
         prof_mark(6, st);
-        rc = ormtr(dtype, n, n, batch, 1, A, lda, sA, tau, Z, ldz, sZ, sub, st);
+        rc = ormtr(dtype, n, nvec, batch, 1, A, lda, sA, tau, Z, ldz, sZ, sub, st);
     }
     prof_mark(7, st);
     return rc;
@@ -138,9 +139,9 @@ NAO_EXPORT int nao_geneig_workspace(int n, int batch, int dtype, unsigned flags,
     return NAO_OK;
 }
 
-NAO_EXPORT int nao_geneig(int n, int batch, int dtype, unsigned flags, const void *dH, long ldh, long strideH, void *dS,
-                          long lds, long strideS, double *dE, void *dC, long ldc, long strideC, void *dwork,
-                          size_t work_bytes, int *d_info, void *cuda_stream) {
+static int geneig_impl(int n, int batch, int dtype, unsigned flags, int nvec, const void *dH, long ldh, long strideH, void *dS,
+                       long lds, long strideS, double *dE, void *dC, long ldc, long strideC, void *dwork,
+                       size_t work_bytes, int *d_info, void *cuda_stream) {
     using namespace nao;
     if (n < 1) return -1;
     if (batch < 1) return -2;
@@ -207,15 +208,41 @@ NAO_EXPORT int nao_geneig(int n, int batch, int dtype, unsigned flags, const voi
         }
 
     // 3. standard problem; eigenvectors into X
-    if ((rc = heev(dtype, n, batch, flags, A, n, sAX, dE, X, n, sAX, w + p.heev, d_info, st))) return rc;
+    if ((rc = heev(dtype, n, batch, flags, A, n, sAX, dE, X, n, sAX, w + p.heev, d_info, st, nvec))) return rc;
 
     // 4. C = W^H Z, per row block
     for (int bi = 0; bi < nb; ++bi) {
-        GemmDesc g = gemm_desc(OP_C, OP_N, nS, n, nS, 1.0, Wm, nS, (char *)X + (size_t)bi * nS * es, n, 0.0,
+        GemmDesc g = gemm_desc(OP_C, OP_N, nS, nvec, nS, 1.0, Wm, nS, (char *)X + (size_t)bi * nS * es, n, 0.0,
                                (char *)dC + (size_t)bi * nS * es, ldc);
         g.sA = sWm; g.sB = sAX; g.sC = strideC; g.maskA = MASK_LOWER;
         if ((rc = gemm_launch(dtype, g, batch, st))) return rc;
     }
     prof_mark(8, st);
+    // partial spectrum: the columns that were not back-transformed read as zero
+    if (nvec < n)
+        for (int b = 0; b < batch; ++b)
+            if (ldc == n) {
+                if ((rc = set_zero((char *)dC + ((size_t)b * strideC + (size_t)nvec * ldc) * es, (size_t)(n - nvec) * n * es, st))) return rc;
+            } else {
+                for (int j = nvec; j < n; ++j)
+                    if ((rc = set_zero((char *)dC + ((size_t)b * strideC + (size_t)j * ldc) * es, (size_t)n * es, st))) return rc;
+            }
     return NAO_OK;
+}
+
+NAO_EXPORT int nao_geneig(int n, int batch, int dtype, unsigned flags, const void *dH, long ldh, long strideH, void *dS,
+                          long lds, long strideS, double *dE, void *dC, long ldc, long strideC, void *dwork,
+                          size_t work_bytes, int *d_info, void *cuda_stream) {
+    return geneig_impl(n, batch, dtype, flags, n, dH, ldh, strideH, dS, lds, strideS, dE, dC, ldc, strideC, dwork, work_bytes,
+                       d_info, cuda_stream);
+}
+
+NAO_EXPORT int nao_geneig_partial(int n, int batch, int dtype, unsigned flags, int n_vec, const void *dH, long ldh, long strideH,
+                                  void *dS, long lds, long strideS, double *dE, void *dC, long ldc, long strideC, void *dwork,
+                                  size_t work_bytes, int *d_info, void *cuda_stream) {
+    if (n < 1) return -1;
+    if (n_vec < 1 || n_vec > n) return -5;
+    int rc = geneig_impl(n, batch, dtype, flags, n_vec, dH, ldh, strideH, dS, lds, strideS, dE, dC, ldc, strideC, dwork,
+                         work_bytes, d_info, cuda_stream);
+    return (rc <= -5) ? rc - 1 : rc;          // argument positions after n_vec are shifted by one
 }

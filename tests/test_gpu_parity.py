@@ -389,3 +389,32 @@ def test_config4_size_heev_properties(nao):
     G = Zm.mH @ Zm
     G.diagonal().sub_(1.0)
     assert float(G.abs().max()) <= 1e-12
+
+
+@pytest.mark.parametrize("two_stage", [False, True])
+def test_partial_spectrum_gives_the_same_density(nao, two_stage):
+    """nao_geneig_partial: only the vectors with f >= 1e-17 (+ margin) are
+    back-transformed; e (all levels), mu and D must match the oracle like the full solve, the unwanted columns are 0."""
+    for idx, nat in ((2, 32), (3, 16)):
+        prob = make_config(idx, nat=nat)
+        ref = oracle.solve_problem(prob)
+        flags = (nao.NAO_NC_BLOCK_S if prob.nc_block_s else 0) | (nao.NAO_TRD_TWO_STAGE if two_stage else 0)
+        H = torch.from_numpy(prob.H).to(DEV)
+        S = torch.from_numpy(prob.S.copy()).to(DEV)
+        E, C, info = nao.geneig(H, S, flags=flags)                      # first SCF step: everything
+        mu, F = nao.fermi_mu(E, prob.weights, prob.n_electrons, prob.kT)
+        n_vec = nao.occupied_count(F)
+        assert 0 < n_vec < prob.n // 2
+        n_vec += 5
+        E2, C2, info2 = nao.geneig(H, S, flags=flags | nao.NAO_S_FACTORED, n_vec=n_vec)   # later step: partial
+        assert int(info2.abs().max()) == 0
+        mu2, F2 = nao.fermi_mu(E2, prob.weights, prob.n_electrons, prob.kT)
+        assert nao.occupied_count(F2) <= n_vec
+        D2 = nao.density_matrix(C2, F2)
+        assert np.abs(E2.cpu().numpy() - ref["e"]).max() <= TOL_E
+        assert abs(mu2 - ref["mu"]) <= TOL_MU
+        for b in range(prob.batch):
+            assert np.abs(to_np(D2)[b] - ref["D"][b]).max() <= TOL_D
+        assert float(C2[:, n_vec:, :].abs().max()) == 0.0              # column-major items: columns are dim 1
+        Cb = to_np(C2)[0][:, :n_vec]
+        assert np.abs(Cb.conj().T @ prob.S_full(0) @ Cb - np.eye(n_vec)).max() <= TOL_ORTH
