@@ -134,11 +134,14 @@ static int ormtr_impl(int dtype, int n, int ncols, int batch, int shift, const T
         NAO_CUDA_CHECK(cudaFuncSetAttribute(larft_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)larft_smem));
         attr = true;
     }
-    const int nblocks = ceil_div(nref, ORM_BLK);
+    // few columns (partial spectrum): the cost of building T (G = V^H V is kb^2 m flops per block) matters next to the
+    // two products, so the block is halved
+    const int BLK = (4 * ncols >= n) ? ORM_BLK : ORM_BLK / 2;
+    const int nblocks = ceil_div(nref, BLK);
     const long sGT = (long)ORM_BLK * ORM_BLK, sX = (long)ORM_BLK * ncols, sX2 = (long)ORM_BLK * std::max(ncols, ORM_BLK);
     T *Gm = (T *)w.G, *Tm = (T *)w.T;
     for (int blk = nblocks - 1; blk >= 0; --blk) {
-        const int jb = blk * ORM_BLK, kb = std::min(ORM_BLK, nref - jb), m = n - jb - shift;
+        const int jb = blk * BLK, kb = std::min(BLK, nref - jb), m = n - jb - shift;
         const long ldv = m, sV = (long)n * ORM_BLK;
         build_v_kernel<T><<<dim3(ceil_div(m, 256), kb, batch), 256, 0, st>>>(n, jb, kb, shift, A, lda, sA, (T *)w.V, ldv, sV);
         NAO_LAUNCHED();

@@ -112,18 +112,18 @@ template <> __device__ __forceinline__ double frag_out<double>(const double (&ac
 template <> __device__ __forceinline__ cplx frag_out<cplx>(const double (&acc)[4], int q) { return make_double2(acc[q], acc[2 + q]); }
 
 template <class T> struct Q2Cfg;
-template <> struct Q2Cfg<double> { static const int NC = 32; };     // columns of Z per CTA
-template <> struct Q2Cfg<cplx> { static const int NC = 16; };
+template <> struct Q2Cfg<double> { static const int NCMAX = 32; };     // most columns of Z per CTA (shared memory)
+template <> struct Q2Cfg<cplx> { static const int NCMAX = 16; };
 
 template <class T> __device__ __forceinline__ void cp_async_elem(T *s, const T *g, bool pred) {
     if constexpr (sizeof(T) == 16) cp_async16(s, g, pred); else cp_async8(s, g, pred);
 }
 
-template <class T>
+template <class T, int NC>
 __global__ void __launch_bounds__(Q2_NT) q2_apply_kernel(int n, int ncols, const T *V2, long ldv, long sV2, const T *Tst,
                                                          long sTst, T *Z, long ldz, long sZ) {
     typedef Ops<T> O;
-    constexpr int b = TRD2_B, NBK = Q2_NBK, LW = Q2_LW, NC = Q2Cfg<T>::NC, NCT = NC / 8, LDV = Q2_LDV, LDW = Q2_LDW, LDT = NBK;
+    constexpr int b = TRD2_B, NBK = Q2_NBK, LW = Q2_LW, NCT = NC / 8, LDV = Q2_LDV, LDW = Q2_LDW, LDT = NBK;
     const int item = blockIdx.y, c0 = blockIdx.x * NC;
     V2 += (long)item * sV2; Tst += (long)item * sTst; Z += (long)item * sZ;
     extern __shared__ __align__(16) unsigned char q2_smem[];
@@ -320,17 +320,30 @@ static int q2_apply_impl(int n, int ncols, int batch, const T *V2, long ldv, lon
     T *Tst = (T *)work;
     const int nS = ceil_div(n - 1, Q2_NBK), kmax = q2_nwin(n, 0);
     const size_t smem_t = (size_t)Q2_NBK * Q2_LDV * sizeof(T);
-    const int NC = Q2Cfg<T>::NC;
-    const size_t smem_a = (size_t)((Q2_NBK + NC) * Q2_LDV + Q2_NBK * Q2_NBK + 2 * NC * Q2_LDW) * sizeof(T);
+    auto smem_a = [](int nc) { return (size_t)((Q2_NBK + nc) * Q2_LDV + Q2_NBK * Q2_NBK + 2 * nc * Q2_LDW) * sizeof(T); };
+    constexpr int NCMAX = Q2Cfg<T>::NCMAX;
     static bool attr = false;
     if (!attr) {
         NAO_CUDA_CHECK(cudaFuncSetAttribute(q2_tfactor_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_t));
-        NAO_CUDA_CHECK(cudaFuncSetAttribute(q2_apply_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_a));
+        NAO_CUDA_CHECK(cudaFuncSetAttribute(q2_apply_kernel<T, NCMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_a(NCMAX)));
+        NAO_CUDA_CHECK(cudaFuncSetAttribute(q2_apply_kernel<T, NCMAX / 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_a(NCMAX / 2)));
+        NAO_CUDA_CHECK(cudaFuncSetAttribute(q2_apply_kernel<T, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_a(8)));
         attr = true;
     }
     q2_tfactor_kernel<T><<<dim3(nS, kmax, batch), 256, smem_t, st>>>(n, V2, ldv, sV2, tau2, sTau2, Tst, sTst);
     NAO_LAUNCHED();
-    q2_apply_kernel<T><<<dim3(ceil_div(ncols, NC), batch), Q2_NT, smem_a, st>>>(n, ncols, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ);
+    // every CTA walks through all diamonds for its slab of columns: with few columns (partial spectrum) narrower slabs keep
+    // all SMs busy
+    int nsm = 148, dev = 0;
+    cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+    int nc = NCMAX;
+    while (nc > 8 && (long)ceil_div(ncols, nc) * batch < 2L * nsm) nc /= 2;
+    if (nc == NCMAX)
+        q2_apply_kernel<T, NCMAX><<<dim3(ceil_div(ncols, nc), batch), Q2_NT, smem_a(nc), st>>>(n, ncols, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ);
+    else if (nc == NCMAX / 2)
+        q2_apply_kernel<T, NCMAX / 2><<<dim3(ceil_div(ncols, nc), batch), Q2_NT, smem_a(nc), st>>>(n, ncols, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ);
+    else
+        q2_apply_kernel<T, 8><<<dim3(ceil_div(ncols, 8), batch), Q2_NT, smem_a(8), st>>>(n, ncols, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ);
     NAO_LAUNCHED();
     NAO_CUDA_CHECK(cudaGetLastError());
     return NAO_OK;
