@@ -98,8 +98,8 @@ __global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
     extern __shared__ __align__(16) unsigned char ch_smem[];
     T *sO = (T *)ch_smem;              // [b][LDS]  off-diagonal block, column-major
     T *sD = sO + b * LDS;              // [b][LDS]  diagonal block (full Hermitian)
-    __shared__ T s_vp[b], s_vn[b], s_w[b], s_part[4][b];
-    __shared__ T s_tau_p, s_tau_n;
+    __shared__ T s_vp[b], s_vn[b], s_w[b], s_u[b], s_z[b], s_part[4][b], s_part2[4][b];
+    __shared__ T s_tau_p, s_tau_n, s_kappa;
     __shared__ double s_beta, s_gamma;
 
     const int iq = tid & (b - 1), qq = tid >> 6;        // (row or column index, quarter)
@@ -216,54 +216,85 @@ __global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
             load_O(q0, Lq, r0, Lp);
             load_D(q0, Lq);
             __syncthreads();
-            // w = O v_prev ; O -= tau_prev w v_prev^H
+            // Fused form of  O <- H_n^H (O H_p),  D <- H_n^H D H_n  with ONE pass over each block:
+            //   w = O v_p ;  x = O[:,0] - tau_p w  -> (v_n, tau_n, beta) ;  kappa = v_n^H w
+            //   q = O^H v_n (on the ORIGINAL O) ;  z_c = q_c - tau_p kappa conj(v_p[c])   (= v_n^H (O H_p)[:,c])
+            //   O[:,c] <- O[:,c] - tau_p w conj(v_p[c]) - conj(tau_n) v_n z_c  (c >= 1);  O[:,0] <- beta e_0
+            //   u = D v_n ; gamma = v_n^H u ; y = tau_n u - 1/2 |tau_n|^2 gamma v_n ;  D <- D - y v_n^H - v_n y^H
+            // (1) w partials: thread <-> (row iq, column quarter qq)
             {
                 T sacc = O::zero();
                 if (iq < Lq) for (int cc = qq; cc < Lp; cc += 4) sacc = O::fma(sO[cc * LDS + iq], s_vp[cc], sacc);
                 s_part[qq][iq] = sacc;
             }
             __syncthreads();
-            {
-                const T tw = iq < Lq ? O::mul(s_tau_p, O::add(O::add(s_part[0][iq], s_part[1][iq]), O::add(s_part[2][iq], s_part[3][iq]))) : O::zero();
-                if (iq < Lq)
-                    for (int cc = qq; cc < Lp; cc += 4) sO[cc * LDS + iq] = O::sub(sO[cc * LDS + iq], O::mul_conj(tw, s_vp[cc]));
+            // (2) w, x
+            if (tid < b) {
+                const T w = tid < Lq ? O::add(O::add(s_part[0][tid], s_part[1][tid]), O::add(s_part[2][tid], s_part[3][tid])) : O::zero();
+                s_w[tid] = w;
+                s_vn[tid] = tid < Lq ? O::sub(sO[tid], O::mul(s_tau_p, w)) : O::zero();      // v_p[0] = 1
             }
             __syncthreads();
-            // new reflector from the first column of O
-            if (tid < b) s_vn[tid] = tid < Lq ? sO[tid] : O::zero();
-            __syncthreads();
-            if (warp == 0) house_warp<T>(s_vn, Lq, &s_tau_n, &s_beta);
-            __syncthreads();
-            if (tid < Lq) {
-                V2[(q0 + tid) + (long)s * p.ldv] = s_vn[tid];
-                sO[tid] = tid == 0 ? O::from_real(s_beta) : O::zero();
+            // (3) reflector, kappa
+            if (warp == 0) {
+                house_warp<T>(s_vn, Lq, &s_tau_n, &s_beta);
+                __syncwarp();
+                T kp = O::zero();
+                for (int i = tid; i < Lq; i += 32) kp = O::add(kp, O::conj_mul(s_vn[i], s_w[i]));
+                kp = warp_sum(kp);
+                if (tid == 0) s_kappa = kp;
             }
+            __syncthreads();
+            if (tid < Lq) V2[(q0 + tid) + (long)s * p.ldv] = s_vn[tid];
             if (tid == 0) tau2[(long)k * n + s] = s_tau_n;
-            // z_c = v^H O[:, c] (c >= 1) ; O[:, c] -= conj(tau) v z_c     thread <-> (column iq, row quarter qq)
+            // (4) q partials: thread <-> (column iq, row quarter qq);  u partials: thread <-> (row iq, column quarter qq)
             {
-                T sacc = O::zero();
-                if (iq >= 1 && iq < Lp) for (int i = qq; i < Lq; i += 4) sacc = O::add(sacc, O::conj_mul(s_vn[i], sO[iq * LDS + i]));
-                s_part[qq][iq] = sacc;
+                T qa = O::zero(), ua = O::zero();
+                if (iq < Lp) for (int i = qq; i < Lq; i += 4) qa = O::add(qa, O::conj_mul(s_vn[i], sO[iq * LDS + i]));
+                if (iq < Lq) for (int cc = qq; cc < Lq; cc += 4) ua = O::fma(sD[cc * LDS + iq], s_vn[cc], ua);
+                s_part[qq][iq] = qa; s_part2[qq][iq] = ua;
             }
             __syncthreads();
-            if (tid < b) s_w[tid] = O::mul(O::conj(s_tau_n), O::add(O::add(s_part[0][tid], s_part[1][tid]), O::add(s_part[2][tid], s_part[3][tid])));
-            __syncthreads();
-            if (iq < Lq)
-                for (int cc = (qq == 0 ? 4 : qq); cc < Lp; cc += 4)
-                    sO[cc * LDS + iq] = O::sub(sO[cc * LDS + iq], O::mul(s_vn[iq], s_w[cc]));
-            __syncthreads();
-            // store O
-            for (int e = tid; e < b * b; e += CH_NT) {
-                const int i = e & (b - 1), cc = e >> 6;
-                if (i < Lq && cc < Lp) AB[(q0 + i - r0 - cc) + (long)(r0 + cc) * ld] = sO[cc * LDS + i];
+            // (5) z (scaled by conj(tau_n)), u, gamma
+            if (tid < b) {
+                const T q = O::add(O::add(s_part[0][tid], s_part[1][tid]), O::add(s_part[2][tid], s_part[3][tid]));
+                const T z = tid < Lp ? O::sub(q, O::mul(O::mul(s_tau_p, s_kappa), O::conj(s_vp[tid]))) : O::zero();
+                s_z[tid] = O::mul(O::conj(s_tau_n), z);
+                s_u[tid] = tid < Lq ? O::add(O::add(s_part2[0][tid], s_part2[1][tid]), O::add(s_part2[2][tid], s_part2[3][tid])) : O::zero();
             }
-            two_sided(Lq);
-            store_D(q0, Lq);
-            if (tid < b) s_vp[tid] = s_vn[tid];
-            if (tid == 0) s_tau_p = s_tau_n;
+            __syncthreads();
+            if (warp == 0) {
+                double gsum = 0.0;
+                for (int i = tid; i < Lq; i += 32) gsum += O::real(O::conj_mul(s_vn[i], s_u[i]));
+                gsum = warp_sum(gsum);
+                if (tid == 0) s_gamma = gsum;
+            }
+            __syncthreads();
+            // (6) one pass over O and D: new values go straight to global memory
+            {
+                const T tau_n = s_tau_n, tau_p = s_tau_p;
+                const double f = -0.5 * O::abs2(tau_n) * s_gamma;
+                auto yv = [&](int i) -> T { return O::add(O::mul(tau_n, s_u[i]), O::scale(s_vn[i], f)); };
+                if (iq < Lq) {
+                    const T twi = O::mul(tau_p, s_w[iq]), vni = s_vn[iq], yi = yv(iq);
+                    for (int cc = qq; cc < Lp; cc += 4) {
+                        T o;
+                        if (cc == 0) o = iq == 0 ? O::from_real(s_beta) : O::zero();
+                        else o = O::sub(O::sub(sO[cc * LDS + iq], O::mul_conj(twi, s_vp[cc])), O::mul(vni, s_z[cc]));
+                        AB[(q0 + iq - r0 - cc) + (long)(r0 + cc) * ld] = o;
+                    }
+                    for (int cc = qq; cc < Lq; cc += 4) {
+                        if (iq < cc) continue;                                   // lower part is what is stored
+                        T a = O::sub(sD[cc * LDS + iq], O::add(O::mul_conj(yi, s_vn[cc]), O::mul_conj(vni, yv(cc))));
+                        if (cc == iq) a = O::from_real(O::real(a));
+                        AB[(iq - cc) + (long)(q0 + cc) * ld] = a;
+                    }
+                }
+            }
             __threadfence();
             __syncthreads();
-            if (tid == 0) st_release(prog + s, k + 1);
+            if (tid < b) s_vp[tid] = s_vn[tid];
+            if (tid == 0) { s_tau_p = s_tau_n; st_release(prog + s, k + 1); }
             r0 = q0; Lp = Lq;
         }
         __syncthreads();
