@@ -418,3 +418,22 @@ def test_partial_spectrum_gives_the_same_density(nao, two_stage):
         assert float(C2[:, n_vec:, :].abs().max()) == 0.0              # column-major items: columns are dim 1
         Cb = to_np(C2)[0][:, :n_vec]
         assert np.abs(Cb.conj().T @ prob.S_full(0) @ Cb - np.eye(n_vec)).max() <= TOL_ORTH
+
+
+@pytest.mark.parametrize("flag", ["NAO_TRD_ONE_STAGE", "NAO_TRD_TWO_STAGE"])
+@pytest.mark.parametrize("cplx", [False, True])
+def test_odd_order_1001_both_paths(nao, flag, cplx):
+    """Odd order and odd leading dimensions (no operand is 16-byte aligned after the first column): the 8-byte GEMM loaders,
+    ragged last panels / band blocks / diamonds.  Invariants plus a LAPACK cross-check of the eigenvalues (numpy, CPU)."""
+    n = 1001
+    rng = np.random.default_rng(1001)
+    A = rng.standard_normal((1, n, n))
+    if cplx:
+        A = A + 1j * rng.standard_normal((1, n, n))
+    A = A + np.swapaxes(A.conj(), -1, -2)
+    E, Z, info = nao.heev(to_dev(A), flags=getattr(nao, flag))
+    assert int(info.abs().max()) == 0
+    e = E.cpu().numpy()[0]; Zn = to_np(Z)[0]
+    assert np.abs(e - np.linalg.eigvalsh(A[0])).max() <= 1e-10
+    assert np.abs(A[0] @ Zn - Zn * e).max() <= 1e-10
+    assert np.abs(Zn.conj().T @ Zn - np.eye(n)).max() <= 1e-12
