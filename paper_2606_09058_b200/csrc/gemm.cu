@@ -203,34 +203,6 @@ gemm_kernel(const GemmDesc hd, const GemmDesc *__restrict__ dd) {
 
     double acc[MI][NI][CPLX ? 4 : 2];
     const double alpha = d.alpha, beta = d.beta;
-    // beta != 0: the accumulators start from (beta/alpha) C, loaded while the first tiles are in flight, so that the
-    // epilogue is store-only (for alpha = +-1, beta = 1 -- every update on the path -- this is exact)
-    const bool preload = (beta != 0.0 && alpha != 0.0);
-    if (preload) {
-        const double r = beta / alpha;
-#pragma unroll
-        for (int i = 0; i < MI; ++i) {
-            const int gi = m0 + wm + i * 8 + lr;
-#pragma unroll
-            for (int j = 0; j < NI; ++j)
-#pragma unroll
-                for (int q = 0; q < 2; ++q) {
-                    const int gj = n0 + wn + j * 8 + 2 * lc + q;
-                    T v;
-                    if constexpr (CPLX) v = make_double2(0.0, 0.0); else v = 0.0;
-                    if (gi < M && gj < N) v = C[gi + (long)gj * ldc];
-                    if constexpr (CPLX) { acc[i][j][q] = r * v.x; acc[i][j][2 + q] = r * v.y; } else acc[i][j][q] = r * v;
-                }
-        }
-    } else {
-#pragma unroll
-        for (int i = 0; i < MI; ++i)
-#pragma unroll
-            for (int j = 0; j < NI; ++j)
-#pragma unroll
-                for (int q = 0; q < (CPLX ? 4 : 2); ++q) acc[i][j][q] = 0.0;
-    }
-
     constexpr int a_sx = AXC ? 1 : (BK + G::PADK), a_sk = AXC ? (BM + G::PADX) : 1;
     constexpr int b_sx = BXC ? 1 : (BK + G::PADK), b_sk = BXC ? (BN + G::PADX) : 1;
 
@@ -277,6 +249,35 @@ gemm_kernel(const GemmDesc hd, const GemmDesc *__restrict__ dd) {
         if (fb_on) { fb.template issue<0>(bs); fb.template issue<1>(bs); fb.template issue<2>(bs); fb.template issue<3>(bs); }
         fa.advance(); fb.advance();
         cp_async_commit();
+    }
+
+    // (after the first tiles have been requested, so that the loads of C overlap the pipeline fill)
+    // beta != 0: the accumulators start from (beta/alpha) C, loaded while the first tiles are in flight, so that the
+    // epilogue is store-only (for alpha = +-1, beta = 1 -- every update on the path -- this is exact)
+    const bool preload = (beta != 0.0 && alpha != 0.0);
+    if (preload) {
+        const double r = beta / alpha;
+#pragma unroll
+        for (int i = 0; i < MI; ++i) {
+            const int gi = m0 + wm + i * 8 + lr;
+#pragma unroll
+            for (int j = 0; j < NI; ++j)
+#pragma unroll
+                for (int q = 0; q < 2; ++q) {
+                    const int gj = n0 + wn + j * 8 + 2 * lc + q;
+                    T v;
+                    if constexpr (CPLX) v = make_double2(0.0, 0.0); else v = 0.0;
+                    if (gi < M && gj < N) v = C[gi + (long)gj * ldc];
+                    if constexpr (CPLX) { acc[i][j][q] = r * v.x; acc[i][j][2 + q] = r * v.y; } else acc[i][j][q] = r * v;
+                }
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < MI; ++i)
+#pragma unroll
+            for (int j = 0; j < NI; ++j)
+#pragma unroll
+                for (int q = 0; q < (CPLX ? 4 : 2); ++q) acc[i][j][q] = 0.0;
     }
 
     for (int kt = 0; kt < nkt; ++kt) {
