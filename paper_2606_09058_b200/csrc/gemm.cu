@@ -168,6 +168,7 @@ gemm_kernel(const GemmDesc hd, const GemmDesc *__restrict__ dd) {
     const int m0 = tm * BM, n0 = tn * BN;
     const int cmode = d.cmode;
     if (cmode == 1 && n0 > m0 + BM - 1) return;
+    if (cmode == 2 && n0 > (m0 + BM - 1) / 2) return;
 
     const int ks = d.ksplit > 1 ? d.ksplit : 1;
     const long b = blockIdx.y / ks;
@@ -398,7 +399,7 @@ static int launch_variant2(const GemmDesc *hd, const GemmDesc *dd, int ngroups, 
     long tiles = (long)ceil_div(max_m, G::BM) * ceil_div(max_n, G::BN);
     dim3 grid((unsigned)tiles, (unsigned)batch, (unsigned)ngroups);
     GemmDesc dummy = hd ? *hd : gemm_desc(0, 0, 0, 0, 0, 0, nullptr, 0, nullptr, 0, 0, nullptr, 0);
-    const double flops = hd ? (CPLX ? 8.0 : 2.0) * hd->m * (double)hd->n * hd->k * (hd->cmode == 1 ? 0.5 : 1.0) *
+    const double flops = hd ? (CPLX ? 8.0 : 2.0) * hd->m * (double)hd->n * hd->k * (hd->cmode != 0 ? 0.5 : 1.0) *
                                   (hd->maskA != MASK_NONE || hd->maskB != MASK_NONE ? 0.5 : 1.0) * batch /
                                   (hd->ksplit > 1 ? hd->ksplit : 1)
                             : 0.0;

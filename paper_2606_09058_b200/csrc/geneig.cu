@@ -183,39 +183,62 @@ static int geneig_impl(int n, int batch, int dtype, unsigned flags, int nvec, co
         if ((rc = unpack_linv(p.sdtype, nS, dS, lds, strideS, W, nS, sW, p.nitemsS, st))) return rc;
     }
     prof_mark(1, st);
-    const void *Wm = W;          // the operand used in the products (complex copy in the NC case)
-    if (nc) {
-        if ((rc = real_to_complex(nS, nS, (const double *)W, nS, sW, (cplx *)(w + p.Wc), nS, sW, p.nitemsS, st))) return rc;
-        Wm = w + p.Wc;
-    }
+    const void *Wm = W;
     const long sWm = shared_S ? 0 : sW;
-
-    // 2. A = W H W^H : full Hermitian copy of H, X = W A (triangular W), A = X W^H (lower tiles)
-    if ((rc = herm_fill(dtype, n, dH, ldh, strideH, A, n, sAX, batch, st))) return rc;
-    const int nb = nc ? 2 : 1;
-    auto blk = [&](void *base, int bi, int bj) { return (void *)((char *)base + ((size_t)bi * nS + (size_t)bj * nS * n) * es); };
-    for (int bi = 0; bi < nb; ++bi)
-        for (int bj = 0; bj <= bi; ++bj) {
-            GemmDesc g = gemm_desc(OP_N, OP_N, nS, nS, nS, 1.0, Wm, nS, blk(A, bi, bj), n, 0.0, blk(X, bi, bj), n);
+    if (!nc) {
+        // 2. A = W H W^H : full Hermitian copy of H, X = W A (triangular W), A = X W^H (lower tiles)
+        if ((rc = herm_fill(dtype, n, dH, ldh, strideH, A, n, sAX, batch, st))) return rc;
+        {
+            GemmDesc g = gemm_desc(OP_N, OP_N, n, n, n, 1.0, Wm, n, A, n, 0.0, X, n);
             g.sA = sWm; g.sB = sAX; g.sC = sAX; g.maskA = MASK_LOWER;
             if ((rc = gemm_launch(dtype, g, batch, st))) return rc;
         }
-    for (int bi = 0; bi < nb; ++bi)
-        for (int bj = 0; bj <= bi; ++bj) {
-            GemmDesc g = gemm_desc(OP_N, OP_C, nS, nS, nS, 1.0, blk(X, bi, bj), n, Wm, nS, 0.0, blk(A, bi, bj), n);
-            g.sA = sAX; g.sB = sWm; g.sC = sAX; g.maskB = MASK_LOWER; g.cmode = (bi == bj) ? 1 : 0;
+        {
+            GemmDesc g = gemm_desc(OP_N, OP_C, n, n, n, 1.0, X, n, Wm, n, 0.0, A, n);
+            g.sA = sAX; g.sB = sWm; g.sC = sAX; g.maskB = MASK_LOWER; g.cmode = 1;
             if ((rc = gemm_launch(dtype, g, batch, st))) return rc;
         }
-
-    // 3. standard problem; eigenvectors into X
-    if ((rc = heev(dtype, n, batch, flags, A, n, sAX, dE, X, n, sAX, w + p.heev, d_info, st, nvec))) return rc;
-
-    // 4. C = W^H Z, per row block
-    for (int bi = 0; bi < nb; ++bi) {
-        GemmDesc g = gemm_desc(OP_C, OP_N, nS, nvec, nS, 1.0, Wm, nS, (char *)X + (size_t)bi * nS * es, n, 0.0,
-                               (char *)dC + (size_t)bi * nS * es, ldc);
+        // 3. standard problem; eigenvectors into X
+        if ((rc = heev(dtype, n, batch, flags, A, n, sAX, dE, X, n, sAX, w + p.heev, d_info, st, nvec))) return rc;
+        // 4. C = W^H Z
+        GemmDesc g = gemm_desc(OP_C, OP_N, n, nvec, n, 1.0, Wm, n, X, n, 0.0, dC, ldc);
         g.sA = sWm; g.sB = sAX; g.sC = strideC; g.maskA = MASK_LOWER;
         if ((rc = gemm_launch(dtype, g, batch, st))) return rc;
+    } else {
+        // Noncollinear: W_NC = diag(W, W) with W REAL (Eq. 25-27).  A complex matrix multiplied from the RIGHT by a real one is
+        // a real GEMM on its interleaved (re, im) rows -- half the DMMA work of a complex product -- so both congruences are
+        // arranged as right-multiplications:
+        //   2. Y = H W_NC^T ;  A = W_NC H W_NC^T = (Y^H) W_NC^T          3. heev          4. C^H = Z^H W_NC
+        // Real view of a complex (ld) matrix: double pointer, leading dimension 2 ld, row 2i / 2i+1 = re / im of row i.
+        double *Ar = (double *)A, *Xr = (double *)X;
+        const double *Wr = (const double *)W;
+        if ((rc = herm_fill(dtype, n, dH, ldh, strideH, A, n, sAX, batch, st))) return rc;
+        for (int bj = 0; bj < 2; ++bj) {           // Y(:, block bj) = H(:, block bj) W^T
+            const long off = 2 * (long)bj * nS * n;
+            GemmDesc g = gemm_desc(OP_N, OP_T, 2 * n, nS, nS, 1.0, Ar + off, 2L * n, Wr, nS, 0.0, Xr + off, 2L * n);
+            g.sA = 2 * sAX; g.sB = sWm; g.sC = 2 * sAX; g.maskB = MASK_LOWER;
+            if ((rc = gemm_launch(NAO_REAL, g, batch, st))) return rc;
+        }
+        if ((rc = conj_transpose(n, n, (const cplx *)X, n, sAX, (cplx *)A, n, sAX, batch, st))) return rc;       // A <- Y^H
+        for (int bi = 0; bi < 2; ++bi)
+            for (int bj = 0; bj <= bi; ++bj) {     // block (bi, bj) of (Y^H) W_NC^T, lower block triangle, into X
+                const long off = 2 * ((long)bi * nS + (long)bj * nS * n);
+                GemmDesc g = gemm_desc(OP_N, OP_T, 2 * nS, nS, nS, 1.0, Ar + off, 2L * n, Wr, nS, 0.0, Xr + off, 2L * n);
+                g.sA = 2 * sAX; g.sB = sWm; g.sC = 2 * sAX; g.maskB = MASK_LOWER; g.cmode = (bi == bj) ? 2 : 0;
+                if ((rc = gemm_launch(NAO_REAL, g, batch, st))) return rc;
+            }
+        if ((rc = copy_matrix(dtype, n, n, X, n, sAX, A, n, sAX, batch, 1, st))) return rc;                      // lower triangle
+        // 3. standard problem; eigenvectors into X
+        if ((rc = heev(dtype, n, batch, flags, A, n, sAX, dE, X, n, sAX, w + p.heev, d_info, st, nvec))) return rc;
+        // 4. C = W_NC^T Z through C^H = Z^H W_NC  (Z^H in A as an nvec x n matrix, C^H in X)
+        if ((rc = conj_transpose(n, nvec, (const cplx *)X, n, sAX, (cplx *)A, nvec, sAX, batch, st))) return rc;
+        for (int bj = 0; bj < 2; ++bj) {
+            const long off = 2 * (long)bj * nS * nvec;
+            GemmDesc g = gemm_desc(OP_N, OP_N, 2 * nvec, nS, nS, 1.0, Ar + off, 2L * nvec, Wr, nS, 0.0, Xr + off, 2L * nvec);
+            g.sA = 2 * sAX; g.sB = sWm; g.sC = 2 * sAX; g.maskB = MASK_LOWER;
+            if ((rc = gemm_launch(NAO_REAL, g, batch, st))) return rc;
+        }
+        if ((rc = conj_transpose(nvec, n, (const cplx *)X, nvec, sAX, (cplx *)dC, ldc, strideC, batch, st))) return rc;
     }
     prof_mark(8, st);
     // partial spectrum: the columns that were not back-transformed read as zero

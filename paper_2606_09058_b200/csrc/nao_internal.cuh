@@ -53,7 +53,8 @@ struct GemmDesc {
     int m, n, k;              // product dimensions: C (m x n) = op(A) (m x k) * op(B) (k x n)
     int opA, opB;
     int maskA, offA, maskB, offB;
-    int cmode;                // 0 full; 1 = skip tiles entirely above the diagonal of C
+    int cmode;                // 0 full; 1 = skip tiles entirely above the diagonal of C; 2 = the same for a complex matrix
+                              // addressed as a real one with interleaved (re, im) rows (row 2i, 2i+1 <-> complex row i)
     int conjC;                // unused (reserved)
     double alpha, beta;
     const double *scaleK;     // optional: op(A)[:,k] is multiplied by scaleK[k]
@@ -95,6 +96,8 @@ int set_zero(void *p, size_t bytes, cudaStream_t st);
 // real n x n (ldq) -> complex n x n (ldz)
 int real_to_complex(int m, int n, const double *Q, long ldq, long sQ, cplx *Z, long ldz, long sZ, int batch,
                     cudaStream_t st);
+// B (n x m) <- A^H, complex
+int conj_transpose(int m, int n, const cplx *A, long lda, long sA, cplx *B, long ldb, long sB, int batch, cudaStream_t st);
 // Linv (n x n lower, explicit zeros above, diagonal = 1/L_ii) from the packed factor in S (see nao.h)
 int unpack_linv(int dtype, int n, const void *S, long lds, long sS, void *W, long ldw, long sW, int batch,
                 cudaStream_t st);

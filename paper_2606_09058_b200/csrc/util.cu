@@ -109,6 +109,29 @@ int real_to_complex(int m, int n, const double *Q, long ldq, long sQ, cplx *Z, l
     return NAO_OK;
 }
 
+// B (n x m, ldb) <- A^H for a complex m x n matrix A (lda): 32x32 tiles through shared memory, both sides coalesced
+__global__ void conj_transpose_kernel(int m, int n, const cplx *A, long lda, long sA, cplx *B, long ldb, long sB) {
+    __shared__ cplx tile[32][33];
+    A += (long)blockIdx.z * sA; B += (long)blockIdx.z * sB;
+    const int i0 = blockIdx.x * 32, j0 = blockIdx.y * 32;
+    for (int c = threadIdx.y; c < 32; c += blockDim.y) {
+        const int i = i0 + threadIdx.x, j = j0 + c;
+        if (i < m && j < n) tile[c][threadIdx.x] = A[i + (long)j * lda];
+    }
+    __syncthreads();
+    for (int c = threadIdx.y; c < 32; c += blockDim.y) {
+        const int j = j0 + threadIdx.x, i = i0 + c;          // B(j, i) = conj(A(i, j))
+        if (i < m && j < n) { const cplx v = tile[threadIdx.x][c]; B[j + (long)i * ldb] = make_double2(v.x, -v.y); }
+    }
+}
+int conj_transpose(int m, int n, const cplx *A, long lda, long sA, cplx *B, long ldb, long sB, int batch, cudaStream_t st) {
+    if (m <= 0 || n <= 0 || batch <= 0) return NAO_OK;
+    conj_transpose_kernel<<<dim3(ceil_div(m, 32), ceil_div(n, 32), batch), dim3(32, 8), 0, st>>>(m, n, A, lda, sA, B, ldb, sB);
+    NAO_LAUNCHED();
+    NAO_CUDA_CHECK(cudaGetLastError());
+    return NAO_OK;
+}
+
 // S holds L in its lower triangle and the strict upper triangle of L^{-H} above it (nao.h).  W <- L^{-1}:
 //   W(i,j) = conj(S(j,i)) for i > j ; W(i,i) = 1/S(i,i) ; 0 above.       (reads go through 32x32 smem tiles)
 template <class T> __device__ __forceinline__ T recip_diag(T x);
