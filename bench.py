@@ -155,7 +155,11 @@ def main():
     flags = nao.NAO_NC_BLOCK_S if prob.nc_block_s else 0
     dt = nao.NAO_COMPLEX if prob.is_complex else nao.NAO_REAL
     # host (pinned) and device copies
-    Hh = torch.from_numpy(prob.H).pin_memory(); Sh = torch.from_numpy(prob.S).pin_memory()
+    # the spin channels of a collinear Gamma-point calculation share one overlap matrix: it is passed once (strideS = 0)
+    S_np = prob.S
+    if not prob.nc_block_s and prob.S.shape[0] > 1 and all(np.array_equal(prob.S[0], prob.S[b]) for b in range(1, prob.S.shape[0])):
+        S_np = np.ascontiguousarray(prob.S[:1])
+    Hh = torch.from_numpy(prob.H).pin_memory(); Sh = torch.from_numpy(S_np).pin_memory()
     H = Hh.to(dev); S0 = Sh.to(dev); S = torch.empty_like(S0)
     work = torch.empty(nao.geneig_workspace(prob.n, prob.batch, dt, flags) + 256, dtype=torch.uint8, device=dev)
     Dbuf = torch.empty_like(H)
@@ -336,7 +340,8 @@ def main():
                        "complex": bool(prob.is_complex), "parallelism": "replicas only (%d)" % world,
                        "l2_policy": ("inputs larger than L2 (H and S are %.0f MB)" % (in_bytes / 1e6)) if flush is None
                                     else "L2 flushed between timed steps (256 MB write)",
-                       "step": "first SCF step: S factored inside the step"},
+                       "step": "first SCF step: S factored inside the step",
+                       "overlap": "one S shared by the items" if Sh.shape[0] == 1 and prob.batch > 1 else "one S per item"},
             "useful_tflops": fl / (ms * 1e-3) / 1e12, "useful_flops_per_step": fl,
             "fp64_dmma_peak_tflops": FP64_DMMA_PEAK_TFLOPS,
             "ms_per_step_later_scf_steps": ms_later,

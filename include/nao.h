@@ -62,7 +62,9 @@ int nao_geneig_workspace(int n, int batch, int dtype, unsigned flags, size_t *by
  *   4 flags    OR of NAO_* flags above
  *   5 dH,ldh,strideH   in : Hermitian H; ONLY the lower triangle (i >= j) is referenced.  Not modified.
  *   8 dS,lds,strideS   in : Hermitian positive definite S, lower triangle referenced (with NAO_NC_BLOCK_S:
- *                           real, order n/2, shared by all batch items if strideS == 0).
+ *                           real, order n/2).  strideS == 0: ONE overlap matrix shared by all batch items (the spin
+ *                           channels of a collinear calculation share S): it is factored once and d_info[0] carries
+ *                           its status.
  *                      out: lower triangle = Cholesky factor L (S = L L^H); strict upper triangle = strict upper
  *                           triangle of L^{-H} (kept so that a later call with NAO_S_FACTORED skips both the
  *                           factorisation and the inversion).  With NAO_S_FACTORED: read only.

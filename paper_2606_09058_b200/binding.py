@@ -163,7 +163,7 @@ def geneig(H: torch.Tensor, S: torch.Tensor, flags: int = 0, work: torch.Tensor 
         strideS = 0 if sb == 1 else sn * sn
         lds = sn
     else:
-        strideS, lds = n * n, n
+        strideS, lds = (0 if (S.shape[0] == 1 and batch > 1) else n * n), n     # one S shared by all items
     E = torch.empty((batch, n), dtype=torch.float64, device=H.device)
     C = torch.empty_like(H)
     info = torch.zeros(batch, dtype=torch.int32, device=H.device)

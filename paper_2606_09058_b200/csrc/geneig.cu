@@ -155,7 +155,6 @@ static int geneig_impl(int n, int batch, int dtype, unsigned flags, int nvec, co
     if (!dS) return -8;
     if (lds < nS) return -9;
     const bool shared_S = (strideS == 0);
-    if (shared_S && !nc && batch > 1) return -10;
     if (!shared_S && batch > 1 && strideS < lds * (long)nS) return -10;
     if (!dE) return -11;
     if (!dC) return -12;

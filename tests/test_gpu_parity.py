@@ -437,3 +437,17 @@ def test_odd_order_1001_both_paths(nao, flag, cplx):
     assert np.abs(e - np.linalg.eigvalsh(A[0])).max() <= 1e-10
     assert np.abs(A[0] @ Zn - Zn * e).max() <= 1e-10
     assert np.abs(Zn.conj().T @ Zn - np.eye(n)).max() <= 1e-12
+
+
+def test_shared_overlap_across_spin_channels(nao):
+    """strideS = 0: the two spin channels of config 2 share S; factoring it once must give the per-item result."""
+    prob = make_config(2, nat=16)
+    assert np.array_equal(prob.S[0], prob.S[1])
+    H = torch.from_numpy(prob.H).to(DEV)
+    E1, C1, i1 = nao.geneig(H, torch.from_numpy(prob.S.copy()).to(DEV))
+    S1 = torch.from_numpy(prob.S[:1].copy()).to(DEV)
+    E2, C2, i2 = nao.geneig(H, S1)
+    assert int(i2.abs().max()) == 0
+    assert torch.equal(E1, E2) and torch.equal(C1, C2)
+    E3, C3, _ = nao.geneig(H, S1, flags=nao.NAO_S_FACTORED)
+    assert torch.equal(E1, E3) and torch.equal(C1, C3)
