@@ -68,12 +68,20 @@ NAO_EXPORT int nao_density_matrix(int n, int batch, int dtype, const void *dC, l
 // nao_occupied_count: 1 + last level (over all items) with f >= threshold
 // ---------------------------------------------------------------------------------------------------------------------
 namespace nao {
-__global__ void occupied_count_kernel(int n, int batch, const double *F, double thr, int *out) {
+// one CTA; the result goes straight to a pinned, device-mapped HOST word (the library allocates no device memory)
+__global__ void __launch_bounds__(1024) occupied_count_kernel(int n, int batch, const double *F, double thr, int *out) {
+    __shared__ int red[32];
     int last = -1;
-    for (long e = blockIdx.x * (long)blockDim.x + threadIdx.x; e < (long)n * batch; e += (long)gridDim.x * blockDim.x)
+    for (long e = threadIdx.x; e < (long)n * batch; e += blockDim.x)
         if (F[e] >= thr) last = max(last, (int)(e % n));
     for (int o = 16; o > 0; o >>= 1) last = max(last, __shfl_xor_sync(0xffffffffu, last, o));
-    if ((threadIdx.x & 31) == 0 && last >= 0) atomicMax(out, last + 1);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = last;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        last = red[threadIdx.x];
+        for (int o = 16; o > 0; o >>= 1) last = max(last, __shfl_xor_sync(0xffffffffu, last, o));
+        if (threadIdx.x == 0) *out = last + 1;
+    }
 }
 }  // namespace nao
 
@@ -84,13 +92,14 @@ NAO_EXPORT int nao_occupied_count(int n, int batch, const double *dF, double thr
     if (!dF) return -3;
     if (!h_count) return -5;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    int *d_out = nullptr;
-    if (cudaMallocAsync((void **)&d_out, sizeof(int), st) != cudaSuccess) return NAO_ERR_CUDA;
-    if (cudaMemsetAsync(d_out, 0, sizeof(int), st) != cudaSuccess) return NAO_ERR_CUDA;
-    occupied_count_kernel<<<64, 256, 0, st>>>(n, batch, dF, threshold, d_out);
+    static int *h_pinned = nullptr, *d_mapped = nullptr;
+    if (!h_pinned) {
+        if (cudaHostAlloc((void **)&h_pinned, sizeof(int), cudaHostAllocMapped) != cudaSuccess) return NAO_ERR_CUDA;
+        if (cudaHostGetDevicePointer((void **)&d_mapped, h_pinned, 0) != cudaSuccess) return NAO_ERR_CUDA;
+    }
+    occupied_count_kernel<<<1, 1024, 0, st>>>(n, batch, dF, threshold, d_mapped);
     NAO_LAUNCHED();
-    if (cudaMemcpyAsync(h_count, d_out, sizeof(int), cudaMemcpyDeviceToHost, st) != cudaSuccess) return NAO_ERR_CUDA;
     if (cudaStreamSynchronize(st) != cudaSuccess) return NAO_ERR_CUDA;
-    cudaFreeAsync(d_out, st);
+    *h_count = *h_pinned;
     return NAO_OK;
 }
