@@ -282,6 +282,32 @@ def main():
     except Exception as exc:
         partial = {"error": str(exc)}
 
+    # ---- fused call (nao_scf_step): the step takes the number of vectors from its own Fermi search; two-stage reduction
+    fused = None
+    try:
+        if big:
+            raise RuntimeError("skipped: the comparison run needs a second workspace (> 40 GB)")
+        res = {}
+        for name, f4, fresh in (("first_step", flags | nao.NAO_TRD_TWO_STAGE, True),
+                                ("later_step", flags | nao.NAO_TRD_TWO_STAGE | nao.NAO_S_FACTORED, False)):
+            def step4():
+                if fresh:
+                    S.copy_(S0)
+                return nao.scf_step(H, S, weights, prob.n_electrons, prob.kT, flags=f4, out_D=Dbuf)
+            Dref = D.clone()
+            r4 = step4(); torch.cuda.synchronize()
+            err = float((r4["D"] - Dref).abs().max())
+            ev0.record()
+            for _ in range(2):
+                step4()
+            ev1.record(); torch.cuda.synchronize()
+            res[name] = {"ms_per_step": ev0.elapsed_time(ev1) / 2, "n_vec": r4["n_vec"], "max_abs_dD_vs_full": err,
+                         "dmu_vs_full": abs(r4["mu"] - mu)}
+            del Dref, r4
+        fused = res
+    except Exception as exc:
+        fused = {"error": str(exc)}
+
     # later SCF steps reuse the factor of S: same path with NAO_S_FACTORED
     ev0.record()
     for _ in range(args.steps):
@@ -357,6 +383,7 @@ def main():
                               "kernel_ms_per_step": kgemm["ms"] / prof_steps, "launches_timed": kgemm["launches"],
                               "executed_flops_timed": kgemm["work"]},
             "partial_spectrum": partial,
+            "scf_step_fused": fused,
             "two_stage": {"ms_per_step": ms_two_stage, "phases_ms": phases_two and {k: round(v, 3) if isinstance(v, float) else v for k, v in phases_two.items()}},
             "e2e": {"value": ms_e2e * 1e-3, "unit": "s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
             "gpu_launches": int(launches) * args.steps,

@@ -104,6 +104,22 @@ int nao_geneig_partial(int n, int batch, int dtype, unsigned flags, int n_vec,
                        void *dwork, size_t work_bytes, int *d_info, void *cuda_stream);
 
 /*
+ * One SCF step of the hot path in one call (the paper's Parts 2-4 / 3-5): eigenvalues of the
+ * pencil, Fermi level and occupations, back-transformation of ONLY the eigenvectors whose occupation is >= 1e-17 (their
+ * number, plus a margin of 2 %, is returned in *h_nvec), D = C diag(f) C^H.  dE, *h_mu, dF and dD equal the results of
+ * nao_geneig + nao_fermi_mu + nao_density_matrix; dC holds the first *h_nvec eigenvectors, its other columns are zero.
+ * Arguments as in those three calls (h_weight, h_mu, h_nvec are HOST pointers); dwork needs nao_scf_step_workspace bytes.
+ * The call synchronises the stream twice (Fermi level, vector count).
+ */
+int nao_scf_step_workspace(int n, int batch, int dtype, unsigned flags, size_t *bytes);
+int nao_scf_step(int n, int batch, int dtype, unsigned flags,
+                 const void *dH, long ldh, long strideH, void *dS, long lds, long strideS,
+                 const double *h_weight, double n_electrons, double kT,
+                 double *dE, double *h_mu, double *dF,
+                 void *dC, long ldc, long strideC, void *dD, long ldd, long strideD,
+                 int *h_nvec, void *dwork, size_t work_bytes, int *d_info, void *cuda_stream);
+
+/*
  * 1 + the largest level index i (over all batch items) with dF[b*n + i] >= threshold: the number of leading
  * eigenvectors nao_density_matrix reads.  Synchronises the stream to write *h_count (HOST int).
  */

@@ -30,6 +30,9 @@ _SIGNATURES = {
     "nao_geneig": ([_i, _i, _i, ctypes.c_uint, _vp, _l, _l, _vp, _l, _l, _vp, _vp, _l, _l, _vp, _sz, _vp, _vp], _i),
     "nao_geneig_partial": ([_i, _i, _i, ctypes.c_uint, _i, _vp, _l, _l, _vp, _l, _l, _vp, _vp, _l, _l, _vp, _sz, _vp, _vp], _i),
     "nao_occupied_count": ([_i, _i, _vp, _d, ctypes.POINTER(ctypes.c_int), _vp], _i),
+    "nao_scf_step_workspace": ([_i, _i, _i, ctypes.c_uint, _szp], _i),
+    "nao_scf_step": ([_i, _i, _i, ctypes.c_uint, _vp, _l, _l, _vp, _l, _l, _dp, _d, _d, _vp, _dp, _vp, _vp, _l, _l, _vp, _l, _l,
+                     ctypes.POINTER(ctypes.c_int), _vp, _sz, _vp, _vp], _i),
     "nao_fermi_workspace": ([_i, _i, _szp], _i),
     "nao_fermi_mu": ([_i, _i, _vp, _dp, _d, _d, _dp, _vp, _vp, _vp], _i),
     "nao_density_workspace": ([_i, _i, _i, _szp], _i),
@@ -180,6 +183,35 @@ def geneig(H: torch.Tensor, S: torch.Tensor, flags: int = 0, work: torch.Tensor 
                                       _dev(info, "info"), _stream(H))
         _check(rc, "nao_geneig_partial")
     return E, C, info
+
+
+def scf_step(H: torch.Tensor, S: torch.Tensor, weights, n_electrons: float, kT: float, flags: int = 0,
+             work: torch.Tensor | None = None, out_D: torch.Tensor | None = None):
+    """nao_scf_step: eigenvalues, Fermi level, the occupied eigenvectors and the density matrix in one call.
+    Returns dict(E, mu, F, C, D, n_vec, info)."""
+    batch, n, _ = H.shape
+    dt = _dtype_code(H)
+    if flags & NAO_NC_BLOCK_S:
+        sn = S.shape[-1]
+        strideS, lds = (0 if S.shape[0] == 1 else sn * sn), sn
+    else:
+        strideS, lds = (0 if (S.shape[0] == 1 and batch > 1) else n * n), n
+    need = ctypes.c_size_t(0)
+    _check(lib().nao_scf_step_workspace(n, batch, dt, flags, ctypes.byref(need)), "nao_scf_step_workspace")
+    if work is None or work.numel() < need.value:
+        work = _workspace(need.value, H.device)
+    E = torch.empty((batch, n), dtype=torch.float64, device=H.device)
+    F = torch.empty_like(E)
+    C = torch.empty_like(H)
+    D = torch.empty_like(H) if out_D is None else out_D
+    info = torch.zeros(batch, dtype=torch.int32, device=H.device)
+    w = (ctypes.c_double * batch)(*[float(x) for x in weights])
+    mu, nvec = ctypes.c_double(0.0), ctypes.c_int(0)
+    rc = lib().nao_scf_step(n, batch, dt, flags, _dev(H, "H"), n, n * n, _dev(S, "S"), lds, strideS, w, float(n_electrons),
+                            float(kT), _dev(E, "E"), ctypes.byref(mu), _dev(F, "F"), _dev(C, "C"), n, n * n, _dev(D, "D"), n, n * n,
+                            ctypes.byref(nvec), _dev(work, "work"), work.numel(), _dev(info, "info"), _stream(H))
+    _check(rc, "nao_scf_step")
+    return dict(E=E, mu=mu.value, F=F, C=C, D=D, n_vec=nvec.value, info=info)
 
 
 def occupied_count(F: torch.Tensor, threshold: float = 1e-17) -> int:

@@ -43,32 +43,38 @@ static HeevPlan heev_plan(int dtype, int n, int batch, unsigned flags) {
 }
 
 static int heev(int dtype, int n, int batch, unsigned flags, void *A, long lda, long sA, double *E, void *Z, long ldz,
-                long sZ, void *work, int *d_info, cudaStream_t st, int nvec = -1) {
-    if (nvec < 0 || nvec > n) nvec = n;      // eigenvectors wanted: the nvec lowest
+                long sZ, void *work, int *d_info, cudaStream_t st, int nvec = -1, int phase = 3) {
+    // phase bit 0: reduction to tridiagonal form + D&C (eigenvalues; Q_T and the reflectors stay in the workspace)
+    // phase bit 1: back-transformation of the nvec lowest eigenvectors
+    if (nvec < 0 || nvec > n) nvec = n;
     HeevPlan p = heev_plan(dtype, n, batch, flags);
     char *w = (char *)work;
     double *d = (double *)(w + p.d), *e = (double *)(w + p.e);
     void *tau = w + p.tau, *sub = w + p.sub;
     void *V2 = w + p.v2, *tau2 = w + p.tau2;
-    int rc;
-    prof_mark(2, st);
-    if (p.two_stage) {
-        if ((rc = he2hb(dtype, n, batch, A, lda, sA, tau, sub, st))) return rc;
-        prof_mark(3, st);
-        if ((rc = hb2st(dtype, n, batch, A, lda, sA, d, e, V2, n, (long)n * n, tau2, sub, st))) return rc;
-    } else {
-        if ((rc = hetrd(dtype, n, batch, A, lda, sA, d, e, tau, sub, st))) return rc;
-        prof_mark(3, st);
+    int rc = NAO_OK;
+    if (phase & 1) {
+        prof_mark(2, st);
+        if (p.two_stage) {
+            if ((rc = he2hb(dtype, n, batch, A, lda, sA, tau, sub, st))) return rc;
+            prof_mark(3, st);
+            if ((rc = hb2st(dtype, n, batch, A, lda, sA, d, e, V2, n, (long)n * n, tau2, sub, st))) return rc;
+        } else {
+            if ((rc = hetrd(dtype, n, batch, A, lda, sA, d, e, tau, sub, st))) return rc;
+            prof_mark(3, st);
+        }
+        prof_mark(4, st);
+        if (dtype == NAO_COMPLEX) {
+            double *qt = (double *)(w + p.qt);
+            if ((rc = stedc(n, batch, d, e, E, qt, n, (long)n * n, sub, d_info, st))) return rc;
+        } else {
+            if ((rc = stedc(n, batch, d, e, E, (double *)Z, ldz, sZ, sub, d_info, st))) return rc;
+        }
+        prof_mark(5, st);
     }
-    prof_mark(4, st);
-    if (dtype == NAO_COMPLEX) {
-        double *qt = (double *)(w + p.qt);
-        if ((rc = stedc(n, batch, d, e, E, qt, n, (long)n * n, sub, d_info, st))) return rc;
-        if ((rc = real_to_complex(n, nvec, qt, n, (long)n * n, (cplx *)Z, ldz, sZ, batch, st))) return rc;
-    } else {
-        if ((rc = stedc(n, batch, d, e, E, (double *)Z, ldz, sZ, sub, d_info, st))) return rc;
-    }
-    prof_mark(5, st);
+    if (!(phase & 2)) return rc;
+    if (dtype == NAO_COMPLEX)
+        if ((rc = real_to_complex(n, nvec, (const double *)(w + p.qt), n, (long)n * n, (cplx *)Z, ldz, sZ, batch, st))) return rc;
     if (p.two_stage) {
         if ((rc = q2_apply(dtype, n, nvec, batch, V2, n, (long)n * n, tau2, Z, ldz, sZ, sub, st))) return rc;
         prof_mark(6, st);
@@ -139,9 +145,12 @@ NAO_EXPORT int nao_geneig_workspace(int n, int batch, int dtype, unsigned flags,
     return NAO_OK;
 }
 
+// phase bit 0: factor S, reduce, tridiagonalise, D&C (eigenvalues in dE; everything the back-transformation needs stays in
+// dwork);  phase bit 1: back-transform the nvec lowest eigenvectors and form C.  A phase-2 call must follow a phase-1 call
+// with the same arguments and an untouched workspace.
 static int geneig_impl(int n, int batch, int dtype, unsigned flags, int nvec, const void *dH, long ldh, long strideH, void *dS,
                        long lds, long strideS, double *dE, void *dC, long ldc, long strideC, void *dwork,
-                       size_t work_bytes, int *d_info, void *cuda_stream) {
+                       size_t work_bytes, int *d_info, void *cuda_stream, int phase = 3) {
     using namespace nao;
     if (n < 1) return -1;
     if (batch < 1) return -2;
@@ -170,6 +179,9 @@ static int geneig_impl(int n, int batch, int dtype, unsigned flags, int nvec, co
     void *W = w + p.W, *A = w + p.A, *X = w + p.X;
     const long sW = (long)nS * nS, sAX = (long)n * n;
     int rc;
+    const void *Wm = W;
+    const long sWm = shared_S ? 0 : sW;
+    if (phase & 1) {
     NAO_CUDA_CHECK(cudaMemsetAsync(d_info, 0, sizeof(int) * batch, st));
 
     // 1. factor (or unpack) S
@@ -182,9 +194,9 @@ static int geneig_impl(int n, int batch, int dtype, unsigned flags, int nvec, co
         if ((rc = unpack_linv(p.sdtype, nS, dS, lds, strideS, W, nS, sW, p.nitemsS, st))) return rc;
     }
     prof_mark(1, st);
-    const void *Wm = W;
-    const long sWm = shared_S ? 0 : sW;
+    }
     if (!nc) {
+        if (phase & 1) {
         // 2. A = W H W^H : full Hermitian copy of H, X = W A (triangular W), A = X W^H (lower tiles)
         if ((rc = herm_fill(dtype, n, dH, ldh, strideH, A, n, sAX, batch, st))) return rc;
         {
@@ -198,7 +210,10 @@ static int geneig_impl(int n, int batch, int dtype, unsigned flags, int nvec, co
             if ((rc = gemm_launch(dtype, g, batch, st))) return rc;
         }
         // 3. standard problem; eigenvectors into X
-        if ((rc = heev(dtype, n, batch, flags, A, n, sAX, dE, X, n, sAX, w + p.heev, d_info, st, nvec))) return rc;
+        if ((rc = heev(dtype, n, batch, flags, A, n, sAX, dE, X, n, sAX, w + p.heev, d_info, st, nvec, 1))) return rc;
+        }
+        if (!(phase & 2)) return NAO_OK;
+        if ((rc = heev(dtype, n, batch, flags, A, n, sAX, dE, X, n, sAX, w + p.heev, d_info, st, nvec, 2))) return rc;
         // 4. C = W^H Z
         GemmDesc g = gemm_desc(OP_C, OP_N, n, nvec, n, 1.0, Wm, n, X, n, 0.0, dC, ldc);
         g.sA = sWm; g.sB = sAX; g.sC = strideC; g.maskA = MASK_LOWER;
@@ -211,6 +226,7 @@ static int geneig_impl(int n, int batch, int dtype, unsigned flags, int nvec, co
         // Real view of a complex (ld) matrix: double pointer, leading dimension 2 ld, row 2i / 2i+1 = re / im of row i.
         double *Ar = (double *)A, *Xr = (double *)X;
         const double *Wr = (const double *)W;
+        if (phase & 1) {
         if ((rc = herm_fill(dtype, n, dH, ldh, strideH, A, n, sAX, batch, st))) return rc;
         for (int bj = 0; bj < 2; ++bj) {           // Y(:, block bj) = H(:, block bj) W^T
             const long off = 2 * (long)bj * nS * n;
@@ -228,7 +244,10 @@ static int geneig_impl(int n, int batch, int dtype, unsigned flags, int nvec, co
             }
         if ((rc = copy_matrix(dtype, n, n, X, n, sAX, A, n, sAX, batch, 1, st))) return rc;                      // lower triangle
         // 3. standard problem; eigenvectors into X
-        if ((rc = heev(dtype, n, batch, flags, A, n, sAX, dE, X, n, sAX, w + p.heev, d_info, st, nvec))) return rc;
+        if ((rc = heev(dtype, n, batch, flags, A, n, sAX, dE, X, n, sAX, w + p.heev, d_info, st, nvec, 1))) return rc;
+        }
+        if (!(phase & 2)) return NAO_OK;
+        if ((rc = heev(dtype, n, batch, flags, A, n, sAX, dE, X, n, sAX, w + p.heev, d_info, st, nvec, 2))) return rc;
         // 4. C = W_NC^T Z through C^H = Z^H W_NC  (Z^H in A as an nvec x n matrix, C^H in X)
         if ((rc = conj_transpose(n, nvec, (const cplx *)X, n, sAX, (cplx *)A, nvec, sAX, batch, st))) return rc;
         for (int bj = 0; bj < 2; ++bj) {
@@ -267,4 +286,57 @@ NAO_EXPORT int nao_geneig_partial(int n, int batch, int dtype, unsigned flags, i
     int rc = geneig_impl(n, batch, dtype, flags, n_vec, dH, ldh, strideH, dS, lds, strideS, dE, dC, ldc, strideC, dwork,
                          work_bytes, d_info, cuda_stream);
     return (rc <= -5) ? rc - 1 : rc;          // argument positions after n_vec are shifted by one
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// nao_scf_step: the whole hot path of one SCF step in one call -- eigenvalues, Fermi level, then only the eigenvectors the
+// density matrix reads are back-transformed (count taken from the step's own occupations), then D.
+// ---------------------------------------------------------------------------------------------------------------------
+extern "C" int nao_fermi_workspace(int n, int batch, size_t *bytes);
+extern "C" int nao_density_workspace(int n, int batch, int dtype, size_t *bytes);
+extern "C" int nao_occupied_count(int n, int batch, const double *dF, double threshold, int *h_count, void *cuda_stream);
+extern "C" int nao_density_matrix(int n, int batch, int dtype, const void *dC, long ldc, long strideC, const double *dF, void *dD,
+                                  long ldd, long strideD, void *dwork, size_t work_bytes, void *cuda_stream);
+
+NAO_EXPORT int nao_scf_step_workspace(int n, int batch, int dtype, unsigned flags, size_t *bytes) {
+    size_t g = 0, f = 0, d = 0;
+    int rc;
+    if ((rc = nao_geneig_workspace(n, batch, dtype, flags, &g))) return rc;
+    if ((rc = nao_fermi_workspace(n, batch, &f))) return rc;
+    if ((rc = nao_density_workspace(n, batch, dtype, &d))) return rc;
+    *bytes = nao::align_up(g) + nao::align_up(f) + nao::align_up(d);
+    return NAO_OK;
+}
+
+NAO_EXPORT int nao_scf_step(int n, int batch, int dtype, unsigned flags, const void *dH, long ldh, long strideH, void *dS,
+                            long lds, long strideS, const double *h_weight, double n_electrons, double kT, double *dE,
+                            double *h_mu, double *dF, void *dC, long ldc, long strideC, void *dD, long ldd, long strideD,
+                            int *h_nvec, void *dwork, size_t work_bytes, int *d_info, void *cuda_stream) {
+    using namespace nao;
+    if (!h_weight) return -11;
+    if (!h_mu) return -15;
+    if (!dF) return -16;
+    if (!dD) return -20;
+    if (ldd < n) return -21;
+    if (batch > 1 && strideD < ldd * (long)n) return -22;
+    size_t g = 0, f = 0, d = 0, total = 0;
+    int rc;
+    if ((rc = nao_scf_step_workspace(n, batch, dtype, flags, &total))) return rc;
+    if (work_bytes < total) return NAO_ERR_WORKSPACE;
+    nao_geneig_workspace(n, batch, dtype, flags, &g); nao_fermi_workspace(n, batch, &f); nao_density_workspace(n, batch, dtype, &d);
+    char *wg = (char *)dwork, *wf = wg + align_up(g), *wd = wf + align_up(f);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    // eigenvalues (phase 1); argument errors of the shared prefix are reported with the positions of nao_geneig
+    rc = geneig_impl(n, batch, dtype, flags, n, dH, ldh, strideH, dS, lds, strideS, dE, dC, ldc, strideC, wg, g, d_info, cuda_stream, 1);
+    if (rc) return rc;
+    if ((rc = fermi_mu(n, batch, dE, h_weight, n_electrons, kT, h_mu, dF, wf, st))) return rc;
+    int cnt = 0;
+    if ((rc = nao_occupied_count(n, batch, dF, 1e-17, &cnt, cuda_stream))) return rc;
+    int nvec = cnt + (cnt / 50 > 8 ? cnt / 50 : 8);          // margin: 2 %, at least 8 states (all of them have f < 1e-17)
+    if (nvec > n) nvec = n;
+    if (nvec < 1) nvec = 1;
+    if (h_nvec) *h_nvec = nvec;
+    rc = geneig_impl(n, batch, dtype, flags, nvec, dH, ldh, strideH, dS, lds, strideS, dE, dC, ldc, strideC, wg, g, d_info, cuda_stream, 2);
+    if (rc) return rc;
+    return nao_density_matrix(n, batch, dtype, dC, ldc, strideC, dF, dD, ldd, strideD, wd, d, cuda_stream);
 }

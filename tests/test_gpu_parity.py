@@ -451,3 +451,25 @@ def test_shared_overlap_across_spin_channels(nao):
     assert torch.equal(E1, E2) and torch.equal(C1, C2)
     E3, C3, _ = nao.geneig(H, S1, flags=nao.NAO_S_FACTORED)
     assert torch.equal(E1, E3) and torch.equal(C1, C3)
+
+
+@pytest.mark.parametrize("two_stage", [False, True])
+def test_scf_step_fused_against_oracle(nao, two_stage):
+    """nao_scf_step: eigenvalues -> Fermi level -> occupied eigenvectors -> D in one call, against the oracle on the
+    config-1 (16 complex items, one shared mu), config-2 and config-3 (block S) recipes."""
+    for idx, nat in ((1, 16), (2, 32), (3, 16)):
+        prob = make_config(idx, nat=nat)
+        ref = oracle.solve_problem(prob)
+        flags = (nao.NAO_NC_BLOCK_S if prob.nc_block_s else 0) | (nao.NAO_TRD_TWO_STAGE if two_stage else 0)
+        H = torch.from_numpy(prob.H).to(DEV)
+        S = torch.from_numpy(prob.S.copy()).to(DEV)
+        r = nao.scf_step(H, S, prob.weights, prob.n_electrons, prob.kT, flags=flags)
+        assert int(r["info"].abs().max()) == 0
+        assert 0 < r["n_vec"] <= prob.n
+        assert np.abs(r["E"].cpu().numpy() - ref["e"]).max() <= TOL_E
+        assert abs(r["mu"] - ref["mu"]) <= TOL_MU
+        assert np.abs(r["F"].cpu().numpy() - ref["f"]).max() <= 1e-7
+        for b in range(prob.batch):
+            assert np.abs(to_np(r["D"])[b] - ref["D"][b]).max() <= TOL_D
+        Cb = to_np(r["C"])[0][:, :r["n_vec"]]
+        assert np.abs(Cb.conj().T @ prob.S_full(0) @ Cb - np.eye(r["n_vec"])).max() <= TOL_ORTH
