@@ -200,9 +200,8 @@ __global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
         store_D(r0, Lp);
         if (tid < b) s_vp[tid] = s_vn[tid];
         if (tid == 0) s_tau_p = s_tau_n;
-        __threadfence();
         __syncthreads();
-        if (tid == 0) st_release(prog + s, 1);
+        if (tid == 0) { __threadfence(); st_release(prog + s, 1); }
         // ------------------------------------------------ steps k >= 1
         for (int k = 1;; ++k) {
             const int q0 = s + 1 + k * b;
@@ -291,10 +290,11 @@ __global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
                     }
                 }
             }
-            __threadfence();
+            // publish: the block barrier orders every thread's stores before thread 0, whose fence + release store make
+            // them visible to the CTA that acquires the counter (the pattern of a cooperative-groups grid sync)
             __syncthreads();
             if (tid < b) s_vp[tid] = s_vn[tid];
-            if (tid == 0) { s_tau_p = s_tau_n; st_release(prog + s, k + 1); }
+            if (tid == 0) { s_tau_p = s_tau_n; __threadfence(); st_release(prog + s, k + 1); }
             r0 = q0; Lp = Lq;
         }
         __syncthreads();
