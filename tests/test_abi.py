@@ -67,6 +67,17 @@ def test_host_side_argument_validation(libpath):
     assert lib.nao_fermi_mu(4, 1, 1, w, 9.0, 1e-3, ctypes.byref(mu), 1, 1, None) == 3      # NAO_ERR_ELECTRONS
     assert lib.nao_fermi_mu(4, 1, 1, w, 2.0, 0.0, ctypes.byref(mu), 1, 1, None) == 3
     assert lib.nao_fermi_mu(4, 1, None, w, 2.0, 1e-3, ctypes.byref(mu), 1, 1, None) == -3
+    # partial spectrum / fused step: the extra arguments are validated on the host as well
+    vp, l, i = ctypes.c_void_p, ctypes.c_long, ctypes.c_int
+    lib.nao_geneig_partial.argtypes = [i, i, i, ctypes.c_uint, i, vp, l, l, vp, l, l, vp, vp, l, l, vp, ctypes.c_size_t, vp, vp]
+    assert lib.nao_geneig_partial(8, 1, 0, 0, 0, 1, 8, 64, 1, 8, 64, 1, 1, 8, 64, 1, 1 << 20, 1, None) == -5     # n_vec < 1
+    assert lib.nao_geneig_partial(8, 1, 0, 0, 9, 1, 8, 64, 1, 8, 64, 1, 1, 8, 64, 1, 1 << 20, 1, None) == -5     # n_vec > n
+    assert lib.nao_geneig_partial(8, 1, 0, 0, 4, None, 8, 64, 1, 8, 64, 1, 1, 8, 64, 1, 1 << 20, 1, None) == -6  # dH
+    assert lib.nao_scf_step_workspace(104, 2, 0, 0, ctypes.byref(sz)) == 0 and sz.value > 2 * 104 * 104 * 8 * 2
+    lib.nao_occupied_count.argtypes = [i, i, vp, ctypes.c_double, ctypes.POINTER(i), vp]
+    cnt = i(0)
+    assert lib.nao_occupied_count(0, 1, 1, 1e-17, ctypes.byref(cnt), None) == -1
+    assert lib.nao_occupied_count(4, 1, None, 1e-17, ctypes.byref(cnt), None) == -3
 
 
 def test_no_product_import_of_oracle():
