@@ -64,15 +64,24 @@ static int heev(int dtype, int n, int batch, unsigned flags, void *A, long lda, 
             prof_mark(3, st);
         }
         prof_mark(4, st);
+        // with both phases in one call the D&C runs through; otherwise it stops at the eigenvalues and is continued below
+        const int dc_phase = (phase & 2) ? 3 : 1;
         if (dtype == NAO_COMPLEX) {
             double *qt = (double *)(w + p.qt);
-            if ((rc = stedc(n, batch, d, e, E, qt, n, (long)n * n, sub, d_info, st))) return rc;
+            if ((rc = stedc(n, batch, d, e, E, qt, n, (long)n * n, sub, d_info, st, nvec, dc_phase))) return rc;
         } else {
-            if ((rc = stedc(n, batch, d, e, E, (double *)Z, ldz, sZ, sub, d_info, st))) return rc;
+            if ((rc = stedc(n, batch, d, e, E, (double *)Z, ldz, sZ, sub, d_info, st, nvec, dc_phase))) return rc;
         }
         prof_mark(5, st);
     }
     if (!(phase & 2)) return rc;
+    if (!(phase & 1)) {        // eigenvectors of the tridiagonal matrix: only the nvec lowest (top merge restricted)
+        if (dtype == NAO_COMPLEX) {
+            if ((rc = stedc(n, batch, d, e, E, (double *)(w + p.qt), n, (long)n * n, sub, d_info, st, nvec, 2))) return rc;
+        } else {
+            if ((rc = stedc(n, batch, d, e, E, (double *)Z, ldz, sZ, sub, d_info, st, nvec, 2))) return rc;
+        }
+    }
     if (dtype == NAO_COMPLEX)
         if ((rc = real_to_complex(n, nvec, (const double *)(w + p.qt), n, (long)n * n, (cplx *)Z, ldz, sZ, batch, st))) return rc;
     if (p.two_stage) {
@@ -210,10 +219,11 @@ static int geneig_impl(int n, int batch, int dtype, unsigned flags, int nvec, co
             if ((rc = gemm_launch(dtype, g, batch, st))) return rc;
         }
         // 3. standard problem; eigenvectors into X
-        if ((rc = heev(dtype, n, batch, flags, A, n, sAX, dE, X, n, sAX, w + p.heev, d_info, st, nvec, 1))) return rc;
+        if ((rc = heev(dtype, n, batch, flags, A, n, sAX, dE, X, n, sAX, w + p.heev, d_info, st, nvec, (phase & 2) ? 3 : 1))) return rc;
         }
         if (!(phase & 2)) return NAO_OK;
-        if ((rc = heev(dtype, n, batch, flags, A, n, sAX, dE, X, n, sAX, w + p.heev, d_info, st, nvec, 2))) return rc;
+        if (!(phase & 1))
+            if ((rc = heev(dtype, n, batch, flags, A, n, sAX, dE, X, n, sAX, w + p.heev, d_info, st, nvec, 2))) return rc;
         // 4. C = W^H Z
         GemmDesc g = gemm_desc(OP_C, OP_N, n, nvec, n, 1.0, Wm, n, X, n, 0.0, dC, ldc);
         g.sA = sWm; g.sB = sAX; g.sC = strideC; g.maskA = MASK_LOWER;
@@ -244,10 +254,11 @@ static int geneig_impl(int n, int batch, int dtype, unsigned flags, int nvec, co
             }
         if ((rc = copy_matrix(dtype, n, n, X, n, sAX, A, n, sAX, batch, 1, st))) return rc;                      // lower triangle
         // 3. standard problem; eigenvectors into X
-        if ((rc = heev(dtype, n, batch, flags, A, n, sAX, dE, X, n, sAX, w + p.heev, d_info, st, nvec, 1))) return rc;
+        if ((rc = heev(dtype, n, batch, flags, A, n, sAX, dE, X, n, sAX, w + p.heev, d_info, st, nvec, (phase & 2) ? 3 : 1))) return rc;
         }
         if (!(phase & 2)) return NAO_OK;
-        if ((rc = heev(dtype, n, batch, flags, A, n, sAX, dE, X, n, sAX, w + p.heev, d_info, st, nvec, 2))) return rc;
+        if (!(phase & 1))
+            if ((rc = heev(dtype, n, batch, flags, A, n, sAX, dE, X, n, sAX, w + p.heev, d_info, st, nvec, 2))) return rc;
         // 4. C = W_NC^T Z through C^H = Z^H W_NC  (Z^H in A as an nvec x n matrix, C^H in X)
         if ((rc = conj_transpose(n, nvec, (const cplx *)X, n, sAX, (cplx *)A, nvec, sAX, batch, st))) return rc;
         for (int bj = 0; bj < 2; ++bj) {

@@ -146,8 +146,9 @@ int q2_apply(int dtype, int n, int ncols, int batch, const void *V2, long ldv, l
 
 // stedc.cu
 size_t stedc_workspace(int n, int batch);
+// nvec: eigenvectors wanted (the nvec lowest); phase 1 = eigenvalues, 2 = eigenvectors (continues a phase-1 call), 3 = both
 int stedc(int n, int batch, double *d, double *e, double *evals, double *Q, long ldq, long sQ, void *work,
-          int *d_info, cudaStream_t st);
+          int *d_info, cudaStream_t st, int nvec = -1, int phase = 3);
 
 // api.cu: phase-boundary event (no-op unless nao_profile_enable(1))
 void prof_mark(int idx, cudaStream_t st);

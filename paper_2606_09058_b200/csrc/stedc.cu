@@ -40,6 +40,7 @@ struct DcBuf {
     double *Qw, *S;                // n x n each, ld n
     double *z, *dlam, *wz, *dcol, *dnew, *zhat, *rot_c, *rot_s, *ds, *zs, *scale;
     int *idxq, *src, *indxp, *coltyp, *gcol, *gsec, *rot_p, *rot_q;
+    int *kneed;                    // per item: secular roots of the top merge among the wanted eigenvalues
     DcOut *out;                    // per node of the current level (max nodes per level entries)
     GemmDesc *desc;                // 2 per node
     int n;
@@ -319,13 +320,14 @@ __global__ void __launch_bounds__(256) dc_zhat_kernel(DcBuf b, const DcNode *__r
 }
 
 // column j of S (grouped row order): s_i = zhat_i / (d_i - lambda_j), normalised
-__global__ void __launch_bounds__(128) dc_vectors_kernel(DcBuf b, const DcNode *__restrict__ nodes, int maxnodes) {
+__global__ void __launch_bounds__(128) dc_vectors_kernel(DcBuf b, const DcNode *__restrict__ nodes, int maxnodes, int restricted) {
     __shared__ double red[4];
     const int node = blockIdx.y, item = blockIdx.z, n = b.n;
     const DcNode nd = nodes[node];
     const int K = b.out[(long)item * maxnodes + node].K;
     const int j = blockIdx.x;
     if (j >= K) return;
+    if (restricted && j >= b.kneed[item]) return;          // top merge, partial spectrum: unwanted columns are skipped
     const long ib = (long)item * n + nd.off;
     const double *dl = b.Q + (long)item * b.sQ + nd.off + (long)(nd.off + j) * b.ldq;
     double *Sc = b.S + (long)item * n * n + nd.off + (long)(nd.off + j) * n;
@@ -367,20 +369,52 @@ __global__ void __launch_bounds__(256) dc_finish_kernel(DcBuf b, const DcNode *_
     }
 }
 
-// eigenvalues (rescaled) in ascending order and the matching permutation of the eigenvector columns
-__global__ void dc_final_kernel(DcBuf b, double *evals, double *Qout, long ldo, long sO) {
+// Top merge with only the nvec lowest eigenpairs wanted: the secular roots dnew[0:K) are ascending, so the
+// wanted ones are a prefix; its length (sorted position of root i = i + #{deflated values below it} < nvec) becomes the
+// column count of the two merge GEMMs.  Runs after dc_finish_kernel-style ranking data (dnew) is complete.
+__global__ void __launch_bounds__(256) dc_restrict_kernel(DcBuf b, const DcNode *__restrict__ nodes, int maxnodes, int nvec) {
+    __shared__ int red[8];
+    const int item = blockIdx.x, n = b.n;
+    const DcNode nd = nodes[0];
+    const int N = nd.n1 + nd.n2;
+    const int K = b.out[(long)item * maxnodes].K;
+    const double *dnew = b.dnew + (long)item * n + nd.off;
+    const int nb = N - K;
+    int cnt = 0;
+    for (int i = threadIdx.x; i < K; i += blockDim.x) {
+        const double a = dnew[i];
+        int lo = 0, hi = nb;
+        while (lo < hi) { int mid = (lo + hi) >> 1; if (dnew[N - 1 - mid] < a) lo = mid + 1; else hi = mid; }
+        if (i + lo < nvec) ++cnt;
+    }
+    for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = cnt;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int t = 0;
+        for (int w = 0; w < 8; ++w) t += red[w];
+        b.kneed[item] = t;
+        b.desc[(long)item * 2].n = t;
+        b.desc[(long)item * 2 + 1].n = t;
+    }
+}
+
+// eigenvalues (rescaled) in ascending order ...
+__global__ void dc_final_evals_kernel(DcBuf b, double *evals) {
+    const int item = blockIdx.y, n = b.n;
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= n) return;
+    evals[(long)item * n + c] = b.scale[item] * b.d[(long)item * n + b.idxq[(long)item * n + c]];
+}
+// ... and the matching permutation of the first ncols eigenvector columns
+__global__ void dc_final_kernel(DcBuf b, double *Qout, long ldo, long sO, int ncols) {
     const int item = blockIdx.z, n = b.n;
     const int row = blockIdx.x * blockDim.x + threadIdx.x;
     if (row >= n) return;
     const double *Q = b.Q + (long)item * b.sQ;
     double *Qo = Qout + (long)item * sO;
     const int *idxq = b.idxq + (long)item * n;
-    const double sc = b.scale[item];
-    for (int c = blockIdx.y; c < n; c += gridDim.y) {
-        const int s = idxq[c];
-        Qo[row + (long)c * ldo] = Q[row + (long)s * b.ldq];
-        if (row == 0) evals[(long)item * n + c] = sc * b.d[(long)item * n + s];
-    }
+    for (int c = blockIdx.y; c < ncols; c += gridDim.y) Qo[row + (long)c * ldo] = Q[row + (long)idxq[c] * b.ldq];
 }
 
 // ------------------------------------------------------------------------------------------------ host driver
@@ -429,6 +463,7 @@ static DcWork dc_carve(int n, int batch, const DcPlan &p, void *work) {
     w.b.scale = ar.get<double>(batch);
     int **ip[] = {&w.b.idxq, &w.b.src, &w.b.indxp, &w.b.coltyp, &w.b.gcol, &w.b.gsec, &w.b.rot_p, &w.b.rot_q};
     for (auto q : ip) *q = ar.get<int>(bn);
+    w.b.kneed = ar.get<int>(batch);
     w.b.out = ar.get<DcOut>((size_t)batch * p.maxnodes);
     w.b.desc = ar.get<GemmDesc>((size_t)batch * p.maxnodes * 2);
     size_t nnodes = 0; for (auto &l : p.levels) nnodes += l.size();
@@ -440,53 +475,83 @@ static DcWork dc_carve(int n, int batch, const DcPlan &p, void *work) {
 }
 size_t stedc_workspace(int n, int batch) { DcPlan p = dc_plan(n); return dc_carve(n, batch, p, nullptr).bytes; }
 
+// phase bit 0: everything up to the eigenvalues (all levels; of the top merge: deflation, secular equation, ranking);
+// phase bit 1: eigenvectors of the top merge -- only the columns that end up among the nvec lowest -- and the sorted copy of
+// the first nvec columns into Qout.  A phase-2 call continues a phase-1 call on the same workspace.
 int stedc(int n, int batch, double *d, double *e, double *evals, double *Qout, long ldq, long sQ, void *work, int *d_info,
-          cudaStream_t st) {
+          cudaStream_t st, int nvec, int phase) {
+    if (nvec < 0 || nvec > n) nvec = n;
     DcPlan p = dc_plan(n);
     DcWork w = dc_carve(n, batch, p, work);
     w.b.d = d; w.b.e = e;
     const int nleaves = (int)p.leaf_off.size() - 1;
-    // host -> device: tree description (tiny; pageable copy is staged before the call returns)
-    std::vector<int> cuts;
-    for (int i = 1; i < nleaves; ++i) cuts.push_back(p.leaf_off[i]);
-    if (!cuts.empty()) NAO_CUDA_CHECK(cudaMemcpyAsync(w.cuts, cuts.data(), cuts.size() * 4, cudaMemcpyHostToDevice, st));
-    NAO_CUDA_CHECK(cudaMemcpyAsync(w.leaf_off, p.leaf_off.data(), p.leaf_off.size() * 4, cudaMemcpyHostToDevice, st));
-    std::vector<DcNode> flat; std::vector<size_t> lvl_off;
-    for (auto &l : p.levels) { lvl_off.push_back(flat.size()); flat.insert(flat.end(), l.begin(), l.end()); }
-    if (!flat.empty()) NAO_CUDA_CHECK(cudaMemcpyAsync(w.nodes, flat.data(), flat.size() * sizeof(DcNode), cudaMemcpyHostToDevice, st));
-    NAO_CUDA_CHECK(cudaStreamSynchronize(st));     // the host vectors above go out of scope at return
-
-    NAO_CUDA_CHECK(cudaMemsetAsync(w.b.Q, 0, (size_t)batch * n * n * 8, st));
-    dc_scale_tear_kernel<<<batch, 256, 0, st>>>(w.b, w.cuts, (int)cuts.size());
-    NAO_LAUNCHED();
-    dc_leaf_kernel<<<dim3(ceil_div(nleaves, 4), batch), 128, 0, st>>>(w.b, w.leaf_off, nleaves, d_info);
-    NAO_LAUNCHED();
-    for (size_t lv = 0; lv < p.levels.size(); ++lv) {
-        const int nn = (int)p.levels[lv].size();
-        const DcNode *nodes = w.nodes + lvl_off[lv];
-        int Nmax = 0, hmax = 0;
+    std::vector<size_t> lvl_off;
+    { size_t o = 0; for (auto &l : p.levels) { lvl_off.push_back(o); o += l.size(); } }
+    const size_t nlev = p.levels.size();
+    auto level_geometry = [&](size_t lv, int &nn, int &Nmax, int &hmax) {
+        nn = (int)p.levels[lv].size(); Nmax = 0; hmax = 0;
         for (auto &nd : p.levels[lv]) { Nmax = max(Nmax, nd.n1 + nd.n2); hmax = max(hmax, max(nd.n1, nd.n2)); }
-        dc_setup_kernel<<<dim3(nn, batch), 1024, 0, st>>>(w.b, nodes, p.maxnodes, nn);
+    };
+    if (phase & 1) {
+        // host -> device: tree description (tiny; pageable copy is staged before the call returns)
+        std::vector<int> cuts;
+        for (int i = 1; i < nleaves; ++i) cuts.push_back(p.leaf_off[i]);
+        if (!cuts.empty()) NAO_CUDA_CHECK(cudaMemcpyAsync(w.cuts, cuts.data(), cuts.size() * 4, cudaMemcpyHostToDevice, st));
+        NAO_CUDA_CHECK(cudaMemcpyAsync(w.leaf_off, p.leaf_off.data(), p.leaf_off.size() * 4, cudaMemcpyHostToDevice, st));
+        std::vector<DcNode> flat;
+        for (auto &l : p.levels) flat.insert(flat.end(), l.begin(), l.end());
+        if (!flat.empty()) NAO_CUDA_CHECK(cudaMemcpyAsync(w.nodes, flat.data(), flat.size() * sizeof(DcNode), cudaMemcpyHostToDevice, st));
+        NAO_CUDA_CHECK(cudaStreamSynchronize(st));     // the host vectors above go out of scope at return
+
+        NAO_CUDA_CHECK(cudaMemsetAsync(w.b.Q, 0, (size_t)batch * n * n * 8, st));
+        dc_scale_tear_kernel<<<batch, 256, 0, st>>>(w.b, w.cuts, (int)cuts.size());
         NAO_LAUNCHED();
-        dc_rotate_kernel<<<dim3(ceil_div(Nmax, 256), nn, batch), 256, 0, st>>>(w.b, nodes, p.maxnodes);
+        dc_leaf_kernel<<<dim3(ceil_div(nleaves, 4), batch), 128, 0, st>>>(w.b, w.leaf_off, nleaves, d_info);
         NAO_LAUNCHED();
-        const int cy = min(Nmax, 1024);
-        dc_permute_kernel<<<dim3(ceil_div(Nmax, 256), cy, nn * batch), 256, 0, st>>>(w.b, nodes, p.maxnodes, nn);
-        NAO_LAUNCHED();
-        dc_copyback_kernel<<<dim3(ceil_div(Nmax, 256), cy, nn * batch), 256, 0, st>>>(w.b, nodes, p.maxnodes, nn);
-        NAO_LAUNCHED();
-        dc_secular_kernel<<<dim3(ceil_div(Nmax, 8), nn, batch), 256, 0, st>>>(w.b, nodes, p.maxnodes, d_info);
-        NAO_LAUNCHED();
-        dc_zhat_kernel<<<dim3(ceil_div(Nmax, 32), nn, batch), 256, 0, st>>>(w.b, nodes, p.maxnodes);
-        NAO_LAUNCHED();
-        dc_vectors_kernel<<<dim3(Nmax, nn, batch), 128, 0, st>>>(w.b, nodes, p.maxnodes);
-        NAO_LAUNCHED();
-        if (int rc = gemm_launch_grouped(NAO_REAL, w.b.desc, batch * nn * 2, hmax, Nmax, 1, OP_N, OP_N, false, st)) return rc;
-        dc_finish_kernel<<<dim3(nn, batch), 256, 0, st>>>(w.b, nodes, p.maxnodes);
+        for (size_t lv = 0; lv < nlev; ++lv) {
+            int nn, Nmax, hmax; level_geometry(lv, nn, Nmax, hmax);
+            const DcNode *nodes = w.nodes + lvl_off[lv];
+            const bool top = (lv + 1 == nlev);
+            dc_setup_kernel<<<dim3(nn, batch), 1024, 0, st>>>(w.b, nodes, p.maxnodes, nn);
+            NAO_LAUNCHED();
+            dc_rotate_kernel<<<dim3(ceil_div(Nmax, 256), nn, batch), 256, 0, st>>>(w.b, nodes, p.maxnodes);
+            NAO_LAUNCHED();
+            const int cy = min(Nmax, 1024);
+            dc_permute_kernel<<<dim3(ceil_div(Nmax, 256), cy, nn * batch), 256, 0, st>>>(w.b, nodes, p.maxnodes, nn);
+            NAO_LAUNCHED();
+            dc_copyback_kernel<<<dim3(ceil_div(Nmax, 256), cy, nn * batch), 256, 0, st>>>(w.b, nodes, p.maxnodes, nn);
+            NAO_LAUNCHED();
+            dc_secular_kernel<<<dim3(ceil_div(Nmax, 8), nn, batch), 256, 0, st>>>(w.b, nodes, p.maxnodes, d_info);
+            NAO_LAUNCHED();
+            dc_zhat_kernel<<<dim3(ceil_div(Nmax, 32), nn, batch), 256, 0, st>>>(w.b, nodes, p.maxnodes);
+            NAO_LAUNCHED();
+            if (!top) {
+                dc_vectors_kernel<<<dim3(Nmax, nn, batch), 128, 0, st>>>(w.b, nodes, p.maxnodes, 0);
+                NAO_LAUNCHED();
+                if (int rc = gemm_launch_grouped(NAO_REAL, w.b.desc, batch * nn * 2, hmax, Nmax, 1, OP_N, OP_N, false, st)) return rc;
+            }
+            dc_finish_kernel<<<dim3(nn, batch), 256, 0, st>>>(w.b, nodes, p.maxnodes);      // eigenvalue order of the merged node
+            NAO_LAUNCHED();
+        }
+        dc_final_evals_kernel<<<dim3(ceil_div(n, 256), batch), 256, 0, st>>>(w.b, evals);
         NAO_LAUNCHED();
     }
-    dc_final_kernel<<<dim3(ceil_div(n, 256), min(n, 1024), batch), 256, 0, st>>>(w.b, evals, Qout, ldq, sQ);
-    NAO_LAUNCHED();
+    if (phase & 2) {
+        if (nlev > 0) {
+            int nn, Nmax, hmax; level_geometry(nlev - 1, nn, Nmax, hmax);
+            const DcNode *nodes = w.nodes + lvl_off[nlev - 1];
+            const int restricted = nvec < n ? 1 : 0;
+            if (restricted) {
+                dc_restrict_kernel<<<batch, 256, 0, st>>>(w.b, nodes, p.maxnodes, nvec);
+                NAO_LAUNCHED();
+            }
+            dc_vectors_kernel<<<dim3(Nmax, nn, batch), 128, 0, st>>>(w.b, nodes, p.maxnodes, restricted);
+            NAO_LAUNCHED();
+            if (int rc = gemm_launch_grouped(NAO_REAL, w.b.desc, batch * nn * 2, hmax, Nmax, 1, OP_N, OP_N, false, st)) return rc;
+        }
+        dc_final_kernel<<<dim3(ceil_div(n, 256), min(nvec, 1024), batch), 256, 0, st>>>(w.b, Qout, ldq, sQ, nvec);
+        NAO_LAUNCHED();
+    }
     NAO_CUDA_CHECK(cudaGetLastError());
     return NAO_OK;
 }
