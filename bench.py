@@ -347,6 +347,7 @@ def main():
         achieved = panel_bytes / (panel_ms * 1e-3) / 1e9 if panel_ms > 0 else 0.0
         fl = useful_flops(prob)
         gemm_tf = kgemm["work"] / (kgemm["ms"] * 1e-3) / 1e12 if kgemm["ms"] > 0 else 0.0
+        dmma_meas = nao.dmma_peak()          # register-resident DMMA loop, measured in this run
         # DRAM traffic of the dominant kernel: ratio (dram bytes / algorithmic bytes) of the committed ncu --set full
         # capture (profiles/r01_traffic.csv) times this run's algorithmic bytes per launch
         traffic, traffic_src = None, None
@@ -369,7 +370,7 @@ def main():
                        "step": "first SCF step: S factored inside the step",
                        "overlap": "one S shared by the items" if Sh.shape[0] == 1 and prob.batch > 1 else "one S per item"},
             "useful_tflops": fl / (ms * 1e-3) / 1e12, "useful_flops_per_step": fl,
-            "fp64_dmma_peak_tflops": FP64_DMMA_PEAK_TFLOPS,
+            "fp64_dmma_peak_tflops": FP64_DMMA_PEAK_TFLOPS, "fp64_dmma_peak_measured_tflops": dmma_meas,
             "ms_per_step_later_scf_steps": ms_later,
             "phases_ms": {k: round(v, 3) for k, v in phases.items()},
             "roofline": {"kernel": kpanel["name"], "bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s",
@@ -377,9 +378,10 @@ def main():
                          "kernel_ms_per_step": panel_ms, "launches_per_step": kpanel["launches"] // prof_steps,
                          "algorithmic_bytes_per_step": panel_bytes,
                          "algorithmic_bytes_per_launch": panel_bytes / max(1, kpanel["launches"] // prof_steps)},
-            "roofline_gemm": {"kernel": kgemm["name"], "bound": "tensor", "achieved": gemm_tf, "peak": FP64_DMMA_PEAK_TFLOPS,
-                              "unit": "TFLOP/s", "frac": gemm_tf / FP64_DMMA_PEAK_TFLOPS,
-                              "peak_source": "derived: 148 SMs x 128 flop/clk x 1.965 GHz (DESIGN.md 5); cuBLAS DGEMM measures 35.6",
+            "roofline_gemm": {"kernel": kgemm["name"], "bound": "tensor", "achieved": gemm_tf, "peak": dmma_meas,
+                              "unit": "TFLOP/s", "frac": gemm_tf / dmma_meas,
+                              "peak_source": "measured in this run: register-resident DMMA.8x8x4 loop (nao_dmma_peak); derived "
+                                             "148 SMs x 128 flop/clk x 1.965 GHz = 37.2; cuBLAS DGEMM reaches 35.6",
                               "kernel_ms_per_step": kgemm["ms"] / prof_steps, "launches_timed": kgemm["launches"],
                               "executed_flops_timed": kgemm["work"]},
             "partial_spectrum": partial,

@@ -178,6 +178,10 @@ long nao_launch_count(void);
  * boundaries (potrf_trtri, reduce, tridiagonalise, stedc, back_transform, C = W^H Z).  nao_profile_read waits for the
  * events of the LAST nao_geneig call and writes the phase durations in milliseconds; returns the number written.
  */
+/* Measured FP64 tensor-pipe peak of the device: a register-resident DMMA.8x8x4 loop on every SM (no memory traffic), in
+ * TFLOP/s.  The roofline denominator of the GEMM-class kernels is checked against it. */
+int nao_dmma_peak(double *h_tflops, void *cuda_stream);
+
 int nao_profile_enable(int on);
 int nao_profile_read(double *h_ms, int max_phases);
 const char *nao_profile_phase_name(int i);

@@ -40,6 +40,7 @@ _SIGNATURES = {
     "nao_status_string": ([_i], ctypes.c_char_p),
     "nao_version": ([], ctypes.c_char_p),
     "nao_launch_count": ([], _l),
+    "nao_dmma_peak": ([_dp, _vp], _i),
     "nao_profile_enable": ([_i], _i),
     "nao_profile_read": ([_dp, _i], _i),
     "nao_profile_phase_name": ([_i], ctypes.c_char_p),
@@ -142,6 +143,13 @@ def profile_kernel_launches(slot: int, max_launches: int = 2048) -> list:
     if k < 0:
         raise NaoError("nao_profile_kernel_launches failed: %d" % k)
     return [buf[i] for i in range(k)]
+
+
+def dmma_peak() -> float:
+    """Measured FP64 tensor-pipe peak (TFLOP/s) of the current device: register-resident DMMA loop."""
+    out = ctypes.c_double(0.0)
+    _check(lib().nao_dmma_peak(ctypes.byref(out), None), "nao_dmma_peak")
+    return out.value
 
 
 def version() -> str:

@@ -98,3 +98,51 @@ NAO_EXPORT int nao_profile_read(double *h_ms, int max_phases) {
     return np;
 }
 NAO_EXPORT const char *nao_profile_phase_name(int i) { return (i >= 0 && i < nao::NPH - 1) ? nao::kPhaseNames[i] : ""; }
+
+// ---- FP64 tensor-pipe peak: register-resident DMMA.8x8x4 loop (no memory traffic), the measured counterpart of the derived
+// ---- 148 SMs x 128 flop/clk x clock roof used in DESIGN.md 5 and bench.py
+namespace nao {
+__global__ void __launch_bounds__(256) dmma_peak_kernel(int iters, double *sink) {
+    double c[16][2];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) { c[i][0] = 0.0; c[i][1] = 0.0; }
+    const double a = 1.0 + threadIdx.x * 1e-9, b = 1.0 - threadIdx.x * 1e-9;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i)
+            asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                         : "+d"(c[i][0]), "+d"(c[i][1]) : "d"(a), "d"(b));
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) s += c[i][0] + c[i][1];
+    if (s == 123.456) sink[0] = s;
+}
+}  // namespace nao
+NAO_EXPORT int nao_dmma_peak(double *h_tflops, void *cuda_stream) {
+    using namespace nao;
+    if (!h_tflops) return -1;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, nsm = 148;
+    cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+    static double *h_sink = nullptr, *d_sink = nullptr;          // pinned host word, never written in practice
+    if (!h_sink) {
+        if (cudaHostAlloc((void **)&h_sink, 8, cudaHostAllocMapped) != cudaSuccess) return NAO_ERR_CUDA;
+        if (cudaHostGetDevicePointer((void **)&d_sink, h_sink, 0) != cudaSuccess) return NAO_ERR_CUDA;
+    }
+    cudaEvent_t e0, e1;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return NAO_ERR_CUDA;
+    const int iters = 20000, ctas = nsm * 4;
+    dmma_peak_kernel<<<ctas, 256, 0, st>>>(iters / 10, d_sink);                 // warm-up
+    cudaEventRecord(e0, st);
+    dmma_peak_kernel<<<ctas, 256, 0, st>>>(iters, d_sink);
+    cudaEventRecord(e1, st);
+    NAO_LAUNCHED(); NAO_LAUNCHED();
+    if (cudaEventSynchronize(e1) != cudaSuccess) return NAO_ERR_CUDA;
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    const double flops = (double)ctas * 8 /*warps*/ * iters * 16.0 * 512.0;      // one DMMA.8x8x4 = 8*8*4*2 flop
+    *h_tflops = flops / (ms * 1e-3) / 1e12;
+    return NAO_OK;
+}
