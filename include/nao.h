@@ -146,10 +146,11 @@ int nao_fermi_mu(int n, int batch, const double *dE, const double *h_weight,
 
 /*
  * Density matrix D_b = C_b diag(f_b) C_b^H per batch item, full Hermitian matrix written (both triangles).
- * Columns with f < 1e-17 are skipped (their contribution is < 1e-17 * |C|^2, reading C6).
+ * Columns after the last one with |f| >= 1e-17 are skipped (their contribution is < 1e-17 * |C|^2, reading C6).
  *   1 n, 2 batch, 3 dtype
  *   4 dC,ldc,strideC  in : eigenvectors (columns)
- *   7 dF              in : device, batch*n occupations (any values >= 0; e.g. f*e gives the energy-weighted DM)
+ *   7 dF              in : device, batch*n weights (occupations f in [0,1]; any real values are allowed, e.g. the f*e of
+ *                          nao_energy_weights gives the energy-weighted density matrix)
  *   8 dD,ldd,strideD  out
  *  11 dwork, work_bytes  device scratch of at least nao_density_workspace() bytes
  *  13 cuda_stream
@@ -160,6 +161,36 @@ int nao_density_matrix(int n, int batch, int dtype,
                        const double *dF,
                        void *dD, long ldd, long strideD,
                        void *dwork, size_t work_bytes, void *cuda_stream);
+
+/*
+ * The step after the hot path (the paper's un-offloaded Part 4/5).
+ *
+ * nao_energy_weights: dFE[b*n + i] = dF[b*n + i] * dE[b*n + i] (device arrays of batch*n doubles).  Passing dFE as the
+ * weights of nao_density_matrix gives the energy-weighted density matrix C diag(f e) C^H.
+ *
+ * nao_fold_density: real-space density matrix from its k-space images, the inverse of the Bloch sum of Eq. 12
+ * (sign convention DESIGN.md reading C8):
+ *     D(R_r) = sum_k h_w[k] * exp(-i k.R_r) * D(k),      r = 0 .. nR-1
+ *   1 n, 2 nk (k-points), 3 nR (lattice vectors)
+ *   4 out_dtype         NAO_COMPLEX: D(R) complex; NAO_REAL: only Re D(R) is formed and stored as doubles (D(R) is real
+ *                       when the k set is inversion symmetric, D(-k) = conj D(k))
+ *   5 dDk,ldd,strideD   in : device, nk complex n x n matrices, column-major
+ *   8 h_k               in : HOST double[3 nk], Cartesian k (1/bohr)
+ *   9 h_w               in : HOST double[nk], k-point weights
+ *  10 h_R               in : HOST double[3 nR], Cartesian lattice vectors (bohr)
+ *  11 dDR,lddr,strideDR out: device, nR matrices of out_dtype, column-major
+ *  14 dwork, work_bytes device scratch of at least nao_fold_workspace(nk, nR) bytes
+ *  16 cuda_stream
+ * The host arrays are copied on entry and may be reused when the call returns.  Errors: -i for argument i, positive
+ * codes as for the other calls.
+ */
+int nao_energy_weights(int n, int batch, const double *dE, const double *dF, double *dFE, void *cuda_stream);
+int nao_fold_workspace(int nk, int nR, size_t *bytes);
+int nao_fold_density(int n, int nk, int nR, int out_dtype,
+                     const void *dDk, long ldd, long strideD,
+                     const double *h_k, const double *h_w, const double *h_R,
+                     void *dDR, long lddr, long strideDR,
+                     void *dwork, size_t work_bytes, void *cuda_stream);
 
 /* Human-readable text for a return code (static storage). */
 const char *nao_status_string(int status);

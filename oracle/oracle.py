@@ -121,6 +121,36 @@ def density(C, f):
     return d.T.copy()
 
 
+def energy_density(C, f, e):
+    """Energy-weighted density matrix C diag(f e) C^H: the definition of `density` with the weights
+    f_i e_i (one FP64 product per state)."""
+    return density(C, np.asarray(f, dtype=np.float64) * np.asarray(e, dtype=np.float64))
+
+
+def fold_density(Dk, kpts, weights, Rvecs):
+    """Real-space density matrix D(R) = sum_k w_k exp(-i k.R) D(k): the inverse of the Bloch sum of Eq. 12 (PAPER.md:79-82,
+    M(k) = sum_R exp(+i k.R) M(R), reading C8).  Dk: (nk, n, n) mathematical matrices; returns (nR, n, n)
+    complex.  Long double throughout (phase, product and sum), written out term by term."""
+    Dk = np.asarray(Dk)
+    nk, n, _ = Dk.shape
+    kp = np.asarray(kpts, dtype=np.longdouble).reshape(nk, 3)
+    w = np.asarray(weights, dtype=np.longdouble).reshape(nk)
+    Rv = np.asarray(Rvecs, dtype=np.longdouble).reshape(-1, 3)
+    dre = Dk.real.astype(np.longdouble)
+    dim = Dk.imag.astype(np.longdouble)
+    out = np.empty((Rv.shape[0], n, n), dtype=np.complex128)
+    for r in range(Rv.shape[0]):
+        are = np.zeros((n, n), dtype=np.longdouble)
+        aim = np.zeros((n, n), dtype=np.longdouble)
+        for k in range(nk):
+            phi = -(kp[k, 0] * Rv[r, 0] + kp[k, 1] * Rv[r, 1] + kp[k, 2] * Rv[r, 2])
+            c, sn = w[k] * np.cos(phi), w[k] * np.sin(phi)
+            are += c * dre[k] - sn * dim[k]
+            aim += c * dim[k] + sn * dre[k]
+        out[r] = are.astype(np.float64) + 1j * aim.astype(np.float64)
+    return out
+
+
 def solve_problem(prob, want_D: bool = True):
     """Whole hot path on a synth.Problem: eigenpairs per item, shared Fermi level, D per item."""
     es, Cs = [], []

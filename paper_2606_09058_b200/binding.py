@@ -37,6 +37,9 @@ _SIGNATURES = {
     "nao_fermi_mu": ([_i, _i, _vp, _dp, _d, _d, _dp, _vp, _vp, _vp], _i),
     "nao_density_workspace": ([_i, _i, _i, _szp], _i),
     "nao_density_matrix": ([_i, _i, _i, _vp, _l, _l, _vp, _vp, _l, _l, _vp, _sz, _vp], _i),
+    "nao_energy_weights": ([_i, _i, _vp, _vp, _vp, _vp], _i),
+    "nao_fold_workspace": ([_i, _i, _szp], _i),
+    "nao_fold_density": ([_i, _i, _i, _i, _vp, _l, _l, _dp, _dp, _dp, _vp, _l, _l, _vp, _sz, _vp], _i),
     "nao_status_string": ([_i], ctypes.c_char_p),
     "nao_version": ([], ctypes.c_char_p),
     "nao_launch_count": ([], _l),
@@ -257,6 +260,34 @@ def density_matrix(C: torch.Tensor, F: torch.Tensor, out: torch.Tensor | None = 
                                   _dev(work, "work"), work.numel(), _stream(C))
     _check(rc, "nao_density_matrix")
     return D
+
+
+def energy_weights(E: torch.Tensor, F: torch.Tensor):
+    """nao_energy_weights: f*e per state; density_matrix(C, energy_weights(E, F)) is the energy-weighted DM."""
+    batch, n = E.shape
+    FE = torch.empty_like(F)
+    _check(lib().nao_energy_weights(n, batch, _dev(E, "E"), _dev(F, "F"), _dev(FE, "FE"), _stream(E)), "nao_energy_weights")
+    return FE
+
+
+def fold_density(Dk: torch.Tensor, kpts, weights, Rvecs, real_out: bool = True):
+    """nao_fold_density: D(R) = sum_k w_k exp(-i k.R) D(k).  Dk: (nk, n, n) complex column-major items; kpts (nk, 3),
+    weights (nk,), Rvecs (nR, 3) host sequences.  Returns (nR, n, n) float64 (real_out) or complex128."""
+    nk, n, _ = Dk.shape
+    if Dk.dtype != torch.complex128:
+        raise TypeError("D(k) must be complex128")
+    hk = (ctypes.c_double * (3 * nk))(*[float(x) for row in kpts for x in row])
+    hw = (ctypes.c_double * nk)(*[float(x) for x in weights])
+    nR = len(Rvecs)
+    hR = (ctypes.c_double * (3 * nR))(*[float(x) for row in Rvecs for x in row])
+    DR = torch.empty((nR, n, n), dtype=torch.float64 if real_out else torch.complex128, device=Dk.device)
+    need = ctypes.c_size_t(0)
+    _check(lib().nao_fold_workspace(nk, nR, ctypes.byref(need)), "nao_fold_workspace")
+    work = _workspace(need.value, Dk.device)
+    rc = lib().nao_fold_density(n, nk, nR, NAO_REAL if real_out else NAO_COMPLEX, _dev(Dk, "Dk"), n, n * n, hk, hw, hR,
+                                _dev(DR, "DR"), n, n * n, _dev(work, "work"), work.numel(), _stream(Dk))
+    _check(rc, "nao_fold_density")
+    return DR
 
 
 # ------------------------------------------------------------------------------------------ building blocks

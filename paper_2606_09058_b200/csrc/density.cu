@@ -1,7 +1,7 @@
 // density.cu -- D = C diag(f) C^H (Eq. 8, Eq. 23; north_star form).
 //
 // HERK-shaped: only the tiles touching the lower triangle are computed on the DMMA GEMM core, with the Fermi
-// weights f[k] fused into the A-fragment load (scaleK) and the k-range cut at the last column with f >= 1e-17
+// weights f[k] fused into the A-fragment load (scaleK) and the k-range cut at the last column with |f| >= 1e-17
 // (decided on the device: the GEMM descriptor lives in device memory and a one-warp kernel writes its k).  The upper
 // triangle is then filled by a coalesced Hermitian mirror.
 #include "nao_internal.cuh"
@@ -14,7 +14,7 @@ __global__ void dm_setup_kernel(int n, int dtype, const void *C, long ldc, long 
     const double *f = F + (long)b * n;
     int last = -1;
     for (int k = threadIdx.x; k < n; k += 32)
-        if (f[k] >= 1e-17) last = k;
+        if (fabs(f[k]) >= 1e-17) last = k;
     for (int o = 16; o > 0; o >>= 1) last = max(last, __shfl_xor_sync(0xffffffffu, last, o));
     if (threadIdx.x == 0) {
         size_t es = dtype == NAO_COMPLEX ? 16 : 8;

@@ -3,6 +3,7 @@
     python -m paper_2606_09058_b200.microbench gemm [--m M --n N --k K] [--complex] [--opa 0|1|2] [--opb 0|1|2]
                                                     [--beta B] [--lower] [--cublas] [--reps R]
     python -m paper_2606_09058_b200.microbench heev [--n N] [--batch B] [--complex] [--two-stage|--one-stage]
+    python -m paper_2606_09058_b200.microbench fold [--n N] [--nk NK] [--nr NR] [--complex]      (config 1: 832, 8, 27)
 
 `--cublas` adds torch.matmul on the same operands as a SIDE comparison (never used by the product path).
 Prints one JSON line per measurement.
@@ -98,9 +99,31 @@ def bench_heev(args):
                       "residual_max": r, "orth_max": o, "info": info.tolist()}))
 
 
+def bench_fold(args):
+    """nao_fold_density: D(R) = sum_k w_k exp(-i k.R) D(k); HBM-bound (every D(k) element read once, every D(R) element
+    written once).  --complex writes complex D(R), default is the real part only."""
+    dev = torch.device("cuda:0")
+    g = torch.Generator(device=dev)
+    g.manual_seed(0)
+    n, nk, nR = args.n, args.nk, args.nr
+    Dk = torch.complex(torch.randn(nk, n, n, dtype=torch.float64, device=dev, generator=g),
+                       torch.randn(nk, n, n, dtype=torch.float64, device=dev, generator=g))
+    L = 10.8
+    kp = [[6.283185307179586 * 0.25 * (1 if (q >> d) & 1 else -1) / L * (1 + q // 8) for d in range(3)] for q in range(nk)]
+    w = [1.0 / nk] * nk
+    Rv = [[L * ((r // 9) % 3 - 1), L * ((r // 3) % 3 - 1), L * (r % 3 - 1 + 3 * (r // 27))] for r in range(nR)]
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    ms = _time(lambda: B.fold_density(Dk, kp, w, Rv, real_out=not args.complex), args.reps, flush)
+    by = n * n * (16.0 * nk + (16.0 if args.complex else 8.0) * nR)
+    print(json.dumps({"kernel": "fold_density", "n": n, "nk": nk, "nR": nR, "complex_out": bool(args.complex), "ms": ms,
+                      "algorithmic_bytes": by, "GBps": by / ms / 1e6}))
+
+
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("what", choices=["gemm", "heev"])
+    ap.add_argument("what", choices=["gemm", "heev", "fold"])
+    ap.add_argument("--nk", type=int, default=8)
+    ap.add_argument("--nr", type=int, default=27)
     ap.add_argument("--m", type=int, default=6656)
     ap.add_argument("--n", type=int, default=6656)
     ap.add_argument("--k", type=int, default=6656)
@@ -118,7 +141,7 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("microbench needs a CUDA device: the product has no CPU path")
     B.lib()
-    (bench_gemm if args.what == "gemm" else bench_heev)(args)
+    {"gemm": bench_gemm, "heev": bench_heev, "fold": bench_fold}[args.what](args)
 
 
 if __name__ == "__main__":

@@ -78,6 +78,19 @@ def test_host_side_argument_validation(libpath):
     cnt = i(0)
     assert lib.nao_occupied_count(0, 1, 1, 1e-17, ctypes.byref(cnt), None) == -1
     assert lib.nao_occupied_count(4, 1, None, 1e-17, ctypes.byref(cnt), None) == -3
+    # the step after the path: energy weights and the k-fold
+    dp = ctypes.POINTER(ctypes.c_double)
+    lib.nao_energy_weights.argtypes = [i, i, vp, vp, vp, vp]
+    assert lib.nao_energy_weights(0, 1, 1, 1, 1, None) == -1
+    assert lib.nao_energy_weights(4, 1, 1, None, 1, None) == -4
+    assert lib.nao_fold_workspace(8, 27, ctypes.byref(sz)) == 0 and sz.value >= 27 * 16 * 16
+    assert lib.nao_fold_workspace(0, 27, ctypes.byref(sz)) == -1
+    lib.nao_fold_density.argtypes = [i, i, i, i, vp, l, l, dp, dp, dp, vp, l, l, vp, ctypes.c_size_t, vp]
+    k3 = (ctypes.c_double * 3)(0, 0, 0)
+    assert lib.nao_fold_density(4, 1, 1, 5, 1, 4, 16, k3, k3, k3, 1, 4, 16, 1, 1 << 20, None) == -4      # out_dtype
+    assert lib.nao_fold_density(4, 1, 1, 0, 1, 3, 16, k3, k3, k3, 1, 4, 16, 1, 1 << 20, None) == -6      # ldd < n
+    assert lib.nao_fold_density(4, 1, 1, 0, 1, 4, 16, k3, None, k3, 1, 4, 16, 1, 1 << 20, None) == -9    # h_w
+    assert lib.nao_fold_density(4, 1, 1, 0, 1, 4, 16, k3, k3, k3, 1, 4, 16, 1, 8, None) == 1             # workspace
 
 
 def test_no_product_import_of_oracle():

@@ -481,3 +481,67 @@ def test_dmma_peak_measurement_matches_the_derived_roof(nao):
     derived = 148 * 128 * 1.965e9 / 1e12
     t = nao.dmma_peak()
     assert 0.8 * derived <= t <= 1.02 * derived, t
+
+
+# ---------------------------------------------------------------- the step after the path
+def test_energy_weighted_density_matrix_against_oracle(nao):
+    """W = C diag(f e) C^H through nao_energy_weights + nao_density_matrix (negative weights: occupied levels lie below
+    zero) against the oracle's W from its own eigenpairs; Tr(W S) = sum f e."""
+    for idx, nat in [(0, None), (1, 6), (3, 4)]:
+        prob = make_config(idx, nat=nat)
+        ref = oracle.solve_problem(prob, want_D=False)
+        H = torch.from_numpy(prob.H).to(DEV)
+        S = torch.from_numpy(prob.S.copy()).to(DEV)
+        E, C, info = nao.geneig(H, S, flags=nao.NAO_NC_BLOCK_S if prob.nc_block_s else 0)
+        mu, F = nao.fermi_mu(E, prob.weights, prob.n_electrons, prob.kT)
+        FE = nao.energy_weights(E, F)
+        assert np.array_equal(FE.cpu().numpy(), F.cpu().numpy() * E.cpu().numpy())
+        W = to_np(nao.density_matrix(C, FE))
+        for b in range(prob.batch):
+            Wref = oracle.energy_density(ref["C"][b], ref["f"][b], ref["e"][b])
+            assert np.abs(W[b] - Wref).max() <= TOL_D
+            assert abs(np.trace(W[b] @ prob.S_full(b)).real - float((ref["f"][b] * ref["e"][b]).sum())) <= 1e-8
+
+
+def _c1_mesh(prob):
+    L = prob.meta["L"]
+    ks = [(sx * 0.25, sy * 0.25, sz * 0.25) for sx in (-1, 1) for sy in (-1, 1) for sz in (-1, 1)]
+    Rv = [(L * a, L * b, L * c) for a in (-1, 0, 1) for b in (-1, 0, 1) for c in (-1, 0, 1)]
+    return 2 * np.pi * np.array(ks) / L, np.full(8, 0.125), np.array(Rv)
+
+
+@pytest.mark.parametrize("nat", [6, 16])
+def test_fold_density_config1_recipe_against_oracle(nao, nat):
+    """D(R) on the 27 images of the config-1 recipe (8 Monkhorst-Pack points, first spin channel) from the GPU's D(k),
+    real and complex output, against the oracle's fold of the oracle's own D(k)."""
+    prob = make_config(1, nat=nat)
+    ref = oracle.solve_problem(prob)
+    got = run_path(nao, prob)
+    kp, w, Rv = _c1_mesh(prob)
+    Dk = to_dev(np.stack(got["D"][:8]))
+    ref_DR = oracle.fold_density(np.stack(ref["D"][:8]), kp, w, Rv)
+    DRc = to_np(nao.fold_density(Dk, kp, w, Rv, real_out=False))
+    DRr = to_np(nao.fold_density(Dk, kp, w, Rv, real_out=True))
+    assert np.abs(DRc - ref_DR).max() <= TOL_D
+    assert np.abs(DRr - ref_DR.real).max() <= TOL_D
+    assert np.abs(ref_DR.imag).max() <= 1e-12          # time reversal: D(-k) = conj D(k) on this mesh
+    # the fold itself, on identical inputs: the oracle's fold of the GPU's D(k), to rounding
+    same = oracle.fold_density(np.stack(got["D"][:8]), kp, w, Rv)
+    assert np.abs(DRc - same).max() <= 1e-13
+
+
+def test_fold_density_ragged_sizes_and_many_k_points(nao):
+    """Sizes that are not multiples of the 128 x 8 tile, more k-points than one register pass holds (16), more lattice
+    vectors than one shared-memory pass holds (128)."""
+    rng = np.random.default_rng(3)
+    for (n, nk, nR) in [(1, 1, 1), (131, 19, 5), (37, 33, 140), (200, 8, 27)]:
+        Dk = rng.standard_normal((nk, n, n)) + 1j * rng.standard_normal((nk, n, n))
+        kp = rng.uniform(-0.6, 0.6, (nk, 3))
+        w = rng.uniform(0.1, 1.0, nk)
+        Rv = rng.uniform(-25, 25, (nR, 3))
+        ref = oracle.fold_density(Dk, kp, w, Rv)
+        scale = np.abs(ref).max()
+        gc = to_np(nao.fold_density(to_dev(Dk), kp, w, Rv, real_out=False))
+        gr = to_np(nao.fold_density(to_dev(Dk), kp, w, Rv, real_out=True))
+        assert np.abs(gc - ref).max() <= 1e-13 * max(1.0, scale) * nk
+        assert np.abs(gr - ref.real).max() <= 1e-13 * max(1.0, scale) * nk

@@ -303,3 +303,63 @@ def test_generator_matrices_are_hermitian_and_spd():
             assert np.abs(H - H.conj().T).max() < 1e-14
             assert np.abs(S - S.conj().T).max() < 1e-14
             assert np.linalg.eigvalsh(S).min() > 0.05
+
+
+# ---------------------------------------------------------------- the step after the path
+def test_energy_weighted_density_matrix_identities():
+    """W = C diag(f e) C^H.  With every f = 1: S W S = H exactly (H C = S C e, C^{-1} = C^H S), whatever the solver;
+    for Fermi occupations Tr(W S) = sum f_i e_i, the band energy (Eq. 7 PAPER.md:59 without the factor 2)."""
+    rng = np.random.default_rng(11)
+    for cplx in (False, True):
+        n = 23
+        H, S = rand_herm(rng, n, cplx), rand_spd(rng, n, cplx)
+        e, C, _ = oracle.geneig(H, S)
+        W1 = oracle.energy_density(C, np.ones(n), e)
+        assert np.abs(S @ W1 @ S - H).max() < 1e-12
+        mu, f = oracle.fermi(e[None], [2.0], 14.0, 0.05)
+        W = oracle.energy_density(C, f[0], e)
+        assert abs(np.trace(W @ S).real - float((f[0] * e).sum())) < 1e-12
+        assert np.abs(W - W.conj().T).max() < 1e-15
+
+
+def _mp_mesh(L):
+    ks = [(sx * 0.25, sy * 0.25, sz * 0.25) for sx in (-1, 1) for sy in (-1, 1) for sz in (-1, 1)]
+    return 2 * np.pi * np.array(ks) / L, np.full(8, 0.125)
+
+
+def test_fold_density_inverts_the_bloch_sum_on_the_2x2x2_mesh():
+    """Eq. 12: M(k) = sum_R exp(+i k.R) M(R).  On the 8 Monkhorst-Pack points k = (2 pi/L)(+-1/4)^3
+    sum_k w_k exp(-i k.(R - R')) = prod_d cos(pi (R - R')_d / 2L), which is delta(R, R') for R, R' in {0, L}^3: the fold of
+    the Bloch sum returns the real-space matrices.  Unsymmetric random M(R) catch a transposed operand, the R = (L,L,L)
+    term catches a phase of the wrong sign."""
+    rng = np.random.default_rng(5)
+    L, n = 10.8, 7
+    kp, w = _mp_mesh(L)
+    Rv = L * np.array([(a, b, c) for a in (0, 1) for b in (0, 1) for c in (0, 1)], dtype=float)
+    M = rng.standard_normal((8, n, n))
+    Dk = np.array([sum(np.exp(1j * (k @ R)) * M[r] for r, R in enumerate(Rv)) for k in kp])
+    DR = oracle.fold_density(Dk, kp, w, Rv)
+    assert np.abs(DR - M).max() < 1e-14
+    # the weighted average at R = 0, antiperiodicity under R -> R + 2L e_x and periodicity 4L of this mesh
+    R0 = np.array([[0.0, 0.0, 0.0], [2 * L, 0.0, 0.0], [4 * L, 0.0, 0.0], [L, L, L], [3 * L, L, L]])
+    D0 = oracle.fold_density(Dk, kp, w, R0)
+    assert np.abs(D0[0] - np.tensordot(w, Dk, axes=1)).max() < 1e-15
+    assert np.abs(D0[1] + D0[0]).max() < 1e-14 and np.abs(D0[2] - D0[0]).max() < 1e-14
+    assert np.abs(D0[4] + D0[3]).max() < 1e-14
+
+
+def test_fold_density_single_k_closed_form_and_reality():
+    rng = np.random.default_rng(6)
+    n = 5
+    D = rng.standard_normal((1, n, n)) + 1j * rng.standard_normal((1, n, n))
+    k = np.array([[0.31, -0.27, 0.11]])
+    Rv = np.array([[3.0, 1.0, -2.0], [0.0, 0.0, 0.0], [-7.5, 2.25, 4.0]])
+    DR = oracle.fold_density(D, k, [0.7], Rv)
+    for r in range(3):
+        ph = 0.7 * complex(np.cos(k[0] @ Rv[r]), -np.sin(k[0] @ Rv[r]))
+        assert np.abs(DR[r] - ph * D[0]).max() < 1e-15
+    # inversion-symmetric set with D(-k) = conj D(k): D(R) is real
+    D2 = np.concatenate([D, D.conj()])
+    DR2 = oracle.fold_density(D2, np.concatenate([k, -k]), [0.5, 0.5], Rv)
+    assert np.abs(DR2.imag).max() < 1e-16
+    assert np.abs(DR2[1].real - D[0].real).max() < 1e-16
