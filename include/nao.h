@@ -43,6 +43,15 @@ extern "C" {
                                   (Eq. 25-27); dS is the N x N REAL overlap (S_NC = diag(S,S)) */
 #define NAO_TRD_ONE_STAGE 4u   /* force the one-stage (HEMV-based, HBM-bound) Householder tridiagonalisation */
 #define NAO_TRD_TWO_STAGE 8u   /* force the two-stage (dense->band->tridiagonal) reduction */
+#define NAO_LOWDIN 16u         /* orthogonalise by the paper's own route: S = U s U^H with this
+                                  library's eigensolver, V = U s^{-1/2}, H' = V^H H V, C = V C'.  Same e, mu, D as the
+                                  default Cholesky route.  dS is overwritten by the DENSE matrix V^H = s^{-1/2} U^H (all of
+                                  it, not just a triangle); NAO_S_FACTORED | NAO_LOWDIN reuses it.  Directions with
+                                  s_i <= rel * s_max (rel set by nao_set_lowdin_threshold, default 0 = none) are pruned:
+                                  their levels come out as NAO_PRUNED_LEVEL at the top of the spectrum with zero vectors,
+                                  so that mu and D are those of the pruned basis.  With rel = 0 a non-positive eigenvalue
+                                  of S sets d_info = (order of S) + 2. */
+#define NAO_PRUNED_LEVEL 1.0e4 /* Hartree; eigenvalue reported for a pruned direction */
 
 /* return codes */
 #define NAO_OK 0
@@ -50,6 +59,9 @@ extern "C" {
 #define NAO_ERR_CUDA 2         /* a CUDA runtime call or kernel launch failed */
 #define NAO_ERR_ELECTRONS 3    /* nao_fermi_mu: n_electrons outside (0, sum of weights * n) or kT <= 0 */
 #define NAO_ERR_UNSUPPORTED 4  /* combination of arguments not implemented */
+
+/* Relative pruning threshold of the NAO_LOWDIN route, 0 <= rel < 1 (process-wide, read when S is decomposed). */
+int nao_set_lowdin_threshold(double rel);
 
 /* Bytes of device workspace nao_geneig needs for (n, batch, dtype, flags).  Host-only, no launch. */
 int nao_geneig_workspace(int n, int batch, int dtype, unsigned flags, size_t *bytes);

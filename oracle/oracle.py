@@ -69,6 +69,23 @@ def geneig_lowdin(H, S):
     return geneig(H, S, lowdin=True)
 
 
+def geneig_lowdin_pruned(H, S, rel: float):
+    """Loewdin route with pruning of near-dependent directions (PAPER.md:147, 159-163 for the route):
+    S = U s U^H by Jacobi; keep the directions with s_i > rel * s_max; V = U_keep s_keep^{-1/2}; H' = V^H H V (long double
+    products); H' C' = C' e by Jacobi; C = V C'.  Returns (e ascending, m values; C of shape (n, m), C^H S C = I_m)."""
+    H = np.asarray(H)
+    S = np.asarray(S)
+    s, U = heev(S)
+    keep = (s > 0) & (s > rel * s.max())
+    ld = np.clongdouble if _is_complex(H, S) else np.longdouble
+    V = U[:, keep].astype(ld) / np.sqrt(s[keep].astype(np.longdouble))
+    Hp = V.conj().T @ (H.astype(ld) @ V)
+    Hp = (Hp + Hp.conj().T) / 2
+    e, Cp = heev(Hp.astype(np.complex128 if _is_complex(H, S) else np.float64))
+    C = V @ Cp.astype(ld)
+    return e, C.astype(np.complex128 if _is_complex(H, S) else np.float64)
+
+
 def cholesky(S):
     """Lower Cholesky factor L of S (S = L L^H)."""
     n = S.shape[0]

@@ -18,7 +18,8 @@ import torch
 from . import build as _build
 
 NAO_REAL, NAO_COMPLEX = 0, 1
-NAO_S_FACTORED, NAO_NC_BLOCK_S, NAO_TRD_ONE_STAGE, NAO_TRD_TWO_STAGE = 1, 2, 4, 8
+NAO_S_FACTORED, NAO_NC_BLOCK_S, NAO_TRD_ONE_STAGE, NAO_TRD_TWO_STAGE, NAO_LOWDIN = 1, 2, 4, 8, 16
+NAO_PRUNED_LEVEL = 1.0e4
 
 _LIB = None
 _vp, _i, _l, _d, _sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_long, ctypes.c_double, ctypes.c_size_t
@@ -40,6 +41,7 @@ _SIGNATURES = {
     "nao_energy_weights": ([_i, _i, _vp, _vp, _vp, _vp], _i),
     "nao_fold_workspace": ([_i, _i, _szp], _i),
     "nao_fold_density": ([_i, _i, _i, _i, _vp, _l, _l, _dp, _dp, _dp, _vp, _l, _l, _vp, _sz, _vp], _i),
+    "nao_set_lowdin_threshold": ([_d], _i),
     "nao_status_string": ([_i], ctypes.c_char_p),
     "nao_version": ([], ctypes.c_char_p),
     "nao_launch_count": ([], _l),
@@ -260,6 +262,11 @@ def density_matrix(C: torch.Tensor, F: torch.Tensor, out: torch.Tensor | None = 
                                   _dev(work, "work"), work.numel(), _stream(C))
     _check(rc, "nao_density_matrix")
     return D
+
+
+def set_lowdin_threshold(rel: float):
+    """nao_set_lowdin_threshold: relative pruning threshold of the NAO_LOWDIN route (0 = no pruning)."""
+    _check(lib().nao_set_lowdin_threshold(float(rel)), "nao_set_lowdin_threshold")
 
 
 def energy_weights(E: torch.Tensor, F: torch.Tensor):

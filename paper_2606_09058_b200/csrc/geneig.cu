@@ -97,6 +97,8 @@ static int heev(int dtype, int n, int batch, unsigned flags, void *A, long lda, 
 }
 
 // ----------------------------------------------------------------------------------------------------- geneig
+static double g_lowdin_rel = 0.0;      // nao_set_lowdin_threshold
+
 struct GePlan { size_t W, Wc, A, X, heev, bytes; int nS, sdtype, nitemsS; };
 static GePlan ge_plan(int n, int batch, int dtype, unsigned flags, bool shared_S) {
     GePlan p; size_t off = 0;
@@ -107,7 +109,9 @@ static GePlan ge_plan(int n, int batch, int dtype, unsigned flags, bool shared_S
     p.Wc = take(nc ? (size_t)p.nitemsS * p.nS * p.nS * 16 : 0);
     p.A = take((size_t)batch * n * n * esize(dtype));
     p.X = take((size_t)batch * n * n * esize(dtype));
-    p.heev = take(heev_plan(dtype, n, batch, flags).bytes);
+    size_t hb = heev_plan(dtype, n, batch, flags).bytes;
+    if (flags & NAO_LOWDIN) hb = std::max(hb, heev_plan(p.sdtype, p.nS, p.nitemsS, flags).bytes);
+    p.heev = take(hb);
     p.bytes = off;
     return p;
 }
@@ -190,12 +194,24 @@ static int geneig_impl(int n, int batch, int dtype, unsigned flags, int nvec, co
     int rc;
     const void *Wm = W;
     const long sWm = shared_S ? 0 : sW;
+    const bool lowdin = flags & NAO_LOWDIN;
+    const int wmask = lowdin ? MASK_NONE : MASK_LOWER;        // the Cholesky route's W = L^{-1} is lower triangular
     if (phase & 1) {
     NAO_CUDA_CHECK(cudaMemsetAsync(d_info, 0, sizeof(int) * batch, st));
 
     // 1. factor (or unpack) S
     prof_mark(0, st);
-    if (!(flags & NAO_S_FACTORED)) {
+    if (lowdin) {
+        // the paper's route: S = U s U^H, W = s^{-1/2} U^H (dense); dS keeps W for the later SCF steps
+        if (!(flags & NAO_S_FACTORED)) {
+            if ((rc = herm_fill(p.sdtype, nS, dS, lds, strideS, X, nS, sW, p.nitemsS, st))) return rc;
+            if ((rc = heev(p.sdtype, nS, p.nitemsS, flags, X, nS, sW, dE, A, nS, sW, w + p.heev, d_info, st))) return rc;
+            if ((rc = lowdin_w(p.sdtype, nS, p.nitemsS, A, nS, sW, dE, g_lowdin_rel, W, nS, sW, d_info, st))) return rc;
+            if ((rc = copy_matrix(p.sdtype, nS, nS, W, nS, sW, dS, lds, strideS, p.nitemsS, 0, st))) return rc;
+        } else {
+            if ((rc = copy_matrix(p.sdtype, nS, nS, dS, lds, strideS, W, nS, sW, p.nitemsS, 0, st))) return rc;
+        }
+    } else if (!(flags & NAO_S_FACTORED)) {
         // with a shared S the (single) status goes to d_info[0]
         if ((rc = potrf_trtri(p.sdtype, nS, p.nitemsS, dS, lds, strideS, W, nS, sW, X, nS, sW, d_info, st))) return rc;
         if ((rc = pack_linv(p.sdtype, nS, dS, lds, strideS, W, nS, sW, p.nitemsS, st))) return rc;
@@ -210,14 +226,15 @@ static int geneig_impl(int n, int batch, int dtype, unsigned flags, int nvec, co
         if ((rc = herm_fill(dtype, n, dH, ldh, strideH, A, n, sAX, batch, st))) return rc;
         {
             GemmDesc g = gemm_desc(OP_N, OP_N, n, n, n, 1.0, Wm, n, A, n, 0.0, X, n);
-            g.sA = sWm; g.sB = sAX; g.sC = sAX; g.maskA = MASK_LOWER;
+            g.sA = sWm; g.sB = sAX; g.sC = sAX; g.maskA = wmask;
             if ((rc = gemm_launch(dtype, g, batch, st))) return rc;
         }
         {
             GemmDesc g = gemm_desc(OP_N, OP_C, n, n, n, 1.0, X, n, Wm, n, 0.0, A, n);
-            g.sA = sAX; g.sB = sWm; g.sC = sAX; g.maskB = MASK_LOWER; g.cmode = 1;
+            g.sA = sAX; g.sB = sWm; g.sC = sAX; g.maskB = wmask; g.cmode = 1;
             if ((rc = gemm_launch(dtype, g, batch, st))) return rc;
         }
+        if (lowdin && (rc = lowdin_shift(dtype, n, nS, batch, A, n, sAX, Wm, p.sdtype, nS, sWm, NAO_PRUNED_LEVEL, st))) return rc;
         // 3. standard problem; eigenvectors into X
         if ((rc = heev(dtype, n, batch, flags, A, n, sAX, dE, X, n, sAX, w + p.heev, d_info, st, nvec, (phase & 2) ? 3 : 1))) return rc;
         }
@@ -226,7 +243,7 @@ static int geneig_impl(int n, int batch, int dtype, unsigned flags, int nvec, co
             if ((rc = heev(dtype, n, batch, flags, A, n, sAX, dE, X, n, sAX, w + p.heev, d_info, st, nvec, 2))) return rc;
         // 4. C = W^H Z
         GemmDesc g = gemm_desc(OP_C, OP_N, n, nvec, n, 1.0, Wm, n, X, n, 0.0, dC, ldc);
-        g.sA = sWm; g.sB = sAX; g.sC = strideC; g.maskA = MASK_LOWER;
+        g.sA = sWm; g.sB = sAX; g.sC = strideC; g.maskA = wmask;
         if ((rc = gemm_launch(dtype, g, batch, st))) return rc;
     } else {
         // Noncollinear: W_NC = diag(W, W) with W REAL (Eq. 25-27).  A complex matrix multiplied from the RIGHT by a real one is
@@ -241,7 +258,7 @@ static int geneig_impl(int n, int batch, int dtype, unsigned flags, int nvec, co
         for (int bj = 0; bj < 2; ++bj) {           // Y(:, block bj) = H(:, block bj) W^T
             const long off = 2 * (long)bj * nS * n;
             GemmDesc g = gemm_desc(OP_N, OP_T, 2 * n, nS, nS, 1.0, Ar + off, 2L * n, Wr, nS, 0.0, Xr + off, 2L * n);
-            g.sA = 2 * sAX; g.sB = sWm; g.sC = 2 * sAX; g.maskB = MASK_LOWER;
+            g.sA = 2 * sAX; g.sB = sWm; g.sC = 2 * sAX; g.maskB = wmask;
             if ((rc = gemm_launch(NAO_REAL, g, batch, st))) return rc;
         }
         if ((rc = conj_transpose(n, n, (const cplx *)X, n, sAX, (cplx *)A, n, sAX, batch, st))) return rc;       // A <- Y^H
@@ -249,10 +266,11 @@ static int geneig_impl(int n, int batch, int dtype, unsigned flags, int nvec, co
             for (int bj = 0; bj <= bi; ++bj) {     // block (bi, bj) of (Y^H) W_NC^T, lower block triangle, into X
                 const long off = 2 * ((long)bi * nS + (long)bj * nS * n);
                 GemmDesc g = gemm_desc(OP_N, OP_T, 2 * nS, nS, nS, 1.0, Ar + off, 2L * n, Wr, nS, 0.0, Xr + off, 2L * n);
-                g.sA = 2 * sAX; g.sB = sWm; g.sC = 2 * sAX; g.maskB = MASK_LOWER; g.cmode = (bi == bj) ? 2 : 0;
+                g.sA = 2 * sAX; g.sB = sWm; g.sC = 2 * sAX; g.maskB = wmask; g.cmode = (bi == bj) ? 2 : 0;
                 if ((rc = gemm_launch(NAO_REAL, g, batch, st))) return rc;
             }
         if ((rc = copy_matrix(dtype, n, n, X, n, sAX, A, n, sAX, batch, 1, st))) return rc;                      // lower triangle
+        if (lowdin && (rc = lowdin_shift(dtype, n, nS, batch, A, n, sAX, Wm, p.sdtype, nS, sWm, NAO_PRUNED_LEVEL, st))) return rc;
         // 3. standard problem; eigenvectors into X
         if ((rc = heev(dtype, n, batch, flags, A, n, sAX, dE, X, n, sAX, w + p.heev, d_info, st, nvec, (phase & 2) ? 3 : 1))) return rc;
         }
@@ -264,7 +282,7 @@ static int geneig_impl(int n, int batch, int dtype, unsigned flags, int nvec, co
         for (int bj = 0; bj < 2; ++bj) {
             const long off = 2 * (long)bj * nS * nvec;
             GemmDesc g = gemm_desc(OP_N, OP_N, 2 * nvec, nS, nS, 1.0, Ar + off, 2L * nvec, Wr, nS, 0.0, Xr + off, 2L * nvec);
-            g.sA = 2 * sAX; g.sB = sWm; g.sC = 2 * sAX; g.maskB = MASK_LOWER;
+            g.sA = 2 * sAX; g.sB = sWm; g.sC = 2 * sAX; g.maskB = wmask;
             if ((rc = gemm_launch(NAO_REAL, g, batch, st))) return rc;
         }
         if ((rc = conj_transpose(nvec, n, (const cplx *)X, nvec, sAX, (cplx *)dC, ldc, strideC, batch, st))) return rc;
@@ -350,4 +368,10 @@ NAO_EXPORT int nao_scf_step(int n, int batch, int dtype, unsigned flags, const v
     rc = geneig_impl(n, batch, dtype, flags, nvec, dH, ldh, strideH, dS, lds, strideS, dE, dC, ldc, strideC, wg, g, d_info, cuda_stream, 2);
     if (rc) return rc;
     return nao_density_matrix(n, batch, dtype, dC, ldc, strideC, dF, dD, ldd, strideD, wd, d, cuda_stream);
+}
+
+NAO_EXPORT int nao_set_lowdin_threshold(double rel) {
+    if (!(rel >= 0.0 && rel < 1.0)) return -1;
+    nao::g_lowdin_rel = rel;
+    return NAO_OK;
 }

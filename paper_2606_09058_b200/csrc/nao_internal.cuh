@@ -98,6 +98,11 @@ int real_to_complex(int m, int n, const double *Q, long ldq, long sQ, cplx *Z, l
                     cudaStream_t st);
 // B (n x m) <- A^H, complex
 int conj_transpose(int m, int n, const cplx *A, long lda, long sA, cplx *B, long ldb, long sB, int batch, cudaStream_t st);
+// lowdin.cu: W = s^{-1/2} U^H with pruning of s_i <= rel * s_max; diagonal shift of the pruned directions of the reduced matrix
+int lowdin_w(int dtype, int n, int batch, const void *U, long ldu, long sU, const double *s, double rel, void *W, long ldw,
+             long sW, int *d_info, cudaStream_t st);
+int lowdin_shift(int dtype, int n, int nS, int batch, void *A, long lda, long sA, const void *W, int wdtype, long ldw, long sW,
+                 double big, cudaStream_t st);
 // Linv (n x n lower, explicit zeros above, diagonal = 1/L_ii) from the packed factor in S (see nao.h)
 int unpack_linv(int dtype, int n, const void *S, long lds, long sS, void *W, long ldw, long sW, int batch,
                 cudaStream_t st);

@@ -91,6 +91,10 @@ def test_host_side_argument_validation(libpath):
     assert lib.nao_fold_density(4, 1, 1, 0, 1, 3, 16, k3, k3, k3, 1, 4, 16, 1, 1 << 20, None) == -6      # ldd < n
     assert lib.nao_fold_density(4, 1, 1, 0, 1, 4, 16, k3, None, k3, 1, 4, 16, 1, 1 << 20, None) == -9    # h_w
     assert lib.nao_fold_density(4, 1, 1, 0, 1, 4, 16, k3, k3, k3, 1, 4, 16, 1, 8, None) == 1             # workspace
+    lib.nao_set_lowdin_threshold.argtypes = [ctypes.c_double]
+    assert lib.nao_set_lowdin_threshold(-1e-3) == -1 and lib.nao_set_lowdin_threshold(1.0) == -1
+    assert lib.nao_set_lowdin_threshold(1e-8) == 0 and lib.nao_set_lowdin_threshold(0.0) == 0
+    assert lib.nao_geneig_workspace(104, 1, 0, 16, ctypes.byref(sz)) == 0 and sz.value > 104 * 104 * 8 * 2      # NAO_LOWDIN
 
 
 def test_no_product_import_of_oracle():

@@ -545,3 +545,64 @@ def test_fold_density_ragged_sizes_and_many_k_points(nao):
         gr = to_np(nao.fold_density(to_dev(Dk), kp, w, Rv, real_out=True))
         assert np.abs(gc - ref).max() <= 1e-13 * max(1.0, scale) * nk
         assert np.abs(gr - ref.real).max() <= 1e-13 * max(1.0, scale) * nk
+
+
+# ---------------------------------------------------------------- the paper's own orthogonalisation
+@pytest.mark.parametrize("idx,nat", [(0, None), (1, 6), (2, 8), (3, 4)])
+def test_lowdin_route_against_oracle(nao, idx, nat):
+    """NAO_LOWDIN (S = U s U^H, V = U s^{-1/2}) gives the same e, mu, D as the oracle; the dense
+    V^H left in dS serves the later SCF steps (NAO_S_FACTORED | NAO_LOWDIN)."""
+    prob = make_config(idx, nat=nat)
+    ref = oracle.solve_problem(prob)
+    got = run_path(nao, prob, flags=nao.NAO_LOWDIN)
+    check_against_oracle(prob, got, ref)
+    H = torch.from_numpy(prob.H).to(DEV)
+    fl = nao.NAO_LOWDIN | nao.NAO_S_FACTORED | (nao.NAO_NC_BLOCK_S if prob.nc_block_s else 0)
+    E2, C2, info2 = nao.geneig(H, got["S_factor"], flags=fl)
+    assert int(info2.abs().max()) == 0
+    assert np.abs(E2.cpu().numpy() - ref["e"]).max() <= TOL_E
+    mu2, F2 = nao.fermi_mu(E2, prob.weights, prob.n_electrons, prob.kT)
+    D2 = to_np(nao.density_matrix(C2, F2))
+    for b in range(prob.batch):
+        assert np.abs(D2[b] - ref["D"][b]).max() <= TOL_D
+
+
+@pytest.mark.parametrize("kind", ["real", "complex", "nc"])
+def test_lowdin_pruning_of_duplicated_orbitals(nao, kind):
+    """A basis in which two orbitals appear twice (S' = P^T S P singular, two exact null directions): with a pruning threshold
+    the GPU path returns the levels of the pruned basis, NAO_PRUNED_LEVEL for the two pruned directions with zero vectors,
+    and the oracle's D of the pruned problem."""
+    prob = make_config({"real": 0, "complex": 1, "nc": 3}[kind], nat={"real": None, "complex": 6, "nc": 4}[kind])
+    nS = prob.S.shape[-1]
+    dup = [3, nS - 2]
+    P = np.hstack([np.eye(nS), np.eye(nS)[:, dup]])
+    S0 = np.swapaxes(prob.S[0], -1, -2)
+    Sd = P.T @ S0 @ P
+    H0 = prob.H_full(0)
+    if kind == "nc":
+        P2 = np.kron(np.eye(2), P)
+        Hd, Sfull = P2.T @ H0 @ P2, np.kron(np.eye(2), Sd)
+    else:
+        Hd, Sfull = P.T @ H0 @ P, Sd
+    m, n = H0.shape[0], Hd.shape[0]
+    e_ref, C_ref = oracle.geneig_lowdin_pruned(Hd, Sfull, 1e-9)
+    assert e_ref.shape == (m,)
+    nel = 0.3 * m
+    mu_ref, f_ref = oracle.fermi(e_ref[None], [1.0], nel, prob.kT)
+    D_ref = oracle.density(np.hstack([C_ref, np.zeros((n, n - m))]), np.append(f_ref[0], np.zeros(n - m)))
+    nao.set_lowdin_threshold(1e-9)
+    try:
+        flags = nao.NAO_LOWDIN | (nao.NAO_NC_BLOCK_S if kind == "nc" else 0)
+        E, C, info = nao.geneig(to_dev(Hd[None]), to_dev(Sd[None]), flags=flags)
+    finally:
+        nao.set_lowdin_threshold(0.0)
+    assert int(info.abs().max()) == 0
+    e = E.cpu().numpy()[0]
+    assert np.abs(e[:m] - e_ref).max() <= TOL_E
+    assert np.abs(e[m:] - nao.NAO_PRUNED_LEVEL).max() <= 1e-6
+    assert np.abs(to_np(C)[0][:, m:]).max() <= 1e-10
+    mu, F = nao.fermi_mu(E, [1.0], nel, prob.kT)
+    assert abs(mu - mu_ref) <= TOL_MU
+    D = to_np(nao.density_matrix(C, F))[0]
+    assert np.abs(D - D_ref).max() <= TOL_D
+    assert abs(np.trace(D @ Sfull).real - nel) <= 1e-8

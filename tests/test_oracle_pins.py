@@ -363,3 +363,33 @@ def test_fold_density_single_k_closed_form_and_reality():
     DR2 = oracle.fold_density(D2, np.concatenate([k, -k]), [0.5, 0.5], Rv)
     assert np.abs(DR2.imag).max() < 1e-16
     assert np.abs(DR2[1].real - D[0].real).max() < 1e-16
+
+
+# ---------------------------------------------------------------- Loewdin route with pruning
+def test_pruned_lowdin_recovers_the_closed_form_spectrum_of_a_basis_with_a_duplicated_orbital():
+    """Chain with overlap (closed form e_k = (eps0 + t tau_k)/(1 + s tau_k)) written in a basis in which orbital q appears
+    twice: H' = P^T H P, S' = P^T S P with P = [I | e_q] is singular; pruning the null direction must give back exactly the
+    n closed-form levels, and the density matrix maps back as P D' P^T = D.  With rel = 0 on a regular pencil the pruned
+    route is the plain one."""
+    n, eps0, t, sov, q = 12, -0.3, -1.0, 0.2, 4
+    T = chain(n)
+    H, S = eps0 * np.eye(n) + t * T, np.eye(n) + sov * T
+    tau = 2 * np.cos(np.arange(1, n + 1) * np.pi / (n + 1))
+    closed = np.sort((eps0 + t * tau) / (1 + sov * tau))
+    P = np.hstack([np.eye(n), np.eye(n)[:, [q]]])
+    Hd, Sd = P.T @ H @ P, P.T @ S @ P
+    assert abs(oracle.heev(Sd)[0][0]) < 1e-14       # singular overlap: one exact null direction
+    e, C = oracle.geneig_lowdin_pruned(Hd, Sd, 1e-10)
+    assert e.shape == (n,) and C.shape == (n + 1, n)
+    assert np.abs(e - closed).max() < 1e-13
+    assert np.abs(C.T @ Sd @ C - np.eye(n)).max() < 1e-13
+    mu, f = oracle.fermi(e[None], [2.0], 10.0, 0.01)
+    e0, C0, _ = oracle.geneig(H, S)
+    D0 = oracle.density(C0, oracle.fermi(e0[None], [2.0], 10.0, 0.01)[1][0])
+    assert np.abs(P @ oracle.density(np.hstack([C, np.zeros((n + 1, 1))]), np.append(f[0], 0.0)) @ P.T - D0).max() < 1e-13
+    rng = np.random.default_rng(2)
+    Hr, Sr = rand_herm(rng, 9, True), rand_spd(rng, 9, True)
+    e1, C1 = oracle.geneig_lowdin_pruned(Hr, Sr, 0.0)
+    e2, C2, _ = oracle.geneig(Hr, Sr)
+    assert np.abs(e1 - e2).max() < 1e-13
+    assert np.abs(oracle.density(C1, np.arange(9) / 9.0) - oracle.density(C2, np.arange(9) / 9.0)).max() < 1e-13
