@@ -18,84 +18,86 @@ static const int CHOL_LEAF = 64;
 
 // One CTA per batch item.  nb <= 64.  S block (lower referenced) -> L in place; W block <- L^{-1} (lower; the
 // strict upper part of the W block is zeroed).  info: first failing pivot (1-based, global index).
+// Right-looking factorisation with ONE barrier per column: the scaled column j of L goes to a second array while the
+// trailing update reads the unscaled column (a(i,k) -= a(i,j) conj(a(k,j)) / a(j,j)); thread <-> (row i, every 4th column).
+// The inverse is a forward substitution per column, 4 adjacent lanes per column, so it needs warp-level barriers only.
 template <class T>
 __global__ void __launch_bounds__(256) chol_leaf_kernel(int nb, int off, T *S, long lds, long sS, T *W, long ldw,
                                                         long sW, int *info) {
+    typedef Ops<T> O;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    T *sL = (T *)smem_raw;                 // [nb][nb+1]  sL[i*(nb+1) + j] = L(i,j)
-    T *sX = sL + nb * (nb + 1);            // inverse, same layout
-    const int ld = nb + 1;
+    constexpr int ld = CHOL_LEAF + 1;
+    T *sA = (T *)smem_raw;                 // [64][65] working copy a(i,j) at sA[i*ld + j]; later the inverse X
+    T *sF = sA + CHOL_LEAF * ld;           // [64][65] the factor L
     const int b = blockIdx.x;
     S += (long)b * sS + off + (long)off * lds;
     W += (long)b * sW + off + (long)off * ldw;
-    const int tid = threadIdx.x, nt = blockDim.x;
-    for (int e = tid; e < nb * nb; e += nt) {
-        int i = e % nb, j = e / nb;
-        sL[i * ld + j] = (i >= j) ? S[i + (long)j * lds] : Ops<T>::zero();
+    const int tid = threadIdx.x;
+    for (int e = tid; e < CHOL_LEAF * CHOL_LEAF; e += 256) {
+        const int i = e & (CHOL_LEAF - 1), j = e >> 6;
+        sA[i * ld + j] = (i < nb && j < nb && i >= j) ? S[i + (long)j * lds] : O::zero();
+        sF[i * ld + j] = O::zero();
     }
     __syncthreads();
-    __shared__ double s_piv;
+    const int ti = tid & (CHOL_LEAF - 1), tq = tid >> 6;
     for (int j = 0; j < nb; ++j) {
-        if (tid == 0) {
-            double ajj = Ops<T>::real(sL[j * ld + j]);
-            if (!(ajj > 0.0)) {
-                if (info[b] == 0) info[b] = off + j + 1;
-                ajj = 1.0;
-            }
-            s_piv = sqrt(ajj);
-            sL[j * ld + j] = Ops<T>::from_real(s_piv);
+        double ajj = O::real(sA[j * ld + j]);
+        if (!(ajj > 0.0)) {
+            if (tid == 0 && info[b] == 0) info[b] = off + j + 1;
+            ajj = 1.0;
         }
-        __syncthreads();
-        const double rinv = 1.0 / s_piv;
-        for (int i = j + 1 + tid; i < nb; i += nt) sL[i * ld + j] = Ops<T>::scale(sL[i * ld + j], rinv);
-        __syncthreads();
-        // trailing update of the lower triangle: (i,k) with j < k <= i
-        const int r = nb - 1 - j;
-        for (int e = tid; e < r * r; e += nt) {
-            int i = j + 1 + e % r, k = j + 1 + e / r;
-            if (i >= k) sL[i * ld + k] = Ops<T>::sub(sL[i * ld + k], Ops<T>::mul_conj(sL[i * ld + j], sL[k * ld + j]));
+        const double piv = sqrt(ajj), rinv = 1.0 / piv, ainv = 1.0 / ajj;
+        if (ti >= j && ti < nb) {
+            const T aij = sA[ti * ld + j];
+            if (tq == 0) sF[ti * ld + j] = ti == j ? O::from_real(piv) : O::scale(aij, rinv);
+            if (ti > j) {
+                const T l = O::scale(aij, ainv);
+                for (int k = j + 1 + tq; k <= ti; k += 4)
+                    sA[ti * ld + k] = O::sub(sA[ti * ld + k], O::mul_conj(l, sA[k * ld + j]));
+            }
         }
         __syncthreads();
     }
-    // inverse by forward substitution, one column per thread group: X(i,c) = (delta_ic - sum_{k=c}^{i-1} L(i,k) X(k,c)) / L(i,i)
-    // 4 threads cooperate on a column (split the k-sum), 64 columns -> 256 threads.
+    // inverse by forward substitution, X(i,c) = (delta_ic - sum_{k=c}^{i-1} L(i,k) X(k,c)) / L(i,i): 4 adjacent lanes
+    // split the k-sum of one column, nobody else touches that column of X
     {
+        T *sX = sA;
         const int c = tid >> 2, part = tid & 3;
         for (int i = 0; i < nb; ++i) {
-            T acc = Ops<T>::zero();
+            T acc = O::zero();
             if (c < nb && i > c)
-                for (int k = c + part; k < i; k += 4) acc = Ops<T>::sub(acc, Ops<T>::mul(sL[i * ld + k], sX[k * ld + c]));
-            // reduce over the 4 cooperating lanes (they are adjacent lanes of one warp)
-            if (sizeof(T) == 8) {
-                double *a = (double *)&acc;
-                a[0] += __shfl_xor_sync(0xffffffffu, a[0], 1); a[0] += __shfl_xor_sync(0xffffffffu, a[0], 2);
-            } else {
-                double *a = (double *)&acc;
-                a[0] += __shfl_xor_sync(0xffffffffu, a[0], 1); a[0] += __shfl_xor_sync(0xffffffffu, a[0], 2);
-                a[1] += __shfl_xor_sync(0xffffffffu, a[1], 1); a[1] += __shfl_xor_sync(0xffffffffu, a[1], 2);
+                for (int k = c + part; k < i; k += 4) acc = O::sub(acc, O::mul(sF[i * ld + k], sX[k * ld + c]));
+            double *a = (double *)&acc;
+#pragma unroll
+            for (int w = 0; w < (int)(sizeof(T) / 8); ++w) {
+                a[w] += __shfl_xor_sync(0xffffffffu, a[w], 1);
+                a[w] += __shfl_xor_sync(0xffffffffu, a[w], 2);
             }
             if (c < nb && part == 0) {
-                double dinv = 1.0 / Ops<T>::real(sL[i * ld + i]);
+                const double dinv = 1.0 / O::real(sF[i * ld + i]);
                 T v;
-                if (i < c) v = Ops<T>::zero();
-                else if (i == c) v = Ops<T>::from_real(dinv);
-                else v = Ops<T>::scale(acc, dinv);
+                if (i < c) v = O::zero();
+                else if (i == c) v = O::from_real(dinv);
+                else v = O::scale(acc, dinv);
                 sX[i * ld + c] = v;
             }
-            __syncthreads();
+            __syncwarp();
         }
     }
-    for (int e = tid; e < nb * nb; e += nt) {
-        int i = e % nb, j = e / nb;
-        if (i >= j) S[i + (long)j * lds] = sL[i * ld + j];
-        W[i + (long)j * ldw] = sX[i * ld + j];
+    __syncthreads();
+    for (int e = tid; e < CHOL_LEAF * CHOL_LEAF; e += 256) {
+        const int i = e & (CHOL_LEAF - 1), j = e >> 6;
+        if (i < nb && j < nb) {
+            if (i >= j) S[i + (long)j * lds] = sF[i * ld + j];
+            W[i + (long)j * ldw] = sA[i * ld + j];
+        }
     }
 }
 
 template <class T>
 static int leaf(int nb, int off, int batch, void *S, long lds, long sS, void *W, long ldw, long sW, int *info,
                 cudaStream_t st) {
-    size_t smem = 2 * (size_t)nb * (nb + 1) * sizeof(T);
+    size_t smem = 2 * (size_t)CHOL_LEAF * (CHOL_LEAF + 1) * sizeof(T);
     static bool attr = false;
     if (!attr) {
         NAO_CUDA_CHECK(cudaFuncSetAttribute(chol_leaf_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
