@@ -40,7 +40,11 @@ __global__ void __launch_bounds__(256) larft_kernel(int kb, const T *G, long ldg
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T *sT_ = (T *)smem_raw;             // packed upper, kb(kb+1)/2
     __shared__ T s_g[ORM_KB];
-    G += (long)blockIdx.x * sG; tau += (long)blockIdx.x * sTau; Tm += (long)blockIdx.x * sT;
+    // blockIdx.y: diagonal block of ORM_KB reflectors of a longer sequence (kb = total length); the blocks are independent
+    const int boff = blockIdx.y * ORM_KB;
+    G += (long)blockIdx.x * sG + boff + (long)boff * ldg; tau += (long)blockIdx.x * sTau + boff;
+    Tm += (long)blockIdx.x * sT + boff + (long)boff * ldt;
+    kb = min(ORM_KB, kb - boff);
     const int tid = threadIdx.x;
     // column i+1 of G and tau_{i+1} are fetched while step i computes (the recurrence is latency bound)
     T gnext = Ops<T>::zero(), tnext = tau[0];
@@ -49,11 +53,24 @@ __global__ void __launch_bounds__(256) larft_kernel(int kb, const T *G, long ldg
         if (tid < i) s_g[tid] = gnext;
         if (i + 1 < kb) { tnext = tau[i + 1]; if (tid < i + 1) gnext = G[tid + (long)(i + 1) * ldg]; }
         __syncthreads();
-        if (tid < i) {
-            // row tid of T(0:i,0:i) times g  (T upper: columns c >= tid)
-            T acc = Ops<T>::zero();
-            for (int c = tid; c < i; ++c) acc = Ops<T>::fma(sT_[c * (c + 1) / 2 + tid], s_g[c], acc);
-            sT_[i * (i + 1) / 2 + tid] = Ops<T>::sub(Ops<T>::zero(), Ops<T>::mul(ti, acc));
+        {
+            // row `row` of T(0:i,0:i) times g (T upper: columns c >= row): two adjacent lanes split the columns, two
+            // accumulators each (the recurrence is bound by the latency of this dependent chain)
+            const int row = tid >> 1, half = tid & 1;
+            T acc0 = Ops<T>::zero(), acc1 = Ops<T>::zero();
+            if (row < i) {
+                int c = row + half;
+                for (; c + 2 < i; c += 4) {
+                    acc0 = Ops<T>::fma(sT_[c * (c + 1) / 2 + row], s_g[c], acc0);
+                    acc1 = Ops<T>::fma(sT_[(c + 2) * (c + 3) / 2 + row], s_g[c + 2], acc1);
+                }
+                for (; c < i; c += 2) acc0 = Ops<T>::fma(sT_[c * (c + 1) / 2 + row], s_g[c], acc0);
+            }
+            T acc = Ops<T>::add(acc0, acc1);
+            double *a = (double *)&acc;
+#pragma unroll
+            for (int w = 0; w < (int)(sizeof(T) / 8); ++w) a[w] += __shfl_xor_sync(0xffffffffu, a[w], 1);
+            if (row < i && half == 0) sT_[i * (i + 1) / 2 + row] = Ops<T>::sub(Ops<T>::zero(), Ops<T>::mul(ti, acc));
         }
         if (tid == 0) sT_[i * (i + 1) / 2 + i] = ti;
         __syncthreads();
@@ -150,11 +167,8 @@ static int ormtr_impl(int dtype, int n, int ncols, int batch, int shift, const T
         g.sA = sV; g.sB = sV; g.sC = sGT;
         if (int rc = gemm_splitk(dtype, g, batch, std::min(w.ksG, ceil_div(m, 256)), w.P, st)) return rc;
         // T: recurrence on the diagonal 128-blocks, then off-diagonal blocks by doubling (two small GEMMs each)
-        for (int off = 0; off < kb; off += ORM_KB) {
-            const int kd = std::min(ORM_KB, kb - off);
-            larft_kernel<T><<<batch, 256, larft_smem, st>>>(kd, Gm + off + (long)off * kb, kb, sGT, tau + jb + off, n, Tm + off + (long)off * kb, kb, sGT);
-            NAO_LAUNCHED();
-        }
+        larft_kernel<T><<<dim3(batch, ceil_div(kb, ORM_KB)), 256, larft_smem, st>>>(kb, Gm, kb, sGT, tau + jb, n, Tm, kb, sGT);
+        NAO_LAUNCHED();
         for (int sz = ORM_KB; sz < kb; sz *= 2)
             for (int off = 0; off + sz < kb; off += 2 * sz) {
                 const int k1 = sz, k2 = std::min(sz, kb - off - sz), o2 = off + sz;
