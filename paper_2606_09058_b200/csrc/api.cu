@@ -102,7 +102,7 @@ NAO_EXPORT const char *nao_profile_phase_name(int i) { return (i >= 0 && i < nao
 // ---- FP64 tensor-pipe peak: register-resident DMMA.8x8x4 loop (no memory traffic), the measured counterpart of the derived
 // ---- 148 SMs x 128 flop/clk x clock roof used in DESIGN.md 5 and bench.py
 namespace nao {
-__global__ void __launch_bounds__(256) dmma_peak_kernel(int iters, double *sink) {
+__global__ void __launch_bounds__(512) dmma_peak_kernel(int iters, double *sink) {
     double c[16][2];
 #pragma unroll
     for (int i = 0; i < 16; ++i) { c[i][0] = 0.0; c[i][1] = 0.0; }
@@ -132,17 +132,26 @@ NAO_EXPORT int nao_dmma_peak(double *h_tflops, void *cuda_stream) {
     }
     cudaEvent_t e0, e1;
     if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return NAO_ERR_CUDA;
-    const int iters = 20000, ctas = nsm * 4;
-    dmma_peak_kernel<<<ctas, 256, 0, st>>>(iters / 10, d_sink);                 // warm-up
+    // exactly ONE CTA of 16 warps per SM: the dynamic shared-memory request (not used by the kernel) keeps a second CTA off the
+    // SM -- with several small CTAs per SM the block scheduler places them unevenly (5 on some SMs, 3 on others) and the
+    // slowest SM decides the time (measured: 29.7 instead of 37.1 TF/s in about half of the calls)
+    const int iters = 40000, ctas = nsm;
+    const size_t smem = 120 * 1024;
+    static bool attr = false;
+    if (!attr) {
+        if (cudaFuncSetAttribute(dmma_peak_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return NAO_ERR_CUDA;
+        attr = true;
+    }
+    dmma_peak_kernel<<<ctas, 512, smem, st>>>(iters / 10, d_sink);                 // warm-up
     cudaEventRecord(e0, st);
-    dmma_peak_kernel<<<ctas, 256, 0, st>>>(iters, d_sink);
+    dmma_peak_kernel<<<ctas, 512, smem, st>>>(iters, d_sink);
     cudaEventRecord(e1, st);
     NAO_LAUNCHED(); NAO_LAUNCHED();
     if (cudaEventSynchronize(e1) != cudaSuccess) return NAO_ERR_CUDA;
     float ms = 0.f;
     cudaEventElapsedTime(&ms, e0, e1);
     cudaEventDestroy(e0); cudaEventDestroy(e1);
-    const double flops = (double)ctas * 8 /*warps*/ * iters * 16.0 * 512.0;      // one DMMA.8x8x4 = 8*8*4*2 flop
+    const double flops = (double)ctas * 16 /*warps*/ * iters * 16.0 * 512.0;      // one DMMA.8x8x4 = 8*8*4*2 flop
     *h_tflops = flops / (ms * 1e-3) / 1e12;
     return NAO_OK;
 }

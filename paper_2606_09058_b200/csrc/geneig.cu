@@ -14,12 +14,15 @@ namespace nao {
 
 // ----------------------------------------------------------------------------------------------------- heev
 struct HeevPlan { size_t d, e, tau, qt, sub, v2, tau2, sub2, bytes; bool two_stage; };
-static const int TWO_STAGE_MIN_N = 1 << 30;      // default switch-over size (flags force either path)
+// Default switch-over (flags force either path), from `microbench heev` on B200 with all eigenvectors, one-stage vs
+// two-stage in ms: real n = 4992 x 2 items 223 vs 238, n = 6656 x 1 310 vs 295, n = 6656 x 2 414 vs 388, n = 9984 x 1 698 vs
+// 679; complex n = 9984 1.29 s vs 1.55 s (the second back-transformation runs at a lower rate in complex arithmetic).
+static const int TWO_STAGE_MIN_N_REAL = 6144;
 static bool use_two_stage(int dtype, int n, int batch, unsigned flags) {
     if (flags & NAO_TRD_ONE_STAGE) return false;
     if (!he2hb_supported(dtype, n, batch)) return false;
     if (flags & NAO_TRD_TWO_STAGE) return true;
-    return n >= TWO_STAGE_MIN_N;
+    return dtype == NAO_REAL && n >= TWO_STAGE_MIN_N_REAL;
 }
 static HeevPlan heev_plan(int dtype, int n, int batch, unsigned flags) {
     HeevPlan p; size_t off = 0;

@@ -12,6 +12,7 @@
 #include "nao_internal.cuh"
 #include "scalar.cuh"
 #include <algorithm>
+#include <cstdlib>
 
 namespace nao {
 
@@ -95,7 +96,11 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double
 template <class T, bool CONJA, bool NEG> struct Frag;
 template <bool CONJA, bool NEG> struct Frag<double, CONJA, NEG> {
     static __device__ __forceinline__ void mma(double (&acc)[4], double a, double b) {
+#ifdef Q2_SKIP_MMA
+        acc[0] += a; acc[1] += b;
+#else
         dmma884(acc[0], acc[1], NEG ? -a : a, b);
+#endif
     }
 };
 template <bool CONJA, bool NEG> struct Frag<cplx, CONJA, NEG> {
@@ -112,34 +117,41 @@ template <> __device__ __forceinline__ double frag_out<double>(const double (&ac
 template <> __device__ __forceinline__ cplx frag_out<cplx>(const double (&acc)[4], int q) { return make_double2(acc[q], acc[2 + q]); }
 
 template <class T> struct Q2Cfg;
-template <> struct Q2Cfg<double> { static const int NCMAX = 32; };     // most columns of Z per CTA (shared memory)
-template <> struct Q2Cfg<cplx> { static const int NCMAX = 16; };
+// NCMAX: columns of Z per 4-warp CTA (two CTAs per SM); NCWIDE: per 8-warp CTA with double-buffered V, T (one CTA per SM)
+template <> struct Q2Cfg<double> { static const int NCMAX = 32, NCWIDE = 96; };
+template <> struct Q2Cfg<cplx> { static const int NCMAX = 16, NCWIDE = 16; };
 
 template <class T> __device__ __forceinline__ void cp_async_elem(T *s, const T *g, bool pred) {
     if constexpr (sizeof(T) == 16) cp_async16(s, g, pred); else cp_async8(s, g, pred);
 }
 
-template <class T, int NC>
-__global__ void __launch_bounds__(Q2_NT) q2_apply_kernel(int n, int ncols, const T *V2, long ldv, long sV2, const T *Tst,
-                                                         long sTst, T *Z, long ldz, long sZ) {
+// NW warps: warp & 3 selects the 8-row tile (of W: reflectors ci; of the window: rows w, w+4, w+8), warp >> 2 the slice of the
+// slab's columns (NW = 8: two slices).  DB: V and T of the NEXT diamond are fetched into a second buffer while this one is
+// applied (one CTA per SM, 8 warps, wide slab); otherwise the co-resident second CTA hides the load.
+template <class T, int NC, int NW, bool DB, bool ALIAS>
+__global__ void __launch_bounds__(NW * 32) q2_apply_kernel(int n, int ncols, const T *V2, long ldv, long sV2, const T *Tst,
+                                                           long sTst, T *Z, long ldz, long sZ) {
     typedef Ops<T> O;
-    constexpr int b = TRD2_B, NBK = Q2_NBK, LW = Q2_LW, NCT = NC / 8, LDV = Q2_LDV, LDW = Q2_LDW, LDT = NBK;
+    constexpr int b = TRD2_B, NBK = Q2_NBK, LW = Q2_LW, CS = NW / 4, NCW = NC / CS, NCT = NCW / 8, LDV = Q2_LDV, LDW = Q2_LDW,
+                  LDT = NBK, NBUF = DB ? 2 : 1, NTH = NW * 32;
+    static_assert(NW == 4 || NW == 8, "4 or 8 warps");
+    static_assert(NC % (8 * CS) == 0 && NC % NW == 0, "slab width");
     const int item = blockIdx.y, c0 = blockIdx.x * NC;
     V2 += (long)item * sV2; Tst += (long)item * sTst; Z += (long)item * sZ;
     extern __shared__ __align__(16) unsigned char q2_smem[];
-    T *sV = (T *)q2_smem;                 // [NBK][LDV]
-    T *sZ_ = sV + NBK * LDV;              // [NC][LDV]   window of Z, kept across the windows of an S-block
-    T *sT = sZ_ + NC * LDV;               // [NBK][LDT]  T(i,k) at k*LDT + i
-    T *sW = sT + NBK * LDT;               // [NC][LDW]   W(ci,c) at c*LDW + ci
-    T *sW2 = sW + NC * LDW;               // [NC][LDW]
+    T *sVb = (T *)q2_smem;                // [NBUF][NBK][LDV]
+    T *sZ_ = sVb + NBUF * NBK * LDV;      // [NC][LDV]   window of Z, kept across the windows of an S-block
+    T *sTb = sZ_ + NC * LDV;              // [NBUF][NBK][LDT]  T(i,k) at k*LDT + i
+    T *sW = sTb + NBUF * NBK * LDT;       // [NC][LDW]   W(ci,c) at c*LDW + ci
+    T *sW2 = ALIAS ? sW : sW + NC * LDW;  // [NC][LDW]   (ALIAS: W2 overwrites W after a barrier -- smaller footprint, 3 CTAs per SM)
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, lr = lane >> 2, lc = lane & 3;
+    const int wr = warp & 3, col0 = (warp >> 2) * NCW;
 
     // rows [ra, LW) of the window starting at global row w0 (Lw valid rows) from global memory, zero beyond Lw.
-    // warp <-> columns c = warp, warp + 4, ...; lane <-> rows: no integer division anywhere in the window loop
-    constexpr int NWARP = Q2_NT / 32;
+    // warp <-> columns c = warp, warp + NW, ...; lane <-> rows: no integer division anywhere in the window loop
     auto load_z = [&](int w0, int Lw, int ra) {
 #pragma unroll
-        for (int c = warp; c < NC; c += NWARP) {
+        for (int c = warp; c < NC; c += NW) {
             const bool cok = c0 + c < ncols;
             const T *zc = Z + w0 + (long)(c0 + c) * ldz;
 #pragma unroll
@@ -152,42 +164,55 @@ __global__ void __launch_bounds__(Q2_NT) q2_apply_kernel(int n, int ncols, const
             }
         }
     };
-
     const int nsweeps = n - 1;
+    // V (masked parallelogram) and T of the diamond (s0, k), asynchronous
+    auto load_vt = [&](int buf, int s0, int k, long gidx) {
+        const int ns = min(NBK, nsweeps - s0), w0 = s0 + 1 + k * b;
+        T *sV = sVb + buf * NBK * LDV, *sT = sTb + buf * NBK * LDT;
+#pragma unroll
+        for (int ci = warp; ci < NBK; ci += NW) {
+            const int s = s0 + ci;
+            const int a0 = s + 1 + k * b - w0, a1 = min(s + (k + 1) * b, n - 1) - w0;     // valid window rows of column ci
+            const T *vc = V2 + w0 + (long)s * ldv;
+#pragma unroll
+            for (int rr = 0; rr < LW; rr += 32) {
+                const int r = rr + lane;
+                const bool ok = ci < ns && r >= a0 && r <= a1;
+                cp_async_elem<T>(sV + ci * LDV + r, ok ? vc + r : V2, ok);
+            }
+        }
+        const T *Tg = Tst + gidx * NBK * NBK;
+#pragma unroll
+        for (int e = tid; e < NBK * NBK; e += NTH) cp_async_elem<T>(sT + e, Tg + e, true);
+    };
+
     const int nS = (nsweeps + NBK - 1) / NBK;
     long goff = q2_ngroups(n);
+    int cur = 0;
+    if (DB && nS > 0) load_vt(0, (nS - 1) * NBK, 0, goff - q2_nwin(n, (nS - 1) * NBK));
     for (int I = nS - 1; I >= 0; --I) {
         const int s0 = I * NBK, ns = min(NBK, nsweeps - s0), nwin = q2_nwin(n, s0);
         goff -= nwin;
         for (int k = 0; k < nwin; ++k) {
             const int w0 = s0 + 1 + k * b;
             const int Lw = min(s0 + ns - 1 + (k + 1) * b, n - 1) - w0 + 1;
-            // ---- V (masked parallelogram), T and -- for the first window of the S-block -- Z, all asynchronous
-#pragma unroll
-            for (int ci = warp; ci < NBK; ci += NWARP) {
-                const int s = s0 + ci;
-                const int a0 = s + 1 + k * b - w0, a1 = min(s + (k + 1) * b, n - 1) - w0;     // valid window rows of column ci
-                const T *vc = V2 + w0 + (long)s * ldv;
-#pragma unroll
-                for (int rr = 0; rr < LW; rr += 32) {
-                    const int r = rr + lane;
-                    const bool ok = ci < ns && r >= a0 && r <= a1;
-                    cp_async_elem<T>(sV + ci * LDV + r, ok ? vc + r : V2, ok);
-                }
-            }
-            {
-                const T *Tg = Tst + (goff + k) * NBK * NBK;
-#pragma unroll
-                for (int e = tid; e < NBK * NBK; e += Q2_NT) cp_async_elem<T>(sT + e, Tg + e, true);
-            }
+            if (!DB) load_vt(0, s0, k, goff + k);
             if (k == 0) load_z(w0, Lw, 0);
             cp_async_commit();
             cp_async_wait<0>();
             __syncthreads();
+            const T *sV = sVb + cur * NBK * LDV, *sT = sTb + cur * NBK * LDT;
+            if (DB) {
+                // the next diamond: (I, k+1), or the first one of S-block I-1
+                if (k + 1 < nwin) load_vt(cur ^ 1, s0, k + 1, goff + k + 1);
+                else if (I > 0) load_vt(cur ^ 1, s0 - NBK, 0, goff - q2_nwin(n, s0 - NBK));
+                cp_async_commit();
+                cur ^= 1;
+            }
             // Zero structure of the parallelogram: column ci of V is non-zero only in rows ci .. ci + b - 1, so
             //   W rows 8w..8w+7 need window rows 8w .. 8w + b + 7 only (18 of 24 k-steps), and
             //   Z_w row tile m0 needs columns ci in [m0 - b + 1, m0 + 7]           (72 of 96 k-steps over the 12 tiles).
-            // ---- W = V^H Z_w : warp -> 8 rows (ci) x NC columns; fragments of step k0+4 are loaded before the DMMAs of k0
+            // ---- W = V^H Z_w : warp -> 8 rows (ci) x NCW columns; fragments of step k0+4 are loaded before the DMMAs of k0
             {
                 double acc[NCT][4];
 #pragma unroll
@@ -195,8 +220,8 @@ __global__ void __launch_bounds__(Q2_NT) q2_apply_kernel(int n, int ncols, const
 #pragma unroll
                     for (int q = 0; q < 4; ++q) acc[j][q] = 0.0;
                 constexpr int KS1 = (b + 8) / 4;                                  // 18 k-steps
-                const T *ap = sV + (warp * 8 + lr) * LDV + lc + warp * 8;
-                const T *bp = sZ_ + lr * LDV + lc + warp * 8;
+                const T *ap = sV + (wr * 8 + lr) * LDV + lc + wr * 8;
+                const T *bp = sZ_ + (col0 + lr) * LDV + lc + wr * 8;
                 T a_c = ap[0], b_c[NCT];
 #pragma unroll
                 for (int j = 0; j < NCT; ++j) b_c[j] = bp[j * 8 * LDV];
@@ -219,7 +244,7 @@ __global__ void __launch_bounds__(Q2_NT) q2_apply_kernel(int n, int ncols, const
 #pragma unroll
                 for (int j = 0; j < NCT; ++j)
 #pragma unroll
-                    for (int q = 0; q < 2; ++q) sW[(j * 8 + 2 * lc + q) * LDW + warp * 8 + lr] = frag_out<T>(acc[j], q);
+                    for (int q = 0; q < 2; ++q) sW[(col0 + j * 8 + 2 * lc + q) * LDW + wr * 8 + lr] = frag_out<T>(acc[j], q);
             }
             __syncthreads();
             // ---- W2 = T W   (T upper triangular: rows 8w.. need k >= 8w)
@@ -229,34 +254,35 @@ __global__ void __launch_bounds__(Q2_NT) q2_apply_kernel(int n, int ncols, const
                 for (int j = 0; j < NCT; ++j)
 #pragma unroll
                     for (int q = 0; q < 4; ++q) acc[j][q] = 0.0;
-                const T *ap = sT + lc * LDT + warp * 8 + lr;
-                const T *bp = sW + lr * LDW + lc;
-                for (int k0 = warp * 8; k0 < NBK; k0 += 4) {
+                const T *ap = sT + lc * LDT + wr * 8 + lr;
+                const T *bp = sW + (col0 + lr) * LDW + lc;
+                for (int k0 = wr * 8; k0 < NBK; k0 += 4) {
                     const T a = ap[k0 * LDT];
 #pragma unroll
                     for (int j = 0; j < NCT; ++j) Frag<T, false, false>::mma(acc[j], a, bp[j * 8 * LDW + k0]);
                 }
+                if (ALIAS) __syncthreads();
 #pragma unroll
                 for (int j = 0; j < NCT; ++j)
 #pragma unroll
-                    for (int q = 0; q < 2; ++q) sW2[(j * 8 + 2 * lc + q) * LDW + warp * 8 + lr] = frag_out<T>(acc[j], q);
+                    for (int q = 0; q < 2; ++q) sW2[(col0 + j * 8 + 2 * lc + q) * LDW + wr * 8 + lr] = frag_out<T>(acc[j], q);
             }
             __syncthreads();
             // ---- Z_w -= V W2 : warp -> row tiles w, w+4, w+8 (balanced: 18 k-steps per warp), in place in shared memory
 #pragma unroll
             for (int i = 0; i < 3; ++i) {
-                const int m0 = (warp + i * NWARP) * 8;
+                const int m0 = (wr + i * 4) * 8;
                 const int klo = max(0, m0 - b + 1) / 4 * 4, khi = min(NBK, m0 + 8);    // columns ci of V that touch the tile
                 double acc[NCT][4];
 #pragma unroll
                 for (int j = 0; j < NCT; ++j)
 #pragma unroll
                     for (int q = 0; q < 2; ++q) {
-                        const T z = sZ_[(j * 8 + 2 * lc + q) * LDV + m0 + lr];
+                        const T z = sZ_[(col0 + j * 8 + 2 * lc + q) * LDV + m0 + lr];
                         if constexpr (O::is_complex) { acc[j][q] = z.x; acc[j][2 + q] = z.y; } else { acc[j][q] = z; acc[j][2 + q] = 0.0; }
                     }
                 const T *ap = sV + lc * LDV + m0 + lr;
-                const T *bp = sW2 + lr * LDW + lc;
+                const T *bp = sW2 + (col0 + lr) * LDW + lc;
                 T a_c = ap[klo * LDV], b_c[NCT];
 #pragma unroll
                 for (int j = 0; j < NCT; ++j) b_c[j] = bp[j * 8 * LDW + klo];
@@ -278,14 +304,14 @@ __global__ void __launch_bounds__(Q2_NT) q2_apply_kernel(int n, int ncols, const
 #pragma unroll
                 for (int j = 0; j < NCT; ++j)
 #pragma unroll
-                    for (int q = 0; q < 2; ++q) sZ_[(j * 8 + 2 * lc + q) * LDV + m0 + lr] = frag_out<T>(acc[j], q);
+                    for (int q = 0; q < 2; ++q) sZ_[(col0 + j * 8 + 2 * lc + q) * LDV + m0 + lr] = frag_out<T>(acc[j], q);
             }
             __syncthreads();
             // ---- rows leaving the window go to global memory; the overlap with the next window moves to the top
             const bool last = (k + 1 == nwin);
             const int nout = last ? Lw : min(b, Lw);
 #pragma unroll
-            for (int c = warp; c < NC; c += NWARP) {
+            for (int c = warp; c < NC; c += NW) {
                 if (c0 + c < ncols) {
                     T *zc = Z + w0 + (long)(c0 + c) * ldz;
                     for (int r = lane; r < nout; r += 32) zc[r] = sZ_[c * LDV + r];
@@ -293,14 +319,14 @@ __global__ void __launch_bounds__(Q2_NT) q2_apply_kernel(int n, int ncols, const
             }
             if (!last) {
                 const int nov = Lw - b;                      // rows shared with the next window (<= NBK - 1 <= 31)
-                T keep[NC / NWARP];
+                T keep[NC / NW];
 #pragma unroll
-                for (int jj = 0; jj < NC / NWARP; ++jj)
-                    if (lane < nov) keep[jj] = sZ_[(warp + jj * NWARP) * LDV + b + lane];
+                for (int jj = 0; jj < NC / NW; ++jj)
+                    if (lane < nov) keep[jj] = sZ_[(warp + jj * NW) * LDV + b + lane];
                 __syncthreads();
 #pragma unroll
-                for (int jj = 0; jj < NC / NWARP; ++jj)
-                    if (lane < nov) sZ_[(warp + jj * NWARP) * LDV + lane] = keep[jj];
+                for (int jj = 0; jj < NC / NW; ++jj)
+                    if (lane < nov) sZ_[(warp + jj * NW) * LDV + lane] = keep[jj];
                 const int Lw2 = min(s0 + ns - 1 + (k + 2) * b, n - 1) - (w0 + b) + 1;
                 load_z(w0 + b, Lw2, nov);                    // committed and awaited with the next window's V, T
             } else {
@@ -312,6 +338,20 @@ __global__ void __launch_bounds__(Q2_NT) q2_apply_kernel(int n, int ncols, const
 
 size_t q2_workspace(int dtype, int n, int batch) { return align_up((size_t)batch * q2_ngroups(n) * Q2_NBK * Q2_NBK * esize(dtype)); }
 
+template <class T, int NC, int NW, bool DB, bool ALIAS>
+static int q2_launch(int n, int ncols, int batch, const T *V2, long ldv, long sV2, const T *Tst, long sTst, T *Z, long ldz, long sZ,
+                     cudaStream_t st) {
+    const size_t smem = (size_t)(((DB ? 2 : 1) * Q2_NBK + NC) * Q2_LDV + (DB ? 2 : 1) * Q2_NBK * Q2_NBK + (ALIAS ? 1 : 2) * NC * Q2_LDW) * sizeof(T);
+    static bool attr = false;
+    if (!attr) {
+        NAO_CUDA_CHECK(cudaFuncSetAttribute(q2_apply_kernel<T, NC, NW, DB, ALIAS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr = true;
+    }
+    q2_apply_kernel<T, NC, NW, DB, ALIAS><<<dim3(ceil_div(ncols, NC), batch), NW * 32, smem, st>>>(n, ncols, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ);
+    NAO_LAUNCHED();
+    return NAO_OK;
+}
+
 template <class T>
 static int q2_apply_impl(int n, int ncols, int batch, const T *V2, long ldv, long sV2, const T *tau2, T *Z, long ldz, long sZ,
                          void *work, cudaStream_t st) {
@@ -320,14 +360,10 @@ static int q2_apply_impl(int n, int ncols, int batch, const T *V2, long ldv, lon
     T *Tst = (T *)work;
     const int nS = ceil_div(n - 1, Q2_NBK), kmax = q2_nwin(n, 0);
     const size_t smem_t = (size_t)Q2_NBK * Q2_LDV * sizeof(T);
-    auto smem_a = [](int nc) { return (size_t)((Q2_NBK + nc) * Q2_LDV + Q2_NBK * Q2_NBK + 2 * nc * Q2_LDW) * sizeof(T); };
-    constexpr int NCMAX = Q2Cfg<T>::NCMAX;
+    constexpr int NCMAX = Q2Cfg<T>::NCMAX, NCWIDE = Q2Cfg<T>::NCWIDE;
     static bool attr = false;
     if (!attr) {
         NAO_CUDA_CHECK(cudaFuncSetAttribute(q2_tfactor_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_t));
-        NAO_CUDA_CHECK(cudaFuncSetAttribute(q2_apply_kernel<T, NCMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_a(NCMAX)));
-        NAO_CUDA_CHECK(cudaFuncSetAttribute(q2_apply_kernel<T, NCMAX / 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_a(NCMAX / 2)));
-        NAO_CUDA_CHECK(cudaFuncSetAttribute(q2_apply_kernel<T, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_a(8)));
         attr = true;
     }
     q2_tfactor_kernel<T><<<dim3(nS, kmax, batch), 256, smem_t, st>>>(n, V2, ldv, sV2, tau2, sTau2, Tst, sTst);
@@ -338,13 +374,22 @@ static int q2_apply_impl(int n, int ncols, int batch, const T *V2, long ldv, lon
     cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
     int nc = NCMAX;
     while (nc > 8 && (long)ceil_div(ncols, nc) * batch < 2L * nsm) nc /= 2;
-    if (nc == NCMAX)
-        q2_apply_kernel<T, NCMAX><<<dim3(ceil_div(ncols, nc), batch), Q2_NT, smem_a(nc), st>>>(n, ncols, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ);
-    else if (nc == NCMAX / 2)
-        q2_apply_kernel<T, NCMAX / 2><<<dim3(ceil_div(ncols, nc), batch), Q2_NT, smem_a(nc), st>>>(n, ncols, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ);
-    else
-        q2_apply_kernel<T, 8><<<dim3(ceil_div(ncols, 8), batch), Q2_NT, smem_a(8), st>>>(n, ncols, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ);
-    NAO_LAUNCHED();
+    int rc;
+    // Many columns: ONE CTA per SM with 8 warps, a slab of NCWIDE columns and V, T of the next diamond prefetched while the
+    // current one is applied -- when those CTAs fit in fewer rounds than the NCMAX-wide ones (two per SM) would need
+    // (config 2, all columns: 140 CTAs on 148 SMs instead of 416 CTAs = 1.4 rounds of 296).
+    if (nc == NCMAX && NCWIDE != NCMAX) {
+        const long ctas = (long)ceil_div(ncols, NCMAX) * batch;
+        if (getenv("NAO_Q2_WIDE"))
+            rc = q2_launch<T, NCWIDE, 8, true, false>(n, ncols, batch, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ, st);
+        else if (ctas > 2L * nsm && ctas <= 3L * nsm)
+            rc = q2_launch<T, NCMAX, 4, false, true>(n, ncols, batch, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ, st);
+        else
+            rc = q2_launch<T, NCMAX, 4, false, false>(n, ncols, batch, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ, st);
+    } else if (nc == NCMAX) rc = q2_launch<T, NCMAX, 4, false, false>(n, ncols, batch, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ, st);
+    else if (nc == NCMAX / 2) rc = q2_launch<T, NCMAX / 2, 4, false, false>(n, ncols, batch, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ, st);
+    else rc = q2_launch<T, 8, 4, false, false>(n, ncols, batch, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ, st);
+    if (rc) return rc;
     NAO_CUDA_CHECK(cudaGetLastError());
     return NAO_OK;
 }
