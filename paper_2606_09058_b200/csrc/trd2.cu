@@ -200,13 +200,21 @@ __global__ void __launch_bounds__(256) he2hb_small_kernel(const T *GS, long sGS,
     }
     if (tid < b) s_tau[tid] = tau[tid];
     __syncthreads();
+    // column i of T: T(0:i, i) = -tau_i T(0:i,0:i) G(0:i, i).  Row `row` of the product by 4 adjacent lanes (the recurrence is
+    // bound by the latency of this dependent chain); 64 rows x 4 lanes = 256 threads
     for (int i = 0; i < b; ++i) {
-        if (tid < i) {
-            T acc = O::zero();
-            for (int c = tid; c < i; ++c) acc = O::fma(sT[tid * LD + c], sG[c * LD + i], acc);
-            sT[tid * LD + i] = O::sub(O::zero(), O::mul(s_tau[i], acc));
+        const int row = tid >> 2, part = tid & 3;
+        T acc = O::zero();
+        if (row < i)
+            for (int c = row + part; c < i; c += 4) acc = O::fma(sT[row * LD + c], sG[c * LD + i], acc);
+        double *a = (double *)&acc;
+#pragma unroll
+        for (int w = 0; w < (int)(sizeof(T) / 8); ++w) {
+            a[w] += __shfl_xor_sync(0xffffffffu, a[w], 1);
+            a[w] += __shfl_xor_sync(0xffffffffu, a[w], 2);
         }
-        if (tid == i) sT[i * LD + i] = s_tau[i];
+        if (row < i && part == 0) sT[row * LD + i] = O::sub(O::zero(), O::mul(s_tau[i], acc));
+        if (tid == 0) sT[i * LD + i] = s_tau[i];
         __syncthreads();
     }
     for (int e = tid; e < b * b; e += 256) {

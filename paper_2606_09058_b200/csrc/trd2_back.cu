@@ -12,7 +12,6 @@
 #include "nao_internal.cuh"
 #include "scalar.cuh"
 #include <algorithm>
-#include <cstdlib>
 
 namespace nao {
 
@@ -117,9 +116,8 @@ template <> __device__ __forceinline__ double frag_out<double>(const double (&ac
 template <> __device__ __forceinline__ cplx frag_out<cplx>(const double (&acc)[4], int q) { return make_double2(acc[q], acc[2 + q]); }
 
 template <class T> struct Q2Cfg;
-// NCMAX: columns of Z per 4-warp CTA (two CTAs per SM); NCWIDE: per 8-warp CTA with double-buffered V, T (one CTA per SM)
-template <> struct Q2Cfg<double> { static const int NCMAX = 32, NCWIDE = 96; };
-template <> struct Q2Cfg<cplx> { static const int NCMAX = 16, NCWIDE = 16; };
+template <> struct Q2Cfg<double> { static const int NCMAX = 32; };     // most columns of Z per CTA (shared memory)
+template <> struct Q2Cfg<cplx> { static const int NCMAX = 16; };
 
 template <class T> __device__ __forceinline__ void cp_async_elem(T *s, const T *g, bool pred) {
     if constexpr (sizeof(T) == 16) cp_async16(s, g, pred); else cp_async8(s, g, pred);
@@ -360,7 +358,7 @@ static int q2_apply_impl(int n, int ncols, int batch, const T *V2, long ldv, lon
     T *Tst = (T *)work;
     const int nS = ceil_div(n - 1, Q2_NBK), kmax = q2_nwin(n, 0);
     const size_t smem_t = (size_t)Q2_NBK * Q2_LDV * sizeof(T);
-    constexpr int NCMAX = Q2Cfg<T>::NCMAX, NCWIDE = Q2Cfg<T>::NCWIDE;
+    constexpr int NCMAX = Q2Cfg<T>::NCMAX;
     static bool attr = false;
     if (!attr) {
         NAO_CUDA_CHECK(cudaFuncSetAttribute(q2_tfactor_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_t));
@@ -375,18 +373,13 @@ static int q2_apply_impl(int n, int ncols, int batch, const T *V2, long ldv, lon
     int nc = NCMAX;
     while (nc > 8 && (long)ceil_div(ncols, nc) * batch < 2L * nsm) nc /= 2;
     int rc;
-    // Many columns: ONE CTA per SM with 8 warps, a slab of NCWIDE columns and V, T of the next diamond prefetched while the
-    // current one is applied -- when those CTAs fit in fewer rounds than the NCMAX-wide ones (two per SM) would need
-    // (config 2, all columns: 140 CTAs on 148 SMs instead of 416 CTAs = 1.4 rounds of 296).
-    if (nc == NCMAX && NCWIDE != NCMAX) {
-        const long ctas = (long)ceil_div(ncols, NCMAX) * batch;
-        if (getenv("NAO_Q2_WIDE"))
-            rc = q2_launch<T, NCWIDE, 8, true, false>(n, ncols, batch, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ, st);
-        else if (ctas > 2L * nsm && ctas <= 3L * nsm)
-            rc = q2_launch<T, NCMAX, 4, false, true>(n, ncols, batch, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ, st);
-        else
-            rc = q2_launch<T, NCMAX, 4, false, false>(n, ncols, batch, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ, st);
-    } else if (nc == NCMAX) rc = q2_launch<T, NCMAX, 4, false, false>(n, ncols, batch, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ, st);
+    // Real slabs of NCMAX columns: with W2 written over W (one more block barrier) three CTAs fit on an SM; used when two
+    // per SM would need a second round of CTAs (config 2, all columns: 416 CTAs > 2 x 148, <= 3 x 148: 117 -> 98 ms;
+    // an 8-warp CTA per SM with a 96-column slab and double-buffered V, T measured 121 ms).
+    const long ctas = (long)ceil_div(ncols, NCMAX) * batch;
+    if (nc == NCMAX && sizeof(T) == 8 && ctas > 2L * nsm)
+        rc = q2_launch<T, NCMAX, 4, false, true>(n, ncols, batch, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ, st);
+    else if (nc == NCMAX) rc = q2_launch<T, NCMAX, 4, false, false>(n, ncols, batch, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ, st);
     else if (nc == NCMAX / 2) rc = q2_launch<T, NCMAX / 2, 4, false, false>(n, ncols, batch, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ, st);
     else rc = q2_launch<T, 8, 4, false, false>(n, ncols, batch, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ, st);
     if (rc) return rc;
