@@ -19,6 +19,8 @@ static const int Q2_NBK = 32;                 // sweeps per diamond
 static const int Q2_LW = 96;                  // padded window rows (>= TRD2_B + Q2_NBK - 1)
 static const int Q2_NT = 128;
 static const int Q2_LDV = 100, Q2_LDW = 36;   // shared-memory leading dimensions (conflict-free fragment loads)
+// T: 36 for real (conflict-free A fragments); complex stays at 32 so that two CTAs of 16 columns still fit on an SM
+template <class T> struct Q2Ldt { static const int value = sizeof(T) == 8 ? 36 : 32; };
 
 __host__ __device__ inline int q2_nwin(int n, int s0) {      // windows of the S-block starting at sweep s0
     return s0 + 1 <= n - 1 ? (n - 2 - s0) / TRD2_B + 1 : 0;
@@ -131,7 +133,7 @@ __global__ void __launch_bounds__(NW * 32) q2_apply_kernel(int n, int ncols, con
                                                            long sTst, T *Z, long ldz, long sZ) {
     typedef Ops<T> O;
     constexpr int b = TRD2_B, NBK = Q2_NBK, LW = Q2_LW, CS = NW / 4, NCW = NC / CS, NCT = NCW / 8, LDV = Q2_LDV, LDW = Q2_LDW,
-                  LDT = NBK, NBUF = DB ? 2 : 1, NTH = NW * 32;
+                  LDT = Q2Ldt<T>::value, NBUF = DB ? 2 : 1, NTH = NW * 32;
     static_assert(NW == 4 || NW == 8, "4 or 8 warps");
     static_assert(NC % (8 * CS) == 0 && NC % NW == 0, "slab width");
     const int item = blockIdx.y, c0 = blockIdx.x * NC;
@@ -147,19 +149,23 @@ __global__ void __launch_bounds__(NW * 32) q2_apply_kernel(int n, int ncols, con
 
     // rows [ra, LW) of the window starting at global row w0 (Lw valid rows) from global memory, zero beyond Lw.
     // warp <-> columns c = warp, warp + NW, ...; lane <-> rows: no integer division anywhere in the window loop
+    T *const zwarp = Z + (long)(c0 + warp) * ldz;          // this warp's first column; its columns are NW apart
+    const long zstep = (long)NW * ldz;
     auto load_z = [&](int w0, int Lw, int ra) {
+        const T *zc = zwarp + w0 + ra + lane;
+        T *sz = sZ_ + warp * LDV + ra + lane;
 #pragma unroll
-        for (int c = warp; c < NC; c += NW) {
-            const bool cok = c0 + c < ncols;
-            const T *zc = Z + w0 + (long)(c0 + c) * ldz;
+        for (int jj = 0; jj < NC / NW; ++jj) {
+            const bool cok = c0 + warp + jj * NW < ncols;
 #pragma unroll
             for (int rr = 0; rr < LW; rr += 32) {
                 const int r = ra + rr + lane;
                 if (r < LW) {
                     const bool ok = cok && r < Lw;
-                    cp_async_elem<T>(sZ_ + c * LDV + r, ok ? zc + r : Z, ok);
+                    cp_async_elem<T>(sz + jj * NW * LDV + rr, ok ? zc + rr : Z, ok);
                 }
             }
+            zc += zstep;
         }
     };
     const int nsweeps = n - 1;
@@ -181,7 +187,7 @@ __global__ void __launch_bounds__(NW * 32) q2_apply_kernel(int n, int ncols, con
         }
         const T *Tg = Tst + gidx * NBK * NBK;
 #pragma unroll
-        for (int e = tid; e < NBK * NBK; e += NTH) cp_async_elem<T>(sT + e, Tg + e, true);
+        for (int e = tid; e < NBK * NBK; e += NTH) cp_async_elem<T>(sT + (e >> 5) * LDT + (e & 31), Tg + e, true);
     };
 
     const int nS = (nsweeps + NBK - 1) / NBK;
@@ -308,11 +314,27 @@ __global__ void __launch_bounds__(NW * 32) q2_apply_kernel(int n, int ncols, con
             // ---- rows leaving the window go to global memory; the overlap with the next window moves to the top
             const bool last = (k + 1 == nwin);
             const int nout = last ? Lw : min(b, Lw);
+            if (nout == b) {
+                // the common case (b = 64 rows leave): all shared-memory reads of the warp's columns first, then the stores
+                T o0[NC / NW], o1[NC / NW];
 #pragma unroll
-            for (int c = warp; c < NC; c += NW) {
-                if (c0 + c < ncols) {
-                    T *zc = Z + w0 + (long)(c0 + c) * ldz;
-                    for (int r = lane; r < nout; r += 32) zc[r] = sZ_[c * LDV + r];
+                for (int jj = 0; jj < NC / NW; ++jj) {
+                    o0[jj] = sZ_[(warp + jj * NW) * LDV + lane];
+                    o1[jj] = sZ_[(warp + jj * NW) * LDV + 32 + lane];
+                }
+                T *zc = zwarp + w0 + lane;
+#pragma unroll
+                for (int jj = 0; jj < NC / NW; ++jj) {
+                    if (c0 + warp + jj * NW < ncols) { zc[0] = o0[jj]; zc[32] = o1[jj]; }
+                    zc += zstep;
+                }
+            } else {
+#pragma unroll
+                for (int c = warp; c < NC; c += NW) {
+                    if (c0 + c < ncols) {
+                        T *zc = Z + w0 + (long)(c0 + c) * ldz;
+                        for (int r = lane; r < nout; r += 32) zc[r] = sZ_[c * LDV + r];
+                    }
                 }
             }
             if (!last) {
@@ -339,7 +361,7 @@ size_t q2_workspace(int dtype, int n, int batch) { return align_up((size_t)batch
 template <class T, int NC, int NW, bool DB, bool ALIAS>
 static int q2_launch(int n, int ncols, int batch, const T *V2, long ldv, long sV2, const T *Tst, long sTst, T *Z, long ldz, long sZ,
                      cudaStream_t st) {
-    const size_t smem = (size_t)(((DB ? 2 : 1) * Q2_NBK + NC) * Q2_LDV + (DB ? 2 : 1) * Q2_NBK * Q2_NBK + (ALIAS ? 1 : 2) * NC * Q2_LDW) * sizeof(T);
+    const size_t smem = (size_t)(((DB ? 2 : 1) * Q2_NBK + NC) * Q2_LDV + (DB ? 2 : 1) * Q2_NBK * Q2Ldt<T>::value + (ALIAS ? 1 : 2) * NC * Q2_LDW) * sizeof(T);
     static bool attr = false;
     if (!attr) {
         NAO_CUDA_CHECK(cudaFuncSetAttribute(q2_apply_kernel<T, NC, NW, DB, ALIAS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
