@@ -96,7 +96,11 @@ __device__ __forceinline__ void house_warp(T *x, int L, T *s_tau, double *s_beta
     if (lane == 0) { x[0] = O::one(); *s_tau = tau; *s_beta = beta; }
 }
 
-template <class T>
+// PF (real only: two pairs of blocks fit in shared memory): the blocks of step k+1 are requested (cp.async, second buffer)
+// while step k is computed.  Only the LAST row of O and of D is written by the predecessor sweep's step k+2; everything
+// else of those blocks is final once the predecessor has finished step k+1 -- which the CTA has already waited for at the
+// start of step k.  The last row is read after the wait of step k+1, with one short round trip.
+template <class T, bool PF>
 __global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
     typedef Ops<T> O;
     constexpr int b = TRD2_B, ld = 2 * b, LDS = b + 1;
@@ -111,6 +115,7 @@ __global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
     extern __shared__ __align__(16) unsigned char ch_smem[];
     T *sO = (T *)ch_smem;              // [b][LDS]  off-diagonal block, column-major
     T *sD = sO + b * LDS;              // [b][LDS]  diagonal block (full Hermitian)
+    T *sO2 = sD + b * LDS, *sD2 = sO2 + b * LDS;      // PF: the pair of the next step
     __shared__ T s_vp[b], s_vn[b], s_w[b], s_u[b], s_z[b], s_part[4][b], s_part2[4][b];
     __shared__ T s_tau_p, s_tau_n, s_kappa;
     __shared__ double s_beta, s_gamma;
@@ -192,6 +197,20 @@ __global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
         }
     };
 
+    // PF: request rows 0..b-2 of the blocks of step k1 of sweep s into (sO2, sD2); D lower part only; zero elsewhere
+    auto prefetch = [&](int s, int k1) {
+        const int q1 = s + 1 + k1 * b;
+        if (q1 > n - 1) return;
+        const int Lq1 = min(s + (k1 + 1) * b, n - 1) - q1 + 1, r1 = q1 - b;      // the column block of O has b columns
+#pragma unroll
+        for (int it = 0; it < b * b / CH_NT; ++it) {
+            const int e = tid + it * CH_NT, i = e & (b - 1), cc = e >> 6;
+            const bool po = i < Lq1 && i < b - 1, pd = po && i >= cc;
+            cp_async8(sO2 + cc * LDS + i, po ? AB + (q1 + i - r1 - cc) + (long)(r1 + cc) * ld : AB, po);
+            cp_async8(sD2 + cc * LDS + i, pd ? AB + (i - cc) + (long)(q1 + cc) * ld : AB, pd);
+        }
+        cp_async_commit();
+    };
 #ifdef NAO_TRACE
     unsigned long long ch_last; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(ch_last));
 #endif
@@ -202,6 +221,7 @@ __global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
             if (tid == 0) { while (ld_acquire(prog + s - 1) < 2) { } }
             __syncthreads();
         }
+        if constexpr (PF) prefetch(s, 1);
         if (tid < b) s_vn[tid] = tid < Lp ? ldcg(AB + (1 + tid) + (long)s * ld) : O::zero();
         load_D(r0, Lp);
         __syncthreads();
@@ -229,7 +249,31 @@ __global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
                 __syncthreads();
             }
             CH_T(1);
-            // load O = B[q0 : q0+Lq, r0 : r0+Lp] and D = B[q0.., q0..]
+            if constexpr (PF) {
+                // the prefetched pair becomes current; its last row arrives now (written by the predecessor's latest step)
+                cp_async_wait<0>();
+                { T *t = sO; sO = sO2; sO2 = t; t = sD; sD = sD2; sD2 = t; }
+                T late = O::zero();
+                const bool has_late = Lq == b && tid < 2 * b;
+                if (has_late) {
+                    const int cc = tid & (b - 1);
+                    late = tid < b ? ldcg(AB + (q0 + b - 1 - r0 - cc) + (long)(r0 + cc) * ld)
+                                   : ldcg(AB + (b - 1 - cc) + (long)(q0 + cc) * ld);
+                }
+                __syncthreads();                 // everybody's prefetched elements have landed; the old pair is free
+                prefetch(s, k + 1);
+                // Hermitian completion of D from its lower part (rows <= b-2 now, row/column b-1 below)
+#pragma unroll
+                for (int it = 0; it < b * b / CH_NT; ++it) {
+                    const int e = tid + it * CH_NT, i = e & (b - 1), cc = e >> 6;
+                    if (i < cc && cc < b - 1) sD[cc * LDS + i] = O::conj(sD[i * LDS + cc]);
+                }
+                if (has_late) {
+                    const int cc = tid & (b - 1);
+                    if (tid < b) sO[cc * LDS + b - 1] = late;
+                    else { sD[cc * LDS + b - 1] = late; sD[(b - 1) * LDS + cc] = O::conj(late); }
+                }           // (short last block: row b-1 does not exist; column b-1 of D was zero-filled by the prefetch)
+            } else
             {   // both blocks in ONE L2 round trip: all 2 x 16 loads of a thread are issued before the first shared-memory store
                 T bo[b * b / CH_NT], bd[b * b / CH_NT];
 #pragma unroll
@@ -255,10 +299,17 @@ __global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
             //   O[:,c] <- O[:,c] - tau_p w conj(v_p[c]) - conj(tau_n) v_n z_c  (c >= 1);  O[:,0] <- beta e_0
             //   u = D v_n ; gamma = v_n^H u ; y = tau_n u - 1/2 |tau_n|^2 gamma v_n ;  D <- D - y v_n^H - v_n y^H
             // (1) w partials: thread <-> (row iq, column quarter qq)
+            // (the blocks and the vectors are zero beyond Lq / Lp: all loops run over the full block with compile-time trip
+            //  counts, two accumulators each)
             {
-                T sacc = O::zero();
-                if (iq < Lq) for (int cc = qq; cc < Lp; cc += 4) sacc = O::fma(sO[cc * LDS + iq], s_vp[cc], sacc);
-                s_part[qq][iq] = sacc;
+                T s0 = O::zero(), s1 = O::zero();
+#pragma unroll
+                for (int t = 0; t < b / 8; ++t) {
+                    const int c0_ = qq + 8 * t, c1_ = c0_ + 4;
+                    s0 = O::fma(sO[c0_ * LDS + iq], s_vp[c0_], s0);
+                    s1 = O::fma(sO[c1_ * LDS + iq], s_vp[c1_], s1);
+                }
+                s_part[qq][iq] = O::add(s0, s1);
             }
             __syncthreads();
             // (2) w, x
@@ -282,10 +333,16 @@ __global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
             if (tid == 0) tau2[(long)k * n + s] = s_tau_n;
             // (4) q partials: thread <-> (column iq, row quarter qq);  u partials: thread <-> (row iq, column quarter qq)
             {
-                T qa = O::zero(), ua = O::zero();
-                if (iq < Lp) for (int i = qq; i < Lq; i += 4) qa = O::add(qa, O::conj_mul(s_vn[i], sO[iq * LDS + i]));
-                if (iq < Lq) for (int cc = qq; cc < Lq; cc += 4) ua = O::fma(sD[cc * LDS + iq], s_vn[cc], ua);
-                s_part[qq][iq] = qa; s_part2[qq][iq] = ua;
+                T qa0 = O::zero(), qa1 = O::zero(), ua0 = O::zero(), ua1 = O::zero();
+#pragma unroll
+                for (int t = 0; t < b / 8; ++t) {
+                    const int i0_ = qq + 8 * t, i1_ = i0_ + 4;
+                    qa0 = O::add(qa0, O::conj_mul(s_vn[i0_], sO[iq * LDS + i0_]));
+                    qa1 = O::add(qa1, O::conj_mul(s_vn[i1_], sO[iq * LDS + i1_]));
+                    ua0 = O::fma(sD[i0_ * LDS + iq], s_vn[i0_], ua0);
+                    ua1 = O::fma(sD[i1_ * LDS + iq], s_vn[i1_], ua1);
+                }
+                s_part[qq][iq] = O::add(qa0, qa1); s_part2[qq][iq] = O::add(ua0, ua1);
             }
             __syncthreads();
             // (5) z (scaled by conj(tau_n)), u, gamma
@@ -311,17 +368,26 @@ __global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
                 auto yv = [&](int i) -> T { return O::add(O::mul(tau_n, s_u[i]), O::scale(s_vn[i], f)); };
                 if (iq < Lq) {
                     const T twi = O::mul(tau_p, s_w[iq]), vni = s_vn[iq], yi = yv(iq);
-                    for (int cc = qq; cc < Lp; cc += 4) {
-                        T o;
-                        if (cc == 0) o = iq == 0 ? O::from_real(s_beta) : O::zero();
-                        else o = O::sub(O::sub(sO[cc * LDS + iq], O::mul_conj(twi, s_vp[cc])), O::mul(vni, s_z[cc]));
-                        AB[(q0 + iq - r0 - cc) + (long)(r0 + cc) * ld] = o;
+                    T *po = AB + (q0 + iq - r0 - qq) + (long)(r0 + qq) * ld;     // element (iq, cc) of O; cc -> cc + 4: += 4 (ld - 1)
+                    T *pd = AB + (iq - qq) + (long)(q0 + qq) * ld;               // element (iq, cc) of D
+#pragma unroll
+                    for (int t = 0; t < b / 4; ++t) {
+                        const int cc = qq + 4 * t;
+                        if (cc < Lp) {
+                            T o;
+                            if (cc == 0) o = iq == 0 ? O::from_real(s_beta) : O::zero();
+                            else o = O::sub(O::sub(sO[cc * LDS + iq], O::mul_conj(twi, s_vp[cc])), O::mul(vni, s_z[cc]));
+                            po[(long)t * 4 * (ld - 1)] = o;
+                        }
                     }
-                    for (int cc = qq; cc < Lq; cc += 4) {
-                        if (iq < cc) continue;                                   // lower part is what is stored
-                        T a = O::sub(sD[cc * LDS + iq], O::add(O::mul_conj(yi, s_vn[cc]), O::mul_conj(vni, yv(cc))));
-                        if (cc == iq) a = O::from_real(O::real(a));
-                        AB[(iq - cc) + (long)(q0 + cc) * ld] = a;
+#pragma unroll
+                    for (int t = 0; t < b / 4; ++t) {
+                        const int cc = qq + 4 * t;
+                        if (cc <= iq) {                                          // lower part is what is stored (iq < Lq)
+                            T a = O::sub(sD[cc * LDS + iq], O::add(O::mul_conj(yi, s_vn[cc]), O::mul_conj(vni, yv(cc))));
+                            if (cc == iq) a = O::from_real(O::real(a));
+                            pd[(long)t * 4 * (ld - 1)] = a;
+                        }
                     }
                 }
             }
@@ -374,10 +440,11 @@ static int hb2st_impl(int dtype, int n, int batch, const T *A, long lda, long sA
                       long sV2, T *tau2, void *work, cudaStream_t st) {
     constexpr int b = TRD2_B;
     ChaseWork w = chase_plan(dtype, n, batch, work);
-    const size_t smem = (size_t)2 * b * (b + 1) * sizeof(T);
+    constexpr bool PF = sizeof(T) == 8;          // double-buffered blocks: real only (complex blocks are twice the size)
+    const size_t smem = (size_t)(PF ? 4 : 2) * b * (b + 1) * sizeof(T);
     static bool attr = false;
     if (!attr) {
-        NAO_CUDA_CHECK(cudaFuncSetAttribute(chase_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        NAO_CUDA_CHECK(cudaFuncSetAttribute(chase_kernel<T, PF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr = true;
     }
     const long sAB = (long)2 * b * n, sTau2 = (long)hb2st_nk(n) * n;
@@ -395,7 +462,7 @@ static int hb2st_impl(int dtype, int n, int batch, const T *A, long lda, long sA
         a.d = d + (long)b0 * n; a.e = e + (long)b0 * n; a.prog = w.prog + (long)b0 * n;
         a.n = n; a.P = w.P;
         void *args[] = {&a};
-        NAO_CUDA_CHECK(cudaLaunchCooperativeKernel((void *)chase_kernel<T>, dim3(nit * w.P), dim3(CH_NT), args, smem, st));
+        NAO_CUDA_CHECK(cudaLaunchCooperativeKernel((void *)chase_kernel<T, PF>, dim3(nit * w.P), dim3(CH_NT), args, smem, st));
         NAO_LAUNCHED();
     }
     NAO_CUDA_CHECK(cudaGetLastError());
