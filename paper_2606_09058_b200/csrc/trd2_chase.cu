@@ -312,21 +312,38 @@ __global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
                 s_part[qq][iq] = O::add(s0, s1);
             }
             __syncthreads();
-            // (2) w, x
-            if (tid < b) {
-                const T w = tid < Lq ? O::add(O::add(s_part[0][tid], s_part[1][tid]), O::add(s_part[2][tid], s_part[3][tid])) : O::zero();
-                s_w[tid] = w;
-                s_vn[tid] = tid < Lq ? O::sub(sO[tid], O::mul(s_tau_p, w)) : O::zero();      // v_p[0] = 1
-            }
-            __syncthreads();
-            // (3) reflector, kappa
+            // (2)+(3) w, x, the reflector (xLARFG) and kappa by warp 0 alone, two elements per lane, reductions in registers
             if (warp == 0) {
-                house_warp<T>(s_vn, Lq, &s_tau_n, &s_beta);
-                __syncwarp();
-                T kp = O::zero();
-                for (int i = tid; i < Lq; i += 32) kp = O::add(kp, O::conj_mul(s_vn[i], s_w[i]));
+                const int i0_ = tid, i1_ = tid + 32;
+                const T w0_ = i0_ < Lq ? O::add(O::add(s_part[0][i0_], s_part[1][i0_]), O::add(s_part[2][i0_], s_part[3][i0_])) : O::zero();
+                const T w1_ = i1_ < Lq ? O::add(O::add(s_part[0][i1_], s_part[1][i1_]), O::add(s_part[2][i1_], s_part[3][i1_])) : O::zero();
+                const T taup = s_tau_p;
+                T x0_ = i0_ < Lq ? O::sub(sO[i0_], O::mul(taup, w0_)) : O::zero();      // v_p[0] = 1
+                T x1_ = i1_ < Lq ? O::sub(sO[i1_], O::mul(taup, w1_)) : O::zero();
+                s_w[i0_] = w0_; s_w[i1_] = w1_;
+                double xn2 = (tid == 0 ? 0.0 : O::abs2(x0_)) + O::abs2(x1_);
+                xn2 = warp_sum(xn2);
+                const double ar = __shfl_sync(0xffffffffu, O::real(x0_), 0), ai = __shfl_sync(0xffffffffu, O::imag(x0_), 0);
+                T tau, scale; double beta;
+                if (xn2 == 0.0 && ai == 0.0) { tau = O::zero(); scale = O::zero(); beta = ar; }
+                else {
+                    const double nrm = sqrt(ar * ar + ai * ai + xn2);
+                    beta = ar >= 0.0 ? -nrm : nrm;
+                    if (O::is_complex) {
+                        cplx t = make_double2((beta - ar) / beta, -ai / beta);
+                        const double dr = ar - beta, di = ai, den = dr * dr + di * di;
+                        cplx sc = make_double2(dr / den, -di / den);
+                        tau = *(T *)&t; scale = *(T *)&sc;
+                    } else {
+                        tau = O::from_real((beta - ar) / beta); scale = O::from_real(1.0 / (ar - beta));
+                    }
+                }
+                x0_ = tid == 0 ? O::one() : O::mul(scale, x0_);
+                x1_ = O::mul(scale, x1_);
+                s_vn[i0_] = x0_; s_vn[i1_] = x1_;
+                T kp = O::add(O::conj_mul(x0_, w0_), O::conj_mul(x1_, w1_));
                 kp = warp_sum(kp);
-                if (tid == 0) s_kappa = kp;
+                if (tid == 0) { s_tau_n = tau; s_beta = beta; s_kappa = kp; }
             }
             __syncthreads();
             if (tid < Lq) V2[(q0 + tid) + (long)s * p.ldv] = s_vn[tid];
@@ -352,12 +369,17 @@ __global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
                 s_z[tid] = O::mul(O::conj(s_tau_n), z);
                 s_u[tid] = tid < Lq ? O::add(O::add(s_part2[0][tid], s_part2[1][tid]), O::add(s_part2[2][tid], s_part2[3][tid])) : O::zero();
             }
-            __syncthreads();
-            if (warp == 0) {
+            else if (warp == 2) {
+                // gamma = v_n^H u straight from the partial sums, beside the threads that form z and u
                 double gsum = 0.0;
-                for (int i = tid; i < Lq; i += 32) gsum += O::real(O::conj_mul(s_vn[i], s_u[i]));
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const int i = (tid & 31) + 32 * h;
+                    const T u = O::add(O::add(s_part2[0][i], s_part2[1][i]), O::add(s_part2[2][i], s_part2[3][i]));
+                    if (i < Lq) gsum += O::real(O::conj_mul(s_vn[i], u));
+                }
                 gsum = warp_sum(gsum);
-                if (tid == 0) s_gamma = gsum;
+                if ((tid & 31) == 0) s_gamma = gsum;
             }
             __syncthreads();
             CH_T(3);
