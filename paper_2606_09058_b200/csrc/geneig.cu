@@ -15,9 +15,10 @@ namespace nao {
 // ----------------------------------------------------------------------------------------------------- heev
 struct HeevPlan { size_t d, e, tau, qt, sub, v2, tau2, sub2, bytes; bool two_stage; };
 // Default switch-over (flags force either path), from `microbench heev` on B200 with all eigenvectors, one-stage vs
-// two-stage in ms: real n = 4992 x 2 items 223 vs 238, n = 6656 x 1 310 vs 295, n = 6656 x 2 414 vs 388, n = 9984 x 1 698 vs
-// 679; complex n = 9984 1.29 s vs 1.55 s (the second back-transformation runs at a lower rate in complex arithmetic).
-static const int TWO_STAGE_MIN_N_REAL = 6144;
+// two-stage in ms: real n = 1664 x 2 items 41.6 vs 40.3, 3328 x 2 106.8 vs 102.3, 3328 x 1 97.6 vs 88.9, 4992 x 2 222.7 vs
+// 211.0, 6656 x 1 309.7 vs 262.2, 6656 x 2 413.6 vs 351, 9984 x 1 698 vs 617; complex n = 9984 1.29 s vs 1.5 s (the second
+// back-transformation runs at a lower rate in complex arithmetic, and the chase cannot double-buffer complex blocks).
+static const int TWO_STAGE_MIN_N_REAL = 1536;
 static bool use_two_stage(int dtype, int n, int batch, unsigned flags) {
     if (flags & NAO_TRD_ONE_STAGE) return false;
     if (!he2hb_supported(dtype, n, batch)) return false;
