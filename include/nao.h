@@ -41,6 +41,8 @@ extern "C" {
                                   (S and V = its orthogonaliser do not change during the SCF loop) */
 #define NAO_NC_BLOCK_S 2u      /* noncollinear fast path: n = 2N, dtype = NAO_COMPLEX, basis spin-major [alpha;beta]
                                   (Eq. 25-27); dS is the N x N REAL overlap (S_NC = diag(S,S)) */
+/* Without either of the next two flags the library picks the reduction: two-stage for real matrices of order >= 1536,
+   one-stage otherwise (measured crossover on B200, reading T1). */
 #define NAO_TRD_ONE_STAGE 4u   /* force the one-stage (HEMV-based, HBM-bound) Householder tridiagonalisation */
 #define NAO_TRD_TWO_STAGE 8u   /* force the two-stage (dense->band->tridiagonal) reduction */
 #define NAO_LOWDIN 16u         /* orthogonalise by the paper's own route: S = U s U^H with this
