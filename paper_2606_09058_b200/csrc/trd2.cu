@@ -86,8 +86,18 @@ __global__ void __launch_bounds__(QR_NT, 1) panel_qr_kernel(QrArgs<T> p) {
             const int c = tid & (b - 1), q = tid >> 6;
             T s = O::zero();
             if (c >= j) {
+                // all partials of a batch are requested before the first add: one L2 round trip per 20 CTAs x 4 quarters
                 const T *pp = part + (long)(j & 1) * G * b + c;
-                for (int gg = q; gg < G; gg += 4) s = O::add(s, ldcg(pp + (long)gg * b));
+                for (int g0 = q; g0 < G; g0 += 80) {
+                    T bt[20];
+#pragma unroll
+                    for (int u = 0; u < 20; ++u) {
+                        const int gg = g0 + 4 * u;
+                        bt[u] = gg < G ? ldcg(pp + (long)gg * b) : O::zero();
+                    }
+#pragma unroll
+                    for (int u = 0; u < 20; ++u) s = O::add(s, bt[u]);
+                }
             }
             s_red[q][c] = s;
             if (q == 0 && c >= j) s_rho[c] = ldcg(rowb + (j & 1) * b + c);
