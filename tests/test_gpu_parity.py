@@ -606,3 +606,33 @@ def test_lowdin_pruning_of_duplicated_orbitals(nao, kind):
     D = to_np(nao.density_matrix(C, F))[0]
     assert np.abs(D - D_ref).max() <= TOL_D
     assert abs(np.trace(D @ Sfull).real - nel) <= 1e-8
+
+
+def test_default_reduction_at_the_switch_over_size(nao):
+    """Config 2 recipe at 128 atoms (n = 1664 real, 2 spins, one shared S): above the switch-over order (1536) the library takes
+    the two-stage reduction by itself.  The step must agree with the forced one-stage step (e, mu, D) and satisfy the invariants
+    of the definition (C^H S C = I, residual, electron count); the closed-form chain at the same order pins the eigenvalues.
+    Full-size runs of the same path: test_config2 / bench.py."""
+    prob = make_config(2, nat=128)
+    assert prob.n == 1664 and not prob.is_complex
+    nao.profile_enable(True)
+    got = run_path(nao, prob)
+    torch.cuda.synchronize()
+    phases = nao.profile_read()
+    nao.profile_enable(False)
+    assert phases["band_to_tridiagonal"] > 0.05          # the two-stage path ran
+    one = run_path(nao, prob, flags=nao.NAO_TRD_ONE_STAGE)
+    assert np.abs(got["e"] - one["e"]).max() <= TOL_E
+    assert abs(got["mu"] - one["mu"]) <= TOL_MU
+    ne = 0.0
+    for b in range(prob.batch):
+        assert np.abs(got["D"][b] - one["D"][b]).max() <= TOL_D
+        Sb, Cb = prob.S_full(b), got["C"][b]
+        assert np.abs(Cb.T @ Sb @ Cb - np.eye(prob.n)).max() <= TOL_ORTH
+        assert np.abs(prob.H_full(b) @ Cb - Sb @ Cb * got["e"][b]).max() <= 1e-10
+        ne += prob.weights[b] * np.trace(got["D"][b] @ Sb)
+    assert abs(ne - prob.n_electrons) <= 1e-8
+    n = 1664
+    chain = np.diag(np.full(n - 1, -1.0), 1) + np.diag(np.full(n - 1, -1.0), -1)
+    E, Z, info = nao.heev(to_dev(chain[None]))
+    assert np.abs(E.cpu().numpy()[0] - np.sort(-2.0 * np.cos(np.arange(1, n + 1) * np.pi / (n + 1)))).max() <= 1e-12
