@@ -134,6 +134,28 @@ int nao_scf_step(int n, int batch, int dtype, unsigned flags,
                  int *h_nvec, void *dwork, size_t work_bytes, int *d_info, void *cuda_stream);
 
 /*
+ * The same step (nao_geneig, all eigenpairs + nao_fermi_mu + nao_density_matrix) with HOST inputs and outputs: the
+ * end-to-end form of the metric.  hH (batch matrices, n x n, column-major, contiguous), hS (batch matrices, or ONE when
+ * shared_S != 0; order n/2 and real with NAO_NC_BLOCK_S) are copied to the device scratch, hE (batch*n), hD (batch matrices),
+ * h_info (batch ints) and *h_mu are written back.  Pinned host memory makes the copies asynchronous: H travels on an internal
+ * copy stream while S is factored on the caller's stream, and D returns item by item behind the density-matrix product of
+ * the next item.  The call synchronises the stream once (Fermi level); when it returns the remaining copies are enqueued
+ * and the caller's stream is ordered behind them -- synchronise it before reading hE, hD, h_info.
+ *   1 n, 2 batch, 3 dtype, 4 flags (NAO_S_FACTORED is rejected: the factor lives in the scratch)
+ *   5 hH, 6 hS, 7 shared_S, 8 h_weight (HOST double[batch]), 9 n_electrons, 10 kT
+ *  11 hE, 12 h_mu, 13 hD, 14 h_info
+ *  15 dwork, work_bytes  device scratch of at least nao_solve_host_workspace() bytes
+ *  17 cuda_stream
+ * Not re-entrant (one internal copy stream per process).
+ */
+int nao_solve_host_workspace(int n, int batch, int dtype, unsigned flags, int shared_S, size_t *bytes);
+int nao_solve_host(int n, int batch, int dtype, unsigned flags,
+                   const void *hH, const void *hS, int shared_S,
+                   const double *h_weight, double n_electrons, double kT,
+                   double *hE, double *h_mu, void *hD, int *h_info,
+                   void *dwork, size_t work_bytes, void *cuda_stream);
+
+/*
  * 1 + the largest level index i (over all batch items) with dF[b*n + i] >= threshold: the number of leading
  * eigenvectors nao_density_matrix reads.  Synchronises the stream to write *h_count (HOST int).
  */

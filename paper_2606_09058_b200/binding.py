@@ -34,6 +34,8 @@ _SIGNATURES = {
     "nao_scf_step_workspace": ([_i, _i, _i, ctypes.c_uint, _szp], _i),
     "nao_scf_step": ([_i, _i, _i, ctypes.c_uint, _vp, _l, _l, _vp, _l, _l, _dp, _d, _d, _vp, _dp, _vp, _vp, _l, _l, _vp, _l, _l,
                      ctypes.POINTER(ctypes.c_int), _vp, _sz, _vp, _vp], _i),
+    "nao_solve_host_workspace": ([_i, _i, _i, ctypes.c_uint, _i, _szp], _i),
+    "nao_solve_host": ([_i, _i, _i, ctypes.c_uint, _vp, _vp, _i, _dp, _d, _d, _vp, _dp, _vp, _vp, _vp, _sz, _vp], _i),
     "nao_fermi_workspace": ([_i, _i, _szp], _i),
     "nao_fermi_mu": ([_i, _i, _vp, _dp, _d, _d, _dp, _vp, _vp, _vp], _i),
     "nao_density_workspace": ([_i, _i, _i, _szp], _i),
@@ -262,6 +264,37 @@ def density_matrix(C: torch.Tensor, F: torch.Tensor, out: torch.Tensor | None = 
                                   _dev(work, "work"), work.numel(), _stream(C))
     _check(rc, "nao_density_matrix")
     return D
+
+
+def solve_host(Hh: torch.Tensor, Sh: torch.Tensor, weights, n_electrons: float, kT: float, flags: int = 0,
+               device=None, work: torch.Tensor | None = None, Eh: torch.Tensor | None = None, Dh: torch.Tensor | None = None):
+    """nao_solve_host: the whole step with HOST tensors (pinned for asynchronous copies): Hh (batch, n, n), Sh (batch or 1,
+    nS, nS) column-major items.  Returns dict(E, mu, D, info) of host tensors; the current stream of `device` is
+    synchronised before returning."""
+    if Hh.is_cuda or Sh.is_cuda:
+        raise NaoError("solve_host takes host tensors")
+    batch, n, _ = Hh.shape
+    dt = _dtype_code(Hh)
+    dev = torch.device(device if device is not None else "cuda:0")
+    shared = 1 if (Sh.shape[0] == 1 and (batch > 1 or bool(flags & NAO_NC_BLOCK_S))) else 0
+    if Sh.shape[0] == 1 and batch == 1:
+        shared = 0
+    need = ctypes.c_size_t(0)
+    _check(lib().nao_solve_host_workspace(n, batch, dt, flags, shared, ctypes.byref(need)), "nao_solve_host_workspace")
+    if work is None or work.numel() < need.value:
+        work = _workspace(need.value, dev)
+    Eh = torch.empty((batch, n), dtype=torch.float64).pin_memory() if Eh is None else Eh
+    Dh = torch.empty_like(Hh).pin_memory() if Dh is None else Dh
+    info = torch.zeros(batch, dtype=torch.int32).pin_memory()
+    w = (ctypes.c_double * batch)(*[float(x) for x in weights])
+    mu = ctypes.c_double(0.0)
+    stream = torch.cuda.current_stream(dev)
+    rc = lib().nao_solve_host(n, batch, dt, flags, Hh.data_ptr(), Sh.data_ptr(), shared, w, float(n_electrons), float(kT),
+                              Eh.data_ptr(), ctypes.byref(mu), Dh.data_ptr(), info.data_ptr(), _dev(work, "work"), work.numel(),
+                              stream.cuda_stream)
+    _check(rc, "nao_solve_host")
+    stream.synchronize()
+    return dict(E=Eh, mu=mu.value, D=Dh, info=info)
 
 
 def set_lowdin_threshold(rel: float):

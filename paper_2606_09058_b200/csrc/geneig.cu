@@ -167,7 +167,7 @@ NAO_EXPORT int nao_geneig_workspace(int n, int batch, int dtype, unsigned flags,
 // with the same arguments and an untouched workspace.
 static int geneig_impl(int n, int batch, int dtype, unsigned flags, int nvec, const void *dH, long ldh, long strideH, void *dS,
                        long lds, long strideS, double *dE, void *dC, long ldc, long strideC, void *dwork,
-                       size_t work_bytes, int *d_info, void *cuda_stream, int phase = 3) {
+                       size_t work_bytes, int *d_info, void *cuda_stream, int phase = 3, cudaEvent_t h_ready = nullptr) {
     using namespace nao;
     if (n < 1) return -1;
     if (batch < 1) return -2;
@@ -223,6 +223,8 @@ static int geneig_impl(int n, int batch, int dtype, unsigned flags, int nvec, co
         if ((rc = unpack_linv(p.sdtype, nS, dS, lds, strideS, W, nS, sW, p.nitemsS, st))) return rc;
     }
     prof_mark(1, st);
+    // nao_solve_host: H arrives on another stream while S is factored
+    if (h_ready) NAO_CUDA_CHECK(cudaStreamWaitEvent(st, h_ready, 0));
     }
     if (!nc) {
         if (phase & 1) {
@@ -372,6 +374,106 @@ NAO_EXPORT int nao_scf_step(int n, int batch, int dtype, unsigned flags, const v
     rc = geneig_impl(n, batch, dtype, flags, nvec, dH, ldh, strideH, dS, lds, strideS, dE, dC, ldc, strideC, wg, g, d_info, cuda_stream, 2);
     if (rc) return rc;
     return nao_density_matrix(n, batch, dtype, dC, ldc, strideC, dF, dD, ldd, strideD, wd, d, cuda_stream);
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// nao_solve_host: the whole step with HOST inputs and outputs (nao.h).  H travels on an internal copy stream while S is
+// factored on the caller's stream; D goes back item by item behind the density-matrix GEMM of the next item.
+// ---------------------------------------------------------------------------------------------------------------------
+namespace nao {
+struct HostPlan { size_t H, S, E, F, C, D, info, work, wbytes, bytes; int nS, nitemsS; size_t esS; };
+static int host_plan(int n, int batch, int dtype, unsigned flags, int shared_S, HostPlan &p) {
+    size_t off = 0;
+    auto take = [&](size_t b) { size_t o = off; off += align_up(b); return o; };
+    const bool nc = flags & NAO_NC_BLOCK_S;
+    const size_t es = esize(dtype);
+    p.nS = nc ? n / 2 : n; p.esS = nc ? 8 : es; p.nitemsS = shared_S ? 1 : batch;
+    p.H = take((size_t)batch * n * n * es);
+    p.S = take((size_t)p.nitemsS * p.nS * p.nS * p.esS);
+    p.E = take((size_t)batch * n * 8); p.F = take((size_t)batch * n * 8);
+    p.C = take((size_t)batch * n * n * es); p.D = take((size_t)batch * n * n * es);
+    p.info = take((size_t)batch * sizeof(int));
+    int rc = nao_scf_step_workspace(n, batch, dtype, flags, &p.wbytes);
+    if (rc) return rc;
+    p.work = take(p.wbytes);
+    p.bytes = off;
+    return NAO_OK;
+}
+}  // namespace nao
+
+NAO_EXPORT int nao_solve_host_workspace(int n, int batch, int dtype, unsigned flags, int shared_S, size_t *bytes) {
+    if (!bytes) return -6;
+    nao::HostPlan p;
+    int rc = nao::host_plan(n, batch, dtype, flags, shared_S, p);
+    if (rc) return rc;
+    *bytes = p.bytes;
+    return NAO_OK;
+}
+
+NAO_EXPORT int nao_solve_host(int n, int batch, int dtype, unsigned flags, const void *hH, const void *hS, int shared_S,
+                              const double *h_weight, double n_electrons, double kT, double *hE, double *h_mu, void *hD,
+                              int *h_info, void *dwork, size_t work_bytes, void *cuda_stream) {
+    using namespace nao;
+    if (n < 1) return -1;
+    if (batch < 1) return -2;
+    if (dtype != NAO_REAL && dtype != NAO_COMPLEX) return -3;
+    if ((flags & NAO_NC_BLOCK_S) && (dtype != NAO_COMPLEX || (n & 1))) return -4;
+    if (flags & NAO_S_FACTORED) return -4;              // the factor lives in the device scratch: not kept between calls
+    if (!hH) return -5;
+    if (!hS) return -6;
+    if (!h_weight) return -8;
+    if (!hE) return -11;
+    if (!h_mu) return -12;
+    if (!hD) return -13;
+    if (!h_info) return -14;
+    if (!dwork) return -15;
+    HostPlan p;
+    int rc = host_plan(n, batch, dtype, flags, shared_S, p);
+    if (rc) return rc;
+    if (work_bytes < p.bytes) return NAO_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    static cudaStream_t cs = nullptr;
+    static cudaEvent_t ev_start = nullptr, ev_h = nullptr, ev_d = nullptr, ev_end = nullptr;
+    if (!cs) {
+        NAO_CUDA_CHECK(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
+        NAO_CUDA_CHECK(cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming));
+        NAO_CUDA_CHECK(cudaEventCreateWithFlags(&ev_h, cudaEventDisableTiming));
+        NAO_CUDA_CHECK(cudaEventCreateWithFlags(&ev_d, cudaEventDisableTiming));
+        NAO_CUDA_CHECK(cudaEventCreateWithFlags(&ev_end, cudaEventDisableTiming));
+    }
+    char *w = (char *)dwork;
+    const size_t es = esize(dtype);
+    const size_t item = (size_t)n * n * es;
+    void *dH = w + p.H, *dS = w + p.S, *dC = w + p.C, *dD = w + p.D;
+    double *dE = (double *)(w + p.E), *dF = (double *)(w + p.F);
+    int *d_info = (int *)(w + p.info);
+    // the copy stream starts behind whatever the caller's stream still does with the scratch
+    NAO_CUDA_CHECK(cudaEventRecord(ev_start, st));
+    NAO_CUDA_CHECK(cudaStreamWaitEvent(cs, ev_start, 0));
+    NAO_CUDA_CHECK(cudaMemcpyAsync(dS, hS, (size_t)p.nitemsS * p.nS * p.nS * p.esS, cudaMemcpyHostToDevice, st));
+    NAO_CUDA_CHECK(cudaMemcpyAsync(dH, hH, (size_t)batch * item, cudaMemcpyHostToDevice, cs));
+    NAO_CUDA_CHECK(cudaEventRecord(ev_h, cs));
+    size_t g = 0, f = 0, d = 0;
+    nao_geneig_workspace(n, batch, dtype, flags, &g); nao_fermi_workspace(n, batch, &f); nao_density_workspace(n, batch, dtype, &d);
+    char *wg = w + p.work, *wf = wg + align_up(g), *wd = wf + align_up(f);
+    rc = geneig_impl(n, batch, dtype, flags, n, dH, n, (long)n * n, dS, p.nS, shared_S ? 0 : (long)p.nS * p.nS, dE, dC, n, (long)n * n,
+                     wg, g, d_info, cuda_stream, 3, ev_h);
+    if (rc) return rc;
+    if ((rc = fermi_mu(n, batch, dE, h_weight, n_electrons, kT, h_mu, dF, wf, st))) return rc;
+    for (int b = 0; b < batch; ++b) {
+        rc = nao_density_matrix(n, 1, dtype, (char *)dC + b * item, n, (long)n * n, dF + (size_t)b * n, (char *)dD + b * item, n,
+                                (long)n * n, wd, d, cuda_stream);
+        if (rc) return rc;
+        NAO_CUDA_CHECK(cudaEventRecord(ev_d, st));
+        NAO_CUDA_CHECK(cudaStreamWaitEvent(cs, ev_d, 0));
+        NAO_CUDA_CHECK(cudaMemcpyAsync((char *)hD + b * item, (char *)dD + b * item, item, cudaMemcpyDeviceToHost, cs));
+    }
+    NAO_CUDA_CHECK(cudaMemcpyAsync(hE, dE, (size_t)batch * n * 8, cudaMemcpyDeviceToHost, st));
+    NAO_CUDA_CHECK(cudaMemcpyAsync(h_info, d_info, (size_t)batch * sizeof(int), cudaMemcpyDeviceToHost, st));
+    // the caller's stream finishes behind the last copy: synchronising it is enough
+    NAO_CUDA_CHECK(cudaEventRecord(ev_end, cs));
+    NAO_CUDA_CHECK(cudaStreamWaitEvent(st, ev_end, 0));
+    return NAO_OK;
 }
 
 NAO_EXPORT int nao_set_lowdin_threshold(double rel) {

@@ -91,6 +91,14 @@ def test_host_side_argument_validation(libpath):
     assert lib.nao_fold_density(4, 1, 1, 0, 1, 3, 16, k3, k3, k3, 1, 4, 16, 1, 1 << 20, None) == -6      # ldd < n
     assert lib.nao_fold_density(4, 1, 1, 0, 1, 4, 16, k3, None, k3, 1, 4, 16, 1, 1 << 20, None) == -9    # h_w
     assert lib.nao_fold_density(4, 1, 1, 0, 1, 4, 16, k3, k3, k3, 1, 4, 16, 1, 8, None) == 1             # workspace
+    # host-buffer form of the step
+    assert lib.nao_solve_host_workspace(104, 2, 0, 0, 1, ctypes.byref(sz)) == 0 and sz.value > 5 * 2 * 104 * 104 * 8
+    lib.nao_solve_host.argtypes = [i, i, i, ctypes.c_uint, vp, vp, i, dp, ctypes.c_double, ctypes.c_double, vp, dp, vp, vp, vp,
+                                   ctypes.c_size_t, vp]
+    w1 = (ctypes.c_double * 1)(2.0)
+    assert lib.nao_solve_host(8, 1, 0, 0, None, 1, 0, w1, 4.0, 1e-3, 1, ctypes.byref(mu), 1, 1, 1, 1 << 30, None) == -5
+    assert lib.nao_solve_host(8, 1, 0, 1, 1, 1, 0, w1, 4.0, 1e-3, 1, ctypes.byref(mu), 1, 1, 1, 1 << 30, None) == -4      # S_FACTORED
+    assert lib.nao_solve_host(8, 1, 0, 0, 1, 1, 0, w1, 4.0, 1e-3, 1, ctypes.byref(mu), 1, 1, 1, 64, None) == 1           # workspace
     lib.nao_set_lowdin_threshold.argtypes = [ctypes.c_double]
     assert lib.nao_set_lowdin_threshold(-1e-3) == -1 and lib.nao_set_lowdin_threshold(1.0) == -1
     assert lib.nao_set_lowdin_threshold(1e-8) == 0 and lib.nao_set_lowdin_threshold(0.0) == 0

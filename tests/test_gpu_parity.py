@@ -636,3 +636,29 @@ def test_default_reduction_at_the_switch_over_size(nao):
     chain = np.diag(np.full(n - 1, -1.0), 1) + np.diag(np.full(n - 1, -1.0), -1)
     E, Z, info = nao.heev(to_dev(chain[None]))
     assert np.abs(E.cpu().numpy()[0] - np.sort(-2.0 * np.cos(np.arange(1, n + 1) * np.pi / (n + 1)))).max() <= 1e-12
+
+
+@pytest.mark.parametrize("idx,nat", [(0, None), (1, 6), (2, 8), (3, 4)])
+def test_solve_host_matches_the_separate_calls_and_the_oracle(nao, idx, nat):
+    """nao_solve_host (host buffers in and out, H copied on a second stream while S is factored, D returned item by item)
+    against the oracle and against the three separate calls on device buffers."""
+    prob = make_config(idx, nat=nat)
+    ref = oracle.solve_problem(prob)
+    flags = nao.NAO_NC_BLOCK_S if prob.nc_block_s else 0
+    Hh = torch.from_numpy(prob.H).pin_memory()
+    S_np = prob.S
+    if idx == 2:
+        S_np = np.ascontiguousarray(prob.S[:1])          # the spin channels share one overlap matrix
+    Sh = torch.from_numpy(S_np.copy()).pin_memory()
+    for rep in range(2):                                  # second call reuses the internal stream and events
+        r = nao.solve_host(Hh, Sh, prob.weights, prob.n_electrons, prob.kT, flags=flags)
+        assert int(r["info"].abs().max()) == 0
+        got = dict(e=r["E"].numpy(), mu=r["mu"], D=np.swapaxes(r["D"].numpy(), -1, -2))
+        assert np.abs(got["e"] - ref["e"]).max() <= TOL_E
+        assert abs(got["mu"] - ref["mu"]) <= TOL_MU
+        for b in range(prob.batch):
+            assert np.abs(got["D"][b] - ref["D"][b]).max() <= TOL_D
+    sep = run_path(nao, prob)
+    assert np.abs(got["e"] - sep["e"]).max() <= 1e-12
+    for b in range(prob.batch):
+        assert np.abs(got["D"][b] - sep["D"][b]).max() <= 1e-12
