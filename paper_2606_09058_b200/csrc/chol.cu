@@ -11,6 +11,7 @@
 // V = U s^{-1/2} and V^H H V / V C' products.
 #include "nao_internal.cuh"
 #include "scalar.cuh"
+#include <algorithm>
 
 namespace nao {
 
@@ -113,10 +114,23 @@ static int leaf(int nb, int off, int batch, void *S, long lds, long sS, void *W,
 struct CholCtx {
     int dtype, batch; size_t es;
     char *S; long lds, sS; char *W; long ldw, sW; char *T; long ldt, sT; int *info; cudaStream_t st;
+    void *scratch; size_t scratch_elems; int nsm;       // split-K partial sums of the mid-level products (optional)
     void *s(int i, int j) const { return S + ((size_t)i + (size_t)j * lds) * es; }
     void *w(int i, int j) const { return W + ((size_t)i + (size_t)j * ldw) * es; }
     void *t(int i, int j) const { return T + ((size_t)i + (size_t)j * ldt) * es; }
 };
+
+// A product of the recursion.  Mid-level nodes have few output tiles and a long k: with scratch they are split along k so
+// that the launch covers the SMs (n = 6656: the 16 products of order 832 take 185 us each on 49 CTAs).
+static int chol_gemm(const CholCtx &c, const GemmDesc &d) {
+    const long tiles = (long)ceil_div(d.m, 128) * ceil_div(d.n, c.dtype == NAO_COMPLEX ? 64 : 128) * c.batch;
+    if (c.scratch && d.cmode == 0 && d.beta == 0.0 && d.k >= 256 && 2 * tiles <= c.nsm) {
+        int ks = (int)std::min<long>(std::min<long>(c.nsm / tiles, d.k / 128), 16);
+        while (ks >= 2 && (size_t)ks * d.m * d.n * c.batch > c.scratch_elems) --ks;
+        if (ks >= 2) return gemm_splitk(c.dtype, d, c.batch, ks, c.scratch, c.st);
+    }
+    return gemm_launch(c.dtype, d, c.batch, c.st);
+}
 
 static int rec(const CholCtx &c, int off, int n) {
     int rc;
@@ -131,7 +145,7 @@ static int rec(const CholCtx &c, int off, int n) {
     // T21 = S21 * W11^H
     GemmDesc d = gemm_desc(OP_N, OP_C, n2, n1, n1, 1.0, c.s(o2, off), c.lds, c.w(off, off), c.ldw, 0.0, c.t(o2, off), c.ldt);
     d.sA = c.sS; d.sB = c.sW; d.sC = c.sT; d.maskB = MASK_LOWER;
-    if ((rc = gemm_launch(c.dtype, d, c.batch, c.st))) return rc;
+    if ((rc = chol_gemm(c, d))) return rc;
     if ((rc = copy_matrix(c.dtype, n2, n1, c.t(o2, off), c.ldt, c.sT, c.s(o2, off), c.lds, c.sS, c.batch, 0, c.st))) return rc;
     // S22 -= L21 L21^H  (lower tiles)
     d = gemm_desc(OP_N, OP_C, n2, n2, n1, -1.0, c.s(o2, off), c.lds, c.s(o2, off), c.lds, 1.0, c.s(o2, o2), c.lds);
@@ -141,16 +155,19 @@ static int rec(const CholCtx &c, int off, int n) {
     // T21 = L21 * W11
     d = gemm_desc(OP_N, OP_N, n2, n1, n1, 1.0, c.s(o2, off), c.lds, c.w(off, off), c.ldw, 0.0, c.t(o2, off), c.ldt);
     d.sA = c.sS; d.sB = c.sW; d.sC = c.sT; d.maskB = MASK_LOWER;
-    if ((rc = gemm_launch(c.dtype, d, c.batch, c.st))) return rc;
+    if ((rc = chol_gemm(c, d))) return rc;
     // W21 = -W22 * T21
     d = gemm_desc(OP_N, OP_N, n2, n1, n2, -1.0, c.w(o2, o2), c.ldw, c.t(o2, off), c.ldt, 0.0, c.w(o2, off), c.ldw);
     d.sA = c.sW; d.sB = c.sT; d.sC = c.sW; d.maskA = MASK_LOWER;
-    return gemm_launch(c.dtype, d, c.batch, c.st);
+    return chol_gemm(c, d);
 }
 
 int potrf_trtri(int dtype, int n, int batch, void *S, long lds, long sS, void *W, long ldw, long sW, void *T, long ldt,
-                long sT, int *d_info, cudaStream_t st) {
-    CholCtx c{dtype, batch, esize(dtype), (char *)S, lds, sS, (char *)W, ldw, sW, (char *)T, ldt, sT, d_info, st};
+                long sT, int *d_info, cudaStream_t st, void *scratch, size_t scratch_bytes) {
+    int nsm = 148, dev = 0;
+    cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+    CholCtx c{dtype, batch, esize(dtype), (char *)S, lds, sS, (char *)W, ldw, sW, (char *)T, ldt, sT, d_info, st,
+              scratch, scratch ? scratch_bytes / esize(dtype) : 0, nsm};
     // W's strict upper triangle must read as zero: leaves write their own blocks, the rest is cleared here
     for (int b = 0; b < batch; ++b) {
         // clear column by column only if ldw != n; the common case is a dense n x n buffer

@@ -217,7 +217,7 @@ static int geneig_impl(int n, int batch, int dtype, unsigned flags, int nvec, co
         }
     } else if (!(flags & NAO_S_FACTORED)) {
         // with a shared S the (single) status goes to d_info[0]
-        if ((rc = potrf_trtri(p.sdtype, nS, p.nitemsS, dS, lds, strideS, W, nS, sW, X, nS, sW, d_info, st))) return rc;
+        if ((rc = potrf_trtri(p.sdtype, nS, p.nitemsS, dS, lds, strideS, W, nS, sW, X, nS, sW, d_info, st, A, (size_t)batch * n * n * es))) return rc;
         if ((rc = pack_linv(p.sdtype, nS, dS, lds, strideS, W, nS, sW, p.nitemsS, st))) return rc;
     } else {
         if ((rc = unpack_linv(p.sdtype, nS, dS, lds, strideS, W, nS, sW, p.nitemsS, st))) return rc;

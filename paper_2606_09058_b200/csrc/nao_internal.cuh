@@ -114,7 +114,7 @@ int pack_linv(int dtype, int n, void *S, long lds, long sS, const void *W, long 
 // ---------------------------------------------------------------------------------------------------------
 // chol.cu: S -> L (in S lower), W <- L^{-1}; T = n*n scratch.  info[b] = 0 or failing pivot (1-based)
 int potrf_trtri(int dtype, int n, int batch, void *S, long lds, long sS, void *W, long ldw, long sW, void *T,
-                long ldt, long sT, int *d_info, cudaStream_t st);
+                long ldt, long sT, int *d_info, cudaStream_t st, void *scratch = nullptr, size_t scratch_bytes = 0);
 
 // trd1.cu: one-stage Householder tridiagonalisation of the lower triangle of A (n x n); reflectors left below the
 // first sub-diagonal of A (LAPACK xHETRD lower convention), d[n], e[n-1] real, tau[n-1].
