@@ -286,14 +286,14 @@ def main():
     except Exception as exc:
         partial = {"error": str(exc)}
 
-    # ---- fused call (nao_scf_step): the step takes the number of vectors from its own Fermi search; two-stage reduction
+    # ---- fused call (nao_scf_step): the step takes the number of vectors from its own Fermi search and picks the reduction
+    #      itself (two-stage from order 1536 on, real or complex)
     fused = None
     try:
         if big:
             raise RuntimeError("skipped: the comparison run needs a second workspace (> 40 GB)")
         res = {}
-        for name, f4, fresh in (("first_step", flags | nao.NAO_TRD_TWO_STAGE, True),
-                                ("later_step", flags | nao.NAO_TRD_TWO_STAGE | nao.NAO_S_FACTORED, False)):
+        for name, f4, fresh in (("first_step", flags, True), ("later_step", flags | nao.NAO_S_FACTORED, False)):
             def step4():
                 if fresh:
                     S.copy_(S0)
