@@ -662,3 +662,30 @@ def test_solve_host_matches_the_separate_calls_and_the_oracle(nao, idx, nat):
     assert np.abs(got["e"] - sep["e"]).max() <= 1e-12
     for b in range(prob.batch):
         assert np.abs(got["D"][b] - sep["D"][b]).max() <= 1e-12
+
+
+def test_config1_full_size_sampled_items(nao):
+    """BASELINE config 1 at full size (64 atoms: n = 832 complex, 8 k-points x 2 spins = 16 items in one batched call, the
+    launch configuration `bench.py --workload c1` times).  The Jacobi oracle needs seconds per item, so four sampled items are
+    solved by it: their eigenvalues, and for two of them the density matrix (oracle eigenvectors, occupations from the shared
+    Fermi level), are compared element by element; mu is checked by the oracle's Fermi solver on all 16 x 832 levels; every
+    item is checked through the invariants of the definition."""
+    prob = make_config(1)
+    assert prob.n == 832 and prob.batch == 16 and prob.is_complex
+    got = run_path(nao, prob)
+    mu_ref, f_ref = oracle.fermi(got["e"], prob.weights, prob.n_electrons, prob.kT)
+    assert abs(got["mu"] - mu_ref) <= TOL_MU
+    assert np.abs(got["f"] - f_ref).max() <= 1e-9
+    ne = 0.0
+    for b in range(prob.batch):
+        Cb, Sb, Hb = got["C"][b], prob.S_full(b), prob.H_full(b)
+        assert np.abs(Cb.conj().T @ (Sb @ Cb) - np.eye(prob.n)).max() <= TOL_ORTH
+        assert np.abs(Hb @ Cb - (Sb @ Cb) * got["e"][b]).max() <= 1e-10
+        ne += prob.weights[b] * np.sum(got["D"][b] * Sb.T).real
+    assert abs(ne - prob.n_electrons) <= 1e-8
+    assert np.abs(got["e"][:8] - got["e"][7::-1]).max() <= 1e-10          # e(k) = e(-k)
+    for b in (0, 3, 9, 12):
+        e_or, C_or, _ = oracle.geneig(prob.H_full(b), prob.S_full(b))
+        assert np.abs(got["e"][b] - e_or).max() <= TOL_E
+        if b in (3, 12):
+            assert np.abs(got["D"][b] - oracle.density(C_or, f_ref[b])).max() <= TOL_D
