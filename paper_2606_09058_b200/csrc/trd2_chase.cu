@@ -125,17 +125,24 @@ __global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
     // D <- H^H D H for the L x L block in sD with v = s_vn, tau = s_tau_n  (u = D v, gamma = v^H u,
     // w = tau u - 1/2 |tau|^2 gamma v,  D -= w v^H + v w^H)
     auto two_sided = [&](int L) {
-        {
-            T s = O::zero();
-            if (iq < L) for (int cc = qq; cc < L; cc += 4) s = O::fma(sD[cc * LDS + iq], s_vn[cc], s);
-            s_part[qq][iq] = s;
+        {   // (block and vector are zero beyond L: full-range loops with compile-time trip counts, two accumulators)
+            T s0 = O::zero(), s1 = O::zero();
+#pragma unroll
+            for (int t = 0; t < b / 8; ++t) {
+                const int c0_ = qq + 8 * t, c1_ = c0_ + 4;
+                s0 = O::fma(sD[c0_ * LDS + iq], s_vn[c0_], s0);
+                s1 = O::fma(sD[c1_ * LDS + iq], s_vn[c1_], s1);
+            }
+            s_part[qq][iq] = O::add(s0, s1);
         }
         __syncthreads();
-        if (tid < b) s_w[tid] = tid < L ? O::add(O::add(s_part[0][tid], s_part[1][tid]), O::add(s_part[2][tid], s_part[3][tid])) : O::zero();
-        __syncthreads();
         if (warp == 0) {
-            double gsum = 0.0;
-            for (int i = tid; i < L; i += 32) gsum += O::real(O::conj_mul(s_vn[i], s_w[i]));
+            // u = D v (two elements per lane) and gamma = v^H u in one go
+            const int i0_ = tid, i1_ = tid + 32;
+            const T u0 = i0_ < L ? O::add(O::add(s_part[0][i0_], s_part[1][i0_]), O::add(s_part[2][i0_], s_part[3][i0_])) : O::zero();
+            const T u1 = i1_ < L ? O::add(O::add(s_part[0][i1_], s_part[1][i1_]), O::add(s_part[2][i1_], s_part[3][i1_])) : O::zero();
+            s_w[i0_] = u0; s_w[i1_] = u1;
+            double gsum = O::real(O::conj_mul(s_vn[i0_], u0)) + O::real(O::conj_mul(s_vn[i1_], u1));
             gsum = warp_sum(gsum);
             if (tid == 0) s_gamma = gsum;
         }
@@ -145,17 +152,22 @@ __global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
             const double f = -0.5 * O::abs2(tau) * s_gamma;
             T wv = O::zero();
             if (tid < L) wv = O::add(O::mul(tau, s_w[tid]), O::scale(s_vn[tid], f));
-            __syncthreads();
-            if (tid < b) s_w[tid] = wv;
+            if (tid < b) s_w[tid] = wv;              // every thread rewrites only the element it has just read
         }
         __syncthreads();
-        if (iq < L)
-            for (int cc = qq; cc < L; cc += 4) {
-                T a = sD[cc * LDS + iq];
-                a = O::sub(a, O::add(O::mul_conj(s_w[iq], s_vn[cc]), O::mul_conj(s_vn[iq], s_w[cc])));
-                if (cc == iq) a = O::from_real(O::real(a));
-                sD[cc * LDS + iq] = a;
+        if (iq < L) {
+            const T wi = s_w[iq], vi = s_vn[iq];
+#pragma unroll
+            for (int t = 0; t < b / 4; ++t) {
+                const int cc = qq + 4 * t;
+                if (cc < L) {
+                    T a = sD[cc * LDS + iq];
+                    a = O::sub(a, O::add(O::mul_conj(wi, s_vn[cc]), O::mul_conj(vi, s_w[cc])));
+                    if (cc == iq) a = O::from_real(O::real(a));
+                    sD[cc * LDS + iq] = a;
+                }
             }
+        }
         __syncthreads();
     };
     // diagonal block rows/cols [g0, g0+L): load (Hermitian completion) / store (lower part)
@@ -217,13 +229,26 @@ __global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
     for (int s = c; s < n - 1; s += P) {
         // ------------------------------------------------ step 0
         int r0 = s + 1, Lp = min(s + b, n - 1) - r0 + 1;
+        // Column s and the diagonal block are final after the predecessor's step 0 except for their last row (global row
+        // s + b), which its step 1 writes: everything else is read as soon as the counter shows 1, the last row after 2.
+        const bool late0 = (Lp == b);
         if (s > 0) {
-            if (tid == 0) { while (ld_acquire(prog + s - 1) < 2) { } }
+            if (tid == 0) { while (ld_acquire(prog + s - 1) < 1) { } }
             __syncthreads();
         }
+        if (tid < b) s_vn[tid] = (tid < Lp && !(late0 && tid == b - 1)) ? ldcg(AB + (1 + tid) + (long)s * ld) : O::zero();
+        load_D(r0, late0 ? b - 1 : Lp);
+        if (late0) {
+            if (s > 0 && tid == 0) { while (ld_acquire(prog + s - 1) < 2) { } }
+            __syncthreads();             // (also orders the zero fill of row b-1 above before the late values below)
+        }
+        if (late0) {
+            if (tid < b) {
+                const T v = ldcg(AB + (b - 1 - tid) + (long)(r0 + tid) * ld);          // D(b-1, tid)
+                sD[tid * LDS + b - 1] = v; sD[(b - 1) * LDS + tid] = O::conj(v);
+            } else if (tid == b) s_vn[b - 1] = ldcg(AB + b + (long)s * ld);
+        }
         if constexpr (PF) prefetch(s, 1);
-        if (tid < b) s_vn[tid] = tid < Lp ? ldcg(AB + (1 + tid) + (long)s * ld) : O::zero();
-        load_D(r0, Lp);
         __syncthreads();
         if (warp == 0) house_warp<T>(s_vn, Lp, &s_tau_n, &s_beta);
         __syncthreads();
