@@ -269,7 +269,7 @@ __global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
             if (q0 > n - 1) break;
             const int Lq = min(s + (k + 1) * b, n - 1) - q0 + 1;
             CH_T(0);
-            if (s > 0) {
+            if (PF && s > 0) {
                 if (tid == 0) { while (ld_acquire(prog + s - 1) < k + 2) { } }
                 __syncthreads();
             }
@@ -299,21 +299,41 @@ __global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
                     else { sD[cc * LDS + b - 1] = late; sD[(b - 1) * LDS + cc] = O::conj(late); }
                 }           // (short last block: row b-1 does not exist; column b-1 of D was zero-filled by the prefetch)
             } else
-            {   // both blocks in ONE L2 round trip: all 2 x 16 loads of a thread are issued before the first shared-memory store
+            {   // No second buffer (complex).  Everything except the last row of the two blocks is final since the predecessor
+                // finished step k+1 -- known since the wait of the previous step -- so those loads are issued BEFORE waiting for
+                // its step k+2; the last row follows with one short round trip.  All loads of a thread are in flight at once.
                 T bo[b * b / CH_NT], bd[b * b / CH_NT];
+                const bool lateK = (Lq == b);
 #pragma unroll
                 for (int it = 0; it < b * b / CH_NT; ++it) {
                     const int e = tid + it * CH_NT, i = e & (b - 1), cc = e >> 6;
                     T vo = O::zero(), vd = O::zero();
-                    if (i < Lq && cc < Lp) vo = ldcg(AB + (q0 + i - r0 - cc) + (long)(r0 + cc) * ld);
-                    if (i < Lq && cc < Lq) vd = (i >= cc) ? ldcg(AB + (i - cc) + (long)(q0 + cc) * ld) : ldcg(AB + (cc - i) + (long)(q0 + i) * ld);
+                    if (i < Lq && cc < Lp && !(lateK && i == b - 1)) vo = ldcg(AB + (q0 + i - r0 - cc) + (long)(r0 + cc) * ld);
+                    if (i < Lq && cc < Lq && !(lateK && (i == b - 1 || cc == b - 1)))
+                        vd = (i >= cc) ? ldcg(AB + (i - cc) + (long)(q0 + cc) * ld) : ldcg(AB + (cc - i) + (long)(q0 + i) * ld);
                     bo[it] = vo; bd[it] = vd;
+                }
+                if (s > 0) {
+                    if (tid == 0) { while (ld_acquire(prog + s - 1) < k + 2) { } }
+                    __syncthreads();
+                }
+                T late = O::zero();
+                const bool has_late = lateK && tid < 2 * b;
+                if (has_late) {
+                    const int cc = tid & (b - 1);
+                    late = tid < b ? ldcg(AB + (q0 + b - 1 - r0 - cc) + (long)(r0 + cc) * ld)
+                                   : ldcg(AB + (b - 1 - cc) + (long)(q0 + cc) * ld);
                 }
 #pragma unroll
                 for (int it = 0; it < b * b / CH_NT; ++it) {
                     const int e = tid + it * CH_NT, i = e & (b - 1), cc = e >> 6;
-                    sO[cc * LDS + i] = bo[it];
-                    sD[cc * LDS + i] = (i >= cc) ? bd[it] : O::conj(bd[it]);
+                    if (!(lateK && i == b - 1)) sO[cc * LDS + i] = bo[it];
+                    if (!(lateK && (i == b - 1 || cc == b - 1))) sD[cc * LDS + i] = (i >= cc) ? bd[it] : O::conj(bd[it]);
+                }
+                if (has_late) {
+                    const int cc = tid & (b - 1);
+                    if (tid < b) sO[cc * LDS + b - 1] = late;
+                    else { sD[cc * LDS + b - 1] = late; sD[(b - 1) * LDS + cc] = O::conj(late); }
                 }
             }
             __syncthreads();
