@@ -106,7 +106,7 @@ int nao_geneig(int n, int batch, int dtype, unsigned flags,
  * vectors equals the one of the full solve as long as every state with f >= 1e-17 lies below n_vec -- check with
  * nao_occupied_count after nao_fermi_mu (an SCF loop takes n_vec from the previous step plus a margin).
  * Combine with NAO_TRD_TWO_STAGE: with few vectors the second back-transformation of the two-stage reduction is cheap and
- * that path is the faster one (config 2: 274 vs 400 ms, config 3: 0.84 vs 1.12 s per step on B200).
+ * that path is the faster one (config 2: 264 vs 400 ms, config 3: 0.83 vs 1.12 s per step on B200).
  *   1..4 as nao_geneig;  5 n_vec in 1..n;  the remaining arguments as nao_geneig arguments 5..18.
  * Negative return values count the arguments of THIS signature.
  */
