@@ -125,7 +125,7 @@ int nao_geneig_partial(int n, int batch, int dtype, unsigned flags, int n_vec,
  * Arguments as in those three calls (h_weight, h_mu, h_nvec are HOST pointers); dwork needs nao_scf_step_workspace bytes.
  * The call synchronises the stream twice (Fermi level, vector count).
  * Without NAO_TRD_ONE_STAGE / NAO_TRD_TWO_STAGE the fused step takes the two-stage reduction from order 1536 on for real AND
- * complex matrices (few vectors are back-transformed, which favours it: config 3 844 vs 1124 ms).
+ * complex matrices (few vectors are back-transformed, which favours it: config 3 831 vs 1141 ms).
  */
 int nao_scf_step_workspace(int n, int batch, int dtype, unsigned flags, size_t *bytes);
 int nao_scf_step(int n, int batch, int dtype, unsigned flags,

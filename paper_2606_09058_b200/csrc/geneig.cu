@@ -334,7 +334,7 @@ extern "C" int nao_density_matrix(int n, int batch, int dtype, const void *dC, l
                                   long ldd, long strideD, void *dwork, size_t work_bytes, void *cuda_stream);
 
 // The fused step back-transforms only the occupied vectors, which favours the two-stage reduction for complex matrices as
-// well (config 3: 844 vs 1124 ms per step); below order 1536 the one-stage path stays ahead (config 1: 34 vs 40 ms).
+// well (config 3: 831 vs 1141 ms per step); below order 1536 the one-stage path stays ahead (config 1: 34 vs 40 ms).
 static unsigned scf_step_flags(int n, unsigned flags) {
     if (!(flags & (NAO_TRD_ONE_STAGE | NAO_TRD_TWO_STAGE)) && n >= nao::TWO_STAGE_MIN_N_REAL) flags |= NAO_TRD_TWO_STAGE;
     return flags;
