@@ -93,9 +93,97 @@ def oracle_sample(workload, budget_atoms=None):
     dt = time.time() - t0
     scale = (full_nat / float(nat)) ** 3
     cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
-    return dict(value=dt * scale, unit="s", cores=cores, kind="oracle",
+    return dict(value=dt * scale, unit="s", cores=cores, kind="oracle", extrapolated=scale != 1.0, measured_s=dt,
                 sample="%s recipe at %d atoms (n=%d, batch %d): %.2f s measured, x%.0f by the N^3 law to %d atoms"
                        % (workload, nat, prob.n, prob.batch, dt, scale, full_nat))
+
+
+def cpu_library_time(workload):
+    """scipy.linalg.eigh(H, S) (LAPACK dsygvd/zhegvd on all host cores) on the FIRST item of the workload: a practical CPU
+    time beside the (deliberately plain) Jacobi oracle (SURVEY.md 8d item ii).  An independent library, not the oracle and
+    not the product path; only timed where it ends within about a minute (configs 0-2)."""
+    import scipy.linalg as sl
+    from paper_2606_09058_b200.synth import make_config
+    idx = WORKLOADS[workload]["idx"]
+    if idx > 2:
+        return None
+    prob = make_config(idx)
+    t0 = time.time()
+    sl.eigh(prob.H_full(0), prob.S_full(0), driver="gvd")
+    dt = time.time() - t0
+    return dict(value=dt * prob.batch, unit="s", cores=os.cpu_count(), kind="scipy.linalg.eigh (LAPACK gvd), eigenpairs only",
+                sample="item 0 of %d measured: %.2f s; value = x%d items (no Fermi level, no density matrix)" % (prob.batch, dt, prob.batch))
+
+
+def read_traffic(kernel, workload):
+    """DRAM bytes per launch of `kernel` from the committed ncu capture of this build (profiles/r02_traffic.csv: one row per
+    kernel and workload, written from `ncu --metrics dram__bytes_read.sum,dram__bytes_write.sum` over one whole step)."""
+    import csv
+    try:
+        with open(os.path.join(ROOT, "profiles", "r02_traffic.csv")) as fh:
+            for r in csv.DictReader(fh):
+                if r["kernel"] == kernel and r["workload"] == workload:
+                    return float(r["dram_bytes_total"]) / max(1, int(r["launches"])), r["source"]
+    except Exception:
+        pass
+    return None, None
+
+
+def side_record(nao, torch, workload, dev, hbm_peak, dmma_meas, steps=3, warmup=2):
+    """A second workload timed in the same run (device-resident inputs, CUDA events, `warmup` + `steps` full steps, then one
+    step with the library's event timers): ms per step, phases, and the rooflines of hetrd_panel_kernel / gemm_kernel."""
+    from paper_2606_09058_b200.synth import make_config
+    prob = make_config(WORKLOADS[workload]["idx"])
+    flags = nao.NAO_NC_BLOCK_S if prob.nc_block_s else 0
+    dt = nao.NAO_COMPLEX if prob.is_complex else nao.NAO_REAL
+    H = torch.from_numpy(prob.H).to(dev); S0 = torch.from_numpy(prob.S).to(dev); S = torch.empty_like(S0)
+    work = torch.empty(nao.geneig_workspace(prob.n, prob.batch, dt, flags) + 256, dtype=torch.uint8, device=dev)
+    Dbuf = torch.empty_like(H)
+    weights = [float(x) for x in prob.weights]
+    in_bytes = H.numel() * H.element_size() + S0.numel() * S0.element_size()
+    flush = None if in_bytes > (256 << 20) else torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+
+    def step():
+        S.copy_(S0)
+        E, C, info = nao.geneig(H, S, flags=flags, work=work)
+        mu, F = nao.fermi_mu(E, weights, prob.n_electrons, prob.kT)
+        nao.density_matrix(C, F, out=Dbuf)
+        return info, mu
+    for _ in range(warmup):
+        info, mu = step()
+    torch.cuda.synchronize()
+    assert int(info.abs().max()) == 0
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = nao.launch_count()
+    tot = 0.0
+    for _ in range(steps):
+        if flush is not None:
+            flush.zero_()
+        ev0.record(); step(); ev1.record(); torch.cuda.synchronize()
+        tot += ev0.elapsed_time(ev1)
+    ms = tot / steps
+    launches = (nao.launch_count() - l0) // steps
+    nao.profile_enable(True); step(); torch.cuda.synchronize()
+    phases = nao.profile_read(); kp = nao.profile_kernel(0); kg = nao.profile_kernel(1)
+    nao.profile_enable(False)
+    fl = useful_flops(prob)
+    rec = {"workload": WORKLOADS[workload]["desc"], "value": ms * 1e-3, "unit": "s", "ms_per_step": ms, "steps": steps, "warmup": warmup,
+           "n": prob.n, "batch": prob.batch, "gpu_launches_per_step": int(launches), "useful_tflops": fl / (ms * 1e-3) / 1e12,
+           "l2_policy": "inputs larger than L2" if flush is None else "L2 flushed between timed steps (256 MB write)",
+           "phases_ms": {k: round(v, 3) for k, v in phases.items()}, "check": {"mu": mu}}
+    if kp["launches"] > 0 and kp["ms"] > 0:
+        ach = kp["work"] / (kp["ms"] * 1e-3) / 1e9
+        tr, src = read_traffic("hetrd_panel_kernel", workload)
+        rec["roofline"] = {"kernel": kp["name"], "bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
+                           "traffic": tr, "traffic_source": src, "kernel_ms_per_step": kp["ms"], "launches_per_step": kp["launches"],
+                           "algorithmic_bytes_per_launch": kp["work"] / kp["launches"]}
+    if kg["ms"] > 0:
+        tf = kg["work"] / (kg["ms"] * 1e-3) / 1e12
+        rec["roofline_gemm"] = {"kernel": kg["name"], "bound": "tensor", "achieved": tf, "peak": dmma_meas, "unit": "TFLOP/s",
+                                "frac": tf / dmma_meas, "kernel_ms_per_step": kg["ms"], "launches_timed": kg["launches"]}
+    del H, S, S0, work, Dbuf
+    torch.cuda.empty_cache()
+    return rec
 
 
 def run_reference(args):
@@ -116,6 +204,9 @@ def run_reference(args):
             "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": v * 1e3,
             "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": WORKLOADS[args.workload]["desc"], "parallelism": "host cores (oracle)"},
+            "extrapolated": bool(cb.get("extrapolated")),
+            "note": "the Jacobi oracle timed on a reduced-size replica of the workload and scaled by its N^3 law: context, "
+                    "not a same-config measurement",
             "cpu_baseline": cb, "e2e": {"value": v, "unit": "s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
@@ -129,6 +220,11 @@ def main():
     ap.add_argument("--workload", default="c2", choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-side", action="store_true", help="skip the c3 / c1 side records of the default (c2) run")
+    ap.add_argument("--reduction", default="default", choices=["default", "one_stage", "two_stage"],
+                    help="force the tridiagonalisation path of the timed step (NAO_TRD_ONE_STAGE / NAO_TRD_TWO_STAGE)")
+    ap.add_argument("--timed-only", action="store_true",
+                    help="warm-up + timed steps only, minimal JSON line (the command the ncu launch lists are taken from)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -154,6 +250,7 @@ def main():
     from paper_2606_09058_b200.replicas import replica_seed
     prob = make_config(WORKLOADS[args.workload]["idx"], seed=replica_seed(rank))       # replicas: each rank its own seed
     flags = nao.NAO_NC_BLOCK_S if prob.nc_block_s else 0
+    flags |= {"default": 0, "one_stage": nao.NAO_TRD_ONE_STAGE, "two_stage": nao.NAO_TRD_TWO_STAGE}[args.reduction]
     dt = nao.NAO_COMPLEX if prob.is_complex else nao.NAO_REAL
     # host (pinned) and device copies
     # the spin channels of a collinear Gamma-point calculation share one overlap matrix: it is passed once (strideS = 0)
@@ -214,6 +311,15 @@ def main():
         ms = tot / args.steps
     launches = (nao.launch_count() - l0) // args.steps
     clocks = sampler.stop()
+    if args.timed_only:
+        if rank == 0:
+            print(json.dumps({"metric": "s per SCF eigensolve+density matrix", "value": ms * 1e-3, "unit": "s", "ms_per_step": ms,
+                              "steps": args.steps, "warmup": W, "timed_only": True, "reduction": args.reduction,
+                              "config": {"workload": WORKLOADS[args.workload]["desc"]}, "gpu_launches": int(launches) * args.steps,
+                              "clocks": clocks}))
+        if dist is not None:
+            dist.destroy_process_group()
+        return
 
     # ---- one more step with the library's event timers on: phase boundaries and per-launch timers of the two
     #      kernel classes (slot 0 = hetrd_panel_kernel with its algorithmic HBM bytes, slot 1 = gemm_kernel with flops)
@@ -225,7 +331,7 @@ def main():
     kgemm = nao.profile_kernel(1)
     nao.profile_enable(False)
     prof_steps = 1
-    # which reduction the library's default took (real n >= 6144: two-stage; otherwise one-stage)
+    # which reduction the library's default took (real n >= 1536: two-stage; otherwise one-stage)
     default_path = "two_stage" if phases.get("band_to_tridiagonal", 0.0) > 0.05 else "one_stage"
     other_path = "one_stage" if default_path == "two_stage" else "two_stage"
 
@@ -363,17 +469,10 @@ def main():
         fl = useful_flops(prob)
         gemm_tf = kgemm["work"] / (kgemm["ms"] * 1e-3) / 1e12 if kgemm["ms"] > 0 else 0.0
         dmma_meas = nao.dmma_peak()          # register-resident DMMA loop, measured in this run
-        # DRAM traffic of the dominant kernel: ratio (dram bytes / algorithmic bytes) of the committed ncu --set full
-        # capture (profiles/r01_traffic.csv) times this run's algorithmic bytes per launch
-        traffic, traffic_src = None, None
-        try:
-            import csv
-            with open(os.path.join(ROOT, "profiles", "r01_traffic.csv")) as fh:
-                tj = [r for r in csv.DictReader(fh) if r["kernel"] == "hetrd_panel_kernel"][0]
-            traffic = float(tj["dram_bytes_per_algorithmic_byte"]) * panel_bytes / max(1, kpanel["launches"] // prof_steps)
-            traffic_src = tj["source"]
-        except Exception:
-            pass
+        # DRAM traffic per launch from the committed ncu capture of this build (profiles/r02_traffic.csv)
+        hetrd_wl = args.workload if hetrd_in_default else args.workload + "_one_stage"
+        traffic, traffic_src = read_traffic("hetrd_panel_kernel", hetrd_wl)
+        gemm_traffic, gemm_traffic_src = read_traffic("gemm_kernel", args.workload)
         line = {
             "metric": "s per SCF eigensolve+density matrix", "value": ms * 1e-3, "unit": "s", "n_gpus": world,
             "steps": args.steps, "warmup": W, "ms_per_step": ms, "higher_is_better": False, "scaling": "weak",
@@ -405,7 +504,7 @@ def main():
                    "algorithmic_bytes_per_launch": panel_bytes / max(1, kpanel["launches"] // prof_steps),
                    "measured_in": "the timed (default) step" if hetrd_in_default else "the one-stage comparison step"}
         r_gemm = {"kernel": kgemm["name"], "bound": "tensor", "achieved": gemm_tf, "peak": dmma_meas,
-                  "unit": "TFLOP/s", "frac": gemm_tf / dmma_meas, "traffic": None,
+                  "unit": "TFLOP/s", "frac": gemm_tf / dmma_meas, "traffic": gemm_traffic, "traffic_source": gemm_traffic_src,
                   "peak_source": "measured in this run: register-resident DMMA.8x8x4 loop (nao_dmma_peak); derived "
                                  "148 SMs x 128 flop/clk x 1.965 GHz = 37.2; cuBLAS DGEMM reaches 35.6",
                   "kernel_ms_per_step": kgemm["ms"] / prof_steps, "launches_timed": kgemm["launches"],
@@ -416,8 +515,19 @@ def main():
             line["roofline"], line["roofline_gemm"] = r_hetrd, r_gemm
         else:
             line["roofline"], line["roofline_hetrd"] = r_gemm, r_hetrd
-        if not args.no_cpu_baseline:
+        # the other headline workload of BASELINE.json's metric ("N=6656 real, 9984 cplx"), timed in the same run
+        if world == 1 and args.workload == "c2" and not args.no_side:
+            for wl in ("c3", "c1"):
+                try:
+                    line[wl] = side_record(nao, torch, wl, dev, hbm_peak, dmma_meas)
+                except Exception as exc:       # reported, never hidden
+                    line[wl] = {"error": str(exc)}
+        if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"] = oracle_sample(args.workload)
+            try:
+                line["cpu_library"] = cpu_library_time(args.workload)
+            except Exception as exc:
+                line["cpu_library"] = {"error": str(exc)}
         print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()

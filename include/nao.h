@@ -17,7 +17,14 @@
  *     is at  base + b*stride + j*ld + i.  dtype NAO_REAL = double, NAO_COMPLEX = interleaved (re,im) doubles.
  *   - The library allocates NO device memory: the caller owns every buffer, the workspace and the stream.
  *     `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Work is enqueued on
- *     that stream; only nao_fermi_mu synchronises it (to hand back *h_mu).
+ *     that stream and the call returns; the only calls that synchronise it are the ones that hand a host scalar
+ *     back: nao_fermi_mu (*h_mu), nao_occupied_count (*h_count), and therefore nao_scf_step and nao_solve_host
+ *     (stated at each).  nao_geneig, nao_geneig_partial, nao_heev, nao_stedc, nao_density_matrix, nao_fold_density
+ *     never block the host (the divide-and-conquer tree is built by a kernel, not copied from the host).
+ *   - Process-wide state: the library keeps per-process settings and caches (nao_set_lowdin_threshold, the profiler,
+ *     kernel attributes, SM count, the copy stream of nao_solve_host, pinned result words) bound to the FIRST device it
+ *     is used on.  Use it from one host thread at a time and on one device per process (one process per GPU is the
+ *     deployment model); the Python binding rejects tensors on any other device.
  *   - Return value: NAO_OK (0); -i if argument number i (1-based) is invalid (checked on the host before any
  *     launch); a positive NAO_ERR_* code for run-time failures.  Numerical outcomes are reported per batch item
  *     in d_info (device int[batch]).

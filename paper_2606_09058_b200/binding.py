@@ -105,9 +105,18 @@ def _dtype_code(t: torch.Tensor) -> int:
     raise TypeError("expected float64 or complex128, got %s" % t.dtype)
 
 
+_DEVICE = None      # the library's per-process state is bound to the first device it is used on (include/nao.h)
+
+
 def _dev(t: torch.Tensor, name: str):
+    global _DEVICE
     if not t.is_cuda:
         raise NaoError("%s must be a CUDA tensor (no CPU path exists)" % name)
+    if _DEVICE is None:
+        _DEVICE = t.device.index
+    if t.device.index != _DEVICE or t.device.index != torch.cuda.current_device():
+        raise NaoError("%s is on cuda:%s; the library is bound to cuda:%s, which must be the current device "
+                       "(one device per process)" % (name, t.device.index, _DEVICE))
     if not t.is_contiguous():
         raise NaoError("%s must be contiguous" % name)
     return t.data_ptr()

@@ -193,8 +193,6 @@ NAO_EXPORT int nao_fermi_mu(int n, int batch, const double *dE, const double *h_
     if (!h_mu) return -7;
     if (!dF) return -8;
     if (!dwork) return -9;
-    double wsum = 0.0;
-    for (int b = 0; b < batch; ++b) { if (!(h_weight[b] > 0.0)) return -4; wsum += h_weight[b] * n; }
-    if (!(n_electrons > 0.0) || !(n_electrons < wsum) || !(kT > 0.0)) return NAO_ERR_ELECTRONS;
+    if (int rc = nao::check_occupation_args(n, batch, h_weight, n_electrons, kT, 4)) return rc;
     return nao::fermi_mu(n, batch, dE, h_weight, n_electrons, kT, h_mu, dF, dwork, (cudaStream_t)cuda_stream);
 }

@@ -340,6 +340,29 @@ static unsigned scf_step_flags(int n, unsigned flags) {
     return flags;
 }
 
+// Host checks of the occupation arguments shared by nao_fermi_mu, nao_scf_step and nao_solve_host (made before any launch):
+// every weight positive (else -arg_weight), 0 < n_electrons < sum_b w_b n and kT > 0 (else NAO_ERR_ELECTRONS).
+int nao::check_occupation_args(int n, int batch, const double *h_weight, double n_electrons, double kT, int arg_weight) {
+    if (!h_weight) return -arg_weight;
+    double wsum = 0.0;
+    for (int b = 0; b < batch; ++b) { if (!(h_weight[b] > 0.0)) return -arg_weight; wsum += h_weight[b] * n; }
+    if (!(n_electrons > 0.0) || !(n_electrons < wsum) || !(kT > 0.0)) return NAO_ERR_ELECTRONS;
+    return NAO_OK;
+}
+
+// argument positions of nao_geneig -> positions of nao_scf_step (negative return codes of the shared implementation)
+static int scf_step_argpos(int rc) {
+    switch (rc) {
+        case -11: return -14;   // dE
+        case -12: return -17;   // dC
+        case -13: return -18;   // ldc
+        case -14: return -19;   // strideC
+        case -15: return -24;   // dwork
+        case -17: return -26;   // d_info
+        default: return rc;     // 1..10 coincide; positive codes pass through
+    }
+}
+
 static int scf_step_workspace_raw(int n, int batch, int dtype, unsigned flags, size_t *bytes) {
     size_t g = 0, f = 0, d = 0;
     int rc;
@@ -366,7 +389,9 @@ NAO_EXPORT int nao_scf_step(int n, int batch, int dtype, unsigned flags, const v
                             int *h_nvec, void *dwork, size_t work_bytes, int *d_info, void *cuda_stream) {
     using namespace nao;
     flags = scf_step_flags(n, flags);
-    if (!h_weight) return -11;
+    if (n < 1) return -1;
+    if (batch < 1) return -2;
+    if (int rc0 = check_occupation_args(n, batch, h_weight, n_electrons, kT, 11)) return rc0;
     if (!h_mu) return -15;
     if (!dF) return -16;
     if (!dD) return -20;
@@ -379,9 +404,9 @@ NAO_EXPORT int nao_scf_step(int n, int batch, int dtype, unsigned flags, const v
     nao_geneig_workspace(n, batch, dtype, flags, &g); nao_fermi_workspace(n, batch, &f); nao_density_workspace(n, batch, dtype, &d);
     char *wg = (char *)dwork, *wf = wg + align_up(g), *wd = wf + align_up(f);
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    // eigenvalues (phase 1); argument errors of the shared prefix are reported with the positions of nao_geneig
+    // eigenvalues (phase 1); argument errors of the shared implementation are renumbered to this signature
     rc = geneig_impl(n, batch, dtype, flags, n, dH, ldh, strideH, dS, lds, strideS, dE, dC, ldc, strideC, wg, g, d_info, cuda_stream, 1);
-    if (rc) return rc;
+    if (rc) return scf_step_argpos(rc);
     if ((rc = fermi_mu(n, batch, dE, h_weight, n_electrons, kT, h_mu, dF, wf, st))) return rc;
     int cnt = 0;
     if ((rc = nao_occupied_count(n, batch, dF, 1e-17, &cnt, cuda_stream))) return rc;
@@ -439,7 +464,7 @@ NAO_EXPORT int nao_solve_host(int n, int batch, int dtype, unsigned flags, const
     if (flags & NAO_S_FACTORED) return -4;              // the factor lives in the device scratch: not kept between calls
     if (!hH) return -5;
     if (!hS) return -6;
-    if (!h_weight) return -8;
+    if (int rc0 = check_occupation_args(n, batch, h_weight, n_electrons, kT, 8)) return rc0;
     if (!hE) return -11;
     if (!h_mu) return -12;
     if (!hD) return -13;

@@ -164,5 +164,7 @@ void prof_kernel_end(int slot, int k, cudaStream_t st);
 // fermi.cu / density
 int fermi_mu(int n, int batch, const double *dE, const double *h_weight, double n_electrons, double kT, double *h_mu,
              double *dF, void *dwork, cudaStream_t st);
+// geneig.cu: host checks of (weights, n_electrons, kT); -arg_weight, NAO_ERR_ELECTRONS or NAO_OK
+int check_occupation_args(int n, int batch, const double *h_weight, double n_electrons, double kT, int arg_weight);
 
 }  // namespace nao

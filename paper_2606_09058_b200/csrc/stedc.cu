@@ -417,6 +417,36 @@ __global__ void dc_final_kernel(DcBuf b, double *Qout, long ldo, long sO, int nc
     for (int c = blockIdx.y; c < ncols; c += gridDim.y) Qo[row + (long)c * ldo] = Q[row + (long)idxq[c] * b.ldq];
 }
 
+// Tree of the divide step, written by the device (mirrors dc_plan): a complete binary tree of `depth` levels in which a
+// node of size s splits into s/2 and s - s/2.  leaf_off[0..2^depth], cuts[i-1] = leaf_off[i] (1 <= i < 2^depth), and the
+// merge nodes level by level, bottom-up (level lv holds 2^(depth-1-lv) nodes).
+__device__ __forceinline__ void dc_descend(int n, int steps, int q, int &off, int &s) {
+    off = 0; s = n;
+    for (int lev = steps - 1; lev >= 0; --lev) {
+        const int h = s / 2;
+        if ((q >> lev) & 1) { off += h; s -= h; } else s = h;
+    }
+}
+__global__ void dc_tree_kernel(int n, int depth, int *leaf_off, int *cuts, DcNode *nodes) {
+    const int nleaves = 1 << depth;
+    for (int q = threadIdx.x; q <= nleaves; q += blockDim.x) {
+        int off = n, s = 0;
+        if (q < nleaves) dc_descend(n, depth, q, off, s);
+        leaf_off[q] = off;
+        if (q >= 1 && q < nleaves) cuts[q - 1] = off;
+    }
+    int base = 0;
+    for (int lv = 0; lv < depth; ++lv) {
+        const int nn = 1 << (depth - 1 - lv);
+        for (int q = threadIdx.x; q < nn; q += blockDim.x) {
+            int off, s;
+            dc_descend(n, depth - 1 - lv, q, off, s);
+            nodes[base + q] = DcNode{off, s / 2, s - s / 2};
+        }
+        base += nn;
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ host driver
 struct DcPlan {
     std::vector<int> leaf_off;                       // nleaves + 1
@@ -493,18 +523,14 @@ int stedc(int n, int batch, double *d, double *e, double *evals, double *Qout, l
         for (auto &nd : p.levels[lv]) { Nmax = max(Nmax, nd.n1 + nd.n2); hmax = max(hmax, max(nd.n1, nd.n2)); }
     };
     if (phase & 1) {
-        // host -> device: tree description (tiny; pageable copy is staged before the call returns)
-        std::vector<int> cuts;
-        for (int i = 1; i < nleaves; ++i) cuts.push_back(p.leaf_off[i]);
-        if (!cuts.empty()) NAO_CUDA_CHECK(cudaMemcpyAsync(w.cuts, cuts.data(), cuts.size() * 4, cudaMemcpyHostToDevice, st));
-        NAO_CUDA_CHECK(cudaMemcpyAsync(w.leaf_off, p.leaf_off.data(), p.leaf_off.size() * 4, cudaMemcpyHostToDevice, st));
-        std::vector<DcNode> flat;
-        for (auto &l : p.levels) flat.insert(flat.end(), l.begin(), l.end());
-        if (!flat.empty()) NAO_CUDA_CHECK(cudaMemcpyAsync(w.nodes, flat.data(), flat.size() * sizeof(DcNode), cudaMemcpyHostToDevice, st));
-        NAO_CUDA_CHECK(cudaStreamSynchronize(st));     // the host vectors above go out of scope at return
+        // tree description (leaf offsets, tear points, merge nodes of every level) built on the device: no host copy, so the
+        // call only enqueues work
+        dc_tree_kernel<<<1, 256, 0, st>>>(n, (int)nlev, w.leaf_off, w.cuts, w.nodes);
+        NAO_LAUNCHED();
+        const int ncuts = nleaves - 1;
 
         NAO_CUDA_CHECK(cudaMemsetAsync(w.b.Q, 0, (size_t)batch * n * n * 8, st));
-        dc_scale_tear_kernel<<<batch, 256, 0, st>>>(w.b, w.cuts, (int)cuts.size());
+        dc_scale_tear_kernel<<<batch, 256, 0, st>>>(w.b, w.cuts, ncuts);
         NAO_LAUNCHED();
         dc_leaf_kernel<<<dim3(ceil_div(nleaves, 4), batch), 128, 0, st>>>(w.b, w.leaf_off, nleaves, d_info);
         NAO_LAUNCHED();

@@ -37,23 +37,6 @@ static const int TRD_CH = 96;        // rows of V/W cached in shared memory per 
 static const int TRD_CHP = TRD_CH + 1;
 static const int TRD_PASS = 128;     // rows finalised per pass in phase A
 
-#ifdef NAO_TRACE
-#ifndef TRD_TRACE_CTA
-#define TRD_TRACE_CTA 0
-#endif
-__device__ unsigned long long g_trd_trace[16];
-__device__ unsigned long long g_trd_stamp[4 * 296];      // per CTA: phase-B start, hemv start, hemv end (own warps), after barrier 2
-__device__ int g_trd_stamp_col = 100;
-#define TRD_T(k)                                                                                   \
-    do {                                                                                           \
-        if (blockIdx.x == TRD_TRACE_CTA && threadIdx.x == 0) {                                     \
-            unsigned long long t__; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t__));      \
-            g_trd_trace[k] += t__ - t_last; t_last = t__;                                          \
-        }                                                                                          \
-    } while (0)
-#else
-#define TRD_T(k)
-#endif
 
 template <class T> struct Hv;
 template <> struct Hv<double> { static const int SW = 32, CPT = 16, HS = 2, CB = 4; };   // 64 x 32 units: finer load balance
@@ -298,12 +281,8 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
     auto getV = [&](int r, int k) -> T { return cached ? sV[k * TRD_CHP + (r - r0)] : A[r + (long)(j0 + k) * lda]; };
     auto getW = [&](int r, int k) -> T { return cached ? sW[k * TRD_CHP + (r - r0)] : Wp[r + (long)k * n]; };
 
-#ifdef NAO_TRACE
-    unsigned long long t_last; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_last));
-#endif
     for (int i = 0; i <= p.nbp; ++i) {
         const int j = j0 + i;
-        TRD_T(0);
         const int ra = max(r0, j);                 // first own row still in play
         // =============================== phase A ===============================
         // row j of the panel's V and W (columns < i resp. < i-1): needed by every CTA, fetched first so that the
@@ -349,7 +328,6 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
                 }
                 __syncthreads();
             }
-            TRD_T(1);
             // (2) w_{i-1} for the own rows r >= j and (redundantly, every CTA) for row j
             const int nown = max(0, r1 - ra);
             const bool extra = !(j >= r0 && j < r1);
@@ -420,7 +398,6 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
                 __syncthreads();
             }
         }
-        TRD_T(2);
         const bool do_col = (i < p.nbp) || (j == n - 1);
         __syncthreads();
         if (do_col) {
@@ -437,9 +414,7 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
             if (tid == 0) pn[g] = nrm;
         }
         if (i == p.nbp) break;
-        TRD_T(3);
         group_barrier(bar, G, ++bar_ord);
-        TRD_T(4);
 
         // =============================== phase B ===============================
         if (warp == 0) {
@@ -472,7 +447,6 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
             }
         }
         __syncthreads();
-        TRD_T(5);
         const T scale = s_scale;
         auto vval = [&](int x) -> T {
             if (x < j + 1 || x >= n) return O::zero();
@@ -505,26 +479,10 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
             if (tid < 2 * TRD_NB)
                 pt[(long)g * 2 * TRD_NB + tid] = O::add(O::add(s_red4[0][tid], s_red4[1][tid]), O::add(s_red4[2][tid], s_red4[3][tid]));
         }
-        TRD_T(6);
-#ifdef NAO_TRACE
-        unsigned long long ts0 = 0, ts1 = 0;
-        if (j == g_trd_stamp_col && tid == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(ts0));
-#endif
         double vav = hemv_warp<T>(A, lda, n, j, nblk, G, g, acol, scale, sx + warp * SW, Prow, Pcol);
         vav = block_sum_d(vav, s_dred);
         if (tid == 0) pvav[g] = vav;
-        TRD_T(7);
-#ifdef NAO_TRACE
-        if (j == g_trd_stamp_col && tid == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(ts1));
-#endif
         group_barrier(bar, G, ++bar_ord);
-#ifdef NAO_TRACE
-        if (j == g_trd_stamp_col && tid == 0) {
-            unsigned long long ts2; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(ts2));
-            g_trd_stamp[4 * blockIdx.x + 1] = ts0; g_trd_stamp[4 * blockIdx.x + 2] = ts1; g_trd_stamp[4 * blockIdx.x + 3] = ts2;
-        }
-#endif
-        TRD_T(8);
     }
 }
 
@@ -629,55 +587,6 @@ static int hetrd_impl(int dtype, int n, int batch, T *A, long lda, long sA, doub
     return NAO_OK;
 }
 
-#ifdef NAO_TRACE
-// HEMV of `ncols` consecutive columns starting at j0 with NOTHING else (no reflector, no barriers, no reductions): isolates
-// the streaming part of hetrd_panel_kernel for timing.  acol must hold n finite values.
-template <class T>
-__global__ void __launch_bounds__(TRD_NT, 1) hemv_only_kernel(const T *A, long lda, long sA, int n, int j0, int ncols, int G,
-                                                              int nblk, const T *acol, T *Prow, T *Pcol, double *out) {
-    extern __shared__ __align__(16) unsigned char trd_smem[];
-    T *sx = (T *)trd_smem;
-    const int item = blockIdx.x / G, g = blockIdx.x % G, warp = threadIdx.x >> 5;
-    A += (long)item * sA; Prow += (long)item * Hv<T>::HS * nblk * n; Pcol += (long)item * nblk * n; acol += (long)item * n;
-    double acc = 0.0;
-    for (int j = j0; j < j0 + ncols; ++j) {
-        acc += hemv_warp<T>(A, lda, n, j, nblk, G, g, acol, Ops<T>::one(), sx + warp * Hv<T>::SW, Prow, Pcol);
-        __syncthreads();
-    }
-    if (acc == 1.2345) out[0] = acc;
-}
-}  // namespace nao
-NAO_EXPORT double nao_debug_hemv_only(int n, int batch, int j0, int ncols, const double *dA, double *dwork, int reps) {
-    using namespace nao;
-    const int G = 148 / batch, nblk = ceil_div(n, TRD_TB);
-    double *acol = dwork, *Prow = acol + (size_t)batch * n, *Pcol = Prow + (size_t)batch * 2 * nblk * n, *out = Pcol + (size_t)batch * nblk * n;
-    cudaMemset(acol, 0, (size_t)batch * n * 8);
-    cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
-    const size_t smem = (size_t)TRD_NW * Hv<double>::SW * 8;
-    hemv_only_kernel<double><<<batch * G, TRD_NT, smem>>>(dA, n, (long)n * n, n, j0, ncols, G, nblk, acol, Prow, Pcol, out);
-    cudaEventRecord(e0);
-    for (int r = 0; r < reps; ++r)
-        hemv_only_kernel<double><<<batch * G, TRD_NT, smem>>>(dA, n, (long)n * n, n, j0, ncols, G, nblk, acol, Prow, Pcol, out);
-    cudaEventRecord(e1); cudaEventSynchronize(e1);
-    float ms = 0.f; cudaEventElapsedTime(&ms, e0, e1);
-    return cudaGetLastError() == cudaSuccess ? ms / reps : -1.0;
-}
-NAO_EXPORT int nao_debug_trd_stamps(int col, unsigned long long *out /* 4*296 */) {
-    cudaDeviceSynchronize();
-    if (out) cudaMemcpyFromSymbol(out, nao::g_trd_stamp, sizeof(unsigned long long) * 4 * 296);
-    cudaMemcpyToSymbol(nao::g_trd_stamp_col, &col, sizeof(int));
-    return 0;
-}
-NAO_EXPORT int nao_debug_trd_trace(double *out_us, int reset) {
-    unsigned long long h[16];
-    cudaDeviceSynchronize();
-    cudaMemcpyFromSymbol(h, nao::g_trd_trace, sizeof(h));
-    for (int i = 0; i < 16; ++i) out_us[i] = h[i] * 1e-3;
-    if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(nao::g_trd_trace, z, sizeof(z)); }
-    return 0;
-}
-namespace nao {
-#endif
 
 int hetrd(int dtype, int n, int batch, void *A, long lda, long sA, double *d, double *e, void *tau, void *work,
           cudaStream_t st) {

@@ -22,18 +22,6 @@ namespace nao {
 
 static const int CH_NT = 256;
 
-#ifdef NAO_TRACE
-__device__ unsigned long long g_chase_trace[8];
-#define CH_T(k)                                                                                 \
-    do {                                                                                        \
-        if (blockIdx.x == 1 && threadIdx.x == 0) {                                              \
-            unsigned long long t__; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t__));   \
-            g_chase_trace[k] += t__ - ch_last; ch_last = t__;                                   \
-        }                                                                                       \
-    } while (0)
-#else
-#define CH_T(k)
-#endif
 
 template <class T>
 __global__ void band_extract_kernel(int n, const T *A, long lda, long sA, T *AB, long sAB) {
@@ -223,9 +211,6 @@ __global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
         }
         cp_async_commit();
     };
-#ifdef NAO_TRACE
-    unsigned long long ch_last; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(ch_last));
-#endif
     for (int s = c; s < n - 1; s += P) {
         // ------------------------------------------------ step 0
         int r0 = s + 1, Lp = min(s + b, n - 1) - r0 + 1;
@@ -268,12 +253,10 @@ __global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
             const int q0 = s + 1 + k * b;
             if (q0 > n - 1) break;
             const int Lq = min(s + (k + 1) * b, n - 1) - q0 + 1;
-            CH_T(0);
             if (PF && s > 0) {
                 if (tid == 0) { while (ld_acquire(prog + s - 1) < k + 2) { } }
                 __syncthreads();
             }
-            CH_T(1);
             if constexpr (PF) {
                 // the prefetched pair becomes current; its last row arrives now (written by the predecessor's latest step)
                 cp_async_wait<0>();
@@ -337,7 +320,6 @@ __global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
                 }
             }
             __syncthreads();
-            CH_T(2);
             // Fused form of  O <- H_n^H (O H_p),  D <- H_n^H D H_n  with ONE pass over each block:
             //   w = O v_p ;  x = O[:,0] - tau_p w  -> (v_n, tau_n, beta) ;  kappa = v_n^H w
             //   q = O^H v_n (on the ORIGINAL O) ;  z_c = q_c - tau_p kappa conj(v_p[c])   (= v_n^H (O H_p)[:,c])
@@ -427,7 +409,6 @@ __global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
                 if ((tid & 31) == 0) s_gamma = gsum;
             }
             __syncthreads();
-            CH_T(3);
             // (6) one pass over O and D: new values go straight to global memory
             {
                 const T tau_n = s_tau_n, tau_p = s_tau_p;
@@ -458,13 +439,11 @@ __global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
                     }
                 }
             }
-            CH_T(4);
             // publish: the block barrier orders every thread's stores before thread 0, whose fence + release store make
             // them visible to the CTA that acquires the counter (the pattern of a cooperative-groups grid sync)
             __syncthreads();
             if (tid < b) s_vp[tid] = s_vn[tid];
             if (tid == 0) { s_tau_p = s_tau_n; __threadfence(); st_release(prog + s, k + 1); }
-            CH_T(5);
             r0 = q0; Lp = Lq;
         }
         __syncthreads();
@@ -536,18 +515,6 @@ static int hb2st_impl(int dtype, int n, int batch, const T *A, long lda, long sA
     return NAO_OK;
 }
 
-#ifdef NAO_TRACE
-}  // namespace nao
-NAO_EXPORT int nao_debug_chase_trace(double *out_us) {
-    unsigned long long h[8];
-    cudaDeviceSynchronize();
-    cudaMemcpyFromSymbol(h, nao::g_chase_trace, sizeof(h));
-    for (int i = 0; i < 8; ++i) out_us[i] = h[i] * 1e-3;
-    unsigned long long z[8] = {0}; cudaMemcpyToSymbol(nao::g_chase_trace, z, sizeof(z));
-    return 0;
-}
-namespace nao {
-#endif
 
 int hb2st(int dtype, int n, int batch, const void *A, long lda, long sA, double *d, double *e, void *V2, long ldv, long sV2,
           void *tau2, void *work, cudaStream_t st) {

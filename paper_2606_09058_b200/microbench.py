@@ -1,11 +1,11 @@
-"""Per-kernel micro-benchmarks of libnao.so building blocks (CUDA events, warm-up, L2 flush between repetitions).
+"""Per-kernel measurement entry of libnao.so building blocks (CUDA events, warm-up, L2 flush between repetitions): the
+command the ncu captures summarised under profiles/ run.  Library kernels only.
 
     python -m paper_2606_09058_b200.microbench gemm [--m M --n N --k K] [--complex] [--opa 0|1|2] [--opb 0|1|2]
-                                                    [--beta B] [--lower] [--cublas] [--reps R]
+                                                    [--beta B] [--lower] [--reps R]
     python -m paper_2606_09058_b200.microbench heev [--n N] [--batch B] [--complex] [--two-stage|--one-stage]
     python -m paper_2606_09058_b200.microbench fold [--n N] [--nk NK] [--nr NR] [--complex]      (config 1: 832, 8, 27)
 
-`--cublas` adds torch.matmul on the same operands as a SIDE comparison (never used by the product path).
 Prints one JSON line per measurement.
 """
 from __future__ import annotations
@@ -63,12 +63,6 @@ def bench_gemm(args):
     out = {"kernel": "gemm_kernel", "m": m, "n": n, "k": k, "complex": args.complex, "opA": args.opa, "opB": args.opb,
            "beta": args.beta, "lower_only": args.lower, "ms": ms, "tflops": flops / ms / 1e9,
            "frac_of_dmma_peak": flops / ms / 1e9 / FP64_DMMA_PEAK_TFLOPS}
-    if args.cublas:
-        At = A[0].T if args.opa == 0 else (A[0] if args.opa == 1 else A[0].conj())   # logical op(A) (m x k) as a view
-        Bt = Bm[0].T if args.opb == 0 else (Bm[0] if args.opb == 1 else Bm[0].conj())
-        ms_c = _time(lambda: torch.matmul(At, Bt), args.reps, flush)
-        out["cublas_ms"] = ms_c
-        out["cublas_tflops"] = (8.0 if args.complex else 2.0) * m * n * k / ms_c / 1e9
     print(json.dumps(out))
 
 
@@ -133,7 +127,6 @@ def main():
     ap.add_argument("--opb", type=int, default=0)
     ap.add_argument("--beta", type=float, default=0.0)
     ap.add_argument("--lower", action="store_true")
-    ap.add_argument("--cublas", action="store_true")
     ap.add_argument("--two-stage", action="store_true")
     ap.add_argument("--one-stage", action="store_true")
     ap.add_argument("--reps", type=int, default=5)

@@ -99,6 +99,28 @@ def test_host_side_argument_validation(libpath):
     assert lib.nao_solve_host(8, 1, 0, 0, None, 1, 0, w1, 4.0, 1e-3, 1, ctypes.byref(mu), 1, 1, 1, 1 << 30, None) == -5
     assert lib.nao_solve_host(8, 1, 0, 1, 1, 1, 0, w1, 4.0, 1e-3, 1, ctypes.byref(mu), 1, 1, 1, 1 << 30, None) == -4      # S_FACTORED
     assert lib.nao_solve_host(8, 1, 0, 0, 1, 1, 0, w1, 4.0, 1e-3, 1, ctypes.byref(mu), 1, 1, 1, 64, None) == 1           # workspace
+    # ... and its occupation arguments are checked before the eigensolve is paid for (same rules as nao_fermi_mu)
+    assert lib.nao_solve_host(8, 1, 0, 0, 1, 1, 0, w1, 17.0, 1e-3, 1, ctypes.byref(mu), 1, 1, 1, 1 << 30, None) == 3     # N_e > sum w n
+    assert lib.nao_solve_host(8, 1, 0, 0, 1, 1, 0, w1, 4.0, 0.0, 1, ctypes.byref(mu), 1, 1, 1, 1 << 30, None) == 3       # kT <= 0
+    wneg = (ctypes.c_double * 1)(-1.0)
+    assert lib.nao_solve_host(8, 1, 0, 0, 1, 1, 0, wneg, 4.0, 1e-3, 1, ctypes.byref(mu), 1, 1, 1, 1 << 30, None) == -8   # h_weight
+    assert lib.nao_solve_host(8, 1, 0, 0, 1, 1, 0, None, 4.0, 1e-3, 1, ctypes.byref(mu), 1, 1, 1, 1 << 30, None) == -8
+    # fused step: the same checks first, and the negative codes of the shared eigensolver count THIS signature's arguments
+    lib.nao_scf_step.argtypes = [i, i, i, ctypes.c_uint, vp, l, l, vp, l, l, dp, ctypes.c_double, ctypes.c_double, vp, dp, vp,
+                                 vp, l, l, vp, l, l, ctypes.POINTER(i), vp, ctypes.c_size_t, vp, vp]
+    nv = i(0)
+
+    def scf(n=8, batch=1, dH=1, ldh=8, dS=1, w=w1, ne=4.0, kT=1e-3, dE=1, dF=1, dC=1, ldc=8, dD=1, ldd=8, work=1, wb=1 << 30, info=1):
+        return lib.nao_scf_step(n, batch, 0, 0, dH, ldh, 64, dS, 8, 64, w, ne, kT, dE, ctypes.byref(mu), dF, dC, ldc, 64, dD, ldd, 64,
+                                ctypes.byref(nv), work, wb, info, None)
+    assert scf(ne=17.0) == 3 and scf(ne=0.0) == 3 and scf(kT=-1.0) == 3
+    assert scf(w=wneg) == -11 and scf(w=None) == -11
+    assert scf(n=0) == -1 and scf(batch=0) == -2
+    assert scf(dH=None) == -5 and scf(ldh=7) == -6 and scf(dS=None) == -8
+    assert scf(dE=None) == -14 and scf(dF=None) == -16 and scf(dC=None) == -17 and scf(ldc=7) == -18
+    assert scf(dD=None) == -20 and scf(ldd=7) == -21
+    assert scf(work=None) == -24 and scf(info=None) == -26
+    assert scf(wb=64) == 1
     lib.nao_set_lowdin_threshold.argtypes = [ctypes.c_double]
     assert lib.nao_set_lowdin_threshold(-1e-3) == -1 and lib.nao_set_lowdin_threshold(1.0) == -1
     assert lib.nao_set_lowdin_threshold(1e-8) == 0 and lib.nao_set_lowdin_threshold(0.0) == 0
