@@ -181,6 +181,32 @@ def side_record(nao, torch, workload, dev, hbm_peak, dmma_meas, steps=3, warmup=
         tf = kg["work"] / (kg["ms"] * 1e-3) / 1e12
         rec["roofline_gemm"] = {"kernel": kg["name"], "bound": "tensor", "achieved": tf, "peak": dmma_meas, "unit": "TFLOP/s",
                                 "frac": tf / dmma_meas, "kernel_ms_per_step": kg["ms"], "launches_timed": kg["launches"]}
+    # concurrent mid-size solves: the same step with the batch spread over 2/4/8 internal streams
+    # (NAO_STREAM_GROUPS_*), against the single batched launch above
+    if prob.batch >= 4:
+        groups = {"1 (batched launches)": ms}
+        for gname, gflag in (("2", nao.NAO_STREAM_GROUPS_2), ("4", nao.NAO_STREAM_GROUPS_4), ("8", nao.NAO_STREAM_GROUPS_8)):
+            gwork = torch.empty(nao.geneig_workspace(prob.n, prob.batch, dt, flags | gflag) + 256, dtype=torch.uint8, device=dev)
+
+            def gstep():
+                S.copy_(S0)
+                E, C, info = nao.geneig(H, S, flags=flags | gflag, work=gwork)
+                mu, F = nao.fermi_mu(E, weights, prob.n_electrons, prob.kT)
+                nao.density_matrix(C, F, out=Dbuf)
+                return mu
+            for _ in range(warmup):
+                mu_g = gstep()
+            torch.cuda.synchronize()
+            assert abs(mu_g - mu) <= 1e-12
+            tot = 0.0
+            for _ in range(steps):
+                if flush is not None:
+                    flush.zero_()
+                ev0.record(); gstep(); ev1.record(); torch.cuda.synchronize()
+                tot += ev0.elapsed_time(ev1)
+            groups[gname] = tot / steps
+            del gwork
+        rec["stream_groups_ms_per_step"] = groups
     del H, S, S0, work, Dbuf
     torch.cuda.empty_cache()
     return rec

@@ -61,6 +61,17 @@ extern "C" {
                                   so that mu and D are those of the pruned basis.  With rel = 0 a non-positive eigenvalue
                                   of S sets d_info = (order of S) + 2. */
 #define NAO_PRUNED_LEVEL 1.0e4 /* Hartree; eigenvalue reported for a pruned direction */
+/* Concurrent mid-size solves: nao_geneig / nao_geneig_partial cut the batch into
+   2, 4 or 8 contiguous groups that run the whole chain on internal streams, forked from and joined back into cuda_stream,
+   each with its own slice of the workspace (nao_geneig_workspace accounts for it when given the same flags) and with its
+   grid-barrier kernels sized for its share of the SMs.  Same results as the single batched call.  Ignored (one group) when
+   the batch is smaller than the group count, when one shared S (strideS = 0) still has to be factored, and by
+   nao_scf_step / nao_solve_host.  Without these flags every kernel of the chain is launched once for the whole batch --
+   on B200 that is the faster arrangement for config 1 (f3). */
+#define NAO_STREAM_GROUPS_2 32u
+#define NAO_STREAM_GROUPS_4 64u
+#define NAO_STREAM_GROUPS_8 96u
+#define NAO_STREAM_GROUPS_MASK 96u
 
 /* return codes */
 #define NAO_OK 0

@@ -19,6 +19,7 @@ from . import build as _build
 
 NAO_REAL, NAO_COMPLEX = 0, 1
 NAO_S_FACTORED, NAO_NC_BLOCK_S, NAO_TRD_ONE_STAGE, NAO_TRD_TWO_STAGE, NAO_LOWDIN = 1, 2, 4, 8, 16
+NAO_STREAM_GROUPS_2, NAO_STREAM_GROUPS_4, NAO_STREAM_GROUPS_8 = 32, 64, 96
 NAO_PRUNED_LEVEL = 1.0e4
 
 _LIB = None

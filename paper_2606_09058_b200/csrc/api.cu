@@ -15,6 +15,19 @@ NAO_EXPORT const char *nao_status_string(int status) {
 NAO_EXPORT const char *nao_version(void) { return "nao-b200 0.1 (sm_100a)"; }
 NAO_EXPORT long nao_launch_count(void) { return nao::g_launch_count; }
 
+namespace nao {
+static int g_sm_limit = 0;
+void set_sm_limit(int limit) { g_sm_limit = limit > 0 ? limit : 0; }
+int sm_count() {
+    static int nsm = 0;
+    if (!nsm) {
+        int dev = 0; cudaGetDevice(&dev);
+        if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm <= 0) nsm = 148;
+    }
+    return (g_sm_limit > 0 && g_sm_limit < nsm) ? g_sm_limit : nsm;
+}
+}  // namespace nao
+
 // ---- optional phase timing (CUDA events recorded on the caller's stream at phase boundaries of nao_geneig) ----
 namespace nao {
 static const int NPH = 9;

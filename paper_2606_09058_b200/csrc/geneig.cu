@@ -103,6 +103,13 @@ static int heev(int dtype, int n, int batch, unsigned flags, void *A, long lda, 
 // ----------------------------------------------------------------------------------------------------- geneig
 static double g_lowdin_rel = 0.0;      // nao_set_lowdin_threshold
 
+// NAO_STREAM_GROUPS_2/4/8: number of internal streams the batch of nao_geneig is spread over
+static int stream_groups(unsigned flags, int batch) {
+    int g = 1 << ((flags & NAO_STREAM_GROUPS_MASK) >> 5);
+    while (g > 1 && batch < g) g >>= 1;
+    return g;
+}
+
 struct GePlan { size_t W, Wc, A, X, heev, bytes; int nS, sdtype, nitemsS; };
 static GePlan ge_plan(int n, int batch, int dtype, unsigned flags, bool shared_S) {
     GePlan p; size_t off = 0;
@@ -158,7 +165,21 @@ NAO_EXPORT int nao_geneig_workspace(int n, int batch, int dtype, unsigned flags,
     if (dtype != NAO_REAL && dtype != NAO_COMPLEX) return -3;
     if ((flags & NAO_NC_BLOCK_S) && (dtype != NAO_COMPLEX || (n & 1))) return -4;
     if (!bytes) return -5;
-    *bytes = nao::ge_plan(n, batch, dtype, flags, false).bytes;
+    const int groups = nao::stream_groups(flags, batch);
+    flags &= ~NAO_STREAM_GROUPS_MASK;
+    size_t plain = nao::ge_plan(n, batch, dtype, flags, false).bytes;
+    if (groups > 1) {
+        // every group carves its own slice, planned with the group's share of the SMs
+        nao::set_sm_limit(nao::sm_count() / groups);
+        size_t total = 0;
+        for (int g = 0; g < groups; ++g) {
+            const int b0 = (int)((long)batch * g / groups), b1 = (int)((long)batch * (g + 1) / groups);
+            total += nao::align_up(nao::ge_plan(n, b1 - b0, dtype, flags, false).bytes);
+        }
+        nao::set_sm_limit(0);
+        if (total > plain) plain = total;
+    }
+    *bytes = plain;
     return NAO_OK;
 }
 
@@ -306,11 +327,67 @@ static int geneig_impl(int n, int batch, int dtype, unsigned flags, int nvec, co
     return NAO_OK;
 }
 
+// Concurrent mid-size solves (the paper's observation that several k-points sharing a GPU fill the gaps
+// of one another): the batch is cut into `groups` contiguous groups, each of which runs the whole
+// chain on its own internal stream (forked from and joined back into the caller's stream) with its own slice of the
+// workspace.  The cooperative kernels of a group are sized for 1/groups of the SMs so that the groups are co-resident.
+static int geneig_grouped(int n, int batch, int dtype, unsigned flags, int nvec, const void *dH, long ldh, long strideH, void *dS,
+                          long lds, long strideS, double *dE, void *dC, long ldc, long strideC, void *dwork,
+                          size_t work_bytes, int *d_info, void *cuda_stream) {
+    using namespace nao;
+    int groups = (n >= 1 && batch >= 1) ? stream_groups(flags, batch) : 1;
+    flags &= ~NAO_STREAM_GROUPS_MASK;
+    // one shared S that still has to be factored is written by every group: run the batch as one group
+    if (strideS == 0 && !(flags & NAO_S_FACTORED)) groups = 1;
+    if (groups <= 1)
+        return geneig_impl(n, batch, dtype, flags, nvec, dH, ldh, strideH, dS, lds, strideS, dE, dC, ldc, strideC, dwork, work_bytes,
+                           d_info, cuda_stream);
+    // argument check of the whole call first (phase 0: no launch)
+    int rc = geneig_impl(n, batch, dtype, flags, nvec, dH, ldh, strideH, dS, lds, strideS, dE, dC, ldc, strideC, dwork, (size_t)-1,
+                         d_info, cuda_stream, 0);
+    if (rc) return rc;
+    static cudaStream_t side[8] = {nullptr};
+    static cudaEvent_t ev_fork = nullptr, ev_join[8] = {nullptr};
+    if (!ev_fork) {
+        NAO_CUDA_CHECK(cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming));
+        for (int g = 0; g < 8; ++g) {
+            NAO_CUDA_CHECK(cudaStreamCreateWithFlags(&side[g], cudaStreamNonBlocking));
+            NAO_CUDA_CHECK(cudaEventCreateWithFlags(&ev_join[g], cudaEventDisableTiming));
+        }
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t es = esize(dtype), esS = (flags & NAO_NC_BLOCK_S) ? 8 : es;
+    set_sm_limit(sm_count() / groups);
+    size_t off = 0;
+    for (int g = 0; g < groups && rc == NAO_OK; ++g) {
+        const int b0 = (int)((long)batch * g / groups), b1 = (int)((long)batch * (g + 1) / groups);
+        off += align_up(ge_plan(n, b1 - b0, dtype, flags, strideS == 0).bytes);
+    }
+    if (off > work_bytes) { set_sm_limit(0); return NAO_ERR_WORKSPACE; }
+    if (cudaEventRecord(ev_fork, st) != cudaSuccess) { set_sm_limit(0); return NAO_ERR_CUDA; }
+    off = 0;
+    for (int g = 0; g < groups; ++g) {
+        const int b0 = (int)((long)batch * g / groups), b1 = (int)((long)batch * (g + 1) / groups), nb = b1 - b0;
+        const size_t need = ge_plan(n, nb, dtype, flags, strideS == 0).bytes;
+        if (cudaStreamWaitEvent(side[g], ev_fork, 0) != cudaSuccess) { rc = NAO_ERR_CUDA; break; }
+        rc = geneig_impl(n, nb, dtype, flags, nvec, (const char *)dH + (size_t)b0 * strideH * es, ldh, strideH,
+                         (char *)dS + (size_t)b0 * strideS * esS, lds, strideS, dE + (size_t)b0 * n,
+                         (char *)dC + (size_t)b0 * strideC * es, ldc, strideC, (char *)dwork + off, need, d_info + b0, side[g]);
+        if (rc) break;
+        off += align_up(need);
+        if (cudaEventRecord(ev_join[g], side[g]) != cudaSuccess || cudaStreamWaitEvent(st, ev_join[g], 0) != cudaSuccess) {
+            rc = NAO_ERR_CUDA; break;
+        }
+    }
+    set_sm_limit(0);
+    return rc;
+}
+
 NAO_EXPORT int nao_geneig(int n, int batch, int dtype, unsigned flags, const void *dH, long ldh, long strideH, void *dS,
                           long lds, long strideS, double *dE, void *dC, long ldc, long strideC, void *dwork,
                           size_t work_bytes, int *d_info, void *cuda_stream) {
-    return geneig_impl(n, batch, dtype, flags, n, dH, ldh, strideH, dS, lds, strideS, dE, dC, ldc, strideC, dwork, work_bytes,
-                       d_info, cuda_stream);
+    return geneig_grouped(n, batch, dtype, flags, n, dH, ldh, strideH, dS, lds, strideS, dE, dC, ldc, strideC, dwork, work_bytes,
+                          d_info, cuda_stream);
 }
 
 NAO_EXPORT int nao_geneig_partial(int n, int batch, int dtype, unsigned flags, int n_vec, const void *dH, long ldh, long strideH,
@@ -318,8 +395,8 @@ NAO_EXPORT int nao_geneig_partial(int n, int batch, int dtype, unsigned flags, i
                                   size_t work_bytes, int *d_info, void *cuda_stream) {
     if (n < 1) return -1;
     if (n_vec < 1 || n_vec > n) return -5;
-    int rc = geneig_impl(n, batch, dtype, flags, n_vec, dH, ldh, strideH, dS, lds, strideS, dE, dC, ldc, strideC, dwork,
-                         work_bytes, d_info, cuda_stream);
+    int rc = geneig_grouped(n, batch, dtype, flags, n_vec, dH, ldh, strideH, dS, lds, strideS, dE, dC, ldc, strideC, dwork,
+                            work_bytes, d_info, cuda_stream);
     return (rc <= -5) ? rc - 1 : rc;          // argument positions after n_vec are shifted by one
 }
 
@@ -336,6 +413,7 @@ extern "C" int nao_density_matrix(int n, int batch, int dtype, const void *dC, l
 // The fused step back-transforms only the occupied vectors, which favours the two-stage reduction for complex matrices as
 // well (config 3: 831 vs 1141 ms per step); below order 1536 the one-stage path stays ahead (config 1: 34 vs 40 ms).
 static unsigned scf_step_flags(int n, unsigned flags) {
+    flags &= ~NAO_STREAM_GROUPS_MASK;          // the fused step runs as one group
     if (!(flags & (NAO_TRD_ONE_STAGE | NAO_TRD_TWO_STAGE)) && n >= nao::TWO_STAGE_MIN_N_REAL) flags |= NAO_TRD_TWO_STAGE;
     return flags;
 }
@@ -462,6 +540,7 @@ NAO_EXPORT int nao_solve_host(int n, int batch, int dtype, unsigned flags, const
     if (dtype != NAO_REAL && dtype != NAO_COMPLEX) return -3;
     if ((flags & NAO_NC_BLOCK_S) && (dtype != NAO_COMPLEX || (n & 1))) return -4;
     if (flags & NAO_S_FACTORED) return -4;              // the factor lives in the device scratch: not kept between calls
+    flags &= ~NAO_STREAM_GROUPS_MASK;
     if (!hH) return -5;
     if (!hS) return -6;
     if (int rc0 = check_occupation_args(n, batch, h_weight, n_electrons, kT, 8)) return rc0;

@@ -16,6 +16,11 @@ typedef double2 cplx;   // interleaved complex FP64 (x = re, y = im)
 // launch bookkeeping
 // ---------------------------------------------------------------------------------------------------------
 extern long g_launch_count;          // host-side count of kernel launches (nao_launch_count)
+// SMs the cooperative (grid-barrier) kernels of the current call may occupy: the device's SM count, or less while a
+// stream group of nao_geneig (NAO_STREAM_GROUPS_*) is being enqueued, so that the groups' cooperative kernels are
+// co-resident on disjoint SMs instead of waiting for one another.
+int sm_count();
+void set_sm_limit(int limit);        // 0 = no limit
 #define NAO_LAUNCHED() (++::nao::g_launch_count)
 
 #define NAO_CUDA_CHECK(expr)                                        \

@@ -496,14 +496,7 @@ static int trd_G(int n, int batch, int nsm) {
     int want = ceil_div(n, 64);
     return per < want ? per : want;
 }
-static int num_sms() {
-    static int nsm = 0;
-    if (!nsm) {
-        int dev = 0; cudaGetDevice(&dev);
-        if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm <= 0) nsm = 148;
-    }
-    return nsm;
-}
+static int num_sms() { return sm_count(); }
 static TrdWork trd_plan(int dtype, int n, int batch, void *work) {
     TrdWork w;
     const size_t es = esize(dtype);

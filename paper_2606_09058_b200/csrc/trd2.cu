@@ -255,14 +255,7 @@ struct He2hbWork {
     void *P4, *GS, *B2, *part, *rowb, *splitk; unsigned *bar;
     int Gq, chunk, ipl, ksX, ksS; size_t smem, bytes;
 };
-static int trd2_num_sms() {
-    static int nsm = 0;
-    if (!nsm) {
-        int dev = 0; cudaGetDevice(&dev);
-        if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm <= 0) nsm = 148;
-    }
-    return nsm;
-}
+static int trd2_num_sms() { return sm_count(); }
 static He2hbWork he2hb_plan(int dtype, int n, int batch, void *work) {
     He2hbWork w; const size_t es = esize(dtype); const int b = TRD2_B;
     const int nsm = trd2_num_sms();

@@ -6,9 +6,24 @@
 //   G(I,k) = H_{s0,k} H_{s0+1,k} ... = I - V T V^H,   V = (b + NBK - 1) x NBK parallelogram (rows s0+1+kb ..).
 // Reflectors of different steps of one sweep commute, and (s,k) overlaps (s',k+1) only for s' < s, so Q2 Z is obtained
 // by applying the groups with I DESCENDING and, inside an S-block, k ASCENDING (checked against the sweep-by-sweep
-// product in tests).  Columns of Z are independent: each CTA owns NC columns and walks through all groups without any
-// inter-CTA synchronisation; the three products per group (W = V^H Z_w, W <- T W, Z_w -= V W) run on FP64 DMMA from
-// shared memory.  T factors of all groups are precomputed by q2_tfactor_kernel.
+// product in tests).  Columns of Z are independent.
+//
+// B200 design (round 2):
+//   q2_pack_kernel   one CTA per diamond: T by the xLARFT recurrence, then the diamond is written as ONE contiguous,
+//                    padded block [V (ci-major) | V (row-major, real only) | T (row-major)] in exactly the
+//                    shared-memory layout the apply kernel reads, so that it arrives with a single 1-D TMA copy.
+//   q2_apply_kernel  every WARP owns 8 or 16 columns of Z and keeps its 96-row window of them in REGISTERS, in the
+//                    accumulator layout of mma.sync.m8n8k4 (lane = (column, row pair)).  The three products of a diamond
+//                    are chained in registers in transposed form,
+//                        W^T = Z_w^T conj(V),   W2^T = W^T T^T,   Z_w^T -= W2^T V^T,
+//                    the accumulator fragments of one product being the A fragments of the next: the contraction index of
+//                    a DMMA may be enumerated in any order, so k-step "even"/"odd" of an 8-row tile contracts over the rows
+//                    2q / 2q+1 a lane already holds.  Only V and T are read from shared memory (B fragments, one 16-byte
+//                    load feeds two k-steps): a third of the shared-memory traffic of a formulation that keeps Z, W and W2
+//                    there, no block-wide barrier in the loop.  A producer warp streams the packed diamonds with
+//                    cp.async.bulk (TMA) into a two-stage ring guarded by full/empty mbarriers; the 64 rows of Z that
+//                    enter the window at the next step are prefetched with cp.async into a per-warp staging area; the 64
+//                    rows that leave are stored from registers.
 #include "nao_internal.cuh"
 #include "scalar.cuh"
 #include <algorithm>
@@ -16,11 +31,22 @@
 namespace nao {
 
 static const int Q2_NBK = 32;                 // sweeps per diamond
-static const int Q2_LW = 96;                  // padded window rows (>= TRD2_B + Q2_NBK - 1)
-static const int Q2_NT = 128;
-static const int Q2_LDV = 100, Q2_LDW = 36;   // shared-memory leading dimensions (conflict-free fragment loads)
-// T: 36 for real (conflict-free A fragments); complex stays at 32 so that two CTAs of 16 columns still fit on an SM
-template <class T> struct Q2Ldt { static const int value = sizeof(T) == 8 ? 36 : 32; };
+static const int Q2_LW = 96;                  // window rows (>= TRD2_B + Q2_NBK - 1), 12 tiles of 8
+static const int Q2_NT = Q2_LW / 8;
+static const int Q2_MAXW = 9;                 // most consumer warps per CTA
+
+// Packed diamond (elements of T).  Leading dimensions make every fragment load conflict free:
+//   real:    16-byte loads of (k, k+1) pairs, quarter-warp = 2 rows x 4 pairs  ->  ld = 8 mod 16
+//   complex: 16-byte loads of one element, quarter-warp = 2 rows x 4 elements 2 apart -> ld odd (1 mod 8)
+template <class T> struct Q2P;
+template <> struct Q2P<double> {
+    static const int LDV = 104, LDVT = 40, LDT = 40, OFF_VT = Q2_NBK * 104, OFF_T = OFF_VT + Q2_LW * 40, BLK = OFF_T + Q2_NBK * 40;
+    static const int CW = 16, LDS = 72;       // widest warp slab (columns), staging leading dimension (64 rows + pad)
+};
+template <> struct Q2P<cplx> {
+    static const int LDV = 97, LDVT = 0, LDT = 33, OFF_VT = 0, OFF_T = Q2_NBK * 97, BLK = OFF_T + Q2_NBK * 33;
+    static const int CW = 8, LDS = 65;
+};
 
 __host__ __device__ inline int q2_nwin(int n, int s0) {      // windows of the S-block starting at sweep s0
     return s0 + 1 <= n - 1 ? (n - 2 - s0) / TRD2_B + 1 : 0;
@@ -31,39 +57,36 @@ __host__ __device__ inline long q2_ngroups(int n) {
     return t;
 }
 
-// masked load of the V parallelogram of group (s0, k) into sV[ci * LDV + r] (zero padded to LW x NBK)
+// ---------------------------------------------------------------------------------------------------------------------
+// pack: V parallelogram of diamond (I, k) -> shared memory, T, packed block
+// ---------------------------------------------------------------------------------------------------------------------
 template <class T>
-__device__ __forceinline__ void q2_load_v(T *sV, const T *V2, long ldv, int n, int s0, int ns, int k, int nthreads) {
-    constexpr int b = TRD2_B;
-    const int w0 = s0 + 1 + k * b;
-    for (int e = threadIdx.x; e < Q2_LW * Q2_NBK; e += nthreads) {
-        const int r = e % Q2_LW, ci = e / Q2_LW;
-        const int s = s0 + ci, gr = w0 + r;
-        T v = Ops<T>::zero();
-        if (ci < ns && gr >= s + 1 + k * b && gr <= min(s + (k + 1) * b, n - 1)) v = V2[gr + (long)s * ldv];
-        sV[ci * Q2_LDV + r] = v;
-    }
-}
-
-template <class T>
-__global__ void __launch_bounds__(256) q2_tfactor_kernel(int n, const T *V2, long ldv, long sV2, const T *tau2, long sTau2,
-                                                         T *Tst, long sTst) {
+__global__ void __launch_bounds__(256) q2_pack_kernel(int n, const T *V2, long ldv, long sV2, const T *tau2, long sTau2,
+                                                      T *Pk, long sPk) {
     typedef Ops<T> O;
-    constexpr int NBK = Q2_NBK;
+    typedef Q2P<T> L;
+    constexpr int NBK = Q2_NBK, b = TRD2_B, LW = Q2_LW;
     const int I = blockIdx.x, k = blockIdx.y, item = blockIdx.z;
     const int s0 = I * NBK;
     if (k >= q2_nwin(n, s0)) return;
     const int ns = min(NBK, n - 1 - s0);
-    V2 += (long)item * sV2; tau2 += (long)item * sTau2; Tst += (long)item * sTst;
+    V2 += (long)item * sV2; tau2 += (long)item * sTau2; Pk += (long)item * sPk;
     long goff = 0;
     for (int s = 0; s < s0; s += NBK) goff += q2_nwin(n, s);
-    T *Tout = Tst + (goff + k) * NBK * NBK;
+    T *out = Pk + (goff + k) * L::BLK;
 
-    extern __shared__ __align__(16) unsigned char q2t_smem[];
-    T *sV = (T *)q2t_smem;                    // [NBK][LDV]
+    extern __shared__ __align__(16) unsigned char q2p_smem[];
+    T *sV = (T *)q2p_smem;                    // [NBK][LDV]
     __shared__ T sG[NBK][NBK + 1], sT[NBK][NBK + 1], s_tau[NBK];
     const int tid = threadIdx.x;
-    q2_load_v<T>(sV, V2, ldv, n, s0, ns, k, 256);
+    const int w0 = s0 + 1 + k * b;
+    for (int e = tid; e < NBK * L::LDV; e += 256) {
+        const int r = e % L::LDV, ci = e / L::LDV;
+        const int s = s0 + ci, gr = w0 + r;
+        T v = O::zero();
+        if (r < LW && ci < ns && gr >= s + 1 + k * b && gr <= min(s + (k + 1) * b, n - 1)) v = V2[gr + (long)s * ldv];
+        sV[e] = v;
+    }
     if (tid < NBK) s_tau[tid] = tid < ns ? tau2[(long)k * n + s0 + tid] : O::zero();
     for (int e = tid; e < NBK * NBK; e += 256) sT[e / NBK][e % NBK] = O::zero();
     __syncthreads();
@@ -71,7 +94,7 @@ __global__ void __launch_bounds__(256) q2_tfactor_kernel(int n, const T *V2, lon
     for (int e = tid; e < NBK * NBK; e += 256) {
         const int i = e % NBK, j = e / NBK;
         T s = O::zero();
-        if (i < j) for (int r = 0; r < Q2_LW; ++r) s = O::add(s, O::conj_mul(sV[i * Q2_LDV + r], sV[j * Q2_LDV + r]));
+        if (i < j) for (int r = 0; r < LW; ++r) s = O::add(s, O::conj_mul(sV[i * L::LDV + r], sV[j * L::LDV + r]));
         sG[i][j] = s;
     }
     __syncthreads();
@@ -85,7 +108,47 @@ __global__ void __launch_bounds__(256) q2_tfactor_kernel(int n, const T *V2, lon
         if (tid == i) sT[i][i] = s_tau[i];
         __syncthreads();
     }
-    for (int e = tid; e < NBK * NBK; e += 256) Tout[e] = sT[e % NBK][e / NBK];      // column-major, ld = NBK
+    for (int e = tid; e < NBK * L::LDV; e += 256) out[e] = sV[e];
+    if constexpr (L::LDVT > 0)
+        for (int e = tid; e < LW * L::LDVT; e += 256) {
+            const int ci = e % L::LDVT, r = e / L::LDVT;
+            out[L::OFF_VT + e] = ci < NBK ? sV[ci * L::LDV + r] : O::zero();
+        }
+    for (int e = tid; e < NBK * L::LDT; e += 256) {
+        const int kk = e % L::LDT, i = e / L::LDT;
+        out[L::OFF_T + e] = kk < NBK ? sT[i][kk] : O::zero();
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// mbarrier / TMA helpers
+// ---------------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "Q2_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra Q2_DONE;\n"
+        "bra Q2_WAIT;\n"
+        "Q2_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// one 1-D bulk copy global -> shared (TMA), completion counted in bytes on `bar`
+__device__ __forceinline__ void tma_load_1d(void *smem_dst, const void *gsrc, unsigned bytes, unsigned long long *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(smem_u32(smem_dst)),
+                 "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
 }
 
 __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double b) {
@@ -93,318 +156,352 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double
                  : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
-// acc (+)= A(8 x 4) B(4 x 8) for real / complex scalars; CONJA conjugates the A fragment, NEG negates it
-template <class T, bool CONJA, bool NEG> struct Frag;
-template <bool CONJA, bool NEG> struct Frag<double, CONJA, NEG> {
-    static __device__ __forceinline__ void mma(double (&acc)[4], double a, double b) {
-#ifdef Q2_SKIP_MMA
-        acc[0] += a; acc[1] += b;
-#else
-        dmma884(acc[0], acc[1], NEG ? -a : a, b);
-#endif
-    }
-};
-template <bool CONJA, bool NEG> struct Frag<cplx, CONJA, NEG> {
-    static __device__ __forceinline__ void mma(double (&acc)[4], cplx a, cplx b) {
-        double ar = NEG ? -a.x : a.x, ai = (CONJA != NEG) ? -a.y : a.y;
-        dmma884(acc[0], acc[1], ar, b.x);
-        dmma884(acc[0], acc[1], -ai, b.y);
-        dmma884(acc[2], acc[3], ar, b.y);
-        dmma884(acc[2], acc[3], ai, b.x);
-    }
-};
-template <class T> __device__ __forceinline__ T frag_out(const double (&acc)[4], int q);
-template <> __device__ __forceinline__ double frag_out<double>(const double (&acc)[4], int q) { return acc[q]; }
-template <> __device__ __forceinline__ cplx frag_out<cplx>(const double (&acc)[4], int q) { return make_double2(acc[q], acc[2 + q]); }
+// ---------------------------------------------------------------------------------------------------------------------
+// per-warp window of Z in registers.  Lane (lr = lane >> 2, lc = lane & 3) holds, for every 8-row tile t and column group
+// mt, the rows 8t + 2lc and 8t + 2lc + 1 of column 8mt + lr (the C-fragment layout with M = column, N = row).
+// ---------------------------------------------------------------------------------------------------------------------
+template <class T, int MT> struct Q2Warp;
 
-template <class T> struct Q2Cfg;
-template <> struct Q2Cfg<double> { static const int NCMAX = 32; };     // most columns of Z per CTA (shared memory)
-template <> struct Q2Cfg<cplx> { static const int NCMAX = 16; };
+template <int MT> struct Q2Warp<double, MT> {
+    typedef Q2P<double> L;
+    double z[Q2_NT][MT][2];
 
-template <class T> __device__ __forceinline__ void cp_async_elem(T *s, const T *g, bool pred) {
-    if constexpr (sizeof(T) == 16) cp_async16(s, g, pred); else cp_async8(s, g, pred);
-}
-
-// NW warps: warp & 3 selects the 8-row tile (of W: reflectors ci; of the window: rows w, w+4, w+8), warp >> 2 the slice of the
-// slab's columns (NW = 8: two slices).  DB: V and T of the NEXT diamond are fetched into a second buffer while this one is
-// applied (one CTA per SM, 8 warps, wide slab); otherwise the co-resident second CTA hides the load.
-template <class T, int NC, int NW, bool DB, bool ALIAS>
-__global__ void __launch_bounds__(NW * 32) q2_apply_kernel(int n, int ncols, const T *V2, long ldv, long sV2, const T *Tst,
-                                                           long sTst, T *Z, long ldz, long sZ) {
-    typedef Ops<T> O;
-    constexpr int b = TRD2_B, NBK = Q2_NBK, LW = Q2_LW, CS = NW / 4, NCW = NC / CS, NCT = NCW / 8, LDV = Q2_LDV, LDW = Q2_LDW,
-                  LDT = Q2Ldt<T>::value, NBUF = DB ? 2 : 1, NTH = NW * 32;
-    static_assert(NW == 4 || NW == 8, "4 or 8 warps");
-    static_assert(NC % (8 * CS) == 0 && NC % NW == 0, "slab width");
-    const int item = blockIdx.y, c0 = blockIdx.x * NC;
-    V2 += (long)item * sV2; Tst += (long)item * sTst; Z += (long)item * sZ;
-    extern __shared__ __align__(16) unsigned char q2_smem[];
-    T *sVb = (T *)q2_smem;                // [NBUF][NBK][LDV]
-    T *sZ_ = sVb + NBUF * NBK * LDV;      // [NC][LDV]   window of Z, kept across the windows of an S-block
-    T *sTb = sZ_ + NC * LDV;              // [NBUF][NBK][LDT]  T(i,k) at k*LDT + i
-    T *sW = sTb + NBUF * NBK * LDT;       // [NC][LDW]   W(ci,c) at c*LDW + ci
-    T *sW2 = ALIAS ? sW : sW + NC * LDW;  // [NC][LDW]   (ALIAS: W2 overwrites W after a barrier -- smaller footprint, 3 CTAs per SM)
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, lr = lane >> 2, lc = lane & 3;
-    const int wr = warp & 3, col0 = (warp >> 2) * NCW;
-
-    // rows [ra, LW) of the window starting at global row w0 (Lw valid rows) from global memory, zero beyond Lw.
-    // warp <-> columns c = warp, warp + NW, ...; lane <-> rows: no integer division anywhere in the window loop
-    T *const zwarp = Z + (long)(c0 + warp) * ldz;          // this warp's first column; its columns are NW apart
-    const long zstep = (long)NW * ldz;
-    auto load_z = [&](int w0, int Lw, int ra) {
-        const T *zc = zwarp + w0 + ra + lane;
-        T *sz = sZ_ + warp * LDV + ra + lane;
+    // rows [8 t0, 8 t1) of the window that starts at global row w0, straight from global memory
+    __device__ __forceinline__ void load_global(const double *Z, long ldz, int n, int ncols, int c0, int w0, int t0, int t1, int lr, int lc) {
 #pragma unroll
-        for (int jj = 0; jj < NC / NW; ++jj) {
-            const bool cok = c0 + warp + jj * NW < ncols;
+        for (int t = 0; t < Q2_NT; ++t) {
+            if (t < t0 || t >= t1) continue;
 #pragma unroll
-            for (int rr = 0; rr < LW; rr += 32) {
-                const int r = ra + rr + lane;
-                if (r < LW) {
-                    const bool ok = cok && r < Lw;
-                    cp_async_elem<T>(sz + jj * NW * LDV + rr, ok ? zc + rr : Z, ok);
+            for (int mt = 0; mt < MT; ++mt) {
+                const int c = c0 + 8 * mt + lr, r = w0 + 8 * t + 2 * lc;
+                const double *p = Z + (long)c * ldz + r;
+                z[t][mt][0] = (c < ncols && r < n) ? p[0] : 0.0;
+                z[t][mt][1] = (c < ncols && r + 1 < n) ? p[1] : 0.0;
+            }
+        }
+    }
+    // rows [0, nrows) of the window to global memory, tiles [0, t1)
+    __device__ __forceinline__ void store_global(double *Z, long ldz, int ncols, int c0, int w0, int t1, int nrows, int lr, int lc) const {
+#pragma unroll
+        for (int t = 0; t < Q2_NT; ++t) {
+            if (t >= t1) continue;
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt) {
+                const int c = c0 + 8 * mt + lr, rr = 8 * t + 2 * lc;
+                double *p = Z + (long)c * ldz + w0 + rr;
+                if (c < ncols && rr < nrows) p[0] = z[t][mt][0];
+                if (c < ncols && rr + 1 < nrows) p[1] = z[t][mt][1];
+            }
+        }
+    }
+    // staging area [column][64 rows] (ld LDS) <- global rows [g0, g0 + 64), asynchronous
+    __device__ __forceinline__ void stage_issue(double *stg, const double *Z, long ldz, int n, int ncols, int c0, int g0, int lane) const {
+#pragma unroll
+        for (int c = 0; c < 8 * MT; ++c) {
+            const double *p = Z + (long)(c0 + c) * ldz + g0;
+            const bool cok = c0 + c < ncols;
+            cp_async8(stg + c * L::LDS + lane, cok && g0 + lane < n ? p + lane : Z, cok && g0 + lane < n);
+            cp_async8(stg + c * L::LDS + 32 + lane, cok && g0 + 32 + lane < n ? p + 32 + lane : Z, cok && g0 + 32 + lane < n);
+        }
+    }
+    // slide by 64 rows: tiles 8..11 -> 0..3, tiles 4..11 <- staging
+    __device__ __forceinline__ void slide(const double *stg, int lr, int lc) {
+#pragma unroll
+        for (int t = 0; t < 4; ++t)
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt) { z[t][mt][0] = z[t + 8][mt][0]; z[t][mt][1] = z[t + 8][mt][1]; }
+#pragma unroll
+        for (int t = 4; t < Q2_NT; ++t)
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt) {
+                const double2 v = *(const double2 *)(stg + (8 * mt + lr) * L::LDS + 8 * (t - 4) + 2 * lc);
+                z[t][mt][0] = v.x; z[t][mt][1] = v.y;
+            }
+    }
+    // one diamond: blk = packed [V | Vt | T] in shared memory
+    __device__ __forceinline__ void apply(const double *blk, int lr, int lc) {
+        const double *sV = blk, *sVt = blk + L::OFF_VT, *sT = blk + L::OFF_T;
+        double w[4][MT][2], w2[4][MT][2];
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt) { w[j][mt][0] = w[j][mt][1] = 0.0; w2[j][mt][0] = w2[j][mt][1] = 0.0; }
+        // W^T = Z_w^T V : row tile t meets reflector tile j iff j <= t <= j + 8 (parallelogram)
+#pragma unroll
+        for (int t = 0; t < Q2_NT; ++t)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                if (j > t || t > j + 8) continue;
+                const double2 bv = *(const double2 *)(sV + (8 * j + lr) * L::LDV + 8 * t + 2 * lc);
+#pragma unroll
+                for (int mt = 0; mt < MT; ++mt) {
+                    dmma884(w[j][mt][0], w[j][mt][1], z[t][mt][0], bv.x);
+                    dmma884(w[j][mt][0], w[j][mt][1], z[t][mt][1], bv.y);
                 }
             }
-            zc += zstep;
+        // W2^T = W^T T^T : T upper triangular, T[i][k] != 0 for k >= i
+#pragma unroll
+        for (int ji = 0; ji < 4; ++ji)
+#pragma unroll
+            for (int u = ji; u < 4; ++u) {
+                const double2 bv = *(const double2 *)(sT + (8 * ji + lr) * L::LDT + 8 * u + 2 * lc);
+#pragma unroll
+                for (int mt = 0; mt < MT; ++mt) {
+                    dmma884(w2[ji][mt][0], w2[ji][mt][1], w[u][mt][0], bv.x);
+                    dmma884(w2[ji][mt][0], w2[ji][mt][1], w[u][mt][1], bv.y);
+                }
+            }
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt) { w2[j][mt][0] = -w2[j][mt][0]; w2[j][mt][1] = -w2[j][mt][1]; }
+        // Z_w^T -= W2^T V^T
+#pragma unroll
+        for (int t = 0; t < Q2_NT; ++t)
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                if (u > t || t > u + 8) continue;
+                const double2 bv = *(const double2 *)(sVt + (8 * t + lr) * L::LDVT + 8 * u + 2 * lc);
+#pragma unroll
+                for (int mt = 0; mt < MT; ++mt) {
+                    dmma884(z[t][mt][0], z[t][mt][1], w2[u][mt][0], bv.x);
+                    dmma884(z[t][mt][0], z[t][mt][1], w2[u][mt][1], bv.y);
+                }
+            }
+    }
+};
+
+template <int MT> struct Q2Warp<cplx, MT> {
+    static_assert(MT == 1, "complex warps own 8 columns");
+    typedef Q2P<cplx> L;
+    double zr[Q2_NT][2], zi[Q2_NT][2];
+
+    __device__ __forceinline__ void load_global(const cplx *Z, long ldz, int n, int ncols, int c0, int w0, int t0, int t1, int lr, int lc) {
+#pragma unroll
+        for (int t = 0; t < Q2_NT; ++t) {
+            if (t < t0 || t >= t1) continue;
+            const int c = c0 + lr, r = w0 + 8 * t + 2 * lc;
+            const cplx *p = Z + (long)c * ldz + r;
+            const cplx a = (c < ncols && r < n) ? p[0] : make_double2(0.0, 0.0);
+            const cplx b2 = (c < ncols && r + 1 < n) ? p[1] : make_double2(0.0, 0.0);
+            zr[t][0] = a.x; zi[t][0] = a.y; zr[t][1] = b2.x; zi[t][1] = b2.y;
         }
-    };
-    const int nsweeps = n - 1;
-    // V (masked parallelogram) and T of the diamond (s0, k), asynchronous
-    auto load_vt = [&](int buf, int s0, int k, long gidx) {
-        const int ns = min(NBK, nsweeps - s0), w0 = s0 + 1 + k * b;
-        T *sV = sVb + buf * NBK * LDV, *sT = sTb + buf * NBK * LDT;
+    }
+    __device__ __forceinline__ void store_global(cplx *Z, long ldz, int ncols, int c0, int w0, int t1, int nrows, int lr, int lc) const {
 #pragma unroll
-        for (int ci = warp; ci < NBK; ci += NW) {
-            const int s = s0 + ci;
-            const int a0 = s + 1 + k * b - w0, a1 = min(s + (k + 1) * b, n - 1) - w0;     // valid window rows of column ci
-            const T *vc = V2 + w0 + (long)s * ldv;
+        for (int t = 0; t < Q2_NT; ++t) {
+            if (t >= t1) continue;
+            const int c = c0 + lr, rr = 8 * t + 2 * lc;
+            cplx *p = Z + (long)c * ldz + w0 + rr;
+            if (c < ncols && rr < nrows) p[0] = make_double2(zr[t][0], zi[t][0]);
+            if (c < ncols && rr + 1 < nrows) p[1] = make_double2(zr[t][1], zi[t][1]);
+        }
+    }
+    __device__ __forceinline__ void stage_issue(cplx *stg, const cplx *Z, long ldz, int n, int ncols, int c0, int g0, int lane) const {
 #pragma unroll
-            for (int rr = 0; rr < LW; rr += 32) {
-                const int r = rr + lane;
-                const bool ok = ci < ns && r >= a0 && r <= a1;
-                cp_async_elem<T>(sV + ci * LDV + r, ok ? vc + r : V2, ok);
+        for (int c = 0; c < 8; ++c) {
+            const cplx *p = Z + (long)(c0 + c) * ldz + g0;
+            const bool cok = c0 + c < ncols;
+            cp_async16(stg + c * L::LDS + lane, cok && g0 + lane < n ? p + lane : Z, cok && g0 + lane < n);
+            cp_async16(stg + c * L::LDS + 32 + lane, cok && g0 + 32 + lane < n ? p + 32 + lane : Z, cok && g0 + 32 + lane < n);
+        }
+    }
+    __device__ __forceinline__ void slide(const cplx *stg, int lr, int lc) {
+#pragma unroll
+        for (int t = 0; t < 4; ++t) { zr[t][0] = zr[t + 8][0]; zr[t][1] = zr[t + 8][1]; zi[t][0] = zi[t + 8][0]; zi[t][1] = zi[t + 8][1]; }
+#pragma unroll
+        for (int t = 4; t < Q2_NT; ++t) {
+            const cplx *p = stg + lr * L::LDS + 8 * (t - 4) + 2 * lc;
+            const cplx a = p[0], b2 = p[1];
+            zr[t][0] = a.x; zi[t][0] = a.y; zr[t][1] = b2.x; zi[t][1] = b2.y;
+        }
+    }
+    __device__ __forceinline__ void apply(const cplx *blk, int lr, int lc) {
+        const cplx *sV = blk, *sT = blk + L::OFF_T;
+        double wr[4][2], wi[4][2], vr[4][2], vi[4][2];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) { wr[j][0] = wr[j][1] = wi[j][0] = wi[j][1] = 0.0; vr[j][0] = vr[j][1] = vi[j][0] = vi[j][1] = 0.0; }
+        // W^T = Z_w^T conj(V):  re += ar br + ai bi,  im += ai br - ar bi
+#pragma unroll
+        for (int t = 0; t < Q2_NT; ++t) {
+            const double nr0 = -zr[t][0], nr1 = -zr[t][1];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                if (j > t || t > j + 8) continue;
+                const cplx *bp = sV + (8 * j + lr) * L::LDV + 8 * t + 2 * lc;
+                const cplx b0 = bp[0], b1 = bp[1];
+                dmma884(wr[j][0], wr[j][1], zr[t][0], b0.x); dmma884(wr[j][0], wr[j][1], zi[t][0], b0.y);
+                dmma884(wi[j][0], wi[j][1], zi[t][0], b0.x); dmma884(wi[j][0], wi[j][1], nr0, b0.y);
+                dmma884(wr[j][0], wr[j][1], zr[t][1], b1.x); dmma884(wr[j][0], wr[j][1], zi[t][1], b1.y);
+                dmma884(wi[j][0], wi[j][1], zi[t][1], b1.x); dmma884(wi[j][0], wi[j][1], nr1, b1.y);
             }
         }
-        const T *Tg = Tst + gidx * NBK * NBK;
+        // W2^T = W^T T^T:  re += ar br - ai bi,  im += ar bi + ai br
 #pragma unroll
-        for (int e = tid; e < NBK * NBK; e += NTH) cp_async_elem<T>(sT + (e >> 5) * LDT + (e & 31), Tg + e, true);
-    };
+        for (int u = 0; u < 4; ++u) {
+            const double ni0 = -wi[u][0], ni1 = -wi[u][1];
+#pragma unroll
+            for (int ji = 0; ji < 4; ++ji) {
+                if (ji > u) continue;
+                const cplx *bp = sT + (8 * ji + lr) * L::LDT + 8 * u + 2 * lc;
+                const cplx b0 = bp[0], b1 = bp[1];
+                dmma884(vr[ji][0], vr[ji][1], wr[u][0], b0.x); dmma884(vr[ji][0], vr[ji][1], ni0, b0.y);
+                dmma884(vi[ji][0], vi[ji][1], wr[u][0], b0.y); dmma884(vi[ji][0], vi[ji][1], wi[u][0], b0.x);
+                dmma884(vr[ji][0], vr[ji][1], wr[u][1], b1.x); dmma884(vr[ji][0], vr[ji][1], ni1, b1.y);
+                dmma884(vi[ji][0], vi[ji][1], wr[u][1], b1.y); dmma884(vi[ji][0], vi[ji][1], wi[u][1], b1.x);
+            }
+        }
+        // Z_w^T -= W2^T V^T:  re += (-ar) br + ai bi,  im += (-ar) bi + (-ai) br      (V[row 8t + lr][i = 8u + 2lc (+1)])
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const double nr0 = -vr[u][0], nr1 = -vr[u][1], ni0 = -vi[u][0], ni1 = -vi[u][1];
+#pragma unroll
+            for (int t = 0; t < Q2_NT; ++t) {
+                if (u > t || t > u + 8) continue;
+                const cplx *bp = sV + (8 * u + 2 * lc) * L::LDV + 8 * t + lr;
+                const cplx b0 = bp[0], b1 = bp[L::LDV];
+                dmma884(zr[t][0], zr[t][1], nr0, b0.x); dmma884(zr[t][0], zr[t][1], vi[u][0], b0.y);
+                dmma884(zi[t][0], zi[t][1], nr0, b0.y); dmma884(zi[t][0], zi[t][1], ni0, b0.x);
+                dmma884(zr[t][0], zr[t][1], nr1, b1.x); dmma884(zr[t][0], zr[t][1], vi[u][1], b1.y);
+                dmma884(zi[t][0], zi[t][1], nr1, b1.y); dmma884(zi[t][0], zi[t][1], ni1, b1.x);
+            }
+        }
+    }
+};
 
-    const int nS = (nsweeps + NBK - 1) / NBK;
-    long goff = q2_ngroups(n);
-    int cur = 0;
-    if (DB && nS > 0) load_vt(0, (nS - 1) * NBK, 0, goff - q2_nwin(n, (nS - 1) * NBK));
+// The per-warp walk through all diamonds for one slab of 8 MT columns starting at column c0.
+template <class T, int MT>
+__device__ __forceinline__ void q2_consumer(int n, int ncols, T *Z, long ldz, int c0, const T *ring, T *stg,
+                                            unsigned long long *full, unsigned long long *empty) {
+    typedef Q2P<T> L;
+    constexpr int b = TRD2_B, NBK = Q2_NBK;
+    const int lane = threadIdx.x & 31, lr = lane >> 2, lc = lane & 3;
+    const int nsweeps = n - 1, nS = (nsweeps + NBK - 1) / NBK;
+    Q2Warp<T, MT> W;
+    unsigned d = 0;                                   // running diamond index (ring stage d & 1, phase (d >> 1) & 1)
     for (int I = nS - 1; I >= 0; --I) {
         const int s0 = I * NBK, ns = min(NBK, nsweeps - s0), nwin = q2_nwin(n, s0);
-        goff -= nwin;
-        for (int k = 0; k < nwin; ++k) {
+        for (int k = 0; k < nwin; ++k, ++d) {
             const int w0 = s0 + 1 + k * b;
-            const int Lw = min(s0 + ns - 1 + (k + 1) * b, n - 1) - w0 + 1;
-            if (!DB) load_vt(0, s0, k, goff + k);
-            if (k == 0) load_z(w0, Lw, 0);
+            const int Lw = min(s0 + ns - 1 + (k + 1) * b, n - 1) - w0 + 1;      // rows of the window the diamond touches
+            if (k == 0) {
+                __syncwarp();                         // the rows were stored by other lanes of this warp (previous S-block)
+                W.load_global(Z, ldz, n, ncols, c0, w0, 0, Q2_NT, lr, lc);
+            } else {
+                cp_async_wait<0>();
+                __syncwarp();
+                W.slide(stg, lr, lc);
+                __syncwarp();                         // everybody has read the staging area before it is refilled
+            }
+            if (k + 1 < nwin) W.stage_issue(stg, Z, ldz, n, ncols, c0, w0 + b + NBK, lane);      // rows entering at step k + 1
             cp_async_commit();
-            cp_async_wait<0>();
-            __syncthreads();
-            const T *sV = sVb + cur * NBK * LDV, *sT = sTb + cur * NBK * LDT;
-            if (DB) {
-                // the next diamond: (I, k+1), or the first one of S-block I-1
-                if (k + 1 < nwin) load_vt(cur ^ 1, s0, k + 1, goff + k + 1);
-                else if (I > 0) load_vt(cur ^ 1, s0 - NBK, 0, goff - q2_nwin(n, s0 - NBK));
-                cp_async_commit();
-                cur ^= 1;
-            }
-            // Zero structure of the parallelogram: column ci of V is non-zero only in rows ci .. ci + b - 1, so
-            //   W rows 8w..8w+7 need window rows 8w .. 8w + b + 7 only (18 of 24 k-steps), and
-            //   Z_w row tile m0 needs columns ci in [m0 - b + 1, m0 + 7]           (72 of 96 k-steps over the 12 tiles).
-            // ---- W = V^H Z_w : warp -> 8 rows (ci) x NCW columns; fragments of step k0+4 are loaded before the DMMAs of k0
-            {
-                double acc[NCT][4];
-#pragma unroll
-                for (int j = 0; j < NCT; ++j)
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) acc[j][q] = 0.0;
-                constexpr int KS1 = (b + 8) / 4;                                  // 18 k-steps
-                const T *ap = sV + (wr * 8 + lr) * LDV + lc + wr * 8;
-                const T *bp = sZ_ + (col0 + lr) * LDV + lc + wr * 8;
-                T a_c = ap[0], b_c[NCT];
-#pragma unroll
-                for (int j = 0; j < NCT; ++j) b_c[j] = bp[j * 8 * LDV];
-#pragma unroll
-                for (int ks = 0; ks < KS1; ++ks) {
-                    T a_n = a_c, b_n[NCT];
-#pragma unroll
-                    for (int j = 0; j < NCT; ++j) b_n[j] = b_c[j];
-                    if (ks + 1 < KS1) {
-                        a_n = ap[(ks + 1) * 4];
-#pragma unroll
-                        for (int j = 0; j < NCT; ++j) b_n[j] = bp[j * 8 * LDV + (ks + 1) * 4];
-                    }
-#pragma unroll
-                    for (int j = 0; j < NCT; ++j) Frag<T, true, false>::mma(acc[j], a_c, b_c[j]);
-                    a_c = a_n;
-#pragma unroll
-                    for (int j = 0; j < NCT; ++j) b_c[j] = b_n[j];
-                }
-#pragma unroll
-                for (int j = 0; j < NCT; ++j)
-#pragma unroll
-                    for (int q = 0; q < 2; ++q) sW[(col0 + j * 8 + 2 * lc + q) * LDW + wr * 8 + lr] = frag_out<T>(acc[j], q);
-            }
-            __syncthreads();
-            // ---- W2 = T W   (T upper triangular: rows 8w.. need k >= 8w)
-            {
-                double acc[NCT][4];
-#pragma unroll
-                for (int j = 0; j < NCT; ++j)
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) acc[j][q] = 0.0;
-                const T *ap = sT + lc * LDT + wr * 8 + lr;
-                const T *bp = sW + (col0 + lr) * LDW + lc;
-                for (int k0 = wr * 8; k0 < NBK; k0 += 4) {
-                    const T a = ap[k0 * LDT];
-#pragma unroll
-                    for (int j = 0; j < NCT; ++j) Frag<T, false, false>::mma(acc[j], a, bp[j * 8 * LDW + k0]);
-                }
-                if (ALIAS) __syncthreads();
-#pragma unroll
-                for (int j = 0; j < NCT; ++j)
-#pragma unroll
-                    for (int q = 0; q < 2; ++q) sW2[(col0 + j * 8 + 2 * lc + q) * LDW + wr * 8 + lr] = frag_out<T>(acc[j], q);
-            }
-            __syncthreads();
-            // ---- Z_w -= V W2 : warp -> row tiles w, w+4, w+8 (balanced: 18 k-steps per warp), in place in shared memory
-#pragma unroll
-            for (int i = 0; i < 3; ++i) {
-                const int m0 = (wr + i * 4) * 8;
-                const int klo = max(0, m0 - b + 1) / 4 * 4, khi = min(NBK, m0 + 8);    // columns ci of V that touch the tile
-                double acc[NCT][4];
-#pragma unroll
-                for (int j = 0; j < NCT; ++j)
-#pragma unroll
-                    for (int q = 0; q < 2; ++q) {
-                        const T z = sZ_[(col0 + j * 8 + 2 * lc + q) * LDV + m0 + lr];
-                        if constexpr (O::is_complex) { acc[j][q] = z.x; acc[j][2 + q] = z.y; } else { acc[j][q] = z; acc[j][2 + q] = 0.0; }
-                    }
-                const T *ap = sV + lc * LDV + m0 + lr;
-                const T *bp = sW2 + (col0 + lr) * LDW + lc;
-                T a_c = ap[klo * LDV], b_c[NCT];
-#pragma unroll
-                for (int j = 0; j < NCT; ++j) b_c[j] = bp[j * 8 * LDW + klo];
-                for (int k0 = klo; k0 < khi; k0 += 4) {
-                    T a_n = a_c, b_n[NCT];
-#pragma unroll
-                    for (int j = 0; j < NCT; ++j) b_n[j] = b_c[j];
-                    if (k0 + 4 < khi) {
-                        a_n = ap[(k0 + 4) * LDV];
-#pragma unroll
-                        for (int j = 0; j < NCT; ++j) b_n[j] = bp[j * 8 * LDW + k0 + 4];
-                    }
-#pragma unroll
-                    for (int j = 0; j < NCT; ++j) Frag<T, false, true>::mma(acc[j], a_c, b_c[j]);
-                    a_c = a_n;
-#pragma unroll
-                    for (int j = 0; j < NCT; ++j) b_c[j] = b_n[j];
-                }
-#pragma unroll
-                for (int j = 0; j < NCT; ++j)
-#pragma unroll
-                    for (int q = 0; q < 2; ++q) sZ_[(col0 + j * 8 + 2 * lc + q) * LDV + m0 + lr] = frag_out<T>(acc[j], q);
-            }
-            __syncthreads();
-            // ---- rows leaving the window go to global memory; the overlap with the next window moves to the top
+            mbar_wait(full + (d & 1), (d >> 1) & 1);
+            W.apply(ring + (size_t)(d & 1) * L::BLK, lr, lc);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty + (d & 1));
             const bool last = (k + 1 == nwin);
-            const int nout = last ? Lw : min(b, Lw);
-            if (nout == b) {
-                // the common case (b = 64 rows leave): all shared-memory reads of the warp's columns first, then the stores
-                T o0[NC / NW], o1[NC / NW];
-#pragma unroll
-                for (int jj = 0; jj < NC / NW; ++jj) {
-                    o0[jj] = sZ_[(warp + jj * NW) * LDV + lane];
-                    o1[jj] = sZ_[(warp + jj * NW) * LDV + 32 + lane];
+            if (last) W.store_global(Z, ldz, ncols, c0, w0, Q2_NT, Lw, lr, lc);
+            else W.store_global(Z, ldz, ncols, c0, w0, 8, b, lr, lc);
+        }
+    }
+    cp_async_wait<0>();
+}
+
+// n2 of the NW consumer warps own 16 columns (real only), the others 8; warp NW is the TMA producer.
+template <class T>
+__global__ void __launch_bounds__((Q2_MAXW + 1) * 32, 1) q2_apply_kernel(int n, int ncols, const T *Pk, long sPk, T *Z, long ldz, long sZ,
+                                                                         int NW, int n2) {
+    typedef Q2P<T> L;
+    constexpr int NBK = Q2_NBK;
+    const int item = blockIdx.y;
+    Pk += (long)item * sPk; Z += (long)item * sZ;
+    extern __shared__ __align__(128) unsigned char q2_smem[];
+    T *ring = (T *)q2_smem;                                              // [2][BLK]
+    T *stg_all = ring + 2 * L::BLK;                                      // [NW][CW * LDS]
+    unsigned long long *bars = (unsigned long long *)(stg_all + (size_t)NW * L::CW * L::LDS);       // full[2], empty[2]
+    unsigned long long *full = bars, *empty = bars + 2;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) {
+        mbar_init(full, 1); mbar_init(full + 1, 1);
+        mbar_init(empty, NW); mbar_init(empty + 1, NW);
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+    }
+    __syncthreads();
+    const int cols_cta = 16 * n2 + 8 * (NW - n2);
+    const int cta_c0 = blockIdx.x * cols_cta;
+    if (warp == NW) {
+        // ---- producer: diamonds in application order (I descending, k ascending), two in flight
+        if (lane == 0) {
+            const int nsweeps = n - 1, nS = (nsweeps + NBK - 1) / NBK;
+            long goff = q2_ngroups(n);
+            unsigned d = 0;
+            for (int I = nS - 1; I >= 0; --I) {
+                const int nwin = q2_nwin(n, I * NBK);
+                goff -= nwin;
+                for (int k = 0; k < nwin; ++k, ++d) {
+                    if (d >= 2) mbar_wait(empty + (d & 1), ((d >> 1) - 1) & 1);
+                    mbar_expect_tx(full + (d & 1), (unsigned)(L::BLK * sizeof(T)));
+                    tma_load_1d(ring + (size_t)(d & 1) * L::BLK, Pk + (goff + k) * L::BLK, (unsigned)(L::BLK * sizeof(T)), full + (d & 1));
                 }
-                T *zc = zwarp + w0 + lane;
-#pragma unroll
-                for (int jj = 0; jj < NC / NW; ++jj) {
-                    if (c0 + warp + jj * NW < ncols) { zc[0] = o0[jj]; zc[32] = o1[jj]; }
-                    zc += zstep;
-                }
-            } else {
-#pragma unroll
-                for (int c = warp; c < NC; c += NW) {
-                    if (c0 + c < ncols) {
-                        T *zc = Z + w0 + (long)(c0 + c) * ldz;
-                        for (int r = lane; r < nout; r += 32) zc[r] = sZ_[c * LDV + r];
-                    }
-                }
-            }
-            if (!last) {
-                const int nov = Lw - b;                      // rows shared with the next window (<= NBK - 1 <= 31)
-                T keep[NC / NW];
-#pragma unroll
-                for (int jj = 0; jj < NC / NW; ++jj)
-                    if (lane < nov) keep[jj] = sZ_[(warp + jj * NW) * LDV + b + lane];
-                __syncthreads();
-#pragma unroll
-                for (int jj = 0; jj < NC / NW; ++jj)
-                    if (lane < nov) sZ_[(warp + jj * NW) * LDV + lane] = keep[jj];
-                const int Lw2 = min(s0 + ns - 1 + (k + 2) * b, n - 1) - (w0 + b) + 1;
-                load_z(w0 + b, Lw2, nov);                    // committed and awaited with the next window's V, T
-            } else {
-                __syncthreads();
             }
         }
+        return;
+    }
+    if (warp > NW) return;
+    T *stg = stg_all + (size_t)warp * L::CW * L::LDS;
+    if constexpr (sizeof(T) == 8) {
+        if (warp < n2) q2_consumer<T, 2>(n, ncols, Z, ldz, cta_c0 + 16 * warp, ring, stg, full, empty);
+        else q2_consumer<T, 1>(n, ncols, Z, ldz, cta_c0 + 16 * n2 + 8 * (warp - n2), ring, stg, full, empty);
+    } else {
+        q2_consumer<T, 1>(n, ncols, Z, ldz, cta_c0 + 8 * warp, ring, stg, full, empty);
     }
 }
 
-size_t q2_workspace(int dtype, int n, int batch) { return align_up((size_t)batch * q2_ngroups(n) * Q2_NBK * Q2_NBK * esize(dtype)); }
-
-template <class T, int NC, int NW, bool DB, bool ALIAS>
-static int q2_launch(int n, int ncols, int batch, const T *V2, long ldv, long sV2, const T *Tst, long sTst, T *Z, long ldz, long sZ,
-                     cudaStream_t st) {
-    const size_t smem = (size_t)(((DB ? 2 : 1) * Q2_NBK + NC) * Q2_LDV + (DB ? 2 : 1) * Q2_NBK * Q2Ldt<T>::value + (ALIAS ? 1 : 2) * NC * Q2_LDW) * sizeof(T);
-    static bool attr = false;
-    if (!attr) {
-        NAO_CUDA_CHECK(cudaFuncSetAttribute(q2_apply_kernel<T, NC, NW, DB, ALIAS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr = true;
-    }
-    q2_apply_kernel<T, NC, NW, DB, ALIAS><<<dim3(ceil_div(ncols, NC), batch), NW * 32, smem, st>>>(n, ncols, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ);
-    NAO_LAUNCHED();
-    return NAO_OK;
+size_t q2_workspace(int dtype, int n, int batch) {
+    const size_t blk = dtype == NAO_COMPLEX ? (size_t)Q2P<cplx>::BLK * 16 : (size_t)Q2P<double>::BLK * 8;
+    return align_up((size_t)batch * q2_ngroups(n) * blk);
 }
 
 template <class T>
 static int q2_apply_impl(int n, int ncols, int batch, const T *V2, long ldv, long sV2, const T *tau2, T *Z, long ldz, long sZ,
                          void *work, cudaStream_t st) {
-    if (n < 2) return NAO_OK;
-    const long ng = q2_ngroups(n), sTst = ng * Q2_NBK * Q2_NBK, sTau2 = (long)hb2st_nk(n) * n;
-    T *Tst = (T *)work;
+    typedef Q2P<T> L;
+    if (n < 2 || ncols < 1) return NAO_OK;
+    const long ng = q2_ngroups(n), sPk = ng * L::BLK, sTau2 = (long)hb2st_nk(n) * n;
+    T *Pk = (T *)work;
     const int nS = ceil_div(n - 1, Q2_NBK), kmax = q2_nwin(n, 0);
-    const size_t smem_t = (size_t)Q2_NBK * Q2_LDV * sizeof(T);
-    constexpr int NCMAX = Q2Cfg<T>::NCMAX;
+    const size_t smem_p = (size_t)Q2_NBK * L::LDV * sizeof(T);
+    const size_t smem_a = (size_t)2 * L::BLK * sizeof(T) + (size_t)Q2_MAXW * L::CW * L::LDS * sizeof(T) + 64;
     static bool attr = false;
     if (!attr) {
-        NAO_CUDA_CHECK(cudaFuncSetAttribute(q2_tfactor_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_t));
+        NAO_CUDA_CHECK(cudaFuncSetAttribute(q2_pack_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p));
+        NAO_CUDA_CHECK(cudaFuncSetAttribute(q2_apply_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_a));
         attr = true;
     }
-    q2_tfactor_kernel<T><<<dim3(nS, kmax, batch), 256, smem_t, st>>>(n, V2, ldv, sV2, tau2, sTau2, Tst, sTst);
+    q2_pack_kernel<T><<<dim3(nS, kmax, batch), 256, smem_p, st>>>(n, V2, ldv, sV2, tau2, sTau2, Pk, sPk);
     NAO_LAUNCHED();
-    // every CTA walks through all diamonds for its slab of columns: with few columns (partial spectrum) narrower slabs keep
-    // all SMs busy
+    // Columns per CTA: one CTA per SM walks through all diamonds, so the slab width is what gives every SM the same share.
+    // Units of 8 columns, spread over the four schedulers of an SM: u units per scheduler as 16-column warps (real) plus at
+    // most one 8-column warp each.
     int nsm = 148, dev = 0;
     cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-    int nc = NCMAX;
-    while (nc > 8 && (long)ceil_div(ncols, nc) * batch < 2L * nsm) nc /= 2;
-    int rc;
-    // Real slabs of NCMAX columns: with W2 written over W (one more block barrier) three CTAs fit on an SM; used when two
-    // per SM would need a second round of CTAs (config 2, all columns: 416 CTAs > 2 x 148, <= 3 x 148: 117 -> 98 ms;
-    // an 8-warp CTA per SM with a 96-column slab and double-buffered V, T measured 121 ms).
-    const long ctas = (long)ceil_div(ncols, NCMAX) * batch;
-    if (nc == NCMAX && sizeof(T) == 8 && ctas > 2L * nsm)
-        rc = q2_launch<T, NCMAX, 4, false, true>(n, ncols, batch, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ, st);
-    else if (nc == NCMAX) rc = q2_launch<T, NCMAX, 4, false, false>(n, ncols, batch, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ, st);
-    else if (nc == NCMAX / 2) rc = q2_launch<T, NCMAX / 2, 4, false, false>(n, ncols, batch, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ, st);
-    else rc = q2_launch<T, 8, 4, false, false>(n, ncols, batch, V2, ldv, sV2, Tst, sTst, Z, ldz, sZ, st);
-    if (rc) return rc;
+    const long units_sm = std::max(1L, ((long)ceil_div(ncols, 8) * batch + nsm - 1) / nsm);      // 8-column units per SM
+    int NW, n2 = 0;
+    if (sizeof(T) == 8) {
+        const int u = (int)std::min(4L, (units_sm + 3) / 4);          // units per scheduler
+        if (units_sm <= 2) { NW = (int)units_sm; n2 = 0; }
+        else if (u == 1) { NW = 4; n2 = 0; }
+        else if (u == 2) { NW = 4; n2 = 4; }
+        else if (u == 3) { NW = 8; n2 = 4; }
+        else { NW = 8; n2 = 8; }
+    } else {
+        NW = (int)std::min((long)Q2_MAXW, units_sm);
+    }
+    const int cols_cta = 16 * n2 + 8 * (NW - n2);
+    const size_t smem = (size_t)2 * L::BLK * sizeof(T) + (size_t)NW * L::CW * L::LDS * sizeof(T) + 64;
+    q2_apply_kernel<T><<<dim3(ceil_div(ncols, cols_cta), batch), (NW + 1) * 32, smem, st>>>(n, ncols, Pk, sPk, Z, ldz, sZ, NW, n2);
+    NAO_LAUNCHED();
     NAO_CUDA_CHECK(cudaGetLastError());
     return NAO_OK;
 }

@@ -458,14 +458,7 @@ __global__ void __launch_bounds__(CH_NT, 1) chase_kernel(ChaseArgs<T> p) {
 }
 
 struct ChaseWork { void *AB; int *prog; int P, ipl; size_t bytes; };
-static int ch_num_sms() {
-    static int nsm = 0;
-    if (!nsm) {
-        int dev = 0; cudaGetDevice(&dev);
-        if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm <= 0) nsm = 148;
-    }
-    return nsm;
-}
+static int ch_num_sms() { return sm_count(); }
 static ChaseWork chase_plan(int dtype, int n, int batch, void *work) {
     ChaseWork w; const size_t es = esize(dtype);
     const int nsm = ch_num_sms();

@@ -121,6 +121,12 @@ def test_host_side_argument_validation(libpath):
     assert scf(dD=None) == -20 and scf(ldd=7) == -21
     assert scf(work=None) == -24 and scf(info=None) == -26
     assert scf(wb=64) == 1
+    # stream groups: the workspace query accounts for one slice per group; a batch smaller than the group count is one group
+    plain, grouped = ctypes.c_size_t(0), ctypes.c_size_t(0)
+    assert lib.nao_geneig_workspace(832, 16, 1, 0, ctypes.byref(plain)) == 0
+    assert lib.nao_geneig_workspace(832, 16, 1, 64, ctypes.byref(grouped)) == 0 and grouped.value >= plain.value
+    assert lib.nao_geneig_workspace(832, 1, 1, 96, ctypes.byref(grouped)) == 0
+    assert lib.nao_geneig_workspace(832, 1, 1, 0, ctypes.byref(plain)) == 0 and grouped.value == plain.value
     lib.nao_set_lowdin_threshold.argtypes = [ctypes.c_double]
     assert lib.nao_set_lowdin_threshold(-1e-3) == -1 and lib.nao_set_lowdin_threshold(1.0) == -1
     assert lib.nao_set_lowdin_threshold(1e-8) == 0 and lib.nao_set_lowdin_threshold(0.0) == 0

@@ -930,3 +930,41 @@ def test_padded_leading_dimensions_strides_and_side_stream(nao, pad, cplx):
         assert rc == 0
         st.synchronize()
         assert torch.equal(E, Eh0) and torch.equal(Zv, Z0) and untouched(Zb, Zv) and untouched(Ab, Av)
+
+
+# ------------------------------------------------------------------------------- concurrent mid-size solves
+@pytest.mark.parametrize("groups", ["NAO_STREAM_GROUPS_2", "NAO_STREAM_GROUPS_4", "NAO_STREAM_GROUPS_8"])
+def test_stream_groups_equal_the_single_batched_call(nao, groups):
+    """NAO_STREAM_GROUPS_*: the 16 (k, spin) items of the config-1 recipe spread over 2/4/8 internal streams (each group with
+    its share of the SMs for the grid-barrier kernels) must give what the single batched call gives.  Not bit for bit: the
+    split-K factors of the blocked Cholesky and of the panel products depend on how many items share a launch, so partial
+    sums are grouped differently; the factor of S, e, mu and D agree to a few ulps (1e-13 / 1e-12) -- with the one-stage and
+    the two-stage reduction, with the cached factor and for the partial spectrum."""
+    gflag = getattr(nao, groups)
+    for nat, extra in ((16, 0), (16, nao.NAO_TRD_TWO_STAGE), (64, 0)):
+        prob = make_config(1, nat=nat)
+        H = torch.from_numpy(prob.H).to(DEV)
+        S1 = torch.from_numpy(prob.S.copy()).to(DEV)
+        S2 = torch.from_numpy(prob.S.copy()).to(DEV)
+        E1, C1, i1 = nao.geneig(H, S1, flags=extra)
+        E2, C2, i2 = nao.geneig(H, S2, flags=extra | gflag)
+        assert int(i1.abs().max()) == 0 and int(i2.abs().max()) == 0
+        assert float((S1 - S2).abs().max()) <= 1e-13                # the factor of S
+        assert float((E1 - E2).abs().max()) <= 1e-13
+        mu1, F1 = nao.fermi_mu(E1, prob.weights, prob.n_electrons, prob.kT)
+        mu2, F2 = nao.fermi_mu(E2, prob.weights, prob.n_electrons, prob.kT)
+        assert abs(mu1 - mu2) <= 1e-13
+        D1, D2 = nao.density_matrix(C1, F1), nao.density_matrix(C2, F2)
+        assert float((D1 - D2).abs().max()) <= 1e-12
+        # later SCF step, occupied vectors only
+        nv = nao.occupied_count(F1) + 4
+        E3, C3, _ = nao.geneig(H, S1, flags=extra | nao.NAO_S_FACTORED, n_vec=nv)
+        E4, C4, _ = nao.geneig(H, S2, flags=extra | nao.NAO_S_FACTORED | gflag, n_vec=nv)
+        assert float((E3 - E4).abs().max()) <= 1e-13
+        D3, D4 = nao.density_matrix(C3, F1), nao.density_matrix(C4, F1)
+        assert float((D3 - D4).abs().max()) <= 1e-12 and float((D3 - D1).abs().max()) <= 1e-12
+        if nat == 16:                                                # against the oracle as well
+            ref = oracle.solve_problem(prob)
+            assert np.abs(E2.cpu().numpy() - ref["e"]).max() <= TOL_E and abs(mu2 - ref["mu"]) <= TOL_MU
+            for b in range(prob.batch):
+                assert np.abs(to_np(D2)[b] - ref["D"][b]).max() <= TOL_D
