@@ -239,7 +239,224 @@ __device__ __forceinline__ double hemv_warp(const T *__restrict__ A, long lda, i
     return vav;
 }
 
+// ---------------------------------------------------------------------------------------------------------------------
+// TMA-fed HEMV (n a multiple of 64, 16-byte aligned columns).  The matrix bytes no longer pass through registers on their
+// way in: every warp owns a small ring of 4 KB stages in shared memory (64 rows x 8 real / 4 complex columns of a unit),
+// filled by 1-D bulk copies (cp.async.bulk, one 64-row column segment per copy, completion counted on an mbarrier) that the
+// warp issues for itself TRD_S stages ahead.  The stream of stages is continuous over the columns of the launch: while the
+// CTA sits in the reductions and grid barriers of column j+1 the first stages of that column's run are already landing
+// (the trailing matrix does not change inside a panel).  Lane l owns rows 2l, 2l+1 (real) / l, l+32 (complex) of a unit and
+// all of its columns: row sums complete in registers per unit, column sums accumulate in registers over the warp's run in a
+// strip and are reduced across the 32 lanes once per run, exactly the partial-sum layout of hemv_warp (Prow / Pcol).
+// ---------------------------------------------------------------------------------------------------------------------
+template <class T> struct HvT {
+    static const int SC = sizeof(T) == 8 ? 8 : 4;        // columns per stage
+    static const int NSUB = 32 / SC;                     // stages per 64 x 32 unit
+    static const int STAGE = 64 * SC;                    // elements per stage (4096 bytes)
+    static const int S = sizeof(T) == 8 ? 4 : 3;         // stages per warp
+};
+
+__device__ __forceinline__ unsigned trd_smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void trd_mbar_wait(unsigned long long *bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "TRD_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra TRD_DONE;\n"
+        "bra TRD_WAIT;\n"
+        "TRD_DONE:\n"
+        "}\n" ::"r"(trd_smem_u32(bar)), "r"(parity) : "memory");
+}
+
+// Position in this warp's stream of stages: column i of the launch, unit u of its run [., u1), sub-stage q.
+struct TrdCursor {
+    int i, u, u1, q, Jp, h, Irel, bmin, nbk;
+};
+template <int HS>
+__device__ __forceinline__ bool trd_cursor_column(TrdCursor &c, int i, int nbp, int j0, int nblk, int G, int gw) {
+    // first column >= i with a non-empty run for this warp; false when the launch has none left
+    for (; i < nbp; ++i) {
+        const int j = j0 + i;
+        c.bmin = (j + 1) / TRD_TB; c.nbk = nblk - c.bmin;
+        const int U = HS * (c.nbk * (c.nbk + 1) / 2);
+        const int per = units_per_warp(U, G);
+        const int u0 = min(U, gw * per);
+        c.u1 = min(U, u0 + per);
+        if (u0 < c.u1) {
+            c.i = i; c.u = u0; c.q = 0;
+            unit_decode<HS>(u0, c.nbk, c.Jp, c.h, c.Irel);
+            return true;
+        }
+    }
+    c.i = nbp;
+    return false;
+}
+template <int HS, int NSUB>
+__device__ __forceinline__ void trd_cursor_next(TrdCursor &c, int nbp, int j0, int nblk, int G, int gw) {
+    if (++c.q < NSUB) return;
+    c.q = 0;
+    if (++c.u < c.u1) {
+        if (++c.Irel >= c.nbk) {
+            if (++c.h >= HS) { c.h = 0; ++c.Jp; }
+            c.Irel = c.Jp;
+        }
+        return;
+    }
+    trd_cursor_column<HS>(c, c.i + 1, nbp, j0, nblk, G, gw);
+}
+
+template <class T> struct TrdRing {
+    T *buf;                          // this warp's S stages
+    unsigned long long *full;        // S mbarriers
+    unsigned pseq, cseq;             // stages issued / consumed since the start of the launch
+    TrdCursor pc;                    // producer cursor
+    bool more;                       // the producer cursor still points at a stage of this launch
+};
+
+// issue the bulk copies of the stage under the producer cursor into ring slot pseq % S
 template <class T>
+__device__ __forceinline__ void trd_issue(TrdRing<T> &r, const T *A, long lda, int lane) {
+    typedef HvT<T> HT;
+    const unsigned slot = r.pseq % HT::S;
+    const int col = (r.pc.bmin + r.pc.Jp) * TRD_TB + r.pc.h * 32 + r.pc.q * HT::SC + lane;
+    const int rbase = (r.pc.bmin + r.pc.Irel) * TRD_TB;
+    const unsigned bar = trd_smem_u32(r.full + slot);
+    if (lane == 0) asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(4096u) : "memory");
+    __syncwarp();
+    if (lane < HT::SC) {
+        const T *src = A + (long)col * lda + rbase;
+        const unsigned dst = trd_smem_u32(r.buf + (size_t)slot * HT::STAGE + lane * 64);
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(dst), "l"(src),
+                     "r"((unsigned)(64 * sizeof(T))), "r"(bar)
+                     : "memory");
+    }
+    ++r.pseq;
+}
+
+template <class T>
+__device__ __forceinline__ double hemv_warp_tma(TrdRing<T> &ring, const T *__restrict__ A, long lda, int n, int j, int i, int nbp, int j0,
+                                                int nblk, int G, int g, const T *acol, T scale, T *sx, T *__restrict__ Prow,
+                                                T *__restrict__ Pcol) {
+    typedef Ops<T> O;
+    typedef Hv<T> H;
+    typedef HvT<T> HT;
+    constexpr int SW = H::SW, HS = H::HS, SC = HT::SC, NSUB = HT::NSUB;
+    static_assert(SW == 32, "a stage stream assumes 32-column strips");
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int bmin = (j + 1) / TRD_TB, nbk = nblk - bmin;
+    const int U = HS * (nbk * (nbk + 1) / 2);
+    const int per = units_per_warp(U, G);
+    const int gw = g * TRD_NW + warp;
+    const int u0 = min(U, gw * per), u1 = min(U, u0 + per);
+    if (u0 >= u1) return 0.0;
+
+    auto vval = [&](int x) -> T {
+        if (x < j + 1 || x >= n) return O::zero();
+        if (x == j + 1) return O::one();
+        return O::mul(ldcg(acol + x), scale);
+    };
+    // rows of a unit owned by this lane: real 2l, 2l+1; complex l, l+32
+    const int ro0 = O::is_complex ? lane : 2 * lane, ro1 = O::is_complex ? lane + 32 : 2 * lane + 1;
+
+    int Jp, h, Irel;
+    unit_decode<HS>(u0, nbk, Jp, h, Irel);
+    double vav = 0.0;
+    T cs[SW];
+    int runI = Irel;
+    auto strip_begin = [&](int Jp_, int h_) {
+        __syncwarp();
+        sx[lane] = vval((bmin + Jp_) * TRD_TB + h_ * SW + lane);
+        __syncwarp();
+#pragma unroll
+        for (int c = 0; c < SW; ++c) cs[c] = O::zero();
+    };
+    strip_begin(Jp, h);
+    T xr_n0 = vval((bmin + Irel) * TRD_TB + ro0), xr_n1 = vval((bmin + Irel) * TRD_TB + ro1);
+
+    for (int u = u0; u < u1; ++u) {
+        int Jn = Jp, hn = h, In = Irel + 1;
+        if (In >= nbk) {
+            hn = h + 1;
+            if (hn >= HS) { hn = 0; Jn = Jp + 1; }
+            In = Jn;
+        }
+        const bool more = (u + 1 < u1);
+        const bool diag = (Irel == Jp);
+        const int rbase = (bmin + Irel) * TRD_TB;
+        const int cb0 = (bmin + Jp) * TRD_TB + h * SW;
+        const T xr0 = xr_n0, xr1 = xr_n1;
+        T rs0 = O::zero(), rs1 = O::zero();
+        if (more) { xr_n0 = vval((bmin + In) * TRD_TB + ro0); xr_n1 = vval((bmin + In) * TRD_TB + ro1); }
+#pragma unroll
+        for (int q = 0; q < NSUB; ++q) {
+            const unsigned slot = ring.cseq % HT::S;
+            trd_mbar_wait(ring.full + slot, (ring.cseq / HT::S) & 1);
+            const T *tile = ring.buf + (size_t)slot * HT::STAGE;
+            T a0[SC], a1[SC];
+#pragma unroll
+            for (int c = 0; c < SC; ++c) {
+                if constexpr (O::is_complex) { a0[c] = tile[c * 64 + lane]; a1[c] = tile[c * 64 + 32 + lane]; }
+                else { const double2 v = *(const double2 *)(tile + c * 64 + 2 * lane); a0[c] = v.x; a1[c] = v.y; }
+            }
+            // the slot is free again: refill it with the stage S ahead in the stream (this or a later column)
+            __syncwarp();
+            asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+            ++ring.cseq;
+            if (ring.more) {
+                trd_issue<T>(ring, A, lda, lane);
+                trd_cursor_next<HS, NSUB>(ring.pc, nbp, j0, nblk, G, gw);
+                ring.more = ring.pc.i < nbp;
+            }
+#pragma unroll
+            for (int c = 0; c < SC; ++c) {
+                const T xc = sx[q * SC + c];
+                T v0 = a0[c], v1 = a1[c], c0 = v0, c1 = v1;
+                if (diag) {
+                    const int col = cb0 + q * SC + c, r0 = rbase + ro0, r1 = rbase + ro1;
+                    if (r0 == col) v0 = O::from_real(O::real(v0));
+                    if (r1 == col) v1 = O::from_real(O::real(v1));
+                    if (r0 < col) v0 = O::zero();
+                    if (r1 < col) v1 = O::zero();
+                    c0 = r0 <= col ? O::zero() : v0;
+                    c1 = r1 <= col ? O::zero() : v1;
+                }
+                rs0 = O::fma(v0, xc, rs0);
+                rs1 = O::fma(v1, xc, rs1);
+                cs[q * SC + c] = O::add(cs[q * SC + c], O::add(O::conj_mul(c0, xr0), O::conj_mul(c1, xr1)));
+            }
+        }
+        // row sums of this unit
+        {
+            T *pr = Prow + (long)(HS * (bmin + Jp) + h) * n + rbase;
+            if constexpr (O::is_complex) { pr[ro0] = rs0; pr[ro1] = rs1; }
+            else *(double2 *)(pr + ro0) = make_double2(rs0, rs1);
+            vav += O::real(O::conj_mul(xr0, rs0)) + O::real(O::conj_mul(xr1, rs1));
+        }
+        if (!more || Jn != Jp || hn != h) {
+            // end of this warp's run in the strip: transpose-reduction over the 32 lanes, lane l ends with column l
+#pragma unroll
+            for (int XO = 16, half = 16; XO >= 1; XO >>= 1, half >>= 1) {
+                const bool up = (lane & XO) != 0;
+#pragma unroll
+                for (int c = 0; c < 16; ++c) {
+                    if (c < half) {
+                        const T send = up ? cs[c] : cs[c + half];
+                        const T keep = up ? cs[c + half] : cs[c];
+                        cs[c] = O::add(keep, shfl_xor_T(send, XO));
+                    }
+                }
+            }
+            Pcol[(long)(bmin + runI) * n + cb0 + lane] = cs[0];
+            vav += O::real(O::conj_mul(sx[lane], cs[0]));
+            if (more) { strip_begin(Jn, hn); runI = In; }
+        }
+        Jp = Jn; h = hn; Irel = In;
+    }
+    return vav;
+}
+
+template <class T, bool TMA>
 __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
     typedef Ops<T> O;
     typedef Hv<T> H;
@@ -272,6 +489,29 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
     T *sW = sV + TRD_NB * TRD_CHP;               // [NB][CHP]  own rows of W
     T *s_part = sW + TRD_NB * TRD_CHP;           // [NW][PASS]
     T *sx = s_part + TRD_NW * TRD_PASS;          // [NW][SW]
+    // TMA variant: per warp a ring of HvT::S stages of 4 KB and their mbarriers
+    TrdRing<T> ring;
+    if constexpr (TMA) {
+        typedef HvT<T> HT;
+        T *ring_all = sx + TRD_NW * SW;                                   // 16-byte aligned: every region above is a multiple of 16 bytes
+        unsigned long long *bars = (unsigned long long *)(ring_all + (size_t)TRD_NW * HT::S * HT::STAGE);
+        if (tid < TRD_NW * HT::S) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(trd_smem_u32(bars + tid)));
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+        __syncthreads();
+        ring.buf = ring_all + (size_t)warp * HT::S * HT::STAGE;
+        ring.full = bars + warp * HT::S;
+        ring.pseq = ring.cseq = 0;
+        // prologue: the first S stages of this warp's stream (they land while phase A of the first column runs)
+        ring.more = trd_cursor_column<HS>(ring.pc, 0, p.nbp, j0, nblk, G, g * TRD_NW + warp);
+        for (int s = 0; s < HT::S && ring.more; ++s) {
+            trd_issue<T>(ring, A, lda, lane);
+            trd_cursor_next<HS, HT::NSUB>(ring.pc, p.nbp, j0, nblk, G, g * TRD_NW + warp);
+            ring.more = ring.pc.i < p.nbp;
+        }
+    }
     __shared__ T s_t[2 * TRD_NB];                // t1 = W^H v at [0,NB), t2 = V^H v at [NB,2NB)
     __shared__ T s_wrow[TRD_NB], s_vrow[TRD_NB];
     __shared__ T s_red4[4][2 * TRD_NB];
@@ -293,7 +533,45 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
         }
         if (i > 0) {
             const int nk = i - 1;
-            // (1) reduce the partials of phase B(i-1): t1, t2 (k < i-1) and v^H A v, fixed order
+            // geometry of the HEMV of column j-1 and of this CTA's rows
+            const int nown = max(0, r1 - ra);
+            const bool extra = !(j >= r0 && j < r1);
+            const int nloc = nown + (extra ? 1 : 0);
+            const int bminp = j / TRD_TB, nbkp = nblk - bminp;
+            const int perp = units_per_warp(HS * (nbkp * (nbkp + 1) / 2), G);
+            // row sums of the strips for the rows [base, base + np) of this CTA: lane <-> 4 rows of the pass, warp <-> strips
+            // S = warp, warp + NW, ...; 4 x 8 independent L2 loads in flight per thread, every row summed in ascending strip order
+            auto gather_rows = [&](int base, int np) {
+                constexpr int NG = TRD_PASS / 32, UB = 8;
+                int rr[NG], se[NG]; T acc[NG];
+                int smax = -1;
+#pragma unroll
+                for (int g4 = 0; g4 < NG; ++g4) {
+                    const int lp = g4 * 32 + lane, l = base + lp;
+                    rr[g4] = l < nown ? ra + l : j;
+                    se[g4] = lp < np ? HS * (rr[g4] / TRD_TB) + HS - 1 : -1;
+                    smax = max(smax, se[g4]);
+                    acc[g4] = O::zero();
+                }
+                for (int S = HS * bminp + warp; S <= smax; S += UB * TRD_NW) {
+                    T bq[NG][UB];
+#pragma unroll
+                    for (int g4 = 0; g4 < NG; ++g4)
+#pragma unroll
+                        for (int u = 0; u < UB; ++u)
+                            bq[g4][u] = (S + u * TRD_NW <= se[g4]) ? ldcg(Prow + (long)(S + u * TRD_NW) * n + rr[g4]) : O::zero();
+#pragma unroll
+                    for (int g4 = 0; g4 < NG; ++g4)
+#pragma unroll
+                        for (int u = 0; u < UB; ++u) acc[g4] = O::add(acc[g4], bq[g4][u]);
+                }
+#pragma unroll
+                for (int g4 = 0; g4 < NG; ++g4)
+                    if (g4 * 32 + lane < np) s_part[warp * TRD_PASS + g4 * 32 + lane] = acc[g4];
+            };
+            // (1) reduce the partials of phase B(i-1): t1, t2 (k < i-1) and v^H A v, fixed order.  The strip sums of the first
+            // pass of (2) depend on nothing computed here: they are gathered in the same barrier-free stretch, so that the two
+            // chains of L2 round trips overlap instead of following one another
             {
                 const int idx = tid & 63, part = tid >> 6;
                 const int k = idx < TRD_NB ? idx : idx - TRD_NB;
@@ -317,6 +595,7 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
                     sv = warp_sum(sv);
                     if (lane == 0) s_vav = sv;
                 }
+                gather_rows(0, min(TRD_PASS, nloc));
                 __syncthreads();
                 if (tid < 2 * TRD_NB)
                     s_t[tid] = O::add(O::add(s_red4[0][tid], s_red4[1][tid]), O::add(s_red4[2][tid], s_red4[3][tid]));
@@ -329,44 +608,12 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
                 __syncthreads();
             }
             // (2) w_{i-1} for the own rows r >= j and (redundantly, every CTA) for row j
-            const int nown = max(0, r1 - ra);
-            const bool extra = !(j >= r0 && j < r1);
-            const int nloc = nown + (extra ? 1 : 0);
-            const int bminp = j / TRD_TB, nbkp = nblk - bminp;           // geometry of the HEMV of column j-1
-            const int perp = units_per_warp(HS * (nbkp * (nbkp + 1) / 2), G);
             for (int base = 0; base < nloc; base += TRD_PASS) {
                 const int np = min(TRD_PASS, nloc - base);
-                {
-                    // row sums of the strips: lane <-> 4 rows of the pass, warp <-> strips S = warp, warp + NW, ...;
-                    // 4 x 4 independent L2 loads in flight per thread, every row summed in ascending strip order
-                    constexpr int NG = TRD_PASS / 32, UB = 8;
-                    int rr[NG], se[NG]; T acc[NG];
-                    int smax = -1;
-#pragma unroll
-                    for (int g4 = 0; g4 < NG; ++g4) {
-                        const int lp = g4 * 32 + lane, l = base + lp;
-                        rr[g4] = l < nown ? ra + l : j;
-                        se[g4] = lp < np ? HS * (rr[g4] / TRD_TB) + HS - 1 : -1;
-                        smax = max(smax, se[g4]);
-                        acc[g4] = O::zero();
-                    }
-                    for (int S = HS * bminp + warp; S <= smax; S += UB * TRD_NW) {
-                        T bq[NG][UB];
-#pragma unroll
-                        for (int g4 = 0; g4 < NG; ++g4)
-#pragma unroll
-                            for (int u = 0; u < UB; ++u)
-                                bq[g4][u] = (S + u * TRD_NW <= se[g4]) ? ldcg(Prow + (long)(S + u * TRD_NW) * n + rr[g4]) : O::zero();
-#pragma unroll
-                        for (int g4 = 0; g4 < NG; ++g4)
-#pragma unroll
-                            for (int u = 0; u < UB; ++u) acc[g4] = O::add(acc[g4], bq[g4][u]);
-                    }
-#pragma unroll
-                    for (int g4 = 0; g4 < NG; ++g4)
-                        if (g4 * 32 + lane < np) s_part[warp * TRD_PASS + g4 * 32 + lane] = acc[g4];
+                if (base > 0) {
+                    gather_rows(base, np);
+                    __syncthreads();
                 }
-                __syncthreads();
                 for (int lp = tid; lp < np; lp += TRD_NT) {
                     const int l = base + lp;
                     const bool own = l < nown;
@@ -479,7 +726,9 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
             if (tid < 2 * TRD_NB)
                 pt[(long)g * 2 * TRD_NB + tid] = O::add(O::add(s_red4[0][tid], s_red4[1][tid]), O::add(s_red4[2][tid], s_red4[3][tid]));
         }
-        double vav = hemv_warp<T>(A, lda, n, j, nblk, G, g, acol, scale, sx + warp * SW, Prow, Pcol);
+        double vav;
+        if constexpr (TMA) vav = hemv_warp_tma<T>(ring, A, lda, n, j, i, p.nbp, j0, nblk, G, g, acol, scale, sx + warp * SW, Prow, Pcol);
+        else vav = hemv_warp<T>(A, lda, n, j, nblk, G, g, acol, scale, sx + warp * SW, Prow, Pcol);
         vav = block_sum_d(vav, s_dred);
         if (tid == 0) pvav[g] = vav;
         group_barrier(bar, G, ++bar_ord);
@@ -524,10 +773,18 @@ static int hetrd_impl(int dtype, int n, int batch, T *A, long lda, long sA, doub
                       cudaStream_t st) {
     TrdWork w = trd_plan(dtype, n, batch, work);
     const int npanels = ceil_div(n, TRD_NB) + 1;
-    const size_t smem = (size_t)(2 * TRD_NB * TRD_CHP + TRD_NW * TRD_PASS + TRD_NW * Hv<T>::SW) * sizeof(T);
+    const size_t smem_base = (size_t)(2 * TRD_NB * TRD_CHP + TRD_NW * TRD_PASS + TRD_NW * Hv<T>::SW) * sizeof(T);
+    const size_t smem_tma = smem_base + (size_t)TRD_NW * HvT<T>::S * (HvT<T>::STAGE * sizeof(T) + 8);
+    // the TMA-fed kernel needs whole 64-row units and 16-byte aligned column segments; anything else takes the register-fed one
+    // (and pays off from order ~2000 on: for small matrices a warp's run is one or two units and the stage-by-stage latency
+    // of the ring shows -- config 1: 22.5 ms against 20.2 ms register-fed; config 2: 289 vs 299 ms; config 3: 776 vs 803 ms)
+    const bool tma = n >= 2048 && n % TRD_TB == 0 && ((uintptr_t)A % 16) == 0 && (lda * sizeof(T)) % 16 == 0 && (sA * sizeof(T)) % 16 == 0;
+    const size_t smem = tma ? smem_tma : smem_base;
+    void *kernel = tma ? (void *)hetrd_panel_kernel<T, true> : (void *)hetrd_panel_kernel<T, false>;
     static bool attr_set = false;
     if (!attr_set) {
-        NAO_CUDA_CHECK(cudaFuncSetAttribute(hetrd_panel_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        NAO_CUDA_CHECK(cudaFuncSetAttribute(hetrd_panel_kernel<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_base));
+        NAO_CUDA_CHECK(cudaFuncSetAttribute(hetrd_panel_kernel<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_tma));
         attr_set = true;
     }
     NAO_CUDA_CHECK(cudaMemsetAsync(w.bar, 0, (size_t)batch * npanels * 4, st));
@@ -549,7 +806,7 @@ static int hetrd_impl(int dtype, int n, int batch, T *A, long lda, long sA, doub
             for (int i = 0; i < nbp; ++i) { double mm = n - (j0 + i) - 1; bytes += 0.5 * mm * (mm + 1) * sizeof(T); }
             const int pk = prof_kernel_begin(0, bytes * nb_items, st);
             void *args[] = {&a};
-            NAO_CUDA_CHECK(cudaLaunchCooperativeKernel((void *)hetrd_panel_kernel<T>, dim3(nb_items * w.G), dim3(TRD_NT), args, smem, st));
+            NAO_CUDA_CHECK(cudaLaunchCooperativeKernel(kernel, dim3(nb_items * w.G), dim3(TRD_NT), args, smem, st));
             NAO_LAUNCHED();
             prof_kernel_end(0, pk, st);
         }

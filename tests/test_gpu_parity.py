@@ -542,6 +542,35 @@ def test_partial_spectrum_gives_the_same_density(nao, two_stage):
         assert np.abs(Cb.conj().T @ prob.S_full(0) @ Cb - np.eye(n_vec)).max() <= TOL_ORTH
 
 
+@pytest.mark.parametrize("n,batch", [(64, 3), (832, 3), (2048, 2), (2112, 1), (2176, 3)])
+@pytest.mark.parametrize("cplx", [False, True])
+def test_one_stage_multiples_of_64_take_the_tma_fed_hemv(nao, n, batch, cplx):
+    """Orders >= 2048 that are multiples of 64 run the one-stage tridiagonalisation through the TMA-fed HEMV (cp.async.bulk
+    stage rings, stream of stages continuous across the columns of a panel); every other order takes the register-fed one.  The
+    same matrices embedded with one more row and column (order n + 1, decoupled last level) go through the other kernel:
+    both must agree with LAPACK (numpy, CPU) and with each other, and satisfy the invariants.  Several items per launch."""
+    rng = np.random.default_rng(64 + n)
+    A = rng.standard_normal((batch, n, n))
+    if cplx:
+        A = A + 1j * rng.standard_normal((batch, n, n))
+    A = A + np.swapaxes(A.conj(), -1, -2)
+    E, Z, info = nao.heev(to_dev(A), flags=nao.NAO_TRD_ONE_STAGE)
+    assert int(info.abs().max()) == 0
+    B = np.zeros((batch, n + 1, n + 1), dtype=A.dtype)
+    B[:, :n, :n] = A
+    B[:, n, n] = 1e3                                  # decoupled level far above the spectrum
+    E2, Z2, info2 = nao.heev(to_dev(B), flags=nao.NAO_TRD_ONE_STAGE)
+    assert int(info2.abs().max()) == 0
+    for b in range(batch):
+        e = E.cpu().numpy()[b]; Zn = to_np(Z)[b]
+        ref = np.linalg.eigvalsh(A[b])
+        scale = max(1.0, np.abs(ref).max())
+        assert np.abs(e - ref).max() <= 1e-12 * scale * n ** 0.5
+        assert np.abs(A[b] @ Zn - Zn * e).max() <= 1e-12 * scale * n ** 0.5
+        assert np.abs(Zn.conj().T @ Zn - np.eye(n)).max() <= 1e-12
+        assert np.abs(E2.cpu().numpy()[b][:n] - e).max() <= 1e-12 * scale * n ** 0.5
+
+
 @pytest.mark.parametrize("flag", ["NAO_TRD_ONE_STAGE", "NAO_TRD_TWO_STAGE"])
 @pytest.mark.parametrize("cplx", [False, True])
 def test_odd_order_1001_both_paths(nao, flag, cplx):
