@@ -33,7 +33,6 @@ namespace nao {
 static const int Q2_NBK = 32;                 // sweeps per diamond
 static const int Q2_LW = 96;                  // window rows (>= TRD2_B + Q2_NBK - 1), 12 tiles of 8
 static const int Q2_NT = Q2_LW / 8;
-static const int Q2_MAXW = 9;                 // most consumer warps per CTA
 
 // Packed diamond (elements of T).  Leading dimensions make every fragment load conflict free:
 //   real:    16-byte loads of (k, k+1) pairs, quarter-warp = 2 rows x 4 pairs  ->  ld = 8 mod 16
@@ -398,18 +397,26 @@ __device__ __forceinline__ void q2_consumer(int n, int ncols, T *Z, long ldz, in
             mbar_wait(full + (d & 1), (d >> 1) & 1);
             W.apply(ring + (size_t)(d & 1) * L::BLK, lr, lc);
             __syncwarp();
+            // The refill of this ring stage is a write through the async proxy (TMA); the fragment loads above went through
+            // the generic proxy.  Without a proxy fence before the release nothing orders the two: with nine warps per CTA
+            // (config 3) a refill now and then overtook the last reads of the warp that runs ahead of the others.
+            asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
             if (lane == 0) mbar_arrive(empty + (d & 1));
             const bool last = (k + 1 == nwin);
-            if (last) W.store_global(Z, ldz, ncols, c0, w0, Q2_NT, Lw, lr, lc);
-            else W.store_global(Z, ldz, ncols, c0, w0, 8, b, lr, lc);
+            if (last) {
+                W.store_global(Z, ldz, ncols, c0, w0, Q2_NT, Lw, lr, lc);
+            } else {
+                W.store_global(Z, ldz, ncols, c0, w0, 8, b, lr, lc);
+            }
         }
     }
     cp_async_wait<0>();
 }
 
 // n2 of the NW consumer warps own 16 columns (real only), the others 8; warp NW is the TMA producer.
-template <class T>
-__global__ void __launch_bounds__((Q2_MAXW + 1) * 32, 1) q2_apply_kernel(int n, int ncols, const T *Pk, long sPk, T *Z, long ldz, long sZ,
+// MAXW = most consumer warps (bounds the registers per thread); MT2 = 16-column warps allowed (real only).
+template <class T, int MAXW, bool MT2>
+__global__ void __launch_bounds__((MAXW + 1) * 32, 1) q2_apply_kernel(int n, int ncols, const T *Pk, long sPk, T *Z, long ldz, long sZ,
                                                                          int NW, int n2) {
     typedef Q2P<T> L;
     constexpr int NBK = Q2_NBK;
@@ -417,8 +424,9 @@ __global__ void __launch_bounds__((Q2_MAXW + 1) * 32, 1) q2_apply_kernel(int n, 
     Pk += (long)item * sPk; Z += (long)item * sZ;
     extern __shared__ __align__(128) unsigned char q2_smem[];
     T *ring = (T *)q2_smem;                                              // [2][BLK]
-    T *stg_all = ring + 2 * L::BLK;                                      // [NW][CW * LDS]
-    unsigned long long *bars = (unsigned long long *)(stg_all + (size_t)NW * L::CW * L::LDS);       // full[2], empty[2]
+    constexpr int CWS = (sizeof(T) == 8 && MT2) ? 16 : 8;                // columns of a warp's staging area
+    T *stg_all = ring + 2 * L::BLK;                                      // [NW][CWS * LDS]
+    unsigned long long *bars = (unsigned long long *)(stg_all + (size_t)NW * CWS * L::LDS);       // full[2], empty[2]
     unsigned long long *full = bars, *empty = bars + 2;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
@@ -449,8 +457,8 @@ __global__ void __launch_bounds__((Q2_MAXW + 1) * 32, 1) q2_apply_kernel(int n, 
         return;
     }
     if (warp > NW) return;
-    T *stg = stg_all + (size_t)warp * L::CW * L::LDS;
-    if constexpr (sizeof(T) == 8) {
+    T *stg = stg_all + (size_t)warp * CWS * L::LDS;
+    if constexpr (sizeof(T) == 8 && MT2) {
         if (warp < n2) q2_consumer<T, 2>(n, ncols, Z, ldz, cta_c0 + 16 * warp, ring, stg, full, empty);
         else q2_consumer<T, 1>(n, ncols, Z, ldz, cta_c0 + 16 * n2 + 8 * (warp - n2), ring, stg, full, empty);
     } else {
@@ -472,11 +480,9 @@ static int q2_apply_impl(int n, int ncols, int batch, const T *V2, long ldv, lon
     T *Pk = (T *)work;
     const int nS = ceil_div(n - 1, Q2_NBK), kmax = q2_nwin(n, 0);
     const size_t smem_p = (size_t)Q2_NBK * L::LDV * sizeof(T);
-    const size_t smem_a = (size_t)2 * L::BLK * sizeof(T) + (size_t)Q2_MAXW * L::CW * L::LDS * sizeof(T) + 64;
     static bool attr = false;
     if (!attr) {
         NAO_CUDA_CHECK(cudaFuncSetAttribute(q2_pack_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p));
-        NAO_CUDA_CHECK(cudaFuncSetAttribute(q2_apply_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_a));
         attr = true;
     }
     q2_pack_kernel<T><<<dim3(nS, kmax, batch), 256, smem_p, st>>>(n, V2, ldv, sV2, tau2, sTau2, Pk, sPk);
@@ -488,19 +494,40 @@ static int q2_apply_impl(int n, int ncols, int batch, const T *V2, long ldv, lon
     cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
     const long units_sm = std::max(1L, ((long)ceil_div(ncols, 8) * batch + nsm - 1) / nsm);      // 8-column units per SM
     int NW, n2 = 0;
+    bool wide = false;                                               // 12 eight-column warps (three per scheduler)
     if (sizeof(T) == 8) {
         const int u = (int)std::min(4L, (units_sm + 3) / 4);          // units per scheduler
         if (units_sm <= 2) { NW = (int)units_sm; n2 = 0; }
         else if (u == 1) { NW = 4; n2 = 0; }
         else if (u == 2) { NW = 4; n2 = 4; }
-        else if (u == 3) { NW = 8; n2 = 4; }
+        else if (u == 3) { NW = 12; n2 = 0; wide = true; }
         else { NW = 8; n2 = 8; }
     } else {
-        NW = (int)std::min((long)Q2_MAXW, units_sm);
+        NW = (int)std::min(9L, units_sm);
     }
     const int cols_cta = 16 * n2 + 8 * (NW - n2);
-    const size_t smem = (size_t)2 * L::BLK * sizeof(T) + (size_t)NW * L::CW * L::LDS * sizeof(T) + 64;
-    q2_apply_kernel<T><<<dim3(ceil_div(ncols, cols_cta), batch), (NW + 1) * 32, smem, st>>>(n, ncols, Pk, sPk, Z, ldz, sZ, NW, n2);
+    const int cws = (sizeof(T) == 8 && !wide) ? 16 : 8;               // staging columns per warp (kernel's CWS)
+    const size_t smem = (size_t)2 * L::BLK * sizeof(T) + (size_t)NW * cws * L::LDS * sizeof(T) + 64;
+    const dim3 grid(ceil_div(ncols, cols_cta), batch);
+    // (kernel instantiations share one function-pointer type: the attribute flag is kept per instantiation, not per lambda)
+    auto launch = [&](auto kernel, int maxw, bool &attr_set) -> int {
+        if (!attr_set) {
+            const size_t smem_max = (size_t)2 * L::BLK * sizeof(T) + (size_t)maxw * cws * L::LDS * sizeof(T) + 64;
+            NAO_CUDA_CHECK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max));
+            attr_set = true;
+        }
+        kernel<<<grid, (NW + 1) * 32, smem, st>>>(n, ncols, Pk, sPk, Z, ldz, sZ, NW, n2);
+        return NAO_OK;
+    };
+    static bool set_wide = false, set_mixed = false, set_cplx = false;
+    int rc;
+    if constexpr (sizeof(T) == 8) {
+        if (wide) rc = launch(q2_apply_kernel<T, 12, false>, 12, set_wide);
+        else rc = launch(q2_apply_kernel<T, 8, true>, 8, set_mixed);
+    } else {
+        rc = launch(q2_apply_kernel<T, 9, false>, 9, set_cplx);
+    }
+    if (rc) return rc;
     NAO_LAUNCHED();
     NAO_CUDA_CHECK(cudaGetLastError());
     return NAO_OK;

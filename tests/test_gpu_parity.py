@@ -997,3 +997,40 @@ def test_stream_groups_equal_the_single_batched_call(nao, groups):
             assert np.abs(E2.cpu().numpy() - ref["e"]).max() <= TOL_E and abs(mu2 - ref["mu"]) <= TOL_MU
             for b in range(prob.batch):
                 assert np.abs(to_np(D2)[b] - ref["D"][b]).max() <= TOL_D
+
+
+# ------------------------------------------------------------------------------- flag-synchronised kernels: reproducibility
+@pytest.mark.parametrize("cplx", [False, True])
+def test_flag_synchronised_kernels_are_bit_reproducible(nao, cplx):
+    """hetrd_panel_kernel / panel_qr_kernel (software grid barrier), chase_kernel (acquire/release progress counters between
+    CTAs), q2_apply_kernel (mbarrier ring, per-warp staging) and the TMA-fed HEMV synchronise through flags in global or
+    shared memory.  compute-sanitizer is closed on this pool, so a missing acquire, release or barrier is looked for the
+    other way: every cross-CTA reduction sums partial results in a fixed order, hence any run of the same input must give
+    the same bits; a race shows up as a difference between repetitions.  Eight repetitions of both reductions on three
+    sizes (several items per launch, ragged and 64-aligned orders), with other work queued in between to vary the timing."""
+    rng = np.random.default_rng(77)
+    # the last size is config 3's (complex) / config 2's (real): the widest launch of q2_apply_kernel, nine / twelve consumer
+    # warps per CTA -- where a missing proxy fence between the fragment loads and the TMA refill of a ring stage showed up as
+    # a handful of wrong columns in most runs, and nowhere else
+    for n, batch in ((333, 3), (832, 4), (2176, 2), (9984 if cplx else 6656, 1 if cplx else 2)):
+        if n > 4000:
+            g = torch.Generator(device=DEV); g.manual_seed(n)
+            A = torch.randn(batch, n, n, dtype=torch.float64, device=DEV, generator=g)
+            if cplx:
+                A = torch.complex(A, torch.randn(batch, n, n, dtype=torch.float64, device=DEV, generator=g))
+            A = A + A.mH
+        else:
+            A = rng.standard_normal((batch, n, n))
+            if cplx:
+                A = A + 1j * rng.standard_normal((batch, n, n))
+            A = to_dev(A + np.swapaxes(A.conj(), -1, -2))
+        for flag in (nao.NAO_TRD_ONE_STAGE, nao.NAO_TRD_TWO_STAGE):
+            if n > 4000 and flag == nao.NAO_TRD_ONE_STAGE:
+                continue
+            E0, Z0, info = nao.heev(A.clone(), flags=flag)
+            assert int(info.abs().max()) == 0
+            for rep in range(7):
+                if rep % 2:
+                    torch.empty(64 << 20, dtype=torch.uint8, device=DEV).zero_()
+                E, Z, _ = nao.heev(A.clone(), flags=flag)
+                assert torch.equal(E, E0) and torch.equal(Z, Z0), (n, flag, rep)
