@@ -533,45 +533,7 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
         }
         if (i > 0) {
             const int nk = i - 1;
-            // geometry of the HEMV of column j-1 and of this CTA's rows
-            const int nown = max(0, r1 - ra);
-            const bool extra = !(j >= r0 && j < r1);
-            const int nloc = nown + (extra ? 1 : 0);
-            const int bminp = j / TRD_TB, nbkp = nblk - bminp;
-            const int perp = units_per_warp(HS * (nbkp * (nbkp + 1) / 2), G);
-            // row sums of the strips for the rows [base, base + np) of this CTA: lane <-> 4 rows of the pass, warp <-> strips
-            // S = warp, warp + NW, ...; 4 x 8 independent L2 loads in flight per thread, every row summed in ascending strip order
-            auto gather_rows = [&](int base, int np) {
-                constexpr int NG = TRD_PASS / 32, UB = 8;
-                int rr[NG], se[NG]; T acc[NG];
-                int smax = -1;
-#pragma unroll
-                for (int g4 = 0; g4 < NG; ++g4) {
-                    const int lp = g4 * 32 + lane, l = base + lp;
-                    rr[g4] = l < nown ? ra + l : j;
-                    se[g4] = lp < np ? HS * (rr[g4] / TRD_TB) + HS - 1 : -1;
-                    smax = max(smax, se[g4]);
-                    acc[g4] = O::zero();
-                }
-                for (int S = HS * bminp + warp; S <= smax; S += UB * TRD_NW) {
-                    T bq[NG][UB];
-#pragma unroll
-                    for (int g4 = 0; g4 < NG; ++g4)
-#pragma unroll
-                        for (int u = 0; u < UB; ++u)
-                            bq[g4][u] = (S + u * TRD_NW <= se[g4]) ? ldcg(Prow + (long)(S + u * TRD_NW) * n + rr[g4]) : O::zero();
-#pragma unroll
-                    for (int g4 = 0; g4 < NG; ++g4)
-#pragma unroll
-                        for (int u = 0; u < UB; ++u) acc[g4] = O::add(acc[g4], bq[g4][u]);
-                }
-#pragma unroll
-                for (int g4 = 0; g4 < NG; ++g4)
-                    if (g4 * 32 + lane < np) s_part[warp * TRD_PASS + g4 * 32 + lane] = acc[g4];
-            };
-            // (1) reduce the partials of phase B(i-1): t1, t2 (k < i-1) and v^H A v, fixed order.  The strip sums of the first
-            // pass of (2) depend on nothing computed here: they are gathered in the same barrier-free stretch, so that the two
-            // chains of L2 round trips overlap instead of following one another
+            // (1) reduce the partials of phase B(i-1): t1, t2 (k < i-1) and v^H A v, fixed order
             {
                 const int idx = tid & 63, part = tid >> 6;
                 const int k = idx < TRD_NB ? idx : idx - TRD_NB;
@@ -595,7 +557,6 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
                     sv = warp_sum(sv);
                     if (lane == 0) s_vav = sv;
                 }
-                gather_rows(0, min(TRD_PASS, nloc));
                 __syncthreads();
                 if (tid < 2 * TRD_NB)
                     s_t[tid] = O::add(O::add(s_red4[0][tid], s_red4[1][tid]), O::add(s_red4[2][tid], s_red4[3][tid]));
@@ -608,12 +569,44 @@ __global__ void __launch_bounds__(TRD_NT, 1) hetrd_panel_kernel(TrdArgs<T> p) {
                 __syncthreads();
             }
             // (2) w_{i-1} for the own rows r >= j and (redundantly, every CTA) for row j
+            const int nown = max(0, r1 - ra);
+            const bool extra = !(j >= r0 && j < r1);
+            const int nloc = nown + (extra ? 1 : 0);
+            const int bminp = j / TRD_TB, nbkp = nblk - bminp;           // geometry of the HEMV of column j-1
+            const int perp = units_per_warp(HS * (nbkp * (nbkp + 1) / 2), G);
             for (int base = 0; base < nloc; base += TRD_PASS) {
                 const int np = min(TRD_PASS, nloc - base);
-                if (base > 0) {
-                    gather_rows(base, np);
-                    __syncthreads();
+                {
+                    // row sums of the strips: lane <-> 4 rows of the pass, warp <-> strips S = warp, warp + NW, ...;
+                    // 4 x 4 independent L2 loads in flight per thread, every row summed in ascending strip order
+                    constexpr int NG = TRD_PASS / 32, UB = 8;
+                    int rr[NG], se[NG]; T acc[NG];
+                    int smax = -1;
+#pragma unroll
+                    for (int g4 = 0; g4 < NG; ++g4) {
+                        const int lp = g4 * 32 + lane, l = base + lp;
+                        rr[g4] = l < nown ? ra + l : j;
+                        se[g4] = lp < np ? HS * (rr[g4] / TRD_TB) + HS - 1 : -1;
+                        smax = max(smax, se[g4]);
+                        acc[g4] = O::zero();
+                    }
+                    for (int S = HS * bminp + warp; S <= smax; S += UB * TRD_NW) {
+                        T bq[NG][UB];
+#pragma unroll
+                        for (int g4 = 0; g4 < NG; ++g4)
+#pragma unroll
+                            for (int u = 0; u < UB; ++u)
+                                bq[g4][u] = (S + u * TRD_NW <= se[g4]) ? ldcg(Prow + (long)(S + u * TRD_NW) * n + rr[g4]) : O::zero();
+#pragma unroll
+                        for (int g4 = 0; g4 < NG; ++g4)
+#pragma unroll
+                            for (int u = 0; u < UB; ++u) acc[g4] = O::add(acc[g4], bq[g4][u]);
+                    }
+#pragma unroll
+                    for (int g4 = 0; g4 < NG; ++g4)
+                        if (g4 * 32 + lane < np) s_part[warp * TRD_PASS + g4 * 32 + lane] = acc[g4];
                 }
+                __syncthreads();
                 for (int lp = tid; lp < np; lp += TRD_NT) {
                     const int l = base + lp;
                     const bool own = l < nown;

@@ -225,48 +225,73 @@ template <int MT> struct Q2Warp<double, MT> {
         for (int j = 0; j < 4; ++j)
 #pragma unroll
             for (int mt = 0; mt < MT; ++mt) { w[j][mt][0] = w[j][mt][1] = 0.0; w2[j][mt][0] = w2[j][mt][1] = 0.0; }
+        // B fragments are fetched one step ahead of the DMMAs that use them (explicit double buffering: the compiler places a
+        // shared-memory load right in front of its first use otherwise, and two or three warps per scheduler do not cover it)
         // W^T = Z_w^T V : row tile t meets reflector tile j iff j <= t <= j + 8 (parallelogram)
+        {
+            double2 bc[4], bn[4];
+            bc[0] = *(const double2 *)(sV + lr * L::LDV + 2 * lc);
 #pragma unroll
-        for (int t = 0; t < Q2_NT; ++t)
+            for (int t = 0; t < Q2_NT; ++t) {
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                if (j > t || t > j + 8) continue;
-                const double2 bv = *(const double2 *)(sV + (8 * j + lr) * L::LDV + 8 * t + 2 * lc);
+                for (int j = 0; j < 4; ++j)
+                    if (t + 1 < Q2_NT && j <= t + 1 && t + 1 <= j + 8) bn[j] = *(const double2 *)(sV + (8 * j + lr) * L::LDV + 8 * (t + 1) + 2 * lc);
 #pragma unroll
-                for (int mt = 0; mt < MT; ++mt) {
-                    dmma884(w[j][mt][0], w[j][mt][1], z[t][mt][0], bv.x);
-                    dmma884(w[j][mt][0], w[j][mt][1], z[t][mt][1], bv.y);
+                for (int j = 0; j < 4; ++j) {
+                    if (j > t || t > j + 8) continue;
+#pragma unroll
+                    for (int mt = 0; mt < MT; ++mt) {
+                        dmma884(w[j][mt][0], w[j][mt][1], z[t][mt][0], bc[j].x);
+                        dmma884(w[j][mt][0], w[j][mt][1], z[t][mt][1], bc[j].y);
+                    }
                 }
+#pragma unroll
+                for (int j = 0; j < 4; ++j) bc[j] = bn[j];
             }
+        }
         // W2^T = W^T T^T : T upper triangular, T[i][k] != 0 for k >= i
+        {
+            double2 bt[4][4];
 #pragma unroll
-        for (int ji = 0; ji < 4; ++ji)
+            for (int ji = 0; ji < 4; ++ji)
 #pragma unroll
-            for (int u = ji; u < 4; ++u) {
-                const double2 bv = *(const double2 *)(sT + (8 * ji + lr) * L::LDT + 8 * u + 2 * lc);
+                for (int u = ji; u < 4; ++u) bt[ji][u] = *(const double2 *)(sT + (8 * ji + lr) * L::LDT + 8 * u + 2 * lc);
 #pragma unroll
-                for (int mt = 0; mt < MT; ++mt) {
-                    dmma884(w2[ji][mt][0], w2[ji][mt][1], w[u][mt][0], bv.x);
-                    dmma884(w2[ji][mt][0], w2[ji][mt][1], w[u][mt][1], bv.y);
-                }
-            }
+            for (int ji = 0; ji < 4; ++ji)
+#pragma unroll
+                for (int u = ji; u < 4; ++u)
+#pragma unroll
+                    for (int mt = 0; mt < MT; ++mt) {
+                        dmma884(w2[ji][mt][0], w2[ji][mt][1], w[u][mt][0], bt[ji][u].x);
+                        dmma884(w2[ji][mt][0], w2[ji][mt][1], w[u][mt][1], bt[ji][u].y);
+                    }
+        }
 #pragma unroll
         for (int j = 0; j < 4; ++j)
 #pragma unroll
             for (int mt = 0; mt < MT; ++mt) { w2[j][mt][0] = -w2[j][mt][0]; w2[j][mt][1] = -w2[j][mt][1]; }
         // Z_w^T -= W2^T V^T
+        {
+            double2 bc[4], bn[4];
+            bc[0] = *(const double2 *)(sVt + lr * L::LDVT + 2 * lc);
 #pragma unroll
-        for (int t = 0; t < Q2_NT; ++t)
+            for (int t = 0; t < Q2_NT; ++t) {
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                if (u > t || t > u + 8) continue;
-                const double2 bv = *(const double2 *)(sVt + (8 * t + lr) * L::LDVT + 8 * u + 2 * lc);
+                for (int u = 0; u < 4; ++u)
+                    if (t + 1 < Q2_NT && u <= t + 1 && t + 1 <= u + 8) bn[u] = *(const double2 *)(sVt + (8 * (t + 1) + lr) * L::LDVT + 8 * u + 2 * lc);
 #pragma unroll
-                for (int mt = 0; mt < MT; ++mt) {
-                    dmma884(z[t][mt][0], z[t][mt][1], w2[u][mt][0], bv.x);
-                    dmma884(z[t][mt][0], z[t][mt][1], w2[u][mt][1], bv.y);
+                for (int u = 0; u < 4; ++u) {
+                    if (u > t || t > u + 8) continue;
+#pragma unroll
+                    for (int mt = 0; mt < MT; ++mt) {
+                        dmma884(z[t][mt][0], z[t][mt][1], w2[u][mt][0], bc[u].x);
+                        dmma884(z[t][mt][0], z[t][mt][1], w2[u][mt][1], bc[u].y);
+                    }
                 }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) bc[u] = bn[u];
             }
+        }
     }
 };
 
@@ -320,30 +345,46 @@ template <int MT> struct Q2Warp<cplx, MT> {
         double wr[4][2], wi[4][2], vr[4][2], vi[4][2];
 #pragma unroll
         for (int j = 0; j < 4; ++j) { wr[j][0] = wr[j][1] = wi[j][0] = wi[j][1] = 0.0; vr[j][0] = vr[j][1] = vi[j][0] = vi[j][1] = 0.0; }
+        // (B fragments one step ahead of their DMMAs, as in the real case)
         // W^T = Z_w^T conj(V):  re += ar br + ai bi,  im += ai br - ar bi
+        {
+            cplx c0[4], c1[4], n0[4], n1[4];
+            { const cplx *bp = sV + lr * L::LDV + 2 * lc; c0[0] = bp[0]; c1[0] = bp[1]; }
 #pragma unroll
-        for (int t = 0; t < Q2_NT; ++t) {
-            const double nr0 = -zr[t][0], nr1 = -zr[t][1];
+            for (int t = 0; t < Q2_NT; ++t) {
+                const double nr0 = -zr[t][0], nr1 = -zr[t][1];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                if (j > t || t > j + 8) continue;
-                const cplx *bp = sV + (8 * j + lr) * L::LDV + 8 * t + 2 * lc;
-                const cplx b0 = bp[0], b1 = bp[1];
-                dmma884(wr[j][0], wr[j][1], zr[t][0], b0.x); dmma884(wr[j][0], wr[j][1], zi[t][0], b0.y);
-                dmma884(wi[j][0], wi[j][1], zi[t][0], b0.x); dmma884(wi[j][0], wi[j][1], nr0, b0.y);
-                dmma884(wr[j][0], wr[j][1], zr[t][1], b1.x); dmma884(wr[j][0], wr[j][1], zi[t][1], b1.y);
-                dmma884(wi[j][0], wi[j][1], zi[t][1], b1.x); dmma884(wi[j][0], wi[j][1], nr1, b1.y);
+                for (int j = 0; j < 4; ++j)
+                    if (t + 1 < Q2_NT && j <= t + 1 && t + 1 <= j + 8) {
+                        const cplx *bp = sV + (8 * j + lr) * L::LDV + 8 * (t + 1) + 2 * lc;
+                        n0[j] = bp[0]; n1[j] = bp[1];
+                    }
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    if (j > t || t > j + 8) continue;
+                    const cplx b0 = c0[j], b1 = c1[j];
+                    dmma884(wr[j][0], wr[j][1], zr[t][0], b0.x); dmma884(wr[j][0], wr[j][1], zi[t][0], b0.y);
+                    dmma884(wi[j][0], wi[j][1], zi[t][0], b0.x); dmma884(wi[j][0], wi[j][1], nr0, b0.y);
+                    dmma884(wr[j][0], wr[j][1], zr[t][1], b1.x); dmma884(wr[j][0], wr[j][1], zi[t][1], b1.y);
+                    dmma884(wi[j][0], wi[j][1], zi[t][1], b1.x); dmma884(wi[j][0], wi[j][1], nr1, b1.y);
+                }
+#pragma unroll
+                for (int j = 0; j < 4; ++j) { c0[j] = n0[j]; c1[j] = n1[j]; }
             }
         }
         // W2^T = W^T T^T:  re += ar br - ai bi,  im += ar bi + ai br
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
             const double ni0 = -wi[u][0], ni1 = -wi[u][1];
+            cplx t0[4], t1[4];
 #pragma unroll
-            for (int ji = 0; ji < 4; ++ji) {
-                if (ji > u) continue;
+            for (int ji = 0; ji <= u; ++ji) {
                 const cplx *bp = sT + (8 * ji + lr) * L::LDT + 8 * u + 2 * lc;
-                const cplx b0 = bp[0], b1 = bp[1];
+                t0[ji] = bp[0]; t1[ji] = bp[1];
+            }
+#pragma unroll
+            for (int ji = 0; ji <= u; ++ji) {
+                const cplx b0 = t0[ji], b1 = t1[ji];
                 dmma884(vr[ji][0], vr[ji][1], wr[u][0], b0.x); dmma884(vr[ji][0], vr[ji][1], ni0, b0.y);
                 dmma884(vi[ji][0], vi[ji][1], wr[u][0], b0.y); dmma884(vi[ji][0], vi[ji][1], wi[u][0], b0.x);
                 dmma884(vr[ji][0], vr[ji][1], wr[u][1], b1.x); dmma884(vr[ji][0], vr[ji][1], ni1, b1.y);
@@ -351,18 +392,31 @@ template <int MT> struct Q2Warp<cplx, MT> {
             }
         }
         // Z_w^T -= W2^T V^T:  re += (-ar) br + ai bi,  im += (-ar) bi + (-ai) br      (V[row 8t + lr][i = 8u + 2lc (+1)])
+        {
+            double nvr[4][2], nvi[4][2];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const double nr0 = -vr[u][0], nr1 = -vr[u][1], ni0 = -vi[u][0], ni1 = -vi[u][1];
+            for (int u = 0; u < 4; ++u) { nvr[u][0] = -vr[u][0]; nvr[u][1] = -vr[u][1]; nvi[u][0] = -vi[u][0]; nvi[u][1] = -vi[u][1]; }
+            cplx c0[4], c1[4], n0[4], n1[4];
+            { const cplx *bp = sV + (2 * lc) * L::LDV + lr; c0[0] = bp[0]; c1[0] = bp[L::LDV]; }
 #pragma unroll
             for (int t = 0; t < Q2_NT; ++t) {
-                if (u > t || t > u + 8) continue;
-                const cplx *bp = sV + (8 * u + 2 * lc) * L::LDV + 8 * t + lr;
-                const cplx b0 = bp[0], b1 = bp[L::LDV];
-                dmma884(zr[t][0], zr[t][1], nr0, b0.x); dmma884(zr[t][0], zr[t][1], vi[u][0], b0.y);
-                dmma884(zi[t][0], zi[t][1], nr0, b0.y); dmma884(zi[t][0], zi[t][1], ni0, b0.x);
-                dmma884(zr[t][0], zr[t][1], nr1, b1.x); dmma884(zr[t][0], zr[t][1], vi[u][1], b1.y);
-                dmma884(zi[t][0], zi[t][1], nr1, b1.y); dmma884(zi[t][0], zi[t][1], ni1, b1.x);
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    if (t + 1 < Q2_NT && u <= t + 1 && t + 1 <= u + 8) {
+                        const cplx *bp = sV + (8 * u + 2 * lc) * L::LDV + 8 * (t + 1) + lr;
+                        n0[u] = bp[0]; n1[u] = bp[L::LDV];
+                    }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    if (u > t || t > u + 8) continue;
+                    const cplx b0 = c0[u], b1 = c1[u];
+                    dmma884(zr[t][0], zr[t][1], nvr[u][0], b0.x); dmma884(zr[t][0], zr[t][1], vi[u][0], b0.y);
+                    dmma884(zi[t][0], zi[t][1], nvr[u][0], b0.y); dmma884(zi[t][0], zi[t][1], nvi[u][0], b0.x);
+                    dmma884(zr[t][0], zr[t][1], nvr[u][1], b1.x); dmma884(zr[t][0], zr[t][1], vi[u][1], b1.y);
+                    dmma884(zi[t][0], zi[t][1], nvr[u][1], b1.y); dmma884(zi[t][0], zi[t][1], nvi[u][1], b1.x);
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) { c0[u] = n0[u]; c1[u] = n1[u]; }
             }
         }
     }
