@@ -305,10 +305,27 @@ static int he2hb_impl(int dtype, int n, int batch, T *A, long lda, long sA, T *t
     T *P4 = (T *)w.P4;
     const long sP4 = (long)n * 4 * b, sGS = (long)2 * b * b;
     T *Xb = P4, *Vb = P4 + (long)n * b, *Wb = P4 + (long)n * 2 * b, *Vb2 = P4 + (long)n * 3 * b;
-    int panel = 0;
-    for (int j0 = 0; n - j0 - b > 1; j0 += b, ++panel) {
-        const int m = n - j0 - b, jr = j0 + b;      // panel rows start at global row jr
-        // 1. panel QR (cooperative), items in groups of ipl
+    // Look-ahead: the panel QR is a chain of 64 grid barriers (latency, ~5 us per column) and needs few SMs; the rank-2b
+    // update of the trailing matrix is a large GEMM.  The update of panel p is therefore split: the 64 columns that form
+    // panel p+1 first, then -- on an internal side stream, on as few CTAs as hold the panel in shared memory -- the QR of
+    // panel p+1 WHILE the rest of the update runs on the caller's stream (its CTAs fill the SMs the QR leaves free).
+    // Disabled while a stream group limits the SMs (the groups overlap one another instead).
+    static cudaStream_t side = nullptr;
+    static cudaEvent_t ev_cols = nullptr, ev_side = nullptr, ev_qr = nullptr;
+    int dev_sms = 0, dev = 0;
+    cudaGetDevice(&dev); cudaDeviceGetAttribute(&dev_sms, cudaDevAttrMultiProcessorCount, dev);
+    const bool lookahead = sm_count() >= dev_sms && n >= 1024;
+    if (lookahead && !side) {
+        int prio_lo = 0, prio_hi = 0;
+        cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);      // the QR's CTAs take freed SMs before the update's
+        NAO_CUDA_CHECK(cudaStreamCreateWithPriority(&side, cudaStreamNonBlocking, prio_hi));
+        NAO_CUDA_CHECK(cudaEventCreateWithFlags(&ev_cols, cudaEventDisableTiming));
+        NAO_CUDA_CHECK(cudaEventCreateWithFlags(&ev_side, cudaEventDisableTiming));
+        NAO_CUDA_CHECK(cudaEventCreateWithFlags(&ev_qr, cudaEventDisableTiming));
+    }
+    const int cap_rows = (int)((200 * 1024) / ((size_t)(b + 1) * sizeof(T))) - 2;       // panel rows one CTA can hold
+    auto launch_qr = [&](int j0, int panel, cudaStream_t qs, bool few_ctas) -> int {
+        const int m = n - j0 - b;
         for (int b0 = 0; b0 < batch; b0 += w.ipl) {
             const int nit = std::min(w.ipl, batch - b0);
             QrArgs<T> a;
@@ -317,12 +334,24 @@ static int he2hb_impl(int dtype, int n, int batch, T *A, long lda, long sA, T *t
             a.bar = w.bar + (size_t)panel * batch + b0;
             a.n = n; a.j0 = j0;
             a.G = std::max(1, std::min(w.Gq, ceil_div(m, 32)));
+            // (measured at config 2, dense->band in ms: 8 CTAs per item 92.2, 16: 88.9, 24: 87.9, 37: 86.2, all 74: 89.5; no look-ahead 96.4)
+            if (few_ctas) a.G = std::max(1, std::min(a.G, std::max(ceil_div(m, cap_rows), 32)));
             a.chunk = ceil_div(m, a.G);
             const size_t smem = ((size_t)b * (a.chunk | 1) + a.chunk) * sizeof(T);
             void *args[] = {&a};
-            NAO_CUDA_CHECK(cudaLaunchCooperativeKernel((void *)panel_qr_kernel<T>, dim3(nit * a.G), dim3(QR_NT), args, smem, st));
+            NAO_CUDA_CHECK(cudaLaunchCooperativeKernel((void *)panel_qr_kernel<T>, dim3(nit * a.G), dim3(QR_NT), args, smem, qs));
             NAO_LAUNCHED();
         }
+        return NAO_OK;
+    };
+    int panel = 0;
+    bool qr_done_ahead = false;            // the QR of the current panel was issued by the previous iteration
+    for (int j0 = 0; n - j0 - b > 1; j0 += b, ++panel) {
+        const int m = n - j0 - b, jr = j0 + b;      // panel rows start at global row jr
+        // 1. panel QR (cooperative), items in groups of ipl
+        if (!qr_done_ahead) { if (int rc = launch_qr(j0, panel, st, false)) return rc; }
+        else NAO_CUDA_CHECK(cudaStreamWaitEvent(st, ev_qr, 0));
+        qr_done_ahead = false;
         // 2. explicit V (m x b, zeros above the unit diagonal) at rows jr.. of both V blocks
         if (int rc = build_v(dtype, n, j0, b, b, A, lda, sA, Vb + jr, n, sP4, batch, st)) return rc;
         if (int rc = copy_matrix(dtype, m, b, Vb + jr, n, sP4, Vb2 + jr, n, sP4, batch, 0, st)) return rc;
@@ -345,10 +374,33 @@ static int he2hb_impl(int dtype, int n, int batch, T *A, long lda, long sA, T *t
         w1.sA = sP4; w1.sB = sGS; w1.sC = sP4;
         if (int rc = gemm_launch(dtype, w1, batch, st)) return rc;
         // 5. A22 -= V W^H + W V^H = [V W] [W V]^H, lower tiles
-        GemmDesc u = gemm_desc(OP_N, OP_C, m, m, 2 * b, -1.0, Vb + jr, n, Wb + jr, n, 1.0, A22, lda);
-        u.sA = sP4; u.sB = sP4; u.sC = sA; u.cmode = 1;
-        if (int rc = gemm_launch(dtype, u, batch, st)) return rc;
+        const bool next_panel = (n - (j0 + b) - b > 1);
+        if (lookahead && next_panel && m - b >= 512) {
+            // 5a. the b columns of the next panel (rows jr.. : its diagonal block and everything below)
+            GemmDesc ua = gemm_desc(OP_N, OP_C, m, b, 2 * b, -1.0, Vb + jr, n, Wb + jr, n, 1.0, A22, lda);
+            ua.sA = sP4; ua.sB = sP4; ua.sC = sA; ua.cmode = 1;
+            if (int rc = gemm_launch(dtype, ua, batch, st)) return rc;
+            NAO_CUDA_CHECK(cudaEventRecord(ev_cols, st));
+            NAO_CUDA_CHECK(cudaStreamWaitEvent(side, ev_cols, 0));
+            NAO_CUDA_CHECK(cudaEventRecord(ev_side, side));
+            // QR of panel p+1 on the (high-priority) side stream; the big update is held back until the side stream has got
+            // past its wait, so that the QR's CTAs are placed first and the update fills the SMs they leave free
+            if (int rc = launch_qr(j0 + b, panel + 1, side, true)) return rc;
+            NAO_CUDA_CHECK(cudaEventRecord(ev_qr, side));
+            qr_done_ahead = true;
+            NAO_CUDA_CHECK(cudaStreamWaitEvent(st, ev_side, 0));
+            // 5b. the rest of the trailing matrix
+            GemmDesc ub = gemm_desc(OP_N, OP_C, m - b, m - b, 2 * b, -1.0, Vb + jr + b, n, Wb + jr + b, n, 1.0,
+                                    A22 + b + (long)b * lda, lda);
+            ub.sA = sP4; ub.sB = sP4; ub.sC = sA; ub.cmode = 1;
+            if (int rc = gemm_launch(dtype, ub, batch, st)) return rc;
+        } else {
+            GemmDesc u = gemm_desc(OP_N, OP_C, m, m, 2 * b, -1.0, Vb + jr, n, Wb + jr, n, 1.0, A22, lda);
+            u.sA = sP4; u.sB = sP4; u.sC = sA; u.cmode = 1;
+            if (int rc = gemm_launch(dtype, u, batch, st)) return rc;
+        }
     }
+    if (qr_done_ahead) NAO_CUDA_CHECK(cudaStreamWaitEvent(st, ev_qr, 0));
     NAO_CUDA_CHECK(cudaGetLastError());
     return NAO_OK;
 }
