@@ -22,7 +22,8 @@
  *     (stated at each).  nao_geneig, nao_geneig_partial, nao_heev, nao_stedc, nao_density_matrix, nao_fold_density
  *     never block the host (the divide-and-conquer tree is built by a kernel, not copied from the host).
  *   - Process-wide state: the library keeps per-process settings and caches (nao_set_lowdin_threshold, the profiler,
- *     kernel attributes, SM count, the copy stream of nao_solve_host, pinned result words) bound to the FIRST device it
+ *     kernel attributes, SM count, the internal side streams and events of nao_solve_host, of the stream groups and of the
+ *     dense-to-band look-ahead, pinned result words) bound to the FIRST device it
  *     is used on.  Use it from one host thread at a time and on one device per process (one process per GPU is the
  *     deployment model); the Python binding rejects tensors on any other device.
  *   - Return value: NAO_OK (0); -i if argument number i (1-based) is invalid (checked on the host before any
@@ -124,7 +125,7 @@ int nao_geneig(int n, int batch, int dtype, unsigned flags,
  * vectors equals the one of the full solve as long as every state with f >= 1e-17 lies below n_vec -- check with
  * nao_occupied_count after nao_fermi_mu (an SCF loop takes n_vec from the previous step plus a margin).
  * Combine with NAO_TRD_TWO_STAGE: with few vectors the second back-transformation of the two-stage reduction is cheap and
- * that path is the faster one (config 2: 264 vs 400 ms, config 3: 0.83 vs 1.12 s per step on B200).
+ * that path is the faster one (config 2: 259 vs 395 ms, config 3: 0.82 vs 1.10 s per step on B200).
  *   1..4 as nao_geneig;  5 n_vec in 1..n;  the remaining arguments as nao_geneig arguments 5..18.
  * Negative return values count the arguments of THIS signature.
  */
@@ -143,7 +144,7 @@ int nao_geneig_partial(int n, int batch, int dtype, unsigned flags, int n_vec,
  * Arguments as in those three calls (h_weight, h_mu, h_nvec are HOST pointers); dwork needs nao_scf_step_workspace bytes.
  * The call synchronises the stream twice (Fermi level, vector count).
  * Without NAO_TRD_ONE_STAGE / NAO_TRD_TWO_STAGE the fused step takes the two-stage reduction from order 1536 on for real AND
- * complex matrices (few vectors are back-transformed, which favours it: config 3 831 vs 1141 ms).
+ * complex matrices (few vectors are back-transformed, which favours it: config 3 824 vs 1096 ms).
  */
 int nao_scf_step_workspace(int n, int batch, int dtype, unsigned flags, size_t *bytes);
 int nao_scf_step(int n, int batch, int dtype, unsigned flags,
