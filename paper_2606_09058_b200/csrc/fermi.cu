@@ -36,27 +36,32 @@ __global__ void fermi_rank_kernel(int ns, int n, const double *__restrict__ e, c
     if (j < ns) { es[rank] = ej; ws[rank] = wItem[j / n]; }
 }
 
+// Block-wide sum / max with ONE block barrier per call: butterfly inside the warp, one partial per warp into one of two
+// alternating buffers, every thread adds the (at most 32) partials in index order.  Fixed order: deterministic.
 struct BlockSum {
-    double *buf;     // blockDim.x doubles of shared memory
+    double *buf;     // 2 x 32 doubles of shared memory
+    int flip;
     __device__ double sum(double v) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        double *b = buf + 32 * flip; flip ^= 1;
+        if ((threadIdx.x & 31) == 0) b[threadIdx.x >> 5] = v;
         __syncthreads();
-        buf[threadIdx.x] = v;
-        __syncthreads();
-        for (int s = blockDim.x >> 1; s > 0; s >>= 1) {
-            if ((int)threadIdx.x < s) buf[threadIdx.x] += buf[threadIdx.x + s];
-            __syncthreads();
-        }
-        return buf[0];
+        double s = 0.0;
+        const int nw = (blockDim.x + 31) >> 5;
+        for (int w = 0; w < nw; ++w) s += b[w];
+        return s;
     }
     __device__ double max(double v) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+        double *b = buf + 32 * flip; flip ^= 1;
+        if ((threadIdx.x & 31) == 0) b[threadIdx.x >> 5] = v;
         __syncthreads();
-        buf[threadIdx.x] = v;
-        __syncthreads();
-        for (int s = blockDim.x >> 1; s > 0; s >>= 1) {
-            if ((int)threadIdx.x < s) buf[threadIdx.x] = fmax(buf[threadIdx.x], buf[threadIdx.x + s]);
-            __syncthreads();
-        }
-        return buf[0];
+        double s = -INFINITY;
+        const int nw = (blockDim.x + 31) >> 5;
+        for (int w = 0; w < nw; ++w) s = fmax(s, b[w]);
+        return s;
     }
 };
 
@@ -64,11 +69,13 @@ struct BlockSum {
 // formed in sorted order (deterministic).
 __global__ void __launch_bounds__(1024) fermi_bisect_kernel(int ns, const double *__restrict__ es,
                                                              const double *__restrict__ ws, double n_electrons,
-                                                             double kT, double *__restrict__ mu_out) {
+                                                             double kT, double *__restrict__ mu_out, int cache) {
+    extern __shared__ double s_tj[];          // ns doubles when cache != 0
     __shared__ double red[1024];
     __shared__ int s_m;
     __shared__ double s_W;
-    BlockSum bs{red};
+    __shared__ double red2[4 * 32];
+    BlockSum bs{red2, 0};
     const int tid = threadIdx.x, nt = blockDim.x;
     const int chunk = (ns + nt - 1) / nt;
     const int j0 = min(ns, tid * chunk), j1 = min(ns, j0 + chunk);
@@ -115,22 +122,27 @@ __global__ void __launch_bounds__(1024) fermi_bisect_kernel(int ns, const double
     double lo = es[0] - 50.0 * kT, hi = es[ns - 1] + 50.0 * kT;
     const bool logform = (r == 0.0 && m > 0);
 
+
     for (int it = 0; it < 400; ++it) {
         double mu = 0.5 * (lo + hi);
         if (!(mu > lo && mu < hi)) break;
         bool positive;
         if (logform) {
+            // t_j = log w_j + log f_j (j >= m) or log w_j + log(1 - f_j) (j < m); kept in shared memory between the two passes
+            // when the states fit there (cache != 0)
             double mp = -INFINITY, mq = -INFINITY;
             for (int j = j0; j < j1; ++j) {
                 double x = (es[j] - mu) / kT;
                 double t = log(ws[j]) - (j >= m ? softplus(x) : softplus(-x));
+                if (cache) s_tj[j] = t;
                 if (j >= m) mp = fmax(mp, t); else mq = fmax(mq, t);
             }
             mp = bs.max(mp); mq = bs.max(mq);
             double sp = 0.0, sq = 0.0;
             for (int j = j0; j < j1; ++j) {
-                double x = (es[j] - mu) / kT;
-                double t = log(ws[j]) - (j >= m ? softplus(x) : softplus(-x));
+                double t;
+                if (cache) t = s_tj[j];
+                else { double x = (es[j] - mu) / kT; t = log(ws[j]) - (j >= m ? softplus(x) : softplus(-x)); }
                 if (j >= m) sp += exp(t - mp); else sq += exp(t - mq);
             }
             sp = bs.sum(sp); sq = bs.sum(sq);
@@ -163,7 +175,16 @@ int fermi_mu(int n, int batch, const double *dE, const double *h_weight, double 
     NAO_CUDA_CHECK(cudaMemcpyAsync(wItem, h_weight, sizeof(double) * batch, cudaMemcpyHostToDevice, st));
     fermi_rank_kernel<<<ceil_div(ns, 256), 256, 0, st>>>(ns, n, dE, wItem, es, ws);
     NAO_LAUNCHED();
-    fermi_bisect_kernel<<<1, 1024, 0, st>>>(ns, es, ws, n_electrons, kT, mu);
+    {
+        const size_t tbytes = (size_t)ns * 8;
+        const int cache = tbytes <= 200 * 1024 ? 1 : 0;
+        static bool attr = false;
+        if (!attr) {
+            NAO_CUDA_CHECK(cudaFuncSetAttribute(fermi_bisect_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+            attr = true;
+        }
+        fermi_bisect_kernel<<<1, 1024, cache ? tbytes : 0, st>>>(ns, es, ws, n_electrons, kT, mu, cache);
+    }
     NAO_LAUNCHED();
     fermi_occ_kernel<<<ceil_div(ns, 256), 256, 0, st>>>(ns, dE, mu, kT, dF);
     NAO_LAUNCHED();
