@@ -96,7 +96,7 @@ def test_golden_config2_is_consistent_with_what_the_mathematics_fixes():
     """The stored config-2 digest cannot be regenerated in a test (hours of Jacobi), so it is pinned by what holds
     independently of the eigen-solver: the generator still produces the same input; sum_i e_i = Tr(S^{-1} H) (LAPACK solve);
     the stored mu is the root of the occupation sum of the stored levels (oracle.fermi, seconds); Tr(D S) = sum_i f_i per
-    item and N_e in total; the three lowest and three highest levels agree with LAPACK's (scipy, an independent library);
+    item and N_e in total; every level agrees with LAPACK's (scipy dsygvd, an independent library) to 1e-10;
     0 <= D_ii <= 1/lambda_min(S)  (D = C f C^H <= C C^H = S^{-1})."""
     import scipy.linalg as sl
     g = read_golden_c2()
@@ -105,14 +105,17 @@ def test_golden_config2_is_consistent_with_what_the_mathematics_fixes():
     assert np.all(np.diff(g["e"], axis=1) >= 0)
     mu, f = oracle.fermi(g["e"], prob.weights, prob.n_electrons, prob.kT)
     assert abs(mu - g["mu"]) <= 1e-13
-    assert abs(g["trace_DS"][0] + g["trace_DS"][1] - prob.n_electrons) <= 1e-9        # weights are 1 per spin item
+    # Tr(D S) = sum_i f_i c_i^H S c_i: the oracle stores C in FP64 after 13 Jacobi sweeps at n = 6656, so c_i^H S c_i = 1 holds to
+    # ~5e-12 per state and the trace to ~1e3 occupied states x 5e-12 = 5e-9 (measured 5.3e-9); the bar here is 1e-7
+    assert abs(g["trace_DS"][0] + g["trace_DS"][1] - prob.n_electrons) <= 1e-7        # weights are 1 per spin item
     for b in range(2):
         Hb, Sb = prob.H_full(b), prob.S_full(b)
-        assert abs(np.sum(g["e"][b]) - np.trace(np.linalg.solve(Sb, Hb))) <= 1e-9     # trace invariant
-        assert abs(np.sum(f[b]) - g["trace_DS"][b]) <= 1e-9                           # Tr(D S) = sum_i f_i
-        lo = sl.eigh(Hb, Sb, eigvals_only=True, subset_by_index=[0, 2])
-        hi = sl.eigh(Hb, Sb, eigvals_only=True, subset_by_index=[prob.n - 3, prob.n - 1])
-        assert np.abs(lo - g["e"][b][:3]).max() <= 1e-10 and np.abs(hi - g["e"][b][-3:]).max() <= 1e-10
+        # trace invariant: sum of 6656 levels, each good to ~1e-12, against a LAPACK solve (measured difference 3e-9)
+        assert abs(np.sum(g["e"][b]) - np.trace(np.linalg.solve(Sb, Hb))) <= 1e-7
+        assert abs(np.sum(f[b]) - g["trace_DS"][b]) <= 1e-7                           # Tr(D S) = sum_i f_i
+        # the whole spectrum against LAPACK's (scipy dsygvd: an independent library, ~20 s per item on 8 cores)
+        ref = sl.eigh(Hb, Sb, eigvals_only=True)
+        assert np.abs(ref - g["e"][b]).max() <= 1e-10
         assert np.all(g["diagD"][b] >= -1e-15) and np.all(g["diagD"][b] <= 1.0 / np.linalg.eigvalsh(Sb)[0] + 1e-12)
         for (bb, i, j, v) in g["D"]:
             if bb == b and i == j:
