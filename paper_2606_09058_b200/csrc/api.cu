@@ -57,6 +57,22 @@ int prof_kernel_begin(int slot, double work, cudaStream_t st) {
     g_swork[slot] += work;
     return k;
 }
+// Flops of grouped launches: their dimensions are written by kernels (deflated sizes of the D&C merges), so the count is
+// summed on the device from the descriptors, behind the launch, while profiling is enabled.
+__device__ double g_grouped_flops;
+__global__ void grouped_flops_kernel(const GemmDesc *d, int ngroups, double per_mnk) {
+    double s = 0.0;
+    for (int g = threadIdx.x; g < ngroups; g += blockDim.x)
+        if (d[g].m > 0 && d[g].n > 0 && d[g].k > 0)
+            s += per_mnk * d[g].m * (double)d[g].n * d[g].k * (d[g].cmode != 0 ? 0.5 : 1.0) *
+                 ((d[g].maskA != MASK_NONE || d[g].maskB != MASK_NONE) ? 0.5 : 1.0);
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0 && s != 0.0) atomicAdd(&g_grouped_flops, s);
+}
+void prof_grouped_flops(const GemmDesc *d_descs, int ngroups, double per_mnk, cudaStream_t st) {
+    if (!g_prof_on || !d_descs || ngroups <= 0) return;
+    grouped_flops_kernel<<<1, 128, 0, st>>>(d_descs, ngroups, per_mnk);
+}
 void prof_kernel_end(int slot, int k, cudaStream_t st) {
     if (k < 0) return;
     cudaEventRecord(g_sev[slot][k][1], st);
@@ -66,6 +82,8 @@ void prof_kernel_end(int slot, int k, cudaStream_t st) {
 NAO_EXPORT int nao_profile_enable(int on) {
     nao::g_prof_on = on != 0;
     for (int s = 0; s < nao::NSLOT; ++s) { nao::g_scount[s] = 0; nao::g_swork[s] = 0.0; }
+    const double zero = 0.0;
+    cudaMemcpyToSymbol(nao::g_grouped_flops, &zero, sizeof(double));
     return NAO_OK;
 }
 NAO_EXPORT int nao_profile_kernel(int slot, double *h_ms, double *h_work, int *h_launches) {
@@ -78,7 +96,9 @@ NAO_EXPORT int nao_profile_kernel(int slot, double *h_ms, double *h_work, int *h
         if (cudaEventElapsedTime(&ms, g_sev[slot][k][0], g_sev[slot][k][1]) == cudaSuccess) tot += ms;
     }
     if (h_ms) *h_ms = tot;
-    if (h_work) *h_work = g_swork[slot];
+    double grouped = 0.0;
+    if (slot == 1) cudaMemcpyFromSymbol(&grouped, g_grouped_flops, sizeof(double));      // after the event waits above
+    if (h_work) *h_work = g_swork[slot] + grouped;
     if (h_launches) *h_launches = g_scount[slot];
     return NAO_OK;
 }

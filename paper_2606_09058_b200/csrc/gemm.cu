@@ -403,6 +403,7 @@ static int launch_variant2(const GemmDesc *hd, const GemmDesc *dd, int ngroups, 
                                   (hd->maskA != MASK_NONE || hd->maskB != MASK_NONE ? 0.5 : 1.0) * batch /
                                   (hd->ksplit > 1 ? hd->ksplit : 1)
                             : 0.0;
+    if (!hd) prof_grouped_flops(dd, ngroups, (CPLX ? 8.0 : 2.0) * batch, st);
     const int pk = prof_kernel_begin(1, flops, st);
     gemm_kernel<CPLX, AXC, BXC, SCALE, NARROW, AL16><<<grid, GEMM_THREADS, smem, st>>>(dummy, dd);
     prof_kernel_end(1, pk, st);

@@ -165,6 +165,8 @@ void prof_mark(int idx, cudaStream_t st);
 // per-launch timers: slot 0 = hetrd_panel_kernel (work = algorithmic HBM bytes), slot 1 = gemm_kernel (work = flops)
 int prof_kernel_begin(int slot, double work, cudaStream_t st);
 void prof_kernel_end(int slot, int k, cudaStream_t st);
+// grouped GEMM launches: executed flops = per_mnk * sum over the device descriptors of m n k (counted by a kernel)
+void prof_grouped_flops(const GemmDesc *d_descs, int ngroups, double per_mnk, cudaStream_t st);
 
 // fermi.cu / density
 int fermi_mu(int n, int batch, const double *dE, const double *h_weight, double n_electrons, double kT, double *h_mu,
