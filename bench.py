@@ -131,7 +131,7 @@ def read_traffic(kernel, workload):
     return None, None
 
 
-def side_record(nao, torch, workload, dev, hbm_peak, dmma_meas, steps=3, warmup=2):
+def side_record(nao, torch, workload, dev, hbm_peak, dmma_meas, steps=3, warmup=2, groups=True):
     """A second workload timed in the same run (device-resident inputs, CUDA events, `warmup` + `steps` full steps, then one
     step with the library's event timers): ms per step, phases, and the rooflines of hetrd_panel_kernel / gemm_kernel."""
     from paper_2606_09058_b200.synth import make_config
@@ -185,7 +185,7 @@ def side_record(nao, torch, workload, dev, hbm_peak, dmma_meas, steps=3, warmup=
                                 "frac": tf / dmma_meas, "kernel_ms_per_step": kg["ms"], "launches_timed": kg["launches"]}
     # concurrent mid-size solves: the same step with the batch spread over 2/4/8 internal streams
     # (NAO_STREAM_GROUPS_*), against the single batched launch above
-    if prob.batch >= 4:
+    if prob.batch >= 4 and groups:
         groups = {"1 (batched launches)": ms}
         for gname, gflag in (("2", nao.NAO_STREAM_GROUPS_2), ("4", nao.NAO_STREAM_GROUPS_4), ("8", nao.NAO_STREAM_GROUPS_8)):
             gwork = torch.empty(nao.geneig_workspace(prob.n, prob.batch, dt, flags | gflag) + 256, dtype=torch.uint8, device=dev)
@@ -248,7 +248,7 @@ def main():
     ap.add_argument("--workload", default="c2", choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-side", action="store_true", help="skip the c3 / c1 side records of the default (c2) run")
+    ap.add_argument("--no-side", action="store_true", help="skip the c3 / c1 / c4 side records of the default (c2) run")
     ap.add_argument("--reduction", default="default", choices=["default", "one_stage", "two_stage"],
                     help="force the tridiagonalisation path of the timed step (NAO_TRD_ONE_STAGE / NAO_TRD_TWO_STAGE)")
     ap.add_argument("--timed-only", action="store_true",
@@ -545,9 +545,13 @@ def main():
             line["roofline"], line["roofline_hetrd"] = r_gemm, r_hetrd
         # the other headline workload of BASELINE.json's metric ("N=6656 real, 9984 cplx"), timed in the same run
         if world == 1 and args.workload == "c2" and not args.no_side:
-            for wl in ("c3", "c1"):
+            del e2e_work
+            torch.cuda.empty_cache()
+            for wl in ("c3", "c1", "c4"):
                 try:
-                    line[wl] = side_record(nao, torch, wl, dev, hbm_peak, dmma_meas)
+                    # config 4 (11.3 GB per matrix, 21 s per step): one warm-up and one timed step
+                    kw = dict(steps=1, warmup=1) if wl == "c4" else {}
+                    line[wl] = side_record(nao, torch, wl, dev, hbm_peak, dmma_meas, **kw)
                 except Exception as exc:       # reported, never hidden
                     line[wl] = {"error": str(exc)}
         if not args.no_cpu_baseline and world == 1:
