@@ -210,23 +210,30 @@ __global__ void __launch_bounds__(256) he2hb_small_kernel(const T *GS, long sGS,
     }
     if (tid < b) s_tau[tid] = tau[tid];
     __syncthreads();
-    // column i of T: T(0:i, i) = -tau_i T(0:i,0:i) G(0:i, i).  Row `row` of the product by 4 adjacent lanes (the recurrence is
-    // bound by the latency of this dependent chain); 64 rows x 4 lanes = 256 threads
-    for (int i = 0; i < b; ++i) {
-        const int row = tid >> 2, part = tid & 3;
-        T acc = O::zero();
-        if (row < i)
-            for (int c = row + part; c < i; c += 4) acc = O::fma(sT[row * LD + c], sG[c * LD + i], acc);
-        double *a = (double *)&acc;
+    // T = U^{-1} with U = diag(1/tau) + striu(G)  (T^{-1} + T^{-H} = V^H V): column j of T by back substitution,
+    //   T(j,j) = tau_j,   T(i,j) = -tau_i sum_{k=i+1..j} G(i,k) T(k,j)   (i = j-1 .. 0),
+    // which needs no division (tau_i = 0, H_i = I, gives a zero row and column) and -- unlike the column-by-column xLARFT
+    // recurrence -- no block barrier: the 64 columns are independent, 4 adjacent lanes share the k-sum of one column.
+    {
+        const int j = tid >> 2, part = tid & 3;
+        if (part == 0) sT[j * LD + j] = s_tau[j];
+        __syncwarp();
+        const int jtop = (tid | 31) >> 2;                  // last column of this warp: warp-uniform trip count
+        for (int i = jtop - 1; i >= 0; --i) {
+            T acc = O::zero();
+            if (i < j)
+                for (int k = i + 1 + part; k <= j; k += 4) acc = O::fma(sG[i * LD + k], sT[k * LD + j], acc);
+            double *a = (double *)&acc;
 #pragma unroll
-        for (int w = 0; w < (int)(sizeof(T) / 8); ++w) {
-            a[w] += __shfl_xor_sync(0xffffffffu, a[w], 1);
-            a[w] += __shfl_xor_sync(0xffffffffu, a[w], 2);
+            for (int w = 0; w < (int)(sizeof(T) / 8); ++w) {
+                a[w] += __shfl_xor_sync(0xffffffffu, a[w], 1);
+                a[w] += __shfl_xor_sync(0xffffffffu, a[w], 2);
+            }
+            if (part == 0 && i < j) sT[i * LD + j] = O::sub(O::zero(), O::mul(s_tau[i], acc));
+            __syncwarp();
         }
-        if (row < i && part == 0) sT[row * LD + i] = O::sub(O::zero(), O::mul(s_tau[i], acc));
-        if (tid == 0) sT[i * LD + i] = s_tau[i];
-        __syncthreads();
     }
+    __syncthreads();
     for (int e = tid; e < b * b; e += 256) {
         const int i = e % b, j = e / b;
         sG[i * LD + j] = GS[(long)j * b + i];              // S0(i,j)
