@@ -77,6 +77,18 @@ static inline GemmDesc gemm_desc(int opA, int opB, int m, int n, int k, double a
     return d;
 }
 
+// Split-K factor that fills the last wave: the GEMM core runs one CTA per SM (255 registers), so `tiles * ks` CTAs take
+// ceil(tiles * ks / nsm) rounds; the factor (<= ksmax) with the best fill, a small penalty per extra slice, is returned.
+static inline int fill_ksplit(long tiles, int nsm, int ksmax) {
+    int best_ks = 1; double best = 0.0;
+    for (int ks = 1; ks <= (ksmax < 1 ? 1 : ksmax); ++ks) {
+        const double waves = (double)tiles * ks / nsm;
+        const double rounds = (double)(long)(waves + 0.999999), eff = waves / rounds - 0.004 * (ks - 1);
+        if (eff > best + 1e-9) { best = eff; best_ks = ks; }
+    }
+    return best_ks;
+}
+
 // One problem described on the host (passed by value), `batch` items via the strides in the descriptor.
 int gemm_launch(int dtype, const GemmDesc &d, int batch, cudaStream_t st);
 // `ngroups` problems described by descriptors in DEVICE memory (their m,n,k may have been written by a kernel);

@@ -129,15 +129,7 @@ static OrmWork orm_plan(int dtype, int n, int ncols, int batch, void *work) {
     // 4.2 waves; the split factor is chosen to fill the last wave: 4 slices = 16.9 waves)
     const int tilesX = (ORM_BLK / 128) * ceil_div(ncols, dtype == NAO_COMPLEX ? 64 : 128) * batch;
     const int nsm = sm_count();
-    w.ksX = 1;
-    {
-        double best = 0.0;
-        const int ksmax = std::max(1, std::min(std::min(8, ceil_div(n, 1024)), std::max(1, 20 * nsm / std::max(1, tilesX))));
-        for (int ks = 1; ks <= ksmax; ++ks) {
-            const double waves = (double)tilesX * ks / nsm, eff = waves / std::ceil(waves) - 0.004 * (ks - 1);
-            if (eff > best + 1e-9) { best = eff; w.ksX = ks; }
-        }
-    }
+    w.ksX = fill_ksplit(tilesX, nsm, std::max(1, std::min(std::min(8, ceil_div(n, 1024)), std::max(1, 20 * nsm / std::max(1, tilesX)))));
     const int tilesG = (ORM_BLK / 128) * (dtype == NAO_COMPLEX ? 4 : 2) * batch;
     w.ksG = std::max(1, std::min(std::min(148 / std::max(1, tilesG), ceil_div(n, 256)), 64));
     w.V = ar.take((size_t)batch * n * ORM_BLK * es);

@@ -275,8 +275,7 @@ static He2hbWork he2hb_plan(int dtype, int n, int batch, void *work) {
     w.chunk = ceil_div(m0, w.Gq);
     w.smem = ((size_t)b * (w.chunk | 1) + w.chunk) * es;
     // split-K factors: X = A22 V (m x b, k = m) fills ~3 CTAs per SM-slot; the b x 2b product one slice per SM
-    const int tilesX = ceil_div(n, 128) * batch;
-    w.ksX = std::max(1, std::min(std::min(3 * nsm / std::max(1, tilesX), ceil_div(n, 256)), 16));
+    w.ksX = 16;          // upper bound (sizes the scratch); the factor is chosen per panel to fill the last wave of CTAs
     w.ksS = std::max(1, std::min(std::min(nsm / std::max(1, batch), ceil_div(n, 256)), 64));
     Arena ar(work, (size_t)-1);
     w.P4 = ar.take((size_t)batch * n * 4 * b * es);            // [X | V | W | V], ld n, rows indexed globally
@@ -364,7 +363,7 @@ static int he2hb_impl(int dtype, int n, int batch, T *A, long lda, long sA, T *t
         if (int rc = copy_matrix(dtype, m, b, Vb + jr, n, sP4, Vb2 + jr, n, sP4, batch, 0, st)) return rc;
         // 3. X = A22 V : lower triangle as stored + strictly lower triangle transposed
         T *A22 = A + jr + (long)jr * lda;
-        const int ksx = std::min(w.ksX, ceil_div(m, 256));
+        const int ksx = fill_ksplit((long)ceil_div(m, 128) * batch, sm_count(), std::min(w.ksX, ceil_div(m, 512)));
         GemmDesc x1 = gemm_desc(OP_N, OP_N, m, b, m, 1.0, A22, lda, Vb + jr, n, 0.0, Xb + jr, n);
         x1.sA = sA; x1.sB = sP4; x1.sC = sP4; x1.maskA = MASK_LOWER;
         if (int rc = gemm_splitk(dtype, x1, batch, ksx, w.splitk, st)) return rc;
