@@ -120,7 +120,7 @@ int larft(int dtype, int kb, const void *G, long ldg, long sG, const void *tau, 
     return NAO_OK;
 }
 
-struct OrmWork { void *V, *G, *T, *X, *X2, *P; size_t bytes; int ksG, ksX; };
+struct OrmWork { void *V, *G, *T, *X, *X2, *P, *Vs, *tmp, *Ps; size_t bytes; int ksG, ksX; };
 static OrmWork orm_plan(int dtype, int n, int ncols, int batch, void *work) {
     OrmWork w; const size_t es = esize(dtype);
     Arena ar(work, (size_t)-1);
@@ -134,10 +134,14 @@ static OrmWork orm_plan(int dtype, int n, int ncols, int batch, void *work) {
     w.ksG = std::max(1, std::min(std::min(148 / std::max(1, tilesG), ceil_div(n, 256)), 64));
     w.V = ar.take((size_t)batch * n * ORM_BLK * es);
     w.G = ar.take((size_t)batch * ORM_BLK * ORM_BLK * es);
-    w.T = ar.take((size_t)batch * ORM_BLK * ORM_BLK * es);
+    w.T = ar.take((size_t)2 * batch * ORM_BLK * ORM_BLK * es);          // two T factors: the next block's is built ahead
     w.X = ar.take((size_t)batch * ORM_BLK * ncols * es);
     w.X2 = ar.take((size_t)batch * ORM_BLK * std::max(ncols, ORM_BLK) * es);
     w.P = ar.take((size_t)batch * std::max((size_t)w.ksX * ORM_BLK * ncols, (size_t)w.ksG * ORM_BLK * ORM_BLK) * es);
+    // look-ahead of the T factor (side stream): its own explicit V, small temporary and split-K scratch
+    w.Vs = ar.take((size_t)batch * n * ORM_BLK * es);
+    w.tmp = ar.take((size_t)batch * ORM_BLK * ORM_BLK * es);
+    w.Ps = ar.take((size_t)batch * w.ksG * ORM_BLK * ORM_BLK * es);
     w.bytes = ar.off;
     return w;
 }
@@ -160,42 +164,85 @@ static int ormtr_impl(int dtype, int n, int ncols, int batch, int shift, const T
     const int BLK = (4 * ncols >= n) ? ORM_BLK : ORM_BLK / 2;
     const int nblocks = ceil_div(nref, BLK);
     const long sGT = (long)ORM_BLK * ORM_BLK, sX = (long)ORM_BLK * ncols, sX2 = (long)ORM_BLK * std::max(ncols, ORM_BLK);
-    T *Gm = (T *)w.G, *Tm = (T *)w.T;
-    for (int blk = nblocks - 1; blk >= 0; --blk) {
+    const long sV = (long)n * ORM_BLK;
+    // The T factor of a block depends on the reflectors only, not on Z: a chain of small launches (explicit V, G = V^H V, the
+    // xLARFT recurrence on the diagonal 128-blocks, off-diagonal blocks by doubling).  The factor of block blk-1 is built on
+    // an internal high-priority side stream while the three large products of block blk run on the caller's stream.
+    // (Not while a stream group limits the SMs: the groups overlap one another instead.)
+    static cudaStream_t side = nullptr;
+    static cudaEvent_t ev_fork = nullptr, ev_T = nullptr;
+    int dev_sms = 0, dev = 0;
+    cudaGetDevice(&dev); cudaDeviceGetAttribute(&dev_sms, cudaDevAttrMultiProcessorCount, dev);
+    const bool ahead = sm_count() >= dev_sms && nblocks > 1 && n >= 1024;
+    if (ahead && !side) {
+        int prio_lo = 0, prio_hi = 0;
+        cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
+        NAO_CUDA_CHECK(cudaStreamCreateWithPriority(&side, cudaStreamNonBlocking, prio_hi));
+        NAO_CUDA_CHECK(cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming));
+        NAO_CUDA_CHECK(cudaEventCreateWithFlags(&ev_T, cudaEventDisableTiming));
+    }
+    // T factor of block blk into Tm (kb x kb, ld kb) on stream qs; Vx = explicit V of the block (output), Gx, tmpx, Px = scratch
+    auto build_t = [&](int blk, T *Tm, T *Vx, T *Gx, T *tmpx, void *Px, cudaStream_t qs) -> int {
         const int jb = blk * BLK, kb = std::min(BLK, nref - jb), m = n - jb - shift;
-        const long ldv = m, sV = (long)n * ORM_BLK;
-        build_v_kernel<T><<<dim3(ceil_div(m, 256), kb, batch), 256, 0, st>>>(n, jb, kb, shift, A, lda, sA, (T *)w.V, ldv, sV);
+        const long ldv = m;
+        build_v_kernel<T><<<dim3(ceil_div(m, 256), kb, batch), 256, 0, qs>>>(n, jb, kb, shift, A, lda, sA, Vx, ldv, sV);
         NAO_LAUNCHED();
         // G = V^H V  (kb x kb, k = m: split-K)
-        GemmDesc g = gemm_desc(OP_C, OP_N, kb, kb, m, 1.0, w.V, ldv, w.V, ldv, 0.0, w.G, kb);
+        GemmDesc g = gemm_desc(OP_C, OP_N, kb, kb, m, 1.0, Vx, ldv, Vx, ldv, 0.0, Gx, kb);
         g.sA = sV; g.sB = sV; g.sC = sGT;
-        if (int rc = gemm_splitk(dtype, g, batch, std::min(w.ksG, ceil_div(m, 256)), w.P, st)) return rc;
+        if (int rc = gemm_splitk(dtype, g, batch, std::min(w.ksG, ceil_div(m, 256)), Px, qs)) return rc;
         // T: recurrence on the diagonal 128-blocks, then off-diagonal blocks by doubling (two small GEMMs each)
-        larft_kernel<T><<<dim3(batch, ceil_div(kb, ORM_KB)), 256, larft_smem, st>>>(kb, Gm, kb, sGT, tau + jb, n, Tm, kb, sGT);
+        larft_kernel<T><<<dim3(batch, ceil_div(kb, ORM_KB)), 256, larft_smem, qs>>>(kb, Gx, kb, sGT, tau + jb, n, Tm, kb, sGT);
         NAO_LAUNCHED();
         for (int sz = ORM_KB; sz < kb; sz *= 2)
             for (int off = 0; off + sz < kb; off += 2 * sz) {
                 const int k1 = sz, k2 = std::min(sz, kb - off - sz), o2 = off + sz;
                 // tmp = G12 T22 ; T12 = -T11 tmp
-                GemmDesc t1 = gemm_desc(OP_N, OP_N, k1, k2, k2, 1.0, Gm + off + (long)o2 * kb, kb, Tm + o2 + (long)o2 * kb, kb, 0.0, w.X2, k1);
-                t1.sA = sGT; t1.sB = sGT; t1.sC = sX2; t1.maskB = MASK_UPPER;
-                if (int rc = gemm_launch(dtype, t1, batch, st)) return rc;
-                GemmDesc t2 = gemm_desc(OP_N, OP_N, k1, k2, k1, -1.0, Tm + off + (long)off * kb, kb, w.X2, k1, 0.0, Tm + off + (long)o2 * kb, kb);
-                t2.sA = sGT; t2.sB = sX2; t2.sC = sGT; t2.maskA = MASK_UPPER;
-                if (int rc = gemm_launch(dtype, t2, batch, st)) return rc;
+                GemmDesc t1 = gemm_desc(OP_N, OP_N, k1, k2, k2, 1.0, Gx + off + (long)o2 * kb, kb, Tm + o2 + (long)o2 * kb, kb, 0.0, tmpx, k1);
+                t1.sA = sGT; t1.sB = sGT; t1.sC = sGT; t1.maskB = MASK_UPPER;
+                if (int rc = gemm_launch(dtype, t1, batch, qs)) return rc;
+                GemmDesc t2 = gemm_desc(OP_N, OP_N, k1, k2, k1, -1.0, Tm + off + (long)off * kb, kb, tmpx, k1, 0.0, Tm + off + (long)o2 * kb, kb);
+                t2.sA = sGT; t2.sB = sGT; t2.sC = sGT; t2.maskA = MASK_UPPER;
+                if (int rc = gemm_launch(dtype, t2, batch, qs)) return rc;
             }
+        return NAO_OK;
+    };
+    T *Tbuf[2] = {(T *)w.T, (T *)w.T + (long)batch * sGT};
+    // first block: everything on the caller's stream
+    if (int rc = build_t(nblocks - 1, Tbuf[(nblocks - 1) & 1], (T *)w.V, (T *)w.G, (T *)w.tmp, w.P, st)) return rc;
+    for (int blk = nblocks - 1; blk >= 0; --blk) {
+        const int jb = blk * BLK, kb = std::min(BLK, nref - jb), m = n - jb - shift;
+        const long ldv = m;
+        T *Tm = Tbuf[blk & 1];
+        if (blk < nblocks - 1) {
+            if (ahead) NAO_CUDA_CHECK(cudaStreamWaitEvent(st, ev_T, 0));          // T(blk) built ahead on the side stream
+            // explicit V of this block for the large products (the side stream used its own copy)
+            build_v_kernel<T><<<dim3(ceil_div(m, 256), kb, batch), 256, 0, st>>>(n, jb, kb, shift, A, lda, sA, (T *)w.V, ldv, sV);
+            NAO_LAUNCHED();
+        }
+        if (blk > 0) {
+            if (ahead) {
+                // everything enqueued so far (incl. the last use of the other T buffer) precedes the side stream's work
+                NAO_CUDA_CHECK(cudaEventRecord(ev_fork, st));
+                NAO_CUDA_CHECK(cudaStreamWaitEvent(side, ev_fork, 0));
+                if (int rc = build_t(blk - 1, Tbuf[(blk - 1) & 1], (T *)w.Vs, (T *)w.G, (T *)w.tmp, w.Ps, side)) return rc;
+                NAO_CUDA_CHECK(cudaEventRecord(ev_T, side));
+            }
+        }
         // X = V^H Z[jb+shift:, :]  (kb x ncols, k = m: split-K)
         GemmDesc x = gemm_desc(OP_C, OP_N, kb, ncols, m, 1.0, w.V, ldv, Z + jb + shift, ldz, 0.0, w.X, kb);
         x.sA = sV; x.sB = sZ; x.sC = sX;
         if (int rc = gemm_splitk(dtype, x, batch, std::min(w.ksX, ceil_div(m, 512)), w.P, st)) return rc;
         // X2 = T X  (T upper triangular: elements below the diagonal are never read)
-        GemmDesc t = gemm_desc(OP_N, OP_N, kb, ncols, kb, 1.0, w.T, kb, w.X, kb, 0.0, w.X2, kb);
+        GemmDesc t = gemm_desc(OP_N, OP_N, kb, ncols, kb, 1.0, Tm, kb, w.X, kb, 0.0, w.X2, kb);
         t.sA = sGT; t.sB = sX; t.sC = sX2; t.maskA = MASK_UPPER;
         if (int rc = gemm_launch(dtype, t, batch, st)) return rc;
         // Z[jb+shift:, :] -= V X2
         GemmDesc u = gemm_desc(OP_N, OP_N, m, ncols, kb, -1.0, w.V, ldv, w.X2, kb, 1.0, Z + jb + shift, ldz);
         u.sA = sV; u.sB = sX2; u.sC = sZ;
         if (int rc = gemm_launch(dtype, u, batch, st)) return rc;
+        if (blk > 0 && !ahead)
+            if (int rc = build_t(blk - 1, Tbuf[(blk - 1) & 1], (T *)w.V, (T *)w.G, (T *)w.tmp, w.P, st)) return rc;
     }
     NAO_CUDA_CHECK(cudaGetLastError());
     return NAO_OK;
