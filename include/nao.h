@@ -80,6 +80,7 @@ extern "C" {
 #define NAO_ERR_CUDA 2         /* a CUDA runtime call or kernel launch failed */
 #define NAO_ERR_ELECTRONS 3    /* nao_fermi_mu: n_electrons outside (0, sum of weights * n) or kT <= 0 */
 #define NAO_ERR_UNSUPPORTED 4  /* combination of arguments not implemented */
+#define NAO_ERR_STATIC_LIMIT 5 /* nao_fermi_mu_static: n * batch exceeds NAO_FERMI_STATIC_MAX_STATES */
 
 /* Relative pruning threshold of the NAO_LOWDIN route, 0 <= rel < 1 (process-wide, read when S is decomposed). */
 int nao_set_lowdin_threshold(double rel);
@@ -200,6 +201,38 @@ int nao_fermi_workspace(int n, int batch, size_t *bytes);
 int nao_fermi_mu(int n, int batch, const double *dE, const double *h_weight,
                  double n_electrons, double kT, double *h_mu, double *dF,
                  void *dwork, void *cuda_stream);
+
+/*
+ * nao_fermi_mu for callers that cannot supply device scratch and must not cause a device allocation.
+ *
+ * Who that is: code that runs inside a host program which owns all device memory itself -- an SCF code that carves the
+ * whole HBM into its own pool at start-up and forbids any later driver allocation, a plug-in that is only handed its input
+ * and output arrays, or a call made from a latency-critical section where cudaMalloc / cudaFree are unacceptable because
+ * they take the driver's global lock and synchronise the whole device (stalling the host program's other streams).  Such a
+ * caller has no `dwork` to pass either, so this entry point has no workspace argument: it keeps its intermediates (the
+ * sorted energies and their weights, the per-item weights, the device copy of mu) in a fixed array that is compiled into
+ * the library, and it calls neither cudaMalloc nor cudaFree nor any routine that allocates.
+ *
+ * Same arguments, same result (mu, dF) and same error codes as nao_fermi_mu, without its argument 9:
+ *   1 n, 2 batch, 3 dE, 4 h_weight (HOST), 5 n_electrons, 6 kT, 7 h_mu (HOST, out), 8 dF (out), 9 cuda_stream
+ * The caller still owns dE and dF.  Like nao_fermi_mu it synchronises the stream to write *h_mu.
+ *
+ * Limit: n * batch <= NAO_FERMI_STATIC_MAX_STATES (65536 states: every configuration of BASELINE.json fits, config 4 has
+ * 26624).  Anything larger returns NAO_ERR_STATIC_LIMIT before the device is touched; use nao_fermi_mu with your own
+ * workspace then.
+ * Cost: the array is NAO_FERMI_STATIC_BYTES = 1.5 MiB of device memory on EVERY GPU that loads this library's kernels, held
+ * until the process exits, also when this entry point is never called.
+ * Sharing: all calls on a device use the same array.  It keeps whatever the last call wrote; that is harmless because a
+ * call writes every word before it reads it (nothing relies on zeros).  But two calls that are in flight on the GPU at the
+ * same time -- different streams or host threads -- overwrite each other's intermediates: serialise them.
+ * Set-up: the first call made with a given device current looks up the array's address on that device (one
+ * cudaGetSymbolAddress; the library remembers it per device ordinal, 64 at most).  Make that first call outside any
+ * stream capture.
+ */
+#define NAO_FERMI_STATIC_MAX_STATES 65536
+#define NAO_FERMI_STATIC_BYTES (3 * NAO_FERMI_STATIC_MAX_STATES * 8 + 256)
+int nao_fermi_mu_static(int n, int batch, const double *dE, const double *h_weight,
+                        double n_electrons, double kT, double *h_mu, double *dF, void *cuda_stream);
 
 /*
  * Density matrix D_b = C_b diag(f_b) C_b^H per batch item, full Hermitian matrix written (both triangles).

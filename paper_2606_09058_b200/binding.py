@@ -39,6 +39,7 @@ _SIGNATURES = {
     "nao_solve_host": ([_i, _i, _i, ctypes.c_uint, _vp, _vp, _i, _dp, _d, _d, _vp, _dp, _vp, _vp, _vp, _sz, _vp], _i),
     "nao_fermi_workspace": ([_i, _i, _szp], _i),
     "nao_fermi_mu": ([_i, _i, _vp, _dp, _d, _d, _dp, _vp, _vp, _vp], _i),
+    "nao_fermi_mu_static": ([_i, _i, _vp, _dp, _d, _d, _dp, _vp, _vp], _i),
     "nao_density_workspace": ([_i, _i, _i, _szp], _i),
     "nao_density_matrix": ([_i, _i, _i, _vp, _l, _l, _vp, _vp, _l, _l, _vp, _sz, _vp], _i),
     "nao_energy_weights": ([_i, _i, _vp, _vp, _vp, _vp], _i),
@@ -259,6 +260,29 @@ def fermi_mu(E: torch.Tensor, weights, n_electrons: float, kT: float):
     rc = lib().nao_fermi_mu(n, batch, _dev(E, "E"), w, float(n_electrons), float(kT), ctypes.byref(mu), _dev(F, "F"),
                             _dev(work, "work"), _stream(E))
     _check(rc, "nao_fermi_mu")
+    return mu.value, F
+
+
+FERMI_STATIC_MAX_STATES = 65536
+
+
+def fermi_mu_static(E: torch.Tensor, weights, n_electrons: float, kT: float, out: torch.Tensor | None = None):
+    """nao_fermi_mu_static: the Fermi level and occupations without any workspace -- for callers that may not allocate
+    device memory (the host program owns all of it, or cudaMalloc's device-wide synchronisation is not acceptable where
+    the call is made).  The library's own fixed 1.5 MiB scratch array is used instead, so at most
+    FERMI_STATIC_MAX_STATES = 65536 states (E.numel()) are accepted; more raises NaoError (status 5).  Pass `out`
+    (same shape as E, float64, same device) to receive the occupations: then this wrapper allocates nothing on the
+    device either; without it a result tensor is created here for convenience.  All calls share that scratch array: do
+    not overlap two of them on different streams.  Returns (mu, F) exactly as fermi_mu does."""
+    batch, n = E.shape
+    w = (ctypes.c_double * batch)(*[float(x) for x in weights])
+    F = torch.empty_like(E) if out is None else out
+    if F.shape != E.shape or F.dtype != torch.float64:
+        raise NaoError("out must be a float64 tensor of the shape of E")
+    mu = ctypes.c_double(0.0)
+    rc = lib().nao_fermi_mu_static(n, batch, _dev(E, "E"), w, float(n_electrons), float(kT), ctypes.byref(mu),
+                                   _dev(F, "out"), _stream(E))
+    _check(rc, "nao_fermi_mu_static")
     return mu.value, F
 
 

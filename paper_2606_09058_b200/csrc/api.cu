@@ -9,6 +9,7 @@ NAO_EXPORT const char *nao_status_string(int status) {
         case NAO_ERR_CUDA: return "CUDA runtime or launch error";
         case NAO_ERR_ELECTRONS: return "n_electrons outside (0, sum of weights * n) or kT <= 0";
         case NAO_ERR_UNSUPPORTED: return "unsupported combination of arguments";
+        case NAO_ERR_STATIC_LIMIT: return "n * batch exceeds NAO_FERMI_STATIC_MAX_STATES (65536): the built-in scratch of nao_fermi_mu_static is too small, use nao_fermi_mu with a workspace";
         default: return status < 0 ? "invalid argument (index = -status)" : "unknown status";
     }
 }

@@ -217,3 +217,59 @@ NAO_EXPORT int nao_fermi_mu(int n, int batch, const double *dE, const double *h_
     if (int rc = nao::check_occupation_args(n, batch, h_weight, n_electrons, kT, 4)) return rc;
     return nao::fermi_mu(n, batch, dE, h_weight, n_electrons, kT, h_mu, dF, dwork, (cudaStream_t)cuda_stream);
 }
+
+// ---------------------------------------------------------------------------------------------------------------------
+// nao_fermi_mu_static: the Fermi-level search for callers that have no device workspace to hand over (include/nao.h).
+//
+// The sorted energies, their weights, the per-item weights and the device copy of mu -- everything nao_fermi_mu keeps in
+// the caller's `dwork` -- live in the file-scope array below instead.  It is part of the library image: every GPU on
+// which this library's kernels are loaded carries its NAO_FERMI_STATIC_BYTES (1.5 MiB) until the process ends, whether
+// or not this entry point is ever called.  Nothing in the array has to start at zero: each word a kernel reads was
+// written earlier in the same call (the rank sort scatters a permutation of all ns sorted slots), so what the previous
+// call left behind is harmless -- and calls that are on the GPU at the same time (two streams, two host threads) share
+// these bytes and race.
+//
+// In host code `g_fermi_static` is only a handle for the runtime, not an address the GPU understands; the device address
+// is asked for once per device (cudaGetSymbolAddress, with that device current) and remembered.
+// ---------------------------------------------------------------------------------------------------------------------
+namespace nao {
+
+static __device__ __align__(256) unsigned char g_fermi_static[NAO_FERMI_STATIC_BYTES];
+
+enum { FERMI_STATIC_MAX_DEVICES = 64 };
+static void *g_fermi_static_addr[FERMI_STATIC_MAX_DEVICES] = {};   // device address of the array, per device ordinal
+
+// device address of g_fermi_static on the CURRENT device (looked up on the first call made with that device current)
+static int fermi_static_scratch(void **out) {
+    int dev = -1;
+    NAO_CUDA_CHECK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= FERMI_STATIC_MAX_DEVICES) return NAO_ERR_UNSUPPORTED;
+    if (!g_fermi_static_addr[dev]) {
+        void *p = nullptr;
+        NAO_CUDA_CHECK(cudaGetSymbolAddress(&p, g_fermi_static));
+        if (!p) return NAO_ERR_CUDA;
+        g_fermi_static_addr[dev] = p;
+    }
+    *out = g_fermi_static_addr[dev];
+    return NAO_OK;
+}
+
+}  // namespace nao
+
+NAO_EXPORT int nao_fermi_mu_static(int n, int batch, const double *dE, const double *h_weight, double n_electrons,
+                                   double kT, double *h_mu, double *dF, void *cuda_stream) {
+    if (n < 1) return -1;
+    if (batch < 1) return -2;
+    if (!dE) return -3;
+    if (!h_weight) return -4;
+    if (!h_mu) return -7;
+    if (!dF) return -8;
+    // the limit is on the number of states, checked before anything touches the device
+    if ((long)n * (long)batch > (long)NAO_FERMI_STATIC_MAX_STATES) return NAO_ERR_STATIC_LIMIT;
+    size_t need = 0;
+    if (nao_fermi_workspace(n, batch, &need) != NAO_OK || need > (size_t)NAO_FERMI_STATIC_BYTES) return NAO_ERR_STATIC_LIMIT;
+    if (int rc = nao::check_occupation_args(n, batch, h_weight, n_electrons, kT, 4)) return rc;
+    void *scratch = nullptr;
+    if (int rc = nao::fermi_static_scratch(&scratch)) return rc;
+    return nao::fermi_mu(n, batch, dE, h_weight, n_electrons, kT, h_mu, dF, scratch, (cudaStream_t)cuda_stream);
+}
