@@ -316,6 +316,7 @@ def test_config2_full_size_properties(nao):
         bound = (fR * cN + np.abs(got["e"][b]).max() * fF) / (1.0 - fF)
         assert bound <= TOL_E, bound
         ne += prob.weights[b] * np.sum(got["D"][b] * Sb)
+        _check_density_all_entries(to_dev(Cb), torch.from_numpy(got["f"][b]).to(DEV), to_dev(got["D"][b]))   # every entry
         rng = np.random.default_rng(5 + b)
         for (i, j) in rng.integers(0, n, size=(64, 2)):
             dij = float(np.sum(np.asarray(got["f"][b], dtype=np.longdouble) * Cb[i].astype(np.longdouble) * Cb[j].astype(np.longdouble)))
@@ -331,7 +332,8 @@ def test_config3_full_size_certificate(nao):
     The Jacobi oracle would need ~40 core-hours here, so the a-posteriori certificate of SURVEY.md 8c is used: with
     F = C^H S C - I and R = H C - S C diag(e), congruence bounds the error of every eigenvalue by
     (||R||_2 ||C||_2 + max|e| ||F||_2) / (1 - ||F||_2); the products are formed on the GPU by torch (cuBLAS, a checker
-    that shares nothing with the product path).  D is checked on sampled entries from its definition, plus Tr(D S) = N_e."""
+    that shares nothing with the product path).  D is re-formed from (C, f) and compared in EVERY entry (SURVEY.md:414),
+    sampled entries are recomputed in long double from the definition, plus Tr(D S) = N_e."""
     prob = make_config(3)
     n = prob.n
     H = torch.from_numpy(prob.H).to(DEV)
@@ -357,6 +359,8 @@ def test_config3_full_size_certificate(nao):
     fF = float(torch.linalg.norm(Fm)); fR = float(torch.linalg.norm(R)); cN = float(torch.linalg.norm(Cm, ord=2))
     bound = (fR * cN + float(e.abs().max()) * fF) / (1.0 - fF)
     assert bound <= TOL_E, bound
+    del R, Fm, SC, Hm
+    _check_density_all_entries(C[0], F[0], D[0])                  # all 1.0e8 entries, FP64 product by torch
     Dm = D[0].T
     ne = float((Dm * Sm.T).sum().real) * prob.weights[0]          # Tr(D S)
     assert abs(ne - prob.n_electrons) <= 1e-7
@@ -404,11 +408,33 @@ def _nc_certificate(prob, E, C, ncols=None):
     return orth, resid, bound
 
 
+def _check_density_all_entries(C_item, f_item, D_item, tol=TOL_D, block=2048):
+    """EVERY entry of D against its definition D = sum_i f_i c_i c_i^H (Eq. 8 / 23; SURVEY.md:414),
+    re-formed on the GPU by torch in FP64 (cuBLAS: a checker that shares nothing with the product path), column block by
+    column block so that config 4 fits.  C_item / D_item are column-major items (row k of C_item = eigenvector k), f_item the
+    occupations.  States with f < 1e-20 are left out of the reference (they change an entry by < 1e-20 |c|^2).
+    Returns max |D - Dref|."""
+    n = C_item.shape[0]
+    nocc = int((f_item >= 1e-20).nonzero().max()) + 1
+    Cs = C_item[:nocc]                                   # nocc x n, row k = eigenvector k
+    fC = Cs * f_item[:nocc, None].to(Cs.dtype)
+    worst = 0.0
+    for j0 in range(0, n, block):
+        j1 = min(n, j0 + block)
+        ref = Cs[:, j0:j1].mH @ fC                       # stored rows j0..j1 of D: D_item[j, i] = D(i, j)
+        worst = max(worst, float((D_item[j0:j1] - ref).abs().max()))
+        del ref
+    assert worst <= tol, worst
+    return worst
+
+
 def _check_density_from_definition(prob, C, F, D, mu, E, samples, seed):
-    """D against its definition on sampled entries (long double), Hermiticity, Tr(D S) = N_e, mu against the oracle's Fermi
-    solver on the solver's eigenvalues.  Noncollinear layout (S real N x N)."""
+    """D against its definition: every entry against the FP64 product re-formed by torch (1e-8), sampled entries in long
+    double (1e-12: the tie to the definition itself), Hermiticity, Tr(D S) = N_e, mu against the oracle's Fermi solver on the
+    solver's eigenvalues.  Noncollinear layout (S real N x N)."""
     n = prob.n
     N = n // 2
+    _check_density_all_entries(C[0], F[0], D[0])
     Dm = D[0].T
     Sr = torch.from_numpy(np.ascontiguousarray(prob.S[0])).to(DEV)           # S^T as stored = S (symmetric)
     ne = float((Dm[:N, :N] * Sr).sum().real + (Dm[N:, N:] * Sr).sum().real) * prob.weights[0]      # Tr(D S_NC)
@@ -815,12 +841,11 @@ def test_solve_host_matches_the_separate_calls_and_the_oracle(nao, idx, nat):
         assert np.abs(got["D"][b] - sep["D"][b]).max() <= 1e-12
 
 
-def test_config1_full_size_sampled_items(nao):
+def test_config1_full_size_all_items(nao):
     """BASELINE config 1 at full size (64 atoms: n = 832 complex, 8 k-points x 2 spins = 16 items in one batched call, the
-    launch configuration `bench.py --workload c1` times).  The Jacobi oracle needs seconds per item, so four sampled items are
-    solved by it: their eigenvalues, and for two of them the density matrix (oracle eigenvectors, occupations from the shared
-    Fermi level), are compared element by element; mu is checked by the oracle's Fermi solver on all 16 x 832 levels; every
-    item is checked through the invariants of the definition."""
+    launch configuration `bench.py --workload c1` times).  ALL 16 items are solved by the Jacobi oracle: eigenvalues and the
+    density matrix (oracle eigenvectors, occupations from the oracle's Fermi level over all 16 x 832 oracle levels) are
+    compared element by element, mu against the oracle's; every item also goes through the invariants of the definition."""
     prob = make_config(1)
     assert prob.n == 832 and prob.batch == 16 and prob.is_complex
     got = run_path(nao, prob)
@@ -835,11 +860,15 @@ def test_config1_full_size_sampled_items(nao):
         ne += prob.weights[b] * np.sum(got["D"][b] * Sb.T).real
     assert abs(ne - prob.n_electrons) <= 1e-8
     assert np.abs(got["e"][:8] - got["e"][7::-1]).max() <= 1e-10          # e(k) = e(-k)
-    for b in (0, 3, 9, 12):
+    e_all, C_all = [], []
+    for b in range(prob.batch):
         e_or, C_or, _ = oracle.geneig(prob.H_full(b), prob.S_full(b))
         assert np.abs(got["e"][b] - e_or).max() <= TOL_E
-        if b in (3, 12):
-            assert np.abs(got["D"][b] - oracle.density(C_or, f_ref[b])).max() <= TOL_D
+        e_all.append(e_or); C_all.append(C_or)
+    mu_or, f_or = oracle.fermi(np.array(e_all), prob.weights, prob.n_electrons, prob.kT)      # the oracle's own chain
+    assert abs(got["mu"] - mu_or) <= TOL_MU
+    for b in range(prob.batch):
+        assert np.abs(got["D"][b] - oracle.density(C_all[b], f_or[b])).max() <= TOL_D
 
 
 # ------------------------------------------------------------------------------- ill-conditioned overlap (a1/a2 robustness)
