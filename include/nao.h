@@ -126,7 +126,7 @@ int nao_geneig(int n, int batch, int dtype, unsigned flags,
  * vectors equals the one of the full solve as long as every state with f >= 1e-17 lies below n_vec -- check with
  * nao_occupied_count after nao_fermi_mu (an SCF loop takes n_vec from the previous step plus a margin).
  * Combine with NAO_TRD_TWO_STAGE: with few vectors the second back-transformation of the two-stage reduction is cheap and
- * that path is the faster one (config 2: 251 vs 386 ms, config 3: 0.81 vs 1.08 s per step on B200).
+ * that path is the faster one at configs 2 and 3 (measured times: BASELINE.md section 5).
  *   1..4 as nao_geneig;  5 n_vec in 1..n;  the remaining arguments as nao_geneig arguments 5..18.
  * Negative return values count the arguments of THIS signature.
  */
@@ -145,7 +145,7 @@ int nao_geneig_partial(int n, int batch, int dtype, unsigned flags, int n_vec,
  * Arguments as in those three calls (h_weight, h_mu, h_nvec are HOST pointers); dwork needs nao_scf_step_workspace bytes.
  * The call synchronises the stream twice (Fermi level, vector count).
  * Without NAO_TRD_ONE_STAGE / NAO_TRD_TWO_STAGE the fused step takes the two-stage reduction from order 1536 on for real AND
- * complex matrices (few vectors are back-transformed, which favours it: config 3 807 vs 1076 ms).
+ * complex matrices (few vectors are back-transformed, which favours it; measured times: BASELINE.md section 5).
  */
 int nao_scf_step_workspace(int n, int batch, int dtype, unsigned flags, size_t *bytes);
 int nao_scf_step(int n, int batch, int dtype, unsigned flags,
@@ -303,6 +303,7 @@ long nao_launch_count(void);
  * TFLOP/s.  The roofline denominator of the GEMM-class kernels is checked against it. */
 int nao_dmma_peak(double *h_tflops, void *cuda_stream);
 
+/* Calls that run their batch as stream groups (NAO_STREAM_GROUPS_*) record nothing: their launches are on internal streams. */
 int nao_profile_enable(int on);
 int nao_profile_read(double *h_ms, int max_phases);
 const char *nao_profile_phase_name(int i);

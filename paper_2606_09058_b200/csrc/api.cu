@@ -19,13 +19,49 @@ NAO_EXPORT long nao_launch_count(void) { return nao::g_launch_count; }
 namespace nao {
 static int g_sm_limit = 0;
 void set_sm_limit(int limit) { g_sm_limit = limit > 0 ? limit : 0; }
-int sm_count() {
-    static int nsm = 0;
-    if (!nsm) {
-        int dev = 0; cudaGetDevice(&dev);
-        if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm <= 0) nsm = 148;
+// The process-wide state (side streams, events, kernel attributes, pinned words) lives on ONE device: the one that is
+// current at the first call that launches.  Later calls made with another device current are refused instead of using that
+// state across devices.
+static int g_bound_dev = -1, g_bound_sms = 0;
+int bind_device() {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) return NAO_ERR_CUDA;
+    if (g_bound_dev < 0) {
+        int nsm = 0;
+        if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm <= 0) return NAO_ERR_CUDA;
+        g_bound_dev = dev; g_bound_sms = nsm;
     }
+    return dev == g_bound_dev ? NAO_OK : NAO_ERR_CUDA;
+}
+int device_sms() {
+    if (g_bound_dev < 0 && bind_device() != NAO_OK) return 148;
+    return g_bound_sms;
+}
+int sm_count() {
+    const int nsm = device_sms();
     return (g_sm_limit > 0 && g_sm_limit < nsm) ? g_sm_limit : nsm;
+}
+// Streams and events are created into locals and published only when every one of them exists.
+int side_set_init(SideSet &out, int nstreams, int nevents, bool high_priority) {
+    if (out.ready) return NAO_OK;
+    if (nstreams > SideSet::MAX_STREAMS || nevents > SideSet::MAX_EVENTS) return NAO_ERR_UNSUPPORTED;
+    SideSet tmp = {};
+    int prio_lo = 0, prio_hi = 0;
+    bool ok = true;
+    if (high_priority) ok = cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi) == cudaSuccess;
+    int ns = 0, ne = 0;
+    for (; ok && ns < nstreams; ++ns)
+        ok = (high_priority ? cudaStreamCreateWithPriority(&tmp.stream[ns], cudaStreamNonBlocking, prio_hi)
+                            : cudaStreamCreateWithFlags(&tmp.stream[ns], cudaStreamNonBlocking)) == cudaSuccess;
+    for (; ok && ne < nevents; ++ne) ok = cudaEventCreateWithFlags(&tmp.event[ne], cudaEventDisableTiming) == cudaSuccess;
+    if (!ok) {
+        for (int i = 0; i < SideSet::MAX_STREAMS; ++i) if (tmp.stream[i]) cudaStreamDestroy(tmp.stream[i]);
+        for (int i = 0; i < SideSet::MAX_EVENTS; ++i) if (tmp.event[i]) cudaEventDestroy(tmp.event[i]);
+        return NAO_ERR_CUDA;
+    }
+    tmp.ready = true;
+    out = tmp;
+    return NAO_OK;
 }
 }  // namespace nao
 
@@ -34,10 +70,15 @@ namespace nao {
 static const int NPH = 9;
 static const char *kPhaseNames[NPH - 1] = {"potrf_trtri", "reduce_WHWh", "tridiagonalise", "band_to_tridiagonal", "stedc", "back_transform_band", "back_transform", "C_WhZ"};
 static bool g_prof_on = false;
+// While nao_geneig runs its batch as stream groups the launches go to internal streams: events recorded there would time
+// nothing meaningful, so the grouped call records nothing (the timers keep what earlier ungrouped calls recorded).
+static bool g_prof_suspended = false;
+void prof_suspend(bool on) { g_prof_suspended = on; }
+static inline bool prof_active() { return g_prof_on && !g_prof_suspended; }
 static cudaEvent_t g_ev[NPH];
 static bool g_ev_made = false, g_ev_rec[NPH];
 void prof_mark(int idx, cudaStream_t st) {
-    if (!g_prof_on || idx < 0 || idx >= NPH) return;
+    if (!prof_active() || idx < 0 || idx >= NPH) return;
     if (!g_ev_made) { for (int i = 0; i < NPH; ++i) cudaEventCreate(&g_ev[i]); g_ev_made = true; }
     if (idx == 0) for (int i = 0; i < NPH; ++i) g_ev_rec[i] = false;
     cudaEventRecord(g_ev[idx], st); g_ev_rec[idx] = true;
@@ -51,7 +92,7 @@ static cudaEvent_t g_sev[NSLOT][SLOT_CAP][2];
 static int g_scount[NSLOT] = {0, 0}, g_smade[NSLOT] = {0, 0};
 static double g_swork[NSLOT] = {0.0, 0.0};
 int prof_kernel_begin(int slot, double work, cudaStream_t st) {
-    if (!g_prof_on || slot < 0 || slot >= NSLOT || g_scount[slot] >= SLOT_CAP) return -1;
+    if (!prof_active() || slot < 0 || slot >= NSLOT || g_scount[slot] >= SLOT_CAP) return -1;
     int k = g_scount[slot];
     if (k >= g_smade[slot]) { cudaEventCreate(&g_sev[slot][k][0]); cudaEventCreate(&g_sev[slot][k][1]); g_smade[slot] = k + 1; }
     cudaEventRecord(g_sev[slot][k][0], st);
@@ -67,12 +108,13 @@ __global__ void grouped_flops_kernel(const GemmDesc *d, int ngroups, double per_
         if (d[g].m > 0 && d[g].n > 0 && d[g].k > 0)
             s += per_mnk * d[g].m * (double)d[g].n * d[g].k * (d[g].cmode != 0 ? 0.5 : 1.0) *
                  ((d[g].maskA != MASK_NONE || d[g].maskB != MASK_NONE) ? 0.5 : 1.0);
+    // one warp, fixed order, one plain add: launches on a stream are ordered, so the total does not depend on timing
     for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-    if ((threadIdx.x & 31) == 0 && s != 0.0) atomicAdd(&g_grouped_flops, s);
+    if (threadIdx.x == 0 && s != 0.0) g_grouped_flops += s;
 }
 void prof_grouped_flops(const GemmDesc *d_descs, int ngroups, double per_mnk, cudaStream_t st) {
-    if (!g_prof_on || !d_descs || ngroups <= 0) return;
-    grouped_flops_kernel<<<1, 128, 0, st>>>(d_descs, ngroups, per_mnk);
+    if (!prof_active() || !d_descs || ngroups <= 0) return;
+    grouped_flops_kernel<<<1, 32, 0, st>>>(d_descs, ngroups, per_mnk);
 }
 void prof_kernel_end(int slot, int k, cudaStream_t st) {
     if (k < 0) return;
@@ -156,6 +198,7 @@ __global__ void __launch_bounds__(512) dmma_peak_kernel(int iters, double *sink)
 NAO_EXPORT int nao_dmma_peak(double *h_tflops, void *cuda_stream) {
     using namespace nao;
     if (!h_tflops) return -1;
+    if (int rcb = nao::bind_device()) return rcb;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int dev = 0, nsm = 148;
     cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);

@@ -191,6 +191,7 @@ NAO_EXPORT int nao_potrf_trtri(int n, int batch, int dtype, void *dS, long lds, 
     if (!dLinv) return -7;
     if (!dtmp) return -8;
     if (!d_info) return -9;
+    if (int rcb = nao::bind_device()) return rcb;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (cudaMemsetAsync(d_info, 0, sizeof(int) * batch, st) != cudaSuccess) return NAO_ERR_CUDA;
     int rc = potrf_trtri(dtype, n, batch, dS, lds, strideS, dLinv, n, (long)n * n, dtmp, n, (long)n * n, d_info, st);

@@ -55,6 +55,7 @@ NAO_EXPORT int nao_density_matrix(int n, int batch, int dtype, const void *dC, l
     if (!dwork) return -11;
     size_t need; nao_density_workspace(n, batch, dtype, &need);
     if (work_bytes < need) return NAO_ERR_WORKSPACE;
+    if (int rcb = nao::bind_device()) return rcb;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     GemmDesc *descs = (GemmDesc *)dwork;
     dm_setup_kernel<<<batch, 32, 0, st>>>(n, dtype, dC, ldc, strideC, dF, dD, ldd, strideD, descs);
@@ -91,6 +92,7 @@ NAO_EXPORT int nao_occupied_count(int n, int batch, const double *dF, double thr
     if (batch < 1) return -2;
     if (!dF) return -3;
     if (!h_count) return -5;
+    if (int rcb = nao::bind_device()) return rcb;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     static int *h_pinned = nullptr, *d_mapped = nullptr;
     if (!h_pinned) {

@@ -215,6 +215,7 @@ NAO_EXPORT int nao_fermi_mu(int n, int batch, const double *dE, const double *h_
     if (!dF) return -8;
     if (!dwork) return -9;
     if (int rc = nao::check_occupation_args(n, batch, h_weight, n_electrons, kT, 4)) return rc;
+    if (int rcb = nao::bind_device()) return rcb;
     return nao::fermi_mu(n, batch, dE, h_weight, n_electrons, kT, h_mu, dF, dwork, (cudaStream_t)cuda_stream);
 }
 
@@ -269,6 +270,7 @@ NAO_EXPORT int nao_fermi_mu_static(int n, int batch, const double *dE, const dou
     size_t need = 0;
     if (nao_fermi_workspace(n, batch, &need) != NAO_OK || need > (size_t)NAO_FERMI_STATIC_BYTES) return NAO_ERR_STATIC_LIMIT;
     if (int rc = nao::check_occupation_args(n, batch, h_weight, n_electrons, kT, 4)) return rc;
+    if (int rc = nao::bind_device()) return rc;
     void *scratch = nullptr;
     if (int rc = nao::fermi_static_scratch(&scratch)) return rc;
     return nao::fermi_mu(n, batch, dE, h_weight, n_electrons, kT, h_mu, dF, scratch, (cudaStream_t)cuda_stream);

@@ -95,6 +95,7 @@ NAO_EXPORT int nao_energy_weights(int n, int batch, const double *dE, const doub
     if (!dE) return -3;
     if (!dF) return -4;
     if (!dFE) return -5;
+    if (int rcb = nao::bind_device()) return rcb;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     long total = (long)n * batch;
     energy_weights_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(total, dE, dF, dFE);
@@ -132,6 +133,7 @@ NAO_EXPORT int nao_fold_density(int n, int nk, int nR, int out_dtype, const void
     if (!dwork) return -14;
     size_t need; nao_fold_workspace(nk, nR, &need);
     if (work_bytes < need) return NAO_ERR_WORKSPACE;
+    if (int rcb = nao::bind_device()) return rcb;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     double *d_k = (double *)dwork, *d_w = d_k + 3 * (size_t)nk, *d_R = d_w + nk;
     cplx *table = (cplx *)((char *)dwork + align_up(sizeof(double) * (4 * (size_t)nk + 3 * (size_t)nR)));

@@ -524,5 +524,6 @@ NAO_EXPORT int nao_gemm(int dtype, int opA, int opB, int m, int n, int k, double
     if (batch < 0) return -18;
     GemmDesc d = gemm_desc(opA, opB, m, n, k, alpha, dA, lda, dB, ldb, beta, dC, ldc);
     d.sA = strideA; d.sB = strideB; d.sC = strideC; d.cmode = uplo_c ? 1 : 0;
+    if (int rcb = nao::bind_device()) return rcb;
     return gemm_launch(dtype, d, batch, (cudaStream_t)cuda_stream);
 }

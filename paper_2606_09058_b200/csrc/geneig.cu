@@ -154,6 +154,7 @@ NAO_EXPORT int nao_heev(int n, int batch, int dtype, unsigned flags, void *dA, l
     if (!dwork) return -12;
     if (work_bytes < heev_plan(dtype, n, batch, flags).bytes) return NAO_ERR_WORKSPACE;
     if (!d_info) return -14;
+    if (int rcb = bind_device()) return rcb;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (cudaMemsetAsync(d_info, 0, sizeof(int) * batch, st) != cudaSuccess) return NAO_ERR_CUDA;
     return heev(dtype, n, batch, flags, dA, lda, strideA, dE, dZ, ldz, strideZ, dwork, d_info, st);
@@ -211,6 +212,7 @@ static int geneig_impl(int n, int batch, int dtype, unsigned flags, int nvec, co
     GePlan p = ge_plan(n, batch, dtype, flags, shared_S);
     if (work_bytes < p.bytes) return NAO_ERR_WORKSPACE;
     if (!d_info) return -17;
+    if (phase != 0) if (int rcb = bind_device()) return rcb;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     char *w = (char *)dwork;
     const size_t es = esize(dtype);
@@ -346,30 +348,29 @@ static int geneig_grouped(int n, int batch, int dtype, unsigned flags, int nvec,
     int rc = geneig_impl(n, batch, dtype, flags, nvec, dH, ldh, strideH, dS, lds, strideS, dE, dC, ldc, strideC, dwork, (size_t)-1,
                          d_info, cuda_stream, 0);
     if (rc) return rc;
-    static cudaStream_t side[8] = {nullptr};
-    static cudaEvent_t ev_fork = nullptr, ev_join[8] = {nullptr};
-    if (!ev_fork) {
-        NAO_CUDA_CHECK(cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming));
-        for (int g = 0; g < 8; ++g) {
-            NAO_CUDA_CHECK(cudaStreamCreateWithFlags(&side[g], cudaStreamNonBlocking));
-            NAO_CUDA_CHECK(cudaEventCreateWithFlags(&ev_join[g], cudaEventDisableTiming));
-        }
-    }
+    if ((rc = bind_device())) return rc;
+    static SideSet ss = {};
+    if ((rc = side_set_init(ss, 8, 9, false))) return rc;
+    cudaStream_t *side = ss.stream;
+    const cudaEvent_t ev_fork = ss.event[8], *ev_join = ss.event;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t es = esize(dtype), esS = (flags & NAO_NC_BLOCK_S) ? 8 : es;
     set_sm_limit(sm_count() / groups);
+    prof_suspend(true);                   // launches go to internal streams: the phase / kernel timers record nothing
     size_t off = 0;
     for (int g = 0; g < groups && rc == NAO_OK; ++g) {
         const int b0 = (int)((long)batch * g / groups), b1 = (int)((long)batch * (g + 1) / groups);
         off += align_up(ge_plan(n, b1 - b0, dtype, flags, strideS == 0).bytes);
     }
-    if (off > work_bytes) { set_sm_limit(0); return NAO_ERR_WORKSPACE; }
-    if (cudaEventRecord(ev_fork, st) != cudaSuccess) { set_sm_limit(0); return NAO_ERR_CUDA; }
+    if (off > work_bytes) { set_sm_limit(0); prof_suspend(false); return NAO_ERR_WORKSPACE; }
+    if (cudaEventRecord(ev_fork, st) != cudaSuccess) { set_sm_limit(0); prof_suspend(false); return NAO_ERR_CUDA; }
     off = 0;
+    int forked = 0;                        // groups whose internal stream has been given work
     for (int g = 0; g < groups; ++g) {
         const int b0 = (int)((long)batch * g / groups), b1 = (int)((long)batch * (g + 1) / groups), nb = b1 - b0;
         const size_t need = ge_plan(n, nb, dtype, flags, strideS == 0).bytes;
         if (cudaStreamWaitEvent(side[g], ev_fork, 0) != cudaSuccess) { rc = NAO_ERR_CUDA; break; }
+        forked = g + 1;
         rc = geneig_impl(n, nb, dtype, flags, nvec, (const char *)dH + (size_t)b0 * strideH * es, ldh, strideH,
                          (char *)dS + (size_t)b0 * strideS * esS, lds, strideS, dE + (size_t)b0 * n,
                          (char *)dC + (size_t)b0 * strideC * es, ldc, strideC, (char *)dwork + off, need, d_info + b0, side[g]);
@@ -380,6 +381,12 @@ static int geneig_grouped(int n, int batch, int dtype, unsigned flags, int nvec,
         }
     }
     set_sm_limit(0);
+    prof_suspend(false);
+    // error exit: whatever the groups already enqueued still runs against the caller's buffers -- order the caller's stream
+    // behind all of it (on the success path every group was joined above)
+    if (rc)
+        for (int g = 0; g < forked; ++g)
+            if (cudaEventRecord(ev_join[g], side[g]) == cudaSuccess) cudaStreamWaitEvent(st, ev_join[g], 0);
     return rc;
 }
 
@@ -411,7 +418,7 @@ extern "C" int nao_density_matrix(int n, int batch, int dtype, const void *dC, l
                                   long ldd, long strideD, void *dwork, size_t work_bytes, void *cuda_stream);
 
 // The fused step back-transforms only the occupied vectors, which favours the two-stage reduction for complex matrices as
-// well (config 3: 831 vs 1141 ms per step); below order 1536 the one-stage path stays ahead (config 1: 34 vs 40 ms).
+// well; below order 1536 the one-stage path stays ahead (measured times of both: BASELINE.md section 5).
 static unsigned scf_step_flags(int n, unsigned flags) {
     flags &= ~NAO_STREAM_GROUPS_MASK;          // the fused step runs as one group
     if (!(flags & (NAO_TRD_ONE_STAGE | NAO_TRD_TWO_STAGE)) && n >= nao::TWO_STAGE_MIN_N_REAL) flags |= NAO_TRD_TWO_STAGE;
@@ -554,15 +561,12 @@ NAO_EXPORT int nao_solve_host(int n, int batch, int dtype, unsigned flags, const
     if (rc) return rc;
     if (work_bytes < p.bytes) return NAO_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    static cudaStream_t cs = nullptr;
-    static cudaEvent_t ev_start = nullptr, ev_h = nullptr, ev_d = nullptr, ev_end = nullptr;
-    if (!cs) {
-        NAO_CUDA_CHECK(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
-        NAO_CUDA_CHECK(cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming));
-        NAO_CUDA_CHECK(cudaEventCreateWithFlags(&ev_h, cudaEventDisableTiming));
-        NAO_CUDA_CHECK(cudaEventCreateWithFlags(&ev_d, cudaEventDisableTiming));
-        NAO_CUDA_CHECK(cudaEventCreateWithFlags(&ev_end, cudaEventDisableTiming));
-    }
+    if ((rc = bind_device())) return rc;
+    static SideSet ss = {};
+    if ((rc = side_set_init(ss, 1, 5, false))) return rc;
+    const cudaStream_t cs = ss.stream[0];
+    const cudaEvent_t ev_start = ss.event[0], ev_h = ss.event[1], ev_d = ss.event[2], ev_end = ss.event[3];
+    SideJoin join(cs, st, ss.event[4]);        // error exits: the caller's stream still ends behind the copy stream
     char *w = (char *)dwork;
     const size_t es = esize(dtype);
     const size_t item = (size_t)n * n * es;
@@ -572,6 +576,7 @@ NAO_EXPORT int nao_solve_host(int n, int batch, int dtype, unsigned flags, const
     // the copy stream starts behind whatever the caller's stream still does with the scratch
     NAO_CUDA_CHECK(cudaEventRecord(ev_start, st));
     NAO_CUDA_CHECK(cudaStreamWaitEvent(cs, ev_start, 0));
+    join.arm();
     NAO_CUDA_CHECK(cudaMemcpyAsync(dS, hS, (size_t)p.nitemsS * p.nS * p.nS * p.esS, cudaMemcpyHostToDevice, st));
     NAO_CUDA_CHECK(cudaMemcpyAsync(dH, hH, (size_t)batch * item, cudaMemcpyHostToDevice, cs));
     NAO_CUDA_CHECK(cudaEventRecord(ev_h, cs));

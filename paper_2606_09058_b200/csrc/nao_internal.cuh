@@ -21,6 +21,26 @@ extern long g_launch_count;          // host-side count of kernel launches (nao_
 // co-resident on disjoint SMs instead of waiting for one another.
 int sm_count();
 void set_sm_limit(int limit);        // 0 = no limit
+// The library's process-wide state belongs to one device (include/nao.h).  bind_device(): records the current device on the
+// first call, afterwards NAO_ERR_CUDA when another device is current -- called by every entry point after its host-side
+// argument checks and before its first launch.  device_sms(): SM count of that device (cached).
+int bind_device();
+int device_sms();
+// Internal streams and events of one call site, created together: all of them exist afterwards, or none (ready stays false).
+struct SideSet {
+    enum { MAX_STREAMS = 8, MAX_EVENTS = 10 };
+    cudaStream_t stream[MAX_STREAMS]; cudaEvent_t event[MAX_EVENTS]; bool ready;
+};
+int side_set_init(SideSet &s, int nstreams, int nevents, bool high_priority);
+// Scope guard of a function that forks work onto an internal stream: once armed, leaving the scope -- by ANY return, error
+// exits included -- orders the caller's stream behind everything enqueued on the internal stream so far, so that no kernel
+// is still running against the caller's buffers on a stream the caller cannot see.
+struct SideJoin {
+    cudaStream_t side, st; cudaEvent_t ev; bool armed;
+    SideJoin(cudaStream_t side_, cudaStream_t st_, cudaEvent_t ev_) : side(side_), st(st_), ev(ev_), armed(false) {}
+    void arm() { armed = true; }
+    ~SideJoin() { if (armed && cudaEventRecord(ev, side) == cudaSuccess) cudaStreamWaitEvent(st, ev, 0); }
+};
 #define NAO_LAUNCHED() (++::nao::g_launch_count)
 
 #define NAO_CUDA_CHECK(expr)                                        \
@@ -174,6 +194,8 @@ int stedc(int n, int batch, double *d, double *e, double *evals, double *Q, long
 
 // api.cu: phase-boundary event (no-op unless nao_profile_enable(1))
 void prof_mark(int idx, cudaStream_t st);
+// on: nothing is recorded until prof_suspend(false) (used around a call that runs as stream groups)
+void prof_suspend(bool on);
 // per-launch timers: slot 0 = hetrd_panel_kernel (work = algorithmic HBM bytes), slot 1 = gemm_kernel (work = flops)
 int prof_kernel_begin(int slot, double work, cudaStream_t st);
 void prof_kernel_end(int slot, int k, cudaStream_t st);

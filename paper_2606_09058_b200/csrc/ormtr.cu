@@ -169,18 +169,12 @@ static int ormtr_impl(int dtype, int n, int ncols, int batch, int shift, const T
     // xLARFT recurrence on the diagonal 128-blocks, off-diagonal blocks by doubling).  The factor of block blk-1 is built on
     // an internal high-priority side stream while the three large products of block blk run on the caller's stream.
     // (Not while a stream group limits the SMs: the groups overlap one another instead.)
-    static cudaStream_t side = nullptr;
-    static cudaEvent_t ev_fork = nullptr, ev_T = nullptr;
-    int dev_sms = 0, dev = 0;
-    cudaGetDevice(&dev); cudaDeviceGetAttribute(&dev_sms, cudaDevAttrMultiProcessorCount, dev);
-    const bool ahead = sm_count() >= dev_sms && nblocks > 1 && n >= 1024;
-    if (ahead && !side) {
-        int prio_lo = 0, prio_hi = 0;
-        cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
-        NAO_CUDA_CHECK(cudaStreamCreateWithPriority(&side, cudaStreamNonBlocking, prio_hi));
-        NAO_CUDA_CHECK(cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming));
-        NAO_CUDA_CHECK(cudaEventCreateWithFlags(&ev_T, cudaEventDisableTiming));
-    }
+    static SideSet ss = {};
+    const bool ahead = sm_count() >= device_sms() && nblocks > 1 && n >= 1024;
+    if (ahead) if (int rc = side_set_init(ss, 1, 3, true)) return rc;
+    const cudaStream_t side = ss.stream[0];
+    const cudaEvent_t ev_fork = ss.event[0], ev_T = ss.event[1];
+    SideJoin join(side, st, ss.event[2]);      // armed at the first fork: every exit path rejoins the side stream
     // T factor of block blk into Tm (kb x kb, ld kb) on stream qs; Vx = explicit V of the block (output), Gx, tmpx, Px = scratch
     auto build_t = [&](int blk, T *Tm, T *Vx, T *Gx, T *tmpx, void *Px, cudaStream_t qs) -> int {
         const int jb = blk * BLK, kb = std::min(BLK, nref - jb), m = n - jb - shift;
@@ -225,6 +219,7 @@ static int ormtr_impl(int dtype, int n, int ncols, int batch, int shift, const T
                 // everything enqueued so far (incl. the last use of the other T buffer) precedes the side stream's work
                 NAO_CUDA_CHECK(cudaEventRecord(ev_fork, st));
                 NAO_CUDA_CHECK(cudaStreamWaitEvent(side, ev_fork, 0));
+                join.arm();
                 if (int rc = build_t(blk - 1, Tbuf[(blk - 1) & 1], (T *)w.Vs, (T *)w.G, (T *)w.tmp, w.Ps, side)) return rc;
                 NAO_CUDA_CHECK(cudaEventRecord(ev_T, side));
             }

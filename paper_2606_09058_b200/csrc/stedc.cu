@@ -604,6 +604,7 @@ NAO_EXPORT int nao_stedc(int n, int batch, double *dD, double *dEoff, double *dE
     if (!dwork) return -9;
     if (work_bytes < nao::stedc_workspace(n, batch)) return NAO_ERR_WORKSPACE;
     if (!d_info) return -11;
+    if (int rcb = nao::bind_device()) return rcb;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (cudaMemsetAsync(d_info, 0, sizeof(int) * batch, st) != cudaSuccess) return NAO_ERR_CUDA;
     return nao::stedc(n, batch, dD, dEoff, dE, dQ, ldq, strideQ, dwork, d_info, st);

@@ -1,7 +1,11 @@
 // stedc_core.cuh -- scalar building blocks of the tridiagonal divide-and-conquer eigensolver (
 // the paper names the method -- "divide-and-conquer ... dominated by matrix multiplications", PAPER.md:744 -- the
 // algorithm itself is Cuppen's rank-one tearing with Gu/Eisenstat deflation and Loewner-formula eigenvectors, restated
-// here from the published algorithm).
+// here from the published algorithm).  The formulations followed are the ones the reference libraries made standard:
+// `deflate_range` is the deflation loop of LAPACK dlaed2 (its column types 1-4 and index names are kept so that the two can be
+// read side by side), `secular_root` follows LAPACK dlaed4's scheme (origin shifted to the nearer pole, the `erretm` stopping
+// test, the two-pole "middle way" step), and `ql_implicit` is the implicit QL iteration of EISPACK tql2 / imtql2 in its
+// textbook form.  No library source is copied; the code is written from the published descriptions of those routines.
 //
 //   T = [T1 0; 0 T2] + rho v v^T  ->  D + rho z z^T  ->  deflation  ->  secular equation  ->  eigenvectors.
 //

@@ -316,19 +316,12 @@ static int he2hb_impl(int dtype, int n, int batch, T *A, long lda, long sA, T *t
     // panel p+1 first, then -- on an internal side stream, on as few CTAs as hold the panel in shared memory -- the QR of
     // panel p+1 WHILE the rest of the update runs on the caller's stream (its CTAs fill the SMs the QR leaves free).
     // Disabled while a stream group limits the SMs (the groups overlap one another instead).
-    static cudaStream_t side = nullptr;
-    static cudaEvent_t ev_cols = nullptr, ev_side = nullptr, ev_qr = nullptr;
-    int dev_sms = 0, dev = 0;
-    cudaGetDevice(&dev); cudaDeviceGetAttribute(&dev_sms, cudaDevAttrMultiProcessorCount, dev);
-    const bool lookahead = sm_count() >= dev_sms && n >= 1024;
-    if (lookahead && !side) {
-        int prio_lo = 0, prio_hi = 0;
-        cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);      // the QR's CTAs take freed SMs before the update's
-        NAO_CUDA_CHECK(cudaStreamCreateWithPriority(&side, cudaStreamNonBlocking, prio_hi));
-        NAO_CUDA_CHECK(cudaEventCreateWithFlags(&ev_cols, cudaEventDisableTiming));
-        NAO_CUDA_CHECK(cudaEventCreateWithFlags(&ev_side, cudaEventDisableTiming));
-        NAO_CUDA_CHECK(cudaEventCreateWithFlags(&ev_qr, cudaEventDisableTiming));
-    }
+    static SideSet ss = {};
+    const bool lookahead = sm_count() >= device_sms() && n >= 1024;
+    if (lookahead) if (int rc = side_set_init(ss, 1, 4, true)) return rc;   // high priority: the QR's CTAs take freed SMs first
+    const cudaStream_t side = ss.stream[0];
+    const cudaEvent_t ev_cols = ss.event[0], ev_side = ss.event[1], ev_qr = ss.event[2];
+    SideJoin join(side, st, ss.event[3]);      // armed at the first fork: every exit path rejoins the side stream
     const int cap_rows = (int)((200 * 1024) / ((size_t)(b + 1) * sizeof(T))) - 2;       // panel rows one CTA can hold
     auto launch_qr = [&](int j0, int panel, cudaStream_t qs, bool few_ctas) -> int {
         const int m = n - j0 - b;
@@ -384,10 +377,11 @@ static int he2hb_impl(int dtype, int n, int batch, T *A, long lda, long sA, T *t
         if (lookahead && next_panel && m - b >= 512) {
             // 5a. the b columns of the next panel (rows jr.. : its diagonal block and everything below)
             GemmDesc ua = gemm_desc(OP_N, OP_C, m, b, 2 * b, -1.0, Vb + jr, n, Wb + jr, n, 1.0, A22, lda);
-            ua.sA = sP4; ua.sB = sP4; ua.sC = sA; ua.cmode = 1;
+            ua.sA = sP4; ua.sB = sP4; ua.sC = sA;        // (cmode 0: one tile column starting at the diagonal, no tile is skipped)
             if (int rc = gemm_launch(dtype, ua, batch, st)) return rc;
             NAO_CUDA_CHECK(cudaEventRecord(ev_cols, st));
             NAO_CUDA_CHECK(cudaStreamWaitEvent(side, ev_cols, 0));
+            join.arm();
             NAO_CUDA_CHECK(cudaEventRecord(ev_side, side));
             // QR of panel p+1 on the (high-priority) side stream; the big update is held back until the side stream has got
             // past its wait, so that the QR's CTAs are placed first and the update fills the SMs they leave free

@@ -544,8 +544,8 @@ static int q2_apply_impl(int n, int ncols, int batch, const T *V2, long ldv, lon
     // Columns per CTA: one CTA per SM walks through all diamonds, so the slab width is what gives every SM the same share.
     // Units of 8 columns, spread over the four schedulers of an SM: u units per scheduler as 16-column warps (real) plus at
     // most one 8-column warp each.
-    int nsm = 148, dev = 0;
-    cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+    // (sm_count(): under NAO_STREAM_GROUPS_* a group's share of the SMs, so that the groups' kernels run side by side)
+    const int nsm = sm_count();
     const long units_sm = std::max(1L, ((long)ceil_div(ncols, 8) * batch + nsm - 1) / nsm);      // 8-column units per SM
     int NW, n2 = 0;
     bool wide = false;                                               // 12 eight-column warps (three per scheduler)

@@ -1028,6 +1028,55 @@ def test_stream_groups_equal_the_single_batched_call(nao, groups):
                 assert np.abs(to_np(D2)[b] - ref["D"][b]).max() <= TOL_D
 
 
+def test_stream_groups_two_stage_order_2080_shared_factor(nao):
+    """The SM-limited plans of the two-stage path only differ from the unlimited ones from order 1024 on (panel-QR CTAs per
+    item, chase CTAs, the look-ahead switched off, q2_apply's slab width): four real items of order 2080 (config-2 recipe at 160
+    atoms, the second pair with H scaled) under NAO_STREAM_GROUPS_4 = one item per group on 37 SMs, full and partial spectrum,
+    against the single batched call.  Then ONE shared overlap (strideS = 0) that is already factored (NAO_S_FACTORED): the
+    only grouped case in which the workspace query (shared S counted once) and the run (every group unpacks the shared factor)
+    see different S layouts."""
+    prob = make_config(2, nat=160)
+    n = prob.n
+    assert n == 2080 and np.array_equal(prob.S[0], prob.S[1])
+    H = torch.from_numpy(np.concatenate([prob.H, 0.5 * prob.H])).to(DEV)
+    S4 = np.concatenate([prob.S, prob.S])
+    g4 = nao.NAO_STREAM_GROUPS_4
+    S1, S2 = torch.from_numpy(S4.copy()).to(DEV), torch.from_numpy(S4.copy()).to(DEV)
+    E1, C1, i1 = nao.geneig(H, S1)                                   # default = two-stage at this order
+    E2, C2, i2 = nao.geneig(H, S2, flags=g4)
+    assert int(i1.abs().max()) == 0 and int(i2.abs().max()) == 0
+    assert float((S1 - S2).abs().max()) <= 1e-12
+    assert float((E1 - E2).abs().max()) <= 1e-12
+    assert float((E1[2:] - 0.5 * E1[:2]).abs().max()) <= 1e-12        # the scaled pair
+    mu, F = nao.fermi_mu(E1, list(prob.weights) * 2, 2 * prob.n_electrons, prob.kT)
+    nv = nao.occupied_count(F) + 8
+    assert nv < n // 2
+    D1, D2 = nao.density_matrix(C1, F), nao.density_matrix(C2, F)
+    assert float((D1 - D2).abs().max()) <= 1e-10
+    Cm = C2[3].T                                                      # an item of the last group: C^T S C = I, residual
+    Sm = torch.from_numpy(prob.S_full(1)).to(DEV)
+    assert float((Cm.T @ Sm @ Cm - torch.eye(n, dtype=torch.float64, device=DEV)).abs().max()) <= TOL_ORTH
+    Hm = 0.5 * torch.from_numpy(prob.H_full(1)).to(DEV)
+    assert float((Hm @ Cm - (Sm @ Cm) * E2[3][None, :]).abs().max()) <= 1e-10
+    # partial spectrum, cached per-item factor
+    E3, C3, _ = nao.geneig(H, S2, flags=g4 | nao.NAO_S_FACTORED, n_vec=nv)
+    assert float((E3 - E1).abs().max()) <= 1e-12
+    assert float((nao.density_matrix(C3, F) - D1).abs().max()) <= 1e-10
+    assert float(C3[:, nv:].abs().max()) == 0.0
+    # one shared overlap: factored by an ungrouped call (the group flag is ignored while S is unfactored), reused by groups
+    Ss = torch.from_numpy(prob.S[:1].copy()).to(DEV)
+    E5, C5, i5 = nao.geneig(H, Ss, flags=g4)
+    assert int(i5.abs().max()) == 0
+    assert float((E5 - E1).abs().max()) <= 1e-12 and float((Ss[0] - S1[0]).abs().max()) <= 1e-12
+    E6, C6, i6 = nao.geneig(H, Ss, flags=g4 | nao.NAO_S_FACTORED)
+    assert int(i6.abs().max()) == 0
+    assert float((E6 - E1).abs().max()) <= 1e-12
+    assert float((nao.density_matrix(C6, F) - D1).abs().max()) <= 1e-10
+    E7, C7, _ = nao.geneig(H, Ss, flags=nao.NAO_STREAM_GROUPS_2 | nao.NAO_S_FACTORED, n_vec=nv)
+    assert float((E7 - E1).abs().max()) <= 1e-12
+    assert float((nao.density_matrix(C7, F) - D1).abs().max()) <= 1e-10
+
+
 # ------------------------------------------------------------------------------- flag-synchronised kernels: reproducibility
 @pytest.mark.parametrize("cplx", [False, True])
 def test_flag_synchronised_kernels_are_bit_reproducible(nao, cplx):
