@@ -121,7 +121,22 @@ __global__ void __launch_bounds__(1024) fermi_bisect_kernel(int ns, const double
     const double r = n_electrons - s_W;
     double lo = es[0] - 50.0 * kT, hi = es[ns - 1] + 50.0 * kT;
     const bool logform = (r == 0.0 && m > 0);
-
+    // States far from mu cost nothing: the bisection would otherwise spend three FP64 transcendentals per state and step on one
+    // SM.  XCUT = 100: exp(-100) = 3.7e-44.  Plain form: for x < -XCUT the occupation is 1 to that accuracy (the sum gets w
+    // itself, which is also what the full expression rounds to), for x > XCUT the term is below 3.7e-44 w and is dropped.
+    // Log form: a term is dropped when it is more than e^-100 below the term of the state next to the split on its side,
+    // which the sorted order makes the largest up to the weight ratio (lw = log(w_max / w_min)).
+    // The states that are left lie next to one another in the sorted order, so inside the bisection the states are dealt
+    // round-robin (thread t takes t, t + 1024, ...) instead of in the contiguous chunks of the scan above: the few hundred
+    // live states then cost one or two evaluations per thread, not 13 in a handful of threads.  Still a fixed order.
+    const double XCUT = 100.0;
+    double lw = 0.0;
+    if (logform) {
+        double wmx = 0.0, wmn = -INFINITY;
+        for (int j = tid; j < ns; j += nt) { wmx = fmax(wmx, ws[j]); wmn = fmax(wmn, -ws[j]); }
+        wmx = bs.max(wmx); wmn = -bs.max(wmn);
+        lw = log(wmx / wmn);
+    }
 
     for (int it = 0; it < 400; ++it) {
         double mu = 0.5 * (lo + hi);
@@ -130,28 +145,41 @@ __global__ void __launch_bounds__(1024) fermi_bisect_kernel(int ns, const double
         if (logform) {
             // t_j = log w_j + log f_j (j >= m) or log w_j + log(1 - f_j) (j < m); kept in shared memory between the two passes
             // when the states fit there (cache != 0)
+            const double cutP = (m < ns ? fmax((es[m] - mu) / kT, 0.0) : 0.0) + XCUT + 1.0 + lw;
+            const double cutQ = fmax((mu - es[m - 1]) / kT, 0.0) + XCUT + 1.0 + lw;
             double mp = -INFINITY, mq = -INFINITY;
-            for (int j = j0; j < j1; ++j) {
-                double x = (es[j] - mu) / kT;
-                double t = log(ws[j]) - (j >= m ? softplus(x) : softplus(-x));
+            for (int j = tid; j < ns; j += nt) {
+                const double xs = (j >= m) ? (es[j] - mu) / kT : (mu - es[j]) / kT;
+                double t = -INFINITY;
+                if (fmax(xs, 0.0) <= (j >= m ? cutP : cutQ)) t = log(ws[j]) - softplus(xs);
                 if (cache) s_tj[j] = t;
                 if (j >= m) mp = fmax(mp, t); else mq = fmax(mq, t);
             }
             mp = bs.max(mp); mq = bs.max(mq);
             double sp = 0.0, sq = 0.0;
-            for (int j = j0; j < j1; ++j) {
+            for (int j = tid; j < ns; j += nt) {
                 double t;
                 if (cache) t = s_tj[j];
-                else { double x = (es[j] - mu) / kT; t = log(ws[j]) - (j >= m ? softplus(x) : softplus(-x)); }
+                else {
+                    const double xs = (j >= m) ? (es[j] - mu) / kT : (mu - es[j]) / kT;
+                    t = (fmax(xs, 0.0) <= (j >= m ? cutP : cutQ)) ? log(ws[j]) - softplus(xs) : -INFINITY;
+                }
+                if (t == -INFINITY) continue;
                 if (j >= m) sp += exp(t - mp); else sq += exp(t - mq);
             }
             sp = bs.sum(sp); sq = bs.sum(sq);
             positive = (mp + log(sp)) > (mq + log(sq));
         } else {
             double P = 0.0, Q = 0.0;
-            for (int j = j0; j < j1; ++j) {
-                double x = (es[j] - mu) / kT;
-                if (j >= m) P += ws[j] * exp(-softplus(x)); else Q += ws[j] * exp(-softplus(-x));
+            for (int j = tid; j < ns; j += nt) {
+                const double x = (es[j] - mu) / kT;
+                if (j >= m) {
+                    if (x > XCUT) continue;
+                    P += (x < -XCUT) ? ws[j] : ws[j] * exp(-softplus(x));
+                } else {
+                    if (x < -XCUT) continue;
+                    Q += (x > XCUT) ? ws[j] : ws[j] * exp(-softplus(-x));
+                }
             }
             P = bs.sum(P); Q = bs.sum(Q);
             positive = (P - Q - r) > 0.0;

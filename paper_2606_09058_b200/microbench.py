@@ -5,6 +5,7 @@ command the ncu captures summarised under profiles/ run.  Library kernels only.
                                                     [--beta B] [--lower] [--reps R]
     python -m paper_2606_09058_b200.microbench heev [--n N] [--batch B] [--complex] [--two-stage|--one-stage]
     python -m paper_2606_09058_b200.microbench fold [--n N] [--nk NK] [--nr NR] [--complex]      (config 1: 832, 8, 27)
+    python -m paper_2606_09058_b200.microbench fermi [--n N] [--batch B]                         (config 2: 6656, 2; config 1: 832, 16)
 
 Prints one JSON line per measurement.
 """
@@ -113,9 +114,33 @@ def bench_fold(args):
                       "algorithmic_bytes": by, "GBps": by / ms / 1e6}))
 
 
+def bench_fermi(args):
+    """nao_fermi_mu (rank sort + single-CTA bisection + occupations; the call synchronises the stream) and its workspace-free
+    twin on a seeded spectrum with a gap at the filling (plain form of the search) and at exact integer filling of a gapped
+    spectrum (log form): n levels per item in [-3, 3] Ha with the levels between -0.05 and 0.05 removed, kT = 9.5e-4 Ha."""
+    n, batch = args.n, args.batch
+    g = torch.Generator(device="cuda"); g.manual_seed(7)
+    E = torch.rand((batch, n), dtype=torch.float64, device="cuda", generator=g) * 2.95 + 0.05
+    E[:, : n // 3] *= -1.0
+    E = torch.sort(E, dim=1).values.contiguous()
+    w = [2.0 / batch] * batch
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    for name, ne in (("plain", 2.0 * (n // 3) - 0.37), ("log", 2.0 * (n // 3))):
+        mu = [0.0]
+
+        def run():
+            mu[0], _ = B.fermi_mu(E, w, ne, 9.5e-4)
+        ms = _time(run, args.reps, flush)
+        mu_static = None
+        if n * batch <= B.FERMI_STATIC_MAX_STATES:
+            mu_static, _ = B.fermi_mu_static(E, w, ne, 9.5e-4)
+        print(json.dumps({"kernel": "nao_fermi_mu", "form": name, "n": n, "batch": batch, "states": n * batch, "ms": ms,
+                          "mu": mu[0], "mu_static_minus_mu": None if mu_static is None else mu_static - mu[0]}))
+
+
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("what", choices=["gemm", "heev", "fold"])
+    ap.add_argument("what", choices=["gemm", "heev", "fold", "fermi"])
     ap.add_argument("--nk", type=int, default=8)
     ap.add_argument("--nr", type=int, default=27)
     ap.add_argument("--m", type=int, default=6656)
@@ -134,7 +159,7 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("microbench needs a CUDA device: the product has no CPU path")
     B.lib()
-    {"gemm": bench_gemm, "heev": bench_heev, "fold": bench_fold}[args.what](args)
+    {"gemm": bench_gemm, "heev": bench_heev, "fold": bench_fold, "fermi": bench_fermi}[args.what](args)
 
 
 if __name__ == "__main__":
