@@ -93,11 +93,62 @@ def oracle_sample(workload, budget_atoms=None):
     dt = time.time() - t0
     scale = (full_nat / float(nat)) ** 3
     cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
-    full_run = ("one full run of this oracle at config 2 (both spin items, written to tests/golden/c2_oracle.txt) took 9957 s of "
-                "eigensolves + 1635 s of density matrices on 7 threads of the 8-core build box") if idx == 2 else None
+    full_run = None
+    if idx == 2:       # wall time of the one full run of this oracle at config 2, as recorded by the script that wrote the digest
+        try:
+            with open(os.path.join(ROOT, "tests", "golden", "c2_oracle_run.json")) as fh:
+                full_run = json.load(fh)
+        except Exception:
+            full_run = None
     return dict(value=dt * scale, unit="s", cores=cores, kind="oracle", extrapolated=scale != 1.0, measured_s=dt, full_run=full_run,
                 sample="%s recipe at %d atoms (n=%d, batch %d): %.2f s measured, x%.0f by the N^3 law to %d atoms"
                        % (workload, nat, prob.n, prob.batch, dt, scale, full_nat))
+
+
+def oracle_in_run():
+    """SURVEY.md 8d protocol: the Jacobi oracle timed in THIS run where it ends in seconds -- config 0 whole (geneig + Fermi +
+    D), config 1 on two of its 16 items (eigensolve + D each; x8 for the batch, flagged as extrapolated)."""
+    import numpy as np
+    import oracle
+    from paper_2606_09058_b200.synth import make_config
+    cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    out = {}
+    prob = make_config(0)
+    t0 = time.time(); oracle.solve_problem(prob); dt = time.time() - t0
+    out["c0"] = dict(value=dt, unit="s", cores=cores, kind="oracle", extrapolated=False,
+                     sample="config 0 whole (n=%d, batch %d)" % (prob.n, prob.batch))
+    prob = make_config(1)
+    t0 = time.time()
+    for b in (0, 9):
+        e, C, _ = oracle.geneig(prob.H_full(b), prob.S_full(b))
+        oracle.density(C, (e < np.median(e)).astype(np.float64))
+    dt = time.time() - t0
+    out["c1"] = dict(value=dt * prob.batch / 2.0, unit="s", cores=cores, kind="oracle", extrapolated=True, measured_s=dt,
+                     sample="items 0 and 9 of %d measured (n=%d complex, eigensolve + density matrix): %.2f s, x%d"
+                            % (prob.batch, prob.n, dt, prob.batch // 2))
+    return out
+
+
+def cpu_certificate_time(prob, E, C, ncols=512):
+    """wall time of the CPU-side a-posteriori certificate (residual H C - S C diag(e) and C^H S C - I, numpy /
+    host BLAS) for the eigenpairs the GPU returned, on a bounded sample of `ncols` evenly spaced eigenvectors; the products
+    are linear in the number of columns, so the full-matrix time is the measured one x n / ncols (flagged)."""
+    import numpy as np
+    n = prob.n
+    cols = np.linspace(0, n - 1, min(ncols, n)).astype(np.int64)
+    Cs = np.ascontiguousarray(C[0][cols].cpu().numpy().T)            # stored row k = eigenvector k
+    e = E[0].cpu().numpy()[cols]
+    Hm, Sm = prob.H_full(0), prob.S_full(0)
+    t0 = time.time()
+    SC = Sm @ Cs
+    R = Hm @ Cs - SC * e[None, :]
+    G = Cs.conj().T @ SC
+    G[np.diag_indices(len(cols))] -= 1.0
+    resid, orth = float(np.abs(R).max()), float(np.abs(G).max())
+    dt = time.time() - t0
+    return dict(value=dt * n / len(cols), unit="s", cores=os.cpu_count(), kind="numpy certificate (residual + S-orthonormality)",
+                extrapolated=True, measured_s=dt, max_residual=resid, max_orthonormality_defect=orth,
+                sample="%d of %d eigenvectors measured: %.2f s, x%.1f" % (len(cols), n, dt, n / len(cols)))
 
 
 def cpu_library_time(workload):
@@ -118,20 +169,22 @@ def cpu_library_time(workload):
 
 
 def read_traffic(kernel, workload):
-    """DRAM bytes per launch of `kernel` from the committed ncu capture of this build (profiles/r02_traffic.csv: one row per
+    """DRAM bytes per launch of `kernel` from the committed ncu captures (profiles/r03_traffic.csv, else r02_traffic.csv: one row per
     kernel and workload, written from `ncu --metrics dram__bytes_read.sum,dram__bytes_write.sum` over one whole step)."""
     import csv
-    try:
-        with open(os.path.join(ROOT, "profiles", "r02_traffic.csv")) as fh:
-            for r in csv.DictReader(fh):
-                if r["kernel"] == kernel and r["workload"] == workload:
-                    return float(r["dram_bytes_total"]) / max(1, int(r["launches"])), r["source"]
-    except Exception:
-        pass
+    for name in ("r03_traffic.csv", "r02_traffic.csv"):      # the newest capture that has the row (the kernels did not change)
+        try:
+            with open(os.path.join(ROOT, "profiles", name)) as fh:
+                for r in csv.DictReader(fh):
+                    if r["kernel"] == kernel and r["workload"] == workload:
+                        return float(r["dram_bytes_total"]) / max(1, int(r["launches"])), r["source"]
+        except Exception:
+            pass
     return None, None
 
 
-def side_record(nao, torch, workload, dev, hbm_peak, dmma_meas, steps=3, warmup=2, groups=True):
+def side_record(nao, torch, workload, dev, hbm_peak, dmma_meas, steps=3, warmup=2, groups=True, cpu_certificate=False,
+                other_reduction=False):
     """A second workload timed in the same run (device-resident inputs, CUDA events, `warmup` + `steps` full steps, then one
     step with the library's event timers): ms per step, phases, and the rooflines of hetrd_panel_kernel / gemm_kernel."""
     from paper_2606_09058_b200.synth import make_config
@@ -145,11 +198,14 @@ def side_record(nao, torch, workload, dev, hbm_peak, dmma_meas, steps=3, warmup=
     in_bytes = H.numel() * H.element_size() + S0.numel() * S0.element_size()
     flush = None if in_bytes > (256 << 20) else torch.empty(256 << 20, dtype=torch.uint8, device=dev)
 
+    last = {}
+
     def step():
         S.copy_(S0)
         E, C, info = nao.geneig(H, S, flags=flags, work=work)
         mu, F = nao.fermi_mu(E, weights, prob.n_electrons, prob.kT)
         nao.density_matrix(C, F, out=Dbuf)
+        last["E"], last["C"] = E, C
         return info, mu
     for _ in range(warmup):
         info, mu = step()
@@ -172,7 +228,45 @@ def side_record(nao, torch, workload, dev, hbm_peak, dmma_meas, steps=3, warmup=
     rec = {"workload": WORKLOADS[workload]["desc"], "value": ms * 1e-3, "unit": "s", "ms_per_step": ms, "steps": steps, "warmup": warmup,
            "n": prob.n, "batch": prob.batch, "gpu_launches_per_step": int(launches), "useful_tflops": fl / (ms * 1e-3) / 1e12,
            "l2_policy": "inputs larger than L2" if flush is None else "L2 flushed between timed steps (256 MB write)",
-           "phases_ms": {k: round(v, 3) for k, v in phases.items()}, "check": {"mu": mu}}
+           "phases_ms": {k: round(v, 3) for k, v in phases.items()}, "check": {"mu": mu},
+           # which reduction the library took by itself: the band -> tridiagonal phase only exists on the two-stage path
+           "reduction": "two_stage" if phases.get("band_to_tridiagonal", 0.0) > 0.02 * phases.get("tridiagonalise", 0.0)
+                        else "one_stage"}
+    if other_reduction:
+        # the same step through the reduction the library did NOT pick (forced by flag): the measurement behind the default
+        oflag = nao.NAO_TRD_ONE_STAGE if rec["reduction"] == "two_stage" else nao.NAO_TRD_TWO_STAGE
+        try:
+            owork = work
+            need = nao.geneig_workspace(prob.n, prob.batch, dt, flags | oflag) + 256
+            if need > work.numel():
+                owork = torch.empty(need, dtype=torch.uint8, device=dev)
+
+            def ostep():
+                S.copy_(S0)
+                E, C, info = nao.geneig(H, S, flags=flags | oflag, work=owork)
+                mu_o, F = nao.fermi_mu(E, weights, prob.n_electrons, prob.kT)
+                nao.density_matrix(C, F, out=Dbuf)
+                return mu_o
+            for _ in range(warmup):
+                mu_o = ostep()
+            torch.cuda.synchronize()
+            tot = 0.0
+            for _ in range(steps):
+                if flush is not None:
+                    flush.zero_()
+                ev0.record(); ostep(); ev1.record(); torch.cuda.synchronize()
+                tot += ev0.elapsed_time(ev1)
+            rec["other_reduction"] = {"reduction": "one_stage" if oflag == nao.NAO_TRD_ONE_STAGE else "two_stage",
+                                      "ms_per_step": tot / steps, "mu_difference": abs(mu_o - mu)}
+            del owork
+        except Exception as exc:
+            rec["other_reduction"] = {"error": str(exc)}
+    if cpu_certificate:
+        try:
+            rec["cpu_certificate"] = cpu_certificate_time(prob, last["E"], last["C"])
+        except Exception as exc:
+            rec["cpu_certificate"] = {"error": str(exc)}
+    last.clear()
     if kp["launches"] > 0 and kp["ms"] > 0:
         ach = kp["work"] / (kp["ms"] * 1e-3) / 1e9
         tr, src = read_traffic("hetrd_panel_kernel", workload)
@@ -238,6 +332,39 @@ def run_reference(args):
             "cpu_baseline": cb, "e2e": {"value": v, "unit": "s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
+
+
+def order_line(line):
+    """Key order of the JSON line: the contract's scalars, then compact scalars of every config (a record that keeps only the
+    head of the line still shows both halves of BASELINE.json's metric), then the contract's objects, then the long
+    per-config sub-records."""
+    def frac(rec, key):
+        r = rec.get(key) if isinstance(rec, dict) else None
+        return r.get("frac") if isinstance(r, dict) else None
+    head = ["metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling", "vs_baseline",
+            "dtype", "data", "config", "gpu_launches", "reduction"]
+    out = {k: line[k] for k in head if k in line}
+    out["roofline_frac"] = frac(line, "roofline")
+    if "roofline_hetrd" in line:
+        out["hetrd_frac_one_stage_step"] = frac(line, "roofline_hetrd")
+    if isinstance(line.get("e2e"), dict):
+        out["e2e_ms_per_step"] = line["e2e"]["value"] * 1e3
+    for wl in ("c3", "c1", "c4"):
+        rec = line.get(wl)
+        if isinstance(rec, dict) and "ms_per_step" in rec:
+            out[wl + "_ms_per_step"] = rec["ms_per_step"]
+            out[wl + "_hetrd_frac"] = frac(rec, "roofline")
+            out[wl + "_gemm_frac"] = frac(rec, "roofline_gemm")
+            out[wl + "_reduction"] = rec.get("reduction")
+            if isinstance(rec.get("other_reduction"), dict) and "ms_per_step" in rec["other_reduction"]:
+                out[wl + "_other_reduction_ms_per_step"] = rec["other_reduction"]["ms_per_step"]
+    for k in ("roofline", "cpu_baseline", "e2e", "clocks", "roofline_hetrd", "roofline_gemm", "cpu_library", "cpu_oracle_c0"):
+        if k in line:
+            out[k] = line[k]
+    for k, v in line.items():
+        if k not in out:
+            out[k] = v
+    return out
 
 
 def main():
@@ -551,6 +678,10 @@ def main():
                 try:
                     # config 4 (11.3 GB per matrix, 21 s per step): one warm-up and one timed step
                     kw = dict(steps=1, warmup=1) if wl == "c4" else {}
+                    if wl == "c3" and not args.no_cpu_baseline:
+                        kw["cpu_certificate"] = True
+                    if wl in ("c3", "c1"):
+                        kw["other_reduction"] = True
                     line[wl] = side_record(nao, torch, wl, dev, hbm_peak, dmma_meas, **kw)
                 except Exception as exc:       # reported, never hidden
                     line[wl] = {"error": str(exc)}
@@ -560,7 +691,15 @@ def main():
                 line["cpu_library"] = cpu_library_time(args.workload)
             except Exception as exc:
                 line["cpu_library"] = {"error": str(exc)}
-        print(json.dumps(line))
+            if args.workload == "c2" and not args.no_side:
+                try:
+                    inrun = oracle_in_run()
+                    line["cpu_oracle_c0"] = inrun["c0"]
+                    if isinstance(line.get("c1"), dict):
+                        line["c1"]["cpu_oracle"] = inrun["c1"]
+                except Exception as exc:
+                    line["cpu_oracle_c0"] = {"error": str(exc)}
+        print(json.dumps(order_line(line)))
     if dist is not None:
         dist.destroy_process_group()
 

@@ -43,6 +43,7 @@ def main():
     hh.update(np.ascontiguousarray(prob.H).tobytes())
     hh.update(np.ascontiguousarray(prob.S).tobytes())
     es, Cs, sweeps = [], [], []
+    t_eig, t_den = 0.0, 0.0          # wall time of the oracle's eigensolves / density matrices of THIS run (cached items add 0)
     for b in range(prob.batch):
         cf = os.path.join(args.cache, "%s_item%d.npz" % (prob.name, b)) if args.cache else None
         if cf and os.path.exists(cf):
@@ -52,6 +53,7 @@ def main():
             t = time.time()
             e, C, info = oracle.geneig(prob.H_full(b), prob.S_full(b))
             sw = info["sweeps"]
+            t_eig += time.time() - t
             print("item %d: %d sweeps, %.0f s" % (b, sw, time.time() - t), flush=True)
             if cf:
                 os.makedirs(args.cache, exist_ok=True)
@@ -74,6 +76,7 @@ def main():
         for b in range(prob.batch):
             t = time.time()
             D = oracle.density(Cs[b], f[b])
+            t_den += time.time() - t
             print("item %d: density %.0f s" % (b, time.time() - t), flush=True)
             fo.write("trace_DS %d %.17e\n" % (b, float(np.sum(D * prob.S_full(b).T))))
             fo.write("norm_D_F %d %.17e\n" % (b, float(np.linalg.norm(D))))
@@ -83,6 +86,14 @@ def main():
                 fo.write("diagD %d %d %.17e\n" % (b, k, D[k, k]))
             for k in range(n):
                 fo.write("e %d %d %.17e\n" % (b, k, e[b, k]))
+    # wall times of this run, read by bench.py (cpu_baseline.full_run, tagged "recorded": a record of this script's run, not a
+    # measurement of the bench run)
+    import json
+    with open(path[:-4] + "_run.json", "w") as fo:
+        json.dump({"recorded": True, "eigensolve_s": round(t_eig), "density_s": round(t_den),
+                   "threads": int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1)), "host_cores": os.cpu_count(),
+                   "sweeps": sweeps, "source": "tests/golden/make_golden_c2.py"}, fo, indent=1)
+        fo.write("\n")
     print(path)
 
 
